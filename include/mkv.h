@@ -1,0 +1,201 @@
+/*
+ * mkv.h — C ABI of libmkv: decode-time attention over a dynamically two-D-compressed KV cache
+ * (MosaicKV, arxiv/paper_2607_00760), hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * The hot path has three steps (§4.2, §5.1-5.3):
+ *   1. compress  — per K/V vector keep the top-r elements by |x|, compute the
+ *                  per-block mean keys, choose a strategy per segment
+ *                   and pack kept elements behind a position bitmap
+ *                  (PAPER.md:194-196);
+ *   2. select    — score every token block with the current query on the packed block keys and
+ *                  keep the top-k blocks;
+ *   3. attention — PackedAttention: QK, softmax and PV over the selected packed tokens only
+ *                  (PAPER.md:214-222), with a split-K combine.
+ *
+ * Conventions
+ *   - Plain C, no torch types.  Every pointer is a DEVICE pointer unless its name ends in
+ *     `_host`.  bf16 tensors are passed as `const void*` to uint16 bit patterns.
+ *   - Every function returns MKV_OK (0) or a negative mkv_status; nothing throws or aborts.
+ *     `mkv_last_error()` returns a thread-local message for the last failing call.
+ *   - Argument errors are detected on the host before anything is enqueued.  Errors only a
+ *     kernel can see (arena overflow, an invalid strategy record in device memory) set a sticky
+ *     device flag that `mkv_cache_status()` reads (it synchronises).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Except for
+ *     create / free / export / bytes / status, calls only enqueue work and return immediately;
+ *     they are CUDA-graph capturable (no allocation, no synchronisation).
+ *   - Ownership: the caller owns every buffer it passes; the cache owns the packed arenas, its
+ *     tables and its scratch.  A cache is not thread-safe; distinct caches are independent.  All
+ *     calls on one cache must be ordered on one stream (or by events).
+ *   - A *unit* is one (layer, request b, KV head h); units never interact.  Query head hq uses
+ *     KV head hq / (n_q_heads / n_kv_heads).
+ *   - Supported on the GPU today: head_dim = 128, token block B = 8, element group g = 1,
+ *     segment_len a multiple of 8 in [8, 4096], group G = n_q_heads/n_kv_heads <= 8.  Anything
+ *     else is MKV_E_UNSUPPORTED (host-visible) or MKV_DEV_BAD_STRATEGY (device-visible).
+ *   - Inputs must be finite; behaviour on NaN/Inf is unspecified.
+ *
+ * Canonical packed format (what mkv_cache_export returns; byte-identical to the CPU oracle):
+ * see DESIGN.md "Canonical packed format".  In short, per unit:
+ *   packed vector   = [bitmap D/g bits, LSB-first little-endian][kept bf16, ascending channel];
+ *                     the bitmap is omitted when r == D
+ *   token block     = [K bitmaps nb][K values nb*r_k][V bitmaps nb][V values nb*r_v], pad to 16 B
+ *   segment         = its token blocks in order; block keys of the segment (separate arena) =
+ *                     [bitmaps nblk][values nblk*r_k], pad to 16 B
+ *   blob            = header(48 B) | strategy[S] (8 B) | tok_off[S] u32 | bk_off[S] u32 | pad16 |
+ *                     token arena | block-key arena          (offsets in 16-B units)
+ */
+#ifndef MKV_H
+#define MKV_H
+
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define MKV_API __attribute__((visibility("default")))
+#else
+#define MKV_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    MKV_OK = 0,
+    MKV_E_ARG = -1,          /* NULL / out-of-range / inconsistent argument */
+    MKV_E_UNSUPPORTED = -2,  /* valid in the format, not built on the GPU yet (see Conventions) */
+    MKV_E_NOMEM = -3,        /* device or host allocation failed */
+    MKV_E_CUDA = -4,         /* a CUDA runtime call failed; message in mkv_last_error() */
+    MKV_E_STATE = -5,        /* append-order violation (segments must arrive in ascending order) */
+    MKV_E_DEVICE = -6        /* sticky device-side flag set; see mkv_cache_status */
+} mkv_status;
+
+/* device-side sticky flags reported by mkv_cache_status */
+#define MKV_DEV_ARENA_OVERFLOW 1u /* a compress call needed more arena than the layer slice holds */
+#define MKV_DEV_BAD_STRATEGY 2u   /* a strategy record in device memory was invalid/unsupported */
+
+typedef struct mkv_cache mkv_cache; /* opaque: packed arenas + tables + scratch of one model */
+
+typedef struct {
+    int32_t n_layers;     /* >= 1 */
+    int32_t batch;        /* requests */
+    int32_t n_kv_heads;
+    int32_t n_q_heads;    /* multiple of n_kv_heads, group <= 8 */
+    int32_t head_dim;     /* D, must be 128 */
+    int32_t max_tokens;   /* capacity per request */
+    int32_t segment_len;  /* L: tokens per segment = granularity of the strategy */
+    int32_t device;       /* CUDA device ordinal */
+    uint64_t arena_bytes; /* packed payload bytes for ALL layers (split evenly per layer);
+                             0 = size for the dense worst case */
+} mkv_cache_desc;
+
+/* Per-segment compression strategy: kept elements per K / V vector (multiples of
+ * g, 1..D; r == D means "not channel-compressed"), element-group size, token-block size. */
+typedef struct {
+    uint8_t r_k, r_v, g, B;
+} mkv_strategy;
+
+/* Create / destroy.  `desc_host` is read during the call only.  Both calls synchronise. */
+MKV_API int mkv_cache_create(const mkv_cache_desc* desc_host, mkv_cache** out);
+MKV_API int mkv_cache_free(mkv_cache* cache); /* NULL is a no-op */
+
+/* Forget every segment of `layer` (-1 = all layers) so it can be compressed again. */
+MKV_API int mkv_cache_reset(mkv_cache* cache, int32_t layer, void* stream);
+
+/*
+ * Step 1c: compression loss of ONE candidate strategy.
+ * k, v: bf16, element [b][h][t][c] at base + (b-b0)*stride_b + h*stride_h + t*stride_t + c
+ * (strides in elements, channels contiguous), holding tokens [seg0*L, seg0*L + n_tok) of requests
+ * [b0, b0+nb); nseg = ceil(n_tok / L), only the last segment may be short.
+ * loss_k, loss_v: double [nb][n_kv_heads][nseg]:  sum of squares of the dropped elements /
+ * sum of squares of all elements of the segment (0 if the segment is all zeros), fp64.
+ */
+MKV_API int mkv_segment_loss(const mkv_cache* cache, const void* k, const void* v, int64_t stride_b,
+                     int64_t stride_h, int64_t stride_t, int32_t b0, int32_t nb, int32_t seg0,
+                     int32_t nseg, int32_t n_tok, mkv_strategy cand, double* loss_k,
+                     double* loss_v, void* stream);
+
+/*
+ * Step 1c, strategy choice.  Both write strat_out [n_units][nseg] (device).
+ * quantile  (BASELINE.json config policy): per unit, the ceil(nseg*dense_num/dense_den) segments
+ *           with the largest importance I = (loss_k+loss_v)/2 (ties -> lower segment index) get
+ *           r_k = r_v = D; all others get `sparse`.
+ * threshold: loss_k/loss_v are [ncand][n_units*nseg]; candidates are ordered most
+ *           -> least aggressive; the first with I <= tau wins, none -> dense (g = 1).
+ */
+MKV_API int mkv_strategy_quantile(const mkv_cache* cache, const double* loss_k, const double* loss_v,
+                          int32_t n_units, int32_t nseg, int32_t dense_num, int32_t dense_den,
+                          mkv_strategy sparse, mkv_strategy* strat_out, void* stream);
+MKV_API int mkv_strategy_threshold(const mkv_cache* cache, const double* loss_k, const double* loss_v,
+                           int32_t ncand, int32_t n_units, int32_t nseg,
+                           const mkv_strategy* cands_host, double tau, mkv_strategy* strat_out,
+                           void* stream);
+
+/*
+ * Steps 1a, 1b, 1d: compress and pack segments [seg0, seg0+nseg) of
+ * requests [b0, b0+nb) of `layer`; nseg = 1 is the literal "compress one segment".
+ * k, v as in mkv_segment_loss.  strat: device, [nb][n_kv_heads][nseg].
+ * Append-only: seg0 must equal the number of segments the request already holds in this layer
+ * and its last segment must be full, else MKV_E_STATE.
+ */
+MKV_API int mkv_compress_segment(mkv_cache* cache, int32_t layer, const void* k, const void* v,
+                         int64_t stride_b, int64_t stride_h, int64_t stride_t, int32_t b0,
+                         int32_t nb, int32_t seg0, int32_t nseg, int32_t n_tok,
+                         const mkv_strategy* strat, void* stream);
+
+/*
+ * Step 2: score every token block of every unit of `layer` with q on
+ * the packed block keys (no 1/sqrt(D)), reduce over the GQA group (0 = max, 1 = sum) and select
+ * blocks by (score descending, index ascending) while they fit in `token_budget` tokens.
+ * q: bf16 [batch][n_q_heads][D].  sel: int32 [batch][n_kv_heads][k_max], first-token index of each
+ * chosen block, ascending; unused tail = -1.  sel_count: int32 [batch][n_kv_heads].
+ * k_max must be >= min(token_budget / 8 + 1, blocks per unit).  scores_opt: float
+ * [batch][n_kv_heads][score_stride] or NULL, score_stride = ceil(max_tokens / 8).
+ */
+MKV_API int mkv_select(const mkv_cache* cache, int32_t layer, const void* q, int32_t token_budget,
+               int32_t reduce, int32_t* sel, int32_t* sel_count, int32_t k_max, float* scores_opt,
+               void* stream);
+
+/*
+ * Step 3: PackedAttention over the tokens of the selected blocks.
+ * sel / sel_count as written by mkv_select (any order of blocks is accepted).
+ * out: float [batch][n_q_heads][D].  lse_opt: float [batch][n_q_heads] or NULL (log-sum-exp of the
+ * scaled logits; -inf and out = 0 for an empty selection).
+ */
+MKV_API int mkv_packed_attention(const mkv_cache* cache, int32_t layer, const void* q, const int32_t* sel,
+                         const int32_t* sel_count, int32_t k_max, float softmax_scale, float* out,
+                         float* lse_opt, void* stream);
+
+/*
+ * Steps 2+3 with HOST buffers (the end-to-end call): copies q_host (bf16 [batch][n_q_heads][D],
+ * pinned for true async) to the device, runs select + attention, copies out_host (float
+ * [batch][n_q_heads][D]) back.  Everything is enqueued on `stream`; the caller synchronises the
+ * stream before reading out_host.  sel_host_opt [batch][n_kv_heads][token_budget/8 + 1] and
+ * sel_count_host_opt [batch][n_kv_heads] may be NULL.
+ */
+MKV_API int mkv_decode_host(mkv_cache* cache, int32_t layer, const void* q_host, int32_t token_budget,
+                    int32_t reduce, float softmax_scale, float* out_host, int32_t* sel_host_opt,
+                    int32_t* sel_count_host_opt, void* stream);
+
+/* Parity / dump: canonical blob of unit (layer, b, h) into host memory.  *need_host receives the
+ * blob size; if cap < need nothing is copied and MKV_E_ARG is returned.  Synchronises. */
+MKV_API int mkv_cache_export(const mkv_cache* cache, int32_t layer, int32_t b, int32_t h, void* buf_host,
+                     uint64_t cap, uint64_t* need_host);
+
+/* Bytes held for `layer`: token payloads, block-key payloads, tables in use.  Synchronises. */
+MKV_API int mkv_cache_bytes(const mkv_cache* cache, int32_t layer, uint64_t* packed_host,
+                    uint64_t* block_keys_host, uint64_t* tables_host);
+
+/* Reads (and keeps) the sticky device flags; returns MKV_E_DEVICE if any is set.  Synchronises. */
+MKV_API int mkv_cache_status(const mkv_cache* cache, uint32_t* flags_host);
+
+/* Launch geometry of the last mkv_packed_attention / mkv_select call (for the bench's
+ * gpu_launches count): number of kernels enqueued by that call. */
+MKV_API int mkv_last_launch_count(const mkv_cache* cache, int32_t* select_kernels_host,
+                          int32_t* attention_kernels_host, int32_t* compress_kernels_host);
+
+MKV_API const char* mkv_last_error(void); /* thread-local, never NULL */
+MKV_API int mkv_version(void);            /* ABI version, currently 1 */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MKV_H */

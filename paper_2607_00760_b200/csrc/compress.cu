@@ -1,0 +1,403 @@
+// compress.cu — step 1 of the hot path: per-vector top-r element selection,
+// per-block mean keys, compression loss + strategy choice
+// and packing behind a position bitmap.  sm_100a.
+//
+// Thread mapping: one warp owns one vector at a time; lane l holds channels l, l+32, l+64, l+96,
+// so `__ballot_sync` of a per-channel predicate IS bitmap word j of the canonical format and
+// the ascending-channel rank of a kept element is popc(words below) + popc(word & lanemask_lt).
+#include "mkv_internal.cuh"
+
+namespace mkv {
+
+namespace {
+
+constexpr unsigned kFull = 0xffffffffu;
+constexpr unsigned long long kNoBase = ~0ull;
+
+__device__ __forceinline__ unsigned lanemask_lt() {
+    unsigned m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+// Top-r mask of one 128-channel vector held as 15-bit magnitudes mag[j] (channel lane + 32 j).
+// Finds the r-th largest magnitude T by a bitwise binary search (count(mag >= cand) via REDUX),
+// keeps everything above T and the lowest-channel elements equal to T until r are kept
+// (ties -> lower index).  Returns the four bitmap words in w (identical in all lanes).
+__device__ __forceinline__ void topr_mask(const uint32_t (&mag)[4], int r, uint32_t (&w)[4]) {
+    uint32_t T = 0;
+#pragma unroll
+    for (int bit = 14; bit >= 0; --bit) {
+        const uint32_t cand = T | (1u << bit);
+        int c = (mag[0] >= cand) + (mag[1] >= cand) + (mag[2] >= cand) + (mag[3] >= cand);
+        c = __reduce_add_sync(kFull, c);
+        if (c >= r) T = cand;
+    }
+    int ngt = (mag[0] > T) + (mag[1] > T) + (mag[2] > T) + (mag[3] > T);
+    ngt = __reduce_add_sync(kFull, ngt);
+    const int need = r - ngt;  // >= 1 elements equal to T are kept, lowest channels first
+    const unsigned lt = lanemask_lt();
+    int seen = 0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const bool eq = (mag[j] == T);
+        const unsigned e = __ballot_sync(kFull, eq);
+        const bool keep = (mag[j] > T) || (eq && (seen + __popc(e & lt) < need));
+        seen += __popc(e);
+        w[j] = __ballot_sync(kFull, keep);
+    }
+}
+
+// Write one packed vector (bitmap + kept values, ascending channel) or a dense copy.
+// x[j]: bf16 bits of channel lane + 32 j.  bm / val: byte pointers (val is 2-byte aligned).
+__device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, uint8_t* bm, uint8_t* val,
+                                            int lane) {
+    uint16_t* v16 = reinterpret_cast<uint16_t*>(val);
+    if (r == kD) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) v16[lane + 32 * j] = (uint16_t)x[j];
+        return;
+    }
+    uint32_t mag[4], w[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) mag[j] = x[j] & 0x7FFFu;
+    topr_mask(mag, r, w);
+    const unsigned lt = lanemask_lt();
+    int base = 0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        if ((w[j] >> lane) & 1u) v16[base + __popc(w[j] & lt)] = (uint16_t)x[j];
+        base += __popc(w[j]);
+    }
+    if (lane < 4) {
+        const uint32_t wl = lane == 0 ? w[0] : lane == 1 ? w[1] : lane == 2 ? w[2] : w[3];
+        reinterpret_cast<uint32_t*>(bm)[lane] = wl;
+    }
+}
+
+__device__ __forceinline__ bool strat_supported(const mkv_strategy& s) {
+    return s.g == 1 && s.B == kB && s.r_k >= 1 && s.r_k <= kD && s.r_v >= 1 && s.r_v <= kD;
+}
+
+// ------------------------------------------------------------------------------------------
+// plan: one CTA per unit of the call.  Sizes every segment from its strategy, claims a
+// contiguous region [block keys | token blocks] of the layer slice with one atomicAdd, and
+// writes the unit's table entries (strategy record, offsets).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) mkv_plan_kernel(CacheGeom g, LayerView lv, CompressArgs a,
+                                                       const mkv_strategy* __restrict__ strat,
+                                                       unsigned long long* __restrict__ call_base,
+                                                       uint32_t* __restrict__ dev_flags) {
+    const int uc = blockIdx.x;
+    const int b = a.b0 + uc / g.n_kv_heads, h = uc % g.n_kv_heads;
+    const int unit = b * g.n_kv_heads + h;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const mkv_strategy* st = strat + (size_t)uc * a.nseg;
+
+    __shared__ unsigned long long s_tok[8], s_bk[8];
+    __shared__ int s_bad[8];
+    __shared__ unsigned long long s_base, s_bk_total;
+
+    unsigned long long tokb = 0, bkb = 0;
+    int bad = 0;
+    for (int i = tid; i < a.nseg; i += 256) {
+        const mkv_strategy s = st[i];
+        const int n_tok = (i == a.nseg - 1) ? a.n_tok - i * g.L : g.L;
+        if (!strat_supported(s)) { bad = 1; continue; }
+        tokb += seg_tok_bytes(s.r_k, s.r_v, n_tok);
+        bkb += seg_bk_bytes(s.r_k, n_tok);
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        tokb += __shfl_xor_sync(kFull, tokb, o);
+        bkb += __shfl_xor_sync(kFull, bkb, o);
+        bad |= __shfl_xor_sync(kFull, bad, o);
+    }
+    if (lane == 0) { s_tok[warp] = tokb; s_bk[warp] = bkb; s_bad[warp] = bad; }
+    __syncthreads();
+    if (tid == 0) {
+        unsigned long long T = 0, K = 0;
+        int B = 0;
+        for (int i = 0; i < 8; ++i) { T += s_tok[i]; K += s_bk[i]; B |= s_bad[i]; }
+        unsigned long long base = kNoBase;
+        if (B) {
+            atomicOr(dev_flags, MKV_DEV_BAD_STRATEGY);
+        } else {
+            base = atomicAdd(lv.bump, T + K);
+            if (base + T + K > lv.slice_bytes) {
+                atomicOr(dev_flags, MKV_DEV_ARENA_OVERFLOW);
+                base = kNoBase;
+            } else {
+                atomicAdd(lv.used_tok, T);
+                atomicAdd(lv.used_bk, K);
+                lv.unit_nseg[unit] = a.seg0 + a.nseg;
+                lv.unit_ntok[unit] = a.seg0 * g.L + a.n_tok;
+            }
+        }
+        s_base = base;
+        s_bk_total = K;
+        call_base[uc] = base;
+    }
+    __syncthreads();
+    const unsigned long long base = s_base;
+    if (base == kNoBase) return;
+    const unsigned long long tok_base = base + s_bk_total;
+
+    // exclusive scan over the segments, 256 at a time, with a running carry
+    __shared__ unsigned long long s_wtok[8], s_wbk[8];
+    unsigned long long carry_tok = 0, carry_bk = 0;
+    for (int i0 = 0; i0 < a.nseg; i0 += 256) {
+        const int i = i0 + tid;
+        unsigned long long t = 0, k = 0;
+        mkv_strategy s = {0, 0, 0, 0};
+        int n_tok = 0;
+        if (i < a.nseg) {
+            s = st[i];
+            n_tok = (i == a.nseg - 1) ? a.n_tok - i * g.L : g.L;
+            t = seg_tok_bytes(s.r_k, s.r_v, n_tok);
+            k = seg_bk_bytes(s.r_k, n_tok);
+        }
+        unsigned long long it = t, ik = k;  // inclusive warp scan
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long ut = __shfl_up_sync(kFull, it, o);
+            const unsigned long long uk = __shfl_up_sync(kFull, ik, o);
+            if (lane >= o) { it += ut; ik += uk; }
+        }
+        if (lane == 31) { s_wtok[warp] = it; s_wbk[warp] = ik; }
+        __syncthreads();
+        unsigned long long wt = 0, wk = 0, tot_t = 0, tot_k = 0;
+        for (int wv = 0; wv < 8; ++wv) {
+            if (wv < warp) { wt += s_wtok[wv]; wk += s_wbk[wv]; }
+            tot_t += s_wtok[wv];
+            tot_k += s_wbk[wv];
+        }
+        if (i < a.nseg) {
+            const size_t e = (size_t)unit * lv.S_max + a.seg0 + i;
+            StratRec rec;
+            rec.r_k = s.r_k; rec.r_v = s.r_v; rec.g = s.g; rec.B = s.B;
+            rec.n_tok = (uint16_t)n_tok;
+            rec.flags = (uint16_t)((s.r_k == kD ? 1 : 0) | (s.r_v == kD ? 2 : 0));
+            lv.strat[e] = rec;
+            lv.tok_off[e] = (uint32_t)((tok_base + carry_tok + wt + it - t) >> 4);
+            lv.bk_off[e] = (uint32_t)((base + carry_bk + wk + ik - k) >> 4);
+        }
+        carry_tok += tot_t;
+        carry_bk += tot_k;
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// compress: CTA = 8 warps = 8 consecutive token blocks of one segment; warp = one token block:
+// nb K vectors, nb V vectors, and the block key (fp32 sum in token order, IEEE /nb, RNE bf16).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) mkv_compress_kernel(CacheGeom g, LayerView lv, CompressArgs a,
+                                                           const unsigned long long* __restrict__ call_base,
+                                                           int chunks_per_seg) {
+    const int uc = blockIdx.y;
+    if (call_base[uc] == kNoBase) return;
+    const int b = a.b0 + uc / g.n_kv_heads, h = uc % g.n_kv_heads;
+    const int unit = b * g.n_kv_heads + h;
+    const int seg_local = blockIdx.x / chunks_per_seg, chunk = blockIdx.x % chunks_per_seg;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const size_t e = (size_t)unit * lv.S_max + a.seg0 + seg_local;
+    const StratRec rec = lv.strat[e];
+    const int n_tok = rec.n_tok, nblk = (n_tok + kB - 1) / kB;
+    const int blk = chunk * 8 + warp;
+    if (blk >= nblk) return;
+    const int nb = min(kB, n_tok - blk * kB);
+    const int r_k = rec.r_k, r_v = rec.r_v;
+    const uint32_t bmk = (r_k == kD) ? 0u : kBitmapBytes, bmv = (r_v == kD) ? 0u : kBitmapBytes;
+
+    uint8_t* base = lv.slice + ((size_t)lv.tok_off[e] << 4) + (size_t)blk * tokblock_bytes(r_k, r_v, kB);
+    uint8_t* k_bm = base;
+    uint8_t* k_val = k_bm + nb * bmk;
+    uint8_t* v_bm = k_val + nb * r_k * 2;
+    uint8_t* v_val = v_bm + nb * bmv;
+    uint8_t* bk_base = lv.slice + ((size_t)lv.bk_off[e] << 4);
+
+    const size_t row0 = (size_t)(b - a.b0) * a.stride_b + (size_t)h * a.stride_h +
+                        (size_t)(seg_local * g.L + blk * kB) * a.stride_t;
+    const uint16_t* ksrc = a.k + row0;
+    const uint16_t* vsrc = a.v + row0;
+
+    float sum[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int t = 0; t < nb; ++t) {
+        uint32_t x[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) x[j] = __ldg(ksrc + (size_t)t * a.stride_t + lane + 32 * j);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) sum[j] = __fadd_rn(sum[j], bf16_bits_to_f32(x[j]));
+        pack_vector(x, r_k, k_bm + t * bmk, k_val + t * r_k * 2, lane);
+    }
+    for (int t = 0; t < nb; ++t) {
+        uint32_t x[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) x[j] = __ldg(vsrc + (size_t)t * a.stride_t + lane + 32 * j);
+        pack_vector(x, r_v, v_bm + t * bmv, v_val + t * r_v * 2, lane);
+    }
+    // zero the pad of a ragged token block
+    {
+        const uint32_t used = (uint32_t)nb * (vec_bytes(r_k) + vec_bytes(r_v));
+        const uint32_t padded = pad16u(used);
+        for (uint32_t o = used + lane; o < padded; o += 32) base[o] = 0;
+    }
+    // block key
+    {
+        uint32_t x[4];
+        const float fnb = (float)nb;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) x[j] = f32_to_bf16_bits_rne(__fdiv_rn(sum[j], fnb));
+        pack_vector(x, r_k, bk_base + blk * bmk, bk_base + nblk * bmk + blk * r_k * 2, lane);
+        if (blk == nblk - 1) {
+            const uint32_t used = (uint32_t)nblk * vec_bytes(r_k);
+            const uint32_t padded = pad16u(used);
+            for (uint32_t o = used + lane; o < padded; o += 32) bk_base[o] = 0;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// loss: CTA = one segment of one unit; warps stride over its tokens.  fp64 sums of the exact
+// fp32 squares of the dropped / all elements (R9).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) mkv_segment_loss_kernel(CacheGeom g, CompressArgs a, int r_k, int r_v,
+                                                               double* __restrict__ loss_k,
+                                                               double* __restrict__ loss_v) {
+    const int uc = blockIdx.y, seg_local = blockIdx.x;
+    const int b = a.b0 + uc / g.n_kv_heads, h = uc % g.n_kv_heads;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int n_tok = (seg_local == a.nseg - 1) ? a.n_tok - seg_local * g.L : g.L;
+    const size_t row0 = (size_t)(b - a.b0) * a.stride_b + (size_t)h * a.stride_h +
+                        (size_t)(seg_local * g.L) * a.stride_t;
+    double acc[4] = {0., 0., 0., 0.};  // dropped_k, total_k, dropped_v, total_v
+    for (int which = 0; which < 2; ++which) {
+        const uint16_t* src = (which ? a.v : a.k) + row0;
+        const int r = which ? r_v : r_k;
+        for (int t = warp; t < n_tok; t += 8) {
+            uint32_t x[4], mag[4], w[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                x[j] = __ldg(src + (size_t)t * a.stride_t + lane + 32 * j);
+                mag[j] = x[j] & 0x7FFFu;
+            }
+            if (r < kD) topr_mask(mag, r, w);
+            else w[0] = w[1] = w[2] = w[3] = kFull;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const float f = bf16_bits_to_f32(x[j]);
+                const double sq = (double)__fmul_rn(f, f);  // exact: 8-bit x 8-bit significands
+                acc[2 * which + 1] += sq;
+                if (!((w[j] >> lane) & 1u)) acc[2 * which] += sq;
+            }
+        }
+    }
+    __shared__ double s_acc[8][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+#pragma unroll
+        for (int o = 16; o; o >>= 1) acc[i] += __shfl_xor_sync(kFull, acc[i], o);
+    }
+    if (lane == 0)
+        for (int i = 0; i < 4; ++i) s_acc[warp][i] = acc[i];
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t[4] = {0., 0., 0., 0.};
+        for (int wv = 0; wv < 8; ++wv)
+            for (int i = 0; i < 4; ++i) t[i] += s_acc[wv][i];
+        const size_t o = (size_t)uc * a.nseg + seg_local;
+        loss_k[o] = t[1] > 0. ? t[0] / t[1] : 0.;
+        loss_v[o] = t[3] > 0. ? t[2] / t[3] : 0.;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// strategy, quantile rule: one CTA per unit; a segment stays dense iff its rank by
+// (importance descending, index ascending) is below n_dense.  Rank by counting.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) mkv_strategy_quantile_kernel(const double* __restrict__ loss_k,
+                                                                    const double* __restrict__ loss_v,
+                                                                    int nseg, int n_dense, mkv_strategy sparse,
+                                                                    mkv_strategy* __restrict__ out) {
+    const int u = blockIdx.x;
+    const double* lk = loss_k + (size_t)u * nseg;
+    const double* lvv = loss_v + (size_t)u * nseg;
+    constexpr int kTile = 1024;
+    __shared__ double s_I[kTile];
+    for (int i0 = 0; i0 < nseg; i0 += 256) {
+        const int i = i0 + threadIdx.x;
+        const double mine = (i < nseg) ? 0.5 * (lk[i] + lvv[i]) : 0.;
+        int rank = 0;
+        for (int j0 = 0; j0 < nseg; j0 += kTile) {
+            __syncthreads();
+            for (int j = threadIdx.x; j < kTile && j0 + j < nseg; j += 256)
+                s_I[j] = 0.5 * (lk[j0 + j] + lvv[j0 + j]);
+            __syncthreads();
+            const int n = min(kTile, nseg - j0);
+            for (int j = 0; j < n; ++j) {
+                const double o = s_I[j];
+                rank += (o > mine) || (o == mine && (j0 + j) < i);
+            }
+        }
+        if (i < nseg) {
+            mkv_strategy s = sparse;
+            if (rank < n_dense) { s.r_k = kD; s.r_v = kD; }
+            out[(size_t)u * nseg + i] = s;
+        }
+    }
+}
+
+__global__ void mkv_strategy_threshold_kernel(const double* __restrict__ loss_k, const double* __restrict__ loss_v,
+                                              int ncand, long long n, const mkv_strategy* __restrict__ cands,
+                                              double tau, mkv_strategy* __restrict__ out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    mkv_strategy s;
+    s.r_k = kD; s.r_v = kD; s.g = 1; s.B = cands[ncand - 1].B;
+    for (int c = 0; c < ncand; ++c) {
+        const double I = 0.5 * (loss_k[(size_t)c * n + i] + loss_v[(size_t)c * n + i]);
+        if (I <= tau) { s = cands[c]; break; }
+    }
+    out[i] = s;
+}
+
+}  // namespace
+
+cudaError_t launch_segment_loss(const CacheGeom& g, const CompressArgs& a, mkv_strategy cand, double* loss_k,
+                                double* loss_v, cudaStream_t s) {
+    dim3 grid(a.nseg, a.nb * g.n_kv_heads);
+    mkv_segment_loss_kernel<<<grid, 256, 0, s>>>(g, a, cand.r_k, cand.r_v, loss_k, loss_v);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_strategy_quantile(const double* loss_k, const double* loss_v, int n_units, int nseg,
+                                     int n_dense, mkv_strategy sparse, mkv_strategy* out, cudaStream_t s) {
+    mkv_strategy_quantile_kernel<<<n_units, 256, 0, s>>>(loss_k, loss_v, nseg, n_dense, sparse, out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_strategy_threshold(const double* loss_k, const double* loss_v, int ncand, long long n,
+                                      const mkv_strategy* cands_dev, double tau, mkv_strategy* out,
+                                      cudaStream_t s) {
+    const int threads = 256;
+    const long long blocks = (n + threads - 1) / threads;
+    mkv_strategy_threshold_kernel<<<(unsigned)blocks, threads, 0, s>>>(loss_k, loss_v, ncand, n, cands_dev, tau, out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_compress(const CacheGeom& g, const LayerView& lv, const CompressArgs& a,
+                            const mkv_strategy* strat, unsigned long long* call_base, uint32_t* dev_flags,
+                            cudaStream_t s, int* n_kernels) {
+    const int units = a.nb * g.n_kv_heads;
+    mkv_plan_kernel<<<units, 256, 0, s>>>(g, lv, a, strat, call_base, dev_flags);
+    cudaError_t err = cudaGetLastError();
+    if (err != cudaSuccess) return err;
+    const int chunks = (g.blocks_per_seg + 7) / 8;
+    dim3 grid(a.nseg * chunks, units);
+    mkv_compress_kernel<<<grid, 256, 0, s>>>(g, lv, a, call_base, chunks);
+    if (n_kernels) *n_kernels = 2;
+    return cudaGetLastError();
+}
+
+}  // namespace mkv

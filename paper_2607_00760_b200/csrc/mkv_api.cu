@@ -1,0 +1,427 @@
+// mkv_api.cu — the C ABI of libmkv (include/mkv.h): cache lifetime, host-side argument checks,
+// export of the canonical blob, and dispatch to the kernels.  No CPU fallback exists: every
+// step of the path runs in the CUDA kernels of this library.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "mkv_internal.cuh"
+
+using namespace mkv;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define MKV_CUDA(expr)                                                                          \
+    do {                                                                                        \
+        cudaError_t e_ = (expr);                                                                \
+        if (e_ != cudaSuccess)                                                                  \
+            return fail(e_ == cudaErrorMemoryAllocation ? MKV_E_NOMEM : MKV_E_CUDA, "%s: %s", #expr, \
+                        cudaGetErrorString(e_));                                                \
+    } while (0)
+
+uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace
+
+struct mkv_cache {
+    mkv_cache_desc desc{};
+    CacheGeom geom{};
+    int sm_count = 0;
+    // device
+    uint8_t* arena = nullptr;
+    uint64_t slice_bytes = 0;
+    StratRec* strat = nullptr;
+    uint32_t* tok_off = nullptr;
+    uint32_t* bk_off = nullptr;
+    int32_t* unit_nseg = nullptr;
+    int32_t* unit_ntok = nullptr;
+    unsigned long long* counters = nullptr;  // [n_layers][4]: bump, used_tok, used_bk, pad
+    uint32_t* dev_flags = nullptr;
+    unsigned long long* call_base = nullptr;  // [n_units]
+    float* scores = nullptr;                  // [n_units][score_stride]
+    AttnScratch attn{};
+    uint16_t* q_dev = nullptr;
+    int32_t* sel_dev = nullptr;
+    int32_t* selcnt_dev = nullptr;
+    float* out_dev = nullptr;
+    mkv_strategy* cands_dev = nullptr;
+    int sel_cap = 0;
+    // host mirrors of the append state, [n_layers][batch]
+    std::vector<int32_t> host_nseg, host_ntok;
+    int last_select = 0, last_attn = 0, last_compress = 0;
+
+    LayerView view(int layer) const {
+        LayerView v;
+        const size_t tu = (size_t)layer * geom.n_units;
+        v.slice = arena + (size_t)layer * slice_bytes;
+        v.slice_bytes = slice_bytes;
+        v.strat = strat + tu * geom.S_max;
+        v.tok_off = tok_off + tu * geom.S_max;
+        v.bk_off = bk_off + tu * geom.S_max;
+        v.unit_nseg = unit_nseg + tu;
+        v.unit_ntok = unit_ntok + tu;
+        v.bump = counters + (size_t)layer * 4;
+        v.used_tok = v.bump + 1;
+        v.used_bk = v.bump + 2;
+        v.S_max = geom.S_max;
+        return v;
+    }
+};
+
+extern "C" {
+
+const char* mkv_last_error(void) { return g_err; }
+int mkv_version(void) { return 1; }
+
+int mkv_cache_free(mkv_cache* c) {
+    if (!c) return MKV_OK;
+    cudaSetDevice(c->desc.device);
+    cudaDeviceSynchronize();
+    void* ptrs[] = {c->arena, c->strat, c->tok_off, c->bk_off, c->unit_nseg, c->unit_ntok, c->counters,
+                    c->dev_flags, c->call_base, c->scores, c->attn.part_o, c->attn.part_ml, c->q_dev,
+                    c->sel_dev, c->selcnt_dev, c->out_dev, c->cands_dev};
+    for (void* p : ptrs)
+        if (p) cudaFree(p);
+    delete c;
+    return MKV_OK;
+}
+
+int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
+    if (!d || !out) return fail(MKV_E_ARG, "mkv_cache_create: NULL argument");
+    *out = nullptr;
+    if (d->n_layers < 1 || d->batch < 1 || d->n_kv_heads < 1 || d->n_q_heads < 1 || d->max_tokens < 1)
+        return fail(MKV_E_ARG, "mkv_cache_create: non-positive size");
+    if (d->n_q_heads % d->n_kv_heads) return fail(MKV_E_ARG, "n_q_heads must be a multiple of n_kv_heads");
+    if (d->head_dim != kD) return fail(MKV_E_UNSUPPORTED, "head_dim %d: only 128 is built", d->head_dim);
+    if (d->n_q_heads / d->n_kv_heads > kMaxGroup)
+        return fail(MKV_E_UNSUPPORTED, "GQA group %d > %d", d->n_q_heads / d->n_kv_heads, kMaxGroup);
+    if (d->segment_len < kB || d->segment_len % kB || d->segment_len > 4096)
+        return fail(MKV_E_UNSUPPORTED, "segment_len %d: need a multiple of 8 in [8, 4096]", d->segment_len);
+    int ndev = 0;
+    MKV_CUDA(cudaGetDeviceCount(&ndev));
+    if (d->device < 0 || d->device >= ndev) return fail(MKV_E_ARG, "device %d of %d", d->device, ndev);
+    MKV_CUDA(cudaSetDevice(d->device));
+
+    mkv_cache* c = new (std::nothrow) mkv_cache();
+    if (!c) return fail(MKV_E_NOMEM, "host allocation failed");
+    c->desc = *d;
+    CacheGeom& g = c->geom;
+    g.n_layers = d->n_layers; g.batch = d->batch; g.n_kv_heads = d->n_kv_heads; g.n_q_heads = d->n_q_heads;
+    g.group = d->n_q_heads / d->n_kv_heads; g.max_tokens = d->max_tokens; g.L = d->segment_len;
+    g.S_max = (d->max_tokens + g.L - 1) / g.L; g.n_units = d->batch * d->n_kv_heads;
+    g.blocks_per_seg = g.L / kB; g.score_stride = (d->max_tokens + kB - 1) / kB;
+    MKV_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, d->device));
+
+    const uint64_t worst = (uint64_t)g.n_units * ((uint64_t)g.score_stride * (4096 + 256) + 64) + 4096;
+    uint64_t per_layer = d->arena_bytes ? d->arena_bytes / (uint64_t)d->n_layers : worst;
+    per_layer = per_layer / 256 * 256;
+    if (per_layer < 256) { delete c; return fail(MKV_E_ARG, "arena_bytes too small"); }
+    c->slice_bytes = per_layer;
+
+    const size_t tu = (size_t)g.n_layers * g.n_units;
+    c->attn.max_splits = 64;
+    c->sel_cap = g.score_stride + 1;
+    struct { void** p; size_t bytes; } allocs[] = {
+        {(void**)&c->arena, (size_t)per_layer * g.n_layers},
+        {(void**)&c->strat, tu * g.S_max * sizeof(StratRec)},
+        {(void**)&c->tok_off, tu * g.S_max * 4},
+        {(void**)&c->bk_off, tu * g.S_max * 4},
+        {(void**)&c->unit_nseg, tu * 4},
+        {(void**)&c->unit_ntok, tu * 4},
+        {(void**)&c->counters, (size_t)g.n_layers * 4 * 8},
+        {(void**)&c->dev_flags, 256},
+        {(void**)&c->call_base, (size_t)g.n_units * 8},
+        {(void**)&c->scores, (size_t)g.n_units * g.score_stride * 4},
+        {(void**)&c->attn.part_o, (size_t)g.n_units * c->attn.max_splits * g.group * kD * 4},
+        {(void**)&c->attn.part_ml, (size_t)g.n_units * c->attn.max_splits * g.group * 2 * 4},
+        {(void**)&c->q_dev, (size_t)g.batch * g.n_q_heads * kD * 2},
+        {(void**)&c->sel_dev, (size_t)g.n_units * c->sel_cap * 4},
+        {(void**)&c->selcnt_dev, (size_t)g.n_units * 4},
+        {(void**)&c->out_dev, (size_t)g.batch * g.n_q_heads * kD * 4},
+        {(void**)&c->cands_dev, 64 * sizeof(mkv_strategy)},
+    };
+    for (auto& a : allocs) {
+        cudaError_t e = cudaMalloc(a.p, a.bytes);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            mkv_cache_free(c);
+            return fail(MKV_E_NOMEM, "cudaMalloc(%zu bytes): %s", a.bytes, cudaGetErrorString(e));
+        }
+    }
+    cudaMemset(c->unit_nseg, 0, tu * 4);
+    cudaMemset(c->unit_ntok, 0, tu * 4);
+    cudaMemset(c->counters, 0, (size_t)g.n_layers * 4 * 8);
+    cudaMemset(c->dev_flags, 0, 256);
+    cudaMemset(c->strat, 0, tu * g.S_max * sizeof(StratRec));
+    c->host_nseg.assign((size_t)g.n_layers * g.batch, 0);
+    c->host_ntok.assign((size_t)g.n_layers * g.batch, 0);
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) {
+        mkv_cache_free(c);
+        return fail(MKV_E_CUDA, "create: %s", cudaGetErrorString(e));
+    }
+    *out = c;
+    return MKV_OK;
+}
+
+int mkv_cache_reset(mkv_cache* c, int32_t layer, void* stream) {
+    if (!c) return fail(MKV_E_ARG, "NULL cache");
+    const CacheGeom& g = c->geom;
+    if (layer < -1 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    cudaStream_t s = (cudaStream_t)stream;
+    const int l0 = layer < 0 ? 0 : layer, l1 = layer < 0 ? g.n_layers : layer + 1;
+    for (int l = l0; l < l1; ++l) {
+        MKV_CUDA(cudaMemsetAsync(c->unit_nseg + (size_t)l * g.n_units, 0, (size_t)g.n_units * 4, s));
+        MKV_CUDA(cudaMemsetAsync(c->unit_ntok + (size_t)l * g.n_units, 0, (size_t)g.n_units * 4, s));
+        MKV_CUDA(cudaMemsetAsync(c->counters + (size_t)l * 4, 0, 32, s));
+        for (int b = 0; b < g.batch; ++b) c->host_nseg[(size_t)l * g.batch + b] = c->host_ntok[(size_t)l * g.batch + b] = 0;
+    }
+    return MKV_OK;
+}
+
+static int check_kv_args(const mkv_cache* c, const char* fn, const void* k, const void* v, int64_t sb, int64_t sh,
+                         int64_t st, int32_t b0, int32_t nb, int32_t seg0, int32_t nseg, int32_t n_tok) {
+    if (!c || !k || !v) return fail(MKV_E_ARG, "%s: NULL argument", fn);
+    const CacheGeom& g = c->geom;
+    if (b0 < 0 || nb < 1 || b0 + nb > g.batch) return fail(MKV_E_ARG, "%s: requests [%d, %d) of %d", fn, b0, b0 + nb, g.batch);
+    if (n_tok < 1 || nseg < 1 || seg0 < 0) return fail(MKV_E_ARG, "%s: empty range", fn);
+    if (nseg != (n_tok + g.L - 1) / g.L) return fail(MKV_E_ARG, "%s: nseg %d != ceil(n_tok %d / L %d)", fn, nseg, n_tok, g.L);
+    if ((int64_t)seg0 * g.L + n_tok > g.max_tokens) return fail(MKV_E_ARG, "%s: tokens exceed max_tokens %d", fn, g.max_tokens);
+    if (st < kD || sh < 0 || sb < 0) return fail(MKV_E_ARG, "%s: bad strides", fn);
+    return MKV_OK;
+}
+
+int mkv_segment_loss(const mkv_cache* c, const void* k, const void* v, int64_t sb, int64_t sh, int64_t st, int32_t b0,
+                     int32_t nb, int32_t seg0, int32_t nseg, int32_t n_tok, mkv_strategy cand, double* loss_k,
+                     double* loss_v, void* stream) {
+    int rc = check_kv_args(c, "mkv_segment_loss", k, v, sb, sh, st, b0, nb, seg0, nseg, n_tok);
+    if (rc) return rc;
+    if (!loss_k || !loss_v) return fail(MKV_E_ARG, "mkv_segment_loss: NULL output");
+    if (cand.r_k < 1 || cand.r_k > kD || cand.r_v < 1 || cand.r_v > kD) return fail(MKV_E_ARG, "candidate r out of range");
+    if (cand.g != 1) return fail(MKV_E_UNSUPPORTED, "element group %d: only g = 1 is built", cand.g);
+    CompressArgs a{(const uint16_t*)k, (const uint16_t*)v, sb, sh, st, b0, nb, seg0, nseg, n_tok};
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(launch_segment_loss(c->geom, a, cand, loss_k, loss_v, (cudaStream_t)stream));
+    return MKV_OK;
+}
+
+int mkv_strategy_quantile(const mkv_cache* c, const double* loss_k, const double* loss_v, int32_t n_units, int32_t nseg,
+                          int32_t dense_num, int32_t dense_den, mkv_strategy sparse, mkv_strategy* out, void* stream) {
+    if (!c || !loss_k || !loss_v || !out) return fail(MKV_E_ARG, "mkv_strategy_quantile: NULL argument");
+    if (n_units < 1 || nseg < 1 || dense_den < 1 || dense_num < 0 || dense_num > dense_den)
+        return fail(MKV_E_ARG, "mkv_strategy_quantile: bad sizes");
+    long long nd = ((long long)nseg * dense_num + dense_den - 1) / dense_den;
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(launch_strategy_quantile(loss_k, loss_v, n_units, nseg, (int)nd, sparse, out, (cudaStream_t)stream));
+    return MKV_OK;
+}
+
+int mkv_strategy_threshold(const mkv_cache* c, const double* loss_k, const double* loss_v, int32_t ncand,
+                           int32_t n_units, int32_t nseg, const mkv_strategy* cands_host, double tau,
+                           mkv_strategy* out, void* stream) {
+    if (!c || !loss_k || !loss_v || !out || !cands_host) return fail(MKV_E_ARG, "mkv_strategy_threshold: NULL argument");
+    if (ncand < 1 || ncand > 64 || n_units < 1 || nseg < 1) return fail(MKV_E_ARG, "mkv_strategy_threshold: bad sizes");
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(cudaMemcpyAsync(c->cands_dev, cands_host, ncand * sizeof(mkv_strategy), cudaMemcpyHostToDevice,
+                             (cudaStream_t)stream));
+    MKV_CUDA(launch_strategy_threshold(loss_k, loss_v, ncand, (long long)n_units * nseg, c->cands_dev, tau, out,
+                                       (cudaStream_t)stream));
+    return MKV_OK;
+}
+
+int mkv_compress_segment(mkv_cache* c, int32_t layer, const void* k, const void* v, int64_t sb, int64_t sh, int64_t st,
+                         int32_t b0, int32_t nb, int32_t seg0, int32_t nseg, int32_t n_tok, const mkv_strategy* strat,
+                         void* stream) {
+    int rc = check_kv_args(c, "mkv_compress_segment", k, v, sb, sh, st, b0, nb, seg0, nseg, n_tok);
+    if (rc) return rc;
+    if (!strat) return fail(MKV_E_ARG, "mkv_compress_segment: NULL strategy");
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    for (int b = b0; b < b0 + nb; ++b) {
+        const int have = c->host_nseg[(size_t)layer * g.batch + b];
+        const int tok = c->host_ntok[(size_t)layer * g.batch + b];
+        if (seg0 != have) return fail(MKV_E_STATE, "request %d holds %d segments; seg0 = %d (append-only)", b, have, seg0);
+        if (tok != have * g.L) return fail(MKV_E_STATE, "request %d ends in a short segment; cannot append", b);
+    }
+    CompressArgs a{(const uint16_t*)k, (const uint16_t*)v, sb, sh, st, b0, nb, seg0, nseg, n_tok};
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(launch_compress(g, c->view(layer), a, strat, c->call_base, c->dev_flags, (cudaStream_t)stream,
+                             &c->last_compress));
+    for (int b = b0; b < b0 + nb; ++b) {
+        c->host_nseg[(size_t)layer * g.batch + b] = seg0 + nseg;
+        c->host_ntok[(size_t)layer * g.batch + b] = seg0 * g.L + n_tok;
+    }
+    return MKV_OK;
+}
+
+int mkv_select(const mkv_cache* cc, int32_t layer, const void* q, int32_t budget, int32_t reduce, int32_t* sel,
+               int32_t* sel_count, int32_t k_max, float* scores_opt, void* stream) {
+    if (!cc || !q || !sel || !sel_count) return fail(MKV_E_ARG, "mkv_select: NULL argument");
+    mkv_cache* c = const_cast<mkv_cache*>(cc);
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    if (budget < 0 || (reduce != 0 && reduce != 1)) return fail(MKV_E_ARG, "mkv_select: bad budget/reduce");
+    const long long need = (long long)budget / kB + 1;
+    if (k_max < 1 || k_max < (need < g.score_stride ? need : g.score_stride))
+        return fail(MKV_E_ARG, "mkv_select: k_max %d too small for budget %d", k_max, budget);
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(launch_select(g, c->view(layer), (const uint16_t*)q, budget, reduce, sel, sel_count, k_max,
+                           scores_opt ? scores_opt : c->scores, (cudaStream_t)stream, &c->last_select));
+    return MKV_OK;
+}
+
+int mkv_packed_attention(const mkv_cache* cc, int32_t layer, const void* q, const int32_t* sel,
+                         const int32_t* sel_count, int32_t k_max, float scale, float* out, float* lse_opt,
+                         void* stream) {
+    if (!cc || !q || !sel || !sel_count || !out) return fail(MKV_E_ARG, "mkv_packed_attention: NULL argument");
+    mkv_cache* c = const_cast<mkv_cache*>(cc);
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    if (k_max < 1) return fail(MKV_E_ARG, "mkv_packed_attention: k_max < 1");
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(launch_attention(g, c->view(layer), (const uint16_t*)q, sel, sel_count, k_max, scale, out, lse_opt,
+                              c->attn, c->sm_count, (cudaStream_t)stream, &c->last_attn));
+    return MKV_OK;
+}
+
+int mkv_decode_host(mkv_cache* c, int32_t layer, const void* q_host, int32_t budget, int32_t reduce, float scale,
+                    float* out_host, int32_t* sel_host_opt, int32_t* sel_count_host_opt, void* stream) {
+    if (!c || !q_host || !out_host) return fail(MKV_E_ARG, "mkv_decode_host: NULL argument");
+    const CacheGeom& g = c->geom;
+    cudaStream_t s = (cudaStream_t)stream;
+    long long k_max = (long long)budget / kB + 1;
+    if (k_max > c->sel_cap) k_max = c->sel_cap;
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(cudaMemcpyAsync(c->q_dev, q_host, (size_t)g.batch * g.n_q_heads * kD * 2, cudaMemcpyHostToDevice, s));
+    int rc = mkv_select(c, layer, c->q_dev, budget, reduce, c->sel_dev, c->selcnt_dev, (int)k_max, nullptr, stream);
+    if (rc) return rc;
+    rc = mkv_packed_attention(c, layer, c->q_dev, c->sel_dev, c->selcnt_dev, (int)k_max, scale, c->out_dev, nullptr, stream);
+    if (rc) return rc;
+    MKV_CUDA(cudaMemcpyAsync(out_host, c->out_dev, (size_t)g.batch * g.n_q_heads * kD * 4, cudaMemcpyDeviceToHost, s));
+    if (sel_host_opt)
+        MKV_CUDA(cudaMemcpyAsync(sel_host_opt, c->sel_dev, (size_t)g.n_units * k_max * 4, cudaMemcpyDeviceToHost, s));
+    if (sel_count_host_opt)
+        MKV_CUDA(cudaMemcpyAsync(sel_count_host_opt, c->selcnt_dev, (size_t)g.n_units * 4, cudaMemcpyDeviceToHost, s));
+    return MKV_OK;
+}
+
+int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, void* buf, uint64_t cap,
+                     uint64_t* need_host) {
+    if (!c || !need_host) return fail(MKV_E_ARG, "mkv_cache_export: NULL argument");
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers || b < 0 || b >= g.batch || h < 0 || h >= g.n_kv_heads)
+        return fail(MKV_E_ARG, "mkv_cache_export: unit out of range");
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(cudaDeviceSynchronize());
+    const int unit = b * g.n_kv_heads + h;
+    const LayerView lv = c->view(layer);
+    int32_t S = 0, N = 0;
+    MKV_CUDA(cudaMemcpy(&S, lv.unit_nseg + unit, 4, cudaMemcpyDeviceToHost));
+    MKV_CUDA(cudaMemcpy(&N, lv.unit_ntok + unit, 4, cudaMemcpyDeviceToHost));
+    std::vector<StratRec> rec(S);
+    std::vector<uint32_t> toff(S), koff(S);
+    if (S) {
+        MKV_CUDA(cudaMemcpy(rec.data(), lv.strat + (size_t)unit * lv.S_max, (size_t)S * 8, cudaMemcpyDeviceToHost));
+        MKV_CUDA(cudaMemcpy(toff.data(), lv.tok_off + (size_t)unit * lv.S_max, (size_t)S * 4, cudaMemcpyDeviceToHost));
+        MKV_CUDA(cudaMemcpy(koff.data(), lv.bk_off + (size_t)unit * lv.S_max, (size_t)S * 4, cudaMemcpyDeviceToHost));
+    }
+    uint64_t tok_bytes = 0, bk_bytes = 0;
+    for (int s = 0; s < S; ++s) {
+        tok_bytes += seg_tok_bytes(rec[s].r_k, rec[s].r_v, rec[s].n_tok);
+        bk_bytes += seg_bk_bytes(rec[s].r_k, rec[s].n_tok);
+    }
+    const uint64_t tables = align_up(48 + (uint64_t)S * 16, 16);
+    const uint64_t need = tables + tok_bytes + bk_bytes;
+    *need_host = need;
+    if (!buf) return MKV_OK;
+    if (cap < need) return fail(MKV_E_ARG, "mkv_cache_export: need %llu bytes, cap %llu", (unsigned long long)need,
+                                (unsigned long long)cap);
+    uint8_t* p = (uint8_t*)buf;
+    memset(p, 0, tables);
+    const uint32_t hdr[6] = {0x31564B4Du, (uint32_t)kD, (uint32_t)N, (uint32_t)g.L, (uint32_t)S, 0u};
+    memcpy(p, hdr, 24);
+    memcpy(p + 24, &tok_bytes, 8);
+    memcpy(p + 32, &bk_bytes, 8);
+    uint8_t* p_strat = p + 48;
+    uint8_t* p_toff = p_strat + (size_t)S * 8;
+    uint8_t* p_koff = p_toff + (size_t)S * 4;
+    uint8_t* tok_arena = p + tables;
+    uint8_t* bk_arena = tok_arena + tok_bytes;
+    // canonical offsets are exclusive prefix sums; physical runs that are contiguous are copied at once
+    uint64_t tpos = 0, kpos = 0;
+    int s = 0;
+    while (s < S) {
+        int e = s;
+        uint64_t trun = 0, krun = 0;
+        while (e < S) {
+            const uint64_t tb = seg_tok_bytes(rec[e].r_k, rec[e].r_v, rec[e].n_tok), kb = seg_bk_bytes(rec[e].r_k, rec[e].n_tok);
+            if (e > s && ((uint64_t)toff[e] * 16 != (uint64_t)toff[s] * 16 + trun || (uint64_t)koff[e] * 16 != (uint64_t)koff[s] * 16 + krun))
+                break;
+            const uint32_t ct = (uint32_t)((tpos + trun) / 16), ck = (uint32_t)((kpos + krun) / 16);
+            memcpy(p_strat + (size_t)e * 8, &rec[e], 8);
+            memcpy(p_toff + (size_t)e * 4, &ct, 4);
+            memcpy(p_koff + (size_t)e * 4, &ck, 4);
+            trun += tb;
+            krun += kb;
+            ++e;
+        }
+        MKV_CUDA(cudaMemcpy(tok_arena + tpos, lv.slice + (uint64_t)toff[s] * 16, trun, cudaMemcpyDeviceToHost));
+        MKV_CUDA(cudaMemcpy(bk_arena + kpos, lv.slice + (uint64_t)koff[s] * 16, krun, cudaMemcpyDeviceToHost));
+        tpos += trun;
+        kpos += krun;
+        s = e;
+    }
+    return MKV_OK;
+}
+
+int mkv_cache_bytes(const mkv_cache* c, int32_t layer, uint64_t* packed, uint64_t* block_keys, uint64_t* tables) {
+    if (!c) return fail(MKV_E_ARG, "NULL cache");
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(cudaDeviceSynchronize());
+    unsigned long long cnt[4];
+    MKV_CUDA(cudaMemcpy(cnt, c->counters + (size_t)layer * 4, 32, cudaMemcpyDeviceToHost));
+    std::vector<int32_t> nseg(g.n_units);
+    MKV_CUDA(cudaMemcpy(nseg.data(), c->unit_nseg + (size_t)layer * g.n_units, (size_t)g.n_units * 4, cudaMemcpyDeviceToHost));
+    uint64_t segs = 0;
+    for (int v : nseg) segs += (uint64_t)v;
+    if (packed) *packed = cnt[1];
+    if (block_keys) *block_keys = cnt[2];
+    if (tables) *tables = segs * 16;
+    return MKV_OK;
+}
+
+int mkv_cache_status(const mkv_cache* c, uint32_t* flags_host) {
+    if (!c) return fail(MKV_E_ARG, "NULL cache");
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(cudaDeviceSynchronize());
+    uint32_t f = 0;
+    MKV_CUDA(cudaMemcpy(&f, c->dev_flags, 4, cudaMemcpyDeviceToHost));
+    if (flags_host) *flags_host = f;
+    if (f) return fail(MKV_E_DEVICE, "device flags 0x%x (%s%s)", f, (f & MKV_DEV_ARENA_OVERFLOW) ? "arena overflow " : "",
+                       (f & MKV_DEV_BAD_STRATEGY) ? "bad strategy" : "");
+    return MKV_OK;
+}
+
+int mkv_last_launch_count(const mkv_cache* c, int32_t* sel_k, int32_t* attn_k, int32_t* comp_k) {
+    if (!c) return fail(MKV_E_ARG, "NULL cache");
+    if (sel_k) *sel_k = c->last_select;
+    if (attn_k) *attn_k = c->last_attn;
+    if (comp_k) *comp_k = c->last_compress;
+    return MKV_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,104 @@
+// mkv_internal.cuh — shared declarations of libmkv's CUDA translation units (sm_100a).
+// Nothing here is used by, or derived from, the CPU oracle under oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "mkv.h"
+
+namespace mkv {
+
+constexpr int kD = 128;          // head_dim supported on the GPU
+constexpr int kB = 8;            // token-block size supported on the GPU
+constexpr int kMaxGroup = 8;     // GQA group size limit
+constexpr int kBitmapBytes = 16; // D/g/8 at g = 1
+
+// strategy record as stored in the per-unit table and in the canonical blob (8 bytes)
+struct __align__(8) StratRec {
+    uint8_t r_k, r_v, g, B;
+    uint16_t n_tok, flags;
+};
+static_assert(sizeof(StratRec) == 8, "strategy record is 8 bytes");
+
+// Device-resident tables of one layer.  Offsets are in 16-byte units from `slice`.
+struct LayerView {
+    uint8_t* slice;               // packed payload slice of this layer (256-B aligned)
+    uint64_t slice_bytes;
+    StratRec* strat;              // [n_units][S_max]
+    uint32_t* tok_off;            // [n_units][S_max]  token-block payloads of a segment
+    uint32_t* bk_off;             // [n_units][S_max]  block-key payload of a segment
+    int32_t* unit_nseg;           // [n_units]
+    int32_t* unit_ntok;           // [n_units]
+    unsigned long long* bump;     // bytes of `slice` in use
+    unsigned long long* used_tok; // token-payload bytes in use (statistics)
+    unsigned long long* used_bk;  // block-key payload bytes in use (statistics)
+    int32_t S_max;
+};
+
+struct CacheGeom {
+    int32_t n_layers, batch, n_kv_heads, n_q_heads, group, max_tokens, L, S_max, n_units;
+    int32_t blocks_per_seg;   // L / 8
+    int32_t score_stride;     // ceil(max_tokens / 8): blocks per unit capacity
+};
+
+// bytes of payloads (canonical sizes)
+__host__ __device__ inline uint32_t pad16u(uint32_t x) { return (x + 15u) & ~15u; }
+__host__ __device__ inline uint32_t vec_bytes(int r) { return (r == kD ? 0u : (uint32_t)kBitmapBytes) + 2u * (uint32_t)r; }
+__host__ __device__ inline uint32_t tokblock_bytes(int r_k, int r_v, int nb) {
+    return pad16u((uint32_t)nb * (vec_bytes(r_k) + vec_bytes(r_v)));
+}
+__host__ __device__ inline uint32_t seg_tok_bytes(int r_k, int r_v, int n_tok) {
+    int full = n_tok / kB, rem = n_tok % kB;
+    return (uint32_t)full * tokblock_bytes(r_k, r_v, kB) + (rem ? tokblock_bytes(r_k, r_v, rem) : 0u);
+}
+__host__ __device__ inline uint32_t seg_bk_bytes(int r_k, int n_tok) {
+    int nblk = (n_tok + kB - 1) / kB;
+    return pad16u((uint32_t)nblk * vec_bytes(r_k));
+}
+
+// ---- launchers (each enqueues on `stream`; returns cudaError) -----------------------------
+struct CompressArgs {
+    const uint16_t* k;
+    const uint16_t* v;
+    int64_t stride_b, stride_h, stride_t;
+    int32_t b0, nb, seg0, nseg, n_tok;
+};
+
+cudaError_t launch_segment_loss(const CacheGeom& g, const CompressArgs& a, mkv_strategy cand,
+                                double* loss_k, double* loss_v, cudaStream_t s);
+cudaError_t launch_strategy_quantile(const double* loss_k, const double* loss_v, int n_units,
+                                     int nseg, int n_dense, mkv_strategy sparse,
+                                     mkv_strategy* out, cudaStream_t s);
+cudaError_t launch_strategy_threshold(const double* loss_k, const double* loss_v, int ncand,
+                                      long long n, const mkv_strategy* cands_dev, double tau,
+                                      mkv_strategy* out, cudaStream_t s);
+cudaError_t launch_compress(const CacheGeom& g, const LayerView& lv, const CompressArgs& a,
+                            const mkv_strategy* strat, unsigned long long* call_base,
+                            uint32_t* dev_flags, cudaStream_t s, int* n_kernels);
+
+cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_t* q, int budget,
+                          int reduce, int32_t* sel, int32_t* sel_count, int k_max, float* scores,
+                          cudaStream_t s, int* n_kernels);
+
+struct AttnScratch {
+    float* part_o;    // [n_units][max_splits][G][D]
+    float* part_ml;   // [n_units][max_splits][G][2]  (running max in log2 units, sum)
+    int32_t max_splits;
+};
+cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q,
+                             const int32_t* sel, const int32_t* sel_count, int k_max, float scale,
+                             float* out, float* lse, const AttnScratch& scr, int sm_count,
+                             cudaStream_t s, int* n_kernels);
+
+// ---- small device helpers -----------------------------------------------------------------
+__device__ __forceinline__ float bf16_bits_to_f32(uint32_t h) { return __uint_as_float(h << 16); }
+
+// round-to-nearest-even fp32 -> bf16 bits (finite inputs)
+__device__ __forceinline__ uint32_t f32_to_bf16_bits_rne(float f) {
+    uint32_t u = __float_as_uint(f);
+    u += 0x7FFFu + ((u >> 16) & 1u);
+    return u >> 16;
+}
+
+}  // namespace mkv
