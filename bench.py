@@ -1,0 +1,414 @@
+#!/usr/bin/env python
+"""bench.py — MosaicKV decode hot path on B200: PackedAttention us/layer and % of the HBM roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload llama8b-128k-b8] [--layers n]
+    python bench.py --impl reference ...        # the CPU oracle on a bounded sample (slow on purpose)
+
+A step = one decode step over all layers of the workload: per layer mkv_select (score + top-k on
+the packed block keys) and mkv_packed_attention (packed QK, softmax, PV, split-K combine), on a
+cache that was compressed (mkv_segment_loss -> mkv_strategy_quantile -> mkv_compress_segment,
+timed and reported under "compress") before the timed region.  Consecutive layers touch different
+packed arenas (1.9 GB each at config 2), so inputs are far larger than L2 (126 MB).
+
+Prints ONE JSON line (see DESIGN.md "Measurement" for every key).
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "PackedAttention us/layer (8B-shape, 128K ctx, batch 8)"
+UNIT = "us/layer"
+NOMINAL_HBM_GBS = 8000.0
+FALLBACK_HBM_GBS = 6650.0
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="llama8b-128k-b8")
+    ap.add_argument("--layers", type=int, default=0, help="0 = all layers of the workload")
+    ap.add_argument("--batch", type=int, default=0)
+    ap.add_argument("--context", type=int, default=0)
+    ap.add_argument("--impl", default="mkv", choices=["mkv", "reference"])
+    ap.add_argument("--no-graph", action="store_true", help="launch eagerly instead of CUDA graphs")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-units", type=int, default=8, help="units of one layer the oracle is timed on")
+    ap.add_argument("--verbose", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """SM clock + throttle reasons sampled through NVML DURING the timed region (same fields as the
+    nvidia-smi line of B200_PROFILING.md, polled every ~2 ms from a thread so that a region of a few
+    tens of milliseconds still gets samples)."""
+
+    def __init__(self, torch_index):
+        self.samples, self.reasons, self.max_mhz, self.h, self._stop, self.th = [], set(), None, None, False, None
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            p = torch.cuda.get_device_properties(torch_index)
+            bus = "%08x:%02x:%02x.0" % (p.pci_domain_id, p.pci_bus_id, p.pci_device_id)
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByPciBusId(bus.encode())
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.h = None
+
+    def _run(self):
+        nv = self.nv
+        bits = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                "hw_power_brake_slowdown": 0x80}
+        while not self._stop:
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for n, b in bits.items():
+                    if r & b:
+                        self.reasons.add(n)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def start(self):
+        if self.h is None:
+            return
+        import threading
+        self._stop = False
+        self.th = threading.Thread(target=self._run, daemon=True)
+        self.th.start()
+
+    def stop(self):
+        if self.th is not None:
+            self._stop = True
+            self.th.join()
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+# ------------------------------------------------------------------------------ timing helpers
+
+def timed_loop(torch, fn, steps, warmup, dist_barrier, graph=True):
+    """W untimed + K timed calls of fn() on torch's current stream; returns ms per call.
+    fn's launches are captured in one CUDA graph (launch-bound inner loop) unless graph=False."""
+    stream = torch.cuda.current_stream()
+    runner = fn
+    if graph:
+        fn()  # warm (lazy module load) before capture
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=torch.cuda.Stream()):
+            fn()
+        runner = g.replay
+    for _ in range(warmup):
+        runner()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dist_barrier()
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(steps):
+        runner()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    dist_barrier()
+    return e0.elapsed_time(e1) / steps
+
+
+def max_over_ranks(torch, dist, x, world):
+    if world == 1:
+        return x
+    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+# ------------------------------------------------------------------------------ the mkv arm
+
+def run_mkv(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    barrier = (lambda: dist.barrier()) if world > 1 else (lambda: None)
+
+    import __graft_entry__
+    if rank == 0:
+        __graft_entry__.build()
+    barrier()
+    from paper_2607_00760_b200 import binding as mkv
+    from paper_2607_00760_b200 import synth, workload
+
+    w = synth.WORKLOADS[args.workload]
+    n_layers = args.layers or w.n_layers
+    Bt = args.batch or w.batch
+    N = args.context or w.context
+    # weak scaling: every rank holds its own batch of Bt requests (units are independent: no collective)
+    if world > 1:
+        w = synth.Workload(**{**w.__dict__, "seed": w.seed + rank, "config_id": w.config_id})
+    t0 = time.time()
+    built = workload.build(w, dev, n_layers=n_layers, batch=Bt, context=N, verbose=args.verbose and rank == 0)
+    build_s = time.time() - t0
+    cache = built.cache
+    Hkv, Hq, G = w.n_kv_heads, w.n_q_heads, w.group
+    budget = w.token_budget
+    k_max = min(budget // 8 + 1, (N + 7) // 8)
+    scale = 1.0 / math.sqrt(128)
+    sel = [torch.full((Bt, Hkv, k_max), -1, dtype=torch.int32, device=dev) for _ in range(n_layers)]
+    cnt = [torch.zeros((Bt, Hkv), dtype=torch.int32, device=dev) for _ in range(n_layers)]
+    out = torch.zeros((n_layers, Bt, Hq, 128), dtype=torch.float32, device=dev)
+
+    def step_select():
+        for l in range(n_layers):
+            cache.select(l, built.q[l], budget, sel[l], cnt[l])
+
+    def step_attention():
+        for l in range(n_layers):
+            cache.packed_attention(l, built.q[l], sel[l], cnt[l], scale, out[l])
+
+    def step_decode():
+        for l in range(n_layers):
+            cache.select(l, built.q[l], budget, sel[l], cnt[l])
+            cache.packed_attention(l, built.q[l], sel[l], cnt[l], scale, out[l])
+
+    step_decode()
+    torch.cuda.synchronize()
+    cache.status()
+    launches = cache.last_launch_count()
+    n_sel_total = [int(c.sum().item()) for c in cnt]
+    attn_bytes = [workload.attention_bytes(built, l, sel[l], cnt[l]) for l in range(n_layers)]
+    sel_bytes = [workload.select_bytes(built, l, n_sel_total[l]) for l in range(n_layers)]
+    comp_bytes = workload.compress_bytes(built, 0)
+
+    graph = not args.no_graph
+    clocks = ClockSampler(local)
+    clocks.start()
+    ms_step = timed_loop(torch, step_decode, args.steps, args.warmup, barrier, graph)
+    ms_attn = timed_loop(torch, step_attention, args.steps, args.warmup, barrier, graph)
+    ms_sel = timed_loop(torch, step_select, args.steps, args.warmup, barrier, graph)
+    clk = clocks.stop()
+
+    # end to end through the public host call: pinned q in, out back, every layer, every step
+    q_host = [q.cpu().pin_memory() for q in built.q]
+    out_host = [torch.zeros((Bt, Hq, 128), dtype=torch.float32).pin_memory() for _ in range(n_layers)]
+
+    def step_e2e():
+        for l in range(n_layers):
+            cache.decode_host(l, q_host[l], budget, scale, out_host[l])
+        torch.cuda.current_stream().synchronize()
+
+    ms_e2e = timed_loop(torch, step_e2e, max(3, args.steps // 2), 3, barrier, graph=False)
+    cache.status()
+
+    ms_step = max_over_ranks(torch, dist, ms_step, world)
+    ms_attn = max_over_ranks(torch, dist, ms_attn, world)
+    ms_sel = max_over_ranks(torch, dist, ms_sel, world)
+    ms_e2e = max_over_ranks(torch, dist, ms_e2e, world)
+
+    peak, peak_src = measured_peak()
+    us_attn = ms_attn * 1e3 / n_layers
+    us_sel = ms_sel * 1e3 / n_layers
+    a_bytes = sum(attn_bytes) / n_layers
+    s_bytes = sum(sel_bytes) / n_layers
+    attn_gbs = a_bytes / (us_attn * 1e-6) / 1e9
+    sel_gbs = s_bytes / (us_sel * 1e-6) / 1e9
+    comp_ms = np.array(built.compress_ms[1:] or built.compress_ms).mean(axis=0)
+    comp_gbs = (comp_bytes["read"] + comp_bytes["write"]) / (comp_ms[2] * 1e-3) / 1e9
+
+    line = {
+        "metric": METRIC, "value": round(us_attn, 3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16 storage, fp32 accumulate", "data": "synthetic",
+        "config": {"workload": w.name, "baseline_config": w.config_id, "n_layers": n_layers, "batch_per_gpu": Bt,
+                   "n_q_heads": Hq, "n_kv_heads": Hkv, "head_dim": 128, "context": N, "segment_len": w.segment_len,
+                   "token_block": 8, "keep_ratio": w.keep_ratio, "r_keep": w.r_keep,
+                   "dense_segments": f"{w.dense_num}/{w.dense_den}", "token_budget": budget,
+                   "l2": "inputs larger than L2: consecutive layers read different packed arenas",
+                   "launch": "cuda-graph of one decode step" if graph else "eager"},
+        "decode_tokens_per_s_attention_only": round(world * Bt / (ms_step * 1e-3), 1),
+        "select_us_per_layer": round(us_sel, 3),
+        "roofline": {"kernel": "mkv_packed_attention", "bound": "hbm", "achieved": round(attn_gbs, 1), "peak": peak,
+                     "unit": "GB/s", "frac": round(attn_gbs / peak, 4), "traffic": None, "peak_source": peak_src,
+                     "frac_of_nominal_8TBs": round(attn_gbs / NOMINAL_HBM_GBS, 4),
+                     "algorithmic_bytes_per_launch": int(a_bytes)},
+        "roofline_select": {"kernel": "mkv_select", "bound": "hbm", "achieved": round(sel_gbs, 1), "peak": peak,
+                            "unit": "GB/s", "frac": round(sel_gbs / peak, 4), "traffic": None,
+                            "algorithmic_bytes_per_launch": int(s_bytes)},
+        "compress": {"loss_ms_per_layer": round(float(comp_ms[0]), 3), "strategy_ms_per_layer": round(float(comp_ms[1]), 3),
+                     "compress_ms_per_layer": round(float(comp_ms[2]), 3), "achieved": round(comp_gbs, 1), "unit": "GB/s",
+                     "frac": round(comp_gbs / peak, 4), "bytes_read": comp_bytes["read"], "bytes_written": comp_bytes["write"],
+                     "build_all_layers_s": round(build_s, 2)},
+        "e2e": {"value": round(ms_e2e * 1e3 / n_layers, 3), "unit": "us/layer (select + attention, host q in, host out back)",
+                "h2d_bytes_per_step": n_layers * Bt * Hq * 128 * 2, "d2h_bytes_per_step": n_layers * Bt * Hq * 128 * 4,
+                "ms_per_step": round(ms_e2e, 4)},
+        "gpu_launches": args.steps * n_layers * (launches["select"] + launches["attention"]),
+        "kernels_per_layer": launches,
+        "clocks": clk,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(args, w, built, dev, n_units=args.cpu_units, repeats=1)
+    built.free()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------ the oracle legs
+
+def oracle_sample(w, units, N, verbose=False):
+    """units: list of (K u16 [N][D], V u16 [N][D], q u16 [G][D]).  Runs the oracle as it stands:
+    prep (loss -> strategy -> compress, one python thread per unit) then timed decode legs."""
+    import numpy as np
+    from concurrent.futures import ThreadPoolExecutor
+
+    import oracle as orc
+
+    r, L = w.r_keep, w.segment_len
+    S = N // L
+
+    def prep(u):
+        K, V, _ = u
+        if w.dense_num > 0:
+            lk, lv = orc.segment_loss(K, V, L, r, r)
+            st = orc.strategy_quantile(lk, lv, w.dense_num, w.dense_den, 128, r, r)
+        else:
+            st = orc.uniform_strategy(S, r, r)
+        return orc.compress_unit(K, V, L, st)
+
+    t0 = time.time()
+    with ThreadPoolExecutor(max(1, min(len(units), os.cpu_count() or 1))) as ex:
+        blobs = list(ex.map(prep, units))
+    prep_s = time.time() - t0
+    q = np.stack([u[2] for u in units])
+    scale = 1.0 / math.sqrt(128)
+
+    def one_step():
+        t0 = time.time()
+        sel, cnt, _, _ = orc.decode_units(blobs, q, w.token_budget, scale, 0, k_max=w.token_budget // 8 + 1)
+        t_decode = time.time() - t0
+        t0 = time.time()
+        orc.attention_units(blobs, q, sel, cnt, scale)
+        return t_decode, time.time() - t0
+
+    return one_step, prep_s, orc.num_threads()
+
+
+def sample_units(w, dev, n_units, Bt, N):
+    """raw K/V/q of n_units units of layer 0, from the same seeded generator the GPU path consumes"""
+    import numpy as np
+    import torch
+    from paper_2607_00760_b200 import synth
+    G, Hkv = w.group, w.n_kv_heads
+    units = []
+    if torch.cuda.is_available():
+        K, V, q = synth.make_layer_torch(w, 0, dev, batch=Bt, context=N)
+        u16 = lambda t: t.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+        for i in range(n_units):
+            u = (i * (Bt * Hkv - 1)) // max(1, n_units - 1) if n_units > 1 else 0  # spread, first and last included
+            b, h = divmod(u, Hkv)
+            units.append((u16(K[b, h]), u16(V[b, h]), u16(q[b, h * G:(h + 1) * G])))
+        del K, V
+        src = "torch CUDA generator (the bytes the GPU path consumed)"
+    else:
+        nb = -(-n_units // Hkv)
+        K, V, q = synth.make_inputs_np(nb, Hkv, w.n_q_heads, N, 128, w.segment_len, seed=1000 * w.config_id)
+        for u in range(n_units):
+            b, h = divmod(u, Hkv)
+            units.append((K[b, h], V[b, h], q[b, h * G:(h + 1) * G]))
+        src = "numpy generator (no GPU present)"
+    return units, src
+
+
+def cpu_baseline(args, w, built, dev, n_units, repeats):
+    Bt = built.batch if built is not None else (args.batch or w.batch)
+    N = built.context if built is not None else (args.context or w.context)
+    n_units = min(n_units, Bt * w.n_kv_heads)
+    units, src = sample_units(w, dev, n_units, Bt, N)
+    one_step, prep_s, threads = oracle_sample(w, units, N)
+    t = [one_step() for _ in range(repeats)]
+    t_dec, t_att = min(x[0] for x in t), min(x[1] for x in t)
+    scale_up = Bt * w.n_kv_heads / n_units
+    return {"value": round(t_att * scale_up * 1e6, 1), "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"{n_units} of {Bt * w.n_kv_heads} units of layer 0 ({src}); oracle attention (O8) on the oracle's own "
+                      f"selection, OpenMP over units, time scaled by {scale_up:g} to one layer; prep (loss, strategy, "
+                      f"compress) {prep_s:.1f} s untimed",
+            "select_plus_attention_us_per_layer": round(t_dec * scale_up * 1e6, 1)}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample of the same workload."""
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    if rank != 0:
+        return
+    import torch
+    from oracle import build as orc_build
+    orc_build.build()
+    from paper_2607_00760_b200 import synth
+    w = synth.WORKLOADS[args.workload]
+    n_layers = args.layers or w.n_layers
+    Bt, N = args.batch or w.batch, args.context or w.context
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", 0))) if torch.cuda.is_available() else None
+    n_units = min(args.cpu_units, Bt * w.n_kv_heads)
+    units, src = sample_units(w, dev, n_units, Bt, N)
+    one_step, prep_s, threads = oracle_sample(w, units, N)
+    for _ in range(min(args.warmup, 3)):
+        one_step()
+    steps = max(1, min(args.steps, 20))
+    t0 = time.time()
+    ts = [one_step() for _ in range(steps)]
+    wall = time.time() - t0
+    scale_up = Bt * w.n_kv_heads / n_units
+    t_att = sum(x[1] for x in ts) / steps
+    t_dec = sum(x[0] for x in ts) / steps
+    value = t_att * scale_up * 1e6
+    sample = (f"{n_units} of {Bt * w.n_kv_heads} units of one layer ({src}); each step = oracle select + attention then "
+              f"attention alone on the sample; us/layer = attention time x {scale_up:g}; prep {prep_s:.1f} s untimed")
+    line = {"impl": "reference", "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world,
+            "steps": steps, "warmup": min(args.warmup, 3), "ms_per_step": round(wall / steps * 1e3, 3),
+            "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "baseline_config": w.config_id, "n_layers": n_layers, "batch_per_gpu": Bt,
+                       "context": N, "token_budget": w.token_budget, "r_keep": w.r_keep},
+            "cpu_baseline": {"value": round(value, 1), "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+                             "select_plus_attention_us_per_layer": round(t_dec * scale_up * 1e6, 1)},
+            "e2e": {"value": round(value, 1), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_mkv(a)

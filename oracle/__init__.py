@@ -55,6 +55,8 @@ def _declare(L):
                                      C.POINTER(u8p), C.POINTER(C.c_uint64)]
     L.orc_decode_units.argtypes = [C.POINTER(u8p), C.c_int, u16p, C.c_int, C.c_int, C.c_int,
                                    C.c_double, i32p, i32p, C.c_int, f64p, f64p]
+    L.orc_attention_units.argtypes = [C.POINTER(u8p), C.c_int, u16p, C.c_int, i32p, i32p, C.c_int,
+                                      C.c_double, f64p, f64p]
     L.orc_num_threads.restype = C.c_int
 
 
@@ -278,3 +280,19 @@ def decode_units(blobs, q, budget: int, scale: float, mode: int = 0, k_max: int 
     if rc:
         raise ValueError(f"orc_decode_units rc={rc}")
     return sel, cnt, out, lse
+
+
+def attention_units(blobs, q, sel, sel_count, scale: float):
+    """O8 for every unit with a given selection (OpenMP over units).
+    q: [U][G][D] bf16 bits; sel: [U][k_max] int32; sel_count: [U]. Returns out [U][G][D], lse [U][G]."""
+    q = _u16(q)
+    U, G, D = q.shape
+    sel = np.ascontiguousarray(sel, np.int32)
+    cnt = np.ascontiguousarray(sel_count, np.int32)
+    ptrs = (C.POINTER(C.c_uint8) * U)(*[_p(b, C.c_uint8) for b in blobs])
+    out, lse = np.zeros((U, G, D)), np.zeros((U, G))
+    rc = lib().orc_attention_units(ptrs, U, _p(q, C.c_uint16), G, _p(sel, C.c_int32), _p(cnt, C.c_int32),
+                                   sel.shape[1], float(scale), _p(out, C.c_double), _p(lse, C.c_double))
+    if rc:
+        raise ValueError(f"orc_attention_units rc={rc}")
+    return out, lse

@@ -683,3 +683,26 @@ int orc_decode_units(uint8_t* const* blobs, int n_units, const uint16_t* q, int 
     }
     return err;
 }
+
+/* attention only (O8) for every unit with a given selection, OpenMP over units */
+int orc_attention_units(uint8_t* const* blobs, int n_units, const uint16_t* q, int G,
+                        const int32_t* sel, const int32_t* sel_count, int k_max, double scale,
+                        double* out, double* lse) {
+    int err = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int u = 0; u < n_units; ++u) {
+        blob_view bv;
+        if (view_blob(blobs[u], &bv)) {
+#pragma omp atomic write
+            err = -1;
+            continue;
+        }
+        int rc = orc_attention(blobs[u], q + (size_t)u * G * bv.D, G, sel + (size_t)u * k_max,
+                               sel_count[u], scale, out + (size_t)u * G * bv.D, lse + (size_t)u * G);
+        if (rc < 0) {
+#pragma omp atomic write
+            err = rc;
+        }
+    }
+    return err;
+}

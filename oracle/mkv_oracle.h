@@ -95,6 +95,9 @@ int orc_decode_units(uint8_t* const* blobs, int n_units, const uint16_t* q /*[n_
                      int G, int mode, int budget, double scale, int32_t* sel /*[n_units][k_max]*/,
                      int32_t* sel_count, int k_max, double* out /*[n_units][G][D]*/,
                      double* lse /*[n_units][G]*/);
+int orc_attention_units(uint8_t* const* blobs, int n_units, const uint16_t* q, int G,
+                        const int32_t* sel, const int32_t* sel_count, int k_max, double scale,
+                        double* out, double* lse);
 int orc_num_threads(void);
 
 #ifdef __cplusplus

@@ -1,0 +1,173 @@
+"""Helpers of the GPU parity tests: move seeded inputs to the device, run the C-ABI path, and
+compare with the oracle by the protocol of DESIGN.md ("GPU <-> oracle comparison protocol")."""
+import math
+
+import numpy as np
+
+import oracle as orc
+from paper_2607_00760_b200 import synth
+
+ATOL_ATTN = 3e-3     # north_star: max-abs 3e-3 ...
+RTOL_L2_ATTN = 1e-3  # ... and relative-L2 1e-3 against the fp64 oracle (bf16 inputs, fp32 accumulation)
+TIE_REL = 1e-5       # north_star: selection may differ only at fp32 score near-ties |d| <= 1e-5 relative
+
+
+def to_dev(a_u16, dev):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a_u16).view(np.int16)).view(torch.bfloat16).to(dev)
+
+
+def uniform_strat(Bt, Hkv, S, r_k, r_v=None, g=1, B=8):
+    st = np.zeros((Bt, Hkv, S, 4), np.uint8)
+    st[:] = (r_k, r_k if r_v is None else r_v, g, B)
+    return st
+
+
+class Case:
+    """One synthetic problem on the device + its oracle blobs."""
+
+    def __init__(self, mkv, dev, Bt, Hkv, Hq, N, L=64, seed=0, n_layers=1):
+        import torch
+        self.mkv, self.dev = mkv, dev
+        self.Bt, self.Hkv, self.Hq, self.N, self.L, self.D = Bt, Hkv, Hq, N, L, 128
+        self.G, self.S = Hq // Hkv, (N + L - 1) // L
+        self.K, self.V, self.q = synth.make_inputs_np(Bt, Hkv, Hq, N, 128, L, seed=seed)
+        self.k_d, self.v_d, self.q_d = to_dev(self.K, dev), to_dev(self.V, dev), to_dev(self.q, dev)
+        self.cache = mkv.Cache(n_layers, Bt, Hkv, Hq, 128, N, L)
+        self.torch = torch
+        self.blobs = None
+
+    def free(self):
+        self.cache.free()
+
+    # ---- step 1
+    def gpu_loss(self, r_k, r_v):
+        torch = self.torch
+        lk = torch.zeros((self.Bt, self.Hkv, self.S), dtype=torch.float64, device=self.dev)
+        lv = torch.zeros_like(lk)
+        self.cache.segment_loss(self.k_d, self.v_d, (r_k, r_v, 1, 8), lk, lv)
+        torch.cuda.synchronize()
+        return lk.cpu().numpy(), lv.cpu().numpy()
+
+    def compress(self, strat, layer=0):
+        """strat: uint8 [Bt][Hkv][S][4]; compresses on the GPU and builds the oracle blobs."""
+        self.strat = strat
+        self.cache.compress_segment(layer, self.k_d, self.v_d, self.torch.from_numpy(strat).to(self.dev))
+        self.torch.cuda.synchronize()
+        self.cache.status()
+        self.blobs = [[orc.compress_unit(self.K[b, h], self.V[b, h], self.L, strat[b, h])
+                       for h in range(self.Hkv)] for b in range(self.Bt)]
+
+    def assert_export_equal(self, layer=0):
+        for b in range(self.Bt):
+            for h in range(self.Hkv):
+                got = self.cache.export(layer, b, h)
+                ref = self.blobs[b][h]
+                assert got.shape == ref.shape, (b, h, got.shape, ref.shape)
+                if not np.array_equal(got, ref):
+                    i = int(np.nonzero(got != ref)[0][0])
+                    raise AssertionError(f"unit ({b},{h}): first differing byte at {i} of {len(ref)}")
+
+    # ---- step 2
+    def gpu_select(self, budget, reduce=0, layer=0, want_scores=False):
+        torch = self.torch
+        nblk = (self.N + 7) // 8
+        k_max = min(budget // 8 + 1, nblk)
+        k_max = max(k_max, 1)
+        sel = torch.full((self.Bt, self.Hkv, k_max), -7, dtype=torch.int32, device=self.dev)
+        cnt = torch.full((self.Bt, self.Hkv), -7, dtype=torch.int32, device=self.dev)
+        scores = None
+        if want_scores:
+            scores = torch.zeros((self.Bt, self.Hkv, self.cache.score_stride), dtype=torch.float32, device=self.dev)
+        self.cache.select(layer, self.q_d, budget, sel, cnt, reduce=reduce, scores=scores)
+        torch.cuda.synchronize()
+        return sel.cpu().numpy(), cnt.cpu().numpy(), (scores.cpu().numpy() if want_scores else None)
+
+    def check_select(self, budget, reduce=0, layer=0):
+        """returns (n_selected_total, n_swaps): bit-exact except counted swaps inside the tie band."""
+        sel, cnt, sc = self.gpu_select(budget, reduce, layer, want_scores=True)
+        total = swaps = 0
+        for b in range(self.Bt):
+            for h in range(self.Hkv):
+                blob = self.blobs[b][h]
+                qh = self.q[b, h * self.G:(h + 1) * self.G]
+                ft, nt = orc.blob_blocks(blob)
+                s = orc.scores(blob, qh, reduce)
+                ref = orc.topk(s, ft, nt, budget)
+                n = int(cnt[b, h])
+                got = sel[b, h, :n]
+                assert np.all(sel[b, h, n:] == -1), "unused tail of sel must be -1"
+                # fp32 scores agree with the fp64 oracle to fp32 accumulation error
+                tol = 1e-5 * max(1.0, np.abs(s).max())
+                assert np.abs(sc[b, h, :len(s)] - s).max() <= 16 * tol, np.abs(sc[b, h, :len(s)] - s).max()
+                total += len(ref)
+                assert n == len(ref), (b, h, n, len(ref))
+                assert np.all(np.diff(got) > 0), "sel must be strictly ascending"
+                if np.array_equal(got, ref):
+                    continue
+                diff = np.setxor1d(got, ref)
+                idx = np.searchsorted(ft, diff)
+                kth = np.sort(s)[::-1][len(ref) - 1]
+                band = TIE_REL * max(abs(kth), 1e-3 * np.abs(s).max())
+                assert np.all(np.abs(s[idx] - kth) <= band), ("selection differs outside the tie band", b, h, diff)
+                swaps += len(diff) // 2
+        return total, swaps
+
+    # ---- step 3
+    def oracle_sel(self, budget, reduce=0):
+        nblk = (self.N + 7) // 8
+        k_max = max(1, min(budget // 8 + 1, nblk))
+        sel = np.full((self.Bt, self.Hkv, k_max), -1, np.int32)
+        cnt = np.zeros((self.Bt, self.Hkv), np.int32)
+        for b in range(self.Bt):
+            for h in range(self.Hkv):
+                blob = self.blobs[b][h]
+                ft, nt = orc.blob_blocks(blob)
+                s = orc.scores(blob, self.q[b, h * self.G:(h + 1) * self.G], reduce)
+                r = orc.topk(s, ft, nt, budget)
+                sel[b, h, :len(r)] = r
+                cnt[b, h] = len(r)
+        return sel, cnt
+
+    def gpu_attention(self, sel, cnt, scale=None, layer=0):
+        torch = self.torch
+        scale = scale if scale is not None else 1.0 / math.sqrt(self.D)
+        sel_d = torch.from_numpy(np.ascontiguousarray(sel)).to(self.dev)
+        cnt_d = torch.from_numpy(np.ascontiguousarray(cnt)).to(self.dev)
+        out = torch.full((self.Bt, self.Hq, self.D), float("nan"), dtype=torch.float32, device=self.dev)
+        lse = torch.full((self.Bt, self.Hq), float("nan"), dtype=torch.float32, device=self.dev)
+        self.cache.packed_attention(layer, self.q_d, sel_d, cnt_d, scale, out, lse)
+        torch.cuda.synchronize()
+        return out.cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64)
+
+    def check_attention(self, sel, cnt, scale=None, layer=0):
+        scale = scale if scale is not None else 1.0 / math.sqrt(self.D)
+        out, lse = self.gpu_attention(sel, cnt, scale, layer)
+        ref = np.zeros_like(out)
+        ref_lse = np.zeros_like(lse)
+        for b in range(self.Bt):
+            for h in range(self.Hkv):
+                o, l = orc.attention(self.blobs[b][h], self.q[b, h * self.G:(h + 1) * self.G],
+                                     sel[b, h, :cnt[b, h]], scale)
+                ref[b, h * self.G:(h + 1) * self.G] = o
+                ref_lse[b, h * self.G:(h + 1) * self.G] = l
+        assert_attention_close(out, lse, ref, ref_lse)
+        return out, ref
+
+
+def assert_attention_close(out, lse, ref, ref_lse):
+    assert np.all(np.isfinite(out))
+    err = np.abs(out - ref).max()
+    assert err <= ATOL_ATTN, f"max-abs {err:.3e} > {ATOL_ATTN}"
+    num = np.linalg.norm((out - ref).reshape(-1, out.shape[-1]), axis=1)
+    den = np.linalg.norm(ref.reshape(-1, out.shape[-1]), axis=1)
+    nz = den > 0
+    if nz.any():
+        rel_rows = (num[nz] / den[nz]).max()
+        assert rel_rows <= RTOL_L2_ATTN, f"per-row relative-L2 {rel_rows:.3e} > {RTOL_L2_ATTN}"
+        rel = np.linalg.norm(out - ref) / np.linalg.norm(ref)
+        assert rel <= RTOL_L2_ATTN, f"relative-L2 {rel:.3e} > {RTOL_L2_ATTN}"
+    fin = np.isfinite(ref_lse)
+    assert np.array_equal(np.isneginf(lse), np.isneginf(ref_lse))
+    if fin.any():
+        assert np.abs(lse[fin] - ref_lse[fin]).max() <= 1e-3

@@ -1,0 +1,376 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Bars (north_star / DESIGN.md): packed layouts, masks and strategy tables
+bit-exact; selection bit-exact except counted swaps at fp32 near-ties (< 0.01 %); attention
+max-abs <= 3e-3 and relative-L2 <= 1e-3 against the fp64 oracle."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle as orc
+from gpu_util import Case, uniform_strat, assert_attention_close, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    import __graft_entry__
+    __graft_entry__.build()
+    from paper_2607_00760_b200 import binding as mkv
+    assert torch.cuda.is_available()
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(dev)
+    return mkv, dev
+
+
+# ------------------------------------------------------------------ config 1 (BASELINE "tiny")
+
+def test_tiny_config_end_to_end(env):
+    """BASELINE config 1: 1 request, 8 q / 2 kv heads, N = 4096, L = 64, r = 38 everywhere,
+    budget 1024, seed 0.  Spans 64 segments, 512 blocks, several CTAs and splits."""
+    mkv, dev = env
+    c = Case(mkv, dev, 1, 2, 8, 4096, seed=0)
+    try:
+        c.compress(uniform_strat(1, 2, c.S, 38))
+        c.assert_export_equal()
+        total, swaps = c.check_select(1024)
+        assert total == 2 * 128 and swaps == 0
+        sel, cnt = c.oracle_sel(1024)
+        c.check_attention(sel, cnt)
+        # end to end on the GPU's own selection
+        gsel, gcnt, _ = c.gpu_select(1024)
+        c.check_attention(gsel, gcnt)
+    finally:
+        c.free()
+
+
+# ------------------------------------------------------------------ step 1
+
+@pytest.mark.parametrize("r_k,r_v", [(38, 38), (128, 128), (1, 127), (90, 64), (128, 38), (38, 128), (64, 1)])
+def test_compress_bit_exact_uniform(env, r_k, r_v):
+    mkv, dev = env
+    c = Case(mkv, dev, 2, 2, 4, 1003, seed=r_k * 7 + r_v)  # ragged: last segment 43 tokens, last block 3
+    try:
+        c.compress(uniform_strat(2, 2, c.S, r_k, r_v))
+        c.assert_export_equal()
+        by = c.cache.bytes(0)
+        ref_tok = sum(orc.blob_header(b)["tok_bytes"] for row in c.blobs for b in row)
+        ref_bk = sum(orc.blob_header(b)["bk_bytes"] for row in c.blobs for b in row)
+        assert by["packed"] == ref_tok and by["block_keys"] == ref_bk
+    finally:
+        c.free()
+
+
+def test_compress_ties_and_zeros_bit_exact(env):
+    """coarse values, +-0 and all-equal vectors: ties must go to the lower channel."""
+    mkv, dev = env
+    c = Case(mkv, dev, 1, 2, 2, 256, seed=3)
+    try:
+        rng = np.random.default_rng(4)
+        from paper_2607_00760_b200 import synth
+        coarse = rng.integers(-2, 3, c.K.shape).astype(np.float32)
+        c.K = synth.f32_to_bf16_bits(coarse)
+        c.K[0, 0, 5] = 0x8000  # a whole vector of -0.0
+        c.K[0, 1, 9] = 0x3F80  # all ones
+        c.V = synth.f32_to_bf16_bits(rng.integers(-1, 2, c.V.shape).astype(np.float32))
+        c.k_d, c.v_d = to_dev(c.K, dev), to_dev(c.V, dev)
+        c.compress(uniform_strat(1, 2, c.S, 38, 17))
+        c.assert_export_equal()
+    finally:
+        c.free()
+
+
+def test_loss_and_quantile_strategy_match_oracle(env):
+    mkv, dev = env
+    import torch
+    c = Case(mkv, dev, 2, 2, 8, 64 * 37 + 20, seed=11)
+    try:
+        lk, lv = c.gpu_loss(38, 38)
+        ref_k = np.zeros_like(lk)
+        ref_v = np.zeros_like(lv)
+        for b in range(2):
+            for h in range(2):
+                ref_k[b, h], ref_v[b, h] = orc.segment_loss(c.K[b, h], c.V[b, h], 64, 38, 38)
+        # fp64 sums of exact fp32 squares; only the summation order differs
+        np.testing.assert_allclose(lk, ref_k, rtol=1e-12, atol=0)
+        np.testing.assert_allclose(lv, ref_v, rtol=1e-12, atol=0)
+        l0k, l0v = c.gpu_loss(128, 128)
+        assert np.all(l0k == 0) and np.all(l0v == 0)
+        # quantile rule on the device from the device's own losses == oracle rule on the oracle's losses
+        strat_d = torch.zeros((2, 2, c.S, 4), dtype=torch.uint8, device=dev)
+        c.cache.strategy_quantile(to_t(lk, dev), to_t(lv, dev), c.S, 1, 10, (38, 38, 1, 8), strat_d)
+        torch.cuda.synchronize()
+        got = strat_d.cpu().numpy()
+        n_boundary = 0
+        for b in range(2):
+            for h in range(2):
+                ref = orc.strategy_quantile(ref_k[b, h], ref_v[b, h], 1, 10, 128, 38, 38)
+                if not np.array_equal(got[b, h], ref):
+                    n_boundary += 1
+                assert (got[b, h, :, 0] == 128).sum() == math.ceil(c.S / 10)
+        assert n_boundary == 0
+        # the device strategy table drives the compressor; layout still bit-exact
+        c.compress(got)
+        c.assert_export_equal()
+        total, swaps = c.check_select(512)
+        assert swaps <= max(1, total // 10000)
+        sel, cnt = c.oracle_sel(512)
+        c.check_attention(sel, cnt)
+    finally:
+        c.free()
+
+
+def to_t(a, dev):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+
+
+def test_quantile_ties_and_threshold_rule(env):
+    mkv, dev = env
+    import torch
+    c = Case(mkv, dev, 1, 1, 1, 64, seed=1)
+    try:
+        S = 20
+        ones = torch.ones((1, S), dtype=torch.float64, device=dev)
+        out = torch.zeros((1, S, 4), dtype=torch.uint8, device=dev)
+        c.cache.strategy_quantile(ones, ones, S, 1, 10, (38, 38, 1, 8), out, n_units=1)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(np.nonzero(out.cpu().numpy()[0, :, 0] == 128)[0], [0, 1])
+        rng = np.random.default_rng(2)
+        ncand, n = 3, 50
+        lk, lv = rng.random((ncand, n)), rng.random((ncand, n))
+        cands = [(16, 16, 1, 8), (32, 32, 1, 8), (48, 48, 1, 8)]
+        out = torch.zeros((n, 4), dtype=torch.uint8, device=dev)
+        for tau in (float("inf"), -1.0, 0.4):
+            c.cache.strategy_threshold(to_t(lk, dev), to_t(lv, dev), n, cands, tau, out, n_units=1)
+            torch.cuda.synchronize()
+            ref = orc.strategy_threshold(lk, lv, np.array(cands, np.uint8), tau, 128)
+            np.testing.assert_array_equal(out.cpu().numpy(), ref)
+    finally:
+        c.free()
+
+
+def test_compress_in_several_calls_appends(env):
+    """segments arrive in three calls (the literal 'compress one segment' included)."""
+    mkv, dev = env
+    import torch
+    c = Case(mkv, dev, 2, 2, 4, 64 * 9 + 13, seed=21)
+    try:
+        strat = uniform_strat(2, 2, c.S, 38)
+        strat[:, :, 1::3, 0:2] = 128
+        strat[0, 1, 4] = (90, 38, 1, 8)
+        sd = torch.from_numpy(strat).to(dev)
+        cuts = [(0, 1), (1, 6), (6, c.S)]
+        for s0, s1 in cuts:
+            t0, t1 = s0 * 64, min(c.N, s1 * 64)
+            c.cache.compress_segment(0, c.k_d[:, :, t0:t1], c.v_d[:, :, t0:t1],
+                                     sd[:, :, s0:s1].contiguous(), seg0=s0)
+        torch.cuda.synchronize()
+        c.cache.status()
+        c.strat = strat
+        c.blobs = [[orc.compress_unit(c.K[b, h], c.V[b, h], 64, strat[b, h]) for h in range(2)] for b in range(2)]
+        c.assert_export_equal()
+        total, swaps = c.check_select(200)
+        assert swaps == 0
+        sel, cnt = c.oracle_sel(200)
+        c.check_attention(sel, cnt)
+        # append-order violations are host-visible
+        with pytest.raises(mkv.MkvError) as e:
+            c.cache.compress_segment(0, c.k_d[:, :, :64], c.v_d[:, :, :64], sd[:, :, :1].contiguous(), seg0=0)
+        assert e.value.code == mkv.MKV_E_STATE
+        # reset lets the layer be compressed again from scratch
+        c.cache.reset(0)
+        c.cache.compress_segment(0, c.k_d, c.v_d, sd)
+        torch.cuda.synchronize()
+        c.assert_export_equal()
+    finally:
+        c.free()
+
+
+# ------------------------------------------------------------------ step 2
+
+@pytest.mark.parametrize("Hq,Hkv", [(8, 2), (7, 1), (2, 2), (8, 1)])
+@pytest.mark.parametrize("reduce", [0, 1])
+def test_select_matches_oracle(env, Hq, Hkv, reduce):
+    mkv, dev = env
+    c = Case(mkv, dev, 2, Hkv, Hq, 64 * 40 + 29, seed=31 + Hq)
+    try:
+        strat = uniform_strat(2, Hkv, c.S, 38)
+        strat[:, :, ::7, 0:2] = 128
+        c.compress(strat)
+        tot = sw = 0
+        for budget in (0, 5, 7, 8, 9, 64, 1000, 1001, 1005, c.N - 1, c.N, c.N + 100):
+            t, s = c.check_select(budget, reduce)
+            tot += t
+            sw += s
+        assert sw <= max(1, tot // 10000)
+    finally:
+        c.free()
+
+
+def test_select_with_massive_ties(env):
+    """all block keys identical -> every score ties; lower block index must win, bit-exact."""
+    mkv, dev = env
+    c = Case(mkv, dev, 1, 2, 8, 64 * 20, seed=5)
+    try:
+        c.K[:] = c.K[:, :, :1, :]
+        c.k_d = to_dev(c.K, dev)
+        c.compress(uniform_strat(1, 2, c.S, 38))
+        for budget in (8, 24, 100, 640):
+            sel, cnt, _ = c.gpu_select(budget)
+            k = budget // 8
+            for h in range(2):
+                assert cnt[0, h] == k
+                np.testing.assert_array_equal(sel[0, h, :k], np.arange(k) * 8)
+            t, s = c.check_select(budget)
+            assert s == 0
+    finally:
+        c.free()
+
+
+# ------------------------------------------------------------------ step 3
+
+@pytest.mark.parametrize("Hq,Hkv,r", [(8, 2, 38), (28, 4, 38), (4, 4, 90), (8, 1, 128), (8, 2, 1)])
+def test_attention_matches_oracle(env, Hq, Hkv, r):
+    mkv, dev = env
+    c = Case(mkv, dev, 2, Hkv, Hq, 64 * 30 + 21, seed=41 + r)
+    try:
+        strat = uniform_strat(2, Hkv, c.S, r)
+        strat[:, :, 2::5, 0:2] = 128
+        strat[:, :, 3::5] = (64, 90, 1, 8)
+        c.compress(strat)
+        c.assert_export_equal()
+        for budget in (0, 8, 100, 512, c.N + 5):
+            sel, cnt = c.oracle_sel(budget)
+            c.check_attention(sel, cnt)
+        # any order of the selected blocks is accepted
+        sel, cnt = c.oracle_sel(512)
+        rng = np.random.default_rng(0)
+        for b in range(2):
+            for h in range(Hkv):
+                sel[b, h, :cnt[b, h]] = rng.permutation(sel[b, h, :cnt[b, h]])
+        c.check_attention(sel, cnt, scale=0.05)
+    finally:
+        c.free()
+
+
+def test_attention_dense_equals_plain_softmax_attention(env):
+    """r = D and budget >= N: the path is ordinary softmax attention."""
+    mkv, dev = env
+    import brute
+    c = Case(mkv, dev, 1, 2, 8, 777, seed=51)
+    try:
+        c.compress(uniform_strat(1, 2, c.S, 128))
+        sel, cnt, _ = c.gpu_select(10 ** 6)
+        assert np.all(cnt == (777 + 7) // 8)
+        out, lse = c.gpu_attention(sel, cnt)
+        ref = np.zeros_like(out)
+        ref_lse = np.zeros_like(lse)
+        for h in range(8):
+            o, l = brute.dense_attention(brute.bf16_to_f64(c.q[0, h:h + 1]), brute.bf16_to_f64(c.K[0, h // 4]),
+                                         brute.bf16_to_f64(c.V[0, h // 4]), 1 / math.sqrt(128))
+            ref[0, h], ref_lse[0, h] = o[0], l[0]
+        assert_attention_close(out, lse, ref, ref_lse)
+    finally:
+        c.free()
+
+
+def test_attention_peaked_softmax(env):
+    """one token carries almost all the mass (needle + heavy hitter): P must not lose precision."""
+    mkv, dev = env
+    from paper_2607_00760_b200 import synth
+    c = Case(mkv, dev, 1, 1, 4, 64 * 16, seed=61)
+    try:
+        kf = synth.bf16_bits_to_f32(c.K[0, 0, 100])
+        c.q[0, :] = synth.f32_to_bf16_bits(kf * 3.0)
+        c.q_d = to_dev(c.q, dev)
+        c.compress(uniform_strat(1, 1, c.S, 38))
+        sel, cnt = c.oracle_sel(256)
+        assert 96 in sel[0, 0]
+        c.check_attention(sel, cnt)
+    finally:
+        c.free()
+
+
+# ------------------------------------------------------------------ multi-layer, host call, errors
+
+def test_layers_are_independent_and_decode_host_matches(env):
+    mkv, dev = env
+    import torch
+    a = Case(mkv, dev, 2, 2, 8, 64 * 12, seed=71, n_layers=3)
+    b = Case(mkv, dev, 2, 2, 8, 64 * 12, seed=72)
+    try:
+        sa, sb = uniform_strat(2, 2, a.S, 38), uniform_strat(2, 2, a.S, 64)
+        sb[:, :, ::3, :2] = 128
+        a.compress(sa, layer=0)
+        blobs0 = a.blobs
+        # layer 2 holds different data (b's K/V) in the same cache
+        a.cache.compress_segment(2, b.k_d, b.v_d, torch.from_numpy(sb).to(dev))
+        torch.cuda.synchronize()
+        a.assert_export_equal(layer=0)
+        blobs2 = [[orc.compress_unit(b.K[i, h], b.V[i, h], 64, sb[i, h]) for h in range(2)] for i in range(2)]
+        for i in range(2):
+            for h in range(2):
+                np.testing.assert_array_equal(a.cache.export(2, i, h), blobs2[i][h])
+        assert a.cache.export(1, 0, 0).shape[0] == 48  # empty layer: header only
+        # the end-to-end host call: pinned q in, out back
+        q_host = torch.from_numpy(a.q.view(np.int16)).view(torch.bfloat16).pin_memory()
+        out_host = torch.zeros((2, 8, 128), dtype=torch.float32).pin_memory()
+        k_max = 256 // 8 + 1
+        sel_host = torch.zeros((2, 2, k_max), dtype=torch.int32).pin_memory()
+        cnt_host = torch.zeros((2, 2), dtype=torch.int32).pin_memory()
+        a.cache.decode_host(0, q_host, 256, 1 / math.sqrt(128), out_host, sel_host=sel_host, sel_count_host=cnt_host)
+        torch.cuda.synchronize()
+        a.blobs = blobs0
+        sel, cnt = sel_host.numpy(), cnt_host.numpy()
+        ref = np.zeros((2, 8, 128))
+        for i in range(2):
+            for h in range(2):
+                ref[i, 4 * h:4 * h + 4], _ = orc.attention(blobs0[i][h], a.q[i, 4 * h:4 * h + 4],
+                                                            sel[i, h, :cnt[i, h]], 1 / math.sqrt(128))
+        o = out_host.numpy().astype(np.float64)
+        assert np.abs(o - ref).max() <= 3e-3 and np.linalg.norm(o - ref) / np.linalg.norm(ref) <= 1e-3
+        t, s = a.check_select(256)
+        assert s == 0
+    finally:
+        a.free()
+        b.free()
+
+
+def test_errors_are_reported_not_thrown(env):
+    mkv, dev = env
+    import torch
+    with pytest.raises(mkv.MkvError) as e:
+        mkv.Cache(1, 1, 2, 8, 64, 1024, 64)
+    assert e.value.code == mkv.MKV_E_UNSUPPORTED
+    with pytest.raises(mkv.MkvError) as e:
+        mkv.Cache(1, 1, 3, 8, 128, 1024, 64)
+    assert e.value.code == mkv.MKV_E_ARG
+    c = Case(mkv, dev, 1, 2, 8, 256, seed=81)
+    try:
+        lk = torch.zeros((1, 2, 4), dtype=torch.float64, device=dev)
+        with pytest.raises(mkv.MkvError) as e:
+            c.cache.segment_loss(c.k_d, c.v_d, (32, 32, 2, 8), lk, lk.clone())
+        assert e.value.code == mkv.MKV_E_UNSUPPORTED
+        # an invalid strategy record in device memory sets the sticky device flag; nothing is written
+        bad = uniform_strat(1, 2, 4, 38)
+        bad[0, 1, 2] = (38, 38, 4, 8)
+        c.cache.compress_segment(0, c.k_d, c.v_d, torch.from_numpy(bad).to(dev))
+        torch.cuda.synchronize()
+        assert c.cache.status(raise_on_flag=False) & mkv.MKV_DEV_BAD_STRATEGY
+        with pytest.raises(mkv.MkvError):
+            c.cache.status()
+    finally:
+        c.free()
+    # arena too small -> overflow flag, no out-of-bounds write
+    small = mkv.Cache(1, 1, 2, 8, 128, 256, 64, arena_bytes=4096)
+    try:
+        c2 = Case(mkv, dev, 1, 2, 8, 256, seed=82)
+        small.compress_segment(0, c2.k_d, c2.v_d, torch.from_numpy(uniform_strat(1, 2, 4, 38)).to(dev))
+        torch.cuda.synchronize()
+        assert small.status(raise_on_flag=False) & mkv.MKV_DEV_ARENA_OVERFLOW
+        c2.free()
+    finally:
+        small.free()
