@@ -24,8 +24,15 @@ __device__ __forceinline__ void load_vector(const uint8_t* bm, const uint8_t* va
         for (int j = 0; j < 4; ++j) x[j] = bf16_bits_to_f32(v16[lane + 32 * j]);
         return;
     }
-    const uint4 w4 = *reinterpret_cast<const uint4*>(bm);
-    const uint32_t w[4] = {w4.x, w4.y, w4.z, w4.w};
+    uint32_t w[4];
+    if ((reinterpret_cast<uintptr_t>(bm) & 15u) == 0) {
+        const uint4 w4 = *reinterpret_cast<const uint4*>(bm);
+        w[0] = w4.x; w[1] = w4.y; w[2] = w4.z; w[3] = w4.w;
+    } else {  // ragged token block: bitmaps are only 2-byte aligned
+        const uint16_t* b16 = reinterpret_cast<const uint16_t*>(bm);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) w[j] = (uint32_t)b16[2 * j] | ((uint32_t)b16[2 * j + 1] << 16);
+    }
     const unsigned lt = lanemask_lt();
     int base = 0;
 #pragma unroll

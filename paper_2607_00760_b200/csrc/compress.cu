@@ -69,9 +69,10 @@ __device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, uint8
         if ((w[j] >> lane) & 1u) v16[base + __popc(w[j] & lt)] = (uint16_t)x[j];
         base += __popc(w[j]);
     }
-    if (lane < 4) {
-        const uint32_t wl = lane == 0 ? w[0] : lane == 1 ? w[1] : lane == 2 ? w[2] : w[3];
-        reinterpret_cast<uint32_t*>(bm)[lane] = wl;
+    if (lane < 8) {  // 2-byte stores: a ragged token block leaves the V bitmaps only 2-byte aligned
+        const int j = lane >> 1;
+        const uint32_t wl = j == 0 ? w[0] : j == 1 ? w[1] : j == 2 ? w[2] : w[3];
+        reinterpret_cast<uint16_t*>(bm)[lane] = (uint16_t)(wl >> (16 * (lane & 1)));
     }
 }
 
