@@ -107,6 +107,8 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     if (d->head_dim != kD) return fail(MKV_E_UNSUPPORTED, "head_dim %d: only 128 is built", d->head_dim);
     if (d->n_q_heads / d->n_kv_heads > kMaxGroup)
         return fail(MKV_E_UNSUPPORTED, "GQA group %d > %d", d->n_q_heads / d->n_kv_heads, kMaxGroup);
+    if ((long long)d->batch * d->n_kv_heads > 2048)
+        return fail(MKV_E_UNSUPPORTED, "batch * n_kv_heads = %lld units: at most 2048 are built", (long long)d->batch * d->n_kv_heads);
     if (d->segment_len < kB || d->segment_len % kB || d->segment_len > 4096)
         return fail(MKV_E_UNSUPPORTED, "segment_len %d: need a multiple of 8 in [8, 4096]", d->segment_len);
     int ndev = 0;
@@ -131,7 +133,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     c->slice_bytes = per_layer;
 
     const size_t tu = (size_t)g.n_layers * g.n_units;
-    c->attn.max_splits = 64;
+    c->attn.slots = attention_partial_slots(c->sm_count);
     c->sel_cap = g.score_stride + 1;
     struct { void** p; size_t bytes; } allocs[] = {
         {(void**)&c->arena, (size_t)per_layer * g.n_layers},
@@ -144,8 +146,8 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         {(void**)&c->dev_flags, 256},
         {(void**)&c->call_base, (size_t)g.n_units * 8},
         {(void**)&c->scores, (size_t)g.n_units * g.score_stride * 4},
-        {(void**)&c->attn.part_o, (size_t)g.n_units * c->attn.max_splits * g.group * kD * 4},
-        {(void**)&c->attn.part_ml, (size_t)g.n_units * c->attn.max_splits * g.group * 2 * 4},
+        {(void**)&c->attn.part_o, (size_t)c->attn.slots * g.group * kD * 4},
+        {(void**)&c->attn.part_ml, (size_t)c->attn.slots * kMaxGroup * 2 * 4},
         {(void**)&c->q_dev, (size_t)g.batch * g.n_q_heads * kD * 2},
         {(void**)&c->sel_dev, (size_t)g.n_units * c->sel_cap * 4},
         {(void**)&c->selcnt_dev, (size_t)g.n_units * 4},

@@ -82,10 +82,11 @@ cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_
                           cudaStream_t s, int* n_kernels);
 
 struct AttnScratch {
-    float* part_o;    // [n_units][max_splits][G][D]
-    float* part_ml;   // [n_units][max_splits][G][2]  (running max in log2 units, sum)
-    int32_t max_splits;
+    float* part_o;    // [slots][G][D]   unnormalised partial outputs (<= 2 slots per warp of the grid)
+    float* part_ml;   // [slots][8][2]   (running max in log2 units, sum)
+    int32_t slots;
 };
+int attention_partial_slots(int sm_count);
 cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q,
                              const int32_t* sel, const int32_t* sel_count, int k_max, float scale,
                              float* out, float* lse, const AttnScratch& scr, int sm_count,
