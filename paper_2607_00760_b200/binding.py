@@ -10,7 +10,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmkv.so")
+LIB_PATH = os.environ.get("MKV_LIB") or os.path.join(_HERE, "libmkv.so")  # MKV_LIB: tuning builds only
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} not found: run `python -m paper_2607_00760_b200.build` "

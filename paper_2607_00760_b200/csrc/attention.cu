@@ -14,6 +14,8 @@
 //     into the same tile and runs PV with P split into bf16 hi + lo (fp32-class accuracy).
 //   * A unit wholly inside one warp's range is normalised and written directly; otherwise the
 //     warp writes an (m, l, O) partial (<= 2 per warp) that the combine kernel merges (step 3d).
+#include <cstdlib>
+
 #include "mkv_internal.cuh"
 
 namespace mkv {
@@ -24,8 +26,7 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 
-constexpr int kWarps = 10;                    // warps per CTA (one CTA per SM)
-constexpr int kStages = 2;                    // groups in flight per warp
+constexpr int kMaxWarps = 16;                 // upper bound on warps per CTA (sizes the partial-slot scratch)
 constexpr int kStageBytes = 6144;             // >= 4 blocks at r = 38 (5888 B), >= 1 dense block (4096 B)
 constexpr int kTileStride = 272;              // bytes per token row: 256 + 16 pad (ldmatrix conflict-free)
 constexpr int kTileBytes = 32 * kTileStride;  // 8704
@@ -45,31 +46,14 @@ struct __align__(16) GInfo {  // one block of an in-flight group
 
 // ---- PTX wrappers ---------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+__device__ __forceinline__ void cp_async_16(uint32_t dst, unsigned long long src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-                 "l"(src), "r"(bytes), "r"(bar)
-                 : "memory");
-}
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void ldmatrix_x4(uint32_t addr, uint32_t (&r)[4]) {
     asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
@@ -121,44 +105,80 @@ __device__ __forceinline__ void sts_128(uint32_t addr, uint4 v) {
 
 // ---- lane = token: expand one packed (or dense) vector into this lane's dense tile row ------
 // row: shared address of the lane's 256-byte tile row; bm / val: shared addresses in the stage.
-// Kept values are consumed from the highest channel down (FLO gives the top set bit directly).
-__device__ __forceinline__ void expand_row(uint32_t row, uint32_t bm, uint32_t val, int r, bool valid) {
-    const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
-    if (!valid) {
+//
+// "Row assembly": the lane walks its 128 channel slots in order.  For slot c the bitmap bit (an
+// immediate mask, so the test is one LOP3 into a predicate) guards a 2-byte load of the next kept
+// value and the advance of the value pointer; a dropped slot keeps the zero its register was
+// initialised with.  Eight slots are packed into four registers and stored with one 16-byte store.
+// Why this shape: it is uniform across lanes (no divergence, no padding
+// to the longest lane), needs no zero-fill pass and no scattered 2-byte stores (bank conflicts),
+// no FLO/POPC (XU pipe), and only ~1.5 ALU-pipe instructions per slot; a dense vector (r = D) is
+// the same code with an all-ones bitmap.  The 32-slot body exists once (word loop rolled): the
+// hot code must stay small, instruction fetch is a shared per-GPC resource.
+template <int BIT>
+__device__ __forceinline__ void take_slot(uint32_t w, uint32_t& v, uint32_t& vptr) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        ".reg .b32 t;\n"
+        "and.b32 t, %2, %3;\n"
+        "setp.ne.u32 p, t, 0;\n"
+        "@p ld.shared.u16 %0, [%1];\n"
+        "@p add.u32 %1, %1, 2;\n"
+        "}\n"
+        : "+r"(v), "+r"(vptr)
+        : "r"(w), "n"(1u << BIT)
+        : "memory");
+}
+
+template <int OCT>
+__device__ __forceinline__ void assemble_octet(uint32_t w, uint32_t& vptr, uint32_t dst) {
+    uint32_t v[8];
 #pragma unroll
-        for (int i = 0; i < 16; ++i) sts_128(row + 16 * i, z4);
-        return;
-    }
-    if (r == kD) {
-        if ((val & 15u) == 0) {
-#pragma unroll
-            for (int i = 0; i < 16; ++i) sts_128(row + 16 * i, lds_128(val + 16 * i));
-        } else {  // ragged token block: values only 2-byte aligned
-            for (int c = 0; c < kD; ++c) sts_u16(row + 2 * c, lds_u16(val + 2 * c));
+    for (int c = 0; c < 8; ++c) v[c] = 0u;
+    take_slot<8 * OCT + 0>(w, v[0], vptr);
+    take_slot<8 * OCT + 1>(w, v[1], vptr);
+    take_slot<8 * OCT + 2>(w, v[2], vptr);
+    take_slot<8 * OCT + 3>(w, v[3], vptr);
+    take_slot<8 * OCT + 4>(w, v[4], vptr);
+    take_slot<8 * OCT + 5>(w, v[5], vptr);
+    take_slot<8 * OCT + 6>(w, v[6], vptr);
+    take_slot<8 * OCT + 7>(w, v[7], vptr);
+    uint4 o;  // hi * 65536 + lo: an IMAD (FMA pipe), not a PRMT/LOP3 (ALU pipe)
+    o.x = v[1] * 65536u + v[0];
+    o.y = v[3] * 65536u + v[2];
+    o.z = v[5] * 65536u + v[4];
+    o.w = v[7] * 65536u + v[6];
+    sts_128(dst + 16 * OCT, o);
+}
+
+__device__ __noinline__ void expand_row(uint32_t row, uint32_t bm, uint32_t val, int r, bool valid) {
+    uint32_t w0 = 0u, w1 = 0u, w2 = 0u, w3 = 0u;
+    if (valid) {
+        if (r == kD) {
+            w0 = w1 = w2 = w3 = 0xffffffffu;
+        } else if ((bm & 15u) == 0) {
+            const uint4 b = lds_128(bm);
+            w0 = b.x; w1 = b.y; w2 = b.z; w3 = b.w;
+        } else {  // ragged token block: bitmaps are only 2-byte aligned
+            w0 = lds_u16(bm) | (lds_u16(bm + 2) << 16);
+            w1 = lds_u16(bm + 4) | (lds_u16(bm + 6) << 16);
+            w2 = lds_u16(bm + 8) | (lds_u16(bm + 10) << 16);
+            w3 = lds_u16(bm + 12) | (lds_u16(bm + 14) << 16);
         }
-        return;
     }
-#pragma unroll
-    for (int i = 0; i < 16; ++i) sts_128(row + 16 * i, z4);
-    uint32_t w[4];
-    if ((bm & 15u) == 0) {
-        const uint4 b = lds_128(bm);
-        w[0] = b.x; w[1] = b.y; w[2] = b.z; w[3] = b.w;
-    } else {
-#pragma unroll
-        for (int j = 0; j < 4; ++j) w[j] = lds_u16(bm + 4 * j) | (lds_u16(bm + 4 * j + 2) << 16);
-    }
-    uint32_t vp = val + 2 * (uint32_t)(r - 1);  // address of the last kept value
-#pragma unroll
-    for (int j = 3; j >= 0; --j) {
-        uint32_t wj = w[j];
-        const uint32_t base = row + 64 * j;
-        while (wj) {
-            const int pos = 31 - __clz(wj);
-            wj ^= 1u << pos;
-            sts_u16(base + 2 * pos, lds_u16(vp));
-            vp -= 2;
-        }
+    uint32_t vptr = val;  // never dereferenced by a lane whose bitmap is empty
+#pragma unroll 1
+    for (int j = 0; j < 4; ++j) {
+        const uint32_t w = w0;
+        w0 = w1; w1 = w2; w2 = w3;
+#ifndef MKV_DBG_NO_DECODE
+        assemble_octet<0>(w, vptr, row);
+        assemble_octet<1>(w, vptr, row);
+        assemble_octet<2>(w, vptr, row);
+        assemble_octet<3>(w, vptr, row);
+#endif
+        row += 64;
     }
 }
 
@@ -205,7 +225,7 @@ __host__ __device__ constexpr int warp_smem_bytes(int nstage) {
 // main kernel: one CTA per SM, kWarps independent warps, each owning the block range
 // [gw*T/GW, (gw+1)*T/GW) of the concatenated selection lists.
 // ------------------------------------------------------------------------------------------
-template <int NSTAGE>
+template <int NSTAGE, int kWarps>
 __global__ void __launch_bounds__(kWarps * 32, 1)
 mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q,
                             const int32_t* __restrict__ sel, const int32_t* __restrict__ sel_count, int k_max,
@@ -230,15 +250,6 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     Desc* desc = reinterpret_cast<Desc*>(wbase + NSTAGE * kStageBytes + kTileBytes);
     GInfo* ginfo = reinterpret_cast<GInfo*>(wbase + NSTAGE * kStageBytes + kTileBytes + kDescRing * 16);
     int2* gmeta = reinterpret_cast<int2*>(reinterpret_cast<uint8_t*>(ginfo) + NSTAGE * 64);  // (unit, n)
-    const uint32_t bar0 = smem_u32(gmeta) + NSTAGE * 8;
-
-    if (lane == 0) {
-#pragma unroll
-        for (int s = 0; s < NSTAGE; ++s) mbar_init(bar0 + 8 * s, 1);
-    }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    fence_proxy_async();
-    __syncwarp();
 
     int pos = 0, built = 0;
 
@@ -272,6 +283,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         if (built - pos <= 8 && built < n_total) build(min(32, n_total - built));
         if (pos >= n_total) {
             if (lane == 0) gmeta[s] = make_int2(-1, 0);
+            cp_async_commit();  // keeps the group count in step with the wait in the main loop
             return;
         }
         const bool have = lane < 4 && pos + lane < built;
@@ -294,19 +306,23 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             gi.off = cum - d.bytes; gi.r_k = d.r_k; gi.r_v = d.r_v; gi.nb = d.nb;
             ginfo[s * 4 + lane] = gi;
         }
-        const uint32_t bar = bar0 + 8 * s;
-        if (lane == 0) {
-            gmeta[s] = make_int2(unit0, n);
-            mbar_expect_tx(bar, total);
+        if (lane == 0) gmeta[s] = make_int2(unit0, n);
+        // every lane copies 16-byte chunks of each block of the group (LDGSTS, L1 bypass)
+        const uint32_t my_dst = stage0 + s * kStageBytes + (cum - d.bytes);
+        const unsigned long long my_src = reinterpret_cast<unsigned long long>(lv.slice) + ((unsigned long long)d.off16 << 4);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            if (i < n) {
+                const uint32_t dst = __shfl_sync(kFull, my_dst, i);
+                const unsigned long long src = __shfl_sync(kFull, my_src, i);
+                const uint32_t nbytes = __shfl_sync(kFull, d.bytes, i);
+                for (uint32_t o = 16u * lane; o < nbytes; o += 512u) cp_async_16(dst + o, src + o);
+            }
         }
-        if (lane < n && d.bytes > 0)
-            bulk_g2s(stage0 + s * kStageBytes + (cum - d.bytes), lv.slice + ((size_t)d.off16 << 4), d.bytes, bar);
+        cp_async_commit();
         pos += n;
     };
 
-    build(min(32, n_total));
-#pragma unroll
-    for (int s = 0; s < NSTAGE; ++s) issue(s);
 
     // per-unit state
     uint32_t bq[8][2];
@@ -361,14 +377,21 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     const uint32_t a_qk = tile + (uint32_t)(((mi & 1) * 8 + mr) * kTileStride + (mi >> 1) * 16);
     const uint32_t a_pv = tile + (uint32_t)(((mi >> 1) * 8 + mr) * kTileStride + (mi & 1) * 16);
 
-    for (int k = 0;; ++k) {
-        const int s = k % NSTAGE;
+    // One call site each for issue() and flush() (code size): iterations k < 0 only fill the pipeline.
+    uint32_t ph[2][2], pl[2][2];  // P = hi + lo in bf16, [k-step of 16 tokens][b0 / b1]
+#pragma unroll 1
+    for (int k = -NSTAGE;; ++k) {
+        const int s = (k + NSTAGE) % NSTAGE;
+        const bool active = k >= 0;
+        float S[2][4];
+        int nbj[4];
+        if (active) {
         __syncwarp();
         const int2 meta = gmeta[s];
         const int n = meta.y;
-        if (n == 0) break;
         if (meta.x != cur_unit) {
             if (cur_unit >= 0) flush();
+            if (n == 0) break;
             cur_unit = meta.x;
             const int bi = cur_unit / g.n_kv_heads, hk = cur_unit % g.n_kv_heads;
             const uint32_t* qrow = reinterpret_cast<const uint32_t*>(
@@ -384,7 +407,6 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             l0 = l1 = 0.f;
         }
         const GInfo gi = ginfo[s * 4 + mi];
-        int nbj[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) nbj[j] = j < n ? (int)ginfo[s * 4 + j].nb : 0;
         const bool valid = mi < n && mr < (int)gi.nb;
@@ -396,12 +418,12 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         const uint32_t v_bm = v_bm0 + mr * bmv;
         const uint32_t v_val = v_bm0 + gi.nb * bmv + mr * gi.r_v * 2;
 
-        mbar_wait(bar0 + 8 * s, (uint32_t)(k / NSTAGE) & 1u);
+        cp_async_wait<NSTAGE - 1>();  // this lane's copies of group k have landed ...
+        __syncwarp();                 // ... and so have every other lane's
 
         // ---- K: expand, S = K q^T on the tensor cores (tokens = M, heads = N)
         expand_row(my_row, k_bm, k_val, (int)gi.r_k, valid);
         __syncwarp();
-        float S[2][4];
 #pragma unroll
         for (int mt = 0; mt < 2; ++mt) {
             S[mt][0] = S[mt][1] = S[mt][2] = S[mt][3] = 0.f;
@@ -416,8 +438,9 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         // ---- V: expand into the same tile (overlaps the softmax arithmetic below)
         expand_row(my_row, v_bm, v_val, (int)gi.r_v, valid);
         __syncwarp();
-        fence_proxy_async();
+        }  // active
         issue(s);  // stage s is free: start the copies of group k + NSTAGE
+        if (!active) continue;
 
         // ---- online softmax in the exp2 domain; this lane: tokens 8j + gq (j = 0..3), heads 2qq, 2qq+1
         float mx0 = -INFINITY, mx1 = -INFINITY;
@@ -446,7 +469,6 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         }
         m0 = mn0; m1 = mn1;
         l0 *= c0; l1 *= c1;
-        uint32_t ph[2][2], pl[2][2];  // [k-step of 16 tokens][b0 / b1], P = hi + lo in bf16
 #pragma unroll
         for (int mt = 0; mt < 2; ++mt) {
 #pragma unroll
@@ -471,19 +493,18 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             }
         }
     }
-    if (cur_unit >= 0) flush();
 }
 
 // ------------------------------------------------------------------------------------------
 // step 3d: merge the partials of every unit that was shared between warps; units with an empty
 // selection get out = 0, lse = -inf; units finished by a single warp are already written.
-// grid = n_units, block = 128 (thread = channel).  GW = warps of the main kernel's grid.
+// grid = (n_units, G), block = 128 (thread = channel).  GW = warps of the main kernel's grid.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) mkv_combine_kernel(CacheGeom g, const int32_t* __restrict__ sel_count, int k_max,
                                                           int GW, const float* __restrict__ part_o,
                                                           const float* __restrict__ part_ml, float* __restrict__ out,
                                                           float* __restrict__ lse) {
-    const int u = blockIdx.x, c = threadIdx.x;
+    const int u = blockIdx.x, gi = blockIdx.y, c = threadIdx.x;
     __shared__ int s_a[4], s_t[4];
     int before = 0, total = 0;
     for (int i = c; i < g.n_units; i += 128) {
@@ -503,12 +524,10 @@ __global__ void __launch_bounds__(128) mkv_combine_kernel(CacheGeom g, const int
     const int b = a + min(max(sel_count[u], 0), k_max);
     const int G = g.group;
     const int bi = u / g.n_kv_heads, hk = u % g.n_kv_heads;
-    const size_t row = (size_t)bi * g.n_q_heads + (size_t)hk * G;
+    const size_t row = (size_t)bi * g.n_q_heads + (size_t)hk * G + gi;
     if (b == a) {
-        for (int gi = 0; gi < G; ++gi) {
-            out[(row + gi) * kD + c] = 0.f;
-            if (lse != nullptr && c == 0) lse[row + gi] = -INFINITY;
-        }
+        out[row * kD + c] = 0.f;
+        if (lse != nullptr && c == 0) lse[row] = -INFINITY;
         return;
     }
     auto lo_of = [&](long long w) { return (int)(w * T / GW); };
@@ -518,53 +537,90 @@ __global__ void __launch_bounds__(128) mkv_combine_kernel(CacheGeom g, const int
     while (last + 1 < GW && lo_of(last + 1) < b) ++last;
     while (lo_of(last) >= b) --last;
     if (first == last) return;  // one warp saw the whole unit and wrote the result itself
-    for (int gi = 0; gi < G; ++gi) {
-        float M = -INFINITY;
-        for (long long w = first; w <= last; ++w) {
+    __shared__ int s_slot[128];
+    __shared__ float s_m[128], s_l[128];
+    float M = -INFINITY, L = 0.f, O = 0.f;
+    for (long long w0 = first; w0 <= last; w0 += 128) {
+        __syncthreads();
+        const long long w = w0 + c;
+        int slot = -1;
+        if (w <= last) {
             const int wl = lo_of(w), wh = lo_of(w + 1);
-            if (wl >= wh) continue;
-            const size_t slot = (size_t)w * 2 + (a < wl ? 0 : 1);
-            M = fmaxf(M, part_ml[slot * (2 * kMaxGroup) + 2 * gi]);
+            if (wl < wh) slot = (int)(w * 2 + (a < wl ? 0 : 1));
         }
-        float L = 0.f, O = 0.f;
-        for (long long w = first; w <= last; ++w) {
-            const int wl = lo_of(w), wh = lo_of(w + 1);
-            if (wl >= wh) continue;
-            const size_t slot = (size_t)w * 2 + (a < wl ? 0 : 1);
-            const float ms = part_ml[slot * (2 * kMaxGroup) + 2 * gi];
-            const float wgt = ms == -INFINITY ? 0.f : ex2(ms - M);
-            L = fmaf(part_ml[slot * (2 * kMaxGroup) + 2 * gi + 1], wgt, L);
-            O = fmaf(part_o[(slot * G + gi) * kD + c], wgt, O);
+        s_slot[c] = slot;
+        s_m[c] = slot >= 0 ? part_ml[(size_t)slot * (2 * kMaxGroup) + 2 * gi] : -INFINITY;
+        s_l[c] = slot >= 0 ? part_ml[(size_t)slot * (2 * kMaxGroup) + 2 * gi + 1] : 0.f;
+        __syncthreads();
+        const int cnt = (int)min((long long)128, last - w0 + 1);
+        float mx = M;
+        for (int i = 0; i < cnt; ++i) mx = fmaxf(mx, s_m[i]);
+        const float bs = mx == -INFINITY ? 0.f : mx;
+        const float co = ex2(M - bs);
+        L *= co; O *= co; M = mx;
+        for (int i0 = 0; i0 < cnt; i0 += 8) {  // eight independent loads in flight
+            float os[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                const int sl = i0 + e < cnt ? s_slot[i0 + e] : -1;
+                os[e] = sl >= 0 ? part_o[((size_t)sl * G + gi) * kD + c] : 0.f;
+            }
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                if (i0 + e < cnt) {
+                    const float wgt = ex2(s_m[i0 + e] - bs);
+                    L = fmaf(s_l[i0 + e], wgt, L);
+                    O = fmaf(os[e], wgt, O);
+                }
+            }
         }
-        out[(row + gi) * kD + c] = L > 0.f ? O / L : 0.f;
-        if (lse != nullptr && c == 0) lse[row + gi] = L > 0.f ? (M + log2f(L)) * kLn2 : -INFINITY;
     }
+    out[row * kD + c] = L > 0.f ? O / L : 0.f;
+    if (lse != nullptr && c == 0) lse[row] = L > 0.f ? (M + log2f(L)) * kLn2 : -INFINITY;
 }
 
 }  // namespace
 
-int attention_partial_slots(int sm_count) { return sm_count * kWarps * 2; }
+int attention_partial_slots(int sm_count) { return sm_count * kMaxWarps * 2; }
+
+template <int NSTAGE, int NWARPS>
+static cudaError_t launch_attention_cfg(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
+                                        const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
+                                        const AttnScratch& scr, int sm_count, cudaStream_t s) {
+    const int smem = NWARPS * warp_smem_bytes(NSTAGE) + (g.n_units + 1) * 4;
+    static int configured = 0;  // largest dynamic shared-memory size opted into so far
+    if (smem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(mkv_packed_attention_kernel<NSTAGE, NWARPS>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        configured = smem;
+    }
+    mkv_packed_attention_kernel<NSTAGE, NWARPS><<<sm_count, NWARPS * 32, smem, s>>>(
+        g, lv, q, sel, sel_count, k_max, scale * kLog2e, out, lse, scr.part_o, scr.part_ml);
+    cudaError_t err = cudaGetLastError();
+    if (err != cudaSuccess) return err;
+    mkv_combine_kernel<<<dim3(g.n_units, g.group), 128, 0, s>>>(g, sel_count, k_max, sm_count * NWARPS, scr.part_o, scr.part_ml,
+                                                                 out, lse);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
                              const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
                              const AttnScratch& scr, int sm_count, cudaStream_t s, int* n_kernels) {
     if (g.n_units > kMaxUnitsSmem) return cudaErrorInvalidValue;
-    const int smem = kWarps * warp_smem_bytes(kStages) + (g.n_units + 1) * 4;
-    static int configured = 0;  // largest dynamic shared-memory size opted into so far
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(mkv_packed_attention_kernel<kStages>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
-    const float scale_log2 = scale * kLog2e;
-    mkv_packed_attention_kernel<kStages><<<sm_count, kWarps * 32, smem, s>>>(g, lv, q, sel, sel_count, k_max, scale_log2,
-                                                                              out, lse, scr.part_o, scr.part_ml);
-    cudaError_t err = cudaGetLastError();
-    if (err != cudaSuccess) return err;
-    mkv_combine_kernel<<<g.n_units, 128, 0, s>>>(g, sel_count, k_max, sm_count * kWarps, scr.part_o, scr.part_ml, out, lse);
     if (n_kernels) *n_kernels = 2;
-    return cudaGetLastError();
+    static int cfg = -1;  // tuning knob (stages * 100 + warps); default chosen from measurements
+    if (cfg < 0) {
+        const char* e = getenv("MKV_ATTN_CFG");
+        cfg = e ? atoi(e) : 210;
+    }
+#define MKV_CFG(S, W) \
+    case S * 100 + W: return launch_attention_cfg<S, W>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, sm_count, s);
+    switch (cfg) {
+        MKV_CFG(1, 12) MKV_CFG(1, 14) MKV_CFG(2, 8) MKV_CFG(2, 10) MKV_CFG(3, 8) MKV_CFG(2, 4) MKV_CFG(2, 6)
+        default: return launch_attention_cfg<2, 10>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, sm_count, s);
+    }
+#undef MKV_CFG
 }
 
 }  // namespace mkv
