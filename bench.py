@@ -165,15 +165,14 @@ def run_mkv(args):
         __graft_entry__.build()
     barrier()
     from paper_2607_00760_b200 import binding as mkv
-    from paper_2607_00760_b200 import synth, workload
+    from paper_2607_00760_b200 import shard, synth, workload
 
     w = synth.WORKLOADS[args.workload]
     n_layers = args.layers or w.n_layers
     Bt = args.batch or w.batch
     N = args.context or w.context
     # weak scaling: every rank holds its own batch of Bt requests (units are independent: no collective)
-    if world > 1:
-        w = synth.Workload(**{**w.__dict__, "seed": w.seed + rank, "config_id": w.config_id})
+    w = shard.rank_workload(w, rank)
     t0 = time.time()
     built = workload.build(w, dev, n_layers=n_layers, batch=Bt, context=N, verbose=args.verbose and rank == 0)
     build_s = time.time() - t0
