@@ -4,14 +4,22 @@
 // Design:
 //   * The selected blocks of all units form one stream of T blocks; it is cut into equal ranges,
 //     one per warp of a one-CTA-per-SM grid (warps are fully independent: no __syncthreads in
-//     the main loop).  A warp walks its range in groups of <= 4 token blocks (32 tokens).
-//   * Each group's packed payloads (one contiguous chunk per block, DESIGN.md format) are brought
-//     into a per-warp shared-memory stage by cp.async.bulk (TMA bulk engine) completing on an
-//     mbarrier; kStages groups are in flight per warp.
-//   * lane = token: every lane expands its token's packed K vector (bitmap + kept bf16) into a
-//     dense bf16 row of a [32 tokens][128 ch] tile, the warp runs QK^T on the tensor cores
-//     (mma.sync m16n8k16, tokens = M, heads = N), an online softmax in the exp2 domain, expands V
-//     into the same tile and runs PV with P split into bf16 hi + lo (fp32-class accuracy).
+//     the main loop).  A warp walks its range in groups of <= 2 token blocks (16 tokens).
+//   * Each group's packed payloads (one contiguous chunk per block, DESIGN.md format) are copied
+//     verbatim into a per-warp shared-memory stage with 16-byte cp.async (LDGSTS, L1 bypass);
+//     kStages groups are in flight per warp.
+//   * Packed vectors are expanded STRAIGHT INTO mma.sync fragments — no dense tile in shared
+//     memory.  QK: S = K q^T with the group's 16 tokens = M (rows 0-7 block 0, rows 8-15 block
+//     1), heads = N, channels = K; lane (gq, qq) owns token gq of each block and bitmap word qq
+//     (32 channels) and walks its 32 slots in order: a set bit loads the next kept bf16 of its
+//     run and bumps the run pointer.  The channel order inside a k-step is a fixed permutation
+//     applied to q's B fragments as well.
+//     PV: O^T = V^T P^T with channels = M, heads = N, the 16 tokens of the group = K; lane
+//     (gq, qq) owns tokens 2qq, 2qq+1 of each block and the 16-channel half-word gq, so a
+//     fragment register pairs two TOKENS of one channel, as the contraction over tokens needs.
+//     P is split into bf16 hi + lo (fp32-class accuracy) and transposed into the B fragment
+//     layout with movmatrix.  Dense vectors (r = D) skip the walk: their fragments are 16-byte
+//     shared loads.
 //   * A unit wholly inside one warp's range is normalised and written directly; otherwise the
 //     warp writes an (m, l, O) partial (<= 2 per warp) that the combine kernel merges (step 3d).
 #include <cstdlib>
@@ -26,22 +34,21 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 
-constexpr int kMaxWarps = 16;                 // upper bound on warps per CTA (sizes the partial-slot scratch)
-constexpr int kStageBytes = 6144;             // >= 4 blocks at r = 38 (5888 B), >= 1 dense block (4096 B)
-constexpr int kTileStride = 272;              // bytes per token row: 256 + 16 pad (ldmatrix conflict-free)
-constexpr int kTileBytes = 32 * kTileStride;  // 8704
-constexpr int kDescRing = 64;                 // block descriptors kept per warp
+constexpr int kMaxWarps = 16;      // upper bound on warps per CTA (sizes the partial-slot scratch)
+constexpr int kStageBytes = 4096;  // one dense block (4096 B) or two packed blocks with r <= 56
+constexpr int kDescRing = 64;      // block descriptors kept per warp
 constexpr int kMaxUnitsSmem = 2048;
 
-struct __align__(16) Desc {   // one selected token block
-    uint32_t off16;           // payload offset in the layer slice, 16-B units
-    uint32_t bytes;           // payload bytes (multiple of 16); 0 = skip (invalid entry)
+struct __align__(16) Desc {  // one selected token block
+    uint32_t off16;          // payload offset in the layer slice, 16-B units
+    uint32_t bytes;          // payload bytes (multiple of 16); 0 = skip (invalid entry)
     int32_t unit;
     uint8_t r_k, r_v, nb, pad;
 };
-struct __align__(16) GInfo {  // one block of an in-flight group
-    uint32_t off;             // byte offset inside the stage
-    uint32_t r_k, r_v, nb;
+struct __align__(16) GMeta {  // one in-flight group (<= 2 blocks of one unit with equal r_k, r_v)
+    int32_t unit, n;          // n = 0: end of the range
+    uint32_t off1;            // stage offset of the second block
+    uint32_t rknb;            // r_k | r_v << 8 | nb0 << 16 | nb1 << 24
 };
 
 // ---- PTX wrappers ---------------------------------------------------------------------------
@@ -54,26 +61,18 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() {
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
-__device__ __forceinline__ void ldmatrix_x4(uint32_t addr, uint32_t (&r)[4]) {
-    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
-                 : "r"(addr));
-}
-__device__ __forceinline__ void ldmatrix_x4_trans(uint32_t addr, uint32_t (&r)[4]) {
-    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
-                 : "r"(addr));
-}
 __device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {
     uint32_t d;
     asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(d) : "r"(a));
     return d;
 }
-__device__ __forceinline__ void mma_bf16(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+// D(16x8) += A(16x16) B(16x8), bf16 inputs, fp32 accumulate
+__device__ __forceinline__ void mma_bf16(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                         uint32_t b0, uint32_t b1) {
     asm volatile(
         "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
         : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+        : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
 __device__ __forceinline__ float ex2(float x) {
     float y;
@@ -86,12 +85,14 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
     return d;
 }
-__device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v) {
-    asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v));
-}
 __device__ __forceinline__ uint32_t lds_u16(uint32_t addr) {
     unsigned short v;
     asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
     return v;
 }
 __device__ __forceinline__ uint4 lds_128(uint32_t addr) {
@@ -99,24 +100,17 @@ __device__ __forceinline__ uint4 lds_128(uint32_t addr) {
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
     return v;
 }
-__device__ __forceinline__ void sts_128(uint32_t addr, uint4 v) {
-    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w));
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
+    uint32_t d;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
+    return d;
 }
 
-// ---- lane = token: expand one packed (or dense) vector into this lane's dense tile row ------
-// row: shared address of the lane's 256-byte tile row; bm / val: shared addresses in the stage.
-//
-// "Row assembly": the lane walks its 128 channel slots in order.  For slot c the bitmap bit (an
-// immediate mask, so the test is one LOP3 into a predicate) guards a 2-byte load of the next kept
-// value and the advance of the value pointer; a dropped slot keeps the zero its register was
-// initialised with.  Eight slots are packed into four registers and stored with one 16-byte store.
-// Why this shape: it is uniform across lanes (no divergence, no padding
-// to the longest lane), needs no zero-fill pass and no scattered 2-byte stores (bank conflicts),
-// no FLO/POPC (XU pipe), and only ~1.5 ALU-pipe instructions per slot; a dense vector (r = D) is
-// the same code with an all-ones bitmap.  The 32-slot body exists once (word loop rolled): the
-// hot code must stay small, instruction fetch is a shared per-GPC resource.
-template <int BIT>
-__device__ __forceinline__ void take_slot(uint32_t w, uint32_t& v, uint32_t& vptr) {
+// One slot of a packed run: if bit MASK of the position bitmap `w` is set, load the next kept
+// bf16 of the run into `v` (which the caller zero-initialised) and advance the run pointer.
+// Predicated, no branch: every lane executes the same instruction stream whatever its bitmap.
+template <uint32_t MASK>
+__device__ __forceinline__ void take_slot(uint32_t w, uint32_t& v, uint32_t& ptr) {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
@@ -126,60 +120,50 @@ __device__ __forceinline__ void take_slot(uint32_t w, uint32_t& v, uint32_t& vpt
         "@p ld.shared.u16 %0, [%1];\n"
         "@p add.u32 %1, %1, 2;\n"
         "}\n"
-        : "+r"(v), "+r"(vptr)
-        : "r"(w), "n"(1u << BIT)
+        : "+r"(v), "+r"(ptr)
+        : "r"(w), "n"(MASK)
         : "memory");
 }
+// hi * 65536 + lo: an IMAD (FMA pipe), not a PRMT/LOP3 (ALU pipe, which the bit tests load)
+__device__ __forceinline__ uint32_t pair16(uint32_t lo, uint32_t hi) { return hi * 65536u + lo; }
 
-template <int OCT>
-__device__ __forceinline__ void assemble_octet(uint32_t w, uint32_t& vptr, uint32_t dst) {
-    uint32_t v[8];
-#pragma unroll
-    for (int c = 0; c < 8; ++c) v[c] = 0u;
-    take_slot<8 * OCT + 0>(w, v[0], vptr);
-    take_slot<8 * OCT + 1>(w, v[1], vptr);
-    take_slot<8 * OCT + 2>(w, v[2], vptr);
-    take_slot<8 * OCT + 3>(w, v[3], vptr);
-    take_slot<8 * OCT + 4>(w, v[4], vptr);
-    take_slot<8 * OCT + 5>(w, v[5], vptr);
-    take_slot<8 * OCT + 6>(w, v[6], vptr);
-    take_slot<8 * OCT + 7>(w, v[7], vptr);
-    uint4 o;  // hi * 65536 + lo: an IMAD (FMA pipe), not a PRMT/LOP3 (ALU pipe)
-    o.x = v[1] * 65536u + v[0];
-    o.y = v[3] * 65536u + v[2];
-    o.z = v[5] * 65536u + v[4];
-    o.w = v[7] * 65536u + v[6];
-    sts_128(dst + 16 * OCT, o);
+// K walk, k-step KS (4 slots of this lane's bitmap word) of two runs at once (token gq of block
+// 0 and of block 1) -> A fragment a0..a3
+template <int KS>
+__device__ __forceinline__ void k_step(uint32_t w0, uint32_t w1, uint32_t& p0, uint32_t& p1, uint32_t (&b)[4]) {
+    uint32_t e[4] = {0u, 0u, 0u, 0u}, f[4] = {0u, 0u, 0u, 0u};
+    take_slot<1u << (4 * KS + 0)>(w0, e[0], p0);
+    take_slot<1u << (4 * KS + 0)>(w1, f[0], p1);
+    take_slot<1u << (4 * KS + 1)>(w0, e[1], p0);
+    take_slot<1u << (4 * KS + 1)>(w1, f[1], p1);
+    take_slot<1u << (4 * KS + 2)>(w0, e[2], p0);
+    take_slot<1u << (4 * KS + 2)>(w1, f[2], p1);
+    take_slot<1u << (4 * KS + 3)>(w0, e[3], p0);
+    take_slot<1u << (4 * KS + 3)>(w1, f[3], p1);
+    b[0] = pair16(e[0], e[1]);  // row gq   (block 0), k = 2qq, 2qq+1
+    b[1] = pair16(f[0], f[1]);  // row gq+8 (block 1)
+    b[2] = pair16(e[2], e[3]);  // row gq,   k = 2qq+8, 2qq+9
+    b[3] = pair16(f[2], f[3]);  // row gq+8
 }
 
-__device__ __noinline__ void expand_row(uint32_t row, uint32_t bm, uint32_t val, int r, bool valid) {
-    uint32_t w0 = 0u, w1 = 0u, w2 = 0u, w3 = 0u;
-    if (valid) {
-        if (r == kD) {
-            w0 = w1 = w2 = w3 = 0xffffffffu;
-        } else if ((bm & 15u) == 0) {
-            const uint4 b = lds_128(bm);
-            w0 = b.x; w1 = b.y; w2 = b.z; w3 = b.w;
-        } else {  // ragged token block: bitmaps are only 2-byte aligned
-            w0 = lds_u16(bm) | (lds_u16(bm + 2) << 16);
-            w1 = lds_u16(bm + 4) | (lds_u16(bm + 6) << 16);
-            w2 = lds_u16(bm + 8) | (lds_u16(bm + 10) << 16);
-            w3 = lds_u16(bm + 12) | (lds_u16(bm + 14) << 16);
-        }
-    }
-    uint32_t vptr = val;  // never dereferenced by a lane whose bitmap is empty
-#pragma unroll 1
-    for (int j = 0; j < 4; ++j) {
-        const uint32_t w = w0;
-        w0 = w1; w1 = w2; w2 = w3;
-#ifndef MKV_DBG_NO_DECODE
-        assemble_octet<0>(w, vptr, row);
-        assemble_octet<1>(w, vptr, row);
-        assemble_octet<2>(w, vptr, row);
-        assemble_octet<3>(w, vptr, row);
-#endif
-        row += 64;
-    }
+// V walk, M tile I (channel slots 2I, 2I+1 of this lane's half-word) of four runs at once
+// (tokens A = 2qq and B = 2qq+1 of block 0 and of block 1) -> A fragment a0..a3
+template <int I>
+__device__ __forceinline__ void v_step(uint32_t hA0, uint32_t hB0, uint32_t hA1, uint32_t hB1, uint32_t& pA0,
+                                       uint32_t& pB0, uint32_t& pA1, uint32_t& pB1, uint32_t (&a)[4]) {
+    uint32_t x[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+    take_slot<1u << (2 * I)>(hA0, x[0], pA0);
+    take_slot<1u << (2 * I)>(hB0, x[1], pB0);
+    take_slot<1u << (2 * I)>(hA1, x[4], pA1);
+    take_slot<1u << (2 * I)>(hB1, x[5], pB1);
+    take_slot<1u << (2 * I + 1)>(hA0, x[2], pA0);
+    take_slot<1u << (2 * I + 1)>(hB0, x[3], pB0);
+    take_slot<1u << (2 * I + 1)>(hA1, x[6], pA1);
+    take_slot<1u << (2 * I + 1)>(hB1, x[7], pB1);
+    a[0] = pair16(x[0], x[1]);  // row gq   (channel 16gq + 2I),     tokens 2qq, 2qq+1 of block 0
+    a[1] = pair16(x[2], x[3]);  // row gq+8 (channel 16gq + 2I + 1), block 0
+    a[2] = pair16(x[4], x[5]);  // row gq,   block 1
+    a[3] = pair16(x[6], x[7]);  // row gq+8, block 1
 }
 
 // prefix sums of the clamped selection counts -> s_cum[0..n_units]; returns the total T
@@ -218,7 +202,7 @@ __device__ __forceinline__ int find_unit(const int* s_cum, int n_units, int i) {
 }
 
 __host__ __device__ constexpr int warp_smem_bytes(int nstage) {
-    return nstage * kStageBytes + kTileBytes + kDescRing * 16 + nstage * 64 + 64;
+    return nstage * kStageBytes + kDescRing * 16 + nstage * 16;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -235,7 +219,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     constexpr int kWS = warp_smem_bytes(NSTAGE);
     int* s_cum = reinterpret_cast<int*>(smem + kWarps * kWS);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int gq = lane >> 2, qq = lane & 3;  // mma fragment coordinates
+    const int gq = lane >> 2, qq = lane & 3;  // mma fragment coordinates (groupID, threadID_in_group)
 
     const int T = scan_counts(sel_count, g.n_units, k_max, s_cum);
     const int GW = gridDim.x * kWarps, gw = blockIdx.x * kWarps + warp;
@@ -246,10 +230,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
 
     uint8_t* wbase = smem + warp * kWS;
     const uint32_t stage0 = smem_u32(wbase);
-    const uint32_t tile = stage0 + NSTAGE * kStageBytes;
-    Desc* desc = reinterpret_cast<Desc*>(wbase + NSTAGE * kStageBytes + kTileBytes);
-    GInfo* ginfo = reinterpret_cast<GInfo*>(wbase + NSTAGE * kStageBytes + kTileBytes + kDescRing * 16);
-    int2* gmeta = reinterpret_cast<int2*>(reinterpret_cast<uint8_t*>(ginfo) + NSTAGE * 64);  // (unit, n)
+    Desc* desc = reinterpret_cast<Desc*>(wbase + NSTAGE * kStageBytes);
+    GMeta* gmeta = reinterpret_cast<GMeta*>(wbase + NSTAGE * kStageBytes + kDescRing * 16);
 
     int pos = 0, built = 0;
 
@@ -278,56 +260,51 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         __syncwarp();
     };
 
-    // form the next group (<= 4 blocks of one unit, <= kStageBytes) and start its bulk copies
+    // form the next group (<= 2 blocks of one unit with the same strategy, <= kStageBytes) and
+    // start its copies into stage s
     auto issue = [&](int s) {
         if (built - pos <= 8 && built < n_total) build(min(32, n_total - built));
         if (pos >= n_total) {
-            if (lane == 0) gmeta[s] = make_int2(-1, 0);
+            if (lane == 0) { GMeta m; m.unit = -1; m.n = 0; m.off1 = 0; m.rknb = 0; gmeta[s] = m; }
             cp_async_commit();  // keeps the group count in step with the wait in the main loop
             return;
         }
-        const bool have = lane < 4 && pos + lane < built;
-        Desc d;
-        d.unit = -2; d.bytes = 0; d.off16 = 0; d.r_k = 0; d.r_v = 0; d.nb = 0; d.pad = 0;
-        if (have) d = desc[(pos + lane) & (kDescRing - 1)];
-        const int unit0 = __shfl_sync(kFull, d.unit, 0);
-        uint32_t cum = d.bytes;
-#pragma unroll
-        for (int o = 1; o < 4; o <<= 1) {
-            const uint32_t v = __shfl_up_sync(kFull, cum, o);
-            if (lane >= o) cum += v;
+        const Desc d0 = desc[pos & (kDescRing - 1)];
+        Desc d1 = d0;
+        bool two = false;
+        if (pos + 1 < n_total) {
+            d1 = desc[(pos + 1) & (kDescRing - 1)];
+            two = d1.unit == d0.unit && d1.r_k == d0.r_k && d1.r_v == d0.r_v && d0.bytes != 0 && d1.bytes != 0 &&
+                  d0.bytes + d1.bytes <= (uint32_t)kStageBytes;
         }
-        const bool ok = have && d.unit == unit0 && cum <= (uint32_t)kStageBytes;
-        const unsigned mask = __ballot_sync(kFull, ok) & 0xFu;
-        const int n = __ffs(~mask) - 1;  // leading run of ok lanes (lane 0 is always ok)
-        const uint32_t total = __shfl_sync(kFull, cum, n - 1);
-        if (lane < n) {
-            GInfo gi;
-            gi.off = cum - d.bytes; gi.r_k = d.r_k; gi.r_v = d.r_v; gi.nb = d.nb;
-            ginfo[s * 4 + lane] = gi;
+        if (lane == 0) {
+            GMeta m;
+            m.unit = d0.unit; m.n = two ? 2 : 1; m.off1 = d0.bytes;
+            m.rknb = (uint32_t)d0.r_k | ((uint32_t)d0.r_v << 8) | ((uint32_t)d0.nb << 16) |
+                     ((two ? (uint32_t)d1.nb : 0u) << 24);
+            gmeta[s] = m;
         }
-        if (lane == 0) gmeta[s] = make_int2(unit0, n);
-        // every lane copies 16-byte chunks of each block of the group (LDGSTS, L1 bypass)
-        const uint32_t my_dst = stage0 + s * kStageBytes + (cum - d.bytes);
-        const unsigned long long my_src = reinterpret_cast<unsigned long long>(lv.slice) + ((unsigned long long)d.off16 << 4);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            if (i < n) {
-                const uint32_t dst = __shfl_sync(kFull, my_dst, i);
-                const unsigned long long src = __shfl_sync(kFull, my_src, i);
-                const uint32_t nbytes = __shfl_sync(kFull, d.bytes, i);
-                for (uint32_t o = 16u * lane; o < nbytes; o += 512u) cp_async_16(dst + o, src + o);
-            }
+        // every lane copies 16-byte pieces of each block of the group (LDGSTS, L1 bypass)
+        const uint32_t dst = stage0 + s * kStageBytes;
+        const unsigned long long base = reinterpret_cast<unsigned long long>(lv.slice);
+        {
+            const unsigned long long src = base + ((unsigned long long)d0.off16 << 4);
+            for (uint32_t o = 16u * lane; o < d0.bytes; o += 512u) cp_async_16(dst + o, src + o);
+        }
+        if (two) {
+            const unsigned long long src = base + ((unsigned long long)d1.off16 << 4);
+            for (uint32_t o = 16u * lane; o < d1.bytes; o += 512u) cp_async_16(dst + d0.bytes + o, src + o);
         }
         cp_async_commit();
-        pos += n;
+        pos += two ? 2 : 1;
     };
 
-
-    // per-unit state
-    uint32_t bq[8][2];
+    // per-unit state.  qa: B fragments of q (column gq = head gq of the unit's group).
+    // acc[i] = O^T tile i: rows gq / gq+8 = channels 16gq + 2i / + 1, columns 2qq, 2qq+1 = heads.
+    uint32_t qa[8][2];
     float acc[8][4];
-    float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+    // heads hA = 2qq, hB = 2qq+1: running max (log2 units) and this lane's share of the sum
+    float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
     int cur_unit = -1;
 
     auto flush = [&]() {
@@ -335,163 +312,203 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         const int a = s_cum[u], b = s_cum[u + 1];
 #pragma unroll
         for (int o = 4; o < 32; o <<= 1) {
-            l0 += __shfl_xor_sync(kFull, l0, o);
-            l1 += __shfl_xor_sync(kFull, l1, o);
+            lA += __shfl_xor_sync(kFull, lA, o);
+            lB += __shfl_xor_sync(kFull, lB, o);
         }
         const int G = g.group;
-        const int h0 = 2 * qq, h1 = 2 * qq + 1;
+        const int hA = 2 * qq, hB = 2 * qq + 1;
         if (lo <= a && b <= hi) {  // the whole unit was processed by this warp: final result
             const int bi = u / g.n_kv_heads, hk = u % g.n_kv_heads;
             const size_t row = (size_t)bi * g.n_q_heads + (size_t)hk * G;
-            const float i0 = l0 > 0.f ? 1.f / l0 : 0.f, i1 = l1 > 0.f ? 1.f / l1 : 0.f;
+            const float iA = lA > 0.f ? 1.f / lA : 0.f, iB = lB > 0.f ? 1.f / lB : 0.f;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                const int ch = 16 * i + gq;
-                if (h0 < G) { out[(row + h0) * kD + ch] = acc[i][0] * i0; out[(row + h0) * kD + ch + 8] = acc[i][2] * i0; }
-                if (h1 < G) { out[(row + h1) * kD + ch] = acc[i][1] * i1; out[(row + h1) * kD + ch + 8] = acc[i][3] * i1; }
+                const int ch = 16 * gq + 2 * i;
+                if (hA < G) *reinterpret_cast<float2*>(out + (row + hA) * kD + ch) = make_float2(acc[i][0] * iA, acc[i][2] * iA);
+                if (hB < G) *reinterpret_cast<float2*>(out + (row + hB) * kD + ch) = make_float2(acc[i][1] * iB, acc[i][3] * iB);
             }
             if (lse != nullptr && gq == 0) {
-                if (h0 < G) lse[row + h0] = l0 > 0.f ? (m0 + log2f(l0)) * kLn2 : -INFINITY;
-                if (h1 < G) lse[row + h1] = l1 > 0.f ? (m1 + log2f(l1)) * kLn2 : -INFINITY;
+                if (hA < G) lse[row + hA] = lA > 0.f ? (mA + log2f(lA)) * kLn2 : -INFINITY;
+                if (hB < G) lse[row + hB] = lB > 0.f ? (mB + log2f(lB)) * kLn2 : -INFINITY;
             }
         } else {
             const size_t slot = (size_t)gw * 2 + (a < lo ? 0 : 1);
             float* po = part_o + slot * (size_t)(G * kD);
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                const int ch = 16 * i + gq;
-                if (h0 < G) { po[h0 * kD + ch] = acc[i][0]; po[h0 * kD + ch + 8] = acc[i][2]; }
-                if (h1 < G) { po[h1 * kD + ch] = acc[i][1]; po[h1 * kD + ch + 8] = acc[i][3]; }
+                const int ch = 16 * gq + 2 * i;
+                if (hA < G) *reinterpret_cast<float2*>(po + hA * kD + ch) = make_float2(acc[i][0], acc[i][2]);
+                if (hB < G) *reinterpret_cast<float2*>(po + hB * kD + ch) = make_float2(acc[i][1], acc[i][3]);
             }
             if (gq == 0) {
                 float* pm = part_ml + slot * (size_t)(2 * kMaxGroup);
-                if (h0 < G) { pm[2 * h0] = m0; pm[2 * h0 + 1] = l0; }
-                if (h1 < G) { pm[2 * h1] = m1; pm[2 * h1 + 1] = l1; }
+                if (hA < G) { pm[2 * hA] = mA; pm[2 * hA + 1] = lA; }
+                if (hB < G) { pm[2 * hB] = mB; pm[2 * hB + 1] = lB; }
             }
         }
     };
 
-    const uint32_t my_row = tile + (uint32_t)lane * kTileStride;
-    const int mi = lane >> 3, mr = lane & 7;
-    // ldmatrix lane addresses: QK (A = K tile rows) and PV (A = V tile transposed)
-    const uint32_t a_qk = tile + (uint32_t)(((mi & 1) * 8 + mr) * kTileStride + (mi >> 1) * 16);
-    const uint32_t a_pv = tile + (uint32_t)(((mi >> 1) * 8 + mr) * kTileStride + (mi & 1) * 16);
-
     // One call site each for issue() and flush() (code size): iterations k < 0 only fill the pipeline.
-    uint32_t ph[2][2], pl[2][2];  // P = hi + lo in bf16, [k-step of 16 tokens][b0 / b1]
 #pragma unroll 1
     for (int k = -NSTAGE;; ++k) {
         const int s = (k + NSTAGE) % NSTAGE;
-        const bool active = k >= 0;
-        float S[2][4];
-        int nbj[4];
-        if (active) {
-        __syncwarp();
-        const int2 meta = gmeta[s];
-        const int n = meta.y;
-        if (meta.x != cur_unit) {
-            if (cur_unit >= 0) flush();
-            if (n == 0) break;
-            cur_unit = meta.x;
-            const int bi = cur_unit / g.n_kv_heads, hk = cur_unit % g.n_kv_heads;
-            const uint32_t* qrow = reinterpret_cast<const uint32_t*>(
-                q + ((size_t)bi * g.n_q_heads + (size_t)hk * g.group + gq) * kD);
+        if (k >= 0) {
+            __syncwarp();
+            const GMeta meta = gmeta[s];
+            const int n = meta.n;
+            if (meta.unit != cur_unit) {
+                if (cur_unit >= 0) flush();
+                if (n == 0) break;
+                cur_unit = meta.unit;
+                const int bi = cur_unit / g.n_kv_heads, hk = cur_unit % g.n_kv_heads;
+                // q[head gq][32qq .. 32qq+31]: k-step ks uses channels 32qq + 4ks .. + 3
+                const uint4* qrow = reinterpret_cast<const uint4*>(
+                    q + ((size_t)bi * g.n_q_heads + (size_t)hk * g.group + gq) * kD + 32 * qq);
 #pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
-                bq[ks][0] = gq < g.group ? __ldg(qrow + ks * 8 + qq) : 0u;
-                bq[ks][1] = gq < g.group ? __ldg(qrow + ks * 8 + 4 + qq) : 0u;
+                for (int h = 0; h < 4; ++h) {
+                    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                    if (gq < g.group) v = __ldg(qrow + h);
+                    qa[2 * h][0] = v.x; qa[2 * h][1] = v.y; qa[2 * h + 1][0] = v.z; qa[2 * h + 1][1] = v.w;
+                }
+#pragma unroll
+                for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
+                mA = mB = -INFINITY;
+                lA = lB = 0.f;
             }
-#pragma unroll
-            for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
-            m0 = m1 = -INFINITY;
-            l0 = l1 = 0.f;
-        }
-        const GInfo gi = ginfo[s * 4 + mi];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) nbj[j] = j < n ? (int)ginfo[s * 4 + j].nb : 0;
-        const bool valid = mi < n && mr < (int)gi.nb;
-        const uint32_t bmk = gi.r_k == kD ? 0u : (uint32_t)kBitmapBytes, bmv = gi.r_v == kD ? 0u : (uint32_t)kBitmapBytes;
-        const uint32_t sp = stage0 + s * kStageBytes + gi.off;
-        const uint32_t k_bm = sp + mr * bmk;
-        const uint32_t k_val = sp + gi.nb * bmk + mr * gi.r_k * 2;
-        const uint32_t v_bm0 = sp + gi.nb * (bmk + 2 * gi.r_k);
-        const uint32_t v_bm = v_bm0 + mr * bmv;
-        const uint32_t v_val = v_bm0 + gi.nb * bmv + mr * gi.r_v * 2;
+            const int r_k = (int)(meta.rknb & 255u), r_v = (int)((meta.rknb >> 8) & 255u);
+            const int nb0 = (int)((meta.rknb >> 16) & 255u), nb1 = (int)(meta.rknb >> 24);
+            const uint32_t sp0 = stage0 + s * kStageBytes, sp1 = sp0 + meta.off1;
+            const bool full = nb0 == kB && (n == 1 || nb1 == kB);
 
-        cp_async_wait<NSTAGE - 1>();  // this lane's copies of group k have landed ...
-        __syncwarp();                 // ... and so have every other lane's
+            cp_async_wait<NSTAGE - 1>();  // this lane's copies of group k have landed ...
+            __syncwarp();                 // ... and so have every other lane's
 
-        // ---- K: expand, S = K q^T on the tensor cores (tokens = M, heads = N)
-        expand_row(my_row, k_bm, k_val, (int)gi.r_k, valid);
-        __syncwarp();
+            // ---- QK: S (tokens x heads); rows 0-7 = block 0, rows 8-15 = block 1
+            float S[4] = {0.f, 0.f, 0.f, 0.f};
+            if (r_k == kD && full) {
+                const uint32_t a0 = sp0 + 256 * gq + 64 * qq, a1 = sp1 + 256 * gq + 64 * qq;
 #pragma unroll
-        for (int mt = 0; mt < 2; ++mt) {
-            S[mt][0] = S[mt][1] = S[mt][2] = S[mt][3] = 0.f;
-#pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
+                for (int h = 0; h < 4; ++h) {
+                    const uint4 x = lds_128(a0 + 16 * h);
+                    uint4 y = make_uint4(0u, 0u, 0u, 0u);
+                    if (n == 2) y = lds_128(a1 + 16 * h);
+                    mma_bf16(S, x.x, y.x, x.y, y.y, qa[2 * h][0], qa[2 * h][1]);
+                    mma_bf16(S, x.z, y.z, x.w, y.w, qa[2 * h + 1][0], qa[2 * h + 1][1]);
+                }
+            } else {
+                // run of (token gq, word qq): starts after the kept elements of the lower words
+                uint32_t w0 = 0u, w1 = 0u, p0, p1;
+                if (r_k == kD) {  // ragged dense block: all slots kept, no bitmap stored
+                    w0 = gq < nb0 ? 0xffffffffu : 0u;
+                    w1 = (n == 2 && gq < nb1) ? 0xffffffffu : 0u;
+                    p0 = sp0 + 256 * gq + 64 * qq;
+                    p1 = sp1 + 256 * gq + 64 * qq;
+                } else {
+                    if (gq < nb0) w0 = lds_u32(sp0 + 4 * lane);
+                    if (n == 2 && gq < nb1) w1 = lds_u32(sp1 + 4 * lane);
+                    uint32_t cnt = (uint32_t)__popc(w0) | ((uint32_t)__popc(w1) << 16), inc = cnt, t;
+                    t = __shfl_up_sync(kFull, inc, 1); if (qq >= 1) inc += t;
+                    t = __shfl_up_sync(kFull, inc, 2); if (qq >= 2) inc += t;
+                    const uint32_t ex = inc - cnt;
+                    p0 = sp0 + 16 * nb0 + 2 * (r_k * gq + (ex & 0xffffu));
+                    p1 = sp1 + 16 * nb1 + 2 * (r_k * gq + (ex >> 16));
+                }
                 uint32_t a[4];
-                ldmatrix_x4(a_qk + mt * 16 * kTileStride + ks * 32, a);
-                mma_bf16(S[mt], a, bq[ks][0], bq[ks][1]);
+#define MKV_KSTEP(KS)                  \
+    k_step<KS>(w0, w1, p0, p1, a);     \
+    mma_bf16(S, a[0], a[1], a[2], a[3], qa[KS][0], qa[KS][1]);
+                MKV_KSTEP(0) MKV_KSTEP(1) MKV_KSTEP(2) MKV_KSTEP(3)
+                MKV_KSTEP(4) MKV_KSTEP(5) MKV_KSTEP(6) MKV_KSTEP(7)
+#undef MKV_KSTEP
             }
+
+            // ---- online softmax in the exp2 domain; this lane: token gq of each block, heads 2qq, 2qq+1
+            const bool v0 = gq < nb0, v1 = n == 2 && gq < nb1;
+            const float sA0 = v0 ? S[0] * scale_log2 : -INFINITY, sB0 = v0 ? S[1] * scale_log2 : -INFINITY;
+            const float sA1 = v1 ? S[2] * scale_log2 : -INFINITY, sB1 = v1 ? S[3] * scale_log2 : -INFINITY;
+            float mxA = fmaxf(sA0, sA1), mxB = fmaxf(sB0, sB1);
+#pragma unroll
+            for (int o = 4; o < 32; o <<= 1) {
+                mxA = fmaxf(mxA, __shfl_xor_sync(kFull, mxA, o));
+                mxB = fmaxf(mxB, __shfl_xor_sync(kFull, mxB, o));
+            }
+            const float mnA = fmaxf(mA, mxA), mnB = fmaxf(mB, mxB);
+            const float bA = mnA == -INFINITY ? 0.f : mnA, bB = mnB == -INFINITY ? 0.f : mnB;
+            const float cA = ex2(mA - bA), cB = ex2(mB - bB);
+            if (__any_sync(kFull, mnA != mA || mnB != mB)) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) { acc[i][0] *= cA; acc[i][1] *= cB; acc[i][2] *= cA; acc[i][3] *= cB; }
+            }
+            mA = mnA; mB = mnB;
+            const float eA0 = ex2(sA0 - bA), eB0 = ex2(sB0 - bB), eA1 = ex2(sA1 - bA), eB1 = ex2(sB1 - bB);
+            lA = lA * cA + (eA0 + eA1);
+            lB = lB * cB + (eB0 + eB1);
+            // P split into bf16 hi + lo, transposed into the B fragment layout of PV (k = token, n = head)
+            const uint32_t h0 = pack_bf16(eA0, eB0), h1 = pack_bf16(eA1, eB1);
+            const uint32_t l0 = pack_bf16(eA0 - __uint_as_float(h0 << 16), eB0 - __uint_as_float(h0 & 0xffff0000u));
+            const uint32_t l1 = pack_bf16(eA1 - __uint_as_float(h1 << 16), eB1 - __uint_as_float(h1 & 0xffff0000u));
+            const uint32_t ph0 = movmatrix_trans(h0), ph1 = movmatrix_trans(h1);
+            const uint32_t pl0 = movmatrix_trans(l0), pl1 = movmatrix_trans(l1);
+
+            // ---- PV: O^T += V^T P^T (channels x heads), K = the group's 16 tokens
+            const uint32_t bmv = r_v == kD ? 0u : (uint32_t)kBitmapBytes;
+            const uint32_t bmk = r_k == kD ? 0u : (uint32_t)kBitmapBytes;
+            const uint32_t vb0 = sp0 + nb0 * (bmk + 2 * r_k), vb1 = sp1 + nb1 * (bmk + 2 * r_k);  // V part of each block
+            if (r_v == kD && full) {
+                const uint32_t rA0 = vb0 + 256 * (2 * qq) + 32 * gq, rA1 = vb1 + 256 * (2 * qq) + 32 * gq;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {  // 16-byte chunk h = channel slots 8h .. 8h+7 = tiles 4h .. 4h+3
+                    const uint4 xa = lds_128(rA0 + 16 * h), xb = lds_128(rA0 + 256 + 16 * h);
+                    uint4 ya = make_uint4(0u, 0u, 0u, 0u), yb = ya;
+                    if (n == 2) { ya = lds_128(rA1 + 16 * h); yb = lds_128(rA1 + 256 + 16 * h); }
+                    const uint32_t xav[4] = {xa.x, xa.y, xa.z, xa.w}, xbv[4] = {xb.x, xb.y, xb.z, xb.w};
+                    const uint32_t yav[4] = {ya.x, ya.y, ya.z, ya.w}, ybv[4] = {yb.x, yb.y, yb.z, yb.w};
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const uint32_t a0 = prmt(xav[j], xbv[j], 0x5410u), a1 = prmt(xav[j], xbv[j], 0x7632u);
+                        const uint32_t a2 = prmt(yav[j], ybv[j], 0x5410u), a3 = prmt(yav[j], ybv[j], 0x7632u);
+                        mma_bf16(acc[4 * h + j], a0, a1, a2, a3, ph0, ph1);
+                        mma_bf16(acc[4 * h + j], a0, a1, a2, a3, pl0, pl1);
+                    }
+                }
+            } else {
+                const int tA = 2 * qq, tB = 2 * qq + 1;
+                uint32_t hA0 = 0u, hB0 = 0u, hA1 = 0u, hB1 = 0u, pA0, pB0, pA1, pB1;
+                if (r_v == kD) {  // ragged dense block
+                    hA0 = tA < nb0 ? 0xffffu : 0u; hB0 = tB < nb0 ? 0xffffu : 0u;
+                    hA1 = (n == 2 && tA < nb1) ? 0xffffu : 0u; hB1 = (n == 2 && tB < nb1) ? 0xffffu : 0u;
+                    pA0 = vb0 + 256 * tA + 32 * gq; pB0 = pA0 + 256;
+                    pA1 = vb1 + 256 * tA + 32 * gq; pB1 = pA1 + 256;
+                } else {
+                    if (tA < nb0) hA0 = lds_u16(vb0 + 16 * tA + 2 * gq);
+                    if (tB < nb0) hB0 = lds_u16(vb0 + 16 * tB + 2 * gq);
+                    if (n == 2 && tA < nb1) hA1 = lds_u16(vb1 + 16 * tA + 2 * gq);
+                    if (n == 2 && tB < nb1) hB1 = lds_u16(vb1 + 16 * tB + 2 * gq);
+                    // exclusive prefix over the lower half-words (lanes gq' < gq, stride 4); four byte counters
+                    const uint32_t cnt = (uint32_t)__popc(hA0) | ((uint32_t)__popc(hB0) << 8) |
+                                         ((uint32_t)__popc(hA1) << 16) | ((uint32_t)__popc(hB1) << 24);
+                    uint32_t inc = cnt, t;
+                    t = __shfl_up_sync(kFull, inc, 4); if (gq >= 1) inc += t;
+                    t = __shfl_up_sync(kFull, inc, 8); if (gq >= 2) inc += t;
+                    t = __shfl_up_sync(kFull, inc, 16); if (gq >= 4) inc += t;
+                    const uint32_t ex = inc - cnt;
+                    pA0 = vb0 + 16 * nb0 + 2 * (r_v * tA + (ex & 255u));
+                    pB0 = vb0 + 16 * nb0 + 2 * (r_v * tB + ((ex >> 8) & 255u));
+                    pA1 = vb1 + 16 * nb1 + 2 * (r_v * tA + ((ex >> 16) & 255u));
+                    pB1 = vb1 + 16 * nb1 + 2 * (r_v * tB + (ex >> 24));
+                }
+                uint32_t a[4];
+#define MKV_VSTEP(I)                                         \
+    v_step<I>(hA0, hB0, hA1, hB1, pA0, pB0, pA1, pB1, a);    \
+    mma_bf16(acc[I], a[0], a[1], a[2], a[3], ph0, ph1);      \
+    mma_bf16(acc[I], a[0], a[1], a[2], a[3], pl0, pl1);
+                MKV_VSTEP(0) MKV_VSTEP(1) MKV_VSTEP(2) MKV_VSTEP(3)
+                MKV_VSTEP(4) MKV_VSTEP(5) MKV_VSTEP(6) MKV_VSTEP(7)
+#undef MKV_VSTEP
+            }
+            __syncwarp();  // every lane is done reading stage s
         }
-        __syncwarp();  // every lane's ldmatrix reads are done: the tile may be overwritten
-        // ---- V: expand into the same tile (overlaps the softmax arithmetic below)
-        expand_row(my_row, v_bm, v_val, (int)gi.r_v, valid);
-        __syncwarp();
-        }  // active
         issue(s);  // stage s is free: start the copies of group k + NSTAGE
-        if (!active) continue;
-
-        // ---- online softmax in the exp2 domain; this lane: tokens 8j + gq (j = 0..3), heads 2qq, 2qq+1
-        float mx0 = -INFINITY, mx1 = -INFINITY;
-#pragma unroll
-        for (int mt = 0; mt < 2; ++mt) {
-#pragma unroll
-            for (int hf = 0; hf < 2; ++hf) {
-                const bool tv = gq < nbj[mt * 2 + hf];
-                S[mt][2 * hf] = tv ? S[mt][2 * hf] * scale_log2 : -INFINITY;
-                S[mt][2 * hf + 1] = tv ? S[mt][2 * hf + 1] * scale_log2 : -INFINITY;
-                mx0 = fmaxf(mx0, S[mt][2 * hf]);
-                mx1 = fmaxf(mx1, S[mt][2 * hf + 1]);
-            }
-        }
-#pragma unroll
-        for (int o = 4; o < 32; o <<= 1) {
-            mx0 = fmaxf(mx0, __shfl_xor_sync(kFull, mx0, o));
-            mx1 = fmaxf(mx1, __shfl_xor_sync(kFull, mx1, o));
-        }
-        const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
-        const float b0 = mn0 == -INFINITY ? 0.f : mn0, b1 = mn1 == -INFINITY ? 0.f : mn1;
-        const float c0 = ex2(m0 - b0), c1 = ex2(m1 - b1);
-        if (__any_sync(kFull, mn0 != m0 || mn1 != m1)) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) { acc[i][0] *= c0; acc[i][1] *= c1; acc[i][2] *= c0; acc[i][3] *= c1; }
-        }
-        m0 = mn0; m1 = mn1;
-        l0 *= c0; l1 *= c1;
-#pragma unroll
-        for (int mt = 0; mt < 2; ++mt) {
-#pragma unroll
-            for (int hf = 0; hf < 2; ++hf) {
-                const float p0 = ex2(S[mt][2 * hf] - b0), p1 = ex2(S[mt][2 * hf + 1] - b1);
-                l0 += p0; l1 += p1;
-                const uint32_t h = pack_bf16(p0, p1);
-                const uint32_t lw = pack_bf16(p0 - __uint_as_float(h << 16), p1 - __uint_as_float(h & 0xffff0000u));
-                ph[mt][hf] = movmatrix_trans(h);
-                pl[mt][hf] = movmatrix_trans(lw);
-            }
-        }
-        // ---- O^T += V^T P  (channels = M, heads = N, tokens = K)
-#pragma unroll
-        for (int kt = 0; kt < 2; ++kt) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                uint32_t a[4];
-                ldmatrix_x4_trans(a_pv + kt * 16 * kTileStride + i * 32, a);
-                mma_bf16(acc[i], a, ph[kt][0], ph[kt][1]);
-                mma_bf16(acc[i], a, pl[kt][0], pl[kt][1]);
-            }
-        }
     }
 }
 
@@ -612,13 +629,13 @@ cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint
     static int cfg = -1;  // tuning knob (stages * 100 + warps); default chosen from measurements
     if (cfg < 0) {
         const char* e = getenv("MKV_ATTN_CFG");
-        cfg = e ? atoi(e) : 210;
+        cfg = e ? atoi(e) : 316;
     }
 #define MKV_CFG(S, W) \
     case S * 100 + W: return launch_attention_cfg<S, W>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, sm_count, s);
     switch (cfg) {
-        MKV_CFG(1, 12) MKV_CFG(1, 14) MKV_CFG(2, 8) MKV_CFG(2, 10) MKV_CFG(3, 8) MKV_CFG(2, 4) MKV_CFG(2, 6)
-        default: return launch_attention_cfg<2, 10>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, sm_count, s);
+        MKV_CFG(3, 16) MKV_CFG(2, 16) MKV_CFG(4, 12) MKV_CFG(3, 12) MKV_CFG(4, 8) MKV_CFG(6, 8)
+        default: return launch_attention_cfg<3, 16>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, sm_count, s);
     }
 #undef MKV_CFG
 }
