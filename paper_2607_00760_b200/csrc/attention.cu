@@ -20,13 +20,23 @@
 //     P is split into bf16 hi + lo (fp32-class accuracy) and transposed into the B fragment
 //     layout with movmatrix.  Dense vectors (r = D) skip the walk: their fragments are 16-byte
 //     shared loads.
-//   * A unit wholly inside one warp's range is normalised and written directly; otherwise the
-//     warp writes an (m, l, O) partial (<= 2 per warp) that the combine kernel merges (step 3d).
+//   * Step 3d (split-K combine) is fused: a unit wholly inside one warp's range is normalised and
+//     written directly; otherwise the warp leaves an (m, l, O) partial (<= 2 per warp), the CTA
+//     merges its warps' partials with the LSE rule, and a unit that spans several CTAs is finished
+//     by the last CTA to arrive at a per-unit ticket (no second kernel).
 #include <cstdlib>
 
 #include "mkv_internal.cuh"
 
 namespace mkv {
+
+#ifdef MKV_DBG_TIMING
+__device__ unsigned long long g_dbg_t[160 * 8];
+__device__ __forceinline__ unsigned long long dbg_now() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define MKV_T(k) do { if (threadIdx.x == 0) g_dbg_t[blockIdx.x * 8 + (k)] = dbg_now(); } while (0)
+#else
+#define MKV_T(k) do {} while (0)
+#endif
 
 namespace {
 
@@ -49,6 +59,12 @@ struct __align__(16) GMeta {  // one in-flight group (<= 2 blocks of one unit wi
     int32_t unit, n;          // n = 0: end of the range
     uint32_t off1;            // stage offset of the second block
     uint32_t rknb;            // r_k | r_v << 8 | nb0 << 16 | nb1 << 24
+};
+
+struct PartRec {  // an (m, l, O) partial of one warp: shared memory (usual) or global scratch
+    int unit;
+    const float* o;   // [G][D] unnormalised
+    const float* ml;  // [8][2] (max in log2 units, sum)
 };
 
 // ---- PTX wrappers ---------------------------------------------------------------------------
@@ -201,6 +217,16 @@ __device__ __forceinline__ int find_unit(const int* s_cum, int n_units, int i) {
     return lo;
 }
 
+// floor(p / d) for p < 2^56 without the 64-bit division subroutine: fp32 estimate, exact fix-up
+__device__ __forceinline__ unsigned div_floor(unsigned long long p, unsigned d, float inv_d) {
+    unsigned q = (unsigned)fminf((float)p * inv_d, 4.0e9f);
+#pragma unroll 1
+    while ((unsigned long long)q * d > p) --q;
+#pragma unroll 1
+    while ((unsigned long long)(q + 1) * d <= p) ++q;
+    return q;
+}
+
 __host__ __device__ constexpr int warp_smem_bytes(int nstage) {
     return nstage * kStageBytes + kDescRing * 16 + nstage * 16;
 }
@@ -214,19 +240,45 @@ __global__ void __launch_bounds__(kWarps * 32, 1)
 mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q,
                             const int32_t* __restrict__ sel, const int32_t* __restrict__ sel_count, int k_max,
                             float scale_log2, float* __restrict__ out, float* __restrict__ lse,
-                            float* __restrict__ part_o, float* __restrict__ part_ml) {
+                            float* __restrict__ part_o, float* __restrict__ part_ml, int32_t* __restrict__ ticket) {
     extern __shared__ __align__(128) uint8_t smem[];
     constexpr int kWS = warp_smem_bytes(NSTAGE);
     int* s_cum = reinterpret_cast<int*>(smem + kWarps * kWS);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int gq = lane >> 2, qq = lane & 3;  // mma fragment coordinates (groupID, threadID_in_group)
 
+    MKV_T(0);
+    __shared__ PartRec s_rec[kWarps * 2];
+    __shared__ int s_last[2];
+    __shared__ float s_w[32 * kMaxGroup], s_M[kMaxGroup], s_L[kMaxGroup];
+    __shared__ const float* s_po[32];
+    __shared__ int s_n;
+    __shared__ int s_clo, s_chi, s_cf[2], s_cl[2];
+    __shared__ size_t s_row[2];
     const int T = scan_counts(sel_count, g.n_units, k_max, s_cum);
-    const int GW = gridDim.x * kWarps, gw = blockIdx.x * kWarps + warp;
-    const int lo = (int)((unsigned long long)gw * (unsigned)T / (unsigned)GW);
-    const int hi = (int)((unsigned long long)(gw + 1) * (unsigned)T / (unsigned)GW);
-    if (lo >= hi) return;
+    // Gd CTAs share the T blocks (every one of them owns >= 1 block); CTA c owns [c T / Gd, (c+1) T / Gd),
+    // cut evenly again over its warps: warp gw of GW owns [gw T / GW, (gw+1) T / GW)
+    const unsigned Gd = min(gridDim.x, (unsigned)max(T, 1));
+    const unsigned GW = Gd * kWarps, gw = blockIdx.x * kWarps + warp;
+    const float inv_GW = 1.f / (float)GW;
+    int lo = 0, hi = 0;
+    if (blockIdx.x < Gd) {
+        lo = (int)div_floor((unsigned long long)gw * (unsigned)T, GW, inv_GW);
+        hi = (int)div_floor((unsigned long long)(gw + 1) * (unsigned)T, GW, inv_GW);
+    }
+    if (lane == 0 && warp == 0) s_clo = lo;
+    if (lane == 0 && warp == kWarps - 1) s_chi = hi;
     const int n_total = hi - lo;
+    const int G = g.group;
+    if (lane < 2) s_rec[warp * 2 + lane].unit = -1;
+    if (blockIdx.x == 0) {  // units with an empty selection: out = 0, lse = -inf
+        for (int u = warp; u < g.n_units; u += kWarps) {
+            if (s_cum[u + 1] != s_cum[u]) continue;
+            const size_t row = (size_t)(u / g.n_kv_heads) * g.n_q_heads + (size_t)(u % g.n_kv_heads) * G;
+            for (int e = lane; e < G * kD; e += 32) out[row * kD + e] = 0.f;
+            if (lse != nullptr && lane < G) lse[row + lane] = -INFINITY;
+        }
+    }
 
     uint8_t* wbase = smem + warp * kWS;
     const uint32_t stage0 = smem_u32(wbase);
@@ -307,7 +359,10 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
     int cur_unit = -1;
 
-    auto flush = [&]() {
+    // end of a unit inside this warp's range.  `last` = the call after the main loop: the stages are
+    // idle, so the partial may live in this warp's own shared memory.
+    int n_rec = 0;
+    auto flush = [&](bool last) {
         const int u = cur_unit;
         const int a = s_cum[u], b = s_cum[u + 1];
 #pragma unroll
@@ -315,7 +370,6 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             lA += __shfl_xor_sync(kFull, lA, o);
             lB += __shfl_xor_sync(kFull, lB, o);
         }
-        const int G = g.group;
         const int hA = 2 * qq, hB = 2 * qq + 1;
         if (lo <= a && b <= hi) {  // the whole unit was processed by this warp: final result
             const int bi = u / g.n_kv_heads, hk = u % g.n_kv_heads;
@@ -332,8 +386,16 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 if (hB < G) lse[row + hB] = lB > 0.f ? (mB + log2f(lB)) * kLn2 : -INFINITY;
             }
         } else {
-            const size_t slot = (size_t)gw * 2 + (a < lo ? 0 : 1);
-            float* po = part_o + slot * (size_t)(G * kD);
+            float* po;
+            float* pm;
+            if (last) {
+                po = reinterpret_cast<float*>(wbase);
+                pm = po + kMaxGroup * kD;
+            } else {  // rare: a unit boundary inside the range while copies are in flight
+                const size_t slot = (size_t)gw * 2 + n_rec;
+                po = part_o + slot * (size_t)(G * kD);
+                pm = part_ml + slot * (size_t)(2 * kMaxGroup);
+            }
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
                 const int ch = 16 * gq + 2 * i;
@@ -341,24 +403,29 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 if (hB < G) *reinterpret_cast<float2*>(po + hB * kD + ch) = make_float2(acc[i][1], acc[i][3]);
             }
             if (gq == 0) {
-                float* pm = part_ml + slot * (size_t)(2 * kMaxGroup);
                 if (hA < G) { pm[2 * hA] = mA; pm[2 * hA + 1] = lA; }
                 if (hB < G) { pm[2 * hB] = mB; pm[2 * hB + 1] = lB; }
             }
+            if (lane == 0) {
+                PartRec r;
+                r.unit = u; r.o = po; r.ml = pm;
+                s_rec[warp * 2 + n_rec] = r;
+            }
+            ++n_rec;
         }
     };
 
     // One call site each for issue() and flush() (code size): iterations k < 0 only fill the pipeline.
 #pragma unroll 1
-    for (int k = -NSTAGE;; ++k) {
+    for (int k = -NSTAGE; n_total > 0; ++k) {
         const int s = (k + NSTAGE) % NSTAGE;
         if (k >= 0) {
             __syncwarp();
             const GMeta meta = gmeta[s];
             const int n = meta.n;
             if (meta.unit != cur_unit) {
-                if (cur_unit >= 0) flush();
                 if (n == 0) break;
+                if (cur_unit >= 0) flush(false);
                 cur_unit = meta.unit;
                 const int bi = cur_unit / g.n_kv_heads, hk = cur_unit % g.n_kv_heads;
                 // q[head gq][32qq .. 32qq+31]: k-step ks uses channels 32qq + 4ks .. + 3
@@ -451,7 +518,6 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             const uint32_t pl0 = movmatrix_trans(l0), pl1 = movmatrix_trans(l1);
 
             // ---- PV: O^T += V^T P^T (channels x heads), K = the group's 16 tokens
-            const uint32_t bmv = r_v == kD ? 0u : (uint32_t)kBitmapBytes;
             const uint32_t bmk = r_k == kD ? 0u : (uint32_t)kBitmapBytes;
             const uint32_t vb0 = sp0 + nb0 * (bmk + 2 * r_k), vb1 = sp1 + nb1 * (bmk + 2 * r_k);  // V part of each block
             if (r_v == kD && full) {
@@ -510,95 +576,176 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         }
         issue(s);  // stage s is free: start the copies of group k + NSTAGE
     }
-}
+#ifdef MKV_DBG_TIMING
+    if (lane == 0) { atomicMin(&g_dbg_t[blockIdx.x * 8 + 5], dbg_now()); atomicMax(&g_dbg_t[blockIdx.x * 8 + 6], dbg_now()); }
+#endif
+    if (cur_unit >= 0) {
+        cp_async_wait<0>();  // only empty groups are pending; the stages are free
+        __syncwarp();
+        flush(true);
+    }
 
-// ------------------------------------------------------------------------------------------
-// step 3d: merge the partials of every unit that was shared between warps; units with an empty
-// selection get out = 0, lse = -inf; units finished by a single warp are already written.
-// grid = (n_units, G), block = 128 (thread = channel).  GW = warps of the main kernel's grid.
-// ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) mkv_combine_kernel(CacheGeom g, const int32_t* __restrict__ sel_count, int k_max,
-                                                          int GW, const float* __restrict__ part_o,
-                                                          const float* __restrict__ part_ml, float* __restrict__ out,
-                                                          float* __restrict__ lse) {
-    const int u = blockIdx.x, gi = blockIdx.y, c = threadIdx.x;
-    __shared__ int s_a[4], s_t[4];
-    int before = 0, total = 0;
-    for (int i = c; i < g.n_units; i += 128) {
-        const int v = min(max(sel_count[i], 0), k_max);
-        total += v;
-        if (i < u) before += v;
-    }
-#pragma unroll
-    for (int o = 16; o; o >>= 1) {
-        before += __shfl_xor_sync(kFull, before, o);
-        total += __shfl_xor_sync(kFull, total, o);
-    }
-    if ((c & 31) == 0) { s_a[c >> 5] = before; s_t[c >> 5] = total; }
-    __syncthreads();
-    const int a = s_a[0] + s_a[1] + s_a[2] + s_a[3];
-    const long long T = (long long)s_t[0] + s_t[1] + s_t[2] + s_t[3];
-    const int b = a + min(max(sel_count[u], 0), k_max);
-    const int G = g.group;
-    const int bi = u / g.n_kv_heads, hk = u % g.n_kv_heads;
-    const size_t row = (size_t)bi * g.n_q_heads + (size_t)hk * G + gi;
-    if (b == a) {
-        out[row * kD + c] = 0.f;
-        if (lse != nullptr && c == 0) lse[row] = -INFINITY;
-        return;
-    }
-    auto lo_of = [&](long long w) { return (int)(w * T / GW); };
-    long long first = (long long)a * GW / T;
-    while (lo_of(first + 1) <= a) ++first;      // first warp whose range reaches past a
-    long long last = (long long)(b - 1) * GW / T;
-    while (last + 1 < GW && lo_of(last + 1) < b) ++last;
-    while (lo_of(last) >= b) --last;
-    if (first == last) return;  // one warp saw the whole unit and wrote the result itself
-    __shared__ int s_slot[128];
-    __shared__ float s_m[128], s_l[128];
-    float M = -INFINITY, L = 0.f, O = 0.f;
-    for (long long w0 = first; w0 <= last; w0 += 128) {
-        __syncthreads();
-        const long long w = w0 + c;
-        int slot = -1;
-        if (w <= last) {
-            const int wl = lo_of(w), wh = lo_of(w + 1);
-            if (wl < wh) slot = (int)(w * 2 + (a < wl ? 0 : 1));
-        }
-        s_slot[c] = slot;
-        s_m[c] = slot >= 0 ? part_ml[(size_t)slot * (2 * kMaxGroup) + 2 * gi] : -INFINITY;
-        s_l[c] = slot >= 0 ? part_ml[(size_t)slot * (2 * kMaxGroup) + 2 * gi + 1] : 0.f;
-        __syncthreads();
-        const int cnt = (int)min((long long)128, last - w0 + 1);
-        float mx = M;
-        for (int i = 0; i < cnt; ++i) mx = fmaxf(mx, s_m[i]);
-        const float bs = mx == -INFINITY ? 0.f : mx;
-        const float co = ex2(M - bs);
-        L *= co; O *= co; M = mx;
-        for (int i0 = 0; i0 < cnt; i0 += 8) {  // eight independent loads in flight
-            float os[8];
-#pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                const int sl = i0 + e < cnt ? s_slot[i0 + e] : -1;
-                os[e] = sl >= 0 ? part_o[((size_t)sl * G + gi) * kD + c] : 0.f;
+    // ---- step 3d, fused: merge the warps' partials; finish units that span several CTAs
+#ifdef MKV_DBG_NO_TAIL
+    return;
+#endif
+    __syncthreads();  // orders the warps' partials (shared memory, or global scratch from flush(false))
+    MKV_T(1);
+    const int clo = s_clo, chi = s_chi;
+    const size_t cta_slot_base = (size_t)gridDim.x * kMaxWarps * 2;
+    const int tid = threadIdx.x;
+    int sh_u[2] = {-1, -1};  // units this CTA shares with others (<= 2: one entering, one leaving its range)
+    int n_shared = 0;
+#pragma unroll 1
+    for (int i = 0; i < kWarps * 2;) {
+        const int u = s_rec[i].unit;
+        if (u < 0) { ++i; continue; }
+        int j = i + 1;
+        while (j < kWarps * 2 && (s_rec[j].unit == u || s_rec[j].unit < 0)) ++j;
+        const int a = s_cum[u], b = s_cum[u + 1];
+        const bool whole = clo <= a && b <= chi;
+        const size_t row = (size_t)(u / g.n_kv_heads) * g.n_q_heads + (size_t)(u % g.n_kv_heads) * G;
+        const size_t slot = cta_slot_base + blockIdx.x * 2 + (a < clo ? 0 : 1);
+        // weights of the run's partials: warp h = head h, lane = partial record i + lane; the
+        // run's members are compacted into s_po / s_w (padded to a multiple of 4 with weight 0)
+        if (warp < G) {
+            float m = -INFINITY, l = 0.f;
+            const bool member = i + lane < j && s_rec[i + lane].unit == u;
+            const float* po = s_rec[i].o;  // record i is a member: a safe pointer for the padding
+            if (member) {
+                const float* ml = s_rec[i + lane].ml;
+                m = ml[2 * warp];
+                l = ml[2 * warp + 1];
+                po = s_rec[i + lane].o;
             }
+            float M = m;
 #pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                if (i0 + e < cnt) {
-                    const float wgt = ex2(s_m[i0 + e] - bs);
-                    L = fmaf(s_l[i0 + e], wgt, L);
-                    O = fmaf(os[e], wgt, O);
+            for (int o = 16; o; o >>= 1) M = fmaxf(M, __shfl_xor_sync(kFull, M, o));
+            const float w = ex2(m - (M == -INFINITY ? 0.f : M));
+            float L = l * w;
+#pragma unroll
+            for (int o = 16; o; o >>= 1) L += __shfl_xor_sync(kFull, L, o);
+            const unsigned mem = __ballot_sync(kFull, member);
+            const int n_mem = __popc(mem), pos = __popc(mem & ((1u << lane) - 1u));
+            if (member) s_w[pos * kMaxGroup + warp] = w;
+            else s_w[(n_mem + lane - pos) * kMaxGroup + warp] = 0.f;  // non-members pad the tail
+            if (warp == 0) {
+                if (member) s_po[pos] = po;
+                else s_po[n_mem + lane - pos] = po;
+                if (lane == 0) s_n = n_mem;
+            }
+            if (lane == 0) { s_M[warp] = M; s_L[warp] = L; }
+        }
+        __syncthreads();
+        const int n_mem4 = (s_n + 3) & ~3;
+#pragma unroll 1
+        for (int e = tid; e < G * kD; e += kWarps * 32) {
+            const int h = e >> 7;
+            float O = 0.f;
+#pragma unroll 1
+            for (int r = 0; r < n_mem4; r += 4) {
+                const float x0 = s_po[r][e], x1 = s_po[r + 1][e], x2 = s_po[r + 2][e], x3 = s_po[r + 3][e];
+                O = fmaf(x0, s_w[r * kMaxGroup + h], O);
+                O = fmaf(x1, s_w[(r + 1) * kMaxGroup + h], O);
+                O = fmaf(x2, s_w[(r + 2) * kMaxGroup + h], O);
+                O = fmaf(x3, s_w[(r + 3) * kMaxGroup + h], O);
+            }
+            const float M = s_M[h], L = s_L[h];
+            if (whole) {
+                out[row * kD + e] = L > 0.f ? O / L : 0.f;
+                if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = L > 0.f ? (M + log2f(L)) * kLn2 : -INFINITY;
+            } else {
+                part_o[slot * (G * kD) + e] = O;
+                if ((e & (kD - 1)) == 0) {
+                    part_ml[slot * (2 * kMaxGroup) + 2 * h] = M;
+                    part_ml[slot * (2 * kMaxGroup) + 2 * h + 1] = L;
                 }
             }
         }
+        if (!whole && n_shared < 2) {
+            if (tid == 0) s_row[n_shared] = row;
+            sh_u[n_shared++] = u;
+        }
+        __syncthreads();  // s_w / s_M / s_L are reused by the next run
+        i = j;
     }
-    out[row * kD + c] = L > 0.f ? O / L : 0.f;
-    if (lse != nullptr && c == 0) lse[row] = L > 0.f ? (M + log2f(L)) * kLn2 : -INFINITY;
+    MKV_T(2);
+    if (n_shared == 0) return;  // uniform over the CTA
+#ifdef MKV_DBG_NO_XCTA
+    return;
+#endif
+
+    // CTA c owns block x  <=>  c T < (x+1) Gd <= (c+1) T.  One thread per shared unit (in different
+    // warps) finds the sharers c_first .. c_last (all non-empty: T >= Gd), releases the CTA's partial
+    // and takes a ticket.  A sharer's slot is 1 for c_first (the unit starts inside it), else 0.
+    if ((tid == 0 || tid == 32) && (tid >> 5) < n_shared) {
+        const int k = tid >> 5, u = sh_u[k];
+        const float inv_T = 1.f / (float)T;
+        int cf = (int)blockIdx.x, cl = (int)blockIdx.x;
+        if (s_cum[u] < clo) cf = (int)div_floor((unsigned long long)(s_cum[u] + 1) * Gd - 1, (unsigned)T, inv_T);
+        if (s_cum[u + 1] > chi) cl = (int)div_floor((unsigned long long)s_cum[u + 1] * Gd - 1, (unsigned)T, inv_T);
+        s_cf[k] = cf; s_cl[k] = cl;
+        asm volatile("fence.acq_rel.gpu;" ::: "memory");  // the CTA's partial (ordered by the barrier) is released
+        const int old = atomicAdd(&ticket[u], 1);
+        asm volatile("fence.acq_rel.gpu;" ::: "memory");  // the other sharers' partials are acquired
+        s_last[k] = old == cl - cf;
+        if (old == cl - cf) ticket[u] = 0;  // self-cleaning: every sharer has arrived
+    }
+    __syncthreads();
+    MKV_T(3);
+#pragma unroll 1
+    for (int k = 0; k < n_shared; ++k) {
+        if (!s_last[k]) continue;  // uniform over the CTA
+        // last arriver: merge the CTA partials (read with ld.global.cg: L2, never a stale L1 line)
+        const int u = sh_u[k], c_first = s_cf[k], c_last = s_cl[k];
+        const size_t row = s_row[k];
+#pragma unroll 1
+        for (int e = tid; e < G * kD; e += kWarps * 32) {
+            const int h = e >> 7;
+            float M = -INFINITY, L = 0.f, O = 0.f;
+#pragma unroll 1
+            for (int c0 = c_first; c0 <= c_last; c0 += 4) {  // four partials' loads in flight at once
+                float pm[4], pl[4], po[4];
+#pragma unroll
+                for (int t = 0; t < 4; ++t) {
+                    const int c = c0 + t;
+                    pm[t] = -INFINITY; pl[t] = 0.f; po[t] = 0.f;
+                    if (c <= c_last) {
+                        const size_t sl = cta_slot_base + (size_t)c * 2 + (c == c_first ? 1 : 0);
+                        pm[t] = __ldcg(part_ml + sl * (2 * kMaxGroup) + 2 * h);
+                        pl[t] = __ldcg(part_ml + sl * (2 * kMaxGroup) + 2 * h + 1);
+                        po[t] = __ldcg(part_o + sl * (size_t)(G * kD) + e);
+                    }
+                }
+                const float Mn = fmaxf(fmaxf(M, fmaxf(pm[0], pm[1])), fmaxf(pm[2], pm[3]));
+                const float Mb = Mn == -INFINITY ? 0.f : Mn;
+                const float c_old = ex2(M - Mb);
+                L *= c_old; O *= c_old; M = Mn;
+#pragma unroll
+                for (int t = 0; t < 4; ++t) {
+                    const float w = ex2(pm[t] - Mb);
+                    L = fmaf(pl[t], w, L);
+                    O = fmaf(po[t], w, O);
+                }
+            }
+            out[row * kD + e] = L > 0.f ? O / L : 0.f;
+            if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = L > 0.f ? (M + log2f(L)) * kLn2 : -INFINITY;
+        }
+        (void)u;
+    }
+    MKV_T(4);
 }
 
 }  // namespace
 
-int attention_partial_slots(int sm_count) { return sm_count * kMaxWarps * 2; }
+#ifdef MKV_DBG_TIMING
+extern "C" __attribute__((visibility("default"))) int mkv_dbg_timing(unsigned long long* host, int reset) {
+    if (reset) { static unsigned long long init[160 * 8]; for (int i = 0; i < 160 * 8; ++i) init[i] = (i % 8 == 5) ? ~0ull : 0ull; return (int)cudaMemcpyToSymbol(g_dbg_t, init, sizeof(init)); }
+    return (int)cudaMemcpyFromSymbol(host, g_dbg_t, sizeof(unsigned long long) * 160 * 8);
+}
+#endif
+
+int attention_partial_slots(int sm_count) { return sm_count * kMaxWarps * 2 + sm_count * 2; }
 
 template <int NSTAGE, int NWARPS>
 static cudaError_t launch_attention_cfg(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
@@ -613,11 +760,7 @@ static cudaError_t launch_attention_cfg(const CacheGeom& g, const LayerView& lv,
         configured = smem;
     }
     mkv_packed_attention_kernel<NSTAGE, NWARPS><<<sm_count, NWARPS * 32, smem, s>>>(
-        g, lv, q, sel, sel_count, k_max, scale * kLog2e, out, lse, scr.part_o, scr.part_ml);
-    cudaError_t err = cudaGetLastError();
-    if (err != cudaSuccess) return err;
-    mkv_combine_kernel<<<dim3(g.n_units, g.group), 128, 0, s>>>(g, sel_count, k_max, sm_count * NWARPS, scr.part_o, scr.part_ml,
-                                                                 out, lse);
+        g, lv, q, sel, sel_count, k_max, scale * kLog2e, out, lse, scr.part_o, scr.part_ml, scr.ticket);
     return cudaGetLastError();
 }
 
@@ -625,7 +768,7 @@ cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint
                              const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
                              const AttnScratch& scr, int sm_count, cudaStream_t s, int* n_kernels) {
     if (g.n_units > kMaxUnitsSmem) return cudaErrorInvalidValue;
-    if (n_kernels) *n_kernels = 2;
+    if (n_kernels) *n_kernels = 1;
     static int cfg = -1;  // tuning knob (stages * 100 + warps); default chosen from measurements
     if (cfg < 0) {
         const char* e = getenv("MKV_ATTN_CFG");

@@ -90,7 +90,7 @@ int mkv_cache_free(mkv_cache* c) {
     cudaSetDevice(c->desc.device);
     cudaDeviceSynchronize();
     void* ptrs[] = {c->arena, c->strat, c->tok_off, c->bk_off, c->unit_nseg, c->unit_ntok, c->counters,
-                    c->dev_flags, c->call_base, c->scores, c->attn.part_o, c->attn.part_ml, c->q_dev,
+                    c->dev_flags, c->call_base, c->scores, c->attn.part_o, c->attn.part_ml, c->attn.ticket, c->q_dev,
                     c->sel_dev, c->selcnt_dev, c->out_dev, c->cands_dev};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -148,6 +148,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         {(void**)&c->scores, (size_t)g.n_units * g.score_stride * 4},
         {(void**)&c->attn.part_o, (size_t)c->attn.slots * g.group * kD * 4},
         {(void**)&c->attn.part_ml, (size_t)c->attn.slots * kMaxGroup * 2 * 4},
+        {(void**)&c->attn.ticket, (size_t)g.n_units * 4},
         {(void**)&c->q_dev, (size_t)g.batch * g.n_q_heads * kD * 2},
         {(void**)&c->sel_dev, (size_t)g.n_units * c->sel_cap * 4},
         {(void**)&c->selcnt_dev, (size_t)g.n_units * 4},
@@ -166,6 +167,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     cudaMemset(c->unit_ntok, 0, tu * 4);
     cudaMemset(c->counters, 0, (size_t)g.n_layers * 4 * 8);
     cudaMemset(c->dev_flags, 0, 256);
+    cudaMemset(c->attn.ticket, 0, (size_t)g.n_units * 4);
     cudaMemset(c->strat, 0, tu * g.S_max * sizeof(StratRec));
     c->host_nseg.assign((size_t)g.n_layers * g.batch, 0);
     c->host_ntok.assign((size_t)g.n_layers * g.batch, 0);

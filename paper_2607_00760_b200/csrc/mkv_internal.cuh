@@ -82,8 +82,9 @@ cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_
                           cudaStream_t s, int* n_kernels);
 
 struct AttnScratch {
-    float* part_o;    // [slots][G][D]   unnormalised partial outputs (<= 2 slots per warp of the grid)
+    float* part_o;    // [slots][G][D]   unnormalised partial outputs (<= 2 slots per warp and per CTA of the grid)
     float* part_ml;   // [slots][8][2]   (running max in log2 units, sum)
+    int32_t* ticket;  // [n_units]       arrivals of the CTAs sharing a unit; zero between launches
     int32_t slots;
 };
 int attention_partial_slots(int sm_count);
