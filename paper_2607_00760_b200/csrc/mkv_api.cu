@@ -282,7 +282,7 @@ int mkv_select(const mkv_cache* cc, int32_t layer, const void* q, int32_t budget
         return fail(MKV_E_ARG, "mkv_select: k_max %d too small for budget %d", k_max, budget);
     MKV_CUDA(cudaSetDevice(c->desc.device));
     MKV_CUDA(launch_select(g, c->view(layer), (const uint16_t*)q, budget, reduce, sel, sel_count, k_max,
-                           scores_opt ? scores_opt : c->scores, (cudaStream_t)stream, &c->last_select));
+                           scores_opt ? scores_opt : c->scores, c->sm_count, (cudaStream_t)stream, &c->last_select));
     return MKV_OK;
 }
 

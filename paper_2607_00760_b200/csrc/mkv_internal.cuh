@@ -77,9 +77,11 @@ cudaError_t launch_compress(const CacheGeom& g, const LayerView& lv, const Compr
                             const mkv_strategy* strat, unsigned long long* call_base,
                             uint32_t* dev_flags, cudaStream_t s, int* n_kernels);
 
+cudaError_t launch_score(const CacheGeom& g, const LayerView& lv, const uint16_t* q, int reduce,
+                         float* scores, int sm_count, cudaStream_t s);
 cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_t* q, int budget,
                           int reduce, int32_t* sel, int32_t* sel_count, int k_max, float* scores,
-                          cudaStream_t s, int* n_kernels);
+                          int sm_count, cudaStream_t s, int* n_kernels);
 
 struct AttnScratch {
     float* part_o;    // [slots][G][D]   unnormalised partial outputs (<= 2 slots per warp and per CTA of the grid)

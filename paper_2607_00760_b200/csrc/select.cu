@@ -1,5 +1,5 @@
-// select.cu — step 2 of the hot path: block scores on the packed block keys (PAPER.md:182,
-// 214-216) and top-k block selection by token budget.  sm_100a.
+// select.cu — step 2b of the hot path: top-k block selection by token budget
+// on the scores of score.cu (step 2a).  sm_100a.
 #include "mkv_internal.cuh"
 
 namespace mkv {
@@ -18,69 +18,6 @@ __device__ __forceinline__ unsigned lanemask_lt() {
 __device__ __forceinline__ uint32_t score_key(float s) {
     const uint32_t u = __float_as_uint(s + 0.0f);
     return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
-}
-
-// ------------------------------------------------------------------------------------------
-// score (v0): one thread per block key; packed vector product by walking the set bits of the
-// position bitmap.  q of the unit's G heads sits in shared memory as fp32.
-// ------------------------------------------------------------------------------------------
-template <int GP>
-__global__ void __launch_bounds__(256) mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q,
-                                                        int reduce, float* __restrict__ scores) {
-    const int unit = blockIdx.y;
-    const int b = unit / g.n_kv_heads, h = unit % g.n_kv_heads;
-    __shared__ float qs[kD][GP];  // [channel][head]: one channel's heads are contiguous
-    for (int i = threadIdx.x; i < kD * GP; i += 256) {
-        const int c = i / GP, gi = i % GP;
-        qs[c][gi] = (gi < g.group)
-                        ? bf16_bits_to_f32(q[((size_t)b * g.n_q_heads + (size_t)h * g.group + gi) * kD + c])
-                        : 0.f;
-    }
-    __syncthreads();
-    const int nseg = lv.unit_nseg[unit];
-    const int blk = blockIdx.x * 256 + threadIdx.x;
-    const int seg = blk / g.blocks_per_seg, i = blk % g.blocks_per_seg;
-    if (seg >= nseg) return;
-    const size_t e = (size_t)unit * lv.S_max + seg;
-    const StratRec rec = lv.strat[e];
-    const int nblk = (rec.n_tok + kB - 1) / kB;
-    if (i >= nblk) return;
-    const int r = rec.r_k;
-    const uint8_t* base = lv.slice + ((size_t)lv.bk_off[e] << 4);
-    float acc[GP];
-#pragma unroll
-    for (int gi = 0; gi < GP; ++gi) acc[gi] = 0.f;
-    if (r < kD) {
-        const uint4 bm = *reinterpret_cast<const uint4*>(base + 16 * i);
-        const uint16_t* val = reinterpret_cast<const uint16_t*>(base + 16 * nblk + (size_t)i * 2 * r);
-        const uint32_t words[4] = {bm.x, bm.y, bm.z, bm.w};
-        int n = 0;
-#pragma unroll
-        for (int w = 0; w < 4; ++w) {
-            uint32_t word = words[w];
-            while (word) {
-                const int c = 32 * w + __ffs(word) - 1;
-                word &= word - 1;
-                const float x = bf16_bits_to_f32(val[n++]);
-#pragma unroll
-                for (int gi = 0; gi < GP; ++gi) acc[gi] = fmaf(qs[c][gi], x, acc[gi]);
-            }
-        }
-    } else {
-        const uint16_t* val = reinterpret_cast<const uint16_t*>(base + (size_t)i * 2 * kD);
-        for (int c = 0; c < kD; ++c) {
-            const float x = bf16_bits_to_f32(val[c]);
-#pragma unroll
-            for (int gi = 0; gi < GP; ++gi) acc[gi] = fmaf(qs[c][gi], x, acc[gi]);
-        }
-    }
-    float s = acc[0];
-    if (reduce == 1) {
-        for (int gi = 1; gi < g.group; ++gi) s += acc[gi];
-    } else {
-        for (int gi = 1; gi < g.group; ++gi) s = fmaxf(s, acc[gi]);
-    }
-    scores[(size_t)unit * g.score_stride + blk] = s + 0.0f;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -210,12 +147,9 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
 }  // namespace
 
 cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_t* q, int budget, int reduce,
-                          int32_t* sel, int32_t* sel_count, int k_max, float* scores, cudaStream_t s,
-                          int* n_kernels) {
-    dim3 grid((g.score_stride + 255) / 256, g.n_units);
-    if (g.group <= 4) mkv_score_kernel<4><<<grid, 256, 0, s>>>(g, lv, q, reduce, scores);
-    else mkv_score_kernel<8><<<grid, 256, 0, s>>>(g, lv, q, reduce, scores);
-    cudaError_t err = cudaGetLastError();
+                          int32_t* sel, int32_t* sel_count, int k_max, float* scores, int sm_count,
+                          cudaStream_t s, int* n_kernels) {
+    cudaError_t err = launch_score(g, lv, q, reduce, scores, sm_count, s);
     if (err != cudaSuccess) return err;
     mkv_topk_kernel<<<g.n_units, 1024, 0, s>>>(g, lv, scores, budget, sel, sel_count, k_max);
     if (n_kernels) *n_kernels = 2;
