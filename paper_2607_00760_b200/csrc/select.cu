@@ -28,20 +28,28 @@ __device__ __forceinline__ uint32_t score_key(float s) {
 // one short block (the unit's last), the walk takes the k0 = budget/8 best blocks, plus one
 // more iff the short block is among the k0+1 best and fits the remainder.
 // ------------------------------------------------------------------------------------------
+// Keys of a unit are cached in shared memory when they fit (kKeyCap), so the four radix passes read
+// global memory once.  Histogram updates are aggregated per warp with match.any (scores cluster in a
+// few bins of the first pass); the emission gives every thread a run of consecutive blocks, so one
+// block-wide scan of packed (greater, equal) counts orders the whole output.
+constexpr int kKeyCap = 16384;  // 64 KB of keys
+
 __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView lv, const float* __restrict__ scores,
                                                         int budget, int32_t* __restrict__ sel,
                                                         int32_t* __restrict__ sel_count, int k_max) {
+    extern __shared__ uint32_t s_keys[];  // key i at [i + i / 32]: conflict-free for strided and for per-thread runs
     const int unit = blockIdx.x;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int ntok = lv.unit_ntok[unit];
     const int nblk = (ntok + kB - 1) / kB;
     const float* s = scores + (size_t)unit * g.score_stride;
     int32_t* out = sel + (size_t)unit * k_max;
+    const bool cached = nblk <= kKeyCap;
 
-    __shared__ unsigned hist[256];
+    __shared__ unsigned hist[4096];
     __shared__ uint32_t s_prefix;
     __shared__ int s_krem, s_neq;
-    __shared__ int s_warp[32], s_warp2[32];
+    __shared__ unsigned long long s_warp[32];
 
     const bool all = (ntok <= budget);
     const int k0 = budget / kB, rem = budget % kB, nbR = ntok % kB;
@@ -50,39 +58,60 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
     uint32_t Ts = 0;
     int take_eq = 0;
     if (!all && kq > 0) {
+        if (cached)
+            for (int i = tid; i < nblk; i += 1024) s_keys[i + (i >> 5)] = score_key(s[i]);
         uint32_t prefix = 0;
         int krem = kq;
-        for (int pass = 0; pass < 4; ++pass) {
-            const int shift = 24 - 8 * pass;
-            if (tid < 256) hist[tid] = 0;
-            __syncthreads();
-            const uint32_t hi_mask = pass == 0 ? 0u : (0xffffffffu << (shift + 8));
+        // MSB-first radix select in three passes of 12 + 12 + 8 bits: with 4096 bins the scores spread
+        // over enough bins for plain shared-memory atomics, and later passes touch few elements
+        for (int pass = 0; pass < 3; ++pass) {
+            const int shift = pass == 0 ? 20 : (pass == 1 ? 8 : 0);
+            const int nbins = pass == 2 ? 256 : 4096;
+            for (int i = tid; i < nbins; i += 1024) hist[i] = 0;
+            __syncthreads();  // also orders the fill of s_keys before the first pass
+            const uint32_t hi_mask = pass == 0 ? 0u : (0xffffffffu << (pass == 1 ? 20 : 8));
             for (int i = tid; i < nblk; i += 1024) {
-                const uint32_t u = score_key(s[i]);
-                if ((u & hi_mask) == prefix) atomicAdd(&hist[(u >> shift) & 255u], 1u);
+                const uint32_t u = cached ? s_keys[i + (i >> 5)] : score_key(s[i]);
+                if ((u & hi_mask) == prefix) atomicAdd(&hist[(u >> shift) & (uint32_t)(nbins - 1)], 1u);
             }
             __syncthreads();
-            if (warp == 0) {
-                unsigned mine[8], tot = 0;
+            // thread t owns bins [t bpt, (t+1) bpt); counts in the bins above it by a block-wide suffix scan
+            const int bpt = nbins >> 10;  // 4 or 0 (256 bins: one bin for each of the first 256 threads)
+            unsigned mine[4] = {0u, 0u, 0u, 0u}, tot = 0;
+            if (bpt) {
 #pragma unroll
-                for (int j = 0; j < 8; ++j) { mine[j] = hist[8 * lane + j]; tot += mine[j]; }
-                // suffix-exclusive sum over lanes: counts in bins above this lane's bins
-                unsigned incl = tot;
+                for (int j = 0; j < 4; ++j) { mine[j] = hist[4 * tid + j]; tot += mine[j]; }
+            } else if (tid < 256) {
+                mine[0] = hist[tid]; tot = mine[0];
+            }
+            unsigned incl = tot;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const unsigned v = __shfl_down_sync(kFull, incl, o);
+                if (lane + o < 32) incl += v;
+            }
+            if (lane == 0) s_warp[warp] = incl;
+            __syncthreads();
+            if (warp == 0) {
+                const unsigned w = (unsigned)s_warp[lane];
+                unsigned wi = w;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
-                    const unsigned v = __shfl_down_sync(kFull, incl, o);
-                    if (lane + o < 32) incl += v;
+                    const unsigned v = __shfl_down_sync(kFull, wi, o);
+                    if (lane + o < 32) wi += v;
                 }
-                unsigned cum = incl - tot;
-#pragma unroll
-                for (int j = 7; j >= 0; --j) {
-                    if (cum < (unsigned)krem && (unsigned)krem <= cum + mine[j]) {
-                        s_prefix = prefix | ((uint32_t)(8 * lane + j) << shift);
-                        s_krem = krem - (int)cum;
-                        s_neq = (int)mine[j];
-                    }
-                    cum += mine[j];
+                s_warp[lane] = wi - w;  // counts in the warps above
+            }
+            __syncthreads();
+            unsigned cum = (unsigned)s_warp[warp] + incl - tot;
+            const int nb_mine = bpt ? 4 : 1, bin0 = bpt ? 4 * tid : tid;
+            for (int j = nb_mine - 1; j >= 0; --j) {
+                if (cum < (unsigned)krem && (unsigned)krem <= cum + mine[j]) {
+                    s_prefix = prefix | ((uint32_t)(bin0 + j) << shift);
+                    s_krem = krem - (int)cum;
+                    s_neq = (int)mine[j];
                 }
+                cum += mine[j];
             }
             __syncthreads();
             prefix = s_prefix;
@@ -100,46 +129,57 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
         }
     }
 
-    // emission in ascending block index
-    int carry_eq = 0, carry_out = 0;
+    // emission in ascending block index: thread t owns blocks [t E, (t+1) E)
+    int count = 0;
     if (kq > 0) {
-        for (int i0 = 0; i0 < nblk; i0 += 1024) {
-            const int i = i0 + tid;
-            bool gt = false, eq = false;
-            if (i < nblk) {
-                if (all) gt = true;
-                else {
-                    const uint32_t u = score_key(s[i]);
-                    gt = u > Ts;
-                    eq = u == Ts;
-                }
+        const int E = (nblk + 1023) / 1024;
+        const int i0 = min(nblk, tid * E), i1 = min(nblk, i0 + E);
+        unsigned long long mine = 0;  // greater | equal << 32 among this thread's blocks
+        if (all) mine = (unsigned long long)(i1 - i0);
+        else
+            for (int i = i0; i < i1; ++i) {
+                const uint32_t u = cached ? s_keys[i + (i >> 5)] : score_key(s[i]);
+                mine += (u > Ts ? 1ull : 0ull) + (u == Ts ? (1ull << 32) : 0ull);
             }
-            const unsigned be = __ballot_sync(kFull, eq);
-            if (lane == 0) s_warp[warp] = __popc(be);
-            __syncthreads();
-            int eq_before = carry_eq + __popc(be & lanemask_lt()), eq_total = 0;
-            for (int w = 0; w < 32; ++w) {
-                const int c = s_warp[w];
-                if (w < warp) eq_before += c;
-                eq_total += c;
+        // block-wide exclusive scan of the packed counts
+        unsigned long long incl = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long v = __shfl_up_sync(kFull, incl, o);
+            if (lane >= o) incl += v;
+        }
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            const unsigned long long w = s_warp[lane];
+            unsigned long long wi = w;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const unsigned long long v = __shfl_up_sync(kFull, wi, o);
+                if (lane >= o) wi += v;
+            }
+            s_warp[lane] = wi - w;
+            if (lane == 31) s_krem = (int)((uint32_t)wi + min((uint32_t)take_eq, (uint32_t)(wi >> 32)));
+        }
+        __syncthreads();
+        const unsigned long long before = s_warp[warp] + incl - mine;
+        int gt_before = (int)(uint32_t)before, eq_before = (int)(before >> 32);
+        count = all ? nblk : s_krem;
+        for (int i = i0; i < i1; ++i) {
+            bool gt = all, eq = false;
+            if (!all) {
+                const uint32_t u = cached ? s_keys[i + (i >> 5)] : score_key(s[i]);
+                gt = u > Ts;
+                eq = u == Ts;
             }
             const bool take = gt || (eq && eq_before < take_eq);
-            const unsigned bt = __ballot_sync(kFull, take);
-            if (lane == 0) s_warp2[warp] = __popc(bt);
-            __syncthreads();
-            int pos = carry_out + __popc(bt & lanemask_lt()), out_total = 0;
-            for (int w = 0; w < 32; ++w) {
-                const int c = s_warp2[w];
-                if (w < warp) pos += c;
-                out_total += c;
-            }
+            const int pos = gt_before + min(eq_before, take_eq);
             if (take && pos < k_max) out[pos] = i * kB;
-            carry_eq += eq_total;
-            carry_out += out_total;
-            __syncthreads();
+            gt_before += gt ? 1 : 0;
+            eq_before += eq ? 1 : 0;
         }
     }
-    const int count = min(carry_out, k_max);
+    count = min(count, k_max);
     for (int p = count + tid; p < k_max; p += 1024) out[p] = -1;
     if (tid == 0) sel_count[unit] = count;
 }
@@ -151,7 +191,15 @@ cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_
                           cudaStream_t s, int* n_kernels) {
     cudaError_t err = launch_score(g, lv, q, reduce, scores, sm_count, s);
     if (err != cudaSuccess) return err;
-    mkv_topk_kernel<<<g.n_units, 1024, 0, s>>>(g, lv, scores, budget, sel, sel_count, k_max);
+    const int n_keys = g.score_stride < kKeyCap ? g.score_stride : kKeyCap;
+    const int key_bytes = 4 * (n_keys + n_keys / 32 + 1);
+    static int configured = 0;
+    if (key_bytes > configured) {
+        err = cudaFuncSetAttribute(mkv_topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, key_bytes);
+        if (err != cudaSuccess) return err;
+        configured = key_bytes;
+    }
+    mkv_topk_kernel<<<g.n_units, 1024, key_bytes, s>>>(g, lv, scores, budget, sel, sel_count, k_max);
     if (n_kernels) *n_kernels = 2;
     return cudaGetLastError();
 }
