@@ -48,14 +48,19 @@ __device__ __forceinline__ void topr_mask(const uint32_t (&mag)[4], int r, uint3
     }
 }
 
-// Write one packed vector (bitmap + kept values, ascending channel) or a dense copy.
-// x[j]: bf16 bits of channel lane + 32 j.  bm / val: byte pointers (val is 2-byte aligned).
-__device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, uint8_t* bm, uint8_t* val,
+// Write one packed vector: vector t of a group of n <= 8 vectors (the K or the V vectors of a token
+// block, or 8 block keys of a segment).  Physical layout of a group:
+// the n position bitmaps, then the kept values RANK-MAJOR: the value of rank rho (ascending
+// channel) of vector t sits at element rho * n + t, so that the vectors' run pointers advance
+// through disjoint shared-memory banks in the decode kernels' walk.  Dense vectors (r = D) carry
+// no bitmap and stay vector-major.  x[j]: bf16 bits of channel lane + 32 j.
+// bm: this vector's bitmap; val: the GROUP's value area (2-byte aligned).
+__device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, uint8_t* bm, uint8_t* val, int t, int n,
                                             int lane) {
     uint16_t* v16 = reinterpret_cast<uint16_t*>(val);
     if (r == kD) {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) v16[lane + 32 * j] = (uint16_t)x[j];
+        for (int j = 0; j < 4; ++j) v16[t * kD + lane + 32 * j] = (uint16_t)x[j];
         return;
     }
     uint32_t mag[4], w[4];
@@ -66,7 +71,7 @@ __device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, uint8
     int base = 0;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-        if ((w[j] >> lane) & 1u) v16[base + __popc(w[j] & lt)] = (uint16_t)x[j];
+        if ((w[j] >> lane) & 1u) v16[(base + __popc(w[j] & lt)) * n + t] = (uint16_t)x[j];
         base += __popc(w[j]);
     }
     if (lane < 8) {  // 2-byte stores: a ragged token block leaves the V bitmaps only 2-byte aligned
@@ -230,13 +235,13 @@ __global__ void __launch_bounds__(256) mkv_compress_kernel(CacheGeom g, LayerVie
         for (int j = 0; j < 4; ++j) x[j] = __ldg(ksrc + (size_t)t * a.stride_t + lane + 32 * j);
 #pragma unroll
         for (int j = 0; j < 4; ++j) sum[j] = __fadd_rn(sum[j], bf16_bits_to_f32(x[j]));
-        pack_vector(x, r_k, k_bm + t * bmk, k_val + t * r_k * 2, lane);
+        pack_vector(x, r_k, k_bm + t * bmk, k_val, t, nb, lane);
     }
     for (int t = 0; t < nb; ++t) {
         uint32_t x[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) x[j] = __ldg(vsrc + (size_t)t * a.stride_t + lane + 32 * j);
-        pack_vector(x, r_v, v_bm + t * bmv, v_val + t * r_v * 2, lane);
+        pack_vector(x, r_v, v_bm + t * bmv, v_val, t, nb, lane);
     }
     // zero the pad of a ragged token block
     {
@@ -250,7 +255,9 @@ __global__ void __launch_bounds__(256) mkv_compress_kernel(CacheGeom g, LayerVie
         const float fnb = (float)nb;
 #pragma unroll
         for (int j = 0; j < 4; ++j) x[j] = f32_to_bf16_bits_rne(__fdiv_rn(sum[j], fnb));
-        pack_vector(x, r_k, bk_base + blk * bmk, bk_base + nblk * bmk + blk * r_k * 2, lane);
+        // the block keys of a segment form groups of 8 (one work item of the score kernel each)
+        const int grp = blk >> 3, gn = min(8, nblk - 8 * grp);
+        pack_vector(x, r_k, bk_base + blk * bmk, bk_base + nblk * bmk + (size_t)grp * 8 * r_k * 2, blk & 7, gn, lane);
         if (blk == nblk - 1) {
             const uint32_t used = (uint32_t)nblk * vec_bytes(r_k);
             const uint32_t padded = pad16u(used);

@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <algorithm>
 #include <vector>
 
 #include "mkv_internal.cuh"
@@ -386,6 +387,31 @@ int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, vo
         tpos += trun;
         kpos += krun;
         s = e;
+    }
+    // The physical value order inside a group of <= 8 vectors is rank-major (compress.cu); the
+    // canonical blob is vector-major: transpose every group of packed (r < D) vectors.
+    auto to_canonical = [](uint8_t* vals, int r, int n) {
+        if (r == kD || n <= 1) return;
+        uint16_t tmp[8 * kD];
+        uint16_t* v = reinterpret_cast<uint16_t*>(vals);
+        for (int rho = 0; rho < r; ++rho)
+            for (int t = 0; t < n; ++t) tmp[t * r + rho] = v[rho * n + t];
+        memcpy(vals, tmp, (size_t)n * r * 2);
+    };
+    uint8_t* tp = tok_arena;
+    uint8_t* kp = bk_arena;
+    for (int sg = 0; sg < S; ++sg) {
+        const int r_k = rec[sg].r_k, r_v = rec[sg].r_v, n_tok = rec[sg].n_tok, nblk = (n_tok + kB - 1) / kB;
+        const uint32_t bmk = r_k == kD ? 0u : (uint32_t)kBitmapBytes, bmv = r_v == kD ? 0u : (uint32_t)kBitmapBytes;
+        for (int blk = 0; blk < nblk; ++blk) {
+            const int nb = std::min(kB, n_tok - blk * kB);
+            to_canonical(tp + nb * bmk, r_k, nb);
+            to_canonical(tp + nb * (bmk + 2 * r_k) + nb * bmv, r_v, nb);
+            tp += tokblock_bytes(r_k, r_v, nb);
+        }
+        for (int grp = 0; grp * 8 < nblk; ++grp)
+            to_canonical(kp + nblk * bmk + (size_t)grp * 8 * r_k * 2, r_k, std::min(8, nblk - 8 * grp));
+        kp += seg_bk_bytes(r_k, n_tok);
     }
     return MKV_OK;
 }

@@ -65,66 +65,91 @@ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
     return d;
 }
 
-// One slot of a packed run: if bit MASK of the position bitmap `w` is set, load the next kept
-// bf16 of the run into `v` (which the caller zero-initialised) and advance the run pointer.
-// Predicated, no branch: every lane executes the same instruction stream whatever its bitmap.
-template <uint32_t MASK>
-__device__ __forceinline__ void take_slot(uint32_t w, uint32_t& v, uint32_t& ptr) {
+// ---- mbarrier + 1-D bulk copy (TMA engine: one instruction moves a whole payload chunk) ------
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_init_fence() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+// global -> this CTA's shared memory; src, dst and bytes are multiples of 16
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, unsigned long long src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        ".reg .b32 t;\n"
-        "and.b32 t, %2, %3;\n"
-        "setp.ne.u32 p, t, 0;\n"
-        "@p ld.shared.u16 %0, [%1];\n"
-        "@p add.u32 %1, %1, 2;\n"
-        "}\n"
-        : "+r"(v), "+r"(ptr)
-        : "r"(w), "n"(MASK)
+        "MKV_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra MKV_DONE;\n"
+        "bra MKV_WAIT;\n"
+        "MKV_DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
         : "memory");
 }
-// hi * 65536 + lo: an IMAD (FMA pipe), not a PRMT/LOP3 (ALU pipe, which the bit tests load)
+
+// Eight slots (byte BYTE of the position-bitmap word `w`) of one packed run: a set bit loads the
+// next kept bf16 of the run and advances the run pointer by `step` bytes (2 n for a group of n
+// vectors stored rank-major, 2 for a dense vector); a clear bit leaves 0.  Written as plain
+// bit tests of ONE word in slot order so that ptxas if-converts them (predicated LDS.U16 + add, no
+// branch) and derives seven predicates at a time with R2P instead of one LOP3 per slot.  The empty
+// asm keeps the values opaque, so the pairing below stays one IMAD on zero-initialised registers.
+template <int BYTE>
+__device__ __forceinline__ void walk8(uint32_t w, uint32_t& ptr, uint32_t step, uint32_t (&v)[8]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        v[i] = 0u;
+        if (w & (1u << (8 * BYTE + i))) {
+            v[i] = lds_u16(ptr);
+            ptr += step;
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) asm volatile("" : "+r"(v[i]));
+}
+// hi * 65536 + lo: an IMAD (FMA pipe), not a PRMT/LOP3 (ALU pipe)
 __device__ __forceinline__ uint32_t pair16(uint32_t lo, uint32_t hi) { return hi * 65536u + lo; }
 
-// K walk, k-step KS (4 slots of this lane's bitmap word) of two runs at once (token gq of block
-// 0 and of block 1) -> A fragment a0..a3
-template <int KS>
-__device__ __forceinline__ void k_step(uint32_t w0, uint32_t w1, uint32_t& p0, uint32_t& p1, uint32_t (&b)[4]) {
-    uint32_t e[4] = {0u, 0u, 0u, 0u}, f[4] = {0u, 0u, 0u, 0u};
-    take_slot<1u << (4 * KS + 0)>(w0, e[0], p0);
-    take_slot<1u << (4 * KS + 0)>(w1, f[0], p1);
-    take_slot<1u << (4 * KS + 1)>(w0, e[1], p0);
-    take_slot<1u << (4 * KS + 1)>(w1, f[1], p1);
-    take_slot<1u << (4 * KS + 2)>(w0, e[2], p0);
-    take_slot<1u << (4 * KS + 2)>(w1, f[2], p1);
-    take_slot<1u << (4 * KS + 3)>(w0, e[3], p0);
-    take_slot<1u << (4 * KS + 3)>(w1, f[3], p1);
-    b[0] = pair16(e[0], e[1]);  // row gq   (block 0), k = 2qq, 2qq+1
-    b[1] = pair16(f[0], f[1]);  // row gq+8 (block 1)
-    b[2] = pair16(e[2], e[3]);  // row gq,   k = 2qq+8, 2qq+9
-    b[3] = pair16(f[2], f[3]);  // row gq+8
+// K walk: byte BYTE (8 channels of this lane's 32-channel word) of two runs -- token gq of block 0
+// (rows 0-7 of the 16-token M tile) and of block 1 (rows 8-15) -- feeds two k-steps of S = K q^T.
+// qa: B fragments of q for the k-steps 2 BYTE and 2 BYTE + 1 (same channel permutation).
+template <int BYTE>
+__device__ __forceinline__ void k_walk_mma(float (&S)[4], uint32_t w0, uint32_t w1, uint32_t& p0, uint32_t& p1,
+                                           uint32_t st0, uint32_t st1, const uint32_t (&qa)[8][2]) {
+    uint32_t e[8], f[8];
+    walk8<BYTE>(w0, p0, st0, e);
+    walk8<BYTE>(w1, p1, st1, f);
+    mma_bf16(S, pair16(e[0], e[1]), pair16(f[0], f[1]), pair16(e[2], e[3]), pair16(f[2], f[3]), qa[2 * BYTE][0],
+             qa[2 * BYTE][1]);
+    mma_bf16(S, pair16(e[4], e[5]), pair16(f[4], f[5]), pair16(e[6], e[7]), pair16(f[6], f[7]), qa[2 * BYTE + 1][0],
+             qa[2 * BYTE + 1][1]);
 }
 
-// V walk, M tile I (channel slots 2I, 2I+1 of this lane's half-word) of four runs at once
-// (tokens A = 2qq and B = 2qq+1 of block 0 and of block 1) -> A fragment a0..a3
-template <int I>
-__device__ __forceinline__ void v_step(uint32_t hA0, uint32_t hB0, uint32_t hA1, uint32_t hB1, uint32_t& pA0,
-                                       uint32_t& pB0, uint32_t& pA1, uint32_t& pB1, uint32_t (&a)[4]) {
-    uint32_t x[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
-    take_slot<1u << (2 * I)>(hA0, x[0], pA0);
-    take_slot<1u << (2 * I)>(hB0, x[1], pB0);
-    take_slot<1u << (2 * I)>(hA1, x[4], pA1);
-    take_slot<1u << (2 * I)>(hB1, x[5], pB1);
-    take_slot<1u << (2 * I + 1)>(hA0, x[2], pA0);
-    take_slot<1u << (2 * I + 1)>(hB0, x[3], pB0);
-    take_slot<1u << (2 * I + 1)>(hA1, x[6], pA1);
-    take_slot<1u << (2 * I + 1)>(hB1, x[7], pB1);
-    a[0] = pair16(x[0], x[1]);  // row gq   (channel 16gq + 2I),     tokens 2qq, 2qq+1 of block 0
-    a[1] = pair16(x[2], x[3]);  // row gq+8 (channel 16gq + 2I + 1), block 0
-    a[2] = pair16(x[4], x[5]);  // row gq,   block 1
-    a[3] = pair16(x[6], x[7]);  // row gq+8, block 1
+// V walk: byte BYTE (8 channels of this lane's 16-channel half-word) of four runs -- tokens
+// A = 2qq and B = 2qq+1 of block 0 and of block 1 -- feeds four M tiles of O^T += V^T P^T with P
+// split into bf16 hi (ph) and lo (pl).  A register pairs two TOKENS of one channel.
+template <int BYTE>
+__device__ __forceinline__ void v_walk_mma(float (&acc)[8][4], uint32_t hA0, uint32_t hB0, uint32_t hA1, uint32_t hB1,
+                                           uint32_t& pA0, uint32_t& pB0, uint32_t& pA1, uint32_t& pB1, uint32_t st0,
+                                           uint32_t st1, uint32_t ph0, uint32_t ph1, uint32_t pl0, uint32_t pl1) {
+    uint32_t a0[8], b0[8], a1[8], b1[8];
+    walk8<BYTE>(hA0, pA0, st0, a0);
+    walk8<BYTE>(hB0, pB0, st0, b0);
+    walk8<BYTE>(hA1, pA1, st1, a1);
+    walk8<BYTE>(hB1, pB1, st1, b1);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {  // tile 4 BYTE + j: rows gq / gq+8 = channels 16gq + 8 BYTE + 2j / + 1
+        const uint32_t x0 = pair16(a0[2 * j], b0[2 * j]), x1 = pair16(a0[2 * j + 1], b0[2 * j + 1]);
+        const uint32_t x2 = pair16(a1[2 * j], b1[2 * j]), x3 = pair16(a1[2 * j + 1], b1[2 * j + 1]);
+        mma_bf16(acc[4 * BYTE + j], x0, x1, x2, x3, ph0, ph1);
+        mma_bf16(acc[4 * BYTE + j], x0, x1, x2, x3, pl0, pl1);
+    }
 }
-
 
 // floor(p / d) for p < 2^56 without the 64-bit division subroutine: fp32 estimate, exact fix-up
 __device__ __forceinline__ unsigned div_floor(unsigned long long p, unsigned d, float inv_d) {

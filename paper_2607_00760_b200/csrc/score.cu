@@ -188,7 +188,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                     mma_bf16(S, x.z, y.z, x.w, y.w, qa[2 * h + 1][0], qa[2 * h + 1][1]);
                 }
             } else {
-                uint32_t w0 = 0u, w1 = 0u, p0, p1;
+                uint32_t w0 = 0u, w1 = 0u, p0, p1, st0 = 2u, st1 = 2u;
                 if (r_k == kD) {  // ragged dense item: all slots kept, no bitmap stored
                     w0 = gq < nb0 ? 0xffffffffu : 0u;
                     w1 = (n == 2 && gq < nb1) ? 0xffffffffu : 0u;
@@ -201,16 +201,14 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                     t = __shfl_up_sync(kFull, inc, 1); if (qq >= 1) inc += t;
                     t = __shfl_up_sync(kFull, inc, 2); if (qq >= 2) inc += t;
                     const uint32_t ex = inc - cnt;
-                    p0 = sp0 + 128 + 2 * (r_k * gq + (ex & 0xffffu));
-                    p1 = sp1 + 128 + 2 * (r_k * gq + (ex >> 16));
+                    st0 = 2u * nb0; st1 = 2u * nb1;  // values rank-major within the item (compress.cu)
+                    p0 = sp0 + 128 + st0 * (ex & 0xffffu) + 2 * gq;
+                    p1 = sp1 + 128 + st1 * (ex >> 16) + 2 * gq;
                 }
-                uint32_t a[4];
-#define MKV_KSTEP(KS)                  \
-    k_step<KS>(w0, w1, p0, p1, a);     \
-    mma_bf16(S, a[0], a[1], a[2], a[3], qa[KS][0], qa[KS][1]);
-                MKV_KSTEP(0) MKV_KSTEP(1) MKV_KSTEP(2) MKV_KSTEP(3)
-                MKV_KSTEP(4) MKV_KSTEP(5) MKV_KSTEP(6) MKV_KSTEP(7)
-#undef MKV_KSTEP
+                k_walk_mma<0>(S, w0, w1, p0, p1, st0, st1, qa);
+                k_walk_mma<1>(S, w0, w1, p0, p1, st0, st1, qa);
+                k_walk_mma<2>(S, w0, w1, p0, p1, st0, st1, qa);
+                k_walk_mma<3>(S, w0, w1, p0, p1, st0, st1, qa);
             }
             __syncwarp();  // every lane is done reading stage s
 
