@@ -3,11 +3,12 @@
 //
 // Design: a streaming kernel over the block-key arena.
 //   * Work item = 8 block keys of one segment (one item per segment at L = 64).  Items are taken in
-//     pairs (16 keys = the M of one mma.sync tile); the pairs of all units form one stream that is
+//     pairs (16 keys = the M of one mma.sync tile); the items of all units form one stream that is
 //     cut into equal contiguous ranges, one per warp of a one-CTA-per-SM grid.  Warps are
-//     independent (no __syncthreads in the main loop).
-//   * Each pair's payload (position bitmaps + kept bf16 values, DESIGN.md format) is copied into a
-//     per-warp shared-memory stage with 16-byte cp.async (LDGSTS, L1 bypass), several pairs in flight.
+//     independent (no __syncthreads at all).
+//   * Staging: an item's position bitmaps and its kept values (DESIGN.md format) are two contiguous
+//     16-B-aligned chunks; one lane moves each with ONE 1-D bulk copy (cp.async.bulk, the TMA
+//     engine) that completes on the stage's mbarrier; kStages groups are in flight per warp.
 //   * The packed keys are expanded straight into mma.sync A fragments by the same walk as
 //     PackedAttention's QK (mkv_walk.cuh): S = Kbar q^T, keys = M, heads = N, channels = K, fp32
 //     accumulate; the group reduction (max or sum over the G heads) is two shuffles.
@@ -22,24 +23,29 @@ namespace {
 
 using namespace walk;
 
-constexpr int kItemRing = 64;       // item descriptors kept per warp (32 pairs)
+constexpr int kRing = 64;           // group descriptors kept per warp
 constexpr int kScoreStage = 4096;   // two items: 2 x (128 B of bitmaps + 16 r_k B of values), or 2 x 2048 B dense
 
-struct __align__(16) Item {  // 8 block keys of one segment
-    uint32_t src16;          // payload offset of the item's bitmaps (values if dense) in the slice, 16-B units
-    uint32_t val16;          // offset of the item's values, 16-B units
-    uint32_t out;            // index of its first score: unit * score_stride + block index
-    uint16_t unit;
-    uint8_t r_k, nb;         // nb = 0: nothing there (segment past the unit's end)
+// One group: <= 2 consecutive items (8 block keys each) of one unit with the same r_k.
+struct __align__(16) SDesc {
+    uint32_t bm0, val0, bm1, val1;  // chunk offsets in the layer slice, 16-B units (dense: bm = the keys, val unused)
+    uint32_t out0, out1;            // index of each item's first score: unit * score_stride + block index
+    uint32_t meta;                  // r_k | nb0 << 8 | nb1 << 12
+    uint32_t unit;
 };
 
-__host__ __device__ constexpr int score_warp_smem(int nstage) { return nstage * kScoreStage + kItemRing * 16 + nstage * 16; }
+__device__ __forceinline__ unsigned lanemask_le() {
+    unsigned m;
+    asm("mov.u32 %0, %%lanemask_le;" : "=r"(m));
+    return m;
+}
+__device__ __forceinline__ unsigned lanemask_lt() {
+    unsigned m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
 
-struct __align__(16) SMeta {  // one in-flight group (<= 2 items of one unit with equal r_k)
-    int32_t unit;
-    uint32_t rknb;            // r_k | nb0 << 8 | nb1 << 16 | n << 24 (n = 0: end of the range)
-    uint32_t out0, out1;
-};
+__host__ __device__ constexpr int score_warp_smem(int nstage) { return nstage * kScoreStage + kRing * 32 + 64; }
 
 // ------------------------------------------------------------------------------------------
 // one CTA per SM, kWarps independent warps; warp gw owns items [gw I / GW, (gw+1) I / GW) of the
@@ -55,110 +61,110 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
     const int gq = lane >> 2, qq = lane & 3;
     const int G = g.group;
 
-    const unsigned long long I = (unsigned long long)g.n_units * items_per_unit;
+    const unsigned I = (unsigned)g.n_units * items_per_unit;  // < 2^32: checked by the launcher
     const unsigned GW = gridDim.x * kWarps, gw = blockIdx.x * kWarps + warp;
-    const unsigned long long lo = I * gw / GW, hi = I * (gw + 1) / GW;
-    const int n_total = (int)(hi - lo);
+    const unsigned ib = I / GW, ir = I - ib * GW;             // the first ir warps hold one more item
+    const unsigned lo = gw * ib + min(gw, ir);
+    const int n_total = (int)(ib + (gw < ir ? 1u : 0u));
     if (n_total <= 0) return;
 
     uint8_t* wbase = smem + warp * kWS;
     const uint32_t stage0 = smem_u32(wbase);
-    Item* ring = reinterpret_cast<Item*>(wbase + NSTAGE * kScoreStage);
-    SMeta* gmeta = reinterpret_cast<SMeta*>(wbase + NSTAGE * kScoreStage + kItemRing * 16);
+    SDesc* ring = reinterpret_cast<SDesc*>(wbase + NSTAGE * kScoreStage);
+    const uint32_t bar0 = stage0 + NSTAGE * kScoreStage + kRing * 32;
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < NSTAGE; ++s) mbar_init(bar0 + 8 * s, 1);
+        mbar_init_fence();
+    }
+    __syncwarp();
 
-    int pos = 0, built = 0;
+    int ibuilt = 0;                        // items described
+    int gposc = 0, gposi = 0, gbuilt = 0;  // groups consumed / issued / described
 
+    // Describe the next <= 32 items of the range (one per lane) and pair them into groups: item i
+    // follows item i - 1 in a group if both hold keys, belong to one unit and have the same r_k;
+    // runs of such items are paired greedily from their start.  Items past a unit's end hold no keys.
     auto build = [&](int count) {
+        uint32_t bm = 0u, val = 0u, out = 0u, r_k = 0u, nb = 0u, u = 0u;
         if (lane < count) {
-            const unsigned long long it = lo + (unsigned)(built + lane);
-            const unsigned u = (unsigned)(it / items_per_unit);
-            const unsigned rem = (unsigned)(it - (unsigned long long)u * items_per_unit);
+            const unsigned it = lo + (unsigned)(ibuilt + lane);
+            u = it / items_per_unit;
+            const unsigned rem = it - u * items_per_unit;
             const unsigned seg = subs == 1 ? rem : rem / (unsigned)subs;
             const unsigned sub = rem - seg * (unsigned)subs;
-            Item d;
-            d.src16 = 0; d.val16 = 0; d.out = 0; d.unit = (uint16_t)u; d.r_k = 0; d.nb = 0;
             if ((int)seg < lv.unit_nseg[u]) {
                 const size_t e = (size_t)u * lv.S_max + seg;
                 const StratRec rec = lv.strat[e];
                 const int nblk = ((int)rec.n_tok + kB - 1) / kB;
-                const int nb = min(8, nblk - 8 * (int)sub);
-                if (nb > 0) {
+                const int n = min(8, nblk - 8 * (int)sub);
+                if (n > 0) {
                     const uint32_t off = lv.bk_off[e];
-                    d.r_k = rec.r_k; d.nb = (uint8_t)nb;
-                    if (rec.r_k == kD) { d.src16 = off + 128u * sub; d.val16 = d.src16; }
-                    else { d.src16 = off + 8u * sub; d.val16 = off + (uint32_t)nblk + (uint32_t)rec.r_k * sub; }
-                    d.out = u * (unsigned)g.score_stride + seg * (unsigned)g.blocks_per_seg + 8u * sub;
+                    r_k = rec.r_k; nb = (uint32_t)n;
+                    if (rec.r_k == kD) { bm = off + 128u * sub; val = bm; }
+                    else { bm = off + 8u * sub; val = off + (uint32_t)nblk + (uint32_t)rec.r_k * sub; }
+                    out = u * (unsigned)g.score_stride + seg * (unsigned)g.blocks_per_seg + 8u * sub;
                 }
             }
-            ring[(built + lane) & (kItemRing - 1)] = d;
         }
-        built += count;
+        const uint32_t pu = __shfl_up_sync(kFull, u, 1), prk = __shfl_up_sync(kFull, r_k, 1), pnb = __shfl_up_sync(kFull, nb, 1);
+        const bool follows = lane > 0 && nb != 0u && pnb != 0u && u == pu && r_k == prk && (r_k == (uint32_t)kD || r_k <= 120u);  // two items must fit one stage
+        const unsigned fm = __ballot_sync(kFull, follows);
+        const int start = 31 - __clz((int)(~fm & lanemask_le()));  // first item of this lane's run (bit 0 of ~fm is set)
+        const bool first = nb != 0u && ((lane - start) & 1) == 0;
+        const bool two = first && ((fm >> 1) >> lane & 1u);
+        const unsigned gm = __ballot_sync(kFull, first);
+        const uint32_t bm1 = __shfl_down_sync(kFull, bm, 1), val1 = __shfl_down_sync(kFull, val, 1);
+        const uint32_t out1 = __shfl_down_sync(kFull, out, 1), nb1 = __shfl_down_sync(kFull, nb, 1);
+        if (first) {
+            SDesc d;
+            d.bm0 = bm; d.val0 = val; d.bm1 = two ? bm1 : 0u; d.val1 = two ? val1 : 0u;
+            d.out0 = out; d.out1 = two ? out1 : 0u;
+            d.meta = r_k | (nb << 8) | ((two ? nb1 : 0u) << 12);
+            d.unit = u;
+            ring[(gbuilt + __popc(gm & lanemask_lt())) & (kRing - 1)] = d;
+        }
+        gbuilt += __popc(gm);
+        ibuilt += count;
         __syncwarp();
     };
 
-    // form the next group and start its copies into stage s
+    // start the copies of the next group into stage s (lane 0: <= 2 bulk copies per item)
+    const unsigned long long slice = reinterpret_cast<unsigned long long>(lv.slice);
     auto issue = [&](int s) {
-        for (;;) {
-            if (built - pos <= 8 && built < n_total) build(min(32, n_total - built));
-            if (pos >= n_total || ring[pos & (kItemRing - 1)].nb != 0) break;
-            ++pos;  // nothing there: a segment past the unit's end
-        }
-        if (pos >= n_total) {
-            if (lane == 0) { SMeta m; m.unit = -1; m.rknb = 0; m.out0 = m.out1 = 0; gmeta[s] = m; }
-            cp_async_commit();
-            return;
-        }
-        const Item d0 = ring[pos & (kItemRing - 1)];
-        Item d1 = d0;
-        bool two = false;
-        if (pos + 1 < n_total) {
-            d1 = ring[(pos + 1) & (kItemRing - 1)];
-            two = d1.nb != 0 && d1.unit == d0.unit && d1.r_k == d0.r_k && (d0.r_k == kD || d0.r_k <= 120);
-        }
-        if (lane == 0) {
-            SMeta m;
-            m.unit = d0.unit;
-            m.rknb = (uint32_t)d0.r_k | ((uint32_t)d0.nb << 8) | ((two ? (uint32_t)d1.nb : 0u) << 16) | ((two ? 2u : 1u) << 24);
-            m.out0 = d0.out; m.out1 = d1.out;
-            gmeta[s] = m;
-        }
-        const unsigned long long base = reinterpret_cast<unsigned long long>(lv.slice);
-        const uint32_t dst = stage0 + s * kScoreStage;
-        const int r = d0.r_k;
 #pragma unroll 1
-        for (int t = 0; t < (two ? 2 : 1); ++t) {
-            const Item& d = t ? d1 : d0;
-            const uint32_t dd = dst + t * 2048;
-            if (r == kD) {
-                const unsigned long long src = base + ((unsigned long long)d.src16 << 4);
-                for (int i = lane; i < 16 * d.nb; i += 32) cp_async_16(dd + 16 * i, src + 16 * i);
-            } else {
-                const unsigned long long sb = base + ((unsigned long long)d.src16 << 4);
-                const unsigned long long sv = base + ((unsigned long long)d.val16 << 4);
-                const int nv = (2 * r * d.nb + 15) >> 4, nbm = d.nb;
-                for (int i = lane; i < nbm + nv; i += 32) {
-                    if (i < nbm) cp_async_16(dd + 16 * i, sb + 16 * i);
-                    else cp_async_16(dd + 128 + 16 * (i - nbm), sv + 16 * (i - nbm));
-                }
-            }
+        while (gposi == gbuilt && ibuilt < n_total) build(min(32, n_total - ibuilt));
+        if (gposi == gbuilt) return;
+        if (lane == 0) {
+            const SDesc d = ring[gposi & (kRing - 1)];
+            const uint32_t r = d.meta & 255u, nb0 = (d.meta >> 8) & 15u, nb1 = (d.meta >> 12) & 15u;
+            const uint32_t bar = bar0 + 8 * s, dst = stage0 + s * kScoreStage;
+            // bitmaps nb x 16 B, then the values padded to 16 B; dense: nb x 256 B in one chunk
+            const uint32_t bb0 = r == (uint32_t)kD ? nb0 * 256u : nb0 * 16u, vb0 = r == (uint32_t)kD ? 0u : pad16u(nb0 * 2u * r);
+            const uint32_t bb1 = r == (uint32_t)kD ? nb1 * 256u : nb1 * 16u, vb1 = r == (uint32_t)kD ? 0u : pad16u(nb1 * 2u * r);
+            mbar_expect_tx(bar, bb0 + vb0 + bb1 + vb1);
+            bulk_g2s(dst, slice + ((unsigned long long)d.bm0 << 4), bb0, bar);
+            if (vb0) bulk_g2s(dst + bb0, slice + ((unsigned long long)d.val0 << 4), vb0, bar);
+            if (bb1) bulk_g2s(dst + 2048, slice + ((unsigned long long)d.bm1 << 4), bb1, bar);
+            if (vb1) bulk_g2s(dst + 2048 + bb1, slice + ((unsigned long long)d.val1 << 4), vb1, bar);
         }
-        cp_async_commit();
-        pos += two ? 2 : 1;
+        ++gposi;
     };
 
     uint32_t qa[8][2];
     int cur_unit = -1;
 
+    // ---- main loop.  Iteration k >= 0 consumes group k from stage k % NSTAGE and refills that stage
+    // with group k + NSTAGE; iterations k < 0 only fill the pipeline (one call site for issue()).
+    int s = 0;
+    uint32_t parity = 0u;
 #pragma unroll 1
     for (int k = -NSTAGE;; ++k) {
-        const int s = (k + NSTAGE) % NSTAGE;
         if (k >= 0) {
-            __syncwarp();
-            const SMeta meta = gmeta[s];
-            const int n = (int)(meta.rknb >> 24);
-            if (n == 0) break;
-            if (meta.unit != cur_unit) {
-                cur_unit = meta.unit;
+            if (gposc == gbuilt) break;  // issue() runs ahead: nothing described means nothing left
+            const SDesc d = ring[gposc & (kRing - 1)];
+            if ((int)d.unit != cur_unit) {
+                cur_unit = (int)d.unit;
                 const int bi = cur_unit / g.n_kv_heads, hk = cur_unit % g.n_kv_heads;
                 const uint4* qrow = reinterpret_cast<const uint4*>(
                     q + ((size_t)bi * g.n_q_heads + (size_t)hk * G + gq) * kD + 32 * qq);
@@ -169,21 +175,19 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                     qa[2 * h][0] = v.x; qa[2 * h][1] = v.y; qa[2 * h + 1][0] = v.z; qa[2 * h + 1][1] = v.w;
                 }
             }
-            const int r_k = (int)(meta.rknb & 255u), nb0 = (int)((meta.rknb >> 8) & 255u), nb1 = (int)((meta.rknb >> 16) & 255u);
+            const int r_k = (int)(d.meta & 255u), nb0 = (int)((d.meta >> 8) & 15u), nb1 = (int)((d.meta >> 12) & 15u);
             const uint32_t sp0 = stage0 + s * kScoreStage, sp1 = sp0 + 2048;
-            const bool full = nb0 == 8 && (n == 1 || nb1 == 8);
 
-            cp_async_wait<NSTAGE - 1>();
-            __syncwarp();
+            mbar_wait(bar0 + 8 * s, parity);  // the group's bulk copies have landed
 
             float S[4] = {0.f, 0.f, 0.f, 0.f};  // rows gq / gq+8 = key gq of item 0 / 1, columns = heads 2qq, 2qq+1
-            if (r_k == kD && full) {
+            if (r_k == kD && nb0 == 8 && (nb1 == 0 || nb1 == 8)) {
                 const uint32_t a0 = sp0 + 256 * gq + 64 * qq, a1 = sp1 + 256 * gq + 64 * qq;
 #pragma unroll
                 for (int h = 0; h < 4; ++h) {
                     const uint4 x = lds_128(a0 + 16 * h);
                     uint4 y = make_uint4(0u, 0u, 0u, 0u);
-                    if (n == 2) y = lds_128(a1 + 16 * h);
+                    if (nb1) y = lds_128(a1 + 16 * h);
                     mma_bf16(S, x.x, y.x, x.y, y.y, qa[2 * h][0], qa[2 * h][1]);
                     mma_bf16(S, x.z, y.z, x.w, y.w, qa[2 * h + 1][0], qa[2 * h + 1][1]);
                 }
@@ -191,19 +195,19 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                 uint32_t w0 = 0u, w1 = 0u, p0, p1, st0 = 2u, st1 = 2u;
                 if (r_k == kD) {  // ragged dense item: all slots kept, no bitmap stored
                     w0 = gq < nb0 ? 0xffffffffu : 0u;
-                    w1 = (n == 2 && gq < nb1) ? 0xffffffffu : 0u;
+                    w1 = gq < nb1 ? 0xffffffffu : 0u;
                     p0 = sp0 + 256 * gq + 64 * qq;
                     p1 = sp1 + 256 * gq + 64 * qq;
-                } else {
+                } else {  // bitmaps nb x 16 B, then the values rank-major within the item (compress.cu)
                     if (gq < nb0) w0 = lds_u32(sp0 + 4 * lane);
-                    if (n == 2 && gq < nb1) w1 = lds_u32(sp1 + 4 * lane);
+                    if (gq < nb1) w1 = lds_u32(sp1 + 4 * lane);
                     uint32_t cnt = (uint32_t)__popc(w0) | ((uint32_t)__popc(w1) << 16), inc = cnt, t;
                     t = __shfl_up_sync(kFull, inc, 1); if (qq >= 1) inc += t;
                     t = __shfl_up_sync(kFull, inc, 2); if (qq >= 2) inc += t;
                     const uint32_t ex = inc - cnt;
-                    st0 = 2u * nb0; st1 = 2u * nb1;  // values rank-major within the item (compress.cu)
-                    p0 = sp0 + 128 + st0 * (ex & 0xffffu) + 2 * gq;
-                    p1 = sp1 + 128 + st1 * (ex >> 16) + 2 * gq;
+                    st0 = 2u * nb0; st1 = 2u * nb1;
+                    p0 = sp0 + 16 * nb0 + st0 * (ex & 0xffffu) + 2 * gq;
+                    p1 = sp1 + 16 * nb1 + st1 * (ex >> 16) + 2 * gq;
                 }
                 k_walk_mma<0>(S, w0, w1, p0, p1, st0, st1, qa);
                 k_walk_mma<1>(S, w0, w1, p0, p1, st0, st1, qa);
@@ -227,11 +231,13 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                 v0 = fmaxf(v0, __shfl_xor_sync(kFull, v0, 2)); v1 = fmaxf(v1, __shfl_xor_sync(kFull, v1, 2));
             }
             if (qq == 0) {
-                if (gq < nb0) scores[meta.out0 + gq] = v0 + 0.0f;
-                if (n == 2 && gq < nb1) scores[meta.out1 + gq] = v1 + 0.0f;
+                if (gq < nb0) scores[d.out0 + gq] = v0 + 0.0f;
+                if (gq < nb1) scores[d.out1 + gq] = v1 + 0.0f;
             }
+            ++gposc;
         }
-        issue(s);
+        issue(s);  // stage s is free (or, for k < 0, still empty): start the copies of group k + NSTAGE
+        if (++s == NSTAGE) { s = 0; if (k >= 0) parity ^= 1u; }
     }
 }
 
@@ -249,6 +255,7 @@ static cudaError_t launch_score_cfg(const CacheGeom& g, const LayerView& lv, con
         configured = smem;
     }
     const int subs = (g.blocks_per_seg + 7) / 8;
+    if ((unsigned long long)g.n_units * g.S_max * subs >= (1ull << 32)) return cudaErrorInvalidValue;
     mkv_score_kernel<NSTAGE, NWARPS><<<sm_count, NWARPS * 32, smem, s>>>(g, lv, q, reduce, subs,
                                                                          (unsigned)g.S_max * (unsigned)subs, scores);
     return cudaGetLastError();
