@@ -24,7 +24,9 @@ namespace {
 using namespace walk;
 
 constexpr int kRing = 64;           // group descriptors kept per warp
-constexpr int kScoreStage = 4096;   // two items: 2 x (128 B of bitmaps + 16 r_k B of values), or 2 x 2048 B dense
+constexpr int kScoreStage = 2176;   // one item of any r_k (<= 128 + 16 * 127 B), or two items with r_k <= kPairMaxR
+constexpr int kItem1 = 1024;        // stage offset of the second item of a pair
+constexpr uint32_t kPairMaxR = 56;  // 128 + 16 r_k <= kItem1
 
 // One group: <= 2 consecutive items (8 block keys each) of one unit with the same r_k.
 struct __align__(16) SDesc {
@@ -108,7 +110,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             }
         }
         const uint32_t pu = __shfl_up_sync(kFull, u, 1), prk = __shfl_up_sync(kFull, r_k, 1), pnb = __shfl_up_sync(kFull, nb, 1);
-        const bool follows = lane > 0 && nb != 0u && pnb != 0u && u == pu && r_k == prk && (r_k == (uint32_t)kD || r_k <= 120u);  // two items must fit one stage
+        const bool follows = lane > 0 && nb != 0u && pnb != 0u && u == pu && r_k == prk && r_k <= kPairMaxR;  // two items must fit one stage
         const unsigned fm = __ballot_sync(kFull, follows);
         const int start = 31 - __clz((int)(~fm & lanemask_le()));  // first item of this lane's run (bit 0 of ~fm is set)
         const bool first = nb != 0u && ((lane - start) & 1) == 0;
@@ -145,8 +147,8 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             mbar_expect_tx(bar, bb0 + vb0 + bb1 + vb1);
             bulk_g2s(dst, slice + ((unsigned long long)d.bm0 << 4), bb0, bar);
             if (vb0) bulk_g2s(dst + bb0, slice + ((unsigned long long)d.val0 << 4), vb0, bar);
-            if (bb1) bulk_g2s(dst + 2048, slice + ((unsigned long long)d.bm1 << 4), bb1, bar);
-            if (vb1) bulk_g2s(dst + 2048 + bb1, slice + ((unsigned long long)d.val1 << 4), vb1, bar);
+            if (bb1) bulk_g2s(dst + kItem1, slice + ((unsigned long long)d.bm1 << 4), bb1, bar);
+            if (vb1) bulk_g2s(dst + kItem1 + bb1, slice + ((unsigned long long)d.val1 << 4), vb1, bar);
         }
         ++gposi;
     };
@@ -176,7 +178,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                 }
             }
             const int r_k = (int)(d.meta & 255u), nb0 = (int)((d.meta >> 8) & 15u), nb1 = (int)((d.meta >> 12) & 15u);
-            const uint32_t sp0 = stage0 + s * kScoreStage, sp1 = sp0 + 2048;
+            const uint32_t sp0 = stage0 + s * kScoreStage, sp1 = sp0 + kItem1;
 
             mbar_wait(bar0 + 8 * s, parity);  // the group's bulk copies have landed
 
@@ -266,13 +268,13 @@ cudaError_t launch_score(const CacheGeom& g, const LayerView& lv, const uint16_t
     static int cfg = -1;  // tuning knob (stages * 100 + warps); default chosen from measurements
     if (cfg < 0) {
         const char* e = getenv("MKV_SCORE_CFG");
-        cfg = e ? atoi(e) : 316;
+        cfg = e ? atoi(e) : 232;
     }
 #define MKV_CFG(S, W) \
     case S * 100 + W: return launch_score_cfg<S, W>(g, lv, q, reduce, scores, sm_count, s);
     switch (cfg) {
-        MKV_CFG(3, 16) MKV_CFG(2, 16) MKV_CFG(4, 12) MKV_CFG(4, 8) MKV_CFG(6, 8)
-        default: return launch_score_cfg<3, 16>(g, lv, q, reduce, scores, sm_count, s);
+        MKV_CFG(2, 32) MKV_CFG(3, 24) MKV_CFG(2, 24) MKV_CFG(3, 16) MKV_CFG(4, 16)
+        default: return launch_score_cfg<2, 32>(g, lv, q, reduce, scores, sm_count, s);
     }
 #undef MKV_CFG
 }
