@@ -28,6 +28,9 @@ METRIC = "PackedAttention us/layer (8B-shape, 128K ctx, batch 8)"
 UNIT = "us/layer"
 NOMINAL_HBM_GBS = 8000.0
 FALLBACK_HBM_GBS = 6650.0
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+# (profiles/r1c_attention_v3.md), valid for the full-size default workload only
+NCU_TRAFFIC = {"llama8b-128k-b8": {"attention": 53390592 + 342784, "score+topk": 115576832 + 4862720 + 4227328}}
 
 
 def parse():
@@ -242,6 +245,8 @@ def run_mkv(args):
     comp_ms = np.array(built.compress_ms[1:] or built.compress_ms).mean(axis=0)
     comp_gbs = (comp_bytes["read"] + comp_bytes["write"]) / (comp_ms[2] * 1e-3) / 1e9
 
+    full_size = Bt == w.batch and N == w.context
+    traffic = NCU_TRAFFIC.get(w.name, {}) if full_size else {}
     line = {
         "metric": METRIC, "value": round(us_attn, 3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": False, "scaling": "weak",
@@ -255,11 +260,12 @@ def run_mkv(args):
         "decode_tokens_per_s_attention_only": round(world * Bt / (ms_step * 1e-3), 1),
         "select_us_per_layer": round(us_sel, 3),
         "roofline": {"kernel": "mkv_packed_attention", "bound": "hbm", "achieved": round(attn_gbs, 1), "peak": peak,
-                     "unit": "GB/s", "frac": round(attn_gbs / peak, 4), "traffic": None, "peak_source": peak_src,
+                     "unit": "GB/s", "frac": round(attn_gbs / peak, 4), "traffic": traffic.get("attention"),
+                     "peak_source": peak_src,
                      "frac_of_nominal_8TBs": round(attn_gbs / NOMINAL_HBM_GBS, 4),
                      "algorithmic_bytes_per_launch": int(a_bytes)},
         "roofline_select": {"kernel": "mkv_select", "bound": "hbm", "achieved": round(sel_gbs, 1), "peak": peak,
-                            "unit": "GB/s", "frac": round(sel_gbs / peak, 4), "traffic": None,
+                            "unit": "GB/s", "frac": round(sel_gbs / peak, 4), "traffic": traffic.get("score+topk"),
                             "algorithmic_bytes_per_launch": int(s_bytes)},
         "compress": {"loss_ms_per_layer": round(float(comp_ms[0]), 3), "strategy_ms_per_layer": round(float(comp_ms[1]), 3),
                      "compress_ms_per_layer": round(float(comp_ms[2]), 3), "achieved": round(comp_gbs, 1), "unit": "GB/s",

@@ -21,10 +21,12 @@
 //     layout with movmatrix.  Dense vectors (r = D) skip the walk: their fragments are 16-byte
 //     shared loads.
 //   * Step 3d (split-K combine) is fused: a unit wholly inside one warp's range is normalised and
-//     written directly; otherwise the warp leaves an (m, l, O) partial (<= 2 per warp), every
-//     thread of the CTA folds the partials of a unit for its own output element with the LSE rule,
-//     and a unit that spans several CTAs is finished by the last CTA to arrive at a per-unit
-//     ticket (no second kernel).
+//     written directly; otherwise the warp leaves a (ref, l, O) partial (<= 2 per warp), the
+//     threads of the CTA fold the partials of a unit (four output channels each, straight-line
+//     code) with the LSE rule, and a unit that spans several CTAs is finished by the last CTA to
+//     arrive at a per-unit ticket (no second kernel).
+//   * Softmax is lazy: 2^(s - ref) with a reference that moves only when a score exceeds it by
+//     more than 60 (log2 units); the common group needs no max reduction and no rescale.
 #include <cstdlib>
 
 #include "mkv_internal.cuh"
