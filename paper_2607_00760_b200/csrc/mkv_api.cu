@@ -52,6 +52,8 @@ struct mkv_cache {
     uint32_t* dev_flags = nullptr;
     unsigned long long* call_base = nullptr;  // [n_units]
     float* scores = nullptr;                  // [n_units][score_stride]
+    uint32_t* cand_key = nullptr;             // [n_units][slices * kTopkSlice]  top-k candidates of long units
+    int32_t* cand_idx = nullptr;
     AttnScratch attn{};
     uint16_t* q_dev = nullptr;
     int32_t* sel_dev = nullptr;
@@ -91,7 +93,7 @@ int mkv_cache_free(mkv_cache* c) {
     cudaSetDevice(c->desc.device);
     cudaDeviceSynchronize();
     void* ptrs[] = {c->arena, c->strat, c->tok_off, c->bk_off, c->unit_nseg, c->unit_ntok, c->counters,
-                    c->dev_flags, c->call_base, c->scores, c->attn.part_o, c->attn.part_ml, c->attn.ticket, c->q_dev,
+                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->attn.part_o, c->attn.part_ml, c->attn.ticket, c->q_dev,
                     c->sel_dev, c->selcnt_dev, c->out_dev, c->cands_dev};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -136,6 +138,8 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     const size_t tu = (size_t)g.n_layers * g.n_units;
     c->attn.slots = attention_partial_slots(c->sm_count);
     c->sel_cap = g.score_stride + 1;
+    const int topk_slices = (g.score_stride + kTopkSlice - 1) / kTopkSlice;
+    const size_t cand_bytes = topk_slices > 1 ? (size_t)g.n_units * topk_slices * kTopkSlice * 4 : 256;
     struct { void** p; size_t bytes; } allocs[] = {
         {(void**)&c->arena, (size_t)per_layer * g.n_layers},
         {(void**)&c->strat, tu * g.S_max * sizeof(StratRec)},
@@ -147,6 +151,8 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         {(void**)&c->dev_flags, 256},
         {(void**)&c->call_base, (size_t)g.n_units * 8},
         {(void**)&c->scores, (size_t)g.n_units * g.score_stride * 4},
+        {(void**)&c->cand_key, cand_bytes},
+        {(void**)&c->cand_idx, cand_bytes},
         {(void**)&c->attn.part_o, (size_t)c->attn.slots * g.group * kD * 4},
         {(void**)&c->attn.part_ml, (size_t)c->attn.slots * kMaxGroup * 2 * 4},
         {(void**)&c->attn.ticket, (size_t)g.n_units * 4},
@@ -283,7 +289,8 @@ int mkv_select(const mkv_cache* cc, int32_t layer, const void* q, int32_t budget
         return fail(MKV_E_ARG, "mkv_select: k_max %d too small for budget %d", k_max, budget);
     MKV_CUDA(cudaSetDevice(c->desc.device));
     MKV_CUDA(launch_select(g, c->view(layer), (const uint16_t*)q, budget, reduce, sel, sel_count, k_max,
-                           scores_opt ? scores_opt : c->scores, c->sm_count, (cudaStream_t)stream, &c->last_select));
+                           scores_opt ? scores_opt : c->scores, c->cand_key, c->cand_idx, c->sm_count, (cudaStream_t)stream,
+                           &c->last_select));
     return MKV_OK;
 }
 

@@ -81,7 +81,8 @@ cudaError_t launch_score(const CacheGeom& g, const LayerView& lv, const uint16_t
                          float* scores, int sm_count, cudaStream_t s);
 cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_t* q, int budget,
                           int reduce, int32_t* sel, int32_t* sel_count, int k_max, float* scores,
-                          int sm_count, cudaStream_t s, int* n_kernels);
+                          uint32_t* cand_key, int32_t* cand_idx, int sm_count, cudaStream_t s, int* n_kernels);
+constexpr int kTopkSlice = 16384;  // blocks per top-k slice (select.cu); longer units are selected in two stages
 
 struct AttnScratch {
     float* part_o;    // [slots][G][D]   unnormalised partial outputs (<= 2 slots per warp and per CTA of the grid)

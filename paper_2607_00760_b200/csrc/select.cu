@@ -33,33 +33,56 @@ __device__ __forceinline__ uint32_t score_key(float s) {
 // few bins of the first pass); the emission gives every thread a run of consecutive blocks, so one
 // block-wide scan of packed (greater, equal) counts orders the whole output.
 constexpr int kKeyCap = 16384;  // 64 KB of keys
+static_assert(kKeyCap == kTopkSlice, "the candidate scratch of mkv_api.cu is sized in slices of kKeyCap blocks");
 
+// MODE 0: the whole unit in one CTA (nblk <= kKeyCap, or any size with uncached keys).
+// Long units (score_stride > kKeyCap, e.g. 1M tokens) are selected in two stages so that every
+// key is read from global memory once and all SMs take part:
+// MODE 1: CTA (unit, p) keeps the kq_cap best blocks of slice p (kKeyCap blocks) as candidates
+//         (order-preserving key + block index, ascending index, padded with key 0);
+// MODE 2: one CTA per unit runs the same selection over the concatenated candidates.  The kq best
+//         of the unit are among the kq best of their slices, and positions stay in index order.
+template <int MODE>
 __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView lv, const float* __restrict__ scores,
                                                         int budget, int32_t* __restrict__ sel,
-                                                        int32_t* __restrict__ sel_count, int k_max) {
+                                                        int32_t* __restrict__ sel_count, int k_max,
+                                                        uint32_t* __restrict__ cand_key, int32_t* __restrict__ cand_idx,
+                                                        int n_slices, int cand_cap) {
     extern __shared__ uint32_t s_keys[];  // key i at [i + i / 32]: conflict-free for strided and for per-thread runs
-    const int unit = blockIdx.x;
+    const int unit = MODE == 1 ? blockIdx.x / n_slices : blockIdx.x;
+    const int slice = MODE == 1 ? blockIdx.x % n_slices : 0;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int ntok = lv.unit_ntok[unit];
-    const int nblk = (ntok + kB - 1) / kB;
+    const int nblk = (ntok + kB - 1) / kB;        // blocks of the unit
     const float* s = scores + (size_t)unit * g.score_stride;
-    int32_t* out = sel + (size_t)unit * k_max;
-    const bool cached = nblk <= kKeyCap;
+    // the elements this CTA selects from: n of them; element i has key keyat(i) and block index idxat(i)
+    const int base = MODE == 1 ? slice * kKeyCap : 0;
+    const int n = MODE == 0 ? nblk : (MODE == 1 ? max(0, min(kKeyCap, nblk - base)) : n_slices * cand_cap);
+    const uint32_t* ck = MODE == 2 ? cand_key + (size_t)unit * n_slices * cand_cap : nullptr;
+    const int32_t* ci = MODE == 2 ? cand_idx + (size_t)unit * n_slices * cand_cap : nullptr;
+    auto keyat = [&](int i) -> uint32_t { return MODE == 2 ? ck[i] : score_key(s[base + i]); };
+    auto idxat = [&](int i) -> int { return MODE == 2 ? ci[i] : base + i; };
+    int32_t* out = MODE == 1 ? nullptr : sel + (size_t)unit * k_max;
+    uint32_t* okey = MODE == 1 ? cand_key + ((size_t)unit * n_slices + slice) * cand_cap : nullptr;
+    int32_t* oidx = MODE == 1 ? cand_idx + ((size_t)unit * n_slices + slice) * cand_cap : nullptr;
+    const int cap = MODE == 1 ? cand_cap : k_max;
+    const bool cached = n <= kKeyCap;
 
     __shared__ unsigned hist[4096];
     __shared__ uint32_t s_prefix;
     __shared__ int s_krem, s_neq;
     __shared__ unsigned long long s_warp[32];
 
-    const bool all = (ntok <= budget);
     const int k0 = budget / kB, rem = budget % kB, nbR = ntok % kB;
-    const bool ragged_try = !all && nbR != 0 && nbR <= rem;
-    int kq = all ? nblk : (ragged_try ? k0 + 1 : k0);  // rank whose key we look for
+    // MODE 1 keeps k0 + 1 per slice (the most the final stage can ask for); every element if fewer
+    const bool all = MODE == 1 ? (n <= k0 + 1) : (ntok <= budget);
+    const bool ragged_try = MODE != 1 && !all && nbR != 0 && nbR <= rem;
+    int kq = MODE == 1 ? min(n, k0 + 1) : (all ? nblk : (ragged_try ? k0 + 1 : k0));  // rank whose key we look for
     uint32_t Ts = 0;
     int take_eq = 0;
     if (!all && kq > 0) {
         if (cached)
-            for (int i = tid; i < nblk; i += 1024) s_keys[i + (i >> 5)] = score_key(s[i]);
+            for (int i = tid; i < n; i += 1024) s_keys[i + (i >> 5)] = keyat(i);
         uint32_t prefix = 0;
         int krem = kq;
         // MSB-first radix select in three passes of 12 + 12 + 8 bits: with 4096 bins the scores spread
@@ -70,8 +93,8 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
             for (int i = tid; i < nbins; i += 1024) hist[i] = 0;
             __syncthreads();  // also orders the fill of s_keys before the first pass
             const uint32_t hi_mask = pass == 0 ? 0u : (0xffffffffu << (pass == 1 ? 20 : 8));
-            for (int i = tid; i < nblk; i += 1024) {
-                const uint32_t u = cached ? s_keys[i + (i >> 5)] : score_key(s[i]);
+            for (int i = tid; i < n; i += 1024) {
+                const uint32_t u = cached ? s_keys[i + (i >> 5)] : keyat(i);
                 if ((u & hi_mask) == prefix) atomicAdd(&hist[(u >> shift) & (uint32_t)(nbins - 1)], 1u);
             }
             __syncthreads();
@@ -119,26 +142,39 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
         }
         Ts = prefix;
         take_eq = krem;            // equals (by ascending index) inside the kq best
-        const int n_eq = s_neq;    // all blocks whose score equals the threshold score
+        const int n_eq = s_neq;    // all elements whose key equals the threshold key
         if (ragged_try) {
             // the short block is the highest index: it is inside the k0+1 best iff it beats Ts or
-            // ties with it and every tie is taken
+            // ties with it and every tie is taken (MODE 2: and it survived as a candidate, i.e. it is
+            // the last real candidate of the last slice)
             const uint32_t uR = score_key(s[nblk - 1]);
-            const bool inside = (uR > Ts) || (uR == Ts && take_eq == n_eq);
+            bool is_elem = true;
+            if (MODE == 2) {
+                const int ls = (nblk - 1) / kKeyCap;  // its slice; real candidates come first in a slice
+                int lo = 0, hi = cand_cap;            // first padding entry of the slice, by bisection
+                while (lo < hi) {
+                    const int mid = (lo + hi) >> 1;
+                    if (ci[ls * cand_cap + mid] >= 0) lo = mid + 1; else hi = mid;
+                }
+                is_elem = lo > 0 && ci[ls * cand_cap + lo - 1] == nblk - 1;
+            }
+            const bool inside = (uR > Ts) || (uR == Ts && take_eq == n_eq && is_elem);
             if (!inside) { take_eq -= 1; kq = k0; }
         }
     }
 
-    // emission in ascending block index: thread t owns blocks [t E, (t+1) E)
+    // emission in ascending position (= ascending block index): thread t owns elements [t E, (t+1) E)
     int count = 0;
     if (kq > 0) {
-        const int E = (nblk + 1023) / 1024;
-        const int i0 = min(nblk, tid * E), i1 = min(nblk, i0 + E);
-        unsigned long long mine = 0;  // greater | equal << 32 among this thread's blocks
-        if (all) mine = (unsigned long long)(i1 - i0);
-        else
+        const int E = (n + 1023) / 1024;
+        const int i0 = min(n, tid * E), i1 = min(n, i0 + E);
+        unsigned long long mine = 0;  // greater | equal << 32 among this thread's elements
+        if (all) {
+            if (MODE == 2) { for (int i = i0; i < i1; ++i) mine += ci[i] >= 0 ? 1ull : 0ull; }
+            else mine = (unsigned long long)(i1 - i0);
+        } else
             for (int i = i0; i < i1; ++i) {
-                const uint32_t u = cached ? s_keys[i + (i >> 5)] : score_key(s[i]);
+                const uint32_t u = cached ? s_keys[i + (i >> 5)] : keyat(i);
                 mine += (u > Ts ? 1ull : 0ull) + (u == Ts ? (1ull << 32) : 0ull);
             }
         // block-wide exclusive scan of the packed counts
@@ -164,43 +200,64 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
         __syncthreads();
         const unsigned long long before = s_warp[warp] + incl - mine;
         int gt_before = (int)(uint32_t)before, eq_before = (int)(before >> 32);
-        count = all ? nblk : s_krem;
+        count = s_krem;
         for (int i = i0; i < i1; ++i) {
             bool gt = all, eq = false;
-            if (!all) {
-                const uint32_t u = cached ? s_keys[i + (i >> 5)] : score_key(s[i]);
+            if (all) {
+                if (MODE == 2) gt = ci[i] >= 0;
+            } else {
+                const uint32_t u = cached ? s_keys[i + (i >> 5)] : keyat(i);
                 gt = u > Ts;
                 eq = u == Ts;
             }
             const bool take = gt || (eq && eq_before < take_eq);
             const int pos = gt_before + min(eq_before, take_eq);
-            if (take && pos < k_max) out[pos] = i * kB;
+            if (take && pos < cap) {
+                if (MODE == 1) { okey[pos] = keyat(i); oidx[pos] = idxat(i); }
+                else out[pos] = idxat(i) * kB;
+            }
             gt_before += gt ? 1 : 0;
             eq_before += eq ? 1 : 0;
         }
     }
-    count = min(count, k_max);
-    for (int p = count + tid; p < k_max; p += 1024) out[p] = -1;
-    if (tid == 0) sel_count[unit] = count;
+    count = min(count, cap);
+    if (MODE == 1) {
+        for (int p = count + tid; p < cap; p += 1024) { okey[p] = 0u; oidx[p] = -1; }  // padding: below every real key
+    } else {
+        for (int p = count + tid; p < k_max; p += 1024) out[p] = -1;
+        if (tid == 0) sel_count[unit] = count;
+    }
 }
 
 }  // namespace
 
 cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_t* q, int budget, int reduce,
-                          int32_t* sel, int32_t* sel_count, int k_max, float* scores, int sm_count,
-                          cudaStream_t s, int* n_kernels) {
+                          int32_t* sel, int32_t* sel_count, int k_max, float* scores, uint32_t* cand_key,
+                          int32_t* cand_idx, int sm_count, cudaStream_t s, int* n_kernels) {
     cudaError_t err = launch_score(g, lv, q, reduce, scores, sm_count, s);
     if (err != cudaSuccess) return err;
-    const int n_keys = g.score_stride < kKeyCap ? g.score_stride : kKeyCap;
+    const int n_slices = (g.score_stride + kKeyCap - 1) / kKeyCap;
+    const int cand_cap = budget / kB + 1 < kKeyCap ? budget / kB + 1 : kKeyCap;  // candidates kept per slice
+    const int n_keys = n_slices > 1 ? kKeyCap : g.score_stride;
     const int key_bytes = 4 * (n_keys + n_keys / 32 + 1);
     static int configured = 0;
     if (key_bytes > configured) {
-        err = cudaFuncSetAttribute(mkv_topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, key_bytes);
-        if (err != cudaSuccess) return err;
+        if ((err = cudaFuncSetAttribute(mkv_topk_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, key_bytes)) != cudaSuccess) return err;
+        if ((err = cudaFuncSetAttribute(mkv_topk_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, key_bytes)) != cudaSuccess) return err;
+        if ((err = cudaFuncSetAttribute(mkv_topk_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, key_bytes)) != cudaSuccess) return err;
         configured = key_bytes;
     }
-    mkv_topk_kernel<<<g.n_units, 1024, key_bytes, s>>>(g, lv, scores, budget, sel, sel_count, k_max);
-    if (n_kernels) *n_kernels = 2;
+    if (n_slices == 1) {
+        mkv_topk_kernel<0><<<g.n_units, 1024, key_bytes, s>>>(g, lv, scores, budget, sel, sel_count, k_max, nullptr, nullptr, 1, 0);
+        if (n_kernels) *n_kernels = 2;
+    } else {
+        mkv_topk_kernel<1><<<g.n_units * n_slices, 1024, key_bytes, s>>>(g, lv, scores, budget, sel, sel_count, k_max,
+                                                                         cand_key, cand_idx, n_slices, cand_cap);
+        if ((err = cudaGetLastError()) != cudaSuccess) return err;
+        mkv_topk_kernel<2><<<g.n_units, 1024, key_bytes, s>>>(g, lv, scores, budget, sel, sel_count, k_max, cand_key,
+                                                              cand_idx, n_slices, cand_cap);
+        if (n_kernels) *n_kernels = 3;
+    }
     return cudaGetLastError();
 }
 

@@ -230,6 +230,35 @@ def test_select_with_massive_ties(env):
         c.free()
 
 
+def test_select_long_unit_two_stage(env):
+    """a unit of more than 16384 blocks is selected in two stages (per-slice candidates, then a merge);
+    ragged last block, budgets around the slice size and the ragged rule, then massive ties"""
+    mkv, dev = env
+    N = 8 * (2 * 16384 + 300) + 5
+    c = Case(mkv, dev, 1, 1, 4, N, seed=47)
+    try:
+        strat = uniform_strat(1, 1, c.S, 38)
+        strat[:, :, ::9, 0:2] = 128
+        c.compress(strat)
+        tot = sw = 0
+        for budget in (0, 8, 1000, 1005, 4096, 8 * 16384 + 3, 8 * 16385 + 5, c.N - 1, c.N):
+            t, s = c.check_select(budget)
+            tot += t
+            sw += s
+        assert sw <= max(1, tot // 10000)
+        c.K[:] = c.K[:, :, :1, :]  # every block key identical: ties cut inside a slice, lower index wins
+        c.k_d = to_dev(c.K, dev)
+        c.cache.reset()
+        c.compress(uniform_strat(1, 1, c.S, 38))
+        for budget in (8 * 100, 8 * 16384 + 8 * 77, 8 * 20000 + 5):
+            sel, cnt, _ = c.gpu_select(budget)
+            k = budget // 8
+            assert cnt[0, 0] == k
+            np.testing.assert_array_equal(sel[0, 0, :k], np.arange(k) * 8)
+    finally:
+        c.free()
+
+
 # ------------------------------------------------------------------ step 3
 
 @pytest.mark.parametrize("Hq,Hkv,r", [(8, 2, 38), (28, 4, 38), (4, 4, 90), (8, 1, 128), (8, 2, 1)])
