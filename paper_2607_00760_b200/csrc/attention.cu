@@ -488,45 +488,58 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     const int tid = threadIdx.x;
     int sh_u0 = -1, sh_u1 = -1;  // units this CTA shares with others (<= 2: one entering, one leaving its range)
     int n_shared = 0;
+    // GD / 4 threads fold one unit (four consecutive channels of one head each), so a CTA folds
+    // kNT / (GD / 4) units side by side: usually all of them (1 or 2 per CTA) in one pass.
+    const int tpr = GD / 4, nslots = max(1, kNT / tpr);
+    const int rs = tid / tpr, e = 4 * (tid - rs * tpr), h = e >> 7;
     int run = -1;
 #pragma unroll 1
-    for (;;) {  // one unit with partial records at a time, in ascending order (usually 1 or 2 per CTA)
-        int nxt = 0x7fffffff;
-        bool any_head = false;
-#pragma unroll
-        for (int r = 0; r < kRec; ++r) {
-            const int u = s_unit[r];
-            if (u > run) nxt = min(nxt, u);
-        }
-        if (nxt == 0x7fffffff) break;
-        run = nxt;
-#pragma unroll
-        for (int w = 0; w < kWarps; ++w) any_head |= s_unit[2 * w] == run;
-        const int a = s_cum[run], b = s_cum[run + 1];
-        const bool whole = clo <= a && b <= chi;
-        const size_t row = (size_t)(run / g.n_kv_heads) * g.n_q_heads + (size_t)(run % g.n_kv_heads) * G;
-        const size_t slot = cta_slot_base + blockIdx.x * 2 + (a < clo ? 0 : 1);
+    for (;;) {
+        // the next <= nslots units with partial records, ascending; `mine` = the one this thread folds
+        int mine = -1, last = run;
 #pragma unroll 1
-        for (int e = 4 * tid; e < GD; e += 4 * kNT) {  // four consecutive channels of one head per thread
-            const int h = e >> 7;
+        for (int k = 0; k < nslots; ++k) {
+            int nxt = 0x7fffffff;
+#pragma unroll
+            for (int r = 0; r < kRec; ++r) {
+                const int u = s_unit[r];
+                if (u > last) nxt = min(nxt, u);
+            }
+            if (nxt == 0x7fffffff) break;
+            last = nxt;
+            if (k == rs) mine = nxt;
+            if (!(clo <= s_cum[nxt] && s_cum[nxt + 1] <= chi) && n_shared < 2) {  // shared with other CTAs
+                if (tid == 0) s_row[n_shared] = (size_t)(nxt / g.n_kv_heads) * g.n_q_heads + (size_t)(nxt % g.n_kv_heads) * G;
+                if (n_shared == 0) sh_u0 = nxt; else sh_u1 = nxt;
+                ++n_shared;
+            }
+        }
+        if (last == run) break;
+        run = last;
+        if (mine < 0) continue;
+        unsigned heads = 0u;  // warps that hold a head partial (record 2w, in global scratch) of this unit: rare
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) heads |= (s_unit[2 * w] == mine ? 1u : 0u) << w;
+        const int a = s_cum[mine], b = s_cum[mine + 1];
+        const bool whole = clo <= a && b <= chi;
+        const size_t row = (size_t)(mine / g.n_kv_heads) * g.n_q_heads + (size_t)(mine % g.n_kv_heads) * G;
+        const size_t slot = cta_slot_base + blockIdx.x * 2 + (a < clo ? 0 : 1);
+        {
             // tail partials (record 2w + 1, in warp w's shared memory): straight-line, every load independent
             float mw[kWarps], lw[kWarps];
             float4 ow[kWarps];
             float Mr = -INFINITY;
 #pragma unroll
             for (int w = 0; w < kWarps; ++w) {
-                const bool mem = s_unit[2 * w + 1] == run;
+                const bool mem = s_unit[2 * w + 1] == mine;
                 const float m = s_ml[2 * w + 1][h][0], l = s_ml[2 * w + 1][h][1];
                 ow[w] = *reinterpret_cast<const float4*>(smem + w * kWS + 4 * e);
                 mw[w] = mem ? m : -INFINITY;
                 lw[w] = mem ? l : 0.f;
                 Mr = fmaxf(Mr, mw[w]);
             }
-            if (any_head) {  // rare: a head partial (record 2w, in global scratch) of this unit
 #pragma unroll 1
-                for (int w = 0; w < kWarps; ++w)
-                    if (s_unit[2 * w] == run) Mr = fmaxf(Mr, s_ml[2 * w][h][0]);
-            }
+            for (unsigned m = heads; m; m &= m - 1u) Mr = fmaxf(Mr, s_ml[2 * (__ffs(m) - 1)][h][0]);
             const float Mb = Mr == -INFINITY ? 0.f : Mr;
             float4 O = make_float4(0.f, 0.f, 0.f, 0.f);
             float Lr = 0.f;
@@ -536,16 +549,14 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 Lr = fmaf(lw[w], wt, Lr);
                 if (wt != 0.f) { O.x = fmaf(ow[w].x, wt, O.x); O.y = fmaf(ow[w].y, wt, O.y); O.z = fmaf(ow[w].z, wt, O.z); O.w = fmaf(ow[w].w, wt, O.w); }
             }
-            if (any_head) {
 #pragma unroll 1
-                for (int w = 0; w < kWarps; ++w)
-                    if (s_unit[2 * w] == run) {
-                        const float wt = ex2(s_ml[2 * w][h][0] - Mb);
-                        Lr = fmaf(s_ml[2 * w][h][1], wt, Lr);
-                        const float4 o = __ldcg(reinterpret_cast<const float4*>(
-                            part_o + ((size_t)blockIdx.x * kWarps + w) * 2 * (size_t)GD + e));
-                        O.x = fmaf(o.x, wt, O.x); O.y = fmaf(o.y, wt, O.y); O.z = fmaf(o.z, wt, O.z); O.w = fmaf(o.w, wt, O.w);
-                    }
+            for (unsigned m = heads; m; m &= m - 1u) {
+                const int w = __ffs(m) - 1;
+                const float wt = ex2(s_ml[2 * w][h][0] - Mb);
+                Lr = fmaf(s_ml[2 * w][h][1], wt, Lr);
+                const float4 o = __ldcg(reinterpret_cast<const float4*>(
+                    part_o + ((size_t)blockIdx.x * kWarps + w) * 2 * (size_t)GD + e));
+                O.x = fmaf(o.x, wt, O.x); O.y = fmaf(o.y, wt, O.y); O.z = fmaf(o.z, wt, O.z); O.w = fmaf(o.w, wt, O.w);
             }
             if (whole) {
                 const float inv = Lr > 0.f ? 1.f / Lr : 0.f;
@@ -558,11 +569,6 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                     part_ml[slot * (2 * kMaxGroup) + 2 * h + 1] = Lr;
                 }
             }
-        }
-        if (!whole && n_shared < 2) {
-            if (tid == 0) s_row[n_shared] = row;
-            if (n_shared == 0) sh_u0 = run; else sh_u1 = run;
-            ++n_shared;
         }
     }
     MKV_T(2);
@@ -578,56 +584,50 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         if (s_cum[u] < clo) cf = (int)cs.owner((unsigned)s_cum[u]);
         if (s_cum[u + 1] > chi) cl = (int)cs.owner((unsigned)s_cum[u + 1] - 1u);
         s_cf[k] = cf; s_cl[k] = cl;
-        asm volatile("fence.acq_rel.gpu;" ::: "memory");
-        const int old = atomicAdd(&ticket[u], 1);
-        asm volatile("fence.acq_rel.gpu;" ::: "memory");  // the other sharers' partials are acquired
+        int old;  // release this CTA's partial (ordered by the barrier), acquire the other sharers'
+        asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(ticket + u) : "memory");
         s_last[k] = old == cl - cf;
         if (old == cl - cf) ticket[u] = 0;  // self-cleaning: every sharer has arrived
     }
     __syncthreads();
     MKV_T(3);
+    // last arrivers: thread group rs merges the CTA partials of shared unit rs (read with ld.global.cg: L2,
+    // never a stale L1 line); with nslots = 1 (G = 8 on a small CTA) the groups take the units in turn
 #pragma unroll 1
-    for (int k = 0; k < n_shared; ++k) {
-        if (!s_last[k]) continue;  // uniform over the CTA
-        // last arriver: merge the CTA partials (read with ld.global.cg: L2, never a stale L1 line)
+    for (int k = rs < nslots ? rs : n_shared; k < n_shared; k += nslots) {
+        if (!s_last[k]) continue;
         const int c_first = s_cf[k], c_last = s_cl[k];
         const size_t row = s_row[k];
+        float Mx = -INFINITY, Lx = 0.f;
+        float4 Ox = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 1
-        for (int e = 4 * tid; e < GD; e += 4 * kNT) {
-            const int h = e >> 7;
-            float Mx = -INFINITY, Lx = 0.f;
-            float4 Ox = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll 1
-            for (int c0 = c_first; c0 <= c_last; c0 += 4) {  // four partials' loads in flight at once
-                float pm[4], pl[4];
-                float4 po[4];
+        for (int c0 = c_first; c0 <= c_last; c0 += 4) {  // four partials' loads in flight at once
+            float pm[4], pl[4];
+            float4 po[4];
 #pragma unroll
-                for (int t = 0; t < 4; ++t) {
-                    const int c = c0 + t;
-                    pm[t] = -INFINITY; pl[t] = 0.f; po[t] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (c <= c_last) {
-                        const size_t sl = cta_slot_base + (size_t)c * 2 + (c == c_first ? 1 : 0);
-                        pm[t] = __ldcg(part_ml + sl * (2 * kMaxGroup) + 2 * h);
-                        pl[t] = __ldcg(part_ml + sl * (2 * kMaxGroup) + 2 * h + 1);
-                        po[t] = __ldcg(reinterpret_cast<const float4*>(part_o + sl * (size_t)GD + e));
-                    }
-                }
-                const float Mn = fmaxf(fmaxf(Mx, fmaxf(pm[0], pm[1])), fmaxf(pm[2], pm[3]));
-                const float Mb = Mn == -INFINITY ? 0.f : Mn;
-                const float c_old = ex2(Mx - Mb);
-                Lx *= c_old; Ox.x *= c_old; Ox.y *= c_old; Ox.z *= c_old; Ox.w *= c_old; Mx = Mn;
-#pragma unroll
-                for (int t = 0; t < 4; ++t) {
-                    const float w = ex2(pm[t] - Mb);
-                    Lx = fmaf(pl[t], w, Lx);
-                    Ox.x = fmaf(po[t].x, w, Ox.x); Ox.y = fmaf(po[t].y, w, Ox.y);
-                    Ox.z = fmaf(po[t].z, w, Ox.z); Ox.w = fmaf(po[t].w, w, Ox.w);
-                }
+            for (int t = 0; t < 4; ++t) {
+                const int c = min(c0 + t, c_last);  // a repeated partial gets weight 0 below
+                const size_t sl = cta_slot_base + (size_t)c * 2 + (c == c_first ? 1 : 0);
+                pm[t] = __ldcg(part_ml + sl * (2 * kMaxGroup) + 2 * h);
+                pl[t] = __ldcg(part_ml + sl * (2 * kMaxGroup) + 2 * h + 1);
+                po[t] = __ldcg(reinterpret_cast<const float4*>(part_o + sl * (size_t)GD + e));
+                if (c0 + t > c_last) { pm[t] = -INFINITY; pl[t] = 0.f; }
             }
-            const float inv = Lx > 0.f ? 1.f / Lx : 0.f;
-            *reinterpret_cast<float4*>(out + row * kD + e) = make_float4(Ox.x * inv, Ox.y * inv, Ox.z * inv, Ox.w * inv);
-            if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = Lx > 0.f ? (Mx + log2f(Lx)) * kLn2 : -INFINITY;
+            const float Mn = fmaxf(fmaxf(Mx, fmaxf(pm[0], pm[1])), fmaxf(pm[2], pm[3]));
+            const float Mb = Mn == -INFINITY ? 0.f : Mn;
+            const float c_old = ex2(Mx - Mb);
+            Lx *= c_old; Ox.x *= c_old; Ox.y *= c_old; Ox.z *= c_old; Ox.w *= c_old; Mx = Mn;
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+                const float w = ex2(pm[t] - Mb);
+                Lx = fmaf(pl[t], w, Lx);
+                Ox.x = fmaf(po[t].x, w, Ox.x); Ox.y = fmaf(po[t].y, w, Ox.y);
+                Ox.z = fmaf(po[t].z, w, Ox.z); Ox.w = fmaf(po[t].w, w, Ox.w);
+            }
         }
+        const float inv = Lx > 0.f ? 1.f / Lx : 0.f;
+        *reinterpret_cast<float4*>(out + row * kD + e) = make_float4(Ox.x * inv, Ox.y * inv, Ox.z * inv, Ox.w * inv);
+        if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = Lx > 0.f ? (Mx + log2f(Lx)) * kLn2 : -INFINITY;
     }
     MKV_T(4);
 }
