@@ -146,7 +146,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
 
     MKV_T(0);
     __shared__ int s_unit[kRec];                 // unit of each partial record, -1 = none
-    __shared__ float s_ml[kRec][kMaxGroup][2];   // its (max in log2 units, sum) per head
+    __shared__ __align__(8) float s_ml[kRec][kMaxGroup][2];   // its (max in log2 units, sum) per head
     __shared__ int s_last[2], s_cf[2], s_cl[2];
     __shared__ size_t s_row[2];
 
@@ -492,6 +492,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     // kNT / (GD / 4) units side by side: usually all of them (1 or 2 per CTA) in one pass.
     const int tpr = GD / 4, nslots = max(1, kNT / tpr);
     const int rs = tid / tpr, e = 4 * (tid - rs * tpr), h = e >> 7;
+    // each lane keeps the units of records lane and lane + 32: searches and membership are votes
+    const int myu0 = lane < kRec ? s_unit[lane] : -1, myu1 = lane + 32 < kRec ? s_unit[lane + 32] : -1;
     int run = -1;
 #pragma unroll 1
     for (;;) {
@@ -499,12 +501,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         int mine = -1, last = run;
 #pragma unroll 1
         for (int k = 0; k < nslots; ++k) {
-            int nxt = 0x7fffffff;
-#pragma unroll
-            for (int r = 0; r < kRec; ++r) {
-                const int u = s_unit[r];
-                if (u > last) nxt = min(nxt, u);
-            }
+            const int c0 = myu0 > last ? myu0 : 0x7fffffff, c1 = myu1 > last ? myu1 : 0x7fffffff;
+            const int nxt = __reduce_min_sync(kFull, min(c0, c1));
             if (nxt == 0x7fffffff) break;
             last = nxt;
             if (k == rs) mine = nxt;
@@ -516,10 +514,13 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         }
         if (last == run) break;
         run = last;
-        if (mine < 0) continue;
+        if (mine < 0) continue;  // uniform over a warp: GD / 4 is a multiple of 32
+        // records of this unit: bit r of `recs` (tail partials are the odd records, head partials the even ones)
+        const unsigned long long recs = (unsigned long long)__ballot_sync(kFull, myu0 == mine) |
+                                        ((unsigned long long)__ballot_sync(kFull, myu1 == mine) << 32);
         unsigned heads = 0u;  // warps that hold a head partial (record 2w, in global scratch) of this unit: rare
 #pragma unroll
-        for (int w = 0; w < kWarps; ++w) heads |= (s_unit[2 * w] == mine ? 1u : 0u) << w;
+        for (int w = 0; w < kWarps; ++w) heads |= (unsigned)((recs >> (2 * w)) & 1ull) << w;
         const int a = s_cum[mine], b = s_cum[mine + 1];
         const bool whole = clo <= a && b <= chi;
         const size_t row = (size_t)(mine / g.n_kv_heads) * g.n_q_heads + (size_t)(mine % g.n_kv_heads) * G;
@@ -531,11 +532,11 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             float Mr = -INFINITY;
 #pragma unroll
             for (int w = 0; w < kWarps; ++w) {
-                const bool mem = s_unit[2 * w + 1] == mine;
-                const float m = s_ml[2 * w + 1][h][0], l = s_ml[2 * w + 1][h][1];
+                const bool mem = (recs >> (2 * w + 1)) & 1ull;
+                const float2 ml = *reinterpret_cast<const float2*>(&s_ml[2 * w + 1][h][0]);
                 ow[w] = *reinterpret_cast<const float4*>(smem + w * kWS + 4 * e);
-                mw[w] = mem ? m : -INFINITY;
-                lw[w] = mem ? l : 0.f;
+                mw[w] = mem ? ml.x : -INFINITY;
+                lw[w] = mem ? ml.y : 0.f;
                 Mr = fmaxf(Mr, mw[w]);
             }
 #pragma unroll 1
