@@ -46,6 +46,8 @@ def parse():
     ap.add_argument("--no-graph", action="store_true", help="launch eagerly instead of CUDA graphs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-units", type=int, default=8, help="units of one layer the oracle is timed on")
+    ap.add_argument("--sweep", action="store_true",
+                    help="BASELINE config 5: keep ratio x token budget on the config-2 shape, 2 layers per point")
     ap.add_argument("--verbose", action="store_true")
     return ap.parse_args()
 
@@ -411,9 +413,70 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_sweep(args):
+    """BASELINE config 5 on one GPU: keep ratio in {1.0, 0.7, 0.5, 0.3} x token budget in {1024, 4096, 16384} (the 10 %
+    dense mix held fixed) plus the dense-full point (r = 128, budget = context).  Two layers per point so that
+    consecutive launches read different arenas (each far larger than L2).  Prints one JSON line."""
+    import dataclasses
+    import torch
+    import __graft_entry__
+    __graft_entry__.build()
+    from paper_2607_00760_b200 import synth, workload
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    base = synth.WORKLOADS[args.workload]
+    Bt, N = args.batch or base.batch, args.context or base.context
+    peak, peak_src = measured_peak()
+    scale = 1.0 / math.sqrt(128)
+    points = []
+    for keep in (1.0, 0.7, 0.5, 0.3):
+        w = dataclasses.replace(base, keep_ratio=keep)
+        built = workload.build(w, dev, n_layers=2, batch=Bt, context=N)
+        cache, Hkv, Hq = built.cache, w.n_kv_heads, w.n_q_heads
+        budgets = [1024, 4096, 16384] + ([N] if keep == 1.0 else [])
+        for budget in budgets:
+            k_max = min(budget // 8 + 1, (N + 7) // 8)
+            sel = [torch.full((Bt, Hkv, k_max), -1, dtype=torch.int32, device=dev) for _ in range(2)]
+            cnt = [torch.zeros((Bt, Hkv), dtype=torch.int32, device=dev) for _ in range(2)]
+            out = torch.zeros((2, Bt, Hq, 128), dtype=torch.float32, device=dev)
+            for l in range(2):
+                cache.select(l, built.q[l], budget, sel[l], cnt[l])
+            torch.cuda.synchronize()
+
+            def step_attention():
+                for l in range(2):
+                    cache.packed_attention(l, built.q[l], sel[l], cnt[l], scale, out[l])
+
+            def step_select():
+                for l in range(2):
+                    cache.select(l, built.q[l], budget, sel[l], cnt[l])
+
+            ms_a = timed_loop(torch, step_attention, args.steps, max(3, args.warmup), lambda: None, True)
+            ms_s = timed_loop(torch, step_select, args.steps, max(3, args.warmup), lambda: None, True)
+            cache.status()
+            ab = sum(workload.attention_bytes(built, l, sel[l], cnt[l]) for l in range(2)) / 2
+            us = ms_a * 1e3 / 2
+            gbs = ab / (us * 1e-6) / 1e9
+            points.append({"keep_ratio": keep, "r_keep": w.r_keep, "token_budget": budget,
+                           "attention_us_per_layer": round(us, 2), "select_us_per_layer": round(ms_s * 1e3 / 2, 2),
+                           "algorithmic_bytes_per_launch": int(ab), "achieved_gbs": round(gbs, 1),
+                           "frac": round(gbs / peak, 4), "frac_of_nominal_8TBs": round(gbs / NOMINAL_HBM_GBS, 4)})
+            del sel, cnt, out
+        built.free()
+        del built
+        torch.cuda.empty_cache()
+    print(json.dumps({"metric": "PackedAttention us/layer, compression sweep (BASELINE config 5)", "unit": UNIT,
+                      "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup), "data": "synthetic",
+                      "config": {"workload": base.name + "-sweep", "batch_per_gpu": Bt, "context": N, "n_layers": 2,
+                                 "dense_segments": f"{base.dense_num}/{base.dense_den} (all dense at keep 1.0)"},
+                      "peak": peak, "peak_source": peak_src, "sweep": points}), flush=True)
+
+
 if __name__ == "__main__":
     a = parse()
-    if a.impl == "reference":
+    if a.sweep:
+        run_sweep(a)
+    elif a.impl == "reference":
         run_reference(a)
     else:
         run_mkv(a)

@@ -81,8 +81,19 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
     uint32_t Ts = 0;
     int take_eq = 0;
     if (!all && kq > 0) {
-        if (cached)
-            for (int i = tid; i < n; i += 1024) s_keys[i + (i >> 5)] = keyat(i);
+        if (cached) {  // n <= kKeyCap = 16 x 1024: all of a thread's loads are in flight before the first store
+            uint32_t kv[kKeyCap / 1024];
+#pragma unroll
+            for (int j = 0; j < kKeyCap / 1024; ++j) {
+                const int i = tid + j * 1024;
+                kv[j] = i < n ? keyat(i) : 0u;
+            }
+#pragma unroll
+            for (int j = 0; j < kKeyCap / 1024; ++j) {
+                const int i = tid + j * 1024;
+                if (i < n) s_keys[i + (i >> 5)] = kv[j];
+            }
+        }
         uint32_t prefix = 0;
         int krem = kq;
         // MSB-first radix select in three passes of 12 + 12 + 8 bits: with 4096 bins the scores spread
