@@ -155,7 +155,8 @@ MKV_API int mkv_select(const mkv_cache* cache, int32_t layer, const void* q, int
                void* stream);
 
 /*
- * Step 3: PackedAttention over the tokens of the selected blocks.
+ * Step 3: PackedAttention over the tokens of the selected blocks, plus the
+ * tokens of the layer's KV update buffer if it holds any (see mkv_update_append).
  * sel / sel_count as written by mkv_select (any order of blocks is accepted).
  * out: float [batch][n_q_heads][D].  lse_opt: float [batch][n_q_heads] or NULL (log-sum-exp of the
  * scaled logits; -inf and out = 0 for an empty selection).
@@ -163,6 +164,27 @@ MKV_API int mkv_select(const mkv_cache* cache, int32_t layer, const void* q, int
 MKV_API int mkv_packed_attention(const mkv_cache* cache, int32_t layer, const void* q, const int32_t* sel,
                          const int32_t* sel_count, int32_t k_max, float softmax_scale, float* out,
                          float* lse_opt, void* stream);
+
+/*
+ * KV update buffer: the newest tokens of every unit are held uncompressed until a
+ * whole segment can be compressed.  mkv_packed_attention attends the buffered tokens of `layer`
+ * densely, after the selected packed blocks, and merges the two by the log-sum-exp rule; mkv_select
+ * does not see them (they are always attended).
+ *   append: k_new, v_new bf16, element [b][h][t][c] at base + b*stride_b + h*stride_h + t*stride_t + c
+ *           for ALL requests b of the cache, t in [0, n_new): the next n_new tokens of every unit.
+ *           The buffer holds at most segment_len tokens: MKV_E_STATE if they do not fit.
+ *   flush:  compress the buffered tokens as the next segment of every unit (steps 1a, 1b, 1d; strat:
+ *           device, [batch][n_kv_heads][1]) and empty the buffer.  Every request must hold the same
+ *           number of full segments, else MKV_E_STATE.  Flushing fewer than segment_len tokens
+ *           leaves a short last segment, after which nothing can be appended to the packed cache.
+ *   count:  tokens currently buffered per unit (host value; no synchronisation).
+ * mkv_cache_reset also empties the buffer.
+ */
+MKV_API int mkv_update_append(mkv_cache* cache, int32_t layer, const void* k_new, const void* v_new,
+                      int64_t stride_b, int64_t stride_h, int64_t stride_t, int32_t n_new,
+                      void* stream);
+MKV_API int mkv_update_flush(mkv_cache* cache, int32_t layer, const mkv_strategy* strat, void* stream);
+MKV_API int mkv_update_count(const mkv_cache* cache, int32_t layer, int32_t* n_host);
 
 /*
  * Steps 2+3 with HOST buffers (the end-to-end call): copies q_host (bf16 [batch][n_q_heads][D],

@@ -243,6 +243,24 @@ def merge(o1, lse1, o2, lse2):
     return out, lse
 
 
+def attention_with_update_buffer(blob, q, sel, scale: float, k_buf, v_buf):
+    """O8 + KV update buffer: the newest tokens are held uncompressed and attended
+    densely next to the selected packed blocks.  fp64: O8 over the packed part, plain softmax
+    attention over the buffer rows k_buf, v_buf [n][D] (bf16 bits), merged with the split-K rule
+    (pinned: equals O8 on a blob that holds the buffer as a dense, fully selected segment)."""
+    out, lse = attention(blob, q, sel, scale)
+    k_buf, v_buf = _u16(k_buf), _u16(v_buf)
+    if k_buf.shape[0] == 0:
+        return out, lse
+    f = lambda a: (a.astype(np.uint32) << np.uint32(16)).view(np.float32).astype(np.float64)
+    logits = float(scale) * (f(_u16(q)) @ f(k_buf).T)  # [G][n]
+    m = logits.max(axis=1)
+    p = np.exp(logits - m[:, None])
+    l = p.sum(axis=1)
+    o_buf, lse_buf = (p @ f(v_buf)) / l[:, None], m + np.log(l)
+    return merge(out, lse, o_buf, lse_buf)
+
+
 def compress_units(k, v, L: int, strat4):
     """Batched O5 over units (OpenMP). k, v: [U][N][D]; strat4: [U][S][4]. Returns list of blobs."""
     k, v = _u16(k), _u16(v)

@@ -23,7 +23,7 @@ MKV_DEV_ARENA_OVERFLOW, MKV_DEV_BAD_STRATEGY = 1, 2
 # every symbol include/mkv.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ["mkv_cache_create", "mkv_cache_free", "mkv_cache_reset", "mkv_segment_loss",
            "mkv_strategy_quantile", "mkv_strategy_threshold", "mkv_compress_segment", "mkv_select",
-           "mkv_packed_attention", "mkv_decode_host", "mkv_cache_export", "mkv_cache_bytes",
+           "mkv_packed_attention", "mkv_update_append", "mkv_update_flush", "mkv_update_count", "mkv_decode_host", "mkv_cache_export", "mkv_cache_bytes",
            "mkv_cache_status", "mkv_last_launch_count", "mkv_last_error", "mkv_version"]
 
 
@@ -50,6 +50,9 @@ _lib.mkv_compress_segment.argtypes = [_vp, _i32, _vp, _vp, _i64, _i64, _i64, _i3
                                       _i32, _vp, _vp]
 _lib.mkv_select.argtypes = [_vp, _i32, _vp, _i32, _i32, _vp, _vp, _i32, _vp, _vp]
 _lib.mkv_packed_attention.argtypes = [_vp, _i32, _vp, _vp, _vp, _i32, C.c_float, _vp, _vp, _vp]
+_lib.mkv_update_append.argtypes = [_vp, _i32, _vp, _vp, _i64, _i64, _i64, _i32, _vp]
+_lib.mkv_update_flush.argtypes = [_vp, _i32, _vp, _vp]
+_lib.mkv_update_count.argtypes = [_vp, _i32, C.POINTER(_i32)]
 _lib.mkv_decode_host.argtypes = [_vp, _i32, _vp, _i32, _i32, C.c_float, _vp, _vp, _vp, _vp]
 _lib.mkv_cache_export.argtypes = [_vp, _i32, _i32, _i32, _vp, _u64, C.POINTER(_u64)]
 _lib.mkv_cache_bytes.argtypes = [_vp, _i32, C.POINTER(_u64), C.POINTER(_u64), C.POINTER(_u64)]
@@ -172,6 +175,23 @@ def mkv_packed_attention(cache, layer, q, sel, sel_count, softmax_scale, out, ls
                                      float(softmax_scale), _ptr(out), _ptr(lse), _stream(stream)))
 
 
+def mkv_update_append(cache, layer, k_new, v_new, stream=None):
+    """k_new, v_new: torch bf16 [batch][Hkv][n_new][D] (any batch/head/token strides)."""
+    sb, sh, st = _kv_strides(k_new, v_new)
+    _check(_lib.mkv_update_append(cache, layer, _ptr(k_new), _ptr(v_new), sb, sh, st, k_new.shape[2], _stream(stream)))
+
+
+def mkv_update_flush(cache, layer, strat, stream=None):
+    """strat: torch uint8 [batch][Hkv][1][4] on the device."""
+    _check(_lib.mkv_update_flush(cache, layer, _ptr(strat), _stream(stream)))
+
+
+def mkv_update_count(cache, layer) -> int:
+    n = _i32(0)
+    _check(_lib.mkv_update_count(cache, layer, C.byref(n)))
+    return n.value
+
+
 def mkv_decode_host(cache, layer, q_host, token_budget, softmax_scale, out_host, reduce=0,
                     sel_host=None, sel_count_host=None, stream=None):
     _check(_lib.mkv_decode_host(cache, layer, _ptr(q_host), token_budget, reduce, float(softmax_scale),
@@ -263,6 +283,15 @@ class Cache:
 
     def packed_attention(self, layer, q, sel, sel_count, softmax_scale, out, lse=None, stream=None):
         mkv_packed_attention(self.h, layer, q, sel, sel_count, softmax_scale, out, lse, stream)
+
+    def update_append(self, layer, k_new, v_new, stream=None):
+        mkv_update_append(self.h, layer, k_new, v_new, stream)
+
+    def update_flush(self, layer, strat, stream=None):
+        mkv_update_flush(self.h, layer, strat, stream)
+
+    def update_count(self, layer):
+        return mkv_update_count(self.h, layer)
 
     def decode_host(self, layer, q_host, token_budget, softmax_scale, out_host, reduce=0,
                     sel_host=None, sel_count_host=None, stream=None):

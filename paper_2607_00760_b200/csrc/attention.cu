@@ -54,12 +54,15 @@ constexpr int kMaxWarps = 24;      // upper bound on warps per CTA (sizes the pa
 constexpr int kStageBytes = 4096;  // one dense block (4096 B) or two packed blocks with r <= 56
 constexpr int kDescRing = 64;      // block descriptors kept per warp
 constexpr int kMaxUnitsSmem = 2048;
+// A group of the KV update buffer: nb0 <= 8 uncompressed recent tokens, attended as one dense
+// block; off0 / off1 are its K rows / V rows in the buffer arrays (two chunks, staged back to back).
+constexpr uint32_t kUpdFlag = 1u << 26;
 
 // One group of the stream: <= 2 consecutive selected token blocks of one unit with the same
 // strategy that fit one stage (16 tokens = the M of one mma tile).
 struct __align__(16) GDesc {
     uint32_t off0, off1;  // payload offsets in the layer slice, 16-B units
-    uint32_t z;           // bytes0 / 16 | bytes1 / 16 << 9 | nb0 << 18 | nb1 << 22   (bytes 0: invalid entry)
+    uint32_t z;           // bytes0 / 16 | bytes1 / 16 << 9 | nb0 << 18 | nb1 << 22 | kUpdFlag   (bytes 0: invalid entry)
     uint32_t w;           // unit | r_k << 16 | r_v << 24
 };
 
@@ -75,7 +78,7 @@ __device__ __forceinline__ unsigned lanemask_lt() {
 }
 
 // prefix sums of the clamped selection counts -> s_cum[0..n_units]; returns the total T
-__device__ __forceinline__ int scan_counts(const int32_t* __restrict__ sel_count, int n_units, int k_max,
+__device__ __forceinline__ int scan_counts(const int32_t* __restrict__ sel_count, int n_units, int k_max, int extra,
                                             int* s_cum) {
     __shared__ int s_carry;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -84,7 +87,7 @@ __device__ __forceinline__ int scan_counts(const int32_t* __restrict__ sel_count
 #pragma unroll 1
         for (int i0 = 0; i0 < n_units; i0 += 32) {
             const int i = i0 + lane;
-            int c = (i < n_units) ? min(max(sel_count[i], 0), k_max) : 0;
+            int c = (i < n_units) ? min(max(sel_count[i], 0), k_max) + extra : 0;  // + blocks of the update buffer
             int inc = c;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -135,7 +138,8 @@ __global__ void __launch_bounds__(kWarps * 32, 1)
 mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q,
                             const int32_t* __restrict__ sel, const int32_t* __restrict__ sel_count, int k_max,
                             float scale_log2, float* __restrict__ out, float* __restrict__ lse,
-                            float* __restrict__ part_o, float* __restrict__ part_ml, int32_t* __restrict__ ticket) {
+                            float* __restrict__ part_o, float* __restrict__ part_ml, int32_t* __restrict__ ticket,
+                            const uint16_t* __restrict__ upd_k, const uint16_t* __restrict__ upd_v, int n_buf) {
     extern __shared__ __align__(128) uint8_t smem[];
     constexpr int kWS = warp_smem_bytes(NSTAGE);
     constexpr int kNT = kWarps * 32;
@@ -161,7 +165,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     }
     if (lane < 2) s_unit[warp * 2 + lane] = -1;
 
-    const int T = scan_counts(sel_count, g.n_units, k_max, s_cum);  // (block barrier inside)
+    const int upd_blocks = (n_buf + kB - 1) / kB;  // every unit ends with the blocks of its update buffer
+    const int T = scan_counts(sel_count, g.n_units, k_max, upd_blocks, s_cum);  // (block barrier inside)
     const unsigned Gd = min(gridDim.x, (unsigned)max(T, 1));        // CTAs that own >= 1 block
     Split cs;                                                       // blocks over CTAs
     cs.b = (unsigned)T / Gd; cs.r = (unsigned)T - cs.b * Gd;
@@ -196,7 +201,14 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         if (lane < count) {
             const int gi = lo + bbuilt + lane;
             u = find_unit(s_cum, g.n_units, gi);
-            const int t0 = sel[(size_t)u * k_max + (gi - s_cum[u])];
+            const int j = gi - s_cum[u], jb = j - (s_cum[u + 1] - s_cum[u] - upd_blocks);
+            if (jb >= 0) {  // block jb of the unit's update buffer: raw rows [u][8 jb ..][128] of upd_k / upd_v
+                nb = (uint32_t)min(kB, n_buf - kB * jb);
+                off16 = (uint32_t)(((size_t)u * g.L + (size_t)kB * jb) * (kD * 2 / 16));
+                bytes = nb * (uint32_t)(kD * 2);
+                rr = (uint32_t)kD | ((uint32_t)kD << 8) | 0x10000u;  // bit 16: update-buffer block
+            }
+            const int t0 = jb >= 0 ? -1 : sel[(size_t)u * k_max + j];
             const int ntok = lv.unit_ntok[u];
             if (t0 >= 0 && t0 < ntok && (t0 & (kB - 1)) == 0) {
                 const int seg = t0 / g.L, in_seg = t0 - seg * g.L;
@@ -211,7 +223,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         const int pu = __shfl_up_sync(kFull, u, 1);
         const uint32_t prr = __shfl_up_sync(kFull, rr, 1), pbytes = __shfl_up_sync(kFull, bytes, 1);
         const bool follows = lane > 0 && lane < count && u == pu && rr == prr && bytes != 0u && pbytes != 0u &&
-                             bytes + pbytes <= (uint32_t)kStageBytes;
+                             bytes + pbytes <= (uint32_t)kStageBytes && !(rr & 0x10000u);
         const unsigned fm = __ballot_sync(kFull, follows);
         const int start = 31 - __clz((int)(~fm & lanemask_le()));  // first block of this lane's run (bit 0 of ~fm is set)
         const bool first = lane < count && ((lane - start) & 1) == 0;
@@ -223,7 +235,11 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             GDesc d;
             d.off0 = off16; d.off1 = two ? off1 : 0u;
             d.z = (bytes >> 4) | ((two ? bytes1 >> 4 : 0u) << 9) | (nb << 18) | ((two ? nb1 : 0u) << 22);
-            d.w = (uint32_t)u | (rr << 16);
+            if (rr & 0x10000u) {  // K rows and V rows: two chunks of the same size at the same offset
+                d.off1 = off16;
+                d.z |= ((bytes >> 4) << 9) | kUpdFlag;
+            }
+            d.w = (uint32_t)u | ((rr & 0xffffu) << 16);
             ring[(gbuilt + __popc(gm & lanemask_lt())) & (kDescRing - 1)] = d;
         }
         gbuilt += __popc(gm);
@@ -241,12 +257,15 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         const uint32_t b0 = (d.z & 511u) << 4, b1 = ((d.z >> 9) & 511u) << 4;
         if (lane == 0) {
             const uint32_t bar = bar0 + 8 * s, dst = stage0 + s * kStageBytes;
+            const bool upd = d.z & kUpdFlag;
+            const unsigned long long src0 = upd ? reinterpret_cast<unsigned long long>(upd_k) : slice;
+            const unsigned long long src1 = upd ? reinterpret_cast<unsigned long long>(upd_v) : slice;
             mbar_expect_tx(bar, b0 + b1);
-            if (b0) bulk_g2s(dst, slice + ((unsigned long long)d.off0 << 4), b0, bar);
-            if (b1) bulk_g2s(dst + b0, slice + ((unsigned long long)d.off1 << 4), b1, bar);
+            if (b0) bulk_g2s(dst, src0 + ((unsigned long long)d.off0 << 4), b0, bar);
+            if (b1) bulk_g2s(dst + b0, src1 + ((unsigned long long)d.off1 << 4), b1, bar);
         }
         ++gposi;
-        bposi += b1 ? 2 : 1;
+        bposi += (b1 && !(d.z & kUpdFlag)) ? 2 : 1;
     };
 
     // per-unit state.  qa: B fragments of q (column gq = head gq of the unit's group).
@@ -647,7 +666,8 @@ int attention_partial_slots(int sm_count) { return sm_count * kMaxWarps * 2 + sm
 template <int NSTAGE, int NWARPS>
 static cudaError_t launch_attention_cfg(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
                                         const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
-                                        const AttnScratch& scr, int sm_count, cudaStream_t s) {
+                                        const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v, int n_buf,
+                                        int sm_count, cudaStream_t s) {
     const int smem = NWARPS * warp_smem_bytes(NSTAGE) + (g.n_units + 1) * 4;
     static int configured = 0;  // largest dynamic shared-memory size opted into so far
     if (smem > configured) {
@@ -657,13 +677,14 @@ static cudaError_t launch_attention_cfg(const CacheGeom& g, const LayerView& lv,
         configured = smem;
     }
     mkv_packed_attention_kernel<NSTAGE, NWARPS><<<sm_count, NWARPS * 32, smem, s>>>(
-        g, lv, q, sel, sel_count, k_max, scale * kLog2e, out, lse, scr.part_o, scr.part_ml, scr.ticket);
+        g, lv, q, sel, sel_count, k_max, scale * kLog2e, out, lse, scr.part_o, scr.part_ml, scr.ticket, upd_k, upd_v, n_buf);
     return cudaGetLastError();
 }
 
 cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
                              const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
-                             const AttnScratch& scr, int sm_count, cudaStream_t s, int* n_kernels) {
+                             const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v, int n_buf,
+                             int sm_count, cudaStream_t s, int* n_kernels) {
     if (g.n_units > kMaxUnitsSmem) return cudaErrorInvalidValue;
     if (n_kernels) *n_kernels = 1;
     static int cfg = -1;  // tuning knob (stages * 100 + warps); default chosen from measurements
@@ -672,10 +693,10 @@ cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint
         cfg = e ? atoi(e) : 316;
     }
 #define MKV_CFG(S, W) \
-    case S * 100 + W: return launch_attention_cfg<S, W>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, sm_count, s);
+    case S * 100 + W: return launch_attention_cfg<S, W>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, n_buf, sm_count, s);
     switch (cfg) {
         MKV_CFG(3, 16) MKV_CFG(2, 16) MKV_CFG(2, 20) MKV_CFG(2, 24) MKV_CFG(4, 12) MKV_CFG(4, 8)
-        default: return launch_attention_cfg<3, 16>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, sm_count, s);
+        default: return launch_attention_cfg<3, 16>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, n_buf, sm_count, s);
     }
 #undef MKV_CFG
 }

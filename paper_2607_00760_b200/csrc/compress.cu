@@ -370,7 +370,35 @@ __global__ void mkv_strategy_threshold_kernel(const double* __restrict__ loss_k,
     out[i] = s;
 }
 
+// ------------------------------------------------------------------------------------------
+// KV update buffer: the newest tokens of every unit are held uncompressed, raw
+// rows [unit][t][128] bf16, until a whole segment can be compressed.  One warp copies one K row
+// and one V row (256 B each, 8 B per lane).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) mkv_update_copy_kernel(CacheGeom g, CompressArgs a, uint16_t* __restrict__ upd_k,
+                                                              uint16_t* __restrict__ upd_v, int n_have) {
+    const int row = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (row >= g.n_units * a.n_tok) return;
+    const int unit = row / a.n_tok, t = row - unit * a.n_tok;
+    const int b = unit / g.n_kv_heads, h = unit % g.n_kv_heads;
+    const size_t src = (size_t)b * a.stride_b + (size_t)h * a.stride_h + (size_t)t * a.stride_t + 4 * lane;
+    const size_t dst = ((size_t)unit * g.L + n_have + t) * kD + 4 * lane;
+    // rows may be only 2-byte aligned in the caller's tensors: element loads, one 8-byte store
+    uint16_t kx[4], vx[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { kx[j] = a.k[src + j]; vx[j] = a.v[src + j]; }
+    *reinterpret_cast<uint2*>(upd_k + dst) = make_uint2(kx[0] | ((uint32_t)kx[1] << 16), kx[2] | ((uint32_t)kx[3] << 16));
+    *reinterpret_cast<uint2*>(upd_v + dst) = make_uint2(vx[0] | ((uint32_t)vx[1] << 16), vx[2] | ((uint32_t)vx[3] << 16));
+}
+
 }  // namespace
+
+cudaError_t launch_update_copy(const CacheGeom& g, const CompressArgs& a, uint16_t* upd_k, uint16_t* upd_v, int n_have,
+                               cudaStream_t s) {
+    const int rows = g.n_units * a.n_tok;
+    mkv_update_copy_kernel<<<(rows + 7) / 8, 256, 0, s>>>(g, a, upd_k, upd_v, n_have);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_segment_loss(const CacheGeom& g, const CompressArgs& a, mkv_strategy cand, double* loss_k,
                                 double* loss_v, cudaStream_t s) {

@@ -54,6 +54,9 @@ struct mkv_cache {
     float* scores = nullptr;                  // [n_units][score_stride]
     uint32_t* cand_key = nullptr;             // [n_units][slices * kTopkSlice]  top-k candidates of long units
     int32_t* cand_idx = nullptr;
+    uint16_t* upd_k = nullptr;                // KV update buffer, raw bf16 [n_layers][n_units][L][D]
+    uint16_t* upd_v = nullptr;
+    std::vector<int32_t> upd_n;               // tokens buffered per layer (every unit holds the same number)
     AttnScratch attn{};
     uint16_t* q_dev = nullptr;
     int32_t* sel_dev = nullptr;
@@ -93,7 +96,7 @@ int mkv_cache_free(mkv_cache* c) {
     cudaSetDevice(c->desc.device);
     cudaDeviceSynchronize();
     void* ptrs[] = {c->arena, c->strat, c->tok_off, c->bk_off, c->unit_nseg, c->unit_ntok, c->counters,
-                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->attn.part_o, c->attn.part_ml, c->attn.ticket, c->q_dev,
+                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->upd_k, c->upd_v, c->attn.part_o, c->attn.part_ml, c->attn.ticket, c->q_dev,
                     c->sel_dev, c->selcnt_dev, c->out_dev, c->cands_dev};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -138,6 +141,8 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     const size_t tu = (size_t)g.n_layers * g.n_units;
     c->attn.slots = attention_partial_slots(c->sm_count);
     c->sel_cap = g.score_stride + 1;
+    const size_t upd_bytes = (size_t)g.n_layers * g.n_units * g.L * kD * 2;
+    c->upd_n.assign(g.n_layers, 0);
     const int topk_slices = (g.score_stride + kTopkSlice - 1) / kTopkSlice;
     const size_t cand_bytes = topk_slices > 1 ? (size_t)g.n_units * topk_slices * kTopkSlice * 4 : 256;
     struct { void** p; size_t bytes; } allocs[] = {
@@ -153,6 +158,8 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         {(void**)&c->scores, (size_t)g.n_units * g.score_stride * 4},
         {(void**)&c->cand_key, cand_bytes},
         {(void**)&c->cand_idx, cand_bytes},
+        {(void**)&c->upd_k, upd_bytes},
+        {(void**)&c->upd_v, upd_bytes},
         {(void**)&c->attn.part_o, (size_t)c->attn.slots * g.group * kD * 4},
         {(void**)&c->attn.part_ml, (size_t)c->attn.slots * kMaxGroup * 2 * 4},
         {(void**)&c->attn.ticket, (size_t)g.n_units * 4},
@@ -198,6 +205,7 @@ int mkv_cache_reset(mkv_cache* c, int32_t layer, void* stream) {
         MKV_CUDA(cudaMemsetAsync(c->unit_ntok + (size_t)l * g.n_units, 0, (size_t)g.n_units * 4, s));
         MKV_CUDA(cudaMemsetAsync(c->counters + (size_t)l * 4, 0, 32, s));
         for (int b = 0; b < g.batch; ++b) c->host_nseg[(size_t)l * g.batch + b] = c->host_ntok[(size_t)l * g.batch + b] = 0;
+        c->upd_n[l] = 0;
     }
     return MKV_OK;
 }
@@ -303,8 +311,55 @@ int mkv_packed_attention(const mkv_cache* cc, int32_t layer, const void* q, cons
     if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
     if (k_max < 1) return fail(MKV_E_ARG, "mkv_packed_attention: k_max < 1");
     MKV_CUDA(cudaSetDevice(c->desc.device));
+    const size_t upd_off = (size_t)layer * g.n_units * g.L * kD;
     MKV_CUDA(launch_attention(g, c->view(layer), (const uint16_t*)q, sel, sel_count, k_max, scale, out, lse_opt,
-                              c->attn, c->sm_count, (cudaStream_t)stream, &c->last_attn));
+                              c->attn, c->upd_k + upd_off, c->upd_v + upd_off, c->upd_n[layer], c->sm_count,
+                              (cudaStream_t)stream, &c->last_attn));
+    return MKV_OK;
+}
+
+int mkv_update_append(mkv_cache* c, int32_t layer, const void* k_new, const void* v_new, int64_t sb, int64_t sh,
+                      int64_t st, int32_t n_new, void* stream) {
+    if (!c || !k_new || !v_new) return fail(MKV_E_ARG, "mkv_update_append: NULL argument");
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    if (n_new < 1 || st < kD || sh < 0 || sb < 0) return fail(MKV_E_ARG, "mkv_update_append: bad n_new / strides");
+    const int have = c->upd_n[layer];
+    if (have + n_new > g.L)
+        return fail(MKV_E_STATE, "mkv_update_append: buffer holds %d of %d tokens; %d more do not fit (flush first)", have,
+                    g.L, n_new);
+    CompressArgs a{(const uint16_t*)k_new, (const uint16_t*)v_new, sb, sh, st, 0, g.batch, 0, 1, n_new};
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    const size_t off = (size_t)layer * g.n_units * g.L * kD;
+    MKV_CUDA(launch_update_copy(g, a, c->upd_k + off, c->upd_v + off, have, (cudaStream_t)stream));
+    c->upd_n[layer] = have + n_new;
+    return MKV_OK;
+}
+
+int mkv_update_flush(mkv_cache* c, int32_t layer, const mkv_strategy* strat, void* stream) {
+    if (!c || !strat) return fail(MKV_E_ARG, "mkv_update_flush: NULL argument");
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    const int n = c->upd_n[layer];
+    if (n == 0) return MKV_OK;
+    const int seg0 = c->host_nseg[(size_t)layer * g.batch];
+    for (int b = 1; b < g.batch; ++b)
+        if (c->host_nseg[(size_t)layer * g.batch + b] != seg0)
+            return fail(MKV_E_STATE, "mkv_update_flush: requests hold different numbers of segments");
+    // the buffer is the raw K/V of the next segment of every unit: [b][h][t][c] with dense strides
+    const int64_t sh = (int64_t)g.L * kD, sb = sh * g.n_kv_heads;
+    const size_t off = (size_t)layer * g.n_units * g.L * kD;
+    const int rc = mkv_compress_segment(c, layer, c->upd_k + off, c->upd_v + off, sb, sh, kD, 0, g.batch, seg0, 1, n, strat,
+                                        stream);
+    if (rc) return rc;
+    c->upd_n[layer] = 0;
+    return MKV_OK;
+}
+
+int mkv_update_count(const mkv_cache* c, int32_t layer, int32_t* n_host) {
+    if (!c || !n_host) return fail(MKV_E_ARG, "mkv_update_count: NULL argument");
+    if (layer < 0 || layer >= c->geom.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    *n_host = c->upd_n[layer];
     return MKV_OK;
 }
 

@@ -368,6 +368,68 @@ def test_layers_are_independent_and_decode_host_matches(env):
         b.free()
 
 
+@pytest.mark.parametrize("Hq,Hkv", [(8, 2), (7, 1)])
+def test_update_buffer_attention_and_flush(env, Hq, Hkv):
+    """KV update buffer (PAPER.md:224): buffered raw tokens are attended densely and merged with the packed part;
+    a full buffer is flushed through step 1 and the packed cache stays bit-exact with the oracle."""
+    mkv, dev = env
+    import torch
+    Bt, L, N0 = 2, 64, 64 * 6
+    c = Case(mkv, dev, Bt, Hkv, Hq, N0 + 2 * L, seed=61 + Hq)  # K/V hold the tokens that arrive later too
+    try:
+        strat = uniform_strat(Bt, Hkv, c.S, 38)
+        strat[:, :, ::4, 0:2] = 128
+        first = torch.from_numpy(strat[:, :, :N0 // L].copy()).to(dev)
+        c.cache.compress_segment(0, c.k_d[:, :, :N0], c.v_d[:, :, :N0], first)
+        blobs = lambda n, st: [[orc.compress_unit(c.K[b, h, :n], c.V[b, h, :n], L, st[b, h, :(n + L - 1) // L])
+                                for h in range(Hkv)] for b in range(Bt)]
+        packed = blobs(N0, strat)
+        scale = 1.0 / math.sqrt(128)
+        sel = np.full((Bt, Hkv, 12), -1, np.int32)
+        cnt = np.zeros((Bt, Hkv), np.int32)
+        rng = np.random.default_rng(3)
+        for b in range(Bt):
+            for h in range(Hkv):
+                k = int(rng.integers(0, 12)) if (b, h) != (0, 0) else 0  # unit (0, 0): empty selection
+                sel[b, h, :k] = np.sort(rng.choice(N0 // 8, k, replace=False)) * 8
+                cnt[b, h] = k
+
+        def check(n_buf, packed_blobs, n_packed):
+            out, lse = c.gpu_attention(sel, cnt, scale)
+            ref, ref_lse = np.zeros_like(out), np.zeros_like(lse)
+            for b in range(Bt):
+                for h in range(Hkv):
+                    o, l = orc.attention_with_update_buffer(
+                        packed_blobs[b][h], c.q[b, h * c.G:(h + 1) * c.G], sel[b, h, :cnt[b, h]], scale,
+                        c.K[b, h, n_packed:n_packed + n_buf], c.V[b, h, n_packed:n_packed + n_buf])
+                    ref[b, h * c.G:(h + 1) * c.G], ref_lse[b, h * c.G:(h + 1) * c.G] = o, l
+            assert_attention_close(out, lse, ref, ref_lse)
+
+        have = 0
+        for n_new in (1, 6, 1, 1, 23, 32):  # 1, 7, 8, 9, 32, 64 tokens buffered
+            c.cache.update_append(0, c.k_d[:, :, N0 + have:N0 + have + n_new], c.v_d[:, :, N0 + have:N0 + have + n_new])
+            have += n_new
+            assert c.cache.update_count(0) == have
+            check(have, packed, N0)
+        with pytest.raises(mkv.MkvError) as e:  # the buffer is full
+            c.cache.update_append(0, c.k_d[:, :, :1], c.v_d[:, :, :1])
+        assert e.value.code == mkv.MKV_E_STATE
+        seg = N0 // L
+        c.cache.update_flush(0, torch.from_numpy(strat[:, :, seg:seg + 1].copy()).to(dev))
+        torch.cuda.synchronize()
+        c.cache.status()
+        assert c.cache.update_count(0) == 0
+        packed = blobs(N0 + L, strat)
+        for b in range(Bt):
+            for h in range(Hkv):
+                np.testing.assert_array_equal(c.cache.export(0, b, h), packed[b][h])
+        check(0, packed, N0 + L)
+        c.cache.update_append(0, c.k_d[:, :, N0 + L:N0 + L + 5], c.v_d[:, :, N0 + L:N0 + L + 5])
+        check(5, packed, N0 + L)
+    finally:
+        c.free()
+
+
 def test_errors_are_reported_not_thrown(env):
     mkv, dev = env
     import torch

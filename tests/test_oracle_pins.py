@@ -371,6 +371,41 @@ def test_P10_merge_of_halves_equals_single_pass():
     np.testing.assert_allclose(om, o, rtol=0, atol=1e-15)
 
 
+# ----------------------------------------------------------------------------- P13: KV update buffer
+
+@pytest.mark.parametrize("n_buf", [1, 7, 8, 13, 32, 64])
+def test_P13_update_buffer_equals_dense_selected_segment(n_buf):
+    """the buffered (uncompressed) tokens are attended next to the selected packed blocks.
+    Pin: the result equals O8 on a blob that holds the buffer as one more, dense and fully selected
+    segment, and the brute-force masked dense attention of tests/brute.py."""
+    N = 192
+    K, V, q = small_unit(seed=21, N=N + n_buf)
+    blob = orc.compress_unit(K[:N], V[:N], 64, orc.uniform_strategy(3, 38, 38))
+    sel = np.array([0, 16, 64, 120, 184], np.int32)
+    o, l = orc.attention_with_update_buffer(blob, q, sel, 0.11, K[N:], V[N:])
+    strat = orc.uniform_strategy(4, 38, 38)
+    strat[3, 0:2] = 128
+    blob2 = orc.compress_unit(K, V, 64, strat)
+    sel2 = np.concatenate([sel, N + 8 * np.arange((n_buf + 7) // 8)]).astype(np.int32)
+    o2, l2 = orc.attention(blob2, q, sel2, 0.11)
+    np.testing.assert_allclose(o, o2, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(l, l2, rtol=0, atol=1e-12)
+    un = orc.unpack_unit(blob2)
+    Kd, Vd, Mk, Mv = un["k"], un["v"], un["k_mask"], un["v_mask"]
+    tok = np.zeros(N + n_buf, bool)
+    for t0 in sel2:
+        tok[t0:t0 + 8] = True
+    ob, lb = brute.masked_dense_attention(brute.bf16_to_f64(q), brute.bf16_to_f64(Kd), brute.bf16_to_f64(Vd),
+                                          Mk.astype(np.float64), Mv.astype(np.float64), tok, 0.11)
+    np.testing.assert_allclose(o, ob, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(l, lb, rtol=0, atol=1e-12)
+    # an empty selection leaves plain dense attention over the buffer
+    oe, le = orc.attention_with_update_buffer(blob, q, sel[:0], 0.11, K[N:], V[N:])
+    od, ld = brute.dense_attention(brute.bf16_to_f64(q), brute.bf16_to_f64(K[N:]), brute.bf16_to_f64(V[N:]), 0.11)
+    np.testing.assert_allclose(oe, od, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(le, ld, rtol=0, atol=1e-12)
+
+
 # ----------------------------------------------------------------------------- P12: strategies (O4)
 
 def test_P12_quantile_and_threshold():
