@@ -280,6 +280,9 @@ def run_mkv(args):
         "kernels_per_layer": launches,
         "clocks": clk,
     }
+    if rank == 0:
+        line["update_buffer"] = measure_update_buffer(torch, mkv, synth, w, dev, Bt, cache, built, step_attention,
+                                                      n_layers, graph, args)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args, w, built, dev, n_units=args.cpu_units, repeats=1)
     built.free()
@@ -288,6 +291,43 @@ def run_mkv(args):
         dist.destroy_process_group()
     if rank == 0:
         print(json.dumps(line), flush=True)
+
+
+def measure_update_buffer(torch, mkv, synth, w, dev, Bt, cache, built, step_attention, n_layers, graph, args):
+    """KV update buffer: (i) flush = compress a full buffer of every unit of one layer through
+    step 1 (the paper's only absolute kernel time: 40.6 us on an H800 for its 32-token buffer), measured for a
+    32-token and a 64-token buffer (buffer = one segment); (ii) PackedAttention with 32 tokens buffered per unit."""
+    Hkv, Hq = w.n_kv_heads, w.n_q_heads
+    res = {"paper_h800_flush_us_32_tokens": 40.6, "units_per_layer": Bt * Hkv}
+    for L in (32, 64):
+        c = mkv.Cache(1, Bt, Hkv, Hq, 128, 4 * L, L, device=dev.index or 0)
+        try:
+            k = torch.randn((Bt, Hkv, L, 128), device=dev).to(torch.bfloat16)
+            v = torch.randn((Bt, Hkv, L, 128), device=dev).to(torch.bfloat16)
+            st = torch.tensor([w.r_keep, w.r_keep, 1, 8], dtype=torch.uint8, device=dev).repeat(Bt, Hkv, 1, 1)
+            ts = []
+            for it in range(8):
+                c.reset()
+                c.update_append(0, k, v)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                c.update_flush(0, st)
+                e1.record()
+                torch.cuda.synchronize()
+                if it >= 3:
+                    ts.append(e0.elapsed_time(e1) * 1e3)
+            c.status()
+            res[f"flush_us_{L}_tokens"] = round(sorted(ts)[len(ts) // 2], 2)
+        finally:
+            c.free()
+    kn = torch.randn((Bt, Hkv, 32, 128), device=dev).to(torch.bfloat16)
+    vn = torch.randn((Bt, Hkv, 32, 128), device=dev).to(torch.bfloat16)
+    for l in range(n_layers):
+        cache.update_append(l, kn, vn)
+    ms = timed_loop(torch, step_attention, args.steps, args.warmup, lambda: None, graph)
+    cache.status()
+    res["attention_us_per_layer_with_32_buffered_tokens"] = round(ms * 1e3 / n_layers, 3)
+    return res
 
 
 # ------------------------------------------------------------------------------ the oracle legs
