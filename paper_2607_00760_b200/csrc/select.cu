@@ -28,8 +28,8 @@ __device__ __forceinline__ uint32_t score_key(float s) {
 // one short block (the unit's last), the walk takes the k0 = budget/8 best blocks, plus one
 // more iff the short block is among the k0+1 best and fits the remainder.
 // ------------------------------------------------------------------------------------------
-// Keys of a unit are cached in shared memory when they fit (kKeyCap), so the four radix passes read
-// global memory once.  Histogram updates are aggregated per warp with match.any (scores cluster in a
+// The keys of a CTA are cached in registers when they fit (kKeyCap = 16 per thread, blocked: thread t
+// holds elements [16 t, 16 t + 16)), so the radix passes and the emission read global memory once.  Histogram updates are aggregated per warp with match.any (scores cluster in a
 // few bins of the first pass); the emission gives every thread a run of consecutive blocks, so one
 // block-wide scan of packed (greater, equal) counts orders the whole output.
 constexpr int kKeyCap = 16384;  // 64 KB of keys
@@ -48,7 +48,6 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
                                                         int32_t* __restrict__ sel_count, int k_max,
                                                         uint32_t* __restrict__ cand_key, int32_t* __restrict__ cand_idx,
                                                         int n_slices, int cand_cap) {
-    extern __shared__ uint32_t s_keys[];  // key i at [i + i / 32]: conflict-free for strided and for per-thread runs
     const int unit = MODE == 1 ? blockIdx.x / n_slices : blockIdx.x;
     const int slice = MODE == 1 ? blockIdx.x % n_slices : 0;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -80,18 +79,24 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
     int kq = MODE == 1 ? min(n, k0 + 1) : (all ? nblk : (ragged_try ? k0 + 1 : k0));  // rank whose key we look for
     uint32_t Ts = 0;
     int take_eq = 0;
+    constexpr int kPerThread = kKeyCap / 1024;
+    uint32_t kv[kPerThread];  // this thread's keys when the CTA's elements fit (cached)
+#pragma unroll
+    for (int j = 0; j < kPerThread; ++j) kv[j] = 0u;
     if (!all && kq > 0) {
-        if (cached) {  // n <= kKeyCap = 16 x 1024: all of a thread's loads are in flight before the first store
-            uint32_t kv[kKeyCap / 1024];
+        if (cached) {  // n <= kKeyCap = 16 x 1024: thread t keeps elements [16 t, 16 t + 16) in registers
+            const int i0 = kPerThread * tid;
+            if (MODE != 2 && (reinterpret_cast<uintptr_t>(s + base) & 15) == 0 && i0 + kPerThread <= n) {
+                const float4* s4 = reinterpret_cast<const float4*>(s + base + i0);
 #pragma unroll
-            for (int j = 0; j < kKeyCap / 1024; ++j) {
-                const int i = tid + j * 1024;
-                kv[j] = i < n ? keyat(i) : 0u;
-            }
+                for (int j = 0; j < kPerThread / 4; ++j) {
+                    const float4 f = s4[j];
+                    kv[4 * j] = score_key(f.x); kv[4 * j + 1] = score_key(f.y);
+                    kv[4 * j + 2] = score_key(f.z); kv[4 * j + 3] = score_key(f.w);
+                }
+            } else {
 #pragma unroll
-            for (int j = 0; j < kKeyCap / 1024; ++j) {
-                const int i = tid + j * 1024;
-                if (i < n) s_keys[i + (i >> 5)] = kv[j];
+                for (int j = 0; j < kPerThread; ++j) kv[j] = i0 + j < n ? keyat(i0 + j) : 0u;
             }
         }
         uint32_t prefix = 0;
@@ -102,11 +107,20 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
             const int shift = pass == 0 ? 20 : (pass == 1 ? 8 : 0);
             const int nbins = pass == 2 ? 256 : 4096;
             for (int i = tid; i < nbins; i += 1024) hist[i] = 0;
-            __syncthreads();  // also orders the fill of s_keys before the first pass
+            __syncthreads();
             const uint32_t hi_mask = pass == 0 ? 0u : (0xffffffffu << (pass == 1 ? 20 : 8));
-            for (int i = tid; i < n; i += 1024) {
-                const uint32_t u = cached ? s_keys[i + (i >> 5)] : keyat(i);
-                if ((u & hi_mask) == prefix) atomicAdd(&hist[(u >> shift) & (uint32_t)(nbins - 1)], 1u);
+            if (cached) {
+#pragma unroll
+                for (int j = 0; j < kPerThread; ++j) {
+                    const uint32_t u = kv[j];
+                    if (kPerThread * tid + j < n && (u & hi_mask) == prefix)
+                        atomicAdd(&hist[(u >> shift) & (uint32_t)(nbins - 1)], 1u);
+                }
+            } else {
+                for (int i = tid; i < n; i += 1024) {
+                    const uint32_t u = keyat(i);
+                    if ((u & hi_mask) == prefix) atomicAdd(&hist[(u >> shift) & (uint32_t)(nbins - 1)], 1u);
+                }
             }
             __syncthreads();
             // thread t owns bins [t bpt, (t+1) bpt); counts in the bins above it by a block-wide suffix scan
@@ -177,16 +191,22 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
     // emission in ascending position (= ascending block index): thread t owns elements [t E, (t+1) E)
     int count = 0;
     if (kq > 0) {
-        const int E = (n + 1023) / 1024;
+        const int E = cached ? kPerThread : (n + 1023) / 1024;
         const int i0 = min(n, tid * E), i1 = min(n, i0 + E);
         unsigned long long mine = 0;  // greater | equal << 32 among this thread's elements
         if (all) {
             if (MODE == 2) { for (int i = i0; i < i1; ++i) mine += ci[i] >= 0 ? 1ull : 0ull; }
             else mine = (unsigned long long)(i1 - i0);
         } else
-            for (int i = i0; i < i1; ++i) {
-                const uint32_t u = cached ? s_keys[i + (i >> 5)] : keyat(i);
-                mine += (u > Ts ? 1ull : 0ull) + (u == Ts ? (1ull << 32) : 0ull);
+            if (cached) {
+#pragma unroll
+                for (int j = 0; j < kPerThread; ++j)
+                    if (i0 + j < i1) mine += (kv[j] > Ts ? 1ull : 0ull) + (kv[j] == Ts ? (1ull << 32) : 0ull);
+            } else {
+                for (int i = i0; i < i1; ++i) {
+                    const uint32_t u = keyat(i);
+                    mine += (u > Ts ? 1ull : 0ull) + (u == Ts ? (1ull << 32) : 0ull);
+                }
             }
         // block-wide exclusive scan of the packed counts
         unsigned long long incl = mine;
@@ -212,23 +232,29 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
         const unsigned long long before = s_warp[warp] + incl - mine;
         int gt_before = (int)(uint32_t)before, eq_before = (int)(before >> 32);
         count = s_krem;
-        for (int i = i0; i < i1; ++i) {
+        auto emit = [&](int i, uint32_t u) {
             bool gt = all, eq = false;
             if (all) {
                 if (MODE == 2) gt = ci[i] >= 0;
             } else {
-                const uint32_t u = cached ? s_keys[i + (i >> 5)] : keyat(i);
                 gt = u > Ts;
                 eq = u == Ts;
             }
             const bool take = gt || (eq && eq_before < take_eq);
             const int pos = gt_before + min(eq_before, take_eq);
             if (take && pos < cap) {
-                if (MODE == 1) { okey[pos] = keyat(i); oidx[pos] = idxat(i); }
+                if (MODE == 1) { okey[pos] = all ? keyat(i) : u; oidx[pos] = idxat(i); }
                 else out[pos] = idxat(i) * kB;
             }
             gt_before += gt ? 1 : 0;
             eq_before += eq ? 1 : 0;
+        };
+        if (cached && !all) {
+#pragma unroll
+            for (int j = 0; j < kPerThread; ++j)
+                if (i0 + j < i1) emit(i0 + j, kv[j]);
+        } else {
+            for (int i = i0; i < i1; ++i) emit(i, all ? 0u : keyat(i));
         }
     }
     count = min(count, cap);
@@ -249,23 +275,14 @@ cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_
     if (err != cudaSuccess) return err;
     const int n_slices = (g.score_stride + kKeyCap - 1) / kKeyCap;
     const int cand_cap = budget / kB + 1 < kKeyCap ? budget / kB + 1 : kKeyCap;  // candidates kept per slice
-    const int n_keys = n_slices > 1 ? kKeyCap : g.score_stride;
-    const int key_bytes = 4 * (n_keys + n_keys / 32 + 1);
-    static int configured = 0;
-    if (key_bytes > configured) {
-        if ((err = cudaFuncSetAttribute(mkv_topk_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, key_bytes)) != cudaSuccess) return err;
-        if ((err = cudaFuncSetAttribute(mkv_topk_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, key_bytes)) != cudaSuccess) return err;
-        if ((err = cudaFuncSetAttribute(mkv_topk_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, key_bytes)) != cudaSuccess) return err;
-        configured = key_bytes;
-    }
     if (n_slices == 1) {
-        mkv_topk_kernel<0><<<g.n_units, 1024, key_bytes, s>>>(g, lv, scores, budget, sel, sel_count, k_max, nullptr, nullptr, 1, 0);
+        mkv_topk_kernel<0><<<g.n_units, 1024, 0, s>>>(g, lv, scores, budget, sel, sel_count, k_max, nullptr, nullptr, 1, 0);
         if (n_kernels) *n_kernels = 2;
     } else {
-        mkv_topk_kernel<1><<<g.n_units * n_slices, 1024, key_bytes, s>>>(g, lv, scores, budget, sel, sel_count, k_max,
+        mkv_topk_kernel<1><<<g.n_units * n_slices, 1024, 0, s>>>(g, lv, scores, budget, sel, sel_count, k_max,
                                                                          cand_key, cand_idx, n_slices, cand_cap);
         if ((err = cudaGetLastError()) != cudaSuccess) return err;
-        mkv_topk_kernel<2><<<g.n_units, 1024, key_bytes, s>>>(g, lv, scores, budget, sel, sel_count, k_max, cand_key,
+        mkv_topk_kernel<2><<<g.n_units, 1024, 0, s>>>(g, lv, scores, budget, sel, sel_count, k_max, cand_key,
                                                               cand_idx, n_slices, cand_cap);
         if (n_kernels) *n_kernels = 3;
     }
