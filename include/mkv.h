@@ -178,7 +178,8 @@ MKV_API int mkv_packed_attention(const mkv_cache* cache, int32_t layer, const vo
  *           number of full segments, else MKV_E_STATE.  Flushing fewer than segment_len tokens
  *           leaves a short last segment, after which nothing can be appended to the packed cache.
  *   count:  tokens currently buffered per unit (host value; no synchronisation).
- * mkv_cache_reset also empties the buffer.
+ * mkv_cache_reset also empties the buffer.  The count lives in device memory and is updated on the stream, so a
+ * captured CUDA graph of mkv_packed_attention stays valid across appends and flushes.
  */
 MKV_API int mkv_update_append(mkv_cache* cache, int32_t layer, const void* k_new, const void* v_new,
                       int64_t stride_b, int64_t stride_h, int64_t stride_t, int32_t n_new,

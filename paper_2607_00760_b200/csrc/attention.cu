@@ -139,7 +139,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                             const int32_t* __restrict__ sel, const int32_t* __restrict__ sel_count, int k_max,
                             float scale_log2, float* __restrict__ out, float* __restrict__ lse,
                             float* __restrict__ part_o, float* __restrict__ part_ml, int32_t* __restrict__ ticket,
-                            const uint16_t* __restrict__ upd_k, const uint16_t* __restrict__ upd_v, int n_buf) {
+                            const uint16_t* __restrict__ upd_k, const uint16_t* __restrict__ upd_v,
+                            const int32_t* __restrict__ upd_count) {
     extern __shared__ __align__(128) uint8_t smem[];
     constexpr int kWS = warp_smem_bytes(NSTAGE);
     constexpr int kNT = kWarps * 32;
@@ -165,6 +166,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     }
     if (lane < 2) s_unit[warp * 2 + lane] = -1;
 
+    // tokens in the layer's update buffer: device-resident, so a captured graph stays valid across appends
+    const int n_buf = min(max(*upd_count, 0), g.L);
     const int upd_blocks = (n_buf + kB - 1) / kB;  // every unit ends with the blocks of its update buffer
     const int T = scan_counts(sel_count, g.n_units, k_max, upd_blocks, s_cum);  // (block barrier inside)
     const unsigned Gd = min(gridDim.x, (unsigned)max(T, 1));        // CTAs that own >= 1 block
@@ -666,8 +669,8 @@ int attention_partial_slots(int sm_count) { return sm_count * kMaxWarps * 2 + sm
 template <int NSTAGE, int NWARPS>
 static cudaError_t launch_attention_cfg(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
                                         const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
-                                        const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v, int n_buf,
-                                        int sm_count, cudaStream_t s) {
+                                        const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v,
+                                        const int32_t* upd_count, int sm_count, cudaStream_t s) {
     const int smem = NWARPS * warp_smem_bytes(NSTAGE) + (g.n_units + 1) * 4;
     static int configured = 0;  // largest dynamic shared-memory size opted into so far
     if (smem > configured) {
@@ -677,14 +680,14 @@ static cudaError_t launch_attention_cfg(const CacheGeom& g, const LayerView& lv,
         configured = smem;
     }
     mkv_packed_attention_kernel<NSTAGE, NWARPS><<<sm_count, NWARPS * 32, smem, s>>>(
-        g, lv, q, sel, sel_count, k_max, scale * kLog2e, out, lse, scr.part_o, scr.part_ml, scr.ticket, upd_k, upd_v, n_buf);
+        g, lv, q, sel, sel_count, k_max, scale * kLog2e, out, lse, scr.part_o, scr.part_ml, scr.ticket, upd_k, upd_v, upd_count);
     return cudaGetLastError();
 }
 
 cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
                              const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
-                             const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v, int n_buf,
-                             int sm_count, cudaStream_t s, int* n_kernels) {
+                             const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v,
+                             const int32_t* upd_count, int sm_count, cudaStream_t s, int* n_kernels) {
     if (g.n_units > kMaxUnitsSmem) return cudaErrorInvalidValue;
     if (n_kernels) *n_kernels = 1;
     static int cfg = -1;  // tuning knob (stages * 100 + warps); default chosen from measurements
@@ -693,10 +696,10 @@ cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint
         cfg = e ? atoi(e) : 316;
     }
 #define MKV_CFG(S, W) \
-    case S * 100 + W: return launch_attention_cfg<S, W>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, n_buf, sm_count, s);
+    case S * 100 + W: return launch_attention_cfg<S, W>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, upd_count, sm_count, s);
     switch (cfg) {
         MKV_CFG(3, 16) MKV_CFG(2, 16) MKV_CFG(2, 20) MKV_CFG(2, 24) MKV_CFG(4, 12) MKV_CFG(4, 8)
-        default: return launch_attention_cfg<3, 16>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, n_buf, sm_count, s);
+        default: return launch_attention_cfg<3, 16>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, upd_count, sm_count, s);
     }
 #undef MKV_CFG
 }

@@ -376,7 +376,9 @@ __global__ void mkv_strategy_threshold_kernel(const double* __restrict__ loss_k,
 // and one V row (256 B each, 8 B per lane).
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) mkv_update_copy_kernel(CacheGeom g, CompressArgs a, uint16_t* __restrict__ upd_k,
-                                                              uint16_t* __restrict__ upd_v, int n_have) {
+                                                              uint16_t* __restrict__ upd_v,
+                                                              int32_t* __restrict__ upd_count, int n_have) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) *upd_count = n_have + a.n_tok;
     const int row = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (row >= g.n_units * a.n_tok) return;
     const int unit = row / a.n_tok, t = row - unit * a.n_tok;
@@ -393,10 +395,10 @@ __global__ void __launch_bounds__(256) mkv_update_copy_kernel(CacheGeom g, Compr
 
 }  // namespace
 
-cudaError_t launch_update_copy(const CacheGeom& g, const CompressArgs& a, uint16_t* upd_k, uint16_t* upd_v, int n_have,
-                               cudaStream_t s) {
+cudaError_t launch_update_copy(const CacheGeom& g, const CompressArgs& a, uint16_t* upd_k, uint16_t* upd_v,
+                               int32_t* upd_count, int n_have, cudaStream_t s) {
     const int rows = g.n_units * a.n_tok;
-    mkv_update_copy_kernel<<<(rows + 7) / 8, 256, 0, s>>>(g, a, upd_k, upd_v, n_have);
+    mkv_update_copy_kernel<<<(rows + 7) / 8, 256, 0, s>>>(g, a, upd_k, upd_v, upd_count, n_have);
     return cudaGetLastError();
 }
 

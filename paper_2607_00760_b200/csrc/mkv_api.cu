@@ -56,7 +56,8 @@ struct mkv_cache {
     int32_t* cand_idx = nullptr;
     uint16_t* upd_k = nullptr;                // KV update buffer, raw bf16 [n_layers][n_units][L][D]
     uint16_t* upd_v = nullptr;
-    std::vector<int32_t> upd_n;               // tokens buffered per layer (every unit holds the same number)
+    int32_t* upd_cnt = nullptr;               // [n_layers] tokens buffered per unit (read by the attention kernel)
+    std::vector<int32_t> upd_n;               // host mirror (every unit of a layer holds the same number)
     AttnScratch attn{};
     uint16_t* q_dev = nullptr;
     int32_t* sel_dev = nullptr;
@@ -96,7 +97,7 @@ int mkv_cache_free(mkv_cache* c) {
     cudaSetDevice(c->desc.device);
     cudaDeviceSynchronize();
     void* ptrs[] = {c->arena, c->strat, c->tok_off, c->bk_off, c->unit_nseg, c->unit_ntok, c->counters,
-                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->upd_k, c->upd_v, c->attn.part_o, c->attn.part_ml, c->attn.ticket, c->q_dev,
+                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->upd_k, c->upd_v, c->upd_cnt, c->attn.part_o, c->attn.part_ml, c->attn.ticket, c->q_dev,
                     c->sel_dev, c->selcnt_dev, c->out_dev, c->cands_dev};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -160,6 +161,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         {(void**)&c->cand_idx, cand_bytes},
         {(void**)&c->upd_k, upd_bytes},
         {(void**)&c->upd_v, upd_bytes},
+        {(void**)&c->upd_cnt, (size_t)g.n_layers * 4 + 252},
         {(void**)&c->attn.part_o, (size_t)c->attn.slots * g.group * kD * 4},
         {(void**)&c->attn.part_ml, (size_t)c->attn.slots * kMaxGroup * 2 * 4},
         {(void**)&c->attn.ticket, (size_t)g.n_units * 4},
@@ -181,6 +183,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     cudaMemset(c->unit_ntok, 0, tu * 4);
     cudaMemset(c->counters, 0, (size_t)g.n_layers * 4 * 8);
     cudaMemset(c->dev_flags, 0, 256);
+    cudaMemset(c->upd_cnt, 0, (size_t)g.n_layers * 4);
     cudaMemset(c->attn.ticket, 0, (size_t)g.n_units * 4);
     cudaMemset(c->strat, 0, tu * g.S_max * sizeof(StratRec));
     c->host_nseg.assign((size_t)g.n_layers * g.batch, 0);
@@ -205,6 +208,7 @@ int mkv_cache_reset(mkv_cache* c, int32_t layer, void* stream) {
         MKV_CUDA(cudaMemsetAsync(c->unit_ntok + (size_t)l * g.n_units, 0, (size_t)g.n_units * 4, s));
         MKV_CUDA(cudaMemsetAsync(c->counters + (size_t)l * 4, 0, 32, s));
         for (int b = 0; b < g.batch; ++b) c->host_nseg[(size_t)l * g.batch + b] = c->host_ntok[(size_t)l * g.batch + b] = 0;
+        MKV_CUDA(cudaMemsetAsync(c->upd_cnt + l, 0, 4, s));
         c->upd_n[l] = 0;
     }
     return MKV_OK;
@@ -313,7 +317,7 @@ int mkv_packed_attention(const mkv_cache* cc, int32_t layer, const void* q, cons
     MKV_CUDA(cudaSetDevice(c->desc.device));
     const size_t upd_off = (size_t)layer * g.n_units * g.L * kD;
     MKV_CUDA(launch_attention(g, c->view(layer), (const uint16_t*)q, sel, sel_count, k_max, scale, out, lse_opt,
-                              c->attn, c->upd_k + upd_off, c->upd_v + upd_off, c->upd_n[layer], c->sm_count,
+                              c->attn, c->upd_k + upd_off, c->upd_v + upd_off, c->upd_cnt + layer, c->sm_count,
                               (cudaStream_t)stream, &c->last_attn));
     return MKV_OK;
 }
@@ -331,7 +335,7 @@ int mkv_update_append(mkv_cache* c, int32_t layer, const void* k_new, const void
     CompressArgs a{(const uint16_t*)k_new, (const uint16_t*)v_new, sb, sh, st, 0, g.batch, 0, 1, n_new};
     MKV_CUDA(cudaSetDevice(c->desc.device));
     const size_t off = (size_t)layer * g.n_units * g.L * kD;
-    MKV_CUDA(launch_update_copy(g, a, c->upd_k + off, c->upd_v + off, have, (cudaStream_t)stream));
+    MKV_CUDA(launch_update_copy(g, a, c->upd_k + off, c->upd_v + off, c->upd_cnt + layer, have, (cudaStream_t)stream));
     c->upd_n[layer] = have + n_new;
     return MKV_OK;
 }
@@ -352,6 +356,7 @@ int mkv_update_flush(mkv_cache* c, int32_t layer, const mkv_strategy* strat, voi
     const int rc = mkv_compress_segment(c, layer, c->upd_k + off, c->upd_v + off, sb, sh, kD, 0, g.batch, seg0, 1, n, strat,
                                         stream);
     if (rc) return rc;
+    MKV_CUDA(cudaMemsetAsync(c->upd_cnt + layer, 0, 4, (cudaStream_t)stream));
     c->upd_n[layer] = 0;
     return MKV_OK;
 }

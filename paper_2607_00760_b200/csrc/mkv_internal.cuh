@@ -94,10 +94,12 @@ int attention_partial_slots(int sm_count);
 cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q,
                              const int32_t* sel, const int32_t* sel_count, int k_max, float scale,
                              float* out, float* lse, const AttnScratch& scr, const uint16_t* upd_k,
-                             const uint16_t* upd_v, int n_buf, int sm_count, cudaStream_t s, int* n_kernels);
+                             const uint16_t* upd_v, const int32_t* upd_count, int sm_count, cudaStream_t s,
+                             int* n_kernels);
 // KV update buffer: copy n_new raw tokens of every unit into rows [n_have, n_have + n_new)
+// and set the layer's device-side count to n_have + n_new
 cudaError_t launch_update_copy(const CacheGeom& g, const CompressArgs& a, uint16_t* upd_k, uint16_t* upd_v,
-                               int n_have, cudaStream_t s);
+                               int32_t* upd_count, int n_have, cudaStream_t s);
 
 // ---- small device helpers -----------------------------------------------------------------
 __device__ __forceinline__ float bf16_bits_to_f32(uint32_t h) { return __uint_as_float(h << 16); }
