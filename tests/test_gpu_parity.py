@@ -46,6 +46,69 @@ def test_tiny_config_end_to_end(env):
         c.free()
 
 
+# ------------------------------------------------------------------ config 2 at full size (the bench's launch configuration)
+
+def test_full_size_config2_sampled_units(env):
+    """BASELINE config 2 (batch 8, 8 KV heads, 131 072 tokens, budget 4096, 10 % dense by the quantile rule), one
+    layer, built exactly as bench.py builds it (same generator, same kernels, same grids).  The oracle recomputes
+    sampled units from the raw bytes the GPU consumed: strategy table, packed blob (bit-exact), selection (tie-band
+    protocol) and attention output on the GPU's own selection."""
+    mkv, dev = env
+    import torch
+    from paper_2607_00760_b200 import synth, workload
+    w = synth.WORKLOADS["llama8b-128k-b8"]
+    units = [(0, 0, 0), (0, 3, 5), (0, 7, 7)]
+    built = workload.build(w, dev, n_layers=1, keep_units=units)
+    cache = built.cache
+    try:
+        Bt, Hkv, Hq, G, N, L = w.batch, w.n_kv_heads, w.n_q_heads, w.group, w.context, w.segment_len
+        budget, scale = w.token_budget, 1.0 / math.sqrt(128)
+        k_max = budget // 8 + 1
+        sel = torch.full((Bt, Hkv, k_max), -1, dtype=torch.int32, device=dev)
+        cnt = torch.zeros((Bt, Hkv), dtype=torch.int32, device=dev)
+        out = torch.zeros((Bt, Hq, 128), dtype=torch.float32, device=dev)
+        lse = torch.zeros((Bt, Hq), dtype=torch.float32, device=dev)
+        cache.select(0, built.q[0], budget, sel, cnt)
+        cache.packed_attention(0, built.q[0], sel, cnt, scale, out, lse)
+        torch.cuda.synchronize()
+        cache.status()
+        sel_h, cnt_h = sel.cpu().numpy(), cnt.cpu().numpy()
+        out_h, lse_h = out.cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64)
+        q_h = built.q[0].view(torch.int16).cpu().numpy().view(np.uint16)
+        strat_h = built.strat[0].cpu().numpy()
+        total = swaps = 0
+        for (_, b, h) in units:
+            K, V = built.raw_units[(0, b, h)]
+            lk, lv = orc.segment_loss(K, V, L, w.r_keep, w.r_keep)
+            st = orc.strategy_quantile(lk, lv, w.dense_num, w.dense_den, 128, w.r_keep, w.r_keep)
+            np.testing.assert_array_equal(strat_h[b, h], st)
+            blob = orc.compress_unit(K, V, L, st)
+            np.testing.assert_array_equal(cache.export(0, b, h), blob)
+            qh = q_h[b, h * G:(h + 1) * G]
+            ft, nt = orc.blob_blocks(blob)
+            s = orc.scores(blob, qh, 0)
+            ref = orc.topk(s, ft, nt, budget)
+            n = int(cnt_h[b, h])
+            got = sel_h[b, h, :n]
+            assert n == len(ref) and np.all(np.diff(got) > 0) and np.all(sel_h[b, h, n:] == -1)
+            total += n
+            if not np.array_equal(got, ref):
+                diff = np.setxor1d(got, ref)
+                kth = np.sort(s)[::-1][len(ref) - 1]
+                band = 1e-5 * max(abs(kth), 1e-3 * np.abs(s).max())
+                assert np.all(np.abs(s[diff // 8] - kth) <= band), "selection differs outside the tie band"
+                swaps += len(diff) // 2
+            o, l = orc.attention(blob, qh, got, scale)
+            assert_attention_close(out_h[b:b + 1, h * G:(h + 1) * G], lse_h[b:b + 1, h * G:(h + 1) * G], o[None], l[None])
+        assert swaps <= max(1, total // 10000)
+        # properties that hold for every unit: counts, order, range
+        assert np.all(cnt_h == budget // 8)
+        assert np.all(np.diff(sel_h[:, :, :budget // 8], axis=-1) > 0) and sel_h.max() < N and np.all(sel_h[:, :, :budget // 8] % 8 == 0)
+        assert np.all(np.isfinite(out_h)) and np.all(np.isfinite(lse_h))
+    finally:
+        built.free()
+
+
 # ------------------------------------------------------------------ step 1
 
 @pytest.mark.parametrize("r_k,r_v", [(38, 38), (128, 128), (1, 127), (90, 64), (128, 38), (38, 128), (64, 1)])
