@@ -220,6 +220,13 @@ def run_mkv(args):
     ms_sel = timed_loop(torch, step_select, args.steps, args.warmup, barrier, graph)
     clk = clocks.stop()
 
+    # calibration: the attention kernel's own staging of the same selected payloads with all arithmetic removed
+    def step_gather():
+        for l in range(n_layers):
+            cache.calibrate_gather(l, sel[l], cnt[l])
+
+    ms_gather = timed_loop(torch, step_gather, args.steps, args.warmup, barrier, graph)
+
     # end to end through the public host call: pinned q in, out back, every layer, every step
     q_host = [q.cpu().pin_memory() for q in built.q]
     out_host = [torch.zeros((Bt, Hq, 128), dtype=torch.float32).pin_memory() for _ in range(n_layers)]
@@ -279,6 +286,10 @@ def run_mkv(args):
                 "launch": "cuda-graph of one decode step of mkv_decode_host calls" if graph else "eager, synchronised per step",
                 "h2d_bytes_per_step": n_layers * Bt * Hq * 128 * 2, "d2h_bytes_per_step": n_layers * Bt * Hq * 128 * 4,
                 "ms_per_step": round(ms_e2e, 4)},
+        "calibration": {"gather_only_us_per_layer": round(ms_gather * 1e3 / n_layers, 3),
+                        "gather_only_gbs": round(a_bytes / (ms_gather * 1e-3 / n_layers) / 1e9, 1),
+                        "what": "mkv_calibrate_gather: same kernel, launch configuration and selected payloads as "
+                                "mkv_packed_attention, bulk-copy staging only (no walk, no MMA, no output)"},
         "gpu_launches": args.steps * n_layers * (launches["select"] + launches["attention"]),
         "kernels_per_layer": launches,
         "clocks": clk,

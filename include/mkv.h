@@ -198,6 +198,15 @@ MKV_API int mkv_decode_host(mkv_cache* cache, int32_t layer, const void* q_host,
                     int32_t reduce, float softmax_scale, float* out_host, int32_t* sel_host_opt,
                     int32_t* sel_count_host_opt, void* stream);
 
+/*
+ * Measurement aid (SURVEY 8(d) calibration row): the PackedAttention kernel in the same launch
+ * configuration with all arithmetic removed — every selected token-block payload is staged into
+ * shared memory exactly as in mkv_packed_attention and one word per lane is read back; nothing is
+ * written.  Its time is the ceiling the memory side sets for this access pattern.
+ */
+MKV_API int mkv_calibrate_gather(const mkv_cache* cache, int32_t layer, const int32_t* sel,
+                         const int32_t* sel_count, int32_t k_max, void* stream);
+
 /* Parity / dump: canonical blob of unit (layer, b, h) into host memory.  *need_host receives the
  * blob size; if cap < need nothing is copied and MKV_E_ARG is returned.  Synchronises. */
 MKV_API int mkv_cache_export(const mkv_cache* cache, int32_t layer, int32_t b, int32_t h, void* buf_host,

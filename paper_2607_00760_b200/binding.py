@@ -23,7 +23,7 @@ MKV_DEV_ARENA_OVERFLOW, MKV_DEV_BAD_STRATEGY = 1, 2
 # every symbol include/mkv.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ["mkv_cache_create", "mkv_cache_free", "mkv_cache_reset", "mkv_segment_loss",
            "mkv_strategy_quantile", "mkv_strategy_threshold", "mkv_compress_segment", "mkv_select",
-           "mkv_packed_attention", "mkv_update_append", "mkv_update_flush", "mkv_update_count", "mkv_decode_host", "mkv_cache_export", "mkv_cache_bytes",
+           "mkv_packed_attention", "mkv_update_append", "mkv_update_flush", "mkv_update_count", "mkv_calibrate_gather", "mkv_decode_host", "mkv_cache_export", "mkv_cache_bytes",
            "mkv_cache_status", "mkv_last_launch_count", "mkv_last_error", "mkv_version"]
 
 
@@ -53,6 +53,7 @@ _lib.mkv_packed_attention.argtypes = [_vp, _i32, _vp, _vp, _vp, _i32, C.c_float,
 _lib.mkv_update_append.argtypes = [_vp, _i32, _vp, _vp, _i64, _i64, _i64, _i32, _vp]
 _lib.mkv_update_flush.argtypes = [_vp, _i32, _vp, _vp]
 _lib.mkv_update_count.argtypes = [_vp, _i32, C.POINTER(_i32)]
+_lib.mkv_calibrate_gather.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp]
 _lib.mkv_decode_host.argtypes = [_vp, _i32, _vp, _i32, _i32, C.c_float, _vp, _vp, _vp, _vp]
 _lib.mkv_cache_export.argtypes = [_vp, _i32, _i32, _i32, _vp, _u64, C.POINTER(_u64)]
 _lib.mkv_cache_bytes.argtypes = [_vp, _i32, C.POINTER(_u64), C.POINTER(_u64), C.POINTER(_u64)]
@@ -192,6 +193,10 @@ def mkv_update_count(cache, layer) -> int:
     return n.value
 
 
+def mkv_calibrate_gather(cache, layer, sel, sel_count, stream=None):
+    _check(_lib.mkv_calibrate_gather(cache, layer, _ptr(sel), _ptr(sel_count), sel.shape[-1], _stream(stream)))
+
+
 def mkv_decode_host(cache, layer, q_host, token_budget, softmax_scale, out_host, reduce=0,
                     sel_host=None, sel_count_host=None, stream=None):
     _check(_lib.mkv_decode_host(cache, layer, _ptr(q_host), token_budget, reduce, float(softmax_scale),
@@ -292,6 +297,9 @@ class Cache:
 
     def update_count(self, layer):
         return mkv_update_count(self.h, layer)
+
+    def calibrate_gather(self, layer, sel, sel_count, stream=None):
+        mkv_calibrate_gather(self.h, layer, sel, sel_count, stream)
 
     def decode_host(self, layer, q_host, token_budget, softmax_scale, out_host, reduce=0,
                     sel_host=None, sel_count_host=None, stream=None):

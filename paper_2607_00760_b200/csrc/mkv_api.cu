@@ -322,6 +322,22 @@ int mkv_packed_attention(const mkv_cache* cc, int32_t layer, const void* q, cons
     return MKV_OK;
 }
 
+int mkv_calibrate_gather(const mkv_cache* cc, int32_t layer, const int32_t* sel, const int32_t* sel_count, int32_t k_max,
+                         void* stream) {
+    if (!cc || !sel || !sel_count) return fail(MKV_E_ARG, "mkv_calibrate_gather: NULL argument");
+    mkv_cache* c = const_cast<mkv_cache*>(cc);
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    if (k_max < 1) return fail(MKV_E_ARG, "mkv_calibrate_gather: k_max < 1");
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    const size_t upd_off = (size_t)layer * g.n_units * g.L * kD;
+    int n = 0;
+    MKV_CUDA(launch_attention(g, c->view(layer), c->q_dev, sel, sel_count, k_max, 1.f, c->out_dev, nullptr, c->attn,
+                              c->upd_k + upd_off, c->upd_v + upd_off, c->upd_cnt + layer, c->sm_count,
+                              (cudaStream_t)stream, &n, true));
+    return MKV_OK;
+}
+
 int mkv_update_append(mkv_cache* c, int32_t layer, const void* k_new, const void* v_new, int64_t sb, int64_t sh,
                       int64_t st, int32_t n_new, void* stream) {
     if (!c || !k_new || !v_new) return fail(MKV_E_ARG, "mkv_update_append: NULL argument");

@@ -95,7 +95,7 @@ cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint
                              const int32_t* sel, const int32_t* sel_count, int k_max, float scale,
                              float* out, float* lse, const AttnScratch& scr, const uint16_t* upd_k,
                              const uint16_t* upd_v, const int32_t* upd_count, int sm_count, cudaStream_t s,
-                             int* n_kernels);
+                             int* n_kernels, bool gather_only = false);
 // KV update buffer: copy n_new raw tokens of every unit into rows [n_have, n_have + n_new)
 // and set the layer's device-side count to n_have + n_new
 cudaError_t launch_update_copy(const CacheGeom& g, const CompressArgs& a, uint16_t* upd_k, uint16_t* upd_v,
