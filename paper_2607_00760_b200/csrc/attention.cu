@@ -167,6 +167,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         mbar_init_fence();
     }
     if (lane < 2) s_unit[warp * 2 + lane] = -1;
+    pdl_wait();               // the producer of sel / sel_count / the cache (and the previous user of the scratch) is done
+    pdl_launch_dependents();  // the next kernel may be scheduled as SMs free up
 
     // tokens in the layer's update buffer: device-resident, so a captured graph stays valid across appends
     const int n_buf = min(max(*upd_count, 0), g.L);
@@ -696,9 +698,9 @@ static cudaError_t launch_attention_cfg(const CacheGeom& g, const LayerView& lv,
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    mkv_packed_attention_kernel<NSTAGE, NWARPS, GATHER><<<sm_count, NWARPS * 32, smem, s>>>(
-        g, lv, q, sel, sel_count, k_max, scale * kLog2e, out, lse, scr.part_o, scr.part_ml, scr.ticket, upd_k, upd_v, upd_count);
-    return cudaGetLastError();
+    return launch_pdl(mkv_packed_attention_kernel<NSTAGE, NWARPS, GATHER>, dim3(sm_count), dim3(NWARPS * 32), (size_t)smem, s,
+                      g, lv, q, sel, sel_count, k_max, scale * kLog2e, out, lse, scr.part_o, scr.part_ml, scr.ticket, upd_k,
+                      upd_v, upd_count);
 }
 
 cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,

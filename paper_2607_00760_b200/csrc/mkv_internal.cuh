@@ -101,6 +101,29 @@ cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint
 cudaError_t launch_update_copy(const CacheGeom& g, const CompressArgs& a, uint16_t* upd_k, uint16_t* upd_v,
                                int32_t* upd_count, int n_have, cudaStream_t s);
 
+// ---- programmatic dependent launch (PDL) ----------------------------------------------------
+// The decode kernels are launched with programmatic stream serialisation: kernel N+1 may be scheduled
+// while kernel N drains, runs its global-memory-free preamble, and blocks in pdl_wait() until kernel N
+// has completed and flushed.  Inside a captured CUDA graph this removes the launch gap between the
+// three kernels of a decode step.  Everything a kernel reads or writes in global memory comes after
+// pdl_wait(); pdl_launch_dependents() right after it lets the next kernel start as SMs free up.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,
+                              Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+#endif
+
 // ---- small device helpers -----------------------------------------------------------------
 __device__ __forceinline__ float bf16_bits_to_f32(uint32_t h) { return __uint_as_float(h << 16); }
 

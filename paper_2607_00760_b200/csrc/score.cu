@@ -63,6 +63,8 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
     const int gq = lane >> 2, qq = lane & 3;
     const int G = g.group;
 
+    pdl_wait();               // the cache and q are complete; the previous reader of `scores` is done
+    pdl_launch_dependents();
     const unsigned I = (unsigned)g.n_units * items_per_unit;  // < 2^32: checked by the launcher
     const unsigned GW = gridDim.x * kWarps, gw = blockIdx.x * kWarps + warp;
     const unsigned ib = I / GW, ir = I - ib * GW;             // the first ir warps hold one more item
@@ -258,9 +260,8 @@ static cudaError_t launch_score_cfg(const CacheGeom& g, const LayerView& lv, con
     }
     const int subs = (g.blocks_per_seg + 7) / 8;
     if ((unsigned long long)g.n_units * g.S_max * subs >= (1ull << 32)) return cudaErrorInvalidValue;
-    mkv_score_kernel<NSTAGE, NWARPS><<<sm_count, NWARPS * 32, smem, s>>>(g, lv, q, reduce, subs,
-                                                                         (unsigned)g.S_max * (unsigned)subs, scores);
-    return cudaGetLastError();
+    return launch_pdl(mkv_score_kernel<NSTAGE, NWARPS>, dim3(sm_count), dim3(NWARPS * 32), (size_t)smem, s, g, lv, q, reduce,
+                      subs, (unsigned)g.S_max * (unsigned)subs, scores);
 }
 
 cudaError_t launch_score(const CacheGeom& g, const LayerView& lv, const uint16_t* q, int reduce, float* scores,

@@ -51,6 +51,8 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
     const int unit = MODE == 1 ? blockIdx.x / n_slices : blockIdx.x;
     const int slice = MODE == 1 ? blockIdx.x % n_slices : 0;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    pdl_wait();  // the scores (MODE 0, 1) / the candidates (MODE 2) are complete
+    pdl_launch_dependents();
     const int ntok = lv.unit_ntok[unit];
     const int nblk = (ntok + kB - 1) / kB;        // blocks of the unit
     const float* s = scores + (size_t)unit * g.score_stride;
@@ -276,14 +278,17 @@ cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_
     const int n_slices = (g.score_stride + kKeyCap - 1) / kKeyCap;
     const int cand_cap = budget / kB + 1 < kKeyCap ? budget / kB + 1 : kKeyCap;  // candidates kept per slice
     if (n_slices == 1) {
-        mkv_topk_kernel<0><<<g.n_units, 1024, 0, s>>>(g, lv, scores, budget, sel, sel_count, k_max, nullptr, nullptr, 1, 0);
+        err = launch_pdl(mkv_topk_kernel<0>, dim3(g.n_units), dim3(1024), 0, s, g, lv, (const float*)scores, budget, sel,
+                         sel_count, k_max, (uint32_t*)nullptr, (int32_t*)nullptr, 1, 0);
+        if (err != cudaSuccess) return err;
         if (n_kernels) *n_kernels = 2;
     } else {
-        mkv_topk_kernel<1><<<g.n_units * n_slices, 1024, 0, s>>>(g, lv, scores, budget, sel, sel_count, k_max,
-                                                                         cand_key, cand_idx, n_slices, cand_cap);
-        if ((err = cudaGetLastError()) != cudaSuccess) return err;
-        mkv_topk_kernel<2><<<g.n_units, 1024, 0, s>>>(g, lv, scores, budget, sel, sel_count, k_max, cand_key,
-                                                              cand_idx, n_slices, cand_cap);
+        err = launch_pdl(mkv_topk_kernel<1>, dim3(g.n_units * n_slices), dim3(1024), 0, s, g, lv, (const float*)scores, budget,
+                         sel, sel_count, k_max, cand_key, cand_idx, n_slices, cand_cap);
+        if (err != cudaSuccess) return err;
+        err = launch_pdl(mkv_topk_kernel<2>, dim3(g.n_units), dim3(1024), 0, s, g, lv, (const float*)scores, budget, sel,
+                         sel_count, k_max, cand_key, cand_idx, n_slices, cand_cap);
+        if (err != cudaSuccess) return err;
         if (n_kernels) *n_kernels = 3;
     }
     return cudaGetLastError();
