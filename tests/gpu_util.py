@@ -170,4 +170,6 @@ def assert_attention_close(out, lse, ref, ref_lse):
     fin = np.isfinite(ref_lse)
     assert np.array_equal(np.isneginf(lse), np.isneginf(ref_lse))
     if fin.any():
-        assert np.abs(lse[fin] - ref_lse[fin]).max() <= 1e-3
+        # lse is an fp32 output: 1e-3 absolute, plus a few fp32 spacings of its own magnitude (DESIGN.md section 6:
+        # logits of the generator's heavy hitters reach several thousand, where one fp32 ulp is 2.4e-4)
+        assert np.all(np.abs(lse[fin] - ref_lse[fin]) <= 1e-3 + 2e-6 * np.abs(ref_lse[fin]))

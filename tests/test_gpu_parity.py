@@ -293,6 +293,51 @@ def test_select_with_massive_ties(env):
         c.free()
 
 
+@pytest.mark.parametrize("L", [8, 32, 128, 200])
+def test_other_segment_lengths_end_to_end(env, L):
+    """segment_len != 64: one block per segment (L = 8), the paper's update-buffer size (32), several score items
+    per segment (L = 128: two items of 8 block keys, L = 200: 25 blocks -> a ragged fourth item), ragged tail."""
+    mkv, dev = env
+    N = L * 9 + (L // 2 + 3 if L > 8 else 5)
+    c = Case(mkv, dev, 2, 2, 8, N, L=L, seed=90 + L)
+    try:
+        strat = uniform_strat(2, 2, c.S, 38, 50)
+        strat[:, :, ::3, 0:2] = 128
+        strat[:, :, 1::4, 0] = 90
+        c.compress(strat)
+        c.assert_export_equal()
+        tot = sw = 0
+        for budget in (8, 100, 333, N // 2, N):
+            t, s_ = c.check_select(budget)
+            tot += t
+            sw += s_
+        assert sw <= max(1, tot // 10000)
+        sel, cnt = c.oracle_sel(N // 2)
+        c.check_attention(sel, cnt)
+        sel, cnt = c.oracle_sel(N)
+        c.check_attention(sel, cnt)
+    finally:
+        c.free()
+
+
+def test_attention_empty_and_tiny_selections(env):
+    """no block selected anywhere (out = 0, lse = -inf), and a single block in one unit (fewer blocks than CTAs)"""
+    mkv, dev = env
+    c = Case(mkv, dev, 2, 2, 8, 64 * 5, seed=77)
+    try:
+        c.compress(uniform_strat(2, 2, c.S, 38))
+        sel = np.full((2, 2, 4), -1, np.int32)
+        cnt = np.zeros((2, 2), np.int32)
+        out, lse = c.gpu_attention(sel, cnt)
+        assert np.all(out == 0) and np.all(np.isneginf(lse))
+        sel[1, 0, 0] = 64 * 3 + 8
+        cnt[1, 0] = 1
+        out, _ = c.check_attention(sel, cnt)
+        assert np.all(out[0] == 0) and np.all(out[1, 4:] == 0) and np.any(out[1, :4] != 0)
+    finally:
+        c.free()
+
+
 def test_select_long_unit_two_stage(env):
     """a unit of more than 16384 blocks is selected in two stages (per-slice candidates, then a merge);
     ragged last block, budgets around the slice size and the ragged rule, then massive ties"""
