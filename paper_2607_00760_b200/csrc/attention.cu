@@ -174,14 +174,20 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     const int n_buf = min(max(*upd_count, 0), g.L);
     const int upd_blocks = (n_buf + kB - 1) / kB;  // every unit ends with the blocks of its update buffer
     const int T = scan_counts(sel_count, g.n_units, k_max, upd_blocks, s_cum);  // (block barrier inside)
-    const unsigned Gd = min(gridDim.x, (unsigned)max(T, 1));        // CTAs that own >= 1 block
-    Split cs;                                                       // blocks over CTAs
-    cs.b = (unsigned)T / Gd; cs.r = (unsigned)T - cs.b * Gd;
+    // The stream is split in units of two positions, so every range starts at an even position: with even
+    // selection counts (units then start at even positions too) a range never holds two odd runs, which
+    // would cost an extra half-empty group -- the slowest warp sets the kernel's time.
+    const unsigned P = ((unsigned)T + 1u) >> 1;                     // position pairs
+    const unsigned Gd = min(gridDim.x, max(P, 1u));                 // CTAs that own >= 1 pair
+    Split cs;                                                       // pairs over CTAs
+    cs.b = P / Gd; cs.r = P - cs.b * Gd;
     int clo = 0, chi = 0;
-    if (blockIdx.x < Gd) { clo = (int)cs.begin(blockIdx.x); chi = (int)cs.begin(blockIdx.x + 1); }
-    Split ws;                                                       // the CTA's blocks over its warps
-    ws.b = (unsigned)(chi - clo) / kWarps; ws.r = (unsigned)(chi - clo) % kWarps;
-    const int lo = clo + (int)ws.begin(warp), hi = clo + (int)ws.begin(warp + 1);
+    unsigned cplo = 0, cphi = 0;
+    if (blockIdx.x < Gd) { cplo = cs.begin(blockIdx.x); cphi = cs.begin(blockIdx.x + 1); }
+    clo = (int)(2u * cplo); chi = min((int)(2u * cphi), T);
+    Split ws;                                                       // the CTA's pairs over its warps
+    ws.b = (cphi - cplo) / kWarps; ws.r = (cphi - cplo) % kWarps;
+    const int lo = min(clo + 2 * (int)ws.begin(warp), chi), hi = min(clo + 2 * (int)ws.begin(warp + 1), chi);
     const unsigned gw = blockIdx.x * kWarps + warp;
     const int n_total = hi - lo;
     const int G = g.group;
@@ -623,8 +629,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     if ((tid == 0 || tid == 32) && (tid >> 5) < n_shared) {
         const int k = tid >> 5, u = k == 0 ? sh_u0 : sh_u1;
         int cf = (int)blockIdx.x, cl = (int)blockIdx.x;
-        if (s_cum[u] < clo) cf = (int)cs.owner((unsigned)s_cum[u]);
-        if (s_cum[u + 1] > chi) cl = (int)cs.owner((unsigned)s_cum[u + 1] - 1u);
+        if (s_cum[u] < clo) cf = (int)cs.owner((unsigned)s_cum[u] >> 1);
+        if (s_cum[u + 1] > chi) cl = (int)cs.owner(((unsigned)s_cum[u + 1] - 1u) >> 1);
         s_cf[k] = cf; s_cl[k] = cl;
         int old;  // release this CTA's partial (ordered by the barrier), acquire the other sharers'
         asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(ticket + u) : "memory");
