@@ -320,6 +320,37 @@ def test_other_segment_lengths_end_to_end(env, L):
         c.free()
 
 
+@pytest.mark.parametrize("seed", range(8))
+def test_attention_random_selections(env, seed):
+    """random unit shapes and selections: odd counts (units then start at odd stream positions), empty units,
+    blocks in arbitrary order, counts from 0 to every block, mixed strategies, ragged tail"""
+    mkv, dev = env
+    rng = np.random.default_rng(1000 + seed)
+    Hq, Hkv = [(8, 2), (7, 1), (4, 4), (8, 1), (16, 2), (6, 3), (2, 2), (5, 1)][seed]
+    Bt = int(rng.integers(1, 4))
+    N = int(rng.integers(9, 900))
+    c = Case(mkv, dev, Bt, Hkv, Hq, N, seed=300 + seed)
+    try:
+        strat = uniform_strat(Bt, Hkv, c.S, 38, 38)
+        pick = rng.integers(0, 4, size=(Bt, Hkv, c.S))
+        strat[..., 0] = np.choose(pick, [38, 128, 90, 7])
+        strat[..., 1] = np.choose(rng.integers(0, 4, size=(Bt, Hkv, c.S)), [38, 128, 64, 1])
+        c.compress(strat)
+        nblk = (N + 7) // 8
+        for rep in range(3):
+            k_max = int(rng.integers(1, nblk + 1))
+            sel = np.full((Bt, Hkv, k_max), -1, np.int32)
+            cnt = np.zeros((Bt, Hkv), np.int32)
+            for b in range(Bt):
+                for h in range(Hkv):
+                    k = int(rng.integers(0, k_max + 1))
+                    sel[b, h, :k] = rng.permutation(nblk)[:k] * 8  # arbitrary order
+                    cnt[b, h] = k
+            c.check_attention(sel, cnt)
+    finally:
+        c.free()
+
+
 def test_attention_empty_and_tiny_selections(env):
     """no block selected anywhere (out = 0, lse = -inf), and a single block in one unit (fewer blocks than CTAs)"""
     mkv, dev = env
