@@ -26,11 +26,15 @@ __device__ __forceinline__ unsigned lanemask_lt() {
 // (ties -> lower index).  Returns the four bitmap words in w (identical in all lanes).
 __device__ __forceinline__ void topr_mask(const uint32_t (&mag)[4], int r, uint32_t (&w)[4]) {
     uint32_t T = 0;
+    // two 15-bit magnitudes per register with bit 15 / 31 set: (pair - cand x 0x10001) keeps that bit exactly
+    // where mag >= cand, and no borrow crosses the halves -- four compares in two subtractions
+    const uint32_t p01 = mag[0] | (mag[1] << 16) | 0x80008000u, p23 = mag[2] | (mag[3] << 16) | 0x80008000u;
 #pragma unroll
     for (int bit = 14; bit >= 0; --bit) {
         const uint32_t cand = T | (1u << bit);
-        int c = (mag[0] >= cand) + (mag[1] >= cand) + (mag[2] >= cand) + (mag[3] >= cand);
-        c = __reduce_add_sync(kFull, c);
+        const uint32_t c2 = cand * 0x10001u;
+        const uint32_t z = ((p01 - c2) & 0x80008000u) | (((p23 - c2) >> 1) & 0x40004000u);
+        const int c = __reduce_add_sync(kFull, __popc(z));
         if (c >= r) T = cand;
     }
     int ngt = (mag[0] > T) + (mag[1] > T) + (mag[2] > T) + (mag[3] > T);
