@@ -29,8 +29,8 @@ UNIT = "us/layer"
 NOMINAL_HBM_GBS = 8000.0
 FALLBACK_HBM_GBS = 6650.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r1e_end_of_round.md), valid for the full-size default workload only
-NCU_TRAFFIC = {"llama8b-128k-b8": {"attention": 53390336 + 419328, "score+topk": 115729664 + 4312064 + 4235264}}
+# (profiles/r1f_final.md), valid for the full-size default workload only
+NCU_TRAFFIC = {"llama8b-128k-b8": {"attention": 53400000 + 430000, "score+topk": 115741000 + 4806000 + 4236000}}
 
 
 def parse():
