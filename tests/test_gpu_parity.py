@@ -100,7 +100,7 @@ def test_full_size_config2_sampled_units(env):
                 swaps += len(diff) // 2
             o, l = orc.attention(blob, qh, got, scale)
             assert_attention_close(out_h[b:b + 1, h * G:(h + 1) * G], lse_h[b:b + 1, h * G:(h + 1) * G], o[None], l[None])
-        assert swaps <= max(1, total // 10000)
+        assert swaps * 10000 <= total, f"{swaps} near-tie swaps in {total} selected blocks (bar: < 0.01 %)"
         # properties that hold for every unit: counts, order, range
         assert np.all(cnt_h == budget // 8)
         assert np.all(np.diff(sel_h[:, :, :budget // 8], axis=-1) > 0) and sel_h.max() < N and np.all(sel_h[:, :, :budget // 8] % 8 == 0)
@@ -178,7 +178,7 @@ def test_loss_and_quantile_strategy_match_oracle(env):
         c.compress(got)
         c.assert_export_equal()
         total, swaps = c.check_select(512)
-        assert swaps <= max(1, total // 10000)
+        assert swaps * 10000 <= total, f"{swaps} near-tie swaps in {total} selected blocks (bar: < 0.01 %)"
         sel, cnt = c.oracle_sel(512)
         c.check_attention(sel, cnt)
     finally:
@@ -268,7 +268,7 @@ def test_select_matches_oracle(env, Hq, Hkv, reduce):
             t, s = c.check_select(budget, reduce)
             tot += t
             sw += s
-        assert sw <= max(1, tot // 10000)
+        assert sw * 10000 <= tot, f"{sw} near-tie swaps in {tot} selected blocks (bar: < 0.01 %)"
     finally:
         c.free()
 
@@ -311,7 +311,7 @@ def test_other_segment_lengths_end_to_end(env, L):
             t, s_ = c.check_select(budget)
             tot += t
             sw += s_
-        assert sw <= max(1, tot // 10000)
+        assert sw * 10000 <= tot, f"{sw} near-tie swaps in {tot} selected blocks (bar: < 0.01 %)"
         sel, cnt = c.oracle_sel(N // 2)
         c.check_attention(sel, cnt)
         sel, cnt = c.oracle_sel(N)
@@ -384,7 +384,7 @@ def test_select_long_unit_two_stage(env):
             t, s = c.check_select(budget)
             tot += t
             sw += s
-        assert sw <= max(1, tot // 10000)
+        assert sw * 10000 <= tot, f"{sw} near-tie swaps in {tot} selected blocks (bar: < 0.01 %)"
         c.K[:] = c.K[:, :, :1, :]  # every block key identical: ties cut inside a slice, lower index wins
         c.k_d = to_dev(c.K, dev)
         c.cache.reset()

@@ -69,6 +69,43 @@ def test_P6_topr_groups(g, r):
         assert keep.sum() == r // g
 
 
+def test_P6_group_mask_is_frobenius_optimal_by_enumeration():
+    """Independent pin of the g > 1 rank key (PAPER.md:196 "selects groups of adjacent elements together";
+    DESIGN.md R4): the kept groups must minimise the dropped energy over ALL C(D/g, r/g) group masks.  The
+    enumeration below knows nothing of the oracle's key (it sums squares in fp64 over explicit masks); a wrong
+    group stride, a key that ranks by max |x| or by the first element only, or keeping the smallest groups
+    fails it.  Inputs are small integers, so energies are exact and ties are real: among equal-energy groups the
+    lower group index must be kept (north_star tie rule)."""
+    import itertools
+    rng = np.random.default_rng(17)
+    for D, g, r in [(8, 2, 4), (8, 2, 2), (8, 2, 6), (16, 4, 8), (16, 4, 4), (12, 2, 6)]:
+        ng, nk = D // g, r // g
+        for trial in range(30):
+            if trial % 3 == 0:   # integers -> exact ties between groups
+                x = synth.f32_to_bf16_bits(rng.integers(-3, 4, D).astype(np.float32))
+            else:
+                x = rand_bf16(rng, D, 2.0)
+            xf = brute.bf16_to_f64(x)
+            e = (xf.reshape(ng, g) ** 2).sum(axis=1)          # exact in fp64 (bf16 squares, <= 4 terms)
+            keep = orc.topr(x, g, r).astype(bool)
+            assert keep.sum() == nk
+            best, best_masks = None, []
+            for comb in itertools.combinations(range(ng), nk):
+                m = np.zeros(ng, bool)
+                m[list(comb)] = True
+                loss = float(e[~m].sum())
+                if best is None or loss < best - 1e-300:
+                    best, best_masks = loss, [m]
+                elif loss == best:
+                    best_masks.append(m)
+            assert float(e[~keep].sum()) == best, (D, g, r, trial)
+            # among the optimal masks the oracle's is the one that prefers lower group indices:
+            # lexicographically largest keep-vector read from group 0 upwards
+            lex = max(best_masks, key=lambda m: tuple(m.astype(int)))
+            if trial % 3 == 0:
+                np.testing.assert_array_equal(keep, lex)
+
+
 # ----------------------------------------------------------------------------- P9: block key (O2)
 
 def test_P9_block_key_constant_block_and_B1():
@@ -432,3 +469,44 @@ def test_P12_quantile_and_threshold():
     assert (st[:, 0] == 128).all() and (st[:, 1] == 128).all() and (st[:, 2] == 1).all()
     st = orc.strategy_threshold(lk, lk, cands, 0.25, 128)
     np.testing.assert_array_equal(st, [[128, 128, 1, 8], [32, 32, 2, 8], [16, 16, 4, 8]])
+
+
+# ----------------------------------------------------------------------------- batched drivers
+
+def test_batched_drivers_equal_per_unit_calls():
+    """orc_compress_units / orc_decode_units / orc_attention_units (the OpenMP drivers that bench.py's cpu_baseline
+    times) against the per-unit functions pinned above, on 3 units with different K, V, q and strategies: a wrong
+    per-unit offset (q + u*G*D, sel + u*k_max, blob pointer) changes a unit's result and fails here."""
+    G, N, L, D = 4, 1000, 64, 128
+    K, V, q = synth.make_inputs_np(3, 1, G, N, D, L, seed=21)
+    K, V, q = K[:, 0], V[:, 0], q  # [3][N][D], [3][G][D]
+    S = (N + L - 1) // L
+    strat = np.stack([orc.uniform_strategy(S, 38, 38), orc.uniform_strategy(S, 64, 90), orc.uniform_strategy(S, 128, 38)])
+    strat[1, ::3, 0:2] = 128
+    blobs = orc.compress_units(K, V, L, strat)
+    for u in range(3):
+        np.testing.assert_array_equal(blobs[u], orc.compress_unit(K[u], V[u], L, strat[u]))
+    scale, budget = 1.0 / math.sqrt(D), 256
+    for mode in (0, 1):
+        sel, cnt, out, lse = orc.decode_units(blobs, q, budget, scale, mode, k_max=budget // 8 + 1)
+        for u in range(3):
+            ft, nt = orc.blob_blocks(blobs[u])
+            s = orc.scores(blobs[u], q[u], mode)
+            ref = orc.topk(s, ft, nt, budget)
+            assert cnt[u] == len(ref)
+            np.testing.assert_array_equal(sel[u, :cnt[u]], ref)
+            o, l = orc.attention(blobs[u], q[u], ref, scale)
+            np.testing.assert_array_equal(out[u], o)
+            np.testing.assert_array_equal(lse[u], l)
+    # attention_units on a selection that differs per unit (different counts, shifted blocks)
+    k_max = 40
+    sel = np.full((3, k_max), -1, np.int32)
+    cnt = np.array([40, 7, 0], np.int32)
+    sel[0, :40] = np.arange(40) * 16
+    sel[1, :7] = np.array([8, 64, 72, 200, 504, 512, 992])
+    out, lse = orc.attention_units(blobs, q, sel, cnt, scale)
+    for u in range(3):
+        o, l = orc.attention(blobs[u], q[u], sel[u, :cnt[u]], scale)
+        np.testing.assert_array_equal(out[u], o)
+        np.testing.assert_array_equal(lse[u], l)
+    assert np.all(out[2] == 0) and np.all(np.isneginf(lse[2]))
