@@ -10,7 +10,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("MKV_LIB") or os.path.join(_HERE, "libmkv.so")  # MKV_LIB: tuning builds only
+LIB_PATH = os.path.join(_HERE, "libmkv.so")
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} not found: run `python -m paper_2607_00760_b200.build` "
@@ -18,12 +18,13 @@ if not os.path.exists(LIB_PATH):
 _lib = C.CDLL(LIB_PATH)
 
 MKV_OK, MKV_E_ARG, MKV_E_UNSUPPORTED, MKV_E_NOMEM, MKV_E_CUDA, MKV_E_STATE, MKV_E_DEVICE = 0, -1, -2, -3, -4, -5, -6
-MKV_DEV_ARENA_OVERFLOW, MKV_DEV_BAD_STRATEGY = 1, 2
+MKV_DEV_ARENA_OVERFLOW, MKV_DEV_BAD_STRATEGY, MKV_DEV_SYNC_TIMEOUT = 1, 2, 4
 
 # every symbol include/mkv.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ["mkv_cache_create", "mkv_cache_free", "mkv_cache_reset", "mkv_segment_loss",
            "mkv_strategy_quantile", "mkv_strategy_threshold", "mkv_compress_segment", "mkv_select",
-           "mkv_packed_attention", "mkv_update_append", "mkv_update_flush", "mkv_update_count", "mkv_calibrate_gather", "mkv_decode_host", "mkv_cache_export", "mkv_cache_bytes",
+           "mkv_packed_attention", "mkv_update_append", "mkv_update_flush", "mkv_update_count", "mkv_calibrate_gather", "mkv_calibrate_stream",
+           "mkv_attention_stats", "mkv_decode_host", "mkv_cache_export", "mkv_cache_bytes",
            "mkv_cache_status", "mkv_last_launch_count", "mkv_last_error", "mkv_version"]
 
 
@@ -54,6 +55,8 @@ _lib.mkv_update_append.argtypes = [_vp, _i32, _vp, _vp, _i64, _i64, _i64, _i32, 
 _lib.mkv_update_flush.argtypes = [_vp, _i32, _vp, _vp]
 _lib.mkv_update_count.argtypes = [_vp, _i32, C.POINTER(_i32)]
 _lib.mkv_calibrate_gather.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp]
+_lib.mkv_calibrate_stream.argtypes = [_vp, _i32, _u64, _vp]
+_lib.mkv_attention_stats.argtypes = [_vp, C.POINTER(_u64), C.POINTER(_u64), C.POINTER(_u64), _i32]
 _lib.mkv_decode_host.argtypes = [_vp, _i32, _vp, _i32, _i32, C.c_float, _vp, _vp, _vp, _vp]
 _lib.mkv_cache_export.argtypes = [_vp, _i32, _i32, _i32, _vp, _u64, C.POINTER(_u64)]
 _lib.mkv_cache_bytes.argtypes = [_vp, _i32, C.POINTER(_u64), C.POINTER(_u64), C.POINTER(_u64)]
@@ -197,6 +200,16 @@ def mkv_calibrate_gather(cache, layer, sel, sel_count, stream=None):
     _check(_lib.mkv_calibrate_gather(cache, layer, _ptr(sel), _ptr(sel_count), sel.shape[-1], _stream(stream)))
 
 
+def mkv_calibrate_stream(cache, layer, nbytes, stream=None):
+    _check(_lib.mkv_calibrate_stream(cache, layer, int(nbytes), _stream(stream)))
+
+
+def mkv_attention_stats(cache, reset=False):
+    a, b, c = _u64(0), _u64(0), _u64(0)
+    _check(_lib.mkv_attention_stats(cache, C.byref(a), C.byref(b), C.byref(c), 1 if reset else 0))
+    return dict(blocks=a.value, v_blocks=b.value, v_bytes=c.value)
+
+
 def mkv_decode_host(cache, layer, q_host, token_budget, softmax_scale, out_host, reduce=0,
                     sel_host=None, sel_count_host=None, stream=None):
     _check(_lib.mkv_decode_host(cache, layer, _ptr(q_host), token_budget, reduce, float(softmax_scale),
@@ -300,6 +313,12 @@ class Cache:
 
     def calibrate_gather(self, layer, sel, sel_count, stream=None):
         mkv_calibrate_gather(self.h, layer, sel, sel_count, stream)
+
+    def calibrate_stream(self, layer, nbytes, stream=None):
+        mkv_calibrate_stream(self.h, layer, nbytes, stream)
+
+    def attention_stats(self, reset=False):
+        return mkv_attention_stats(self.h, reset)
 
     def decode_host(self, layer, q_host, token_budget, softmax_scale, out_host, reduce=0,
                     sel_host=None, sel_count_host=None, stream=None):

@@ -1,48 +1,35 @@
 // attention.cu — step 3 of the hot path: PackedAttention: QK over the
-// selected packed keys, online softmax, PV over the packed values, split-K combine.  sm_100a.
+// selected packed keys, softmax, PV over the packed values, split-K combine.  sm_100a.
 //
-// Design:
+// Design: one launch, two phases, one CTA per SM.
 //   * The selected blocks of all units form one stream of T blocks; it is cut into equal ranges,
-//     one per warp of a one-CTA-per-SM grid (warps are fully independent: no __syncthreads in
-//     the main loop).  A warp walks its range in groups of <= 2 token blocks (16 tokens).
-//   * Staging: every token block is one contiguous 16-B-aligned chunk (DESIGN.md format); one lane
-//     moves it into the warp's shared-memory stage with ONE 1-D bulk copy (cp.async.bulk, the TMA
-//     engine) that completes on the stage's mbarrier; kStages groups are in flight per warp.
-//   * Packed vectors are expanded STRAIGHT INTO mma.sync fragments — no dense tile in shared
-//     memory.  QK: S = K q^T with the group's 16 tokens = M (rows 0-7 block 0, rows 8-15 block
-//     1), heads = N, channels = K; lane (gq, qq) owns token gq of each block and bitmap word qq
-//     (32 channels) and walks its 32 slots in order: a set bit loads the next kept bf16 of its
-//     run and bumps the run pointer (mkv_walk.cuh).  The channel order inside a k-step is a fixed
-//     permutation applied to q's B fragments as well.
-//     PV: O^T = V^T P^T with channels = M, heads = N, the 16 tokens of the group = K; lane
-//     (gq, qq) owns tokens 2qq, 2qq+1 of each block and the 16-channel half-word gq, so a
-//     fragment register pairs two TOKENS of one channel, as the contraction over tokens needs.
-//     P is split into bf16 hi + lo (fp32-class accuracy) and transposed into the B fragment
-//     layout with movmatrix.  Dense vectors (r = D) skip the walk: their fragments are 16-byte
-//     shared loads.
+//     one per warp (warps are independent inside a phase).  A warp walks its range in groups of
+//     <= 2 token blocks (16 tokens = the M of one mma tile).  What a block is (payload offset,
+//     tokens, r_k, r_v) comes from the plan record mkv_select wrote next to `sel`, verified against
+//     the `sel` entry; a record that does not match is replaced by the table lookup.
+//   * Staging: a block's K part and its V part are contiguous 16-B-aligned chunks (DESIGN.md
+//     format); one lane moves a chunk into the warp's shared-memory ring with ONE 1-D bulk copy
+//     (cp.async.bulk, the TMA engine) that completes on the slot's mbarrier.  The ring is
+//     byte-granular (a group takes what it needs), up to kSlots groups are in flight per warp.
+//   * Phase 1 (QK): S = K q^T with the group's 16 tokens = M, heads = N, channels = K; packed
+//     vectors are expanded straight into mma.sync fragments (mkv_walk.cuh).  The scaled logits go
+//     to the warp's logit cache (shared memory; global scratch beyond its capacity) and the
+//     per-(unit, head) maximum to global memory with one atomic max per warp, unit and head.
+//   * Between the phases the CTAs that share a unit meet at a per-unit arrival counter; after it
+//     every warp knows the unit's exact maximum M, so all probabilities are 2^(z - M), no partial
+//     result is ever rescaled, and partial results of one unit simply add.
+//   * Phase 2 (PV, deferred): the softmax sum runs over every selected token; the V part of a block
+//     is fetched and walked only if one of its probabilities is >= 2^-40 (error bound).
+//     O^T = V^T P^T with channels = M, heads = N, the group's 16 tokens = K; P is split into bf16
+//     hi + lo (fp32-class accuracy).  Dense vectors (r = D) skip the walk.
 //   * Step 3d (split-K combine) is fused: a unit wholly inside one warp's range is normalised and
-//     written directly; otherwise the warp leaves a (ref, l, O) partial (<= 2 per warp), the
-//     threads of the CTA fold the partials of a unit (four output channels each, straight-line
-//     code) with the LSE rule, and a unit that spans several CTAs is finished by the last CTA to
-//     arrive at a per-unit ticket (no second kernel).
-//   * Softmax is lazy: 2^(s - ref) with a reference that moves only when a score exceeds it by
-//     more than 60 (log2 units); the common group needs no max reduction and no rescale.
-#include <cstdlib>
-
+//     written directly; otherwise the warp leaves an (l, O) partial (<= 2 per warp), the threads of
+//     the CTA add the partials of a unit (four output channels each), and a unit that spans several
+//     CTAs is finished by the last CTA to arrive at a per-unit ticket (no second kernel).
 #include "mkv_internal.cuh"
 #include "mkv_walk.cuh"
 
 namespace mkv {
-
-#ifdef MKV_DBG_TIMING
-__device__ unsigned long long g_dbg_t[160 * 16];
-__device__ __forceinline__ unsigned long long dbg_now() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define MKV_T(k) do { if (threadIdx.x == 0) g_dbg_t[blockIdx.x * 16 + (k)] = dbg_now(); } while (0)
-#define MKV_TV(k, v) do { if (threadIdx.x == 0 && (v) != -12345) g_dbg_t[blockIdx.x * 16 + (k)] = dbg_now(); } while (0)
-#else
-#define MKV_T(k) do {} while (0)
-#define MKV_TV(k, v) do {} while (0)
-#endif
 
 namespace {
 
@@ -50,20 +37,22 @@ using namespace walk;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 
-constexpr int kMaxWarps = 24;      // upper bound on warps per CTA (sizes the partial-slot scratch)
-constexpr int kStageBytes = 4096;  // one dense block (4096 B) or two packed blocks with r <= 56
-constexpr int kDescRing = 64;      // block descriptors kept per warp
+constexpr int kWarps = 16;         // warps per CTA (one CTA per SM)
+constexpr int kRingBytes = 8192;   // per-warp staging ring: two dense groups or five groups at r = 38
+constexpr int kSlots = 8;          // groups in flight per warp (one mbarrier each)
+constexpr int kGroupMax = 4096;    // largest group: two dense K (or V) parts
+constexpr int kDescRing = 64;      // group descriptors kept per warp
+constexpr int kZBytes = 4096;      // per-warp logit cache: 32 blocks at G = 4
 constexpr int kMaxUnitsSmem = 2048;
-// A group of the KV update buffer: nb0 <= 8 uncompressed recent tokens, attended as one dense
-// block; off0 / off1 are its K rows / V rows in the buffer arrays (two chunks, staged back to back).
-constexpr uint32_t kUpdFlag = 1u << 26;
+constexpr float kSkip = 40.f;      // a block whose probabilities are all < 2^-40 is not walked in phase 2
+constexpr int kSpinLimit = 1 << 22;
 
 // One group of the stream: <= 2 consecutive selected token blocks of one unit with the same
-// strategy that fit one stage (16 tokens = the M of one mma tile).
+// strategy whose K parts and V parts each fit kGroupMax.
 struct __align__(16) GDesc {
-    uint32_t off0, off1;  // payload offsets in the layer slice, 16-B units
-    uint32_t z;           // bytes0 / 16 | bytes1 / 16 << 9 | nb0 << 18 | nb1 << 22 | kUpdFlag   (bytes 0: invalid entry)
-    uint32_t w;           // unit | r_k << 16 | r_v << 24
+    uint32_t off0, off1;  // payload offsets in the layer slice (update buffer: row offsets), 16-B units
+    uint32_t a;           // unit | r_k << 16 | r_v << 24
+    uint32_t b;           // nb0 | nb1 << 4 | upd << 8 | pos << 9   (nb0 = 0: invalid entry; pos: block 0's index in the warp's range)
 };
 
 __device__ __forceinline__ unsigned lanemask_le() {
@@ -75,6 +64,25 @@ __device__ __forceinline__ unsigned lanemask_lt() {
     unsigned m;
     asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
     return m;
+}
+__device__ __forceinline__ uint32_t vecb(uint32_t r) { return r == (uint32_t)kD ? 256u : 16u + 2u * r; }
+// order-preserving map fp32 -> u32 and back (larger float <=> larger key; every key of a float is > 0)
+__device__ __forceinline__ uint32_t fkey(float f) {
+    const uint32_t u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float funkey(uint32_t k) {
+    return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
+}
+__device__ __forceinline__ uint32_t ld_relaxed_u32(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ int ld_acquire(const int32_t* p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
 }
 
 // prefix sums of the clamped selection counts -> s_cum[0..n_units]; returns the total T
@@ -114,8 +122,8 @@ __device__ __forceinline__ int find_unit(const int* s_cum, int n_units, int i) {
     return lo;
 }
 
-// per warp: the stages, the group-descriptor ring, one mbarrier per stage (64 B reserved)
-__host__ __device__ constexpr int warp_smem_bytes(int nstage) { return nstage * kStageBytes + kDescRing * 16 + 64; }
+// per warp: staging ring | group descriptors | logit cache | slot table (offset, bytes) | mbarriers | phase-2 slot groups
+constexpr int kWS = kRingBytes + kDescRing * 16 + kZBytes + kSlots * 8 + kSlots * 8 + kSlots * 16;
 
 // Even split of n items over p parts: part i owns [i b + min(i, r), ...) with b = n / p, r = n % p
 // (the first r parts hold one more).  One runtime division per level.
@@ -130,44 +138,43 @@ struct Split {
 };
 
 // ------------------------------------------------------------------------------------------
-// main kernel: one CTA per SM, kWarps independent warps.  The T selected blocks are split evenly
-// over the CTAs, a CTA's range evenly over its warps; every warp owns one contiguous range.
+// kGatherOnly: calibration build of the same kernel (mkv_calibrate_gather): every K part and every
+// V part of the selection is staged exactly as in the real run (nothing is skipped), one word per
+// lane and group is read back, and all arithmetic, synchronisation and output are left out.
 // ------------------------------------------------------------------------------------------
-// kGatherOnly: calibration build of the same kernel (mkv_calibrate_gather): every selected payload is staged
-// exactly as in the real run, one word per lane and group is read back, and all arithmetic is skipped.
-template <int NSTAGE, int kWarps, bool kGatherOnly>
+template <bool kGatherOnly>
 __global__ void __launch_bounds__(kWarps * 32, 1)
 mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q,
                             const int32_t* __restrict__ sel, const int32_t* __restrict__ sel_count, int k_max,
-                            float scale_log2, float* __restrict__ out, float* __restrict__ lse,
-                            float* __restrict__ part_o, float* __restrict__ part_ml, int32_t* __restrict__ ticket,
+                            float scale_log2, float* __restrict__ out, float* __restrict__ lse, AttnScratch scr,
                             const uint16_t* __restrict__ upd_k, const uint16_t* __restrict__ upd_v,
-                            const int32_t* __restrict__ upd_count) {
+                            const int32_t* __restrict__ upd_count, uint32_t* __restrict__ dev_flags) {
     extern __shared__ __align__(128) uint8_t smem[];
-    constexpr int kWS = warp_smem_bytes(NSTAGE);
     constexpr int kNT = kWarps * 32;
     constexpr int kRec = 2 * kWarps;  // partial records of the CTA: warp w -> 2w (head), 2w + 1 (tail)
     int* s_cum = reinterpret_cast<int*>(smem + kWarps * kWS);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int gq = lane >> 2, qq = lane & 3;  // mma fragment coordinates (groupID, threadID_in_group)
 
-    MKV_T(0);
-    __shared__ int s_unit[kRec];                 // unit of each partial record, -1 = none
-    __shared__ __align__(8) float s_ml[kRec][kMaxGroup][2];   // its (max in log2 units, sum) per head
+    __shared__ int s_unit[kRec];                              // unit of each partial record, -1 = none
+    __shared__ __align__(8) float s_ml[kRec][kMaxGroup][2];   // its (global max in log2 units, sum) per head
     __shared__ int s_last[2], s_cf[2], s_cl[2];
     __shared__ size_t s_row[2];
 
     uint8_t* wbase = smem + warp * kWS;
-    const uint32_t stage0 = smem_u32(wbase);
-    GDesc* ring = reinterpret_cast<GDesc*>(wbase + NSTAGE * kStageBytes);
-    const uint32_t bar0 = stage0 + NSTAGE * kStageBytes + kDescRing * 16;
+    const uint32_t ring0 = smem_u32(wbase);
+    GDesc* ring = reinterpret_cast<GDesc*>(wbase + kRingBytes);
+    float* zs = reinterpret_cast<float*>(wbase + kRingBytes + kDescRing * 16);
+    uint2* slot_tab = reinterpret_cast<uint2*>(wbase + kRingBytes + kDescRing * 16 + kZBytes);
+    const uint32_t bar0 = ring0 + kRingBytes + kDescRing * 16 + kZBytes + kSlots * 8;
+    GDesc* slot_grp = reinterpret_cast<GDesc*>(wbase + kRingBytes + kDescRing * 16 + kZBytes + kSlots * 16);
     if (lane == 0) {
 #pragma unroll
-        for (int s = 0; s < NSTAGE; ++s) mbar_init(bar0 + 8 * s, 1);
+        for (int s = 0; s < kSlots; ++s) mbar_init(bar0 + 8 * s, 1);
         mbar_init_fence();
     }
     if (lane < 2) s_unit[warp * 2 + lane] = -1;
-    pdl_wait();               // the producer of sel / sel_count / the cache (and the previous user of the scratch) is done
+    pdl_wait();               // the producer of sel / sel_count / the plan / the cache (and the previous user of the scratch) is done
     pdl_launch_dependents();  // the next kernel may be scheduled as SMs free up
 
     // tokens in the layer's update buffer: device-resident, so a captured graph stays valid across appends
@@ -191,7 +198,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     const unsigned gw = blockIdx.x * kWarps + warp;
     const int n_total = hi - lo;
     const int G = g.group;
-    if (blockIdx.x == 0) {  // units with an empty selection: out = 0, lse = -inf
+    const int zcap = kZBytes / (32 * G);  // blocks of the range whose logits stay in shared memory
+    if (blockIdx.x == 0 && !kGatherOnly) {  // units with an empty selection: out = 0, lse = -inf
 #pragma unroll 1
         for (int u = warp; u < g.n_units; u += kWarps) {
             if (s_cum[u + 1] != s_cum[u]) continue;
@@ -201,58 +209,60 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             if (lse != nullptr && lane < G) lse[row + lane] = -INFINITY;
         }
     }
+    // logits of block i of the range: [head][token], 8 G floats
+    auto zptr = [&](int i) -> float* {
+        return i < zcap ? zs + i * (8 * G) : scr.zbuf + (size_t)(lo + i) * (size_t)(8 * G);
+    };
 
-    int bposc = 0, bposi = 0, bbuilt = 0;  // blocks consumed / issued / described
-    int gposc = 0, gposi = 0, gbuilt = 0;  // groups consumed / issued / described
+    int bbuilt = 0, gbuilt = 0;  // blocks / groups described so far (per phase)
 
     // Describe the next <= 32 blocks of the range (one per lane) and pair them into groups: block i
-    // follows block i - 1 in a group if both belong to one unit, have the same strategy and fit one
-    // stage together; runs of such blocks are paired greedily from their start.
-    auto build = [&](int count) {
-        uint32_t off16 = 0u, bytes = 0u, rr = 0u, nb = 0u;
+    // follows block i - 1 in a group if both belong to one unit, have the same strategy and their K
+    // parts and V parts fit one group; runs of such blocks are paired greedily from their start.
+    // A pure function of the inputs: phase 2 describes the range again and gets the same groups.
+    auto describe = [&](int count) {
+        uint32_t off16 = 0u, meta = 0u, updf = 0u;
         int u = -1;
         if (lane < count) {
             const int gi = lo + bbuilt + lane;
             u = find_unit(s_cum, g.n_units, gi);
             const int j = gi - s_cum[u], jb = j - (s_cum[u + 1] - s_cum[u] - upd_blocks);
             if (jb >= 0) {  // block jb of the unit's update buffer: raw rows [u][8 jb ..][128] of upd_k / upd_v
-                nb = (uint32_t)min(kB, n_buf - kB * jb);
+                const uint32_t nb = (uint32_t)min(kB, n_buf - kB * jb);
                 off16 = (uint32_t)(((size_t)u * g.L + (size_t)kB * jb) * (kD * 2 / 16));
-                bytes = nb * (uint32_t)(kD * 2);
-                rr = (uint32_t)kD | ((uint32_t)kD << 8) | 0x10000u;  // bit 16: update-buffer block
-            }
-            const int t0 = jb >= 0 ? -1 : sel[(size_t)u * k_max + j];
-            const int ntok = lv.unit_ntok[u];
-            if (t0 >= 0 && t0 < ntok && (t0 & (kB - 1)) == 0) {
-                const int seg = t0 / g.L, in_seg = t0 - seg * g.L;
-                const size_t e = (size_t)u * lv.S_max + seg;
-                const StratRec rec = lv.strat[e];
-                nb = (uint32_t)min(kB, (int)rec.n_tok - in_seg);
-                off16 = lv.tok_off[e] + (uint32_t)(in_seg >> 3) * (tokblock_bytes(rec.r_k, rec.r_v, kB) >> 4);
-                bytes = tokblock_bytes(rec.r_k, rec.r_v, (int)nb);
-                rr = (uint32_t)rec.r_k | ((uint32_t)rec.r_v << 8);
+                meta = (uint32_t)kD | ((uint32_t)kD << 8) | (nb << 16);
+                updf = 1u;
+            } else {
+                const int t0 = sel[(size_t)u * k_max + j];
+                PlanRec pr;
+                pr.t0 = -1; pr.off16 = 0u; pr.meta = 0u; pr.tag = 0u;
+                if (scr.plan != nullptr && j < scr.plan_stride)
+                    pr = *reinterpret_cast<const PlanRec*>(
+                        __builtin_assume_aligned(scr.plan + (size_t)u * scr.plan_stride + j, 16));
+                if (pr.tag == scr.plan_tag && pr.t0 == t0 && t0 >= 0) { off16 = pr.off16; meta = pr.meta; }
+                else plan_lookup(g, lv, u, t0, off16, meta);
             }
         }
+        const uint32_t nb = meta >> 16, rk = meta & 255u, rv = (meta >> 8) & 255u;
+        const uint32_t kb = nb * vecb(rk), vb = nb * vecb(rv);
+        const uint32_t kc = pad16u(kb), vc = pad16u((kb & 15u) + vb);  // bytes staged in phase 1 / phase 2
         const int pu = __shfl_up_sync(kFull, u, 1);
-        const uint32_t prr = __shfl_up_sync(kFull, rr, 1), pbytes = __shfl_up_sync(kFull, bytes, 1);
-        const bool follows = lane > 0 && lane < count && u == pu && rr == prr && bytes != 0u && pbytes != 0u &&
-                             bytes + pbytes <= (uint32_t)kStageBytes && !(rr & 0x10000u);
+        const uint32_t pmeta = __shfl_up_sync(kFull, meta, 1), pkc = __shfl_up_sync(kFull, kc, 1);
+        const uint32_t pvc = __shfl_up_sync(kFull, vc, 1), pupd = __shfl_up_sync(kFull, updf, 1);
+        const bool follows = lane > 0 && lane < count && u == pu && ((meta ^ pmeta) & 0xffffu) == 0u && nb != 0u &&
+                             (pmeta >> 16) != 0u && kc + pkc <= (uint32_t)kGroupMax && vc + pvc <= (uint32_t)kGroupMax &&
+                             !updf && !pupd;
         const unsigned fm = __ballot_sync(kFull, follows);
         const int start = 31 - __clz((int)(~fm & lanemask_le()));  // first block of this lane's run (bit 0 of ~fm is set)
         const bool first = lane < count && ((lane - start) & 1) == 0;
         const bool two = first && ((fm >> 1) >> lane & 1u);        // lane + 1 follows (and is therefore < count)
         const unsigned gm = __ballot_sync(kFull, first);
-        const uint32_t off1 = __shfl_down_sync(kFull, off16, 1), bytes1 = __shfl_down_sync(kFull, bytes, 1);
-        const uint32_t nb1 = __shfl_down_sync(kFull, nb, 1);
+        const uint32_t off1 = __shfl_down_sync(kFull, off16, 1), nb1 = __shfl_down_sync(kFull, nb, 1);
         if (first) {
             GDesc d;
             d.off0 = off16; d.off1 = two ? off1 : 0u;
-            d.z = (bytes >> 4) | ((two ? bytes1 >> 4 : 0u) << 9) | (nb << 18) | ((two ? nb1 : 0u) << 22);
-            if (rr & 0x10000u) {  // K rows and V rows: two chunks of the same size at the same offset
-                d.off1 = off16;
-                d.z |= ((bytes >> 4) << 9) | kUpdFlag;
-            }
-            d.w = (uint32_t)u | ((rr & 0xffffu) << 16);
+            d.a = (uint32_t)u | (rk << 16) | (rv << 24);
+            d.b = nb | ((two ? nb1 : 0u) << 4) | (updf << 8) | ((uint32_t)(bbuilt + lane) << 9);
             ring[(gbuilt + __popc(gm & lanemask_lt())) & (kDescRing - 1)] = d;
         }
         gbuilt += __popc(gm);
@@ -260,51 +270,212 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         __syncwarp();
     };
 
-    // start the copies of the next group into stage s: one bulk copy per block, issued by lane 0,
-    // completing on the stage's mbarrier
+    // ---- staging ring (all scalars below are warp-uniform)
+    uint32_t rhead = 0u, rused = 0u, parbits = 0u;
+    int pend = 0, si = 0, sc = 0;
     const unsigned long long slice = reinterpret_cast<unsigned long long>(lv.slice);
-    auto issue = [&](int s) {
-        if (bposi >= n_total) return;
-        if (gposi == gbuilt) build(min(32, n_total - bbuilt));
-        const GDesc d = ring[gposi & (kDescRing - 1)];
-        const uint32_t b0 = (d.z & 511u) << 4, b1 = ((d.z >> 9) & 511u) << 4;
-        if (lane == 0) {
-            const uint32_t bar = bar0 + 8 * s, dst = stage0 + s * kStageBytes;
-            const bool upd = d.z & kUpdFlag;
-            const unsigned long long src0 = upd ? reinterpret_cast<unsigned long long>(upd_k) : slice;
-            const unsigned long long src1 = upd ? reinterpret_cast<unsigned long long>(upd_v) : slice;
-            mbar_expect_tx(bar, b0 + b1);
-            if (b0) bulk_g2s(dst, src0 + ((unsigned long long)d.off0 << 4), b0, bar);
-            if (b1) bulk_g2s(dst + b0, src1 + ((unsigned long long)d.off1 << 4), b1, bar);
-        }
-        ++gposi;
-        bposi += (b1 && !(d.z & kUpdFlag)) ? 2 : 1;
+    // claim `sz` bytes (a multiple of 16, <= kGroupMax) for the next group; false: no room yet
+    auto ring_alloc = [&](uint32_t sz, uint32_t& off) -> bool {
+        uint32_t need = sz, h = pend == 0 ? 0u : rhead;  // an idle ring restarts at its beginning
+        if (h + sz > (uint32_t)kRingBytes) { need += (uint32_t)kRingBytes - h; h = 0u; }  // wrap: the tail stays unused
+        if (pend == kSlots || rused + need > (uint32_t)kRingBytes) return false;
+        off = h;
+        rhead = h + sz;
+        rused += need;
+        if (lane == 0) slot_tab[si] = make_uint2(h, need);
+        return true;
+    };
+    auto ring_release = [&]() {  // the oldest group has been consumed
+        rused -= slot_tab[sc].y;
+        parbits ^= 1u << sc;
+        sc = (sc + 1) & (kSlots - 1);
+        --pend;
+    };
+    auto ring_commit = [&]() {
+        si = (si + 1) & (kSlots - 1);
+        ++pend;
+        __syncwarp();  // the slot table entry is visible to the whole warp
     };
 
-    // per-unit state.  qa: B fragments of q (column gq = head gq of the unit's group).
-    // acc[i] = O^T tile i: rows gq / gq+8 = channels 16gq + 2i / + 1, columns 2qq, 2qq+1 = heads.
+    // =====================================================================================
+    // Phase 1: QK.  Logits (log2 domain, scaled) -> logit cache; per-(unit, head) maxima -> global.
+    // =====================================================================================
     uint32_t qa[8][2];
-    float acc[8][4];
-    // heads hA = 2qq, hB = 2qq+1: reference exponent (log2 units; -inf = not set yet) and this lane's
-    // share of the sum.  Softmax is LAZY: probabilities are 2^(s - ref) with a reference that only
-    // moves when a score exceeds it by more than kRefSlack, so the common group needs no max
-    // reduction and no rescale of the accumulators (fp32 has the exponent range to spare).
-    constexpr float kRefSlack = 60.f;
-    float mA = -INFINITY, mB = -INFINITY, lA = 0.f, lB = 0.f;
+    float mxA = -INFINITY, mxB = -INFINITY;  // this lane's maxima for heads 2qq, 2qq+1 of the current unit
     int cur_unit = -1;
+    uint32_t calib = 0u;
 
-    // end of a unit inside this warp's range.  `last`: the range is finished and the stages are
-    // idle, so the partial lives in this warp's own shared memory (record 2w + 1); a unit that
-    // ends inside the range while copies are in flight leaves its partial in global scratch (2w).
+    auto publish_max = [&]() {  // the warp's maxima of cur_unit: one atomic max per head
+#pragma unroll
+        for (int o = 4; o < 32; o <<= 1) {
+            mxA = fmaxf(mxA, __shfl_xor_sync(kFull, mxA, o));
+            mxB = fmaxf(mxB, __shfl_xor_sync(kFull, mxB, o));
+        }
+        if (gq == 0) {
+            if (2 * qq < G) atomicMax(scr.umax + (size_t)cur_unit * kMaxGroup + 2 * qq, fkey(mxA));
+            if (2 * qq + 1 < G) atomicMax(scr.umax + (size_t)cur_unit * kMaxGroup + 2 * qq + 1, fkey(mxB));
+        }
+    };
+
+    {
+        int bposi = 0, gposi = 0, bposc = 0, gposc = 0;
+#pragma unroll 1
+        for (;;) {
+            // ---- issue: K parts of the next groups while the ring has room
+#pragma unroll 1
+            while (bposi < n_total) {
+                if (gposi == gbuilt) describe(min(32, n_total - bbuilt));
+                const GDesc d = ring[gposi & (kDescRing - 1)];
+                const uint32_t nb0 = d.b & 15u, nb1 = (d.b >> 4) & 15u, rk = (d.a >> 16) & 255u;
+                const uint32_t c0 = pad16u(nb0 * vecb(rk)), c1 = pad16u(nb1 * vecb(rk));
+                uint32_t off;
+                if (!ring_alloc(c0 + c1, off)) break;
+                if (lane == 0) {
+                    const uint32_t bar = bar0 + 8 * si, dst = ring0 + off;
+                    const unsigned long long src = (d.b & 256u) ? reinterpret_cast<unsigned long long>(upd_k) : slice;
+                    mbar_expect_tx(bar, c0 + c1);
+                    if (c0) bulk_g2s(dst, src + ((unsigned long long)d.off0 << 4), c0, bar);
+                    if (c1) bulk_g2s(dst + c0, src + ((unsigned long long)d.off1 << 4), c1, bar);
+                }
+                ring_commit();
+                ++gposi;
+                bposi += nb1 ? 2 : 1;
+            }
+            if (pend == 0) break;  // nothing in flight and nothing left to issue
+
+            // ---- consume the oldest group
+            const GDesc d = ring[gposc & (kDescRing - 1)];
+            const int u = (int)(d.a & 0xffffu);
+            const int r_k = (int)((d.a >> 16) & 255u);
+            const int nb0 = (int)(d.b & 15u), nb1 = (int)((d.b >> 4) & 15u), pos = (int)(d.b >> 9);
+            const bool two = nb1 != 0;
+            const uint32_t sp0 = ring0 + slot_tab[sc].x, sp1 = sp0 + pad16u((uint32_t)nb0 * vecb((uint32_t)r_k));
+            if (kGatherOnly) {
+                mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);
+                calib ^= lds_u32(sp0 + 4 * lane);
+                __syncwarp();
+                ring_release();
+                ++gposc;
+                bposc += two ? 2 : 1;
+                continue;
+            }
+            if (u != cur_unit) {
+                if (cur_unit >= 0) publish_max();
+                cur_unit = u;
+                mxA = mxB = -INFINITY;
+                const int bi = u / g.n_kv_heads, hk = u % g.n_kv_heads;
+                // q[head gq][32qq .. 32qq+31]: k-step ks uses channels 32qq + 4ks .. + 3
+                const uint4* qrow = reinterpret_cast<const uint4*>(
+                    q + ((size_t)bi * g.n_q_heads + (size_t)hk * g.group + gq) * kD + 32 * qq);
+#pragma unroll
+                for (int h = 0; h < 4; ++h) {
+                    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                    if (gq < g.group) v = __ldg(qrow + h);
+                    qa[2 * h][0] = v.x; qa[2 * h][1] = v.y; qa[2 * h + 1][0] = v.z; qa[2 * h + 1][1] = v.w;
+                }
+            }
+            const bool full = nb0 == kB && (!two || nb1 == kB);
+
+            mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);  // the group's K parts have landed
+
+            // ---- QK: S (tokens x heads); rows 0-7 = block 0, rows 8-15 = block 1
+            float S[4] = {0.f, 0.f, 0.f, 0.f};
+            if (nb0 != 0) {
+                if (r_k == kD && full) {
+                    const uint32_t a0 = sp0 + 256 * gq + 64 * qq, a1 = sp1 + 256 * gq + 64 * qq;
+#pragma unroll
+                    for (int h = 0; h < 4; ++h) {
+                        const uint4 x = lds_128(a0 + 16 * h);
+                        uint4 y = make_uint4(0u, 0u, 0u, 0u);
+                        if (two) y = lds_128(a1 + 16 * h);
+                        mma_bf16(S, x.x, y.x, x.y, y.y, qa[2 * h][0], qa[2 * h][1]);
+                        mma_bf16(S, x.z, y.z, x.w, y.w, qa[2 * h + 1][0], qa[2 * h + 1][1]);
+                    }
+                } else {
+                    // run of (token gq, word qq): starts after the kept elements of the lower words
+                    uint32_t w0 = 0u, w1 = 0u, p0, p1, st0 = 2u, st1 = 2u;
+                    if (r_k == kD) {  // ragged dense block: all slots kept, no bitmap stored
+                        w0 = gq < nb0 ? 0xffffffffu : 0u;
+                        w1 = gq < nb1 ? 0xffffffffu : 0u;
+                        p0 = sp0 + 256 * gq + 64 * qq;
+                        p1 = sp1 + 256 * gq + 64 * qq;
+                    } else {  // values rank-major: rank rho of token t at element rho * nb + t
+                        if (gq < nb0) w0 = lds_u32(sp0 + 4 * lane);
+                        if (gq < nb1) w1 = lds_u32(sp1 + 4 * lane);
+                        uint32_t cnt = (uint32_t)__popc(w0) | ((uint32_t)__popc(w1) << 16), inc = cnt, t;
+                        t = __shfl_up_sync(kFull, inc, 1); if (qq >= 1) inc += t;
+                        t = __shfl_up_sync(kFull, inc, 2); if (qq >= 2) inc += t;
+                        const uint32_t ex = inc - cnt;
+                        st0 = 2u * nb0; st1 = 2u * nb1;
+                        p0 = sp0 + 16 * nb0 + st0 * (ex & 0xffffu) + 2 * gq;
+                        p1 = sp1 + 16 * nb1 + st1 * (ex >> 16) + 2 * gq;
+                    }
+                    k_walk_mma<0>(S, w0, w1, p0, p1, st0, st1, qa);
+                    k_walk_mma<1>(S, w0, w1, p0, p1, st0, st1, qa);
+                    k_walk_mma<2>(S, w0, w1, p0, p1, st0, st1, qa);
+                    k_walk_mma<3>(S, w0, w1, p0, p1, st0, st1, qa);
+                }
+                // ---- scaled logits of token gq of each block, heads 2qq, 2qq+1 -> cache [head][token]
+                const bool v0 = gq < nb0, v1 = gq < nb1;
+                const float zA0 = v0 ? S[0] * scale_log2 : -INFINITY, zB0 = v0 ? S[1] * scale_log2 : -INFINITY;
+                const float zA1 = v1 ? S[2] * scale_log2 : -INFINITY, zB1 = v1 ? S[3] * scale_log2 : -INFINITY;
+                mxA = fmaxf(mxA, fmaxf(zA0, zA1));
+                mxB = fmaxf(mxB, fmaxf(zB0, zB1));
+                float* z0 = zptr(pos);
+                if (2 * qq < G) z0[(2 * qq) * 8 + gq] = zA0;
+                if (2 * qq + 1 < G) z0[(2 * qq + 1) * 8 + gq] = zB0;
+                if (two) {
+                    float* z1 = zptr(pos + 1);
+                    if (2 * qq < G) z1[(2 * qq) * 8 + gq] = zA1;
+                    if (2 * qq + 1 < G) z1[(2 * qq + 1) * 8 + gq] = zB1;
+                }
+            }
+            __syncwarp();  // every lane is done reading the slot
+            ring_release();
+            ++gposc;
+            bposc += two ? 2 : 1;
+        }
+        if (!kGatherOnly && cur_unit >= 0) publish_max();
+    }
+
+    // =====================================================================================
+    // The CTAs that share a unit meet: every warp of this CTA has issued its atomic maxima (barrier), then one
+    // thread per unit of the CTA's range releases them (fence, cumulative over the barrier) and arrives.
+    // =====================================================================================
+    if (!kGatherOnly) {
+        __syncthreads();
+        if (clo < chi) {
+            const int u_first = find_unit(s_cum, g.n_units, clo), u_last = find_unit(s_cum, g.n_units, chi - 1);
+#pragma unroll 1
+            for (int u = u_first + (int)threadIdx.x; u <= u_last; u += kNT) {
+                if (s_cum[u + 1] == s_cum[u] || (clo <= s_cum[u] && s_cum[u + 1] <= chi)) continue;  // empty, or nobody else waits
+                __threadfence();
+                atomicAdd(scr.uarrive + u, 1);
+            }
+        }
+    }
+
+    // =====================================================================================
+    // Phase 2: softmax sums over every selected token, PV over the blocks that matter.
+    // =====================================================================================
+    float acc[8][4];    // O^T tile i: rows gq / gq+8 = channels 16gq + 2i / + 1, columns 2qq, 2qq+1 = heads
+    float lsum = 0.f;   // this lane's share of the softmax sum of head gq
+    float Mh = 0.f;     // the unit's maximum logit of head gq (log2 domain); 0 if the unit has no valid token
+    float Mraw = -INFINITY;
+    cur_unit = -1;
+    unsigned long long st_vblocks = 0ull, st_vbytes = 0ull;
+
+    // end of a unit inside this warp's range.  `last`: the range is finished and the ring is idle, so the
+    // partial lives in this warp's own shared memory (record 2w + 1); a unit that ends inside the range
+    // leaves its partial in global scratch (2w).
     auto flush = [&](bool last) {
         const int u = cur_unit;
         const int a = s_cum[u], b = s_cum[u + 1];
-#pragma unroll
-        for (int o = 4; o < 32; o <<= 1) {
-            lA += __shfl_xor_sync(kFull, lA, o);
-            lB += __shfl_xor_sync(kFull, lB, o);
-        }
+        lsum += __shfl_xor_sync(kFull, lsum, 1);
+        lsum += __shfl_xor_sync(kFull, lsum, 2);  // lanes (gq, *): the warp's sum of head gq
         const int hA = 2 * qq, hB = 2 * qq + 1;
+        const float lA = __shfl_sync(kFull, lsum, (4 * hA) & 31), lB = __shfl_sync(kFull, lsum, (4 * hB) & 31);
+        const float mA = __shfl_sync(kFull, Mraw, (4 * hA) & 31), mB = __shfl_sync(kFull, Mraw, (4 * hB) & 31);
         const bool whole = lo <= a && b <= hi;  // the whole unit was processed by this warp: final result
         float fA = 1.f, fB = 1.f;
         float* po;
@@ -313,7 +484,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             fA = lA > 0.f ? 1.f / lA : 0.f;
             fB = lB > 0.f ? 1.f / lB : 0.f;
         } else {
-            po = last ? reinterpret_cast<float*>(wbase) : part_o + (size_t)gw * 2 * (size_t)(G * kD);
+            po = last ? reinterpret_cast<float*>(wbase) : scr.part_o + (size_t)gw * 2 * (size_t)(G * kD);
         }
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
@@ -327,6 +498,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 if (hA < G) pl[hA] = lA > 0.f ? (mA + log2f(lA)) * kLn2 : -INFINITY;
                 if (hB < G) pl[hB] = lB > 0.f ? (mB + log2f(lB)) * kLn2 : -INFINITY;
             }
+            if (lane < kMaxGroup) scr.umax[(size_t)u * kMaxGroup + lane] = 0u;  // only this warp ever read them: reset for the next launch
         } else {
             const int rec = warp * 2 + (last ? 1 : 0);
             if (gq == 0) {
@@ -337,210 +509,206 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         }
     };
 
-    // ---- main loop.  Iteration k >= 0 consumes group k from stage k % NSTAGE and refills that stage
-    // with group k + NSTAGE; iterations k < 0 only fill the pipeline.  One call site each for
-    // issue() and flush(): code executed once costs ~4 cycles per instruction (instruction fetch).
-    int s = 0;
-    uint32_t parity = 0u, calib = 0u;
+    // wait until every CTA that shares unit u has published its maxima, then read them
+    auto begin_unit = [&](int u) {
+        cur_unit = u;
+        lsum = 0.f;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
+        const int a = s_cum[u], b = s_cum[u + 1];
+        if (!(clo <= a && b <= chi)) {  // shared with other CTAs
+            if (lane == 0) {
+                const int expected = (int)cs.owner(((unsigned)b - 1u) >> 1) - (int)cs.owner((unsigned)a >> 1) + 1;
+                int it = 0;
 #pragma unroll 1
-    for (int k = -NSTAGE;; ++k) {
-        if (k >= 0) {
-            const bool end = bposc >= n_total;
-            GDesc d;
-            d.off0 = d.off1 = d.z = 0u; d.w = 0xffffu;
-            if (!end) d = ring[gposc & (kDescRing - 1)];
+                while (ld_acquire(scr.uarrive + u) < expected) {
+                    if (++it > kSpinLimit) { atomicOr(dev_flags, MKV_DEV_SYNC_TIMEOUT); break; }
+                }
+            }
+            __syncwarp();
+        }
+        Mraw = gq < G ? funkey(ld_relaxed_u32(scr.umax + (size_t)u * kMaxGroup + gq)) : -INFINITY;
+        Mh = Mraw == -INFINITY ? 0.f : Mraw;
+    };
+
+    {
+        bbuilt = 0; gbuilt = 0;
+        int bposd = 0, gposd = 0;  // blocks / groups decided
+#pragma unroll 1
+        for (;;) {
+            // ---- decide: softmax sums of the next groups; start the V copies of the groups that matter
+#pragma unroll 1
+            while (bposd < n_total) {
+                if (gposd == gbuilt) describe(min(32, n_total - bbuilt));
+                const GDesc d = ring[gposd & (kDescRing - 1)];
+                const int u = (int)(d.a & 0xffffu);
+                if (!kGatherOnly && u != cur_unit) {
+                    if (pend != 0) break;  // drain the unit's groups in flight first
+                    if (cur_unit >= 0) flush(false);
+                    begin_unit(u);
+                }
+                uint32_t nb0 = d.b & 15u, nb1 = (d.b >> 4) & 15u;
+                const uint32_t rk = (d.a >> 16) & 255u, rv = d.a >> 24;
+                const int pos = (int)(d.b >> 9);
+                const bool two = nb1 != 0u;
+                bool need0 = nb0 != 0u, need1 = two;
+                float add = 0.f;
+                if (!kGatherOnly && nb0 != 0u) {
+                    // lane (gq, qq): head gq, tokens 2qq, 2qq+1 of each block
+                    float2 za = make_float2(-INFINITY, -INFINITY), zb = za;
+                    if (gq < G) {
+                        za = *reinterpret_cast<const float2*>(zptr(pos) + gq * 8 + 2 * qq);
+                        if (two) zb = *reinterpret_cast<const float2*>(zptr(pos + 1) + gq * 8 + 2 * qq);
+                    }
+                    add = (ex2(za.x - Mh) + ex2(za.y - Mh)) + (ex2(zb.x - Mh) + ex2(zb.y - Mh));
+                    need0 = __any_sync(kFull, fmaxf(za.x, za.y) - Mh >= -kSkip);
+                    need1 = __any_sync(kFull, fmaxf(zb.x, zb.y) - Mh >= -kSkip);
+                }
+                if (need0 || need1) {
+                    // a group with one block that matters becomes a one-block group
+                    uint32_t off0 = d.off0, off1 = d.off1, p = (uint32_t)pos;
+                    if (!need0) { off0 = d.off1; nb0 = nb1; nb1 = 0u; p += 1u; }
+                    else if (!need1) nb1 = 0u;
+                    const bool upd = d.b & 256u;
+                    // V part of a block: starts kb bytes into its payload (update buffer: the V rows, same offset)
+                    const uint32_t kb0 = upd ? 0u : nb0 * vecb(rk), kb1 = upd ? 0u : nb1 * vecb(rk);
+                    const uint32_t c0 = pad16u((kb0 & 15u) + nb0 * vecb(rv));
+                    const uint32_t c1 = nb1 ? pad16u((kb1 & 15u) + nb1 * vecb(rv)) : 0u;
+                    uint32_t off;
+                    if (!ring_alloc(c0 + c1, off)) break;  // no room yet: decide this group again after a consume
+                    if (lane == 0) {
+                        const uint32_t bar = bar0 + 8 * si, dst = ring0 + off;
+                        const unsigned long long src = upd ? reinterpret_cast<unsigned long long>(upd_v) : slice;
+                        mbar_expect_tx(bar, c0 + c1);
+                        bulk_g2s(dst, src + ((unsigned long long)off0 << 4) + (kb0 & ~15u), c0, bar);
+                        if (c1) bulk_g2s(dst + c0, src + ((unsigned long long)off1 << 4) + (kb1 & ~15u), c1, bar);
+                        GDesc e;
+                        e.off0 = (kb0 & 15u) | (c0 << 8) | ((kb1 & 15u) << 4);  // skews of the V parts, bytes of the first chunk
+                        e.off1 = 0u;
+                        e.a = d.a;
+                        e.b = nb0 | (nb1 << 4) | (d.b & 256u) | (p << 9);
+                        slot_grp[si] = e;
+                    }
+                    st_vblocks += nb1 ? 2ull : 1ull;
+                    st_vbytes += c0 + c1;
+                    ring_commit();
+                }
+                lsum += add;
+                ++gposd;
+                bposd += two ? 2 : 1;
+            }
+            if (pend == 0) {
+                if (bposd >= n_total) break;
+                continue;  // (a unit boundary with nothing in flight: the next pass begins the unit)
+            }
+
+            // ---- consume the oldest group in flight: PV
+            const GDesc d = slot_grp[sc];
+            const int r_v = (int)(d.a >> 24);
+            const int nb0 = (int)(d.b & 15u), nb1 = (int)((d.b >> 4) & 15u), pos = (int)(d.b >> 9);
+            const bool two = nb1 != 0;
+            const uint32_t vb0 = ring0 + slot_tab[sc].x + (d.off0 & 15u);
+            const uint32_t vb1 = ring0 + slot_tab[sc].x + (d.off0 >> 8) + ((d.off0 >> 4) & 15u);
             if (kGatherOnly) {
-                if (end) break;
-                mbar_wait(bar0 + 8 * s, parity);
-                calib ^= lds_u32(stage0 + s * kStageBytes + 4 * lane);
+                mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);
+                calib ^= lds_u32((vb0 & ~3u) + 4 * lane);
                 __syncwarp();
-                bposc += ((d.z >> 22) & 15u) ? 2 : 1;
-                ++gposc;
-                issue(s);
-                if (++s == NSTAGE) { s = 0; parity ^= 1u; }
+                ring_release();
                 continue;
             }
-            const int u = end ? -1 : (int)(d.w & 0xffffu);
-            if (u != cur_unit) {
-                if (cur_unit >= 0) flush(end);
-                if (end) break;
-                cur_unit = u;
-                const int bi = u / g.n_kv_heads, hk = u % g.n_kv_heads;
-                // q[head gq][32qq .. 32qq+31]: k-step ks uses channels 32qq + 4ks .. + 3
-                const uint4* qrow = reinterpret_cast<const uint4*>(
-                    q + ((size_t)bi * g.n_q_heads + (size_t)hk * g.group + gq) * kD + 32 * qq);
-#pragma unroll
-                for (int h = 0; h < 4; ++h) {
-                    uint4 v = make_uint4(0u, 0u, 0u, 0u);
-                    if (gq < g.group) v = __ldg(qrow + h);
-                    qa[2 * h][0] = v.x; qa[2 * h][1] = v.y; qa[2 * h + 1][0] = v.z; qa[2 * h + 1][1] = v.w;
-                }
-#pragma unroll
-                for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
-                mA = mB = -INFINITY;
-                lA = lB = 0.f;
-            } else if (end) {
-                break;  // empty range
+            // probabilities of head gq, tokens 2qq, 2qq+1 of each block, split into bf16 hi + lo:
+            // exactly the B fragments of O^T += V^T P^T (k = token, n = head)
+            float2 za = make_float2(-INFINITY, -INFINITY), zb = za;
+            if (gq < G) {
+                za = *reinterpret_cast<const float2*>(zptr(pos) + gq * 8 + 2 * qq);
+                if (two) zb = *reinterpret_cast<const float2*>(zptr(pos + 1) + gq * 8 + 2 * qq);
             }
-            const int r_k = (int)((d.w >> 16) & 255u), r_v = (int)(d.w >> 24);
-            const int nb0 = (int)((d.z >> 18) & 15u), nb1 = (int)((d.z >> 22) & 15u);
-            const uint32_t sp0 = stage0 + s * kStageBytes, sp1 = sp0 + ((d.z & 511u) << 4);
-            const bool two = nb1 != 0;
+            const float e00 = ex2(za.x - Mh), e01 = ex2(za.y - Mh), e10 = ex2(zb.x - Mh), e11 = ex2(zb.y - Mh);
+            const uint32_t ph0 = pack_bf16(e00, e01), ph1 = pack_bf16(e10, e11);
+            const uint32_t pl0 = pack_bf16(e00 - __uint_as_float(ph0 << 16), e01 - __uint_as_float(ph0 & 0xffff0000u));
+            const uint32_t pl1 = pack_bf16(e10 - __uint_as_float(ph1 << 16), e11 - __uint_as_float(ph1 & 0xffff0000u));
             const bool full = nb0 == kB && (!two || nb1 == kB);
 
-            mbar_wait(bar0 + 8 * s, parity);  // the group's bulk copies have landed
+            mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);  // the group's V parts have landed
 
-            // ---- QK: S (tokens x heads); rows 0-7 = block 0, rows 8-15 = block 1
-            float S[4] = {0.f, 0.f, 0.f, 0.f};
-            if (r_k == kD && full) {
-                const uint32_t a0 = sp0 + 256 * gq + 64 * qq, a1 = sp1 + 256 * gq + 64 * qq;
+            if (r_v == kD && full) {
+                const uint32_t rA0 = vb0 + 256 * (2 * qq) + 32 * gq, rA1 = vb1 + 256 * (2 * qq) + 32 * gq;
 #pragma unroll
-                for (int h = 0; h < 4; ++h) {
-                    const uint4 x = lds_128(a0 + 16 * h);
-                    uint4 y = make_uint4(0u, 0u, 0u, 0u);
-                    if (two) y = lds_128(a1 + 16 * h);
-                    mma_bf16(S, x.x, y.x, x.y, y.y, qa[2 * h][0], qa[2 * h][1]);
-                    mma_bf16(S, x.z, y.z, x.w, y.w, qa[2 * h + 1][0], qa[2 * h + 1][1]);
+                for (int h = 0; h < 2; ++h) {  // 16-byte chunk h = channel slots 8h .. 8h+7 = tiles 4h .. 4h+3
+                    const uint4 xa = lds_128(rA0 + 16 * h), xb = lds_128(rA0 + 256 + 16 * h);
+                    uint4 ya = make_uint4(0u, 0u, 0u, 0u), yb = ya;
+                    if (two) { ya = lds_128(rA1 + 16 * h); yb = lds_128(rA1 + 256 + 16 * h); }
+                    const uint32_t xav[4] = {xa.x, xa.y, xa.z, xa.w}, xbv[4] = {xb.x, xb.y, xb.z, xb.w};
+                    const uint32_t yav[4] = {ya.x, ya.y, ya.z, ya.w}, ybv[4] = {yb.x, yb.y, yb.z, yb.w};
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const uint32_t a0 = prmt(xav[j], xbv[j], 0x5410u), a1 = prmt(xav[j], xbv[j], 0x7632u);
+                        const uint32_t a2 = prmt(yav[j], ybv[j], 0x5410u), a3 = prmt(yav[j], ybv[j], 0x7632u);
+                        mma_bf16(acc[4 * h + j], a0, a1, a2, a3, ph0, ph1);
+                        mma_bf16(acc[4 * h + j], a0, a1, a2, a3, pl0, pl1);
+                    }
                 }
             } else {
-                // run of (token gq, word qq): starts after the kept elements of the lower words
-                uint32_t w0 = 0u, w1 = 0u, p0, p1, st0 = 2u, st1 = 2u;
-                if (r_k == kD) {  // ragged dense block: all slots kept, no bitmap stored
-                    w0 = gq < nb0 ? 0xffffffffu : 0u;
-                    w1 = gq < nb1 ? 0xffffffffu : 0u;
-                    p0 = sp0 + 256 * gq + 64 * qq;
-                    p1 = sp1 + 256 * gq + 64 * qq;
-                } else {  // values rank-major: rank rho of token t at element rho * nb + t
-                    if (gq < nb0) w0 = lds_u32(sp0 + 4 * lane);
-                    if (gq < nb1) w1 = lds_u32(sp1 + 4 * lane);
-                    uint32_t cnt = (uint32_t)__popc(w0) | ((uint32_t)__popc(w1) << 16), inc = cnt, t;
-                    t = __shfl_up_sync(kFull, inc, 1); if (qq >= 1) inc += t;
-                    t = __shfl_up_sync(kFull, inc, 2); if (qq >= 2) inc += t;
+                const int tA = 2 * qq, tB = 2 * qq + 1;
+                uint32_t hA0 = 0u, hB0 = 0u, hA1 = 0u, hB1 = 0u, pA0, pB0, pA1, pB1, st0 = 2u, st1 = 2u;
+                if (r_v == kD) {  // ragged dense block
+                    hA0 = tA < nb0 ? 0xffffu : 0u; hB0 = tB < nb0 ? 0xffffu : 0u;
+                    hA1 = tA < nb1 ? 0xffffu : 0u; hB1 = tB < nb1 ? 0xffffu : 0u;
+                    pA0 = vb0 + 256 * tA + 32 * gq; pB0 = pA0 + 256;
+                    pA1 = vb1 + 256 * tA + 32 * gq; pB1 = pA1 + 256;
+                } else {
+                    if (tA < nb0) hA0 = lds_u16(vb0 + 16 * tA + 2 * gq);
+                    if (tB < nb0) hB0 = lds_u16(vb0 + 16 * tB + 2 * gq);
+                    if (tA < nb1) hA1 = lds_u16(vb1 + 16 * tA + 2 * gq);
+                    if (tB < nb1) hB1 = lds_u16(vb1 + 16 * tB + 2 * gq);
+                    // exclusive prefix over the lower half-words (lanes gq' < gq, stride 4); four byte counters
+                    const uint32_t cnt = (uint32_t)__popc(hA0) | ((uint32_t)__popc(hB0) << 8) |
+                                         ((uint32_t)__popc(hA1) << 16) | ((uint32_t)__popc(hB1) << 24);
+                    uint32_t inc = cnt, t;
+                    t = __shfl_up_sync(kFull, inc, 4); if (gq >= 1) inc += t;
+                    t = __shfl_up_sync(kFull, inc, 8); if (gq >= 2) inc += t;
+                    t = __shfl_up_sync(kFull, inc, 16); if (gq >= 4) inc += t;
                     const uint32_t ex = inc - cnt;
                     st0 = 2u * nb0; st1 = 2u * nb1;
-                    p0 = sp0 + 16 * nb0 + st0 * (ex & 0xffffu) + 2 * gq;
-                    p1 = sp1 + 16 * nb1 + st1 * (ex >> 16) + 2 * gq;
+                    pA0 = vb0 + 16 * nb0 + st0 * (ex & 255u) + 2 * tA;
+                    pB0 = vb0 + 16 * nb0 + st0 * ((ex >> 8) & 255u) + 2 * tB;
+                    pA1 = vb1 + 16 * nb1 + st1 * ((ex >> 16) & 255u) + 2 * tA;
+                    pB1 = vb1 + 16 * nb1 + st1 * (ex >> 24) + 2 * tB;
                 }
-                k_walk_mma<0>(S, w0, w1, p0, p1, st0, st1, qa);
-                k_walk_mma<1>(S, w0, w1, p0, p1, st0, st1, qa);
-                k_walk_mma<2>(S, w0, w1, p0, p1, st0, st1, qa);
-                k_walk_mma<3>(S, w0, w1, p0, p1, st0, st1, qa);
+                v_walk_mma<0>(acc, hA0, hB0, hA1, hB1, pA0, pB0, pA1, pB1, st0, st1, ph0, ph1, pl0, pl1);
+                v_walk_mma<1>(acc, hA0, hB0, hA1, hB1, pA0, pB0, pA1, pB1, st0, st1, ph0, ph1, pl0, pl1);
             }
-
-            // ---- lazy softmax in the exp2 domain; this lane: token gq of each block, heads 2qq, 2qq+1
-            const bool v0 = gq < nb0, v1 = gq < nb1;
-            const float sA0 = v0 ? S[0] * scale_log2 : -INFINITY, sB0 = v0 ? S[1] * scale_log2 : -INFINITY;
-            const float sA1 = v1 ? S[2] * scale_log2 : -INFINITY, sB1 = v1 ? S[3] * scale_log2 : -INFINITY;
-            float mxA = fmaxf(sA0, sA1), mxB = fmaxf(sB0, sB1);
-            if (__any_sync(kFull, mxA > mA + kRefSlack || mxB > mB + kRefSlack)) {
-                // move the reference (always taken by the first group of a unit: ref = -inf)
-#pragma unroll
-                for (int o = 4; o < 32; o <<= 1) {
-                    mxA = fmaxf(mxA, __shfl_xor_sync(kFull, mxA, o));
-                    mxB = fmaxf(mxB, __shfl_xor_sync(kFull, mxB, o));
-                }
-                const float mnA = fmaxf(mA, mxA), mnB = fmaxf(mB, mxB);
-                const float cA = ex2(mA - (mnA == -INFINITY ? 0.f : mnA)), cB = ex2(mB - (mnB == -INFINITY ? 0.f : mnB));
-#pragma unroll
-                for (int i = 0; i < 8; ++i) { acc[i][0] *= cA; acc[i][1] *= cB; acc[i][2] *= cA; acc[i][3] *= cB; }
-                lA *= cA; lB *= cB;
-                mA = mnA; mB = mnB;
-            }
-            const float bA = mA == -INFINITY ? 0.f : mA, bB = mB == -INFINITY ? 0.f : mB;
-            const float eA0 = ex2(sA0 - bA), eB0 = ex2(sB0 - bB), eA1 = ex2(sA1 - bA), eB1 = ex2(sB1 - bB);
-            lA += eA0 + eA1;
-            lB += eB0 + eB1;
-            // P split into bf16 hi + lo, transposed into the B fragment layout of PV (k = token, n = head)
-            const uint32_t h0 = pack_bf16(eA0, eB0), h1 = pack_bf16(eA1, eB1);
-            const uint32_t l0 = pack_bf16(eA0 - __uint_as_float(h0 << 16), eB0 - __uint_as_float(h0 & 0xffff0000u));
-            const uint32_t l1 = pack_bf16(eA1 - __uint_as_float(h1 << 16), eB1 - __uint_as_float(h1 & 0xffff0000u));
-            const uint32_t ph0 = movmatrix_trans(h0), ph1 = movmatrix_trans(h1);
-            const uint32_t pl0 = movmatrix_trans(l0), pl1 = movmatrix_trans(l1);
-
-            // ---- PV: O^T += V^T P^T (channels x heads), K = the group's 16 tokens
-            {
-                const uint32_t bmk = r_k == kD ? 0u : (uint32_t)kBitmapBytes;
-                const uint32_t vb0 = sp0 + nb0 * (bmk + 2 * r_k), vb1 = sp1 + nb1 * (bmk + 2 * r_k);  // V part of each block
-                if (r_v == kD && full) {
-                    const uint32_t rA0 = vb0 + 256 * (2 * qq) + 32 * gq, rA1 = vb1 + 256 * (2 * qq) + 32 * gq;
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {  // 16-byte chunk h = channel slots 8h .. 8h+7 = tiles 4h .. 4h+3
-                        const uint4 xa = lds_128(rA0 + 16 * h), xb = lds_128(rA0 + 256 + 16 * h);
-                        uint4 ya = make_uint4(0u, 0u, 0u, 0u), yb = ya;
-                        if (two) { ya = lds_128(rA1 + 16 * h); yb = lds_128(rA1 + 256 + 16 * h); }
-                        const uint32_t xav[4] = {xa.x, xa.y, xa.z, xa.w}, xbv[4] = {xb.x, xb.y, xb.z, xb.w};
-                        const uint32_t yav[4] = {ya.x, ya.y, ya.z, ya.w}, ybv[4] = {yb.x, yb.y, yb.z, yb.w};
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const uint32_t a0 = prmt(xav[j], xbv[j], 0x5410u), a1 = prmt(xav[j], xbv[j], 0x7632u);
-                            const uint32_t a2 = prmt(yav[j], ybv[j], 0x5410u), a3 = prmt(yav[j], ybv[j], 0x7632u);
-                            mma_bf16(acc[4 * h + j], a0, a1, a2, a3, ph0, ph1);
-                            mma_bf16(acc[4 * h + j], a0, a1, a2, a3, pl0, pl1);
-                        }
-                    }
-                } else {
-                    const int tA = 2 * qq, tB = 2 * qq + 1;
-                    uint32_t hA0 = 0u, hB0 = 0u, hA1 = 0u, hB1 = 0u, pA0, pB0, pA1, pB1, st0 = 2u, st1 = 2u;
-                    if (r_v == kD) {  // ragged dense block
-                        hA0 = tA < nb0 ? 0xffffu : 0u; hB0 = tB < nb0 ? 0xffffu : 0u;
-                        hA1 = tA < nb1 ? 0xffffu : 0u; hB1 = tB < nb1 ? 0xffffu : 0u;
-                        pA0 = vb0 + 256 * tA + 32 * gq; pB0 = pA0 + 256;
-                        pA1 = vb1 + 256 * tA + 32 * gq; pB1 = pA1 + 256;
-                    } else {
-                        if (tA < nb0) hA0 = lds_u16(vb0 + 16 * tA + 2 * gq);
-                        if (tB < nb0) hB0 = lds_u16(vb0 + 16 * tB + 2 * gq);
-                        if (tA < nb1) hA1 = lds_u16(vb1 + 16 * tA + 2 * gq);
-                        if (tB < nb1) hB1 = lds_u16(vb1 + 16 * tB + 2 * gq);
-                        // exclusive prefix over the lower half-words (lanes gq' < gq, stride 4); four byte counters
-                        const uint32_t cnt = (uint32_t)__popc(hA0) | ((uint32_t)__popc(hB0) << 8) |
-                                             ((uint32_t)__popc(hA1) << 16) | ((uint32_t)__popc(hB1) << 24);
-                        uint32_t inc = cnt, t;
-                        t = __shfl_up_sync(kFull, inc, 4); if (gq >= 1) inc += t;
-                        t = __shfl_up_sync(kFull, inc, 8); if (gq >= 2) inc += t;
-                        t = __shfl_up_sync(kFull, inc, 16); if (gq >= 4) inc += t;
-                        const uint32_t ex = inc - cnt;
-                        st0 = 2u * nb0; st1 = 2u * nb1;
-                        pA0 = vb0 + 16 * nb0 + st0 * (ex & 255u) + 2 * tA;
-                        pB0 = vb0 + 16 * nb0 + st0 * ((ex >> 8) & 255u) + 2 * tB;
-                        pA1 = vb1 + 16 * nb1 + st1 * ((ex >> 16) & 255u) + 2 * tA;
-                        pB1 = vb1 + 16 * nb1 + st1 * (ex >> 24) + 2 * tB;
-                    }
-                    v_walk_mma<0>(acc, hA0, hB0, hA1, hB1, pA0, pB0, pA1, pB1, st0, st1, ph0, ph1, pl0, pl1);
-                    v_walk_mma<1>(acc, hA0, hB0, hA1, hB1, pA0, pB0, pA1, pB1, st0, st1, ph0, ph1, pl0, pl1);
-                }
-            }
-            __syncwarp();  // every lane is done reading stage s
-            bposc += two ? 2 : 1;
-            ++gposc;
+            __syncwarp();  // every lane is done reading the slot
+            ring_release();
         }
-        issue(s);  // stage s is free (or, for k < 0, still empty): start the copies of group k + NSTAGE
-        if (++s == NSTAGE) { s = 0; if (k >= 0) parity ^= 1u; }
+        if (!kGatherOnly && cur_unit >= 0) flush(true);
     }
-#ifdef MKV_DBG_TIMING
-    if (lane == 0) { atomicMin(&g_dbg_t[blockIdx.x * 16 + 5], dbg_now()); atomicMax(&g_dbg_t[blockIdx.x * 16 + 6], dbg_now()); }
-#endif
     if (kGatherOnly) {  // keep the read-back alive; nothing else is written
-        if (calib == 0x9e3779b9u && lane == 0) part_ml[(size_t)gw * 2 * (2 * kMaxGroup)] = 0.f;
+        if (calib == 0x9e3779b9u && lane == 0) scr.part_l[(size_t)gw * 2 * (2 * kMaxGroup)] = 0.f;
         return;
     }
+    if (lane == 0 && st_vblocks != 0ull) {
+        atomicAdd(scr.stats + 1, st_vblocks);
+        atomicAdd(scr.stats + 2, st_vbytes);
+    }
+    if (threadIdx.x == 0 && blockIdx.x == 0) atomicAdd(scr.stats + 0, (unsigned long long)T);
 
-    // ---- step 3d, fused: fold the warps' partials; finish units that span several CTAs.
+    // ---- step 3d, fused: add the warps' partials; finish units that span several CTAs.
     // Records are in warp order (2w = head, 2w + 1 = tail), hence in non-decreasing unit order: the
-    // partials of one unit form a run.  Thread tid owns output elements e = tid + j kNT of [G][D]
-    // and folds a run with the LSE rule (pinned by oracle pin P10).
+    // partials of one unit form a run.  Thread tid owns four consecutive output channels of one head.
+    // All partials of a unit are relative to the same maximum, so folding is plain addition (the
+    // split-K rule of oracle pin P10 with equal references).
     __syncthreads();  // orders the warps' partials (shared memory, or global scratch from flush(false))
-    MKV_TV(1, *(volatile int*)&s_unit[1]);
     const int GD = G * kD;
-    const size_t cta_slot_base = (size_t)gridDim.x * kMaxWarps * 2;
+    const size_t cta_slot_base = (size_t)gridDim.x * kWarps * 2;
     const int tid = threadIdx.x;
     int sh_u0 = -1, sh_u1 = -1;  // units this CTA shares with others (<= 2: one entering, one leaving its range)
     int n_shared = 0;
-    // GD / 4 threads fold one unit (four consecutive channels of one head each), so a CTA folds
-    // kNT / (GD / 4) units side by side: usually all of them (1 or 2 per CTA) in one pass.
+    // GD / 4 threads fold one unit, so a CTA folds kNT / (GD / 4) units side by side
     const int tpr = GD / 4, nslots = max(1, kNT / tpr);
     const int rs = tid / tpr, e = 4 * (tid - rs * tpr), h = e >> 7;
-    // each lane keeps the units of records lane and lane + 32: searches and membership are votes
-    const int myu0 = lane < kRec ? s_unit[lane] : -1, myu1 = lane + 32 < kRec ? s_unit[lane + 32] : -1;
+    // each lane keeps the unit of record `lane`: searches and membership are votes
+    const int myu0 = lane < kRec ? s_unit[lane] : -1;
     int run = -1;
 #pragma unroll 1
     for (;;) {
@@ -548,12 +716,15 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         int mine = -1, last = run;
 #pragma unroll 1
         for (int k = 0; k < nslots; ++k) {
-            const int c0 = myu0 > last ? myu0 : 0x7fffffff, c1 = myu1 > last ? myu1 : 0x7fffffff;
-            const int nxt = __reduce_min_sync(kFull, min(c0, c1));
+            const int nxt = __reduce_min_sync(kFull, myu0 > last ? myu0 : 0x7fffffff);
             if (nxt == 0x7fffffff) break;
             last = nxt;
             if (k == rs) mine = nxt;
-            if (!(clo <= s_cum[nxt] && s_cum[nxt + 1] <= chi) && n_shared < 2) {  // shared with other CTAs
+            const bool inside = clo <= s_cum[nxt] && s_cum[nxt + 1] <= chi;
+            if (inside) {
+                // wholly inside this CTA and past phase 2 in every warp: reset its maxima for the next launch
+                if (tid < kMaxGroup) scr.umax[(size_t)nxt * kMaxGroup + tid] = 0u;
+            } else if (n_shared < 2) {  // shared with other CTAs
                 if (tid == 0) s_row[n_shared] = (size_t)(nxt / g.n_kv_heads) * g.n_q_heads + (size_t)(nxt % g.n_kv_heads) * G;
                 if (n_shared == 0) sh_u0 = nxt; else sh_u1 = nxt;
                 ++n_shared;
@@ -563,63 +734,43 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         run = last;
         if (mine < 0) continue;  // uniform over a warp: GD / 4 is a multiple of 32
         // records of this unit: bit r of `recs` (tail partials are the odd records, head partials the even ones)
-        const unsigned long long recs = (unsigned long long)__ballot_sync(kFull, myu0 == mine) |
-                                        ((unsigned long long)__ballot_sync(kFull, myu1 == mine) << 32);
-        unsigned heads = 0u;  // warps that hold a head partial (record 2w, in global scratch) of this unit: rare
-#pragma unroll
-        for (int w = 0; w < kWarps; ++w) heads |= (unsigned)((recs >> (2 * w)) & 1ull) << w;
+        const unsigned recs = __ballot_sync(kFull, myu0 == mine);
         const int a = s_cum[mine], b = s_cum[mine + 1];
         const bool whole = clo <= a && b <= chi;
         const size_t row = (size_t)(mine / g.n_kv_heads) * g.n_q_heads + (size_t)(mine % g.n_kv_heads) * G;
         const size_t slot = cta_slot_base + blockIdx.x * 2 + (a < clo ? 0 : 1);
-        {
-            // tail partials (record 2w + 1, in warp w's shared memory): straight-line, every load independent
-            float mw[kWarps], lw[kWarps];
-            float4 ow[kWarps];
-            float Mr = -INFINITY;
+        float4 O = make_float4(0.f, 0.f, 0.f, 0.f);
+        float Lr = 0.f, Mr = -INFINITY;
+        // tail partials (record 2w + 1, in warp w's shared memory): straight-line, every load independent
 #pragma unroll
-            for (int w = 0; w < kWarps; ++w) {
-                const bool mem = (recs >> (2 * w + 1)) & 1ull;
-                const float2 ml = *reinterpret_cast<const float2*>(&s_ml[2 * w + 1][h][0]);
-                ow[w] = *reinterpret_cast<const float4*>(smem + w * kWS + 4 * e);
-                mw[w] = mem ? ml.x : -INFINITY;
-                lw[w] = mem ? ml.y : 0.f;
-                Mr = fmaxf(Mr, mw[w]);
-            }
+        for (int w = 0; w < kWarps; ++w) {
+            const bool mem = (recs >> (2 * w + 1)) & 1u;
+            const float2 ml = *reinterpret_cast<const float2*>(&s_ml[2 * w + 1][h][0]);
+            const float4 o = *reinterpret_cast<const float4*>(smem + w * kWS + 4 * e);
+            if (mem) { Mr = ml.x; Lr += ml.y; O.x += o.x; O.y += o.y; O.z += o.z; O.w += o.w; }
+        }
+        // head partials (record 2w, in global scratch): rare
 #pragma unroll 1
-            for (unsigned m = heads; m; m &= m - 1u) Mr = fmaxf(Mr, s_ml[2 * (__ffs(m) - 1)][h][0]);
-            const float Mb = Mr == -INFINITY ? 0.f : Mr;
-            float4 O = make_float4(0.f, 0.f, 0.f, 0.f);
-            float Lr = 0.f;
-#pragma unroll
-            for (int w = 0; w < kWarps; ++w) {
-                const float wt = ex2(mw[w] - Mb);  // 0 for a record of another unit (its O may be stale bits)
-                Lr = fmaf(lw[w], wt, Lr);
-                if (wt != 0.f) { O.x = fmaf(ow[w].x, wt, O.x); O.y = fmaf(ow[w].y, wt, O.y); O.z = fmaf(ow[w].z, wt, O.z); O.w = fmaf(ow[w].w, wt, O.w); }
-            }
-#pragma unroll 1
-            for (unsigned m = heads; m; m &= m - 1u) {
-                const int w = __ffs(m) - 1;
-                const float wt = ex2(s_ml[2 * w][h][0] - Mb);
-                Lr = fmaf(s_ml[2 * w][h][1], wt, Lr);
-                const float4 o = __ldcg(reinterpret_cast<const float4*>(
-                    part_o + ((size_t)blockIdx.x * kWarps + w) * 2 * (size_t)GD + e));
-                O.x = fmaf(o.x, wt, O.x); O.y = fmaf(o.y, wt, O.y); O.z = fmaf(o.z, wt, O.z); O.w = fmaf(o.w, wt, O.w);
-            }
-            if (whole) {
-                const float inv = Lr > 0.f ? 1.f / Lr : 0.f;
-                *reinterpret_cast<float4*>(out + row * kD + e) = make_float4(O.x * inv, O.y * inv, O.z * inv, O.w * inv);
-                if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = Lr > 0.f ? (Mr + log2f(Lr)) * kLn2 : -INFINITY;
-            } else {
-                *reinterpret_cast<float4*>(part_o + slot * GD + e) = O;
-                if ((e & (kD - 1)) == 0) {
-                    part_ml[slot * (2 * kMaxGroup) + 2 * h] = Mr;
-                    part_ml[slot * (2 * kMaxGroup) + 2 * h + 1] = Lr;
-                }
+        for (unsigned m = recs & 0x55555555u; m; m &= m - 1u) {
+            const int w = (__ffs(m) - 1) >> 1;
+            Mr = s_ml[2 * w][h][0];
+            Lr += s_ml[2 * w][h][1];
+            const float4 o = __ldcg(reinterpret_cast<const float4*>(
+                scr.part_o + ((size_t)blockIdx.x * kWarps + w) * 2 * (size_t)GD + e));
+            O.x += o.x; O.y += o.y; O.z += o.z; O.w += o.w;
+        }
+        if (whole) {
+            const float inv = Lr > 0.f ? 1.f / Lr : 0.f;
+            *reinterpret_cast<float4*>(out + row * kD + e) = make_float4(O.x * inv, O.y * inv, O.z * inv, O.w * inv);
+            if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = Lr > 0.f ? (Mr + log2f(Lr)) * kLn2 : -INFINITY;
+        } else {
+            *reinterpret_cast<float4*>(scr.part_o + slot * GD + e) = O;
+            if ((e & (kD - 1)) == 0) {
+                scr.part_l[slot * (2 * kMaxGroup) + 2 * h] = Mr;
+                scr.part_l[slot * (2 * kMaxGroup) + 2 * h + 1] = Lr;
             }
         }
     }
-    MKV_T(2);
     if (n_shared == 0) return;  // uniform over the CTA
 
     // One thread per shared unit releases the CTA's partial (the barrier orders the other threads'
@@ -633,14 +784,18 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         if (s_cum[u + 1] > chi) cl = (int)cs.owner(((unsigned)s_cum[u + 1] - 1u) >> 1);
         s_cf[k] = cf; s_cl[k] = cl;
         int old;  // release this CTA's partial (ordered by the barrier), acquire the other sharers'
-        asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(ticket + u) : "memory");
+        asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(scr.ticket + u) : "memory");
         s_last[k] = old == cl - cf;
-        if (old == cl - cf) ticket[u] = 0;  // self-cleaning: every sharer has arrived
+        if (old == cl - cf) {  // every sharer has arrived (and is past phase 2): reset the unit's state for the next launch
+            scr.ticket[u] = 0;
+            scr.uarrive[u] = 0;
+#pragma unroll
+            for (int hh = 0; hh < kMaxGroup; ++hh) scr.umax[(size_t)u * kMaxGroup + hh] = 0u;
+        }
     }
     __syncthreads();
-    MKV_T(3);
-    // last arrivers: thread group rs merges the CTA partials of shared unit rs (read with ld.global.cg: L2,
-    // never a stale L1 line); with nslots = 1 (G = 8 on a small CTA) the groups take the units in turn
+    // last arrivers: thread group rs adds the CTA partials of shared unit rs (read with ld.global.cg: L2,
+    // never a stale L1 line), in CTA order; with nslots = 1 (G = 8) the groups take the units in turn
 #pragma unroll 1
     for (int k = rs < nslots ? rs : n_shared; k < n_shared; k += nslots) {
         if (!s_last[k]) continue;
@@ -654,82 +809,95 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             float4 po[4];
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
-                const int c = min(c0 + t, c_last);  // a repeated partial gets weight 0 below
+                const int c = min(c0 + t, c_last);  // a repeated partial is not added below
                 const size_t sl = cta_slot_base + (size_t)c * 2 + (c == c_first ? 1 : 0);
-                pm[t] = __ldcg(part_ml + sl * (2 * kMaxGroup) + 2 * h);
-                pl[t] = __ldcg(part_ml + sl * (2 * kMaxGroup) + 2 * h + 1);
-                po[t] = __ldcg(reinterpret_cast<const float4*>(part_o + sl * (size_t)GD + e));
-                if (c0 + t > c_last) { pm[t] = -INFINITY; pl[t] = 0.f; }
+                pm[t] = __ldcg(scr.part_l + sl * (2 * kMaxGroup) + 2 * h);
+                pl[t] = __ldcg(scr.part_l + sl * (2 * kMaxGroup) + 2 * h + 1);
+                po[t] = __ldcg(reinterpret_cast<const float4*>(scr.part_o + sl * (size_t)GD + e));
             }
-            const float Mn = fmaxf(fmaxf(Mx, fmaxf(pm[0], pm[1])), fmaxf(pm[2], pm[3]));
-            const float Mb = Mn == -INFINITY ? 0.f : Mn;
-            const float c_old = ex2(Mx - Mb);
-            Lx *= c_old; Ox.x *= c_old; Ox.y *= c_old; Ox.z *= c_old; Ox.w *= c_old; Mx = Mn;
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
-                const float w = ex2(pm[t] - Mb);
-                Lx = fmaf(pl[t], w, Lx);
-                Ox.x = fmaf(po[t].x, w, Ox.x); Ox.y = fmaf(po[t].y, w, Ox.y);
-                Ox.z = fmaf(po[t].z, w, Ox.z); Ox.w = fmaf(po[t].w, w, Ox.w);
+                if (c0 + t > c_last) continue;
+                Mx = pm[t];
+                Lx += pl[t];
+                Ox.x += po[t].x; Ox.y += po[t].y; Ox.z += po[t].z; Ox.w += po[t].w;
             }
         }
         const float inv = Lx > 0.f ? 1.f / Lx : 0.f;
         *reinterpret_cast<float4*>(out + row * kD + e) = make_float4(Ox.x * inv, Ox.y * inv, Ox.z * inv, Ox.w * inv);
         if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = Lx > 0.f ? (Mx + log2f(Lx)) * kLn2 : -INFINITY;
     }
-    MKV_T(4);
+}
+
+// calibration row (i) of SURVEY 8(d): a plain streaming read of `bytes` bytes in the attention kernel's launch shape
+__global__ void __launch_bounds__(kWarps * 32, 1)
+mkv_stream_read_kernel(const uint4* __restrict__ base, unsigned long long n16, unsigned long long* __restrict__ sink) {
+    pdl_wait();
+    pdl_launch_dependents();
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    uint32_t acc = 0u;
+    unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+#pragma unroll 1
+    for (; i + 3ull * stride < n16; i += 4ull * stride) {  // four independent 16-byte loads in flight per thread
+        uint4 v[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                         : "=r"(v[j].x), "=r"(v[j].y), "=r"(v[j].z), "=r"(v[j].w) : "l"(base + i + j * stride));
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc ^= v[j].x ^ v[j].y ^ v[j].z ^ v[j].w;
+    }
+#pragma unroll 1
+    for (; i < n16; i += stride) {
+        uint4 v;
+        asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                     : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(base + i));
+        acc ^= v.x ^ v.y ^ v.z ^ v.w;
+    }
+    if (acc == 0x9e3779b9u) *sink = acc;  // keeps the loads alive
 }
 
 }  // namespace
 
-#ifdef MKV_DBG_TIMING
-extern "C" __attribute__((visibility("default"))) int mkv_dbg_timing(unsigned long long* host, int reset) {
-    if (reset) { static unsigned long long init[160 * 16]; for (int i = 0; i < 160 * 16; ++i) init[i] = (i % 16 == 5) ? ~0ull : 0ull; return (int)cudaMemcpyToSymbol(g_dbg_t, init, sizeof(init)); }
-    return (int)cudaMemcpyFromSymbol(host, g_dbg_t, sizeof(unsigned long long) * 160 * 16);
+int attention_partial_slots(int sm_count) { return sm_count * kWarps * 2 + sm_count * 2; }
+
+// logit scratch: one entry of 8 G floats per position of the block stream (selected blocks + update-buffer blocks)
+size_t attention_zbuf_floats(const CacheGeom& g) {
+    return (size_t)g.n_units * ((size_t)g.score_stride + 1 + (size_t)(g.L + kB - 1) / kB) * 8 * (size_t)g.group;
 }
-#endif
 
-int attention_partial_slots(int sm_count) { return sm_count * kMaxWarps * 2 + sm_count * 2; }
-
-template <int NSTAGE, int NWARPS, bool GATHER>
+template <bool GATHER>
 static cudaError_t launch_attention_cfg(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
                                         const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
                                         const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v,
-                                        const int32_t* upd_count, int sm_count, cudaStream_t s) {
-    const int smem = NWARPS * warp_smem_bytes(NSTAGE) + (g.n_units + 1) * 4;
-    static int configured = 0;  // largest dynamic shared-memory size opted into so far
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(mkv_packed_attention_kernel<NSTAGE, NWARPS, GATHER>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
-    return launch_pdl(mkv_packed_attention_kernel<NSTAGE, NWARPS, GATHER>, dim3(sm_count), dim3(NWARPS * 32), (size_t)smem, s,
-                      g, lv, q, sel, sel_count, k_max, scale * kLog2e, out, lse, scr.part_o, scr.part_ml, scr.ticket, upd_k,
-                      upd_v, upd_count);
+                                        const int32_t* upd_count, uint32_t* dev_flags, int sm_count, cudaStream_t s) {
+    const int smem = kWarps * kWS + (g.n_units + 1) * 4;
+    // the dynamic shared-memory opt-in is a per-device attribute of the function: set it on every launch (a cheap
+    // host-side call) so that caches on different devices of one process are independent
+    cudaError_t e = cudaFuncSetAttribute(mkv_packed_attention_kernel<GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    return launch_pdl(mkv_packed_attention_kernel<GATHER>, dim3(sm_count), dim3(kWarps * 32), (size_t)smem, s, g, lv, q, sel,
+                      sel_count, k_max, scale * kLog2e, out, lse, scr, upd_k, upd_v, upd_count, dev_flags);
 }
 
 cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
                              const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
                              const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v,
-                             const int32_t* upd_count, int sm_count, cudaStream_t s, int* n_kernels, bool gather_only) {
+                             const int32_t* upd_count, uint32_t* dev_flags, int sm_count, cudaStream_t s, int* n_kernels,
+                             bool gather_only) {
     if (g.n_units > kMaxUnitsSmem) return cudaErrorInvalidValue;
     if (n_kernels) *n_kernels = 1;
     if (gather_only)
-        return launch_attention_cfg<3, 16, true>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, upd_count,
-                                                 sm_count, s);
-    static int cfg = -1;  // tuning knob (stages * 100 + warps); default chosen from measurements
-    if (cfg < 0) {
-        const char* e = getenv("MKV_ATTN_CFG");
-        cfg = e ? atoi(e) : 316;
-    }
-#define MKV_CFG(S, W) \
-    case S * 100 + W: return launch_attention_cfg<S, W, false>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, upd_count, sm_count, s);
-    switch (cfg) {
-        MKV_CFG(3, 16) MKV_CFG(2, 16) MKV_CFG(2, 20) MKV_CFG(2, 24) MKV_CFG(4, 12) MKV_CFG(4, 8)
-        default: return launch_attention_cfg<3, 16, false>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, upd_count, sm_count, s);
-    }
-#undef MKV_CFG
+        return launch_attention_cfg<true>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, upd_count,
+                                          dev_flags, sm_count, s);
+    return launch_attention_cfg<false>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, upd_count,
+                                       dev_flags, sm_count, s);
+}
+
+cudaError_t launch_stream_read(const uint8_t* base, unsigned long long bytes, int sm_count, unsigned long long* sink,
+                               cudaStream_t s) {
+    return launch_pdl(mkv_stream_read_kernel, dim3(sm_count), dim3(kWarps * 32), (size_t)0, s,
+                      reinterpret_cast<const uint4*>(base), bytes / 16ull, sink);
 }
 
 }  // namespace mkv

@@ -130,7 +130,9 @@ __global__ void __launch_bounds__(256) mkv_plan_kernel(CacheGeom g, LayerView lv
         int B = 0;
         for (int i = 0; i < 8; ++i) { T += s_tok[i]; K += s_bk[i]; B |= s_bad[i]; }
         unsigned long long base = kNoBase;
-        if (B) {
+        if (B || lv.unit_nseg[unit] != a.seg0) {
+            // a bad strategy, or an earlier call for this unit was rejected on the device (the host's append
+            // state ran ahead): never leave a hole of unwritten table entries behind
             atomicOr(dev_flags, MKV_DEV_BAD_STRATEGY);
         } else {
             base = atomicAdd(lv.bump, T + K);
@@ -360,16 +362,19 @@ __global__ void __launch_bounds__(256) mkv_strategy_quantile_kernel(const double
     }
 }
 
+struct CandList {
+    mkv_strategy c[64];
+};
 __global__ void mkv_strategy_threshold_kernel(const double* __restrict__ loss_k, const double* __restrict__ loss_v,
-                                              int ncand, long long n, const mkv_strategy* __restrict__ cands,
-                                              double tau, mkv_strategy* __restrict__ out) {
+                                              int ncand, long long n, const CandList cands, double tau,
+                                              mkv_strategy* __restrict__ out) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     mkv_strategy s;
-    s.r_k = kD; s.r_v = kD; s.g = 1; s.B = cands[ncand - 1].B;
+    s.r_k = kD; s.r_v = kD; s.g = 1; s.B = cands.c[ncand - 1].B;
     for (int c = 0; c < ncand; ++c) {
         const double I = 0.5 * (loss_k[(size_t)c * n + i] + loss_v[(size_t)c * n + i]);
-        if (I <= tau) { s = cands[c]; break; }
+        if (I <= tau) { s = cands.c[c]; break; }
     }
     out[i] = s;
 }
@@ -420,11 +425,13 @@ cudaError_t launch_strategy_quantile(const double* loss_k, const double* loss_v,
 }
 
 cudaError_t launch_strategy_threshold(const double* loss_k, const double* loss_v, int ncand, long long n,
-                                      const mkv_strategy* cands_dev, double tau, mkv_strategy* out,
+                                      const mkv_strategy* cands_host, double tau, mkv_strategy* out,
                                       cudaStream_t s) {
     const int threads = 256;
     const long long blocks = (n + threads - 1) / threads;
-    mkv_strategy_threshold_kernel<<<(unsigned)blocks, threads, 0, s>>>(loss_k, loss_v, ncand, n, cands_dev, tau, out);
+    CandList cl;  // by value: read during this call only, so the call is capturable and needs no staging buffer
+    for (int i = 0; i < 64; ++i) cl.c[i] = cands_host[i < ncand ? i : ncand - 1];
+    mkv_strategy_threshold_kernel<<<(unsigned)blocks, threads, 0, s>>>(loss_k, loss_v, ncand, n, cl, tau, out);
     return cudaGetLastError();
 }
 

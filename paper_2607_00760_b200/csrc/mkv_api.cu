@@ -59,16 +59,25 @@ struct mkv_cache {
     int32_t* upd_cnt = nullptr;               // [n_layers] tokens buffered per unit (read by the attention kernel)
     std::vector<int32_t> upd_n;               // host mirror (every unit of a layer holds the same number)
     AttnScratch attn{};
+    PlanRec* plan = nullptr;                  // [n_layers][n_units][sel_cap]: what top-k tells attention about each selected block
+    uint32_t generation = 1;                  // bumped by mkv_cache_reset: invalidates every plan record
+    unsigned long long* sink = nullptr;
     uint16_t* q_dev = nullptr;
     int32_t* sel_dev = nullptr;
     int32_t* selcnt_dev = nullptr;
     float* out_dev = nullptr;
-    mkv_strategy* cands_dev = nullptr;
     int sel_cap = 0;
     // host mirrors of the append state, [n_layers][batch]
     std::vector<int32_t> host_nseg, host_ntok;
     int last_select = 0, last_attn = 0, last_compress = 0;
 
+    AttnScratch attn_scratch(int layer) const {
+        AttnScratch a = attn;
+        a.plan = plan + (size_t)layer * geom.n_units * sel_cap;
+        a.plan_stride = sel_cap;
+        a.plan_tag = plan_tag(generation, layer);
+        return a;
+    }
     LayerView view(int layer) const {
         LayerView v;
         const size_t tu = (size_t)layer * geom.n_units;
@@ -97,8 +106,8 @@ int mkv_cache_free(mkv_cache* c) {
     cudaSetDevice(c->desc.device);
     cudaDeviceSynchronize();
     void* ptrs[] = {c->arena, c->strat, c->tok_off, c->bk_off, c->unit_nseg, c->unit_ntok, c->counters,
-                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->upd_k, c->upd_v, c->upd_cnt, c->attn.part_o, c->attn.part_ml, c->attn.ticket, c->q_dev,
-                    c->sel_dev, c->selcnt_dev, c->out_dev, c->cands_dev};
+                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->upd_k, c->upd_v, c->upd_cnt, c->attn.part_o, c->attn.part_l, c->attn.ticket, c->attn.umax, c->attn.uarrive, c->attn.zbuf, c->attn.stats, c->plan, c->sink, c->q_dev,
+                    c->sel_dev, c->selcnt_dev, c->out_dev};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     delete c;
@@ -133,7 +142,8 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     g.blocks_per_seg = g.L / kB; g.score_stride = (d->max_tokens + kB - 1) / kB;
     MKV_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, d->device));
 
-    const uint64_t worst = (uint64_t)g.n_units * ((uint64_t)g.score_stride * (4096 + 256) + 64) + 4096;
+    // largest payloads: r = 127 on both sides (bitmap + 254 B per vector): 8 * 2 * 270 B per token block, 270 B per block key
+    const uint64_t worst = (uint64_t)g.n_units * ((uint64_t)g.score_stride * (4320 + 272) + 64 + 16ull * g.S_max) + 4096;
     uint64_t per_layer = d->arena_bytes ? d->arena_bytes / (uint64_t)d->n_layers : worst;
     per_layer = per_layer / 256 * 256;
     if (per_layer < 256) { delete c; return fail(MKV_E_ARG, "arena_bytes too small"); }
@@ -163,13 +173,18 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         {(void**)&c->upd_v, upd_bytes},
         {(void**)&c->upd_cnt, (size_t)g.n_layers * 4 + 252},
         {(void**)&c->attn.part_o, (size_t)c->attn.slots * g.group * kD * 4},
-        {(void**)&c->attn.part_ml, (size_t)c->attn.slots * kMaxGroup * 2 * 4},
+        {(void**)&c->attn.part_l, (size_t)c->attn.slots * kMaxGroup * 2 * 4},
         {(void**)&c->attn.ticket, (size_t)g.n_units * 4},
+        {(void**)&c->attn.umax, (size_t)g.n_units * kMaxGroup * 4},
+        {(void**)&c->attn.uarrive, (size_t)g.n_units * 4},
+        {(void**)&c->attn.zbuf, attention_zbuf_floats(g) * 4},
+        {(void**)&c->attn.stats, 64},
+        {(void**)&c->plan, tu * (size_t)c->sel_cap * sizeof(PlanRec)},
+        {(void**)&c->sink, 64},
         {(void**)&c->q_dev, (size_t)g.batch * g.n_q_heads * kD * 2},
         {(void**)&c->sel_dev, (size_t)g.n_units * c->sel_cap * 4},
         {(void**)&c->selcnt_dev, (size_t)g.n_units * 4},
         {(void**)&c->out_dev, (size_t)g.batch * g.n_q_heads * kD * 4},
-        {(void**)&c->cands_dev, 64 * sizeof(mkv_strategy)},
     };
     for (auto& a : allocs) {
         cudaError_t e = cudaMalloc(a.p, a.bytes);
@@ -185,6 +200,10 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     cudaMemset(c->dev_flags, 0, 256);
     cudaMemset(c->upd_cnt, 0, (size_t)g.n_layers * 4);
     cudaMemset(c->attn.ticket, 0, (size_t)g.n_units * 4);
+    cudaMemset(c->attn.umax, 0, (size_t)g.n_units * kMaxGroup * 4);
+    cudaMemset(c->attn.uarrive, 0, (size_t)g.n_units * 4);
+    cudaMemset(c->attn.stats, 0, 64);
+    cudaMemset(c->plan, 0, tu * (size_t)c->sel_cap * sizeof(PlanRec));
     cudaMemset(c->strat, 0, tu * g.S_max * sizeof(StratRec));
     c->host_nseg.assign((size_t)g.n_layers * g.batch, 0);
     c->host_ntok.assign((size_t)g.n_layers * g.batch, 0);
@@ -203,6 +222,10 @@ int mkv_cache_reset(mkv_cache* c, int32_t layer, void* stream) {
     if (layer < -1 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
     cudaStream_t s = (cudaStream_t)stream;
     const int l0 = layer < 0 ? 0 : layer, l1 = layer < 0 ? g.n_layers : layer + 1;
+    ++c->generation;  // plan records written before the reset no longer match
+    MKV_CUDA(cudaMemsetAsync(c->attn.ticket, 0, (size_t)g.n_units * 4, s));  // (a launch that timed out leaves these dirty)
+    MKV_CUDA(cudaMemsetAsync(c->attn.umax, 0, (size_t)g.n_units * kMaxGroup * 4, s));
+    MKV_CUDA(cudaMemsetAsync(c->attn.uarrive, 0, (size_t)g.n_units * 4, s));
     for (int l = l0; l < l1; ++l) {
         MKV_CUDA(cudaMemsetAsync(c->unit_nseg + (size_t)l * g.n_units, 0, (size_t)g.n_units * 4, s));
         MKV_CUDA(cudaMemsetAsync(c->unit_ntok + (size_t)l * g.n_units, 0, (size_t)g.n_units * 4, s));
@@ -257,9 +280,8 @@ int mkv_strategy_threshold(const mkv_cache* c, const double* loss_k, const doubl
     if (!c || !loss_k || !loss_v || !out || !cands_host) return fail(MKV_E_ARG, "mkv_strategy_threshold: NULL argument");
     if (ncand < 1 || ncand > 64 || n_units < 1 || nseg < 1) return fail(MKV_E_ARG, "mkv_strategy_threshold: bad sizes");
     MKV_CUDA(cudaSetDevice(c->desc.device));
-    MKV_CUDA(cudaMemcpyAsync(c->cands_dev, cands_host, ncand * sizeof(mkv_strategy), cudaMemcpyHostToDevice,
-                             (cudaStream_t)stream));
-    MKV_CUDA(launch_strategy_threshold(loss_k, loss_v, ncand, (long long)n_units * nseg, c->cands_dev, tau, out,
+    // the candidates travel as a kernel argument (read during this call only: capturable, no staging buffer)
+    MKV_CUDA(launch_strategy_threshold(loss_k, loss_v, ncand, (long long)n_units * nseg, cands_host, tau, out,
                                        (cudaStream_t)stream));
     return MKV_OK;
 }
@@ -301,8 +323,9 @@ int mkv_select(const mkv_cache* cc, int32_t layer, const void* q, int32_t budget
         return fail(MKV_E_ARG, "mkv_select: k_max %d too small for budget %d", k_max, budget);
     MKV_CUDA(cudaSetDevice(c->desc.device));
     MKV_CUDA(launch_select(g, c->view(layer), (const uint16_t*)q, budget, reduce, sel, sel_count, k_max,
-                           scores_opt ? scores_opt : c->scores, c->cand_key, c->cand_idx, c->sm_count, (cudaStream_t)stream,
-                           &c->last_select));
+                           scores_opt ? scores_opt : c->scores, c->cand_key, c->cand_idx,
+                           c->plan + (size_t)layer * g.n_units * c->sel_cap, c->sel_cap, plan_tag(c->generation, layer),
+                           c->sm_count, (cudaStream_t)stream, &c->last_select));
     return MKV_OK;
 }
 
@@ -317,8 +340,8 @@ int mkv_packed_attention(const mkv_cache* cc, int32_t layer, const void* q, cons
     MKV_CUDA(cudaSetDevice(c->desc.device));
     const size_t upd_off = (size_t)layer * g.n_units * g.L * kD;
     MKV_CUDA(launch_attention(g, c->view(layer), (const uint16_t*)q, sel, sel_count, k_max, scale, out, lse_opt,
-                              c->attn, c->upd_k + upd_off, c->upd_v + upd_off, c->upd_cnt + layer, c->sm_count,
-                              (cudaStream_t)stream, &c->last_attn));
+                              c->attn_scratch(layer), c->upd_k + upd_off, c->upd_v + upd_off, c->upd_cnt + layer,
+                              c->dev_flags, c->sm_count, (cudaStream_t)stream, &c->last_attn));
     return MKV_OK;
 }
 
@@ -332,9 +355,34 @@ int mkv_calibrate_gather(const mkv_cache* cc, int32_t layer, const int32_t* sel,
     MKV_CUDA(cudaSetDevice(c->desc.device));
     const size_t upd_off = (size_t)layer * g.n_units * g.L * kD;
     int n = 0;
-    MKV_CUDA(launch_attention(g, c->view(layer), c->q_dev, sel, sel_count, k_max, 1.f, c->out_dev, nullptr, c->attn,
-                              c->upd_k + upd_off, c->upd_v + upd_off, c->upd_cnt + layer, c->sm_count,
-                              (cudaStream_t)stream, &n, true));
+    MKV_CUDA(launch_attention(g, c->view(layer), c->q_dev, sel, sel_count, k_max, 1.f, c->out_dev, nullptr,
+                              c->attn_scratch(layer), c->upd_k + upd_off, c->upd_v + upd_off, c->upd_cnt + layer,
+                              c->dev_flags, c->sm_count, (cudaStream_t)stream, &n, true));
+    return MKV_OK;
+}
+
+int mkv_calibrate_stream(const mkv_cache* cc, int32_t layer, uint64_t bytes, void* stream) {
+    if (!cc) return fail(MKV_E_ARG, "mkv_calibrate_stream: NULL argument");
+    mkv_cache* c = const_cast<mkv_cache*>(cc);
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    if (bytes > c->slice_bytes) bytes = c->slice_bytes;
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(launch_stream_read(c->arena + (size_t)layer * c->slice_bytes, bytes, c->sm_count, c->sink, (cudaStream_t)stream));
+    return MKV_OK;
+}
+
+int mkv_attention_stats(const mkv_cache* c, uint64_t* blocks_host, uint64_t* v_blocks_host, uint64_t* v_bytes_host,
+                        int32_t reset) {
+    if (!c) return fail(MKV_E_ARG, "NULL cache");
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(cudaDeviceSynchronize());
+    unsigned long long st[8];
+    MKV_CUDA(cudaMemcpy(st, c->attn.stats, 64, cudaMemcpyDeviceToHost));
+    if (blocks_host) *blocks_host = st[0];
+    if (v_blocks_host) *v_blocks_host = st[1];
+    if (v_bytes_host) *v_bytes_host = st[2];
+    if (reset) MKV_CUDA(cudaMemset(c->attn.stats, 0, 64));
     return MKV_OK;
 }
 
@@ -524,8 +572,8 @@ int mkv_cache_status(const mkv_cache* c, uint32_t* flags_host) {
     uint32_t f = 0;
     MKV_CUDA(cudaMemcpy(&f, c->dev_flags, 4, cudaMemcpyDeviceToHost));
     if (flags_host) *flags_host = f;
-    if (f) return fail(MKV_E_DEVICE, "device flags 0x%x (%s%s)", f, (f & MKV_DEV_ARENA_OVERFLOW) ? "arena overflow " : "",
-                       (f & MKV_DEV_BAD_STRATEGY) ? "bad strategy" : "");
+    if (f) return fail(MKV_E_DEVICE, "device flags 0x%x (%s%s%s)", f, (f & MKV_DEV_ARENA_OVERFLOW) ? "arena overflow " : "",
+                       (f & MKV_DEV_BAD_STRATEGY) ? "bad strategy " : "", (f & MKV_DEV_SYNC_TIMEOUT) ? "attention sync timeout" : "");
     return MKV_OK;
 }
 

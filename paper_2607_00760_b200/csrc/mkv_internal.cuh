@@ -71,7 +71,7 @@ cudaError_t launch_strategy_quantile(const double* loss_k, const double* loss_v,
                                      int nseg, int n_dense, mkv_strategy sparse,
                                      mkv_strategy* out, cudaStream_t s);
 cudaError_t launch_strategy_threshold(const double* loss_k, const double* loss_v, int ncand,
-                                      long long n, const mkv_strategy* cands_dev, double tau,
+                                      long long n, const mkv_strategy* cands_host, double tau,
                                       mkv_strategy* out, cudaStream_t s);
 cudaError_t launch_compress(const CacheGeom& g, const LayerView& lv, const CompressArgs& a,
                             const mkv_strategy* strat, unsigned long long* call_base,
@@ -79,23 +79,65 @@ cudaError_t launch_compress(const CacheGeom& g, const LayerView& lv, const Compr
 
 cudaError_t launch_score(const CacheGeom& g, const LayerView& lv, const uint16_t* q, int reduce,
                          float* scores, int sm_count, cudaStream_t s);
+struct PlanRec;
 cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_t* q, int budget,
                           int reduce, int32_t* sel, int32_t* sel_count, int k_max, float* scores,
-                          uint32_t* cand_key, int32_t* cand_idx, int sm_count, cudaStream_t s, int* n_kernels);
+                          uint32_t* cand_key, int32_t* cand_idx, PlanRec* plan, int plan_stride, uint32_t tag,
+                          int sm_count, cudaStream_t s, int* n_kernels);
 constexpr int kTopkSlice = 16384;  // blocks per top-k slice (select.cu); longer units are selected in two stages
 
+// One selected token block as the attention kernel needs it: a cache of the table lookups
+// (strategy record + offset table) keyed by (layer, unit, position, first token).  mkv_select's top-k
+// writes one record per selected block next to `sel`; mkv_packed_attention uses a record only if its
+// tag and first token match the `sel` entry it reads (the packed arena is append-only, so a matching
+// record is valid whatever call wrote it) and falls back to the tables otherwise.
+struct __align__(16) PlanRec {
+    int32_t t0;      // first token of the block
+    uint32_t off16;  // payload offset in the layer slice, 16-B units
+    uint32_t meta;   // r_k | r_v << 8 | nb << 16   (nb = tokens in the block, 1..8)
+    uint32_t tag;    // plan_tag(generation, layer); 0 = never written
+};
+__host__ __device__ inline uint32_t plan_tag(uint32_t generation, int layer) {
+    return ((generation & 0xffffu) << 16) | ((uint32_t)layer & 0xffffu) | 0x80000000u;
+}
+#ifdef __CUDACC__
+// table lookup of the block that starts at token t0 of `unit`; meta = 0 if t0 is not a block start of the unit
+__device__ __forceinline__ void plan_lookup(const CacheGeom& g, const LayerView& lv, int unit, int t0, uint32_t& off16,
+                                            uint32_t& meta) {
+    off16 = 0u; meta = 0u;
+    if (t0 < 0 || t0 >= lv.unit_ntok[unit] || (t0 & (kB - 1)) != 0) return;
+    const int seg = t0 / g.L, in_seg = t0 - seg * g.L;
+    const size_t e = (size_t)unit * lv.S_max + seg;
+    const StratRec rec = lv.strat[e];
+    if ((int)rec.n_tok <= in_seg) return;
+    const uint32_t nb = (uint32_t)min(kB, (int)rec.n_tok - in_seg);
+    off16 = lv.tok_off[e] + (uint32_t)(in_seg >> 3) * (tokblock_bytes(rec.r_k, rec.r_v, kB) >> 4);
+    meta = (uint32_t)rec.r_k | ((uint32_t)rec.r_v << 8) | (nb << 16);
+}
+#endif
+
 struct AttnScratch {
-    float* part_o;    // [slots][G][D]   unnormalised partial outputs (<= 2 slots per warp and per CTA of the grid)
-    float* part_ml;   // [slots][8][2]   (running max in log2 units, sum)
-    int32_t* ticket;  // [n_units]       arrivals of the CTAs sharing a unit; zero between launches
+    float* part_o;        // [slots][G][D]   unnormalised partial outputs (<= 2 slots per warp and per CTA of the grid)
+    float* part_l;        // [slots][8]      partial softmax sums, all relative to the unit's global maximum
+    int32_t* ticket;      // [n_units]       arrivals of the CTAs sharing a unit (step 3d); zero between launches
+    uint32_t* umax;       // [n_units][8]    per (unit, head) maximum logit as an order-preserving key; zero between launches
+    int32_t* uarrive;     // [n_units]       CTAs that have published their maxima of a unit; zero between launches
+    float* zbuf;          // [z_cap][8 G]    logits of blocks that do not fit a warp's shared-memory cache
+    unsigned long long* stats;  // [8]       counters of mkv_attention_stats
+    PlanRec* plan;        // [n_units][plan_stride] of this layer (may be nullptr)
+    int32_t plan_stride;
+    uint32_t plan_tag;
     int32_t slots;
 };
 int attention_partial_slots(int sm_count);
+size_t attention_zbuf_floats(const CacheGeom& g);
 cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q,
                              const int32_t* sel, const int32_t* sel_count, int k_max, float scale,
                              float* out, float* lse, const AttnScratch& scr, const uint16_t* upd_k,
-                             const uint16_t* upd_v, const int32_t* upd_count, int sm_count, cudaStream_t s,
-                             int* n_kernels, bool gather_only = false);
+                             const uint16_t* upd_v, const int32_t* upd_count, uint32_t* dev_flags, int sm_count,
+                             cudaStream_t s, int* n_kernels, bool gather_only = false);
+cudaError_t launch_stream_read(const uint8_t* base, unsigned long long bytes, int sm_count, unsigned long long* sink,
+                               cudaStream_t s);
 // KV update buffer: copy n_new raw tokens of every unit into rows [n_have, n_have + n_new)
 // and set the layer's device-side count to n_have + n_new
 cudaError_t launch_update_copy(const CacheGeom& g, const CompressArgs& a, uint16_t* upd_k, uint16_t* upd_v,

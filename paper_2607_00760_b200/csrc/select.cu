@@ -47,7 +47,8 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
                                                         int budget, int32_t* __restrict__ sel,
                                                         int32_t* __restrict__ sel_count, int k_max,
                                                         uint32_t* __restrict__ cand_key, int32_t* __restrict__ cand_idx,
-                                                        int n_slices, int cand_cap) {
+                                                        int n_slices, int cand_cap, PlanRec* __restrict__ plan,
+                                                        int plan_stride, uint32_t tag) {
     const int unit = MODE == 1 ? blockIdx.x / n_slices : blockIdx.x;
     const int slice = MODE == 1 ? blockIdx.x % n_slices : 0;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -246,7 +247,16 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
             const int pos = gt_before + min(eq_before, take_eq);
             if (take && pos < cap) {
                 if (MODE == 1) { okey[pos] = all ? keyat(i) : u; oidx[pos] = idxat(i); }
-                else out[pos] = idxat(i) * kB;
+                else {
+                    const int t0 = idxat(i) * kB;
+                    out[pos] = t0;
+                    if (plan != nullptr && pos < plan_stride) {  // what mkv_packed_attention needs to know about the block
+                        PlanRec pr;
+                        pr.t0 = t0; pr.tag = tag;
+                        plan_lookup(g, lv, unit, t0, pr.off16, pr.meta);
+                        plan[(size_t)unit * plan_stride + pos] = pr;
+                    }
+                }
             }
             gt_before += gt ? 1 : 0;
             eq_before += eq ? 1 : 0;
@@ -272,22 +282,23 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
 
 cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_t* q, int budget, int reduce,
                           int32_t* sel, int32_t* sel_count, int k_max, float* scores, uint32_t* cand_key,
-                          int32_t* cand_idx, int sm_count, cudaStream_t s, int* n_kernels) {
+                          int32_t* cand_idx, PlanRec* plan, int plan_stride, uint32_t tag, int sm_count, cudaStream_t s,
+                          int* n_kernels) {
     cudaError_t err = launch_score(g, lv, q, reduce, scores, sm_count, s);
     if (err != cudaSuccess) return err;
     const int n_slices = (g.score_stride + kKeyCap - 1) / kKeyCap;
     const int cand_cap = budget / kB + 1 < kKeyCap ? budget / kB + 1 : kKeyCap;  // candidates kept per slice
     if (n_slices == 1) {
         err = launch_pdl(mkv_topk_kernel<0>, dim3(g.n_units), dim3(1024), 0, s, g, lv, (const float*)scores, budget, sel,
-                         sel_count, k_max, (uint32_t*)nullptr, (int32_t*)nullptr, 1, 0);
+                         sel_count, k_max, (uint32_t*)nullptr, (int32_t*)nullptr, 1, 0, plan, plan_stride, tag);
         if (err != cudaSuccess) return err;
         if (n_kernels) *n_kernels = 2;
     } else {
         err = launch_pdl(mkv_topk_kernel<1>, dim3(g.n_units * n_slices), dim3(1024), 0, s, g, lv, (const float*)scores, budget,
-                         sel, sel_count, k_max, cand_key, cand_idx, n_slices, cand_cap);
+                         sel, sel_count, k_max, cand_key, cand_idx, n_slices, cand_cap, (PlanRec*)nullptr, 0, 0u);
         if (err != cudaSuccess) return err;
         err = launch_pdl(mkv_topk_kernel<2>, dim3(g.n_units), dim3(1024), 0, s, g, lv, (const float*)scores, budget, sel,
-                         sel_count, k_max, cand_key, cand_idx, n_slices, cand_cap);
+                         sel_count, k_max, cand_key, cand_idx, n_slices, cand_cap, plan, plan_stride, tag);
         if (err != cudaSuccess) return err;
         if (n_kernels) *n_kernels = 3;
     }

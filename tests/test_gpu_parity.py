@@ -462,6 +462,99 @@ def test_attention_peaked_softmax(env):
         c.free()
 
 
+def test_attention_flat_softmax_nothing_skipped(env):
+    """q = 0: every probability is equal, so phase 2 may skip no block (the deferred-PV rule drops a block only if
+    all its probabilities are < 2^-40 of the unit's largest); the counters must say every V part was fetched.
+    Beside it the peaked case: one key scaled up carries the mass, most V parts are skipped, the result still
+    matches the oracle (which skips nothing)."""
+    mkv, dev = env
+    from paper_2607_00760_b200 import synth
+    c = Case(mkv, dev, 2, 2, 8, 64 * 40 + 13, seed=91)
+    try:
+        c.q[:] = 0
+        c.q_d = to_dev(c.q, dev)
+        strat = uniform_strat(2, 2, c.S, 38)
+        strat[:, :, 1::4, 0:2] = 128
+        c.compress(strat)
+        sel, cnt = c.oracle_sel(1024)
+        c.cache.attention_stats(reset=True)
+        out, ref = c.check_attention(sel, cnt)
+        st = c.cache.attention_stats(reset=True)
+        assert st["blocks"] == int(cnt.sum()) and st["v_blocks"] == st["blocks"], st
+        # flat weights: the output is the plain mean of the masked V rows
+        assert np.abs(out - ref).max() < 1e-5
+        # peaked: q = 6 x one key
+        kf = synth.bf16_bits_to_f32(c.K[0, 0, 777])
+        c.q[:] = synth.f32_to_bf16_bits(kf * 6.0)
+        c.q_d = to_dev(c.q, dev)
+        sel, cnt = c.oracle_sel(1024)
+        c.check_attention(sel, cnt)
+        st = c.cache.attention_stats(reset=True)
+        assert st["blocks"] == int(cnt.sum()) and 0 < st["v_blocks"] < st["blocks"], st
+    finally:
+        c.free()
+
+
+def test_attention_verifies_the_plan_against_sel(env):
+    """mkv_select leaves one record per selected block for mkv_packed_attention; the attention kernel must use a
+    record only where it matches the `sel` it is given: (i) the caller edits `sel` after mkv_select (other blocks,
+    other order, other counts, other k_max), (ii) two layers are selected before either is attended, (iii) the cache
+    is reset and refilled with different strategies (stale records of the old generation)."""
+    mkv, dev = env
+    import torch
+    c = Case(mkv, dev, 2, 2, 8, 64 * 20 + 5, seed=93, n_layers=2)
+    try:
+        strat = uniform_strat(2, 2, c.S, 38)
+        strat[:, :, ::3, 0:2] = 128
+        for layer in (0, 1):
+            c.compress(strat, layer=layer)
+        gsel, gcnt, _ = c.gpu_select(512, layer=0)
+        gsel1, gcnt1, _ = c.gpu_select(256, layer=1)      # (ii) layer 1 selected before layer 0 is attended
+        c.check_attention(gsel, gcnt, layer=0)
+        c.check_attention(gsel1, gcnt1, layer=1)
+        rng = np.random.default_rng(5)
+        nblk = (c.N + 7) // 8
+        sel = gsel.copy()
+        cnt = gcnt.copy()
+        for b in range(2):                                # (i) edited after select
+            for h in range(2):
+                n = cnt[b, h]
+                sel[b, h, :n] = rng.permutation(sel[b, h, :n])
+                sel[b, h, ::5] = rng.integers(0, nblk, size=len(sel[b, h, ::5])) * 8
+        cnt[1, 1] = 3
+        c.check_attention(sel, cnt, layer=0)
+        wide = np.full((2, 2, sel.shape[2] + 7), -1, np.int32)
+        wide[:, :, :sel.shape[2]] = sel                    # another k_max: positions no longer line up with the records
+        c.check_attention(wide, cnt, layer=0)
+        c.cache.reset()                                    # (iii)
+        strat2 = uniform_strat(2, 2, c.S, 64, 90)
+        for layer in (0, 1):
+            c.compress(strat2, layer=layer)
+        c.check_attention(gsel, gcnt, layer=0)
+    finally:
+        c.free()
+
+
+@pytest.mark.parametrize("r_k,r_v", [(127, 127), (128, 124), (121, 128), (120, 120), (124, 3)])
+def test_attention_largest_packed_blocks(env, r_k, r_v):
+    """packed vectors with r in [121, 127] are LARGER than dense ones (bitmap + values): a token block's K part or V
+    part then exceeds half a staging group, so such blocks are attended one per group (the old 4096-byte
+    stage overran at r_k + r_v > 240)."""
+    mkv, dev = env
+    c = Case(mkv, dev, 1, 2, 8, 64 * 6 + 3, seed=95)
+    try:
+        strat = uniform_strat(1, 2, c.S, r_k, r_v)
+        strat[:, :, 2] = (38, 38, 1, 8)
+        c.compress(strat)
+        c.assert_export_equal()
+        total, swaps = c.check_select(128)
+        assert swaps == 0
+        sel, cnt = c.oracle_sel(c.N)
+        c.check_attention(sel, cnt)
+    finally:
+        c.free()
+
+
 # ------------------------------------------------------------------ multi-layer, host call, errors
 
 def test_layers_are_independent_and_decode_host_matches(env):
