@@ -3,29 +3,30 @@
 //
 // Design: one launch, two phases, one CTA per SM.
 //   * The selected blocks of all units form one stream of T blocks; it is cut into equal ranges,
-//     one per warp (warps are independent inside a phase).  A warp walks its range in groups of
+//     one per warp (warps never meet before the combine).  A warp walks its range in groups of
 //     <= 2 token blocks (16 tokens = the M of one mma tile).  What a block is (payload offset,
 //     tokens, r_k, r_v) comes from the plan record mkv_select wrote next to `sel`, verified against
 //     the `sel` entry; a record that does not match is replaced by the table lookup.
-//   * Staging: a block's K part and its V part are contiguous 16-B-aligned chunks (DESIGN.md
-//     format); one lane moves a chunk into the warp's shared-memory ring with ONE 1-D bulk copy
-//     (cp.async.bulk, the TMA engine) that completes on the slot's mbarrier.  The ring is
-//     byte-granular (a group takes what it needs), up to kSlots groups are in flight per warp.
+//   * Staging: a block's K part and its V part are contiguous chunks (DESIGN.md format); one lane
+//     moves a chunk into the warp's shared-memory ring with ONE 1-D bulk copy (cp.async.bulk, the
+//     TMA engine) that completes on the slot's mbarrier.  The ring is byte-granular (a group takes
+//     what it needs); up to kSlots groups are in flight per warp.
 //   * Phase 1 (QK): S = K q^T with the group's 16 tokens = M, heads = N, channels = K; packed
 //     vectors are expanded straight into mma.sync fragments (mkv_walk.cuh).  The scaled logits go
-//     to the warp's logit cache (shared memory; global scratch beyond its capacity) and the
-//     per-(unit, head) maximum to global memory with one atomic max per warp, unit and head.
-//   * Between the phases the CTAs that share a unit meet at a per-unit arrival counter; after it
-//     every warp knows the unit's exact maximum M, so all probabilities are 2^(z - M), no partial
-//     result is ever rescaled, and partial results of one unit simply add.
-//   * Phase 2 (PV, deferred): the softmax sum runs over every selected token; the V part of a block
-//     is fetched and walked only if one of its probabilities is >= 2^-40 (error bound).
-//     O^T = V^T P^T with channels = M, heads = N, the group's 16 tokens = K; P is split into bf16
-//     hi + lo (fp32-class accuracy).  Dense vectors (r = D) skip the walk.
+//     to the warp's logit cache (shared memory; global scratch beyond its capacity).  At the end of
+//     a unit the warp publishes its per-head maxima (atomic max) and arrives at the unit's counter.
+//   * Phase 2 (PV, deferred) starts per unit when every warp that holds a part of it has arrived:
+//     the warp then knows the unit's exact maximum M, so all probabilities are 2^(z - M), nothing
+//     is ever rescaled, and partial results of one unit simply add.  The softmax sum runs over
+//     every selected token; the V part of a block is fetched and walked only if one of its
+//     probabilities is >= 2^-40 (error bound).  O^T = V^T P^T with channels = M,
+//     heads = N, the group's 16 tokens = K; P is split into bf16 hi + lo (fp32-class accuracy).
+//     Dense vectors (r = D) skip the walk.
 //   * Step 3d (split-K combine) is fused: a unit wholly inside one warp's range is normalised and
 //     written directly; otherwise the warp leaves an (l, O) partial (<= 2 per warp), the threads of
 //     the CTA add the partials of a unit (four output channels each), and a unit that spans several
-//     CTAs is finished by the last CTA to arrive at a per-unit ticket (no second kernel).
+//     CTAs is finished, four channels at a time, by the last thread to arrive at a per-(unit,
+//     channel quad) ticket (no second kernel, no barrier after the fold).
 #include "mkv_internal.cuh"
 #include "mkv_walk.cuh"
 
@@ -40,19 +41,22 @@ constexpr float kLn2 = 0.6931471805599453f;
 constexpr int kWarps = 16;         // warps per CTA (one CTA per SM)
 constexpr int kRingBytes = 8192;   // per-warp staging ring: two dense groups or five groups at r = 38
 constexpr int kSlots = 8;          // groups in flight per warp (one mbarrier each)
-constexpr int kGroupMax = 4096;    // largest group: two dense K (or V) parts
-constexpr int kDescRing = 64;      // group descriptors kept per warp
+constexpr int kGroupMax16 = 256;   // largest group in 16-B units: two dense K (or V) parts
+constexpr int kDesc = 32;          // group descriptors kept per warp and phase
+constexpr int kDescribe = 24;      // blocks described per call: kDescribe + kSlots <= kDesc
 constexpr int kZBytes = 4096;      // per-warp logit cache: 32 blocks at G = 4
 constexpr int kMaxUnitsSmem = 2048;
 constexpr float kSkip = 40.f;      // a block whose probabilities are all < 2^-40 is not walked in phase 2
 constexpr int kSpinLimit = 1 << 22;
 
-// One group of the stream: <= 2 consecutive selected token blocks of one unit with the same
-// strategy whose K parts and V parts each fit kGroupMax.
+// One group of the stream: <= 2 consecutive selected token blocks of one unit with the same strategy whose K
+// parts and V parts each fit kGroupMax16.  Every size the hot loops need is worked out once, by the describing lane.
 struct __align__(16) GDesc {
-    uint32_t off0, off1;  // payload offsets in the layer slice (update buffer: row offsets), 16-B units
-    uint32_t a;           // unit | r_k << 16 | r_v << 24
-    uint32_t b;           // nb0 | nb1 << 4 | upd << 8 | pos << 9   (nb0 = 0: invalid entry; pos: block 0's index in the warp's range)
+    // phase 1 (K parts)                                     phase 2 (V parts)
+    uint32_t off0, off1;  // chunk offsets, 16-B units       first 16-B unit of each V part
+    uint32_t x;           // kc0 | kc1 << 8 | nb0 << 16      vc0 | vc1 << 8 | skew0 << 16 | skew1 << 20 | r_v << 24
+                          //   | nb1 << 20 | r_k << 24         (chunk sizes in 16-B units; skew: bytes before the V part)
+    uint32_t y;           // unit | upd << 16                 unit | upd << 16 | nb0 << 20 | nb1 << 24
 };
 
 __device__ __forceinline__ unsigned lanemask_le() {
@@ -84,31 +88,14 @@ __device__ __forceinline__ int ld_acquire(const int32_t* p) {
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-
-// prefix sums of the clamped selection counts -> s_cum[0..n_units]; returns the total T
-__device__ __forceinline__ int scan_counts(const int32_t* __restrict__ sel_count, int n_units, int k_max, int extra,
-                                            int* s_cum) {
-    __shared__ int s_carry;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (warp == 0) {
-        int carry = 0;
-#pragma unroll 1
-        for (int i0 = 0; i0 < n_units; i0 += 32) {
-            const int i = i0 + lane;
-            int c = (i < n_units) ? min(max(sel_count[i], 0), k_max) + extra : 0;  // + blocks of the update buffer
-            int inc = c;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int v = __shfl_up_sync(kFull, inc, o);
-                if (lane >= o) inc += v;
-            }
-            if (i < n_units) s_cum[i] = carry + inc - c;
-            carry += __shfl_sync(kFull, inc, 31);
-        }
-        if (lane == 0) { s_cum[n_units] = carry; s_carry = carry; }
-    }
-    __syncthreads();
-    return s_carry;
+__device__ __forceinline__ void red_release_add(int32_t* p, int v) {
+    asm volatile("red.release.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void sts_f32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ float2 lds_f32x2(uint32_t a) {
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a));
+    return v;
 }
 
 // largest u with s_cum[u] <= i (i < T guaranteed; zero-count units are skipped by construction)
@@ -122,8 +109,10 @@ __device__ __forceinline__ int find_unit(const int* s_cum, int n_units, int i) {
     return lo;
 }
 
-// per warp: staging ring | group descriptors | logit cache | slot table (offset, bytes) | mbarriers | phase-2 slot groups
-constexpr int kWS = kRingBytes + kDescRing * 16 + kZBytes + kSlots * 8 + kSlots * 8 + kSlots * 16;
+// per warp: staging ring | phase-1 descriptors | phase-2 descriptors | logit cache | slot table (offset, bytes) |
+// mbarriers | groups in flight in phase 2
+constexpr int kOffD1 = kRingBytes, kOffD2 = kOffD1 + kDesc * 16, kOffZ = kOffD2 + kDesc * 16, kOffSlot = kOffZ + kZBytes;
+constexpr int kOffBar = kOffSlot + kSlots * 8, kOffGrp = kOffBar + kSlots * 8, kWS = kOffGrp + kSlots * 16;
 
 // Even split of n items over p parts: part i owns [i b + min(i, r), ...) with b = n / p, r = n % p
 // (the first r parts hold one more).  One runtime division per level.
@@ -158,16 +147,15 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
 
     __shared__ int s_unit[kRec];                              // unit of each partial record, -1 = none
     __shared__ __align__(8) float s_ml[kRec][kMaxGroup][2];   // its (global max in log2 units, sum) per head
-    __shared__ int s_last[2], s_cf[2], s_cl[2];
-    __shared__ size_t s_row[2];
 
     uint8_t* wbase = smem + warp * kWS;
     const uint32_t ring0 = smem_u32(wbase);
-    GDesc* ring = reinterpret_cast<GDesc*>(wbase + kRingBytes);
-    float* zs = reinterpret_cast<float*>(wbase + kRingBytes + kDescRing * 16);
-    uint2* slot_tab = reinterpret_cast<uint2*>(wbase + kRingBytes + kDescRing * 16 + kZBytes);
-    const uint32_t bar0 = ring0 + kRingBytes + kDescRing * 16 + kZBytes + kSlots * 8;
-    GDesc* slot_grp = reinterpret_cast<GDesc*>(wbase + kRingBytes + kDescRing * 16 + kZBytes + kSlots * 16);
+    GDesc* d1 = reinterpret_cast<GDesc*>(wbase + kOffD1);
+    GDesc* d2 = reinterpret_cast<GDesc*>(wbase + kOffD2);
+    const uint32_t zs0 = ring0 + kOffZ;
+    uint2* slot_tab = reinterpret_cast<uint2*>(wbase + kOffSlot);
+    const uint32_t bar0 = ring0 + kOffBar;
+    GDesc* slot_grp = reinterpret_cast<GDesc*>(wbase + kOffGrp);
     if (lane == 0) {
 #pragma unroll
         for (int s = 0; s < kSlots; ++s) mbar_init(bar0 + 8 * s, 1);
@@ -178,9 +166,28 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     pdl_launch_dependents();  // the next kernel may be scheduled as SMs free up
 
     // tokens in the layer's update buffer: device-resident, so a captured graph stays valid across appends
-    const int n_buf = min(max(*upd_count, 0), g.L);
+    const int n_buf = min(max(__ldg(upd_count), 0), g.L);
     const int upd_blocks = (n_buf + kB - 1) / kB;  // every unit ends with the blocks of its update buffer
-    const int T = scan_counts(sel_count, g.n_units, k_max, upd_blocks, s_cum);  // (block barrier inside)
+    // Prefix sums of the clamped selection counts -> s_cum[0 .. n_units].  Every warp runs the scan itself
+    // and writes the same values: no warp waits for another one before its first copy is in flight.
+    int T = 0;
+    {
+#pragma unroll 1
+        for (int i0 = 0; i0 < g.n_units; i0 += 32) {
+            const int i = i0 + lane;
+            const int c = (i < g.n_units) ? min(max(__ldg(sel_count + i), 0), k_max) + upd_blocks : 0;
+            int inc = c;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int v = __shfl_up_sync(kFull, inc, o);
+                if (lane >= o) inc += v;
+            }
+            if (i < g.n_units) s_cum[i] = T + inc - c;
+            T += __shfl_sync(kFull, inc, 31);
+        }
+        if (lane == 0) s_cum[g.n_units] = T;
+        __syncwarp();
+    }
     // The stream is split in units of two positions, so every range starts at an even position: with even
     // selection counts (units then start at even positions too) a range never holds two odd runs, which
     // would cost an extra half-empty group -- the slowest warp sets the kernel's time.
@@ -198,7 +205,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     const unsigned gw = blockIdx.x * kWarps + warp;
     const int n_total = hi - lo;
     const int G = g.group;
-    const int zcap = kZBytes / (32 * G);  // blocks of the range whose logits stay in shared memory
+    const uint32_t zstride = 32u * (uint32_t)G;         // bytes of one block's logits: [head][token] floats
+    const int zcap = kZBytes / (int)zstride;            // blocks of the range whose logits stay in shared memory
     if (blockIdx.x == 0 && !kGatherOnly) {  // units with an empty selection: out = 0, lse = -inf
 #pragma unroll 1
         for (int u = warp; u < g.n_units; u += kWarps) {
@@ -209,23 +217,37 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             if (lse != nullptr && lane < G) lse[row + lane] = -INFINITY;
         }
     }
-    // logits of block i of the range: [head][token], 8 G floats
-    auto zptr = [&](int i) -> float* {
-        return i < zcap ? zs + i * (8 * G) : scr.zbuf + (size_t)(lo + i) * (size_t)(8 * G);
+    // the number of warps of the grid whose ranges meet positions [a, b) (a < b): what a unit's arrival counter reaches
+    auto warps_meeting = [&](int a, int b) -> int {
+        const unsigned pa = (unsigned)a >> 1, pb = ((unsigned)b - 1u) >> 1;
+        const unsigned cf = cs.owner(pa), cl = cs.owner(pb);
+        auto in_cta = [&](unsigned c, unsigned p_lo, unsigned p_hi) -> int {  // pairs p_lo..p_hi all lie in CTA c
+            const unsigned c0 = cs.begin(c), n = cs.begin(c + 1) - c0;
+            Split w;
+            w.b = n / kWarps; w.r = n % kWarps;
+            return (int)w.owner(p_hi - c0) - (int)w.owner(p_lo - c0) + 1;
+        };
+        if (cf == cl) return in_cta(cf, pa, pb);
+        int n = in_cta(cf, pa, cs.begin(cf + 1) - 1u) + in_cta(cl, cs.begin(cl), pb);
+#pragma unroll 1
+        for (unsigned c = cf + 1; c < cl; ++c) n += (int)min((unsigned)kWarps, cs.begin(c + 1) - cs.begin(c));
+        return n;
     };
 
-    int bbuilt = 0, gbuilt = 0;  // blocks / groups described so far (per phase)
+    int bbuilt = 0, gbuilt = 0;  // blocks / groups described so far
+    int ucur = n_total > 0 ? find_unit(s_cum, g.n_units, lo) : 0;  // unit of the first block not yet described (warp-uniform)
 
-    // Describe the next <= 32 blocks of the range (one per lane) and pair them into groups: block i
-    // follows block i - 1 in a group if both belong to one unit, have the same strategy and their K
-    // parts and V parts fit one group; runs of such blocks are paired greedily from their start.
-    // A pure function of the inputs: phase 2 describes the range again and gets the same groups.
+    // Describe the next <= kDescribe blocks of the range (one per lane) and pair them into groups: block i
+    // follows block i - 1 in a group if both belong to one unit, have the same strategy and their K parts
+    // and V parts fit one group; runs of such blocks are paired greedily from their start.
+    // A pure function of the inputs: when phase 2 has to describe a long range again it gets the same groups.
     auto describe = [&](int count) {
         uint32_t off16 = 0u, meta = 0u, updf = 0u;
-        int u = -1;
+        int u = ucur;
         if (lane < count) {
             const int gi = lo + bbuilt + lane;
-            u = find_unit(s_cum, g.n_units, gi);
+#pragma unroll 1
+            while (gi >= s_cum[u + 1]) ++u;
             const int j = gi - s_cum[u], jb = j - (s_cum[u + 1] - s_cum[u] - upd_blocks);
             if (jb >= 0) {  // block jb of the unit's update buffer: raw rows [u][8 jb ..][128] of upd_k / upd_v
                 const uint32_t nb = (uint32_t)min(kB, n_buf - kB * jb);
@@ -233,24 +255,29 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 meta = (uint32_t)kD | ((uint32_t)kD << 8) | (nb << 16);
                 updf = 1u;
             } else {
-                const int t0 = sel[(size_t)u * k_max + j];
+                const int t0 = __ldg(sel + (size_t)u * k_max + j);
                 PlanRec pr;
                 pr.t0 = -1; pr.off16 = 0u; pr.meta = 0u; pr.tag = 0u;
-                if (scr.plan != nullptr && j < scr.plan_stride)
-                    pr = *reinterpret_cast<const PlanRec*>(
-                        __builtin_assume_aligned(scr.plan + (size_t)u * scr.plan_stride + j, 16));
+                if (scr.plan != nullptr && j < scr.plan_stride) {
+                    const uint4 v = __ldg(reinterpret_cast<const uint4*>(scr.plan + (size_t)u * scr.plan_stride + j));
+                    pr.t0 = (int32_t)v.x; pr.off16 = v.y; pr.meta = v.z; pr.tag = v.w;
+                }
                 if (pr.tag == scr.plan_tag && pr.t0 == t0 && t0 >= 0) { off16 = pr.off16; meta = pr.meta; }
                 else plan_lookup(g, lv, u, t0, off16, meta);
             }
         }
+        ucur = __shfl_sync(kFull, u, max(count - 1, 0));
+        if (lane >= count) u = -1;
         const uint32_t nb = meta >> 16, rk = meta & 255u, rv = (meta >> 8) & 255u;
-        const uint32_t kb = nb * vecb(rk), vb = nb * vecb(rv);
-        const uint32_t kc = pad16u(kb), vc = pad16u((kb & 15u) + vb);  // bytes staged in phase 1 / phase 2
+        const uint32_t kb = nb * vecb(rk);                      // bytes of the K part
+        const uint32_t sk = updf ? 0u : (kb & 15u);             // bytes between the last 16-B boundary and the V part
+        const uint32_t kc = (kb + 15u) >> 4, vc = (sk + nb * vecb(rv) + 15u) >> 4;  // 16-B units staged in phase 1 / 2
+        const uint32_t voff = updf ? off16 : off16 + (kb >> 4);
         const int pu = __shfl_up_sync(kFull, u, 1);
         const uint32_t pmeta = __shfl_up_sync(kFull, meta, 1), pkc = __shfl_up_sync(kFull, kc, 1);
         const uint32_t pvc = __shfl_up_sync(kFull, vc, 1), pupd = __shfl_up_sync(kFull, updf, 1);
         const bool follows = lane > 0 && lane < count && u == pu && ((meta ^ pmeta) & 0xffffu) == 0u && nb != 0u &&
-                             (pmeta >> 16) != 0u && kc + pkc <= (uint32_t)kGroupMax && vc + pvc <= (uint32_t)kGroupMax &&
+                             (pmeta >> 16) != 0u && kc + pkc <= (uint32_t)kGroupMax16 && vc + pvc <= (uint32_t)kGroupMax16 &&
                              !updf && !pupd;
         const unsigned fm = __ballot_sync(kFull, follows);
         const int start = 31 - __clz((int)(~fm & lanemask_le()));  // first block of this lane's run (bit 0 of ~fm is set)
@@ -258,12 +285,19 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         const bool two = first && ((fm >> 1) >> lane & 1u);        // lane + 1 follows (and is therefore < count)
         const unsigned gm = __ballot_sync(kFull, first);
         const uint32_t off1 = __shfl_down_sync(kFull, off16, 1), nb1 = __shfl_down_sync(kFull, nb, 1);
+        const uint32_t kc1 = __shfl_down_sync(kFull, kc, 1), vc1 = __shfl_down_sync(kFull, vc, 1);
+        const uint32_t voff1 = __shfl_down_sync(kFull, voff, 1), sk1 = __shfl_down_sync(kFull, sk, 1);
         if (first) {
-            GDesc d;
-            d.off0 = off16; d.off1 = two ? off1 : 0u;
-            d.a = (uint32_t)u | (rk << 16) | (rv << 24);
-            d.b = nb | ((two ? nb1 : 0u) << 4) | (updf << 8) | ((uint32_t)(bbuilt + lane) << 9);
-            ring[(gbuilt + __popc(gm & lanemask_lt())) & (kDescRing - 1)] = d;
+            const int slot = (gbuilt + __popc(gm & lanemask_lt())) & (kDesc - 1);
+            GDesc a, b;
+            a.off0 = off16; a.off1 = two ? off1 : 0u;
+            a.x = kc | ((two ? kc1 : 0u) << 8) | (nb << 16) | ((two ? nb1 : 0u) << 20) | (rk << 24);
+            a.y = (uint32_t)u | (updf << 16);
+            b.off0 = voff; b.off1 = two ? voff1 : 0u;
+            b.x = vc | ((two ? vc1 : 0u) << 8) | (sk << 16) | ((two ? sk1 : 0u) << 20) | (rv << 24);
+            b.y = (uint32_t)u | (updf << 16) | (nb << 20) | ((two ? nb1 : 0u) << 24);
+            d1[slot] = a;
+            d2[slot] = b;
         }
         gbuilt += __popc(gm);
         bbuilt += count;
@@ -274,7 +308,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     uint32_t rhead = 0u, rused = 0u, parbits = 0u;
     int pend = 0, si = 0, sc = 0;
     const unsigned long long slice = reinterpret_cast<unsigned long long>(lv.slice);
-    // claim `sz` bytes (a multiple of 16, <= kGroupMax) for the next group; false: no room yet
+    // claim `sz` bytes (a multiple of 16, <= 4096) for the next group; false: no room yet
     auto ring_alloc = [&](uint32_t sz, uint32_t& off) -> bool {
         uint32_t need = sz, h = pend == 0 ? 0u : rhead;  // an idle ring restarts at its beginning
         if (h + sz > (uint32_t)kRingBytes) { need += (uint32_t)kRingBytes - h; h = 0u; }  // wrap: the tail stays unused
@@ -285,16 +319,16 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         if (lane == 0) slot_tab[si] = make_uint2(h, need);
         return true;
     };
+    auto ring_commit = [&]() {
+        si = (si + 1) & (kSlots - 1);
+        ++pend;
+        __syncwarp();  // the slot table entry is visible to the whole warp
+    };
     auto ring_release = [&]() {  // the oldest group has been consumed
         rused -= slot_tab[sc].y;
         parbits ^= 1u << sc;
         sc = (sc + 1) & (kSlots - 1);
         --pend;
-    };
-    auto ring_commit = [&]() {
-        si = (si + 1) & (kSlots - 1);
-        ++pend;
-        __syncwarp();  // the slot table entry is visible to the whole warp
     };
 
     // =====================================================================================
@@ -304,52 +338,66 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     float mxA = -INFINITY, mxB = -INFINITY;  // this lane's maxima for heads 2qq, 2qq+1 of the current unit
     int cur_unit = -1;
     uint32_t calib = 0u;
+    // this lane's slots inside a block's logits ([head][token] floats): phase 1 writes token gq of heads 2qq, 2qq+1;
+    // phase 2 reads tokens 2qq, 2qq+1 of head gq
+    const uint32_t zw = (uint32_t)(16 * qq + gq) * 4u, zr = (uint32_t)(8 * gq + 2 * qq) * 4u;
 
-    auto publish_max = [&]() {  // the warp's maxima of cur_unit: one atomic max per head
+    // The warp has seen every block it holds of cur_unit: publish its maxima (one atomic max per head) and arrive
+    // at the unit's counter.  One lane issues everything, so the release of the arrival covers the maxima.
+    auto publish_max = [&]() {
 #pragma unroll
         for (int o = 4; o < 32; o <<= 1) {
             mxA = fmaxf(mxA, __shfl_xor_sync(kFull, mxA, o));
             mxB = fmaxf(mxB, __shfl_xor_sync(kFull, mxB, o));
         }
-        if (gq == 0) {
-            if (2 * qq < G) atomicMax(scr.umax + (size_t)cur_unit * kMaxGroup + 2 * qq, fkey(mxA));
-            if (2 * qq + 1 < G) atomicMax(scr.umax + (size_t)cur_unit * kMaxGroup + 2 * qq + 1, fkey(mxB));
+        // lanes 0..3 hold heads 2qq, 2qq+1: bring them to lane 0
+        float m[kMaxGroup];
+#pragma unroll
+        for (int h = 0; h < kMaxGroup / 2; ++h) {
+            m[2 * h] = __shfl_sync(kFull, mxA, h);
+            m[2 * h + 1] = __shfl_sync(kFull, mxB, h);
+        }
+        if (lane == 0) {
+            uint32_t* um = scr.umax + (size_t)cur_unit * kMaxGroup;
+#pragma unroll
+            for (int h = 0; h < kMaxGroup; ++h)
+                if (h < G) atomicMax(um + h, fkey(m[h]));
+            red_release_add(scr.uarrive + cur_unit, 1);
         }
     };
 
-    {
-        int bposi = 0, gposi = 0, bposc = 0, gposc = 0;
+    if (n_total > 0) {
+        int bposi = 0, gposi = 0, gposc = 0, bposc = 0;
 #pragma unroll 1
         for (;;) {
             // ---- issue: K parts of the next groups while the ring has room
 #pragma unroll 1
             while (bposi < n_total) {
-                if (gposi == gbuilt) describe(min(32, n_total - bbuilt));
-                const GDesc d = ring[gposi & (kDescRing - 1)];
-                const uint32_t nb0 = d.b & 15u, nb1 = (d.b >> 4) & 15u, rk = (d.a >> 16) & 255u;
-                const uint32_t c0 = pad16u(nb0 * vecb(rk)), c1 = pad16u(nb1 * vecb(rk));
+                if (gposi == gbuilt) describe(min(kDescribe, n_total - bbuilt));
+                const GDesc d = d1[gposi & (kDesc - 1)];
+                const uint32_t c0 = (d.x & 255u) << 4, c1 = ((d.x >> 8) & 255u) << 4;
                 uint32_t off;
                 if (!ring_alloc(c0 + c1, off)) break;
                 if (lane == 0) {
                     const uint32_t bar = bar0 + 8 * si, dst = ring0 + off;
-                    const unsigned long long src = (d.b & 256u) ? reinterpret_cast<unsigned long long>(upd_k) : slice;
+                    const unsigned long long src = (d.y & 0x10000u) ? reinterpret_cast<unsigned long long>(upd_k) : slice;
                     mbar_expect_tx(bar, c0 + c1);
                     if (c0) bulk_g2s(dst, src + ((unsigned long long)d.off0 << 4), c0, bar);
                     if (c1) bulk_g2s(dst + c0, src + ((unsigned long long)d.off1 << 4), c1, bar);
                 }
                 ring_commit();
                 ++gposi;
-                bposi += nb1 ? 2 : 1;
+                bposi += c1 ? 2 : 1;
             }
             if (pend == 0) break;  // nothing in flight and nothing left to issue
 
             // ---- consume the oldest group
-            const GDesc d = ring[gposc & (kDescRing - 1)];
-            const int u = (int)(d.a & 0xffffu);
-            const int r_k = (int)((d.a >> 16) & 255u);
-            const int nb0 = (int)(d.b & 15u), nb1 = (int)((d.b >> 4) & 15u), pos = (int)(d.b >> 9);
+            const GDesc d = d1[gposc & (kDesc - 1)];
+            const int u = (int)(d.y & 0xffffu);
+            const int r_k = (int)(d.x >> 24);
+            const int nb0 = (int)((d.x >> 16) & 15u), nb1 = (int)((d.x >> 20) & 15u);
             const bool two = nb1 != 0;
-            const uint32_t sp0 = ring0 + slot_tab[sc].x, sp1 = sp0 + pad16u((uint32_t)nb0 * vecb((uint32_t)r_k));
+            const uint32_t sp0 = ring0 + slot_tab[sc].x, sp1 = sp0 + ((d.x & 255u) << 4);
             if (kGatherOnly) {
                 mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);
                 calib ^= lds_u32(sp0 + 4 * lane);
@@ -379,8 +427,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);  // the group's K parts have landed
 
             // ---- QK: S (tokens x heads); rows 0-7 = block 0, rows 8-15 = block 1
-            float S[4] = {0.f, 0.f, 0.f, 0.f};
             if (nb0 != 0) {
+                float S[4] = {0.f, 0.f, 0.f, 0.f};
                 if (r_k == kD && full) {
                     const uint32_t a0 = sp0 + 256 * gq + 64 * qq, a1 = sp1 + 256 * gq + 64 * qq;
 #pragma unroll
@@ -421,13 +469,14 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 const float zA1 = v1 ? S[2] * scale_log2 : -INFINITY, zB1 = v1 ? S[3] * scale_log2 : -INFINITY;
                 mxA = fmaxf(mxA, fmaxf(zA0, zA1));
                 mxB = fmaxf(mxB, fmaxf(zB0, zB1));
-                float* z0 = zptr(pos);
-                if (2 * qq < G) z0[(2 * qq) * 8 + gq] = zA0;
-                if (2 * qq + 1 < G) z0[(2 * qq + 1) * 8 + gq] = zB0;
-                if (two) {
-                    float* z1 = zptr(pos + 1);
-                    if (2 * qq < G) z1[(2 * qq) * 8 + gq] = zA1;
-                    if (2 * qq + 1 < G) z1[(2 * qq + 1) * 8 + gq] = zB1;
+                if (bposc + 1 < zcap) {  // both blocks in the shared-memory cache
+                    const uint32_t za = zs0 + (uint32_t)bposc * zstride + zw;
+                    if (2 * qq < G) { sts_f32(za, zA0); if (two) sts_f32(za + zstride, zA1); }
+                    if (2 * qq + 1 < G) { sts_f32(za + 32, zB0); if (two) sts_f32(za + zstride + 32, zB1); }
+                } else {
+                    float* z0 = scr.zbuf + (size_t)(lo + bposc) * (size_t)(8 * G) + (zw >> 2);
+                    if (2 * qq < G) { z0[0] = zA0; if (two) z0[8 * G] = zA1; }
+                    if (2 * qq + 1 < G) { z0[8] = zB0; if (two) z0[8 * G + 8] = zB1; }
                 }
             }
             __syncwarp();  // every lane is done reading the slot
@@ -439,23 +488,6 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     }
 
     // =====================================================================================
-    // The CTAs that share a unit meet: every warp of this CTA has issued its atomic maxima (barrier), then one
-    // thread per unit of the CTA's range releases them (fence, cumulative over the barrier) and arrives.
-    // =====================================================================================
-    if (!kGatherOnly) {
-        __syncthreads();
-        if (clo < chi) {
-            const int u_first = find_unit(s_cum, g.n_units, clo), u_last = find_unit(s_cum, g.n_units, chi - 1);
-#pragma unroll 1
-            for (int u = u_first + (int)threadIdx.x; u <= u_last; u += kNT) {
-                if (s_cum[u + 1] == s_cum[u] || (clo <= s_cum[u] && s_cum[u + 1] <= chi)) continue;  // empty, or nobody else waits
-                __threadfence();
-                atomicAdd(scr.uarrive + u, 1);
-            }
-        }
-    }
-
-    // =====================================================================================
     // Phase 2: softmax sums over every selected token, PV over the blocks that matter.
     // =====================================================================================
     float acc[8][4];    // O^T tile i: rows gq / gq+8 = channels 16gq + 2i / + 1, columns 2qq, 2qq+1 = heads
@@ -463,7 +495,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     float Mh = 0.f;     // the unit's maximum logit of head gq (log2 domain); 0 if the unit has no valid token
     float Mraw = -INFINITY;
     cur_unit = -1;
-    unsigned long long st_vblocks = 0ull, st_vbytes = 0ull;
+    unsigned st_vblocks = 0u, st_vbytes = 0u;
 
     // end of a unit inside this warp's range.  `last`: the range is finished and the ring is idle, so the
     // partial lives in this warp's own shared memory (record 2w + 1); a unit that ends inside the range
@@ -474,8 +506,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         lsum += __shfl_xor_sync(kFull, lsum, 1);
         lsum += __shfl_xor_sync(kFull, lsum, 2);  // lanes (gq, *): the warp's sum of head gq
         const int hA = 2 * qq, hB = 2 * qq + 1;
-        const float lA = __shfl_sync(kFull, lsum, (4 * hA) & 31), lB = __shfl_sync(kFull, lsum, (4 * hB) & 31);
-        const float mA = __shfl_sync(kFull, Mraw, (4 * hA) & 31), mB = __shfl_sync(kFull, Mraw, (4 * hB) & 31);
+        const float lA = __shfl_sync(kFull, lsum, 4 * hA), lB = __shfl_sync(kFull, lsum, 4 * hB);
+        const float mA = __shfl_sync(kFull, Mraw, 4 * hA), mB = __shfl_sync(kFull, Mraw, 4 * hB);
         const bool whole = lo <= a && b <= hi;  // the whole unit was processed by this warp: final result
         float fA = 1.f, fB = 1.f;
         float* po;
@@ -498,7 +530,9 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 if (hA < G) pl[hA] = lA > 0.f ? (mA + log2f(lA)) * kLn2 : -INFINITY;
                 if (hB < G) pl[hB] = lB > 0.f ? (mB + log2f(lB)) * kLn2 : -INFINITY;
             }
-            if (lane < kMaxGroup) scr.umax[(size_t)u * kMaxGroup + lane] = 0u;  // only this warp ever read them: reset for the next launch
+            // only this warp ever read the unit's meeting state: reset it for the next launch
+            if (lane < kMaxGroup) scr.umax[(size_t)u * kMaxGroup + lane] = 0u;
+            if (lane == kMaxGroup) scr.uarrive[u] = 0;
         } else {
             const int rec = warp * 2 + (last ? 1 : 0);
             if (gq == 0) {
@@ -509,47 +543,47 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         }
     };
 
-    // wait until every CTA that shares unit u has published its maxima, then read them
+    // wait until every warp that holds a part of unit u has published its maxima, then read them
     auto begin_unit = [&](int u) {
         cur_unit = u;
         lsum = 0.f;
 #pragma unroll
         for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
-        const int a = s_cum[u], b = s_cum[u + 1];
-        if (!(clo <= a && b <= chi)) {  // shared with other CTAs
-            if (lane == 0) {
-                const int expected = (int)cs.owner(((unsigned)b - 1u) >> 1) - (int)cs.owner((unsigned)a >> 1) + 1;
-                int it = 0;
+        if (lane == 0) {
+            const int expected = warps_meeting(s_cum[u], s_cum[u + 1]);
+            int it = 0;
 #pragma unroll 1
-                while (ld_acquire(scr.uarrive + u) < expected) {
-                    if (++it > kSpinLimit) { atomicOr(dev_flags, MKV_DEV_SYNC_TIMEOUT); break; }
-                }
+            while (ld_acquire(scr.uarrive + u) < expected) {
+                __nanosleep(100);  // leave the issue slots to the warps that are still in phase 1
+                if (++it > kSpinLimit) { atomicOr(dev_flags, MKV_DEV_SYNC_TIMEOUT); break; }
             }
-            __syncwarp();
         }
+        __syncwarp();
         Mraw = gq < G ? funkey(ld_relaxed_u32(scr.umax + (size_t)u * kMaxGroup + gq)) : -INFINITY;
         Mh = Mraw == -INFINITY ? 0.f : Mraw;
     };
 
-    {
-        bbuilt = 0; gbuilt = 0;
+    if (n_total > 0) {
+        // the range's descriptors are still in shared memory unless it was longer than one ring: then describe again
+        const bool redo = gbuilt > kDesc;
+        if (redo) { bbuilt = 0; gbuilt = 0; ucur = find_unit(s_cum, g.n_units, lo); }
+        const int gtotal = gbuilt;
         int bposd = 0, gposd = 0;  // blocks / groups decided
 #pragma unroll 1
         for (;;) {
             // ---- decide: softmax sums of the next groups; start the V copies of the groups that matter
 #pragma unroll 1
             while (bposd < n_total) {
-                if (gposd == gbuilt) describe(min(32, n_total - bbuilt));
-                const GDesc d = ring[gposd & (kDescRing - 1)];
-                const int u = (int)(d.a & 0xffffu);
+                if (redo) { if (gposd == gbuilt) describe(min(kDescribe, n_total - bbuilt)); }
+                else if (gposd == gtotal) break;
+                const GDesc d = d2[gposd & (kDesc - 1)];
+                const int u = (int)(d.y & 0xffffu);
                 if (!kGatherOnly && u != cur_unit) {
                     if (pend != 0) break;  // drain the unit's groups in flight first
                     if (cur_unit >= 0) flush(false);
                     begin_unit(u);
                 }
-                uint32_t nb0 = d.b & 15u, nb1 = (d.b >> 4) & 15u;
-                const uint32_t rk = (d.a >> 16) & 255u, rv = d.a >> 24;
-                const int pos = (int)(d.b >> 9);
+                uint32_t nb0 = (d.y >> 20) & 15u, nb1 = (d.y >> 24) & 15u;
                 const bool two = nb1 != 0u;
                 bool need0 = nb0 != 0u, need1 = two;
                 float add = 0.f;
@@ -557,8 +591,15 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                     // lane (gq, qq): head gq, tokens 2qq, 2qq+1 of each block
                     float2 za = make_float2(-INFINITY, -INFINITY), zb = za;
                     if (gq < G) {
-                        za = *reinterpret_cast<const float2*>(zptr(pos) + gq * 8 + 2 * qq);
-                        if (two) zb = *reinterpret_cast<const float2*>(zptr(pos + 1) + gq * 8 + 2 * qq);
+                        if (bposd + 1 < zcap) {
+                            const uint32_t a = zs0 + (uint32_t)bposd * zstride + zr;
+                            za = lds_f32x2(a);
+                            if (two) zb = lds_f32x2(a + zstride);
+                        } else {
+                            const float* z0 = scr.zbuf + (size_t)(lo + bposd) * (size_t)(8 * G) + (zr >> 2);
+                            za = __ldcg(reinterpret_cast<const float2*>(z0));
+                            if (two) zb = __ldcg(reinterpret_cast<const float2*>(z0 + 8 * G));
+                        }
                     }
                     add = (ex2(za.x - Mh) + ex2(za.y - Mh)) + (ex2(zb.x - Mh) + ex2(zb.y - Mh));
                     need0 = __any_sync(kFull, fmaxf(za.x, za.y) - Mh >= -kSkip);
@@ -566,30 +607,26 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 }
                 if (need0 || need1) {
                     // a group with one block that matters becomes a one-block group
-                    uint32_t off0 = d.off0, off1 = d.off1, p = (uint32_t)pos;
-                    if (!need0) { off0 = d.off1; nb0 = nb1; nb1 = 0u; p += 1u; }
-                    else if (!need1) nb1 = 0u;
-                    const bool upd = d.b & 256u;
-                    // V part of a block: starts kb bytes into its payload (update buffer: the V rows, same offset)
-                    const uint32_t kb0 = upd ? 0u : nb0 * vecb(rk), kb1 = upd ? 0u : nb1 * vecb(rk);
-                    const uint32_t c0 = pad16u((kb0 & 15u) + nb0 * vecb(rv));
-                    const uint32_t c1 = nb1 ? pad16u((kb1 & 15u) + nb1 * vecb(rv)) : 0u;
+                    uint32_t off0 = d.off0, off1 = d.off1, c0 = (d.x & 255u) << 4, c1 = ((d.x >> 8) & 255u) << 4;
+                    uint32_t sk0 = (d.x >> 16) & 15u, sk1 = (d.x >> 20) & 15u, shift = 0u;
+                    if (!need0) { off0 = off1; c0 = c1; sk0 = sk1; nb0 = nb1; nb1 = 0u; c1 = 0u; shift = 1u; }
+                    else if (!need1) { nb1 = 0u; c1 = 0u; }
                     uint32_t off;
                     if (!ring_alloc(c0 + c1, off)) break;  // no room yet: decide this group again after a consume
                     if (lane == 0) {
                         const uint32_t bar = bar0 + 8 * si, dst = ring0 + off;
-                        const unsigned long long src = upd ? reinterpret_cast<unsigned long long>(upd_v) : slice;
+                        const unsigned long long src = (d.y & 0x10000u) ? reinterpret_cast<unsigned long long>(upd_v) : slice;
                         mbar_expect_tx(bar, c0 + c1);
-                        bulk_g2s(dst, src + ((unsigned long long)off0 << 4) + (kb0 & ~15u), c0, bar);
-                        if (c1) bulk_g2s(dst + c0, src + ((unsigned long long)off1 << 4) + (kb1 & ~15u), c1, bar);
+                        bulk_g2s(dst, src + ((unsigned long long)off0 << 4), c0, bar);
+                        if (c1) bulk_g2s(dst + c0, src + ((unsigned long long)off1 << 4), c1, bar);
                         GDesc e;
-                        e.off0 = (kb0 & 15u) | (c0 << 8) | ((kb1 & 15u) << 4);  // skews of the V parts, bytes of the first chunk
-                        e.off1 = 0u;
-                        e.a = d.a;
-                        e.b = nb0 | (nb1 << 4) | (d.b & 256u) | (p << 9);
+                        e.off0 = sk0 | (sk1 << 4) | (c0 << 8);                   // skews of the V parts, bytes of the first chunk
+                        e.off1 = (uint32_t)bposd;                                // index of the group's first block in the range
+                        e.x = d.x;
+                        e.y = nb0 | (nb1 << 4) | (shift << 8);                   // shift: only the group's second block is walked
                         slot_grp[si] = e;
                     }
-                    st_vblocks += nb1 ? 2ull : 1ull;
+                    st_vblocks += nb1 ? 2u : 1u;
                     st_vbytes += c0 + c1;
                     ring_commit();
                 }
@@ -604,8 +641,9 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
 
             // ---- consume the oldest group in flight: PV
             const GDesc d = slot_grp[sc];
-            const int r_v = (int)(d.a >> 24);
-            const int nb0 = (int)(d.b & 15u), nb1 = (int)((d.b >> 4) & 15u), pos = (int)(d.b >> 9);
+            const int r_v = (int)(d.x >> 24);
+            const int nb0 = (int)(d.y & 15u), nb1 = (int)((d.y >> 4) & 15u), pos = (int)d.off1;
+            const uint32_t zsh = (d.y >> 8) & 1u;
             const bool two = nb1 != 0;
             const uint32_t vb0 = ring0 + slot_tab[sc].x + (d.off0 & 15u);
             const uint32_t vb1 = ring0 + slot_tab[sc].x + (d.off0 >> 8) + ((d.off0 >> 4) & 15u);
@@ -620,8 +658,15 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             // exactly the B fragments of O^T += V^T P^T (k = token, n = head)
             float2 za = make_float2(-INFINITY, -INFINITY), zb = za;
             if (gq < G) {
-                za = *reinterpret_cast<const float2*>(zptr(pos) + gq * 8 + 2 * qq);
-                if (two) zb = *reinterpret_cast<const float2*>(zptr(pos + 1) + gq * 8 + 2 * qq);
+                if (pos + 1 < zcap) {  // (the same test as when the group's logits were stored)
+                    const uint32_t a = zs0 + ((uint32_t)pos + zsh) * zstride + zr;
+                    za = lds_f32x2(a);
+                    if (two) zb = lds_f32x2(a + zstride);
+                } else {
+                    const float* z0 = scr.zbuf + (size_t)(lo + pos + (int)zsh) * (size_t)(8 * G) + (zr >> 2);
+                    za = __ldcg(reinterpret_cast<const float2*>(z0));
+                    if (two) zb = __ldcg(reinterpret_cast<const float2*>(z0 + 8 * G));
+                }
             }
             const float e00 = ex2(za.x - Mh), e01 = ex2(za.y - Mh), e10 = ex2(zb.x - Mh), e11 = ex2(zb.y - Mh);
             const uint32_t ph0 = pack_bf16(e00, e01), ph1 = pack_bf16(e10, e11);
@@ -687,9 +732,9 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         if (calib == 0x9e3779b9u && lane == 0) scr.part_l[(size_t)gw * 2 * (2 * kMaxGroup)] = 0.f;
         return;
     }
-    if (lane == 0 && st_vblocks != 0ull) {
-        atomicAdd(scr.stats + 1, st_vblocks);
-        atomicAdd(scr.stats + 2, st_vbytes);
+    if (lane == 0 && st_vblocks != 0u) {
+        atomicAdd(scr.stats + 1, (unsigned long long)st_vblocks);
+        atomicAdd(scr.stats + 2, (unsigned long long)st_vbytes);
     }
     if (threadIdx.x == 0 && blockIdx.x == 0) atomicAdd(scr.stats + 0, (unsigned long long)T);
 
@@ -697,13 +742,11 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     // Records are in warp order (2w = head, 2w + 1 = tail), hence in non-decreasing unit order: the
     // partials of one unit form a run.  Thread tid owns four consecutive output channels of one head.
     // All partials of a unit are relative to the same maximum, so folding is plain addition (the
-    // split-K rule of oracle pin P10 with equal references).
+    // split-K rule of oracle pin P10 with equal references), always in the same order.
     __syncthreads();  // orders the warps' partials (shared memory, or global scratch from flush(false))
     const int GD = G * kD;
     const size_t cta_slot_base = (size_t)gridDim.x * kWarps * 2;
     const int tid = threadIdx.x;
-    int sh_u0 = -1, sh_u1 = -1;  // units this CTA shares with others (<= 2: one entering, one leaving its range)
-    int n_shared = 0;
     // GD / 4 threads fold one unit, so a CTA folds kNT / (GD / 4) units side by side
     const int tpr = GD / 4, nslots = max(1, kNT / tpr);
     const int rs = tid / tpr, e = 4 * (tid - rs * tpr), h = e >> 7;
@@ -720,15 +763,6 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             if (nxt == 0x7fffffff) break;
             last = nxt;
             if (k == rs) mine = nxt;
-            const bool inside = clo <= s_cum[nxt] && s_cum[nxt + 1] <= chi;
-            if (inside) {
-                // wholly inside this CTA and past phase 2 in every warp: reset its maxima for the next launch
-                if (tid < kMaxGroup) scr.umax[(size_t)nxt * kMaxGroup + tid] = 0u;
-            } else if (n_shared < 2) {  // shared with other CTAs
-                if (tid == 0) s_row[n_shared] = (size_t)(nxt / g.n_kv_heads) * g.n_q_heads + (size_t)(nxt % g.n_kv_heads) * G;
-                if (n_shared == 0) sh_u0 = nxt; else sh_u1 = nxt;
-                ++n_shared;
-            }
         }
         if (last == run) break;
         run = last;
@@ -738,18 +772,9 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         const int a = s_cum[mine], b = s_cum[mine + 1];
         const bool whole = clo <= a && b <= chi;
         const size_t row = (size_t)(mine / g.n_kv_heads) * g.n_q_heads + (size_t)(mine % g.n_kv_heads) * G;
-        const size_t slot = cta_slot_base + blockIdx.x * 2 + (a < clo ? 0 : 1);
         float4 O = make_float4(0.f, 0.f, 0.f, 0.f);
         float Lr = 0.f, Mr = -INFINITY;
-        // tail partials (record 2w + 1, in warp w's shared memory): straight-line, every load independent
-#pragma unroll
-        for (int w = 0; w < kWarps; ++w) {
-            const bool mem = (recs >> (2 * w + 1)) & 1u;
-            const float2 ml = *reinterpret_cast<const float2*>(&s_ml[2 * w + 1][h][0]);
-            const float4 o = *reinterpret_cast<const float4*>(smem + w * kWS + 4 * e);
-            if (mem) { Mr = ml.x; Lr += ml.y; O.x += o.x; O.y += o.y; O.z += o.z; O.w += o.w; }
-        }
-        // head partials (record 2w, in global scratch): rare
+        // head partials (record 2w, in global scratch): at most one per CTA in practice (the unit entering its range)
 #pragma unroll 1
         for (unsigned m = recs & 0x55555555u; m; m &= m - 1u) {
             const int w = (__ffs(m) - 1) >> 1;
@@ -759,67 +784,57 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 scr.part_o + ((size_t)blockIdx.x * kWarps + w) * 2 * (size_t)GD + e));
             O.x += o.x; O.y += o.y; O.z += o.z; O.w += o.w;
         }
+        // tail partials (record 2w + 1, in warp w's shared memory): straight-line, every load independent
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) {
+            const bool mem = (recs >> (2 * w + 1)) & 1u;
+            const float2 ml = *reinterpret_cast<const float2*>(&s_ml[2 * w + 1][h][0]);
+            const float4 o = *reinterpret_cast<const float4*>(smem + w * kWS + 4 * e);
+            if (mem) { Mr = ml.x; Lr += ml.y; O.x += o.x; O.y += o.y; O.z += o.z; O.w += o.w; }
+        }
         if (whole) {
+            // wholly inside this CTA and past phase 2 in every warp: reset its meeting state for the next launch
+            if (e < 4 * kMaxGroup) scr.umax[(size_t)mine * kMaxGroup + (e >> 2)] = 0u;
+            if (e == 4 * kMaxGroup) scr.uarrive[mine] = 0;
             const float inv = Lr > 0.f ? 1.f / Lr : 0.f;
             *reinterpret_cast<float4*>(out + row * kD + e) = make_float4(O.x * inv, O.y * inv, O.z * inv, O.w * inv);
             if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = Lr > 0.f ? (Mr + log2f(Lr)) * kLn2 : -INFINITY;
-        } else {
-            *reinterpret_cast<float4*>(scr.part_o + slot * GD + e) = O;
-            if ((e & (kD - 1)) == 0) {
-                scr.part_l[slot * (2 * kMaxGroup) + 2 * h] = Mr;
-                scr.part_l[slot * (2 * kMaxGroup) + 2 * h + 1] = Lr;
-            }
+            continue;
         }
-    }
-    if (n_shared == 0) return;  // uniform over the CTA
-
-    // One thread per shared unit releases the CTA's partial (the barrier orders the other threads'
-    // stores before its fence), finds the sharers c_first .. c_last (CTAs whose ranges meet the unit)
-    // and takes a ticket.  A sharer's slot is 1 for c_first (the unit starts inside it), else 0.
-    __syncthreads();
-    if ((tid == 0 || tid == 32) && (tid >> 5) < n_shared) {
-        const int k = tid >> 5, u = k == 0 ? sh_u0 : sh_u1;
-        int cf = (int)blockIdx.x, cl = (int)blockIdx.x;
-        if (s_cum[u] < clo) cf = (int)cs.owner((unsigned)s_cum[u] >> 1);
-        if (s_cum[u + 1] > chi) cl = (int)cs.owner(((unsigned)s_cum[u + 1] - 1u) >> 1);
-        s_cf[k] = cf; s_cl[k] = cl;
-        int old;  // release this CTA's partial (ordered by the barrier), acquire the other sharers'
-        asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(scr.ticket + u) : "memory");
-        s_last[k] = old == cl - cf;
-        if (old == cl - cf) {  // every sharer has arrived (and is past phase 2): reset the unit's state for the next launch
-            scr.ticket[u] = 0;
-            scr.uarrive[u] = 0;
-#pragma unroll
-            for (int hh = 0; hh < kMaxGroup; ++hh) scr.umax[(size_t)u * kMaxGroup + hh] = 0u;
-        }
-    }
-    __syncthreads();
-    // last arrivers: thread group rs adds the CTA partials of shared unit rs (read with ld.global.cg: L2,
-    // never a stale L1 line), in CTA order; with nslots = 1 (G = 8) the groups take the units in turn
-#pragma unroll 1
-    for (int k = rs < nslots ? rs : n_shared; k < n_shared; k += nslots) {
-        if (!s_last[k]) continue;
-        const int c_first = s_cf[k], c_last = s_cl[k];
-        const size_t row = s_row[k];
+        // The unit spans CTAs c_first .. c_last.  This thread stores its four channels of the CTA's partial (slot 1 for
+        // c_first: the unit starts inside it, else slot 0) and takes a ticket of its own channel quad; the last of the
+        // sharers' threads to arrive adds the partials in CTA order.  Every quad proceeds on its own: no barrier.
+        const int c_first = (int)cs.owner((unsigned)a >> 1), c_last = (int)cs.owner(((unsigned)b - 1u) >> 1);
+        const size_t slot = cta_slot_base + blockIdx.x * 2 + (a < clo ? 0 : 1);
+        float* my_o = scr.part_o + slot * GD + e;
+        float* my_l = scr.part_l + slot * (2 * kMaxGroup) + 2 * h;
+        __stcg(reinterpret_cast<float4*>(my_o), O);
+        if ((e & (kD - 1)) == 0) __stcg(reinterpret_cast<float2*>(my_l), make_float2(Mr, Lr));
+        int32_t* tk = scr.ticket + (size_t)mine * (kMaxGroup * kD / 4) + (e >> 2);
+        int old;  // release this thread's partial, acquire the other sharers'
+        asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(tk) : "memory");
+        if (old != c_last - c_first) continue;
+        *tk = 0;  // self-cleaning: every sharer has arrived (and is past phase 2)
+        if (e < 4 * kMaxGroup) scr.umax[(size_t)mine * kMaxGroup + (e >> 2)] = 0u;
+        if (e == 4 * kMaxGroup) scr.uarrive[mine] = 0;
         float Mx = -INFINITY, Lx = 0.f;
         float4 Ox = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 1
         for (int c0 = c_first; c0 <= c_last; c0 += 4) {  // four partials' loads in flight at once
-            float pm[4], pl[4];
+            float2 pm[4];
             float4 po[4];
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
                 const int c = min(c0 + t, c_last);  // a repeated partial is not added below
                 const size_t sl = cta_slot_base + (size_t)c * 2 + (c == c_first ? 1 : 0);
-                pm[t] = __ldcg(scr.part_l + sl * (2 * kMaxGroup) + 2 * h);
-                pl[t] = __ldcg(scr.part_l + sl * (2 * kMaxGroup) + 2 * h + 1);
+                pm[t] = __ldcg(reinterpret_cast<const float2*>(scr.part_l + sl * (2 * kMaxGroup) + 2 * h));
                 po[t] = __ldcg(reinterpret_cast<const float4*>(scr.part_o + sl * (size_t)GD + e));
             }
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
                 if (c0 + t > c_last) continue;
-                Mx = pm[t];
-                Lx += pl[t];
+                Mx = pm[t].x;
+                Lx += pm[t].y;
                 Ox.x += po[t].x; Ox.y += po[t].y; Ox.z += po[t].z; Ox.w += po[t].w;
             }
         }
@@ -860,6 +875,7 @@ mkv_stream_read_kernel(const uint4* __restrict__ base, unsigned long long n16, u
 }  // namespace
 
 int attention_partial_slots(int sm_count) { return sm_count * kWarps * 2 + sm_count * 2; }
+size_t attention_ticket_ints(const CacheGeom& g) { return (size_t)g.n_units * (kMaxGroup * kD / 4); }
 
 // logit scratch: one entry of 8 G floats per position of the block stream (selected blocks + update-buffer blocks)
 size_t attention_zbuf_floats(const CacheGeom& g) {

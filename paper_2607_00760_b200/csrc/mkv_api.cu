@@ -174,7 +174,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         {(void**)&c->upd_cnt, (size_t)g.n_layers * 4 + 252},
         {(void**)&c->attn.part_o, (size_t)c->attn.slots * g.group * kD * 4},
         {(void**)&c->attn.part_l, (size_t)c->attn.slots * kMaxGroup * 2 * 4},
-        {(void**)&c->attn.ticket, (size_t)g.n_units * 4},
+        {(void**)&c->attn.ticket, attention_ticket_ints(g) * 4},
         {(void**)&c->attn.umax, (size_t)g.n_units * kMaxGroup * 4},
         {(void**)&c->attn.uarrive, (size_t)g.n_units * 4},
         {(void**)&c->attn.zbuf, attention_zbuf_floats(g) * 4},
@@ -199,7 +199,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     cudaMemset(c->counters, 0, (size_t)g.n_layers * 4 * 8);
     cudaMemset(c->dev_flags, 0, 256);
     cudaMemset(c->upd_cnt, 0, (size_t)g.n_layers * 4);
-    cudaMemset(c->attn.ticket, 0, (size_t)g.n_units * 4);
+    cudaMemset(c->attn.ticket, 0, attention_ticket_ints(g) * 4);
     cudaMemset(c->attn.umax, 0, (size_t)g.n_units * kMaxGroup * 4);
     cudaMemset(c->attn.uarrive, 0, (size_t)g.n_units * 4);
     cudaMemset(c->attn.stats, 0, 64);
@@ -223,7 +223,7 @@ int mkv_cache_reset(mkv_cache* c, int32_t layer, void* stream) {
     cudaStream_t s = (cudaStream_t)stream;
     const int l0 = layer < 0 ? 0 : layer, l1 = layer < 0 ? g.n_layers : layer + 1;
     ++c->generation;  // plan records written before the reset no longer match
-    MKV_CUDA(cudaMemsetAsync(c->attn.ticket, 0, (size_t)g.n_units * 4, s));  // (a launch that timed out leaves these dirty)
+    MKV_CUDA(cudaMemsetAsync(c->attn.ticket, 0, attention_ticket_ints(g) * 4, s));  // (a launch that timed out leaves these dirty)
     MKV_CUDA(cudaMemsetAsync(c->attn.umax, 0, (size_t)g.n_units * kMaxGroup * 4, s));
     MKV_CUDA(cudaMemsetAsync(c->attn.uarrive, 0, (size_t)g.n_units * 4, s));
     for (int l = l0; l < l1; ++l) {

@@ -119,9 +119,9 @@ __device__ __forceinline__ void plan_lookup(const CacheGeom& g, const LayerView&
 struct AttnScratch {
     float* part_o;        // [slots][G][D]   unnormalised partial outputs (<= 2 slots per warp and per CTA of the grid)
     float* part_l;        // [slots][8]      partial softmax sums, all relative to the unit's global maximum
-    int32_t* ticket;      // [n_units]       arrivals of the CTAs sharing a unit (step 3d); zero between launches
+    int32_t* ticket;      // [n_units][256]  per channel quad: arrivals of the CTAs sharing a unit (step 3d); zero between launches
     uint32_t* umax;       // [n_units][8]    per (unit, head) maximum logit as an order-preserving key; zero between launches
-    int32_t* uarrive;     // [n_units]       CTAs that have published their maxima of a unit; zero between launches
+    int32_t* uarrive;     // [n_units]       warps that have published their maxima of a unit; zero between launches
     float* zbuf;          // [z_cap][8 G]    logits of blocks that do not fit a warp's shared-memory cache
     unsigned long long* stats;  // [8]       counters of mkv_attention_stats
     PlanRec* plan;        // [n_units][plan_stride] of this layer (may be nullptr)
@@ -131,6 +131,7 @@ struct AttnScratch {
 };
 int attention_partial_slots(int sm_count);
 size_t attention_zbuf_floats(const CacheGeom& g);
+size_t attention_ticket_ints(const CacheGeom& g);
 cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q,
                              const int32_t* sel, const int32_t* sel_count, int k_max, float scale,
                              float* out, float* lse, const AttnScratch& scr, const uint16_t* upd_k,

@@ -247,16 +247,7 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
             const int pos = gt_before + min(eq_before, take_eq);
             if (take && pos < cap) {
                 if (MODE == 1) { okey[pos] = all ? keyat(i) : u; oidx[pos] = idxat(i); }
-                else {
-                    const int t0 = idxat(i) * kB;
-                    out[pos] = t0;
-                    if (plan != nullptr && pos < plan_stride) {  // what mkv_packed_attention needs to know about the block
-                        PlanRec pr;
-                        pr.t0 = t0; pr.tag = tag;
-                        plan_lookup(g, lv, unit, t0, pr.off16, pr.meta);
-                        plan[(size_t)unit * plan_stride + pos] = pr;
-                    }
-                }
+                else out[pos] = idxat(i) * kB;
             }
             gt_before += gt ? 1 : 0;
             eq_before += eq ? 1 : 0;
@@ -270,6 +261,17 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
         }
     }
     count = min(count, cap);
+    if (MODE != 1 && plan != nullptr) {
+        // what mkv_packed_attention needs to know about every selected block (payload offset, tokens, r_k, r_v): one
+        // record per block, looked up by all threads at once (one round of table reads for the whole unit)
+        __syncthreads();  // the CTA's writes to `out` are visible to its own threads
+        for (int p = tid; p < min(count, plan_stride); p += 1024) {
+            PlanRec pr;
+            pr.t0 = out[p]; pr.tag = tag;
+            plan_lookup(g, lv, unit, pr.t0, pr.off16, pr.meta);
+            plan[(size_t)unit * plan_stride + p] = pr;
+        }
+    }
     if (MODE == 1) {
         for (int p = count + tid; p < cap; p += 1024) { okey[p] = 0u; oidx[p] = -1; }  // padding: below every real key
     } else {
