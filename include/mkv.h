@@ -71,7 +71,6 @@ typedef enum {
 /* device-side sticky flags reported by mkv_cache_status */
 #define MKV_DEV_ARENA_OVERFLOW 1u /* a compress call needed more arena than the layer slice holds */
 #define MKV_DEV_BAD_STRATEGY 2u   /* a strategy record in device memory was invalid/unsupported */
-#define MKV_DEV_SYNC_TIMEOUT 4u   /* mkv_packed_attention: the CTAs sharing a unit did not all arrive (result invalid) */
 
 typedef struct mkv_cache mkv_cache; /* opaque: packed arenas + tables + scratch of one model */
 
@@ -160,8 +159,7 @@ MKV_API int mkv_select(const mkv_cache* cache, int32_t layer, const void* q, int
  * tokens of the layer's KV update buffer if it holds any (see mkv_update_append).
  * sel / sel_count as written by mkv_select (any order of blocks is accepted; entries the caller changed after
  * mkv_select are honoured: the per-block records mkv_select leaves for this call are verified against `sel`).
- * One launch of one CTA per SM whose CTAs meet at per-unit counters in device memory: it needs the whole GPU
- * (do not run it next to other work that pins SMs).  A missed meeting sets MKV_DEV_SYNC_TIMEOUT.
+ * One launch of one CTA per SM; no CTA waits for another one.
  * out: float [batch][n_q_heads][D].  lse_opt: float [batch][n_q_heads] or NULL (log-sum-exp of the
  * scaled logits; -inf and out = 0 for an empty selection).
  */
@@ -211,8 +209,8 @@ MKV_API int mkv_decode_host(mkv_cache* cache, int32_t layer, const void* q_host,
  * stream: a plain streaming read of the first `bytes` bytes of the layer's packed arena (clamped to its size) in
  *         the same launch shape (one 512-thread CTA per SM, 16-byte loads): launch + pure-bandwidth floor.
  * stats:  counters accumulated by mkv_packed_attention since the last reset: token blocks attended, token blocks
- *         whose V part was fetched (phase 2 skips a block whose probabilities are all < 2^-40 of the unit's
- *         largest), bytes of those V copies.  Synchronises.
+ *         whose V part was fetched (phase 2 skips a block whose probabilities are all < 2^-40 of the largest
+ *         the CTA holds of the unit), bytes of those V copies.  Synchronises.
  */
 MKV_API int mkv_calibrate_gather(const mkv_cache* cache, int32_t layer, const int32_t* sel,
                          const int32_t* sel_count, int32_t k_max, void* stream);

@@ -18,7 +18,7 @@ if not os.path.exists(LIB_PATH):
 _lib = C.CDLL(LIB_PATH)
 
 MKV_OK, MKV_E_ARG, MKV_E_UNSUPPORTED, MKV_E_NOMEM, MKV_E_CUDA, MKV_E_STATE, MKV_E_DEVICE = 0, -1, -2, -3, -4, -5, -6
-MKV_DEV_ARENA_OVERFLOW, MKV_DEV_BAD_STRATEGY, MKV_DEV_SYNC_TIMEOUT = 1, 2, 4
+MKV_DEV_ARENA_OVERFLOW, MKV_DEV_BAD_STRATEGY = 1, 2
 
 # every symbol include/mkv.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ["mkv_cache_create", "mkv_cache_free", "mkv_cache_reset", "mkv_segment_loss",

@@ -14,19 +14,21 @@
 //   * Phase 1 (QK): S = K q^T with the group's 16 tokens = M, heads = N, channels = K; packed
 //     vectors are expanded straight into mma.sync fragments (mkv_walk.cuh).  The scaled logits go
 //     to the warp's logit cache (shared memory; global scratch beyond its capacity).  At the end of
-//     a unit the warp publishes its per-head maxima (atomic max) and arrives at the unit's counter.
-//   * Phase 2 (PV, deferred) starts per unit when every warp that holds a part of it has arrived:
-//     the warp then knows the unit's exact maximum M, so all probabilities are 2^(z - M), nothing
-//     is ever rescaled, and partial results of one unit simply add.  The softmax sum runs over
-//     every selected token; the V part of a block is fetched and walked only if one of its
-//     probabilities is >= 2^-40 (error bound).  O^T = V^T P^T with channels = M,
-//     heads = N, the group's 16 tokens = K; P is split into bf16 hi + lo (fp32-class accuracy).
-//     Dense vectors (r = D) skip the walk.
+//     a unit the warp folds its per-head maxima into the CTA's table (shared-memory atomic max).
+//   * One CTA barrier separates the phases.  Phase 2 (PV, deferred) then knows, for every unit of
+//     the CTA's range, the maximum logit M_c over ALL the tokens the CTA holds of it (about 1 800 of
+//     a unit's 4 096 at config 2): probabilities are 2^(z - M_c), nothing is ever rescaled inside a
+//     CTA, and the partials of one unit inside a CTA simply add.  The softmax sum runs over every
+//     selected token; the V part of a block is fetched and walked only if one of its probabilities
+//     is >= 2^-40 of the CTA's largest (error bound; M_c <= the unit's true maximum, so
+//     the test is conservative).  O^T = V^T P^T with channels = M, heads = N, the group's 16 tokens
+//     = K; P is split into bf16 hi + lo (fp32-class accuracy).  Dense vectors (r = D) skip the walk.
 //   * Step 3d (split-K combine) is fused: a unit wholly inside one warp's range is normalised and
-//     written directly; otherwise the warp leaves an (l, O) partial (<= 2 per warp), the threads of
-//     the CTA add the partials of a unit (four output channels each), and a unit that spans several
-//     CTAs is finished, four channels at a time, by the last thread to arrive at a per-(unit,
-//     channel quad) ticket (no second kernel, no barrier after the fold).
+//     written directly; otherwise the warp leaves an (m, l, O) partial (<= 2 per warp), the threads
+//     of the CTA fold the partials of a unit (four output channels each) with the LSE rule, and a
+//     unit that spans several CTAs is finished, four channels at a time, by the last thread to
+//     arrive at a per-(unit, channel quad) ticket (no second kernel, no barrier after the fold).
+//     Nothing in the kernel waits for another CTA.
 #include "mkv_internal.cuh"
 #include "mkv_walk.cuh"
 
@@ -47,7 +49,7 @@ constexpr int kDescribe = 24;      // blocks described per call: kDescribe + kSl
 constexpr int kZBytes = 4096;      // per-warp logit cache: 32 blocks at G = 4
 constexpr int kMaxUnitsSmem = 2048;
 constexpr float kSkip = 40.f;      // a block whose probabilities are all < 2^-40 is not walked in phase 2
-constexpr int kSpinLimit = 1 << 22;
+constexpr int kCtaUnits = 32;     // units of a CTA's range whose maxima are shared through the CTA's table
 
 // One group of the stream: <= 2 consecutive selected token blocks of one unit with the same strategy whose K
 // parts and V parts each fit kGroupMax16.  Every size the hot loops need is worked out once, by the describing lane.
@@ -77,19 +79,6 @@ __device__ __forceinline__ uint32_t fkey(float f) {
 }
 __device__ __forceinline__ float funkey(uint32_t k) {
     return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
-}
-__device__ __forceinline__ uint32_t ld_relaxed_u32(const uint32_t* p) {
-    uint32_t v;
-    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ int ld_acquire(const int32_t* p) {
-    int v;
-    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void red_release_add(int32_t* p, int v) {
-    asm volatile("red.release.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 __device__ __forceinline__ void sts_f32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
 __device__ __forceinline__ float2 lds_f32x2(uint32_t a) {
@@ -137,7 +126,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                             const int32_t* __restrict__ sel, const int32_t* __restrict__ sel_count, int k_max,
                             float scale_log2, float* __restrict__ out, float* __restrict__ lse, AttnScratch scr,
                             const uint16_t* __restrict__ upd_k, const uint16_t* __restrict__ upd_v,
-                            const int32_t* __restrict__ upd_count, uint32_t* __restrict__ dev_flags) {
+                            const int32_t* __restrict__ upd_count) {
     extern __shared__ __align__(128) uint8_t smem[];
     constexpr int kNT = kWarps * 32;
     constexpr int kRec = 2 * kWarps;  // partial records of the CTA: warp w -> 2w (head), 2w + 1 (tail)
@@ -146,7 +135,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     const int gq = lane >> 2, qq = lane & 3;  // mma fragment coordinates (groupID, threadID_in_group)
 
     __shared__ int s_unit[kRec];                              // unit of each partial record, -1 = none
-    __shared__ __align__(8) float s_ml[kRec][kMaxGroup][2];   // its (global max in log2 units, sum) per head
+    __shared__ __align__(8) float s_ml[kRec][kMaxGroup][2];   // its (reference maximum in log2 units, sum) per head
+    __shared__ uint32_t s_umax[kCtaUnits][kMaxGroup];         // the CTA's maxima of the first kCtaUnits units of its range (keys)
 
     uint8_t* wbase = smem + warp * kWS;
     const uint32_t ring0 = smem_u32(wbase);
@@ -162,6 +152,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         mbar_init_fence();
     }
     if (lane < 2) s_unit[warp * 2 + lane] = -1;
+    if (threadIdx.x < kCtaUnits * kMaxGroup) (&s_umax[0][0])[threadIdx.x] = 0u;  // below the key of every float
+    __syncthreads();
     pdl_wait();               // the producer of sel / sel_count / the plan / the cache (and the previous user of the scratch) is done
     pdl_launch_dependents();  // the next kernel may be scheduled as SMs free up
 
@@ -217,22 +209,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             if (lse != nullptr && lane < G) lse[row + lane] = -INFINITY;
         }
     }
-    // the number of warps of the grid whose ranges meet positions [a, b) (a < b): what a unit's arrival counter reaches
-    auto warps_meeting = [&](int a, int b) -> int {
-        const unsigned pa = (unsigned)a >> 1, pb = ((unsigned)b - 1u) >> 1;
-        const unsigned cf = cs.owner(pa), cl = cs.owner(pb);
-        auto in_cta = [&](unsigned c, unsigned p_lo, unsigned p_hi) -> int {  // pairs p_lo..p_hi all lie in CTA c
-            const unsigned c0 = cs.begin(c), n = cs.begin(c + 1) - c0;
-            Split w;
-            w.b = n / kWarps; w.r = n % kWarps;
-            return (int)w.owner(p_hi - c0) - (int)w.owner(p_lo - c0) + 1;
-        };
-        if (cf == cl) return in_cta(cf, pa, pb);
-        int n = in_cta(cf, pa, cs.begin(cf + 1) - 1u) + in_cta(cl, cs.begin(cl), pb);
-#pragma unroll 1
-        for (unsigned c = cf + 1; c < cl; ++c) n += (int)min((unsigned)kWarps, cs.begin(c + 1) - cs.begin(c));
-        return n;
-    };
+    const int u_first = clo < chi ? find_unit(s_cum, g.n_units, clo) : 0;  // first unit of the CTA's range: slot 0 of its table
 
     int bbuilt = 0, gbuilt = 0;  // blocks / groups described so far
     int ucur = n_total > 0 ? find_unit(s_cum, g.n_units, lo) : 0;  // unit of the first block not yet described (warp-uniform)
@@ -342,27 +319,18 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     // phase 2 reads tokens 2qq, 2qq+1 of head gq
     const uint32_t zw = (uint32_t)(16 * qq + gq) * 4u, zr = (uint32_t)(8 * gq + 2 * qq) * 4u;
 
-    // The warp has seen every block it holds of cur_unit: publish its maxima (one atomic max per head) and arrive
-    // at the unit's counter.  One lane issues everything, so the release of the arrival covers the maxima.
+    // The warp has seen every block it holds of cur_unit: fold its maxima into the CTA's table
     auto publish_max = [&]() {
+        const int slot = cur_unit - u_first;
+        if (slot >= kCtaUnits) return;  // (a CTA that holds many tiny units: phase 2 rescans the warp's own logits)
 #pragma unroll
         for (int o = 4; o < 32; o <<= 1) {
             mxA = fmaxf(mxA, __shfl_xor_sync(kFull, mxA, o));
             mxB = fmaxf(mxB, __shfl_xor_sync(kFull, mxB, o));
         }
-        // lanes 0..3 hold heads 2qq, 2qq+1: bring them to lane 0
-        float m[kMaxGroup];
-#pragma unroll
-        for (int h = 0; h < kMaxGroup / 2; ++h) {
-            m[2 * h] = __shfl_sync(kFull, mxA, h);
-            m[2 * h + 1] = __shfl_sync(kFull, mxB, h);
-        }
-        if (lane == 0) {
-            uint32_t* um = scr.umax + (size_t)cur_unit * kMaxGroup;
-#pragma unroll
-            for (int h = 0; h < kMaxGroup; ++h)
-                if (h < G) atomicMax(um + h, fkey(m[h]));
-            red_release_add(scr.uarrive + cur_unit, 1);
+        if (gq == 0) {  // lanes 0..3 hold heads 2qq, 2qq+1
+            if (2 * qq < G) atomicMax(&s_umax[slot][2 * qq], fkey(mxA));
+            if (2 * qq + 1 < G) atomicMax(&s_umax[slot][2 * qq + 1], fkey(mxB));
         }
     };
 
@@ -469,14 +437,36 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 const float zA1 = v1 ? S[2] * scale_log2 : -INFINITY, zB1 = v1 ? S[3] * scale_log2 : -INFINITY;
                 mxA = fmaxf(mxA, fmaxf(zA0, zA1));
                 mxB = fmaxf(mxB, fmaxf(zB0, zB1));
-                if (bposc + 1 < zcap) {  // both blocks in the shared-memory cache
+                // block i of the range keeps its logits in shared memory iff i < zcap, else in global scratch
+                if (bposc < zcap) {
                     const uint32_t za = zs0 + (uint32_t)bposc * zstride + zw;
-                    if (2 * qq < G) { sts_f32(za, zA0); if (two) sts_f32(za + zstride, zA1); }
-                    if (2 * qq + 1 < G) { sts_f32(za + 32, zB0); if (two) sts_f32(za + zstride + 32, zB1); }
+                    if (2 * qq < G) sts_f32(za, zA0);
+                    if (2 * qq + 1 < G) sts_f32(za + 32, zB0);
                 } else {
                     float* z0 = scr.zbuf + (size_t)(lo + bposc) * (size_t)(8 * G) + (zw >> 2);
-                    if (2 * qq < G) { z0[0] = zA0; if (two) z0[8 * G] = zA1; }
-                    if (2 * qq + 1 < G) { z0[8] = zB0; if (two) z0[8 * G + 8] = zB1; }
+                    if (2 * qq < G) z0[0] = zA0;
+                    if (2 * qq + 1 < G) z0[8] = zB0;
+                }
+                if (two) {
+                    if (bposc + 1 < zcap) {
+                        const uint32_t za = zs0 + (uint32_t)(bposc + 1) * zstride + zw;
+                        if (2 * qq < G) sts_f32(za, zA1);
+                        if (2 * qq + 1 < G) sts_f32(za + 32, zB1);
+                    } else {
+                        float* z1 = scr.zbuf + (size_t)(lo + bposc + 1) * (size_t)(8 * G) + (zw >> 2);
+                        if (2 * qq < G) z1[0] = zA1;
+                        if (2 * qq + 1 < G) z1[8] = zB1;
+                    }
+                }
+            }
+            else {  // an invalid `sel` entry: its block takes no part; -inf keeps every later reader of the cache honest
+                if (bposc < zcap) {
+                    if (lane < 8 * G) sts_f32(zs0 + (uint32_t)bposc * zstride + 4u * (uint32_t)lane, -INFINITY);
+                    if (lane + 32 < 8 * G) sts_f32(zs0 + (uint32_t)bposc * zstride + 4u * (uint32_t)lane + 128u, -INFINITY);
+                } else {
+                    float* zg = scr.zbuf + (size_t)(lo + bposc) * (size_t)(8 * G) + lane;
+                    if (lane < 8 * G) zg[0] = -INFINITY;
+                    if (lane + 32 < 8 * G) zg[32] = -INFINITY;
                 }
             }
             __syncwarp();  // every lane is done reading the slot
@@ -487,15 +477,23 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         if (!kGatherOnly && cur_unit >= 0) publish_max();
     }
 
+    if (!kGatherOnly) __syncthreads();  // the CTA's table of maxima is complete
+
     // =====================================================================================
     // Phase 2: softmax sums over every selected token, PV over the blocks that matter.
     // =====================================================================================
     float acc[8][4];    // O^T tile i: rows gq / gq+8 = channels 16gq + 2i / + 1, columns 2qq, 2qq+1 = heads
     float lsum = 0.f;   // this lane's share of the softmax sum of head gq
-    float Mh = 0.f;     // the unit's maximum logit of head gq (log2 domain); 0 if the unit has no valid token
+    float Mh = 0.f;     // reference of head gq: the CTA's maximum logit of the unit (log2 domain); 0 if it holds no valid token
     float Mraw = -INFINITY;
     cur_unit = -1;
     unsigned st_vblocks = 0u, st_vbytes = 0u;
+
+    // logits of head gq, tokens 2qq, 2qq+1 of block i of the range (shared-memory cache, or global scratch beyond it)
+    auto z_pair = [&](int i) -> float2 {
+        if (i < zcap) return lds_f32x2(zs0 + (uint32_t)i * zstride + zr);
+        return __ldcg(reinterpret_cast<const float2*>(scr.zbuf + (size_t)(lo + i) * (size_t)(8 * G) + (zr >> 2)));
+    };
 
     // end of a unit inside this warp's range.  `last`: the range is finished and the ring is idle, so the
     // partial lives in this warp's own shared memory (record 2w + 1); a unit that ends inside the range
@@ -530,9 +528,6 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 if (hA < G) pl[hA] = lA > 0.f ? (mA + log2f(lA)) * kLn2 : -INFINITY;
                 if (hB < G) pl[hB] = lB > 0.f ? (mB + log2f(lB)) * kLn2 : -INFINITY;
             }
-            // only this warp ever read the unit's meeting state: reset it for the next launch
-            if (lane < kMaxGroup) scr.umax[(size_t)u * kMaxGroup + lane] = 0u;
-            if (lane == kMaxGroup) scr.uarrive[u] = 0;
         } else {
             const int rec = warp * 2 + (last ? 1 : 0);
             if (gq == 0) {
@@ -543,23 +538,43 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         }
     };
 
-    // wait until every warp that holds a part of unit u has published its maxima, then read them
-    auto begin_unit = [&](int u) {
+    // reference of unit u for this warp: the CTA's maxima; beyond the table, the maxima of the warp's own logits
+    // of the unit, which are blocks [p0, p1) of its range
+    auto begin_unit = [&](int u, int p0) {
         cur_unit = u;
         lsum = 0.f;
 #pragma unroll
         for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
-        if (lane == 0) {
-            const int expected = warps_meeting(s_cum[u], s_cum[u + 1]);
-            int it = 0;
+        const int slot = u - u_first;
+        if (slot < kCtaUnits) {
+            Mraw = gq < G ? funkey(s_umax[slot][gq]) : -INFINITY;
+        } else {
+            // lane l looks at elements l and l + 32 of each block's [head][token] floats: heads l / 8 and l / 8 + 4
+            const int p1 = min(n_total, s_cum[u + 1] - lo);
+            float m_lo = -INFINITY, m_hi = -INFINITY;
 #pragma unroll 1
-            while (ld_acquire(scr.uarrive + u) < expected) {
-                __nanosleep(100);  // leave the issue slots to the warps that are still in phase 1
-                if (++it > kSpinLimit) { atomicOr(dev_flags, MKV_DEV_SYNC_TIMEOUT); break; }
+            for (int i = p0; i < p1; ++i) {
+                float v0 = -INFINITY, v1 = -INFINITY;
+                if (i < zcap) {
+                    const uint32_t a = zs0 + (uint32_t)i * zstride + 4u * (uint32_t)lane;
+                    if (lane < 8 * G) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v0) : "r"(a));
+                    if (lane + 32 < 8 * G) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v1) : "r"(a + 128u));
+                } else {
+                    const float* zg = scr.zbuf + (size_t)(lo + i) * (size_t)(8 * G) + lane;
+                    if (lane < 8 * G) v0 = __ldcg(zg);
+                    if (lane + 32 < 8 * G) v1 = __ldcg(zg + 32);
+                }
+                m_lo = fmaxf(m_lo, v0);
+                m_hi = fmaxf(m_hi, v1);
             }
+#pragma unroll
+            for (int o = 1; o < 8; o <<= 1) {
+                m_lo = fmaxf(m_lo, __shfl_xor_sync(kFull, m_lo, o));
+                m_hi = fmaxf(m_hi, __shfl_xor_sync(kFull, m_hi, o));
+            }
+            const float t_lo = __shfl_sync(kFull, m_lo, 8 * (gq & 3)), t_hi = __shfl_sync(kFull, m_hi, 8 * (gq & 3));
+            Mraw = gq < G ? (gq < 4 ? t_lo : t_hi) : -INFINITY;
         }
-        __syncwarp();
-        Mraw = gq < G ? funkey(ld_relaxed_u32(scr.umax + (size_t)u * kMaxGroup + gq)) : -INFINITY;
         Mh = Mraw == -INFINITY ? 0.f : Mraw;
     };
 
@@ -581,7 +596,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 if (!kGatherOnly && u != cur_unit) {
                     if (pend != 0) break;  // drain the unit's groups in flight first
                     if (cur_unit >= 0) flush(false);
-                    begin_unit(u);
+                    begin_unit(u, bposd);
                 }
                 uint32_t nb0 = (d.y >> 20) & 15u, nb1 = (d.y >> 24) & 15u;
                 const bool two = nb1 != 0u;
@@ -591,15 +606,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                     // lane (gq, qq): head gq, tokens 2qq, 2qq+1 of each block
                     float2 za = make_float2(-INFINITY, -INFINITY), zb = za;
                     if (gq < G) {
-                        if (bposd + 1 < zcap) {
-                            const uint32_t a = zs0 + (uint32_t)bposd * zstride + zr;
-                            za = lds_f32x2(a);
-                            if (two) zb = lds_f32x2(a + zstride);
-                        } else {
-                            const float* z0 = scr.zbuf + (size_t)(lo + bposd) * (size_t)(8 * G) + (zr >> 2);
-                            za = __ldcg(reinterpret_cast<const float2*>(z0));
-                            if (two) zb = __ldcg(reinterpret_cast<const float2*>(z0 + 8 * G));
-                        }
+                        za = z_pair(bposd);
+                        if (two) zb = z_pair(bposd + 1);
                     }
                     add = (ex2(za.x - Mh) + ex2(za.y - Mh)) + (ex2(zb.x - Mh) + ex2(zb.y - Mh));
                     need0 = __any_sync(kFull, fmaxf(za.x, za.y) - Mh >= -kSkip);
@@ -658,15 +666,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             // exactly the B fragments of O^T += V^T P^T (k = token, n = head)
             float2 za = make_float2(-INFINITY, -INFINITY), zb = za;
             if (gq < G) {
-                if (pos + 1 < zcap) {  // (the same test as when the group's logits were stored)
-                    const uint32_t a = zs0 + ((uint32_t)pos + zsh) * zstride + zr;
-                    za = lds_f32x2(a);
-                    if (two) zb = lds_f32x2(a + zstride);
-                } else {
-                    const float* z0 = scr.zbuf + (size_t)(lo + pos + (int)zsh) * (size_t)(8 * G) + (zr >> 2);
-                    za = __ldcg(reinterpret_cast<const float2*>(z0));
-                    if (two) zb = __ldcg(reinterpret_cast<const float2*>(z0 + 8 * G));
-                }
+                za = z_pair(pos + (int)zsh);
+                if (two) zb = z_pair(pos + (int)zsh + 1);
             }
             const float e00 = ex2(za.x - Mh), e01 = ex2(za.y - Mh), e10 = ex2(zb.x - Mh), e11 = ex2(zb.y - Mh);
             const uint32_t ph0 = pack_bf16(e00, e01), ph1 = pack_bf16(e10, e11);
@@ -774,28 +775,40 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         const size_t row = (size_t)(mine / g.n_kv_heads) * g.n_q_heads + (size_t)(mine % g.n_kv_heads) * G;
         float4 O = make_float4(0.f, 0.f, 0.f, 0.f);
         float Lr = 0.f, Mr = -INFINITY;
-        // head partials (record 2w, in global scratch): at most one per CTA in practice (the unit entering its range)
-#pragma unroll 1
-        for (unsigned m = recs & 0x55555555u; m; m &= m - 1u) {
-            const int w = (__ffs(m) - 1) >> 1;
-            Mr = s_ml[2 * w][h][0];
-            Lr += s_ml[2 * w][h][1];
-            const float4 o = __ldcg(reinterpret_cast<const float4*>(
-                scr.part_o + ((size_t)blockIdx.x * kWarps + w) * 2 * (size_t)GD + e));
-            O.x += o.x; O.y += o.y; O.z += o.z; O.w += o.w;
-        }
-        // tail partials (record 2w + 1, in warp w's shared memory): straight-line, every load independent
+        {
+            // tail partials (record 2w + 1, in warp w's shared memory): straight-line, every load independent
+            float mw[kWarps], lw[kWarps];
+            float4 ow[kWarps];
 #pragma unroll
-        for (int w = 0; w < kWarps; ++w) {
-            const bool mem = (recs >> (2 * w + 1)) & 1u;
-            const float2 ml = *reinterpret_cast<const float2*>(&s_ml[2 * w + 1][h][0]);
-            const float4 o = *reinterpret_cast<const float4*>(smem + w * kWS + 4 * e);
-            if (mem) { Mr = ml.x; Lr += ml.y; O.x += o.x; O.y += o.y; O.z += o.z; O.w += o.w; }
+            for (int w = 0; w < kWarps; ++w) {
+                const bool mem = (recs >> (2 * w + 1)) & 1u;
+                const float2 ml = *reinterpret_cast<const float2*>(&s_ml[2 * w + 1][h][0]);
+                ow[w] = *reinterpret_cast<const float4*>(smem + w * kWS + 4 * e);
+                mw[w] = mem ? ml.x : -INFINITY;
+                lw[w] = mem ? ml.y : 0.f;
+                Mr = fmaxf(Mr, mw[w]);
+            }
+            // head partials (record 2w, in global scratch): at most one per CTA in practice (the unit entering its range)
+#pragma unroll 1
+            for (unsigned m = recs & 0x55555555u; m; m &= m - 1u) Mr = fmaxf(Mr, s_ml[2 * ((__ffs(m) - 1) >> 1)][h][0]);
+            const float Mb = Mr == -INFINITY ? 0.f : Mr;
+#pragma unroll
+            for (int w = 0; w < kWarps; ++w) {
+                const float wt = ex2(mw[w] - Mb);  // 1 inside a CTA's table; 0 for a record of another unit (its O may be stale bits)
+                Lr = fmaf(lw[w], wt, Lr);
+                if (wt != 0.f) { O.x = fmaf(ow[w].x, wt, O.x); O.y = fmaf(ow[w].y, wt, O.y); O.z = fmaf(ow[w].z, wt, O.z); O.w = fmaf(ow[w].w, wt, O.w); }
+            }
+#pragma unroll 1
+            for (unsigned m = recs & 0x55555555u; m; m &= m - 1u) {
+                const int w = (__ffs(m) - 1) >> 1;
+                const float wt = ex2(s_ml[2 * w][h][0] - Mb);
+                Lr = fmaf(s_ml[2 * w][h][1], wt, Lr);
+                const float4 o = __ldcg(reinterpret_cast<const float4*>(
+                    scr.part_o + ((size_t)blockIdx.x * kWarps + w) * 2 * (size_t)GD + e));
+                O.x = fmaf(o.x, wt, O.x); O.y = fmaf(o.y, wt, O.y); O.z = fmaf(o.z, wt, O.z); O.w = fmaf(o.w, wt, O.w);
+            }
         }
         if (whole) {
-            // wholly inside this CTA and past phase 2 in every warp: reset its meeting state for the next launch
-            if (e < 4 * kMaxGroup) scr.umax[(size_t)mine * kMaxGroup + (e >> 2)] = 0u;
-            if (e == 4 * kMaxGroup) scr.uarrive[mine] = 0;
             const float inv = Lr > 0.f ? 1.f / Lr : 0.f;
             *reinterpret_cast<float4*>(out + row * kD + e) = make_float4(O.x * inv, O.y * inv, O.z * inv, O.w * inv);
             if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = Lr > 0.f ? (Mr + log2f(Lr)) * kLn2 : -INFINITY;
@@ -814,28 +827,30 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         int old;  // release this thread's partial, acquire the other sharers'
         asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(tk) : "memory");
         if (old != c_last - c_first) continue;
-        *tk = 0;  // self-cleaning: every sharer has arrived (and is past phase 2)
-        if (e < 4 * kMaxGroup) scr.umax[(size_t)mine * kMaxGroup + (e >> 2)] = 0u;
-        if (e == 4 * kMaxGroup) scr.uarrive[mine] = 0;
+        *tk = 0;  // self-cleaning: every sharer has arrived
         float Mx = -INFINITY, Lx = 0.f;
         float4 Ox = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 1
-        for (int c0 = c_first; c0 <= c_last; c0 += 4) {  // four partials' loads in flight at once
+        for (int c0 = c_first; c0 <= c_last; c0 += 4) {  // four partials' loads in flight at once; LSE rule (oracle pin P10)
             float2 pm[4];
             float4 po[4];
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
-                const int c = min(c0 + t, c_last);  // a repeated partial is not added below
+                const int c = min(c0 + t, c_last);  // a repeated partial gets weight 0 below
                 const size_t sl = cta_slot_base + (size_t)c * 2 + (c == c_first ? 1 : 0);
                 pm[t] = __ldcg(reinterpret_cast<const float2*>(scr.part_l + sl * (2 * kMaxGroup) + 2 * h));
                 po[t] = __ldcg(reinterpret_cast<const float4*>(scr.part_o + sl * (size_t)GD + e));
+                if (c0 + t > c_last) pm[t] = make_float2(-INFINITY, 0.f);
             }
+            const float Mn = fmaxf(fmaxf(Mx, fmaxf(pm[0].x, pm[1].x)), fmaxf(pm[2].x, pm[3].x));
+            const float Mb = Mn == -INFINITY ? 0.f : Mn;
+            const float c_old = ex2(Mx - Mb);
+            Lx *= c_old; Ox.x *= c_old; Ox.y *= c_old; Ox.z *= c_old; Ox.w *= c_old; Mx = Mn;
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
-                if (c0 + t > c_last) continue;
-                Mx = pm[t].x;
-                Lx += pm[t].y;
-                Ox.x += po[t].x; Ox.y += po[t].y; Ox.z += po[t].z; Ox.w += po[t].w;
+                const float w = ex2(pm[t].x - Mb);
+                Lx = fmaf(pm[t].y, w, Lx);
+                if (w != 0.f) { Ox.x = fmaf(po[t].x, w, Ox.x); Ox.y = fmaf(po[t].y, w, Ox.y); Ox.z = fmaf(po[t].z, w, Ox.z); Ox.w = fmaf(po[t].w, w, Ox.w); }
             }
         }
         const float inv = Lx > 0.f ? 1.f / Lx : 0.f;
@@ -886,28 +901,27 @@ template <bool GATHER>
 static cudaError_t launch_attention_cfg(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
                                         const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
                                         const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v,
-                                        const int32_t* upd_count, uint32_t* dev_flags, int sm_count, cudaStream_t s) {
+                                        const int32_t* upd_count, int sm_count, cudaStream_t s) {
     const int smem = kWarps * kWS + (g.n_units + 1) * 4;
     // the dynamic shared-memory opt-in is a per-device attribute of the function: set it on every launch (a cheap
     // host-side call) so that caches on different devices of one process are independent
     cudaError_t e = cudaFuncSetAttribute(mkv_packed_attention_kernel<GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     return launch_pdl(mkv_packed_attention_kernel<GATHER>, dim3(sm_count), dim3(kWarps * 32), (size_t)smem, s, g, lv, q, sel,
-                      sel_count, k_max, scale * kLog2e, out, lse, scr, upd_k, upd_v, upd_count, dev_flags);
+                      sel_count, k_max, scale * kLog2e, out, lse, scr, upd_k, upd_v, upd_count);
 }
 
 cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
                              const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
                              const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v,
-                             const int32_t* upd_count, uint32_t* dev_flags, int sm_count, cudaStream_t s, int* n_kernels,
-                             bool gather_only) {
+                             const int32_t* upd_count, int sm_count, cudaStream_t s, int* n_kernels, bool gather_only) {
     if (g.n_units > kMaxUnitsSmem) return cudaErrorInvalidValue;
     if (n_kernels) *n_kernels = 1;
     if (gather_only)
         return launch_attention_cfg<true>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, upd_count,
-                                          dev_flags, sm_count, s);
+                                          sm_count, s);
     return launch_attention_cfg<false>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, upd_count,
-                                       dev_flags, sm_count, s);
+                                       sm_count, s);
 }
 
 cudaError_t launch_stream_read(const uint8_t* base, unsigned long long bytes, int sm_count, unsigned long long* sink,

@@ -106,7 +106,7 @@ int mkv_cache_free(mkv_cache* c) {
     cudaSetDevice(c->desc.device);
     cudaDeviceSynchronize();
     void* ptrs[] = {c->arena, c->strat, c->tok_off, c->bk_off, c->unit_nseg, c->unit_ntok, c->counters,
-                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->upd_k, c->upd_v, c->upd_cnt, c->attn.part_o, c->attn.part_l, c->attn.ticket, c->attn.umax, c->attn.uarrive, c->attn.zbuf, c->attn.stats, c->plan, c->sink, c->q_dev,
+                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->upd_k, c->upd_v, c->upd_cnt, c->attn.part_o, c->attn.part_l, c->attn.ticket, c->attn.zbuf, c->attn.stats, c->plan, c->sink, c->q_dev,
                     c->sel_dev, c->selcnt_dev, c->out_dev};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -175,8 +175,6 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         {(void**)&c->attn.part_o, (size_t)c->attn.slots * g.group * kD * 4},
         {(void**)&c->attn.part_l, (size_t)c->attn.slots * kMaxGroup * 2 * 4},
         {(void**)&c->attn.ticket, attention_ticket_ints(g) * 4},
-        {(void**)&c->attn.umax, (size_t)g.n_units * kMaxGroup * 4},
-        {(void**)&c->attn.uarrive, (size_t)g.n_units * 4},
         {(void**)&c->attn.zbuf, attention_zbuf_floats(g) * 4},
         {(void**)&c->attn.stats, 64},
         {(void**)&c->plan, tu * (size_t)c->sel_cap * sizeof(PlanRec)},
@@ -200,8 +198,6 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     cudaMemset(c->dev_flags, 0, 256);
     cudaMemset(c->upd_cnt, 0, (size_t)g.n_layers * 4);
     cudaMemset(c->attn.ticket, 0, attention_ticket_ints(g) * 4);
-    cudaMemset(c->attn.umax, 0, (size_t)g.n_units * kMaxGroup * 4);
-    cudaMemset(c->attn.uarrive, 0, (size_t)g.n_units * 4);
     cudaMemset(c->attn.stats, 0, 64);
     cudaMemset(c->plan, 0, tu * (size_t)c->sel_cap * sizeof(PlanRec));
     cudaMemset(c->strat, 0, tu * g.S_max * sizeof(StratRec));
@@ -223,9 +219,7 @@ int mkv_cache_reset(mkv_cache* c, int32_t layer, void* stream) {
     cudaStream_t s = (cudaStream_t)stream;
     const int l0 = layer < 0 ? 0 : layer, l1 = layer < 0 ? g.n_layers : layer + 1;
     ++c->generation;  // plan records written before the reset no longer match
-    MKV_CUDA(cudaMemsetAsync(c->attn.ticket, 0, attention_ticket_ints(g) * 4, s));  // (a launch that timed out leaves these dirty)
-    MKV_CUDA(cudaMemsetAsync(c->attn.umax, 0, (size_t)g.n_units * kMaxGroup * 4, s));
-    MKV_CUDA(cudaMemsetAsync(c->attn.uarrive, 0, (size_t)g.n_units * 4, s));
+    MKV_CUDA(cudaMemsetAsync(c->attn.ticket, 0, attention_ticket_ints(g) * 4, s));
     for (int l = l0; l < l1; ++l) {
         MKV_CUDA(cudaMemsetAsync(c->unit_nseg + (size_t)l * g.n_units, 0, (size_t)g.n_units * 4, s));
         MKV_CUDA(cudaMemsetAsync(c->unit_ntok + (size_t)l * g.n_units, 0, (size_t)g.n_units * 4, s));
@@ -341,7 +335,7 @@ int mkv_packed_attention(const mkv_cache* cc, int32_t layer, const void* q, cons
     const size_t upd_off = (size_t)layer * g.n_units * g.L * kD;
     MKV_CUDA(launch_attention(g, c->view(layer), (const uint16_t*)q, sel, sel_count, k_max, scale, out, lse_opt,
                               c->attn_scratch(layer), c->upd_k + upd_off, c->upd_v + upd_off, c->upd_cnt + layer,
-                              c->dev_flags, c->sm_count, (cudaStream_t)stream, &c->last_attn));
+                              c->sm_count, (cudaStream_t)stream, &c->last_attn));
     return MKV_OK;
 }
 
@@ -357,7 +351,7 @@ int mkv_calibrate_gather(const mkv_cache* cc, int32_t layer, const int32_t* sel,
     int n = 0;
     MKV_CUDA(launch_attention(g, c->view(layer), c->q_dev, sel, sel_count, k_max, 1.f, c->out_dev, nullptr,
                               c->attn_scratch(layer), c->upd_k + upd_off, c->upd_v + upd_off, c->upd_cnt + layer,
-                              c->dev_flags, c->sm_count, (cudaStream_t)stream, &n, true));
+                              c->sm_count, (cudaStream_t)stream, &n, true));
     return MKV_OK;
 }
 
@@ -572,8 +566,8 @@ int mkv_cache_status(const mkv_cache* c, uint32_t* flags_host) {
     uint32_t f = 0;
     MKV_CUDA(cudaMemcpy(&f, c->dev_flags, 4, cudaMemcpyDeviceToHost));
     if (flags_host) *flags_host = f;
-    if (f) return fail(MKV_E_DEVICE, "device flags 0x%x (%s%s%s)", f, (f & MKV_DEV_ARENA_OVERFLOW) ? "arena overflow " : "",
-                       (f & MKV_DEV_BAD_STRATEGY) ? "bad strategy " : "", (f & MKV_DEV_SYNC_TIMEOUT) ? "attention sync timeout" : "");
+    if (f) return fail(MKV_E_DEVICE, "device flags 0x%x (%s%s)", f, (f & MKV_DEV_ARENA_OVERFLOW) ? "arena overflow " : "",
+                       (f & MKV_DEV_BAD_STRATEGY) ? "bad strategy" : "");
     return MKV_OK;
 }
 

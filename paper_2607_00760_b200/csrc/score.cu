@@ -12,8 +12,6 @@
 //   * The packed keys are expanded straight into mma.sync A fragments by the same walk as
 //     PackedAttention's QK (mkv_walk.cuh): S = Kbar q^T, keys = M, heads = N, channels = K, fp32
 //     accumulate; the group reduction (max or sum over the G heads) is two shuffles.
-#include <cstdlib>
-
 #include "mkv_internal.cuh"
 #include "mkv_walk.cuh"
 
@@ -251,33 +249,19 @@ template <int NSTAGE, int NWARPS>
 static cudaError_t launch_score_cfg(const CacheGeom& g, const LayerView& lv, const uint16_t* q, int reduce,
                                     float* scores, int sm_count, cudaStream_t s) {
     const int smem = NWARPS * score_warp_smem(NSTAGE);
-    static int configured = 0;
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(mkv_score_kernel<NSTAGE, NWARPS>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
+    // (a per-device attribute of the function: set on every launch, see attention.cu)
+    cudaError_t e = cudaFuncSetAttribute(mkv_score_kernel<NSTAGE, NWARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
     const int subs = (g.blocks_per_seg + 7) / 8;
     if ((unsigned long long)g.n_units * g.S_max * subs >= (1ull << 32)) return cudaErrorInvalidValue;
     return launch_pdl(mkv_score_kernel<NSTAGE, NWARPS>, dim3(sm_count), dim3(NWARPS * 32), (size_t)smem, s, g, lv, q, reduce,
                       subs, (unsigned)g.S_max * (unsigned)subs, scores);
 }
 
+// two stages x 32 warps: the kernel needs 64 registers, and warps are what hides the walk's dependent loads
 cudaError_t launch_score(const CacheGeom& g, const LayerView& lv, const uint16_t* q, int reduce, float* scores,
                          int sm_count, cudaStream_t s) {
-    static int cfg = -1;  // tuning knob (stages * 100 + warps); default chosen from measurements
-    if (cfg < 0) {
-        const char* e = getenv("MKV_SCORE_CFG");
-        cfg = e ? atoi(e) : 232;
-    }
-#define MKV_CFG(S, W) \
-    case S * 100 + W: return launch_score_cfg<S, W>(g, lv, q, reduce, scores, sm_count, s);
-    switch (cfg) {
-        MKV_CFG(2, 32) MKV_CFG(3, 24) MKV_CFG(2, 24) MKV_CFG(3, 16) MKV_CFG(4, 16)
-        default: return launch_score_cfg<2, 32>(g, lv, q, reduce, scores, sm_count, s);
-    }
-#undef MKV_CFG
+    return launch_score_cfg<2, 32>(g, lv, q, reduce, scores, sm_count, s);
 }
 
 }  // namespace mkv
