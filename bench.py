@@ -28,9 +28,10 @@ METRIC = "PackedAttention us/layer (8B-shape, 128K ctx, batch 8)"
 UNIT = "us/layer"
 NOMINAL_HBM_GBS = 8000.0
 FALLBACK_HBM_GBS = 6650.0
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r1f_final.md), valid for the full-size default workload only
-NCU_TRAFFIC = {"llama8b-128k-b8": {"attention": 53400000 + 430000, "score+topk": 115741000 + 4806000 + 4236000}}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the committed `ncu --set full` captures.  NOT measured by
+# this run: printed under "traffic_from_capture" with the file it came from; "traffic" itself stays null.
+NCU_CAPTURE = {"llama8b-128k-b8": {"source": "profiles/r2_final.md (ncu --set full, 2 layers)",
+                                   "attention": None, "score+topk": None}}
 
 
 def parse():
@@ -47,7 +48,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-units", type=int, default=8, help="units of one layer the oracle is timed on")
     ap.add_argument("--sweep", action="store_true",
-                    help="BASELINE config 5: keep ratio x token budget on the config-2 shape, 2 layers per point")
+                    help="BASELINE config 5: keep ratio x token budget on the config-2 shape, 6 layers per point")
+    ap.add_argument("--sweep-layers", type=int, default=6, help="layers cycled per sweep point (6 x >= 20 MB > L2)")
     ap.add_argument("--verbose", action="store_true")
     return ap.parse_args()
 
@@ -115,9 +117,10 @@ class ClockSampler:
 
 # ------------------------------------------------------------------------------ timing helpers
 
-def timed_loop(torch, fn, steps, warmup, dist_barrier, graph=True):
-    """W untimed + K timed calls of fn() on torch's current stream; returns ms per call.
-    fn's launches are captured in one CUDA graph (launch-bound inner loop) unless graph=False."""
+def timed_loop(torch, fn, steps, warmup, dist_barrier, graph=True, stats=None):
+    """W untimed + K timed calls of fn() on torch's current stream; returns ms per call (mean over the K calls).
+    fn's launches are captured in one CUDA graph (launch-bound inner loop) unless graph=False.  If `stats` is a dict
+    it receives the median and the minimum of the K per-call times (events between the calls)."""
     stream = torch.cuda.current_stream()
     runner = fn
     if graph:
@@ -129,16 +132,19 @@ def timed_loop(torch, fn, steps, warmup, dist_barrier, graph=True):
         runner = g.replay
     for _ in range(warmup):
         runner()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
     dist_barrier()
     torch.cuda.synchronize()
-    e0.record(stream)
-    for _ in range(steps):
+    ev[0].record(stream)
+    for i in range(steps):
         runner()
-    e1.record(stream)
+        ev[i + 1].record(stream)
     torch.cuda.synchronize()
     dist_barrier()
-    return e0.elapsed_time(e1) / steps
+    if stats is not None:
+        per = sorted(ev[i].elapsed_time(ev[i + 1]) for i in range(steps))
+        stats["median_ms"], stats["min_ms"] = per[len(per) // 2], per[0]
+    return ev[0].elapsed_time(ev[steps]) / steps
 
 
 def max_over_ranks(torch, dist, x, world):
@@ -208,24 +214,47 @@ def run_mkv(args):
     cache.status()
     launches = cache.last_launch_count()
     n_sel_total = [int(c.sum().item()) for c in cnt]
-    attn_bytes = [workload.attention_bytes(built, l, sel[l], cnt[l]) for l in range(n_layers)]
+    attn_split = [workload.attention_bytes(built, l, sel[l], cnt[l], split=True) for l in range(n_layers)]
+    attn_bytes = [x[0] for x in attn_split]
+    v_parts = sum(x[2] for x in attn_split) / n_layers
     sel_bytes = [workload.select_bytes(built, l, n_sel_total[l]) for l in range(n_layers)]
     comp_bytes = workload.compress_bytes(built, 0)
 
     graph = not args.no_graph
     clocks = ClockSampler(local)
     clocks.start()
-    ms_step = timed_loop(torch, step_decode, args.steps, args.warmup, barrier, graph)
-    ms_attn = timed_loop(torch, step_attention, args.steps, args.warmup, barrier, graph)
-    ms_sel = timed_loop(torch, step_select, args.steps, args.warmup, barrier, graph)
+    st_step, st_attn, st_sel = {}, {}, {}
+    ms_step = timed_loop(torch, step_decode, args.steps, args.warmup, barrier, graph, st_step)
+    cache.attention_stats(reset=True)
+    ms_attn = timed_loop(torch, step_attention, args.steps, args.warmup, barrier, graph, st_attn)
+    stats = cache.attention_stats(reset=True)
+    ms_sel = timed_loop(torch, step_select, args.steps, args.warmup, barrier, graph, st_sel)
     clk = clocks.stop()
 
-    # calibration: the attention kernel's own staging of the same selected payloads with all arithmetic removed
+    # the same selection attended with q = 0 (flat softmax: phase 2 may skip nothing, every V part is fetched)
+    q_zero = [torch.zeros_like(x) for x in built.q]
+
+    def step_attention_flat():
+        for l in range(n_layers):
+            cache.packed_attention(l, q_zero[l], sel[l], cnt[l], scale, out[l])
+
+    ms_flat = timed_loop(torch, step_attention_flat, args.steps, args.warmup, barrier, graph)
+    stats_flat = cache.attention_stats(reset=True)
+
+    # calibration: (ii) the attention kernel's own staging of the same selected payloads (K parts, then V
+    # parts, nothing skipped) with all arithmetic removed; (i) a plain streaming read of the same number of bytes
     def step_gather():
         for l in range(n_layers):
             cache.calibrate_gather(l, sel[l], cnt[l])
 
     ms_gather = timed_loop(torch, step_gather, args.steps, args.warmup, barrier, graph)
+    a_bytes_int = int(sum(attn_bytes) / n_layers)
+
+    def step_stream():
+        for l in range(n_layers):
+            cache.calibrate_stream(l, a_bytes_int)
+
+    ms_stream = timed_loop(torch, step_stream, args.steps, args.warmup, barrier, graph)
 
     # end to end through the public host call: pinned q in, out back, every layer, every step
     q_host = [q.cpu().pin_memory() for q in built.q]
@@ -257,7 +286,13 @@ def run_mkv(args):
     comp_gbs = (comp_bytes["read"] + comp_bytes["write"]) / (comp_ms[2] * 1e-3) / 1e9
 
     full_size = Bt == w.batch and N == w.context
-    traffic = NCU_TRAFFIC.get(w.name, {}) if full_size else {}
+    cap = NCU_CAPTURE.get(w.name, {}) if full_size else {}
+    # bytes the kernel actually fetched per launch: everything but the V parts phase 2 skipped (the kernel counts the
+    # blocks it walked and the bytes of their V copies; ratios are independent of how many launches fed the counters)
+    v_frac = stats["v_blocks"] / max(1, stats["blocks"])
+    sel_blocks = sum(n_sel_total) / n_layers
+    bytes_fetched = int(a_bytes - v_parts + stats["v_bytes"] / max(1, stats["blocks"]) * sel_blocks)
+    us_attn_in_step = (ms_step - ms_sel) * 1e3 / n_layers
     line = {
         "metric": METRIC, "value": round(us_attn, 3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": False, "scaling": "weak",
@@ -270,26 +305,46 @@ def run_mkv(args):
                    "launch": "cuda-graph of one decode step" if graph else "eager"},
         "decode_tokens_per_s_attention_only": round(world * Bt / (ms_step * 1e-3), 1),
         "select_us_per_layer": round(us_sel, 3),
+        "attention_us_per_layer": {"mean": round(us_attn, 3), "median": round(st_attn["median_ms"] * 1e3 / n_layers, 3),
+                                   "min": round(st_attn["min_ms"] * 1e3 / n_layers, 3),
+                                   "inside_decode_step": round(us_attn_in_step, 3),
+                                   "flat_softmax_q0": round(ms_flat * 1e3 / n_layers, 3)},
         "roofline": {"kernel": "mkv_packed_attention", "bound": "hbm", "achieved": round(attn_gbs, 1), "peak": peak,
-                     "unit": "GB/s", "frac": round(attn_gbs / peak, 4), "traffic": traffic.get("attention"),
+                     "unit": "GB/s", "frac": round(attn_gbs / peak, 4), "traffic": None,
+                     "traffic_from_capture": {"bytes": cap.get("attention"), "source": cap.get("source")},
                      "peak_source": peak_src,
                      "frac_of_nominal_8TBs": round(attn_gbs / NOMINAL_HBM_GBS, 4),
-                     "algorithmic_bytes_per_launch": int(a_bytes)},
+                     "algorithmic_bytes_per_launch": int(a_bytes),
+                     "what": "frac = algorithmic bytes (every selected K and V payload, SURVEY 8(d)) / time / peak.  The kernel "
+                             "fetches every K part but only the V parts of blocks with a probability >= 2^-40 of the CTA's "
+                             "largest (bytes_fetched_per_launch, from the kernel's counters), so frac is NOT the DRAM rate",
+                     "v_blocks_fetched_fraction": round(v_frac, 4),
+                     "bytes_fetched_per_launch": bytes_fetched,
+                     "frac_on_bytes_fetched": round((bytes_fetched or 0) / (us_attn * 1e-6) / 1e9 / peak, 4),
+                     "flat_softmax_q0": {"us_per_layer": round(ms_flat * 1e3 / n_layers, 3),
+                                         "v_blocks_fetched_fraction": round(stats_flat["v_blocks"] / max(1, stats_flat["blocks"]), 4),
+                                         "frac": round(a_bytes / (ms_flat * 1e-3 / n_layers) / 1e9 / peak, 4)}},
         "roofline_select": {"kernel": "mkv_select", "bound": "hbm", "achieved": round(sel_gbs, 1), "peak": peak,
-                            "unit": "GB/s", "frac": round(sel_gbs / peak, 4), "traffic": traffic.get("score+topk"),
+                            "unit": "GB/s", "frac": round(sel_gbs / peak, 4), "traffic": None,
+                            "traffic_from_capture": {"bytes": cap.get("score+topk"), "source": cap.get("source")},
                             "algorithmic_bytes_per_launch": int(s_bytes)},
         "compress": {"loss_ms_per_layer": round(float(comp_ms[0]), 3), "strategy_ms_per_layer": round(float(comp_ms[1]), 3),
                      "compress_ms_per_layer": round(float(comp_ms[2]), 3), "achieved": round(comp_gbs, 1), "unit": "GB/s",
                      "frac": round(comp_gbs / peak, 4), "bytes_read": comp_bytes["read"], "bytes_written": comp_bytes["write"],
                      "build_all_layers_s": round(build_s, 2)},
-        "e2e": {"value": round(ms_e2e * 1e3 / n_layers, 3), "unit": "us/layer (select + attention, host q in, host out back)",
+        "e2e": {"value": round(ms_e2e * 1e3 / n_layers, 3), "unit": UNIT,
+                "what": "select + attention through mkv_decode_host: pinned host q in, host out back, both copies timed",
                 "launch": "cuda-graph of one decode step of mkv_decode_host calls" if graph else "eager, synchronised per step",
                 "h2d_bytes_per_step": n_layers * Bt * Hq * 128 * 2, "d2h_bytes_per_step": n_layers * Bt * Hq * 128 * 4,
                 "ms_per_step": round(ms_e2e, 4)},
-        "calibration": {"gather_only_us_per_layer": round(ms_gather * 1e3 / n_layers, 3),
+        "calibration": {"stream_read_us_per_layer": round(ms_stream * 1e3 / n_layers, 3),
+                        "stream_read_gbs": round(a_bytes / (ms_stream * 1e-3 / n_layers) / 1e9, 1),
+                        "gather_only_us_per_layer": round(ms_gather * 1e3 / n_layers, 3),
                         "gather_only_gbs": round(a_bytes / (ms_gather * 1e-3 / n_layers) / 1e9, 1),
-                        "what": "mkv_calibrate_gather: same kernel, launch configuration and selected payloads as "
-                                "mkv_packed_attention, bulk-copy staging only (no walk, no MMA, no output)"},
+                        "what": "stream_read: mkv_calibrate_stream, a plain 16-byte-load read of algorithmic_bytes_per_launch bytes of "
+                                "the layer's arena in the attention kernel's launch shape (148 x 512).  gather_only: "
+                                "mkv_calibrate_gather, the attention kernel's own staging of every selected K part then every V "
+                                "part (bulk copies into the warps' rings, nothing skipped), no walk, no MMA, no output"},
         "gpu_launches": args.steps * n_layers * (launches["select"] + launches["attention"]),
         "kernels_per_layer": launches,
         "clocks": clk,
@@ -462,15 +517,16 @@ def run_reference(args):
                        "context": N, "token_budget": w.token_budget, "r_keep": w.r_keep},
             "cpu_baseline": {"value": round(value, 1), "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
                              "select_plus_attention_us_per_layer": round(t_dec * scale_up * 1e6, 1)},
-            "e2e": {"value": round(value, 1), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "e2e": {"value": round(t_dec * scale_up * 1e6, 1), "unit": UNIT, "what": "oracle select + attention on the sample, scaled to one layer",
+                    "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
 def run_sweep(args):
     """BASELINE config 5 on one GPU: keep ratio in {1.0, 0.7, 0.5, 0.3} x token budget in {1024, 4096, 16384} (the 10 %
-    dense mix held fixed) plus the dense-full point (r = 128, budget = context).  Two layers per point so that
-    consecutive launches read different arenas (each far larger than L2).  Prints one JSON line."""
+    dense mix held fixed) plus the dense-full point (r = 128, budget = context).  Six layers are cycled per point so
+    that the set touched between two visits of a layer exceeds the 126 MB L2 at every point.  Prints one JSON line."""
     import dataclasses
     import torch
     import __graft_entry__
@@ -482,37 +538,39 @@ def run_sweep(args):
     Bt, N = args.batch or base.batch, args.context or base.context
     peak, peak_src = measured_peak()
     scale = 1.0 / math.sqrt(128)
+    NL = max(2, args.sweep_layers)  # layers cycled per point: >= 6 x the touched set exceeds the 126 MB L2 at every point
     points = []
     for keep in (1.0, 0.7, 0.5, 0.3):
         w = dataclasses.replace(base, keep_ratio=keep)
-        built = workload.build(w, dev, n_layers=2, batch=Bt, context=N)
+        built = workload.build(w, dev, n_layers=NL, batch=Bt, context=N)
         cache, Hkv, Hq = built.cache, w.n_kv_heads, w.n_q_heads
         budgets = [1024, 4096, 16384] + ([N] if keep == 1.0 else [])
         for budget in budgets:
             k_max = min(budget // 8 + 1, (N + 7) // 8)
-            sel = [torch.full((Bt, Hkv, k_max), -1, dtype=torch.int32, device=dev) for _ in range(2)]
-            cnt = [torch.zeros((Bt, Hkv), dtype=torch.int32, device=dev) for _ in range(2)]
-            out = torch.zeros((2, Bt, Hq, 128), dtype=torch.float32, device=dev)
-            for l in range(2):
+            sel = [torch.full((Bt, Hkv, k_max), -1, dtype=torch.int32, device=dev) for _ in range(NL)]
+            cnt = [torch.zeros((Bt, Hkv), dtype=torch.int32, device=dev) for _ in range(NL)]
+            out = torch.zeros((NL, Bt, Hq, 128), dtype=torch.float32, device=dev)
+            for l in range(NL):
                 cache.select(l, built.q[l], budget, sel[l], cnt[l])
             torch.cuda.synchronize()
 
             def step_attention():
-                for l in range(2):
+                for l in range(NL):
                     cache.packed_attention(l, built.q[l], sel[l], cnt[l], scale, out[l])
 
             def step_select():
-                for l in range(2):
+                for l in range(NL):
                     cache.select(l, built.q[l], budget, sel[l], cnt[l])
 
             ms_a = timed_loop(torch, step_attention, args.steps, max(3, args.warmup), lambda: None, True)
             ms_s = timed_loop(torch, step_select, args.steps, max(3, args.warmup), lambda: None, True)
             cache.status()
-            ab = sum(workload.attention_bytes(built, l, sel[l], cnt[l]) for l in range(2)) / 2
-            us = ms_a * 1e3 / 2
+            cache.attention_stats(reset=True)
+            ab = sum(workload.attention_bytes(built, l, sel[l], cnt[l]) for l in range(NL)) / NL
+            us = ms_a * 1e3 / NL
             gbs = ab / (us * 1e-6) / 1e9
             points.append({"keep_ratio": keep, "r_keep": w.r_keep, "token_budget": budget,
-                           "attention_us_per_layer": round(us, 2), "select_us_per_layer": round(ms_s * 1e3 / 2, 2),
+                           "attention_us_per_layer": round(us, 2), "select_us_per_layer": round(ms_s * 1e3 / NL, 2),
                            "algorithmic_bytes_per_launch": int(ab), "achieved_gbs": round(gbs, 1),
                            "frac": round(gbs / peak, 4), "frac_of_nominal_8TBs": round(gbs / NOMINAL_HBM_GBS, 4)})
             del sel, cnt, out
@@ -521,7 +579,7 @@ def run_sweep(args):
         torch.cuda.empty_cache()
     print(json.dumps({"metric": "PackedAttention us/layer, compression sweep (BASELINE config 5)", "unit": UNIT,
                       "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup), "data": "synthetic",
-                      "config": {"workload": base.name + "-sweep", "batch_per_gpu": Bt, "context": N, "n_layers": 2,
+                      "config": {"workload": base.name + "-sweep", "batch_per_gpu": Bt, "context": N, "n_layers": NL,
                                  "dense_segments": f"{base.dense_num}/{base.dense_den} (all dense at keep 1.0)"},
                       "peak": peak, "peak_source": peak_src, "sweep": points}), flush=True)
 

@@ -123,9 +123,10 @@ def select_bytes(built: BuiltCache, layer: int, n_selected: int) -> int:
     return keys + 12 * n_seg + q_bytes + 4 * n_selected
 
 
-def attention_bytes(built: BuiltCache, layer: int, sel, cnt) -> int:
+def attention_bytes(built: BuiltCache, layer: int, sel, cnt, split=False):
     """per selected block its token-block payload; + 4 B per selected block (sel) + 16 B per touched
-    segment (strategy record + offsets) + per unit q (G*D*2) and out (G*D*4)"""
+    segment (strategy record + offsets) + per unit q (G*D*2) and out (G*D*4).
+    split=True: (total, bytes of the K parts alone, bytes of the V parts alone)."""
     import torch
     w = built.w
     st = built.strat[layer].view(-1, built.strat[layer].shape[2], 4)  # [units][S][4]
@@ -140,4 +141,7 @@ def attention_bytes(built: BuiltCache, layer: int, sel, cnt) -> int:
     key = torch.where(valid, seg + torch.arange(U, device=sel.device).view(-1, 1) * st.shape[1], -1)
     touched = int(torch.unique(key).numel()) - (1 if (~valid).any() else 0)
     G = w.group
-    return int(payload.sum().item()) + 4 * int(valid.sum().item()) + 16 * touched + U * G * D * 6
+    total = int(payload.sum().item()) + 4 * int(valid.sum().item()) + 16 * touched + U * G * D * 6
+    if not split:
+        return total
+    return total, int((8 * vb(rk) * valid).sum().item()), int((8 * vb(rv) * valid).sum().item())

@@ -170,6 +170,16 @@ def assert_attention_close(out, lse, ref, ref_lse):
     fin = np.isfinite(ref_lse)
     assert np.array_equal(np.isneginf(lse), np.isneginf(ref_lse))
     if fin.any():
-        # lse is an fp32 output: 1e-3 absolute, plus a few fp32 spacings of its own magnitude (DESIGN.md section 6:
-        # logits of the generator's heavy hitters reach several thousand, where one fp32 ulp is 2.4e-4)
-        assert np.all(np.abs(lse[fin] - ref_lse[fin]) <= 1e-3 + 2e-6 * np.abs(ref_lse[fin]))
+        # lse is an fp32 output computed from fp32 logits: 1e-3 absolute plus LSE_ULPS fp32 spacings of its own
+        # magnitude (the generator's heavy hitters push logits into the thousands, where one spacing is 2.4e-4; the
+        # largest error seen over the whole GPU suite is recorded in LSE_ULPS_SEEN and printed by its last test)
+        a = np.abs(ref_lse[fin])
+        ulp = np.spacing(np.maximum(a, 1e-30).astype(np.float32)).astype(np.float64)
+        err = np.abs(lse[fin] - ref_lse[fin])
+        over = np.maximum(err - 1e-3, 0.0) / ulp
+        LSE_ULPS_SEEN[0] = max(LSE_ULPS_SEEN[0], float(over.max()))
+        assert np.all(err <= 1e-3 + LSE_ULPS * ulp), (float(over.max()), LSE_ULPS)
+
+
+LSE_ULPS = 2            # fp32 spacings of |lse| allowed on top of 1e-3 (measured maximum: see test_zz_report_lse_ulps)
+LSE_ULPS_SEEN = [0.0]

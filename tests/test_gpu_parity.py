@@ -46,67 +46,101 @@ def test_tiny_config_end_to_end(env):
         c.free()
 
 
-# ------------------------------------------------------------------ config 2 at full size (the bench's launch configuration)
+# ------------------------------------------------------------------ configs 2-4 at full size (the bench's launch configuration)
 
-def test_full_size_config2_sampled_units(env):
-    """BASELINE config 2 (batch 8, 8 KV heads, 131 072 tokens, budget 4096, 10 % dense by the quantile rule), one
-    layer, built exactly as bench.py builds it (same generator, same kernels, same grids).  The oracle recomputes
-    sampled units from the raw bytes the GPU consumed: strategy table, packed blob (bit-exact), selection (tie-band
-    protocol) and attention output on the GPU's own selection."""
+def _full_size_sampled(env, name, n_layers, units_per_layer):
+    """One BASELINE workload at FULL size, built exactly as bench.py builds it (same generator, kernels and grids).
+    For `units_per_layer` units of each of `n_layers` layers (always unit (0, 0) and the last unit) the oracle
+    recomputes everything from the raw bytes the GPU consumed: strategy table (equal), packed blob (bit-exact),
+    selection (tie-band protocol, swaps counted) and the attention output on the GPU's own selection; plus count /
+    order / range properties on every unit of every layer."""
     mkv, dev = env
+    import os
+    from concurrent.futures import ThreadPoolExecutor
     import torch
     from paper_2607_00760_b200 import synth, workload
-    w = synth.WORKLOADS["llama8b-128k-b8"]
-    units = [(0, 0, 0), (0, 3, 5), (0, 7, 7)]
-    built = workload.build(w, dev, n_layers=1, keep_units=units)
+    w = synth.WORKLOADS[name]
+    Bt, Hkv, Hq, G, N, L = w.batch, w.n_kv_heads, w.n_q_heads, w.group, w.context, w.segment_len
+    n_units = Bt * Hkv
+    pick = sorted({(i * (n_units - 1)) // max(1, units_per_layer - 1) for i in range(units_per_layer)})
+    units = [(l, u // Hkv, u % Hkv) for l in range(n_layers) for u in pick]
+    built = workload.build(w, dev, n_layers=n_layers, keep_units=units)
     cache = built.cache
     try:
-        Bt, Hkv, Hq, G, N, L = w.batch, w.n_kv_heads, w.n_q_heads, w.group, w.context, w.segment_len
         budget, scale = w.token_budget, 1.0 / math.sqrt(128)
-        k_max = budget // 8 + 1
-        sel = torch.full((Bt, Hkv, k_max), -1, dtype=torch.int32, device=dev)
-        cnt = torch.zeros((Bt, Hkv), dtype=torch.int32, device=dev)
-        out = torch.zeros((Bt, Hq, 128), dtype=torch.float32, device=dev)
-        lse = torch.zeros((Bt, Hq), dtype=torch.float32, device=dev)
-        cache.select(0, built.q[0], budget, sel, cnt)
-        cache.packed_attention(0, built.q[0], sel, cnt, scale, out, lse)
-        torch.cuda.synchronize()
-        cache.status()
-        sel_h, cnt_h = sel.cpu().numpy(), cnt.cpu().numpy()
-        out_h, lse_h = out.cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64)
-        q_h = built.q[0].view(torch.int16).cpu().numpy().view(np.uint16)
-        strat_h = built.strat[0].cpu().numpy()
-        total = swaps = 0
-        for (_, b, h) in units:
-            K, V = built.raw_units[(0, b, h)]
+        k0 = budget // 8
+        k_max = k0 + 1
+        res = {}
+        for l in range(n_layers):
+            sel = torch.full((Bt, Hkv, k_max), -1, dtype=torch.int32, device=dev)
+            cnt = torch.zeros((Bt, Hkv), dtype=torch.int32, device=dev)
+            out = torch.zeros((Bt, Hq, 128), dtype=torch.float32, device=dev)
+            lse = torch.zeros((Bt, Hq), dtype=torch.float32, device=dev)
+            cache.select(l, built.q[l], budget, sel, cnt)
+            cache.packed_attention(l, built.q[l], sel, cnt, scale, out, lse)
+            torch.cuda.synchronize()
+            cache.status()
+            sel_h, cnt_h = sel.cpu().numpy(), cnt.cpu().numpy()
+            out_h, lse_h = out.cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64)
+            # properties that hold for every unit: counts, order, range
+            assert np.all(cnt_h == k0)
+            assert np.all(np.diff(sel_h[:, :, :k0], axis=-1) > 0) and sel_h.max() < N and np.all(sel_h[:, :, :k0] % 8 == 0)
+            assert np.all(sel_h[:, :, k0:] == -1)
+            assert np.all(np.isfinite(out_h)) and np.all(np.isfinite(lse_h))
+            res[l] = (sel_h, cnt_h, out_h, lse_h, built.q[l].view(torch.int16).cpu().numpy().view(np.uint16),
+                      built.strat[l].cpu().numpy())
+
+        def check(unit):
+            l, b, h = unit
+            sel_h, cnt_h, out_h, lse_h, q_h, strat_h = res[l]
+            K, V = built.raw_units[(l, b, h)]
             lk, lv = orc.segment_loss(K, V, L, w.r_keep, w.r_keep)
             st = orc.strategy_quantile(lk, lv, w.dense_num, w.dense_den, 128, w.r_keep, w.r_keep)
             np.testing.assert_array_equal(strat_h[b, h], st)
             blob = orc.compress_unit(K, V, L, st)
-            np.testing.assert_array_equal(cache.export(0, b, h), blob)
+            np.testing.assert_array_equal(cache.export(l, b, h), blob)
             qh = q_h[b, h * G:(h + 1) * G]
             ft, nt = orc.blob_blocks(blob)
             s = orc.scores(blob, qh, 0)
             ref = orc.topk(s, ft, nt, budget)
             n = int(cnt_h[b, h])
             got = sel_h[b, h, :n]
-            assert n == len(ref) and np.all(np.diff(got) > 0) and np.all(sel_h[b, h, n:] == -1)
-            total += n
+            assert n == len(ref)
+            swaps = 0
             if not np.array_equal(got, ref):
                 diff = np.setxor1d(got, ref)
                 kth = np.sort(s)[::-1][len(ref) - 1]
                 band = 1e-5 * max(abs(kth), 1e-3 * np.abs(s).max())
-                assert np.all(np.abs(s[diff // 8] - kth) <= band), "selection differs outside the tie band"
-                swaps += len(diff) // 2
-            o, l = orc.attention(blob, qh, got, scale)
-            assert_attention_close(out_h[b:b + 1, h * G:(h + 1) * G], lse_h[b:b + 1, h * G:(h + 1) * G], o[None], l[None])
+                assert np.all(np.abs(s[diff // 8] - kth) <= band), ("selection differs outside the tie band", unit)
+                swaps = len(diff) // 2
+            o, lref = orc.attention(blob, qh, got, scale)
+            assert_attention_close(out_h[b:b + 1, h * G:(h + 1) * G], lse_h[b:b + 1, h * G:(h + 1) * G], o[None], lref[None])
+            return n, swaps
+
+        # the oracle is single-threaded C behind ctypes (the GIL is released): one thread per unit
+        with ThreadPoolExecutor(max(1, min(len(units), os.cpu_count() or 1, 16))) as ex:
+            results = list(ex.map(check, units))
+        total, swaps = sum(r[0] for r in results), sum(r[1] for r in results)
         assert swaps * 10000 <= total, f"{swaps} near-tie swaps in {total} selected blocks (bar: < 0.01 %)"
-        # properties that hold for every unit: counts, order, range
-        assert np.all(cnt_h == budget // 8)
-        assert np.all(np.diff(sel_h[:, :, :budget // 8], axis=-1) > 0) and sel_h.max() < N and np.all(sel_h[:, :, :budget // 8] % 8 == 0)
-        assert np.all(np.isfinite(out_h)) and np.all(np.isfinite(lse_h))
     finally:
         built.free()
+
+
+def test_full_size_config2_sampled_units(env):
+    """BASELINE config 2 (llama8b-128k-b8: batch 8, 8 KV heads, 131 072 tokens, budget 4096, 10 % dense by the quantile
+    rule): 8 units on each of 4 layers (SURVEY 8(c) protocol); every unit spans >= 2 CTAs of the attention kernel."""
+    _full_size_sampled(env, "llama8b-128k-b8", 4, 8)
+
+
+def test_full_size_config3_sampled_units(env):
+    """BASELINE config 3 (llama8b-1m-b1: 1 request, 1 048 576 tokens, budget 8192): all 8 units of 2 layers; top-k runs
+    in two stages over 8 slices of 16 384 blocks, and every unit spans ~18 CTAs of the attention kernel."""
+    _full_size_sampled(env, "llama8b-1m-b1", 2, 8)
+
+
+def test_full_size_config4_sampled_units(env):
+    """BASELINE config 4 (qwen7b-64k-b16: batch 16, 4 KV heads, GQA group 7, 65 536 tokens): 8 units on each of 4 layers."""
+    _full_size_sampled(env, "qwen7b-64k-b16", 4, 8)
 
 
 # ------------------------------------------------------------------ step 1
@@ -697,3 +731,10 @@ def test_errors_are_reported_not_thrown(env):
         c2.free()
     finally:
         small.free()
+
+
+def test_zz_report_lse_ulps(env):
+    """runs last: the largest lse error, in fp32 spacings of |lse| beyond the 1e-3 absolute term, seen by this session"""
+    import gpu_util
+    print(f"\nmax lse error beyond 1e-3: {gpu_util.LSE_ULPS_SEEN[0]:.2f} fp32 spacings (allowed {gpu_util.LSE_ULPS})")
+    assert gpu_util.LSE_ULPS_SEEN[0] <= gpu_util.LSE_ULPS
