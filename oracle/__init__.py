@@ -58,6 +58,10 @@ def _declare(L):
     L.orc_attention_units.argtypes = [C.POINTER(u8p), C.c_int, u16p, C.c_int, i32p, i32p, C.c_int,
                                       C.c_double, f64p, f64p]
     L.orc_num_threads.restype = C.c_int
+    L.orc_rotate_query.argtypes = [u16p, C.c_int, C.c_int, C.POINTER(C.c_float), u16p]
+    L.orc_rotate_query.restype = None
+    L.orc_rotate_output.argtypes = [f64p, C.c_int, C.c_int, C.POINTER(C.c_float)]
+    L.orc_rotate_output.restype = None
 
 
 def _u16(a):
@@ -314,3 +318,25 @@ def attention_units(blobs, q, sel, sel_count, scale: float):
     if rc:
         raise ValueError(f"orc_attention_units rc={rc}")
     return out, lse
+
+
+def rotate_query(q, R):
+    """Rotation fold: q' = q R_k^T, fp32 FMA chain in ascending j, RNE to bf16.
+    q: [n][D] bf16 bits, R: [D][D] float32.  Returns [n][D] bf16 bits."""
+    q = _u16(q)
+    n, D = q.shape
+    R = np.ascontiguousarray(R, np.float32)
+    assert R.shape == (D, D)
+    out = np.zeros((n, D), np.uint16)
+    lib().orc_rotate_query(_p(q, C.c_uint16), n, D, _p(R, C.c_float), _p(out, C.c_uint16))
+    return out
+
+
+def rotate_output(o, R):
+    """out = o' R_v (the rotated cache 'must be transformed back'), fp64.  o: [n][D] float64."""
+    o = np.array(o, np.float64, copy=True, order="C")
+    n, D = o.shape
+    R = np.ascontiguousarray(R, np.float32)
+    assert R.shape == (D, D)
+    lib().orc_rotate_output(_p(o, C.c_double), n, D, _p(R, C.c_float))
+    return o

@@ -706,3 +706,42 @@ int orc_attention_units(uint8_t* const* blobs, int n_units, const uint16_t* q, i
     }
     return err;
 }
+
+/* ---------------------------------------------------------------- rotation fold */
+
+/*
+ * PAPER.md:114 (§2.3): "Given a matrix K, SVD decomposes it as K = K' R ... applies the rotations (K R_k^T and
+ * V R_v^T)"; PAPER.md:218-220 (§5.3): "Instead of rotating the large matrix, MosaicKV merges the rotation into the
+ * single query vector and uses the rotated query to compute the attention scores.  This approach is mathematically
+ * equivalent".  With K' = K R_k^T stored, q K^T = (q R_k^T) K'^T, so the folded query is q' = q R_k^T:
+ *   q'[i] = sum_j q[j] * R_k[i][j].
+ * Reading (R22): q' is an INPUT of the bf16 kernels, so its rounding is part of the definition: the sum is
+ * accumulated in fp32 with one fused multiply-add per j in ascending j, then rounded to bf16 (RNE).
+ * q: [n][D] bf16, R: [D][D] fp32 row-major, out: [n][D] bf16.
+ */
+void orc_rotate_query(const uint16_t* q, int n, int D, const float* R, uint16_t* out) {
+    for (int v = 0; v < n; ++v)
+        for (int i = 0; i < D; ++i) {
+            float acc = 0.0f;
+            for (int j = 0; j < D; ++j) acc = fmaf(bf16_to_f32(q[(size_t)v * D + j]), R[(size_t)i * D + j], acc);
+            out[(size_t)v * D + i] = f32_to_bf16_rne(acc);
+        }
+}
+
+/*
+ * The attention output of the rotated cache lives in the rotated space of V' = V R_v^T: O = P V = (P V') R_v, so
+ *   out[j] = sum_i o'[i] * R_v[i][j]          (fp64).
+ * o: [n][D] double (in place allowed: a temporary row is used), R: [D][D] fp32 row-major.
+ */
+void orc_rotate_output(double* o, int n, int D, const float* R) {
+    double* tmp = (double*)malloc(sizeof(double) * (size_t)D);
+    for (int v = 0; v < n; ++v) {
+        for (int j = 0; j < D; ++j) {
+            double acc = 0.0;
+            for (int i = 0; i < D; ++i) acc += o[(size_t)v * D + i] * (double)R[(size_t)i * D + j];
+            tmp[j] = acc;
+        }
+        for (int j = 0; j < D; ++j) o[(size_t)v * D + j] = tmp[j];
+    }
+    free(tmp);
+}

@@ -100,6 +100,11 @@ int orc_attention_units(uint8_t* const* blobs, int n_units, const uint16_t* q, i
                         double* out, double* lse);
 int orc_num_threads(void);
 
+/* Rotation fold: q' = q R_k^T (fp32 FMA chain in ascending j, RNE to bf16) and
+ * out = o' R_v (fp64).  R: [D][D] fp32 row-major. */
+void orc_rotate_query(const uint16_t* q, int n, int D, const float* R, uint16_t* out);
+void orc_rotate_output(double* o, int n, int D, const float* R);
+
 #ifdef __cplusplus
 }
 #endif

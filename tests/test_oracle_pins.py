@@ -510,3 +510,45 @@ def test_batched_drivers_equal_per_unit_calls():
         np.testing.assert_array_equal(out[u], o)
         np.testing.assert_array_equal(lse[u], l)
     assert np.all(out[2] == 0) and np.all(np.isneginf(lse[2]))
+
+
+# ----------------------------------------------------------------------------- P14: rotation fold (NEXT-3)
+
+def test_P14_rotation_fold_is_mathematically_equivalent():
+    """folding the rotation into the query (and the inverse into the output) "is mathematically
+    equivalent" to attention in the original space.  Pinned three ways, none of which repeats the oracle's loops:
+    (i) with a SIGNED PERMUTATION R (orthogonal, and K R^T, q R^T are exact in bf16) and no compression, attention on the
+    rotated cache with the folded query, rotated back, equals numpy dense attention on the ORIGINAL K, V, q to 1e-12;
+    (ii) rotate_query equals the numpy matmul q R^T to bf16 rounding, and exactly for the permutation; a transposed R
+    fails both; (iii) rotate_output equals numpy o @ R."""
+    rng = np.random.default_rng(31)
+    D, N, G = 128, 96, 4
+    K, V, q = small_unit(seed=9, N=N, D=D, G=G)
+    perm_k, perm_v = rng.permutation(D), rng.permutation(D)
+    sgn_k, sgn_v = rng.choice([-1.0, 1.0], D), rng.choice([-1.0, 1.0], D)
+    Rk = np.zeros((D, D), np.float32); Rk[np.arange(D), perm_k] = sgn_k   # K'[:, i] = sgn_k[i] * K[:, perm_k[i]]
+    Rv = np.zeros((D, D), np.float32); Rv[np.arange(D), perm_v] = sgn_v
+    f = brute.bf16_to_f64
+    Kp = synth.f32_to_bf16_bits((f(K) @ Rk.T.astype(np.float64)).astype(np.float32))  # exact: one nonzero per column
+    Vp = synth.f32_to_bf16_bits((f(V) @ Rv.T.astype(np.float64)).astype(np.float32))
+    assert np.array_equal(f(Kp), f(K) @ Rk.T) and np.array_equal(f(Vp), f(V) @ Rv.T)
+    qp = orc.rotate_query(q, Rk)
+    np.testing.assert_array_equal(f(qp), f(q) @ Rk.T.astype(np.float64))                 # (ii) exact for a permutation
+    assert not np.array_equal(f(orc.rotate_query(q, Rk.T.copy())), f(q) @ Rk.T)          # a transposed operand is caught
+    S = (N + 63) // 64
+    blob = orc.compress_unit(Kp, Vp, 64, orc.uniform_strategy(S, D, D))
+    ft, nt = orc.blob_blocks(blob)
+    scale = 1.0 / math.sqrt(D)
+    o_rot, lse_rot = orc.attention(blob, qp, ft, scale)
+    o_back = orc.rotate_output(o_rot, Rv)
+    o_ref, lse_ref = brute.dense_attention(f(q), f(K), f(V), scale)
+    np.testing.assert_allclose(o_back, o_ref, rtol=0, atol=1e-12)                        # (i)
+    np.testing.assert_allclose(lse_rot, lse_ref, rtol=0, atol=1e-12)
+    # a general orthogonal matrix: bf16 rounding of q' only; rotate_output against numpy
+    Q, _ = np.linalg.qr(rng.standard_normal((D, D)))
+    Q = Q.astype(np.float32)
+    qr = f(orc.rotate_query(q, Q))
+    exact = f(q) @ Q.T.astype(np.float64)
+    assert np.abs(qr - exact).max() <= 2.0 ** -8 * np.abs(exact).max() + 1e-6           # one bf16 rounding + fp32 sums
+    o = rng.standard_normal((G, D))
+    np.testing.assert_allclose(orc.rotate_output(o, Q), o @ Q.astype(np.float64), rtol=0, atol=1e-13)
