@@ -190,6 +190,22 @@ MKV_API int mkv_update_flush(mkv_cache* cache, int32_t layer, const mkv_strategy
 MKV_API int mkv_update_count(const mkv_cache* cache, int32_t layer, int32_t* n_host);
 
 /*
+ * Per-head rotation fold.  The paper stores SVD-rotated K' = K R_k^T and V' = V R_v^T and
+ * "merges the rotation into the single query vector" instead of rotating the matrices back.  The rotation itself is
+ * the caller's (CPU-side management): compress K', V'; install the matrices with mkv_rotation_set; then
+ *   rotate_query:  q_out = bf16(q R_k^T), q_out[i] = sum_j q[j] R_k[h][i][j], fp32, one FMA per j in ascending j
+ *                  (q, q_out: bf16 [batch][n_q_heads][D], distinct buffers); feed q_out to mkv_select / mkv_packed_attention;
+ *   rotate_output: out[j] = sum_i out[i] R_v[h][i][j] in place (float [batch][n_q_heads][D]), h = the head's KV head.
+ * r_k, r_v: device, float [n_kv_heads][D][D] row-major, copied into the cache on `stream` (the first call of a cache
+ * allocates: not capturable); both NULL removes the layer's rotation.  mkv_decode_host applies both folds on its own
+ * when the layer has a rotation.  rotate_* on a layer without one is MKV_E_STATE.
+ * Channel truncation is not built: a bitmap of 96 bits would break the 16-byte rows of the format.
+ */
+MKV_API int mkv_rotation_set(mkv_cache* cache, int32_t layer, const float* r_k, const float* r_v, void* stream);
+MKV_API int mkv_rotate_query(const mkv_cache* cache, int32_t layer, const void* q, void* q_out, void* stream);
+MKV_API int mkv_rotate_output(const mkv_cache* cache, int32_t layer, float* out, void* stream);
+
+/*
  * Steps 2+3 with HOST buffers (the end-to-end call): copies q_host (bf16 [batch][n_q_heads][D],
  * pinned for true async) to the device, runs select + attention, copies out_host (float
  * [batch][n_q_heads][D]) back.  Everything is enqueued on `stream`; the caller synchronises the

@@ -24,7 +24,7 @@ MKV_DEV_ARENA_OVERFLOW, MKV_DEV_BAD_STRATEGY = 1, 2
 SYMBOLS = ["mkv_cache_create", "mkv_cache_free", "mkv_cache_reset", "mkv_segment_loss",
            "mkv_strategy_quantile", "mkv_strategy_threshold", "mkv_compress_segment", "mkv_select",
            "mkv_packed_attention", "mkv_update_append", "mkv_update_flush", "mkv_update_count", "mkv_calibrate_gather", "mkv_calibrate_stream",
-           "mkv_attention_stats", "mkv_decode_host", "mkv_cache_export", "mkv_cache_bytes",
+           "mkv_attention_stats", "mkv_rotation_set", "mkv_rotate_query", "mkv_rotate_output", "mkv_decode_host", "mkv_cache_export", "mkv_cache_bytes",
            "mkv_cache_status", "mkv_last_launch_count", "mkv_last_error", "mkv_version"]
 
 
@@ -57,6 +57,9 @@ _lib.mkv_update_count.argtypes = [_vp, _i32, C.POINTER(_i32)]
 _lib.mkv_calibrate_gather.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp]
 _lib.mkv_calibrate_stream.argtypes = [_vp, _i32, _u64, _vp]
 _lib.mkv_attention_stats.argtypes = [_vp, C.POINTER(_u64), C.POINTER(_u64), C.POINTER(_u64), _i32]
+_lib.mkv_rotation_set.argtypes = [_vp, _i32, _vp, _vp, _vp]
+_lib.mkv_rotate_query.argtypes = [_vp, _i32, _vp, _vp, _vp]
+_lib.mkv_rotate_output.argtypes = [_vp, _i32, _vp, _vp]
 _lib.mkv_decode_host.argtypes = [_vp, _i32, _vp, _i32, _i32, C.c_float, _vp, _vp, _vp, _vp]
 _lib.mkv_cache_export.argtypes = [_vp, _i32, _i32, _i32, _vp, _u64, C.POINTER(_u64)]
 _lib.mkv_cache_bytes.argtypes = [_vp, _i32, C.POINTER(_u64), C.POINTER(_u64), C.POINTER(_u64)]
@@ -210,6 +213,19 @@ def mkv_attention_stats(cache, reset=False):
     return dict(blocks=a.value, v_blocks=b.value, v_bytes=c.value)
 
 
+def mkv_rotation_set(cache, layer, r_k, r_v, stream=None):
+    """r_k, r_v: torch float32 [Hkv][D][D] on the device, or both None to remove the layer's rotation."""
+    _check(_lib.mkv_rotation_set(cache, layer, _ptr(r_k), _ptr(r_v), _stream(stream)))
+
+
+def mkv_rotate_query(cache, layer, q, q_out, stream=None):
+    _check(_lib.mkv_rotate_query(cache, layer, _ptr(q), _ptr(q_out), _stream(stream)))
+
+
+def mkv_rotate_output(cache, layer, out, stream=None):
+    _check(_lib.mkv_rotate_output(cache, layer, _ptr(out), _stream(stream)))
+
+
 def mkv_decode_host(cache, layer, q_host, token_budget, softmax_scale, out_host, reduce=0,
                     sel_host=None, sel_count_host=None, stream=None):
     _check(_lib.mkv_decode_host(cache, layer, _ptr(q_host), token_budget, reduce, float(softmax_scale),
@@ -319,6 +335,15 @@ class Cache:
 
     def attention_stats(self, reset=False):
         return mkv_attention_stats(self.h, reset)
+
+    def rotation_set(self, layer, r_k, r_v, stream=None):
+        mkv_rotation_set(self.h, layer, r_k, r_v, stream)
+
+    def rotate_query(self, layer, q, q_out, stream=None):
+        mkv_rotate_query(self.h, layer, q, q_out, stream)
+
+    def rotate_output(self, layer, out, stream=None):
+        mkv_rotate_output(self.h, layer, out, stream)
 
     def decode_host(self, layer, q_host, token_budget, softmax_scale, out_host, reduce=0,
                     sel_host=None, sel_count_host=None, stream=None):

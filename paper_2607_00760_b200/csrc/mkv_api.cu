@@ -62,6 +62,10 @@ struct mkv_cache {
     PlanRec* plan = nullptr;                  // [n_layers][n_units][sel_cap]: what top-k tells attention about each selected block
     uint32_t generation = 1;                  // bumped by mkv_cache_reset: invalidates every plan record
     unsigned long long* sink = nullptr;
+    float* rot_k = nullptr;                   // [n_layers][n_kv_heads][D][D] rotation matrices (allocated by the first mkv_rotation_set)
+    float* rot_v = nullptr;
+    std::vector<uint8_t> rot_set;             // per layer: a rotation is installed
+    uint16_t* q_rot = nullptr;                // [batch][n_q_heads][D] folded query of mkv_decode_host
     uint16_t* q_dev = nullptr;
     int32_t* sel_dev = nullptr;
     int32_t* selcnt_dev = nullptr;
@@ -106,7 +110,7 @@ int mkv_cache_free(mkv_cache* c) {
     cudaSetDevice(c->desc.device);
     cudaDeviceSynchronize();
     void* ptrs[] = {c->arena, c->strat, c->tok_off, c->bk_off, c->unit_nseg, c->unit_ntok, c->counters,
-                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->upd_k, c->upd_v, c->upd_cnt, c->attn.part_o, c->attn.part_l, c->attn.ticket, c->attn.zbuf, c->attn.stats, c->plan, c->sink, c->q_dev,
+                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->upd_k, c->upd_v, c->upd_cnt, c->attn.part_o, c->attn.part_l, c->attn.ticket, c->attn.zbuf, c->attn.stats, c->plan, c->sink, c->rot_k, c->rot_v, c->q_rot, c->q_dev,
                     c->sel_dev, c->selcnt_dev, c->out_dev};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -154,6 +158,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     c->sel_cap = g.score_stride + 1;
     const size_t upd_bytes = (size_t)g.n_layers * g.n_units * g.L * kD * 2;
     c->upd_n.assign(g.n_layers, 0);
+    c->rot_set.assign(g.n_layers, 0);
     const int topk_slices = (g.score_stride + kTopkSlice - 1) / kTopkSlice;
     const size_t cand_bytes = topk_slices > 1 ? (size_t)g.n_units * topk_slices * kTopkSlice * 4 : 256;
     struct { void** p; size_t bytes; } allocs[] = {
@@ -180,6 +185,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         {(void**)&c->plan, tu * (size_t)c->sel_cap * sizeof(PlanRec)},
         {(void**)&c->sink, 64},
         {(void**)&c->q_dev, (size_t)g.batch * g.n_q_heads * kD * 2},
+        {(void**)&c->q_rot, (size_t)g.batch * g.n_q_heads * kD * 2},
         {(void**)&c->sel_dev, (size_t)g.n_units * c->sel_cap * 4},
         {(void**)&c->selcnt_dev, (size_t)g.n_units * 4},
         {(void**)&c->out_dev, (size_t)g.batch * g.n_q_heads * kD * 4},
@@ -380,6 +386,51 @@ int mkv_attention_stats(const mkv_cache* c, uint64_t* blocks_host, uint64_t* v_b
     return MKV_OK;
 }
 
+int mkv_rotation_set(mkv_cache* c, int32_t layer, const float* r_k, const float* r_v, void* stream) {
+    if (!c) return fail(MKV_E_ARG, "NULL cache");
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    if ((r_k == nullptr) != (r_v == nullptr)) return fail(MKV_E_ARG, "mkv_rotation_set: pass both matrices or neither");
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    if (!r_k) { c->rot_set[layer] = 0; return MKV_OK; }
+    const size_t per_layer = (size_t)g.n_kv_heads * kD * kD;
+    if (!c->rot_k) {  // first use: this call allocates (it is the only non-capturable path of the call)
+        cudaError_t e1 = cudaMalloc((void**)&c->rot_k, per_layer * g.n_layers * 4);
+        cudaError_t e2 = e1 == cudaSuccess ? cudaMalloc((void**)&c->rot_v, per_layer * g.n_layers * 4) : e1;
+        if (e2 != cudaSuccess) {
+            cudaGetLastError();
+            if (c->rot_k) { cudaFree(c->rot_k); c->rot_k = nullptr; }
+            return fail(MKV_E_NOMEM, "mkv_rotation_set: cudaMalloc: %s", cudaGetErrorString(e2));
+        }
+    }
+    MKV_CUDA(cudaMemcpyAsync(c->rot_k + per_layer * layer, r_k, per_layer * 4, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    MKV_CUDA(cudaMemcpyAsync(c->rot_v + per_layer * layer, r_v, per_layer * 4, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    c->rot_set[layer] = 1;
+    return MKV_OK;
+}
+
+int mkv_rotate_query(const mkv_cache* c, int32_t layer, const void* q, void* q_out, void* stream) {
+    if (!c || !q || !q_out) return fail(MKV_E_ARG, "mkv_rotate_query: NULL argument");
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    if (!c->rot_set[layer]) return fail(MKV_E_STATE, "mkv_rotate_query: layer %d has no rotation (mkv_rotation_set)", layer);
+    if (q == q_out) return fail(MKV_E_ARG, "mkv_rotate_query: q_out must not alias q");
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(launch_rotate_query(g, (const uint16_t*)q, c->rot_k + (size_t)layer * g.n_kv_heads * kD * kD, (uint16_t*)q_out,
+                                 (cudaStream_t)stream));
+    return MKV_OK;
+}
+
+int mkv_rotate_output(const mkv_cache* c, int32_t layer, float* out, void* stream) {
+    if (!c || !out) return fail(MKV_E_ARG, "mkv_rotate_output: NULL argument");
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    if (!c->rot_set[layer]) return fail(MKV_E_STATE, "mkv_rotate_output: layer %d has no rotation (mkv_rotation_set)", layer);
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(launch_rotate_output(g, out, c->rot_v + (size_t)layer * g.n_kv_heads * kD * kD, (cudaStream_t)stream));
+    return MKV_OK;
+}
+
 int mkv_update_append(mkv_cache* c, int32_t layer, const void* k_new, const void* v_new, int64_t sb, int64_t sh,
                       int64_t st, int32_t n_new, void* stream) {
     if (!c || !k_new || !v_new) return fail(MKV_E_ARG, "mkv_update_append: NULL argument");
@@ -435,10 +486,17 @@ int mkv_decode_host(mkv_cache* c, int32_t layer, const void* q_host, int32_t bud
     if (k_max > c->sel_cap) k_max = c->sel_cap;
     MKV_CUDA(cudaSetDevice(c->desc.device));
     MKV_CUDA(cudaMemcpyAsync(c->q_dev, q_host, (size_t)g.batch * g.n_q_heads * kD * 2, cudaMemcpyHostToDevice, s));
-    int rc = mkv_select(c, layer, c->q_dev, budget, reduce, c->sel_dev, c->selcnt_dev, (int)k_max, nullptr, stream);
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    const uint16_t* qd = c->q_dev;
+    if (c->rot_set[layer]) {  // rotation fold: the cache holds K R_k^T, V R_v^T; attend with q R_k^T
+        MKV_CUDA(launch_rotate_query(g, c->q_dev, c->rot_k + (size_t)layer * g.n_kv_heads * kD * kD, c->q_rot, s));
+        qd = c->q_rot;
+    }
+    int rc = mkv_select(c, layer, qd, budget, reduce, c->sel_dev, c->selcnt_dev, (int)k_max, nullptr, stream);
     if (rc) return rc;
-    rc = mkv_packed_attention(c, layer, c->q_dev, c->sel_dev, c->selcnt_dev, (int)k_max, scale, c->out_dev, nullptr, stream);
+    rc = mkv_packed_attention(c, layer, qd, c->sel_dev, c->selcnt_dev, (int)k_max, scale, c->out_dev, nullptr, stream);
     if (rc) return rc;
+    if (c->rot_set[layer]) MKV_CUDA(launch_rotate_output(g, c->out_dev, c->rot_v + (size_t)layer * g.n_kv_heads * kD * kD, s));
     MKV_CUDA(cudaMemcpyAsync(out_host, c->out_dev, (size_t)g.batch * g.n_q_heads * kD * 4, cudaMemcpyDeviceToHost, s));
     if (sel_host_opt)
         MKV_CUDA(cudaMemcpyAsync(sel_host_opt, c->sel_dev, (size_t)g.n_units * k_max * 4, cudaMemcpyDeviceToHost, s));

@@ -142,6 +142,10 @@ cudaError_t launch_stream_read(const uint8_t* base, unsigned long long bytes, in
 cudaError_t launch_update_copy(const CacheGeom& g, const CompressArgs& a, uint16_t* upd_k, uint16_t* upd_v,
                                int32_t* upd_count, int n_have, cudaStream_t s);
 
+// rotation fold: q' = q R_k^T (bf16, fp32 FMA chain) and out = o' R_v (fp32, in place); R: [Hkv][D][D] fp32
+cudaError_t launch_rotate_query(const CacheGeom& g, const uint16_t* q, const float* Rk, uint16_t* q_out, cudaStream_t s);
+cudaError_t launch_rotate_output(const CacheGeom& g, float* out, const float* Rv, cudaStream_t s);
+
 // ---- programmatic dependent launch (PDL) ----------------------------------------------------
 // The decode kernels are launched with programmatic stream serialisation: kernel N+1 may be scheduled
 // while kernel N drains, runs its global-memory-free preamble, and blocks in pdl_wait() until kernel N

@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 import oracle as orc
-from gpu_util import Case, uniform_strat, assert_attention_close, to_dev
+from gpu_util import Case, uniform_strat, assert_attention_close, to_dev, ATOL_ATTN as ATOL, RTOL_L2_ATTN as RTOL
 
 pytestmark = pytest.mark.gpu
 
@@ -731,6 +731,78 @@ def test_errors_are_reported_not_thrown(env):
         c2.free()
     finally:
         small.free()
+
+
+def test_rotation_fold(env):
+    """the cache holds K R_k^T, V R_v^T; the rotation is folded into the query
+    and out of the result.  mkv_rotate_query is bit-exact against the oracle (same fp32 FMA chain, RNE to bf16),
+    mkv_rotate_output within fp32 rounding, and mkv_decode_host on the rotated cache equals the oracle's
+    rotate_query -> scores -> top-k -> attention -> rotate_output."""
+    mkv, dev = env
+    import torch
+    Bt, Hkv, Hq, N = 2, 2, 8, 64 * 10 + 24
+    G, D = Hq // Hkv, 128
+    rng = np.random.default_rng(41)
+    c = Case(mkv, dev, Bt, Hkv, Hq, N, seed=97)
+    try:
+        Rk = np.stack([np.linalg.qr(rng.standard_normal((D, D)))[0] for _ in range(Hkv)]).astype(np.float32)
+        Rv = np.stack([np.linalg.qr(rng.standard_normal((D, D)))[0] for _ in range(Hkv)]).astype(np.float32)
+        f = lambda a: (a.astype(np.uint32) << np.uint32(16)).view(np.float32)
+        from paper_2607_00760_b200 import synth
+        # the caller rotates K and V before compressing (CPU-side management in the paper)
+        for h in range(Hkv):
+            c.K[:, h] = synth.f32_to_bf16_bits(f(c.K[:, h]) @ Rk[h].T)
+            c.V[:, h] = synth.f32_to_bf16_bits(f(c.V[:, h]) @ Rv[h].T)
+        c.k_d, c.v_d = to_dev(c.K, dev), to_dev(c.V, dev)
+        strat = uniform_strat(Bt, Hkv, c.S, 38)
+        strat[:, :, ::4, 0:2] = 128
+        c.compress(strat)
+        with pytest.raises(mkv.MkvError) as e:  # no rotation installed yet
+            c.cache.rotate_query(0, c.q_d, torch.empty_like(c.q_d))
+        assert e.value.code == mkv.MKV_E_STATE
+        c.cache.rotation_set(0, torch.from_numpy(Rk).to(dev), torch.from_numpy(Rv).to(dev))
+        q_rot = torch.empty_like(c.q_d)
+        c.cache.rotate_query(0, c.q_d, q_rot)
+        torch.cuda.synchronize()
+        got = q_rot.view(torch.int16).cpu().numpy().view(np.uint16)
+        ref_q = np.stack([np.stack([orc.rotate_query(c.q[b, hq:hq + 1], Rk[hq // G])[0] for hq in range(Hq)]) for b in range(Bt)])
+        np.testing.assert_array_equal(got, ref_q)
+        o = rng.standard_normal((Bt, Hq, D)).astype(np.float32)
+        o_d = torch.from_numpy(o).to(dev)
+        c.cache.rotate_output(0, o_d)
+        torch.cuda.synchronize()
+        ref_o = np.stack([np.stack([orc.rotate_output(o[b, hq:hq + 1].astype(np.float64), Rv[hq // G])[0] for hq in range(Hq)])
+                          for b in range(Bt)])
+        assert np.abs(o_d.cpu().numpy() - ref_o).max() <= 1e-5
+        # end to end through the host call
+        budget, scale = 256, 1.0 / math.sqrt(D)
+        q_host = torch.from_numpy(c.q.view(np.int16)).view(torch.bfloat16).pin_memory()
+        out_host = torch.zeros((Bt, Hq, D), dtype=torch.float32).pin_memory()
+        k_max = budget // 8 + 1
+        sel_host = torch.zeros((Bt, Hkv, k_max), dtype=torch.int32).pin_memory()
+        cnt_host = torch.zeros((Bt, Hkv), dtype=torch.int32).pin_memory()
+        c.cache.decode_host(0, q_host, budget, scale, out_host, sel_host=sel_host, sel_count_host=cnt_host)
+        torch.cuda.synchronize()
+        sel, cnt = sel_host.numpy(), cnt_host.numpy()
+        ref = np.zeros((Bt, Hq, D))
+        for b in range(Bt):
+            for h in range(Hkv):
+                qh = ref_q[b, h * G:(h + 1) * G]
+                blob = c.blobs[b][h]
+                ft, nt = orc.blob_blocks(blob)
+                s_ = orc.scores(blob, qh, 0)
+                want = orc.topk(s_, ft, nt, budget)
+                np.testing.assert_array_equal(sel[b, h, :cnt[b, h]], want)
+                o_, _ = orc.attention(blob, qh, want, scale)
+                ref[b, h * G:(h + 1) * G] = orc.rotate_output(o_, Rv[h])
+        got_o = out_host.numpy().astype(np.float64)
+        assert np.abs(got_o - ref).max() <= ATOL and np.linalg.norm(got_o - ref) / np.linalg.norm(ref) <= RTOL
+        c.cache.rotation_set(0, None, None)  # removed again: the host call attends with q itself
+        c.cache.decode_host(0, q_host, budget, scale, out_host)
+        torch.cuda.synchronize()
+        assert np.abs(out_host.numpy().astype(np.float64) - ref).max() > 1e-3
+    finally:
+        c.free()
 
 
 def test_zz_report_lse_ulps(env):
