@@ -1,34 +1,31 @@
 // attention.cu — step 3 of the hot path: PackedAttention: QK over the
 // selected packed keys, softmax, PV over the packed values, split-K combine.  sm_100a.
 //
-// Design: one launch, two phases, one CTA per SM.
-//   * The selected blocks of all units form one stream of T blocks; it is cut into equal ranges,
-//     one per warp (warps never meet before the combine).  A warp walks its range in groups of
-//     <= 2 token blocks (16 tokens = the M of one mma tile).  What a block is (payload offset,
-//     tokens, r_k, r_v) comes from the plan record mkv_select wrote next to `sel`, verified against
-//     the `sel` entry; a record that does not match is replaced by the table lookup.
+// Design: one launch; every unit is attended by ONE thread-block
+// cluster of C CTAs (C = 2 for 64 units on 148 SMs, 16 for 8 units), one CTA per SM.
+//   * The unit's selected blocks are cut into equal ranges, one per warp of the cluster.  A warp
+//     walks its range in groups of <= 2 token blocks (16 tokens = the M of one mma tile).  What a
+//     block is (payload offset, tokens, r_k, r_v) comes from the plan record mkv_select wrote next
+//     to `sel`, verified against the `sel` entry; a record that does not match is replaced by the
+//     table lookup.
 //   * Staging: a block's K part and its V part are contiguous chunks (DESIGN.md format); one lane
 //     moves a chunk into the warp's shared-memory ring with ONE 1-D bulk copy (cp.async.bulk, the
 //     TMA engine) that completes on the slot's mbarrier.  The ring is byte-granular (a group takes
 //     what it needs); up to kSlots groups are in flight per warp.
 //   * Phase 1 (QK): S = K q^T with the group's 16 tokens = M, heads = N, channels = K; packed
 //     vectors are expanded straight into mma.sync fragments (mkv_walk.cuh).  The scaled logits go
-//     to the warp's logit cache (shared memory; global scratch beyond its capacity).  At the end of
-//     a unit the warp folds its per-head maxima into the CTA's table (shared-memory atomic max).
-//   * One CTA barrier separates the phases.  Phase 2 (PV, deferred) then knows, for every unit of
-//     the CTA's range, the maximum logit M_c over ALL the tokens the CTA holds of it (about 1 800 of
-//     a unit's 4 096 at config 2): probabilities are 2^(z - M_c), nothing is ever rescaled inside a
-//     CTA, and the partials of one unit inside a CTA simply add.  The softmax sum runs over every
-//     selected token; the V part of a block is fetched and walked only if one of its probabilities
-//     is >= 2^-40 of the CTA's largest (error bound; M_c <= the unit's true maximum, so
-//     the test is conservative).  O^T = V^T P^T with channels = M, heads = N, the group's 16 tokens
-//     = K; P is split into bf16 hi + lo (fp32-class accuracy).  Dense vectors (r = D) skip the walk.
-//   * Step 3d (split-K combine) is fused: a unit wholly inside one warp's range is normalised and
-//     written directly; otherwise the warp leaves an (m, l, O) partial (<= 2 per warp), the threads
-//     of the CTA fold the partials of a unit (four output channels each) with the LSE rule, and a
-//     unit that spans several CTAs is finished, four channels at a time, by the last thread to
-//     arrive at a per-(unit, channel quad) ticket (no second kernel, no barrier after the fold).
-//     Nothing in the kernel waits for another CTA.
+//     to the warp's logit cache (shared memory; global scratch beyond its capacity), the warp's
+//     per-head maxima into the CTA's table (shared-memory atomic max).
+//   * The CTAs of the cluster exchange their maxima through distributed shared memory (one cluster
+//     barrier).  Every warp then knows the unit's exact maximum M: probabilities are 2^(z - M),
+//     nothing is ever rescaled, and partial results simply add.
+//   * Phase 2 (PV, deferred): the softmax sum runs over every selected token; the V part of a block
+//     is fetched and walked only if one of its probabilities is >= 2^-40 (error bound).
+//     O^T = V^T P^T with channels = M, heads = N, the group's 16 tokens = K; P is split into bf16
+//     hi + lo (fp32-class accuracy).  Dense vectors (r = D) skip the walk.
+//   * Step 3d (split-K combine): the warps' partials are added inside the CTA (shared memory), the
+//     CTAs' partials by the cluster's first CTA through distributed shared memory, in a fixed order:
+//     no global scratch, no atomics, no second kernel, bit-reproducible.
 #include "mkv_internal.cuh"
 #include "mkv_walk.cuh"
 
@@ -47,18 +44,17 @@ constexpr int kGroupMax16 = 256;   // largest group in 16-B units: two dense K (
 constexpr int kDesc = 32;          // group descriptors kept per warp and phase
 constexpr int kDescribe = 24;      // blocks described per call: kDescribe + kSlots <= kDesc
 constexpr int kZBytes = 4096;      // per-warp logit cache: 32 blocks at G = 4
-constexpr int kMaxUnitsSmem = 2048;
+constexpr int kMaxCluster = 16;
 constexpr float kSkip = 40.f;      // a block whose probabilities are all < 2^-40 is not walked in phase 2
-constexpr int kCtaUnits = 32;     // units of a CTA's range whose maxima are shared through the CTA's table
 
-// One group of the stream: <= 2 consecutive selected token blocks of one unit with the same strategy whose K
-// parts and V parts each fit kGroupMax16.  Every size the hot loops need is worked out once, by the describing lane.
+// One group of the stream: <= 2 consecutive selected token blocks with the same strategy whose K parts and V
+// parts each fit kGroupMax16.  Every size the hot loops need is worked out once, by the describing lane.
 struct __align__(16) GDesc {
     // phase 1 (K parts)                                     phase 2 (V parts)
     uint32_t off0, off1;  // chunk offsets, 16-B units       first 16-B unit of each V part
     uint32_t x;           // kc0 | kc1 << 8 | nb0 << 16      vc0 | vc1 << 8 | skew0 << 16 | skew1 << 20 | r_v << 24
                           //   | nb1 << 20 | r_k << 24         (chunk sizes in 16-B units; skew: bytes before the V part)
-    uint32_t y;           // unit | upd << 16                 unit | upd << 16 | nb0 << 20 | nb1 << 24
+    uint32_t y;           // upd                              upd | nb0 << 4 | nb1 << 8
 };
 
 __device__ __forceinline__ unsigned lanemask_le() {
@@ -86,16 +82,29 @@ __device__ __forceinline__ float2 lds_f32x2(uint32_t a) {
     asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a));
     return v;
 }
-
-// largest u with s_cum[u] <= i (i < T guaranteed; zero-count units are skipped by construction)
-__device__ __forceinline__ int find_unit(const int* s_cum, int n_units, int i) {
-    int lo = 0, hi = n_units;  // invariant: s_cum[lo] <= i < s_cum[hi]
-#pragma unroll 1
-    while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (s_cum[mid] <= i) lo = mid; else hi = mid;
-    }
-    return lo;
+// ---- thread-block cluster: rank, barrier, distributed shared memory
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync() {  // also orders shared-memory accesses cluster-wide (release / acquire)
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t dsmem_addr(uint32_t local, uint32_t rank) {  // the same offset in CTA `rank` of the cluster
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ uint32_t ld_dsmem_u32(uint32_t a) {
+    uint32_t v;
+    asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ float ld_dsmem_f32(uint32_t a) {
+    float v;
+    asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory");
+    return v;
 }
 
 // per warp: staging ring | phase-1 descriptors | phase-2 descriptors | logit cache | slot table (offset, bytes) |
@@ -104,18 +113,14 @@ constexpr int kOffD1 = kRingBytes, kOffD2 = kOffD1 + kDesc * 16, kOffZ = kOffD2 
 constexpr int kOffBar = kOffSlot + kSlots * 8, kOffGrp = kOffBar + kSlots * 8, kWS = kOffGrp + kSlots * 16;
 
 // Even split of n items over p parts: part i owns [i b + min(i, r), ...) with b = n / p, r = n % p
-// (the first r parts hold one more).  One runtime division per level.
+// (the first r parts hold one more).
 struct Split {
     unsigned b, r;
     __device__ __forceinline__ unsigned begin(unsigned i) const { return i * b + min(i, r); }
-    // the part that owns item x (x < n)
-    __device__ __forceinline__ unsigned owner(unsigned x) const {
-        const unsigned big = r * (b + 1);
-        return x < big ? x / (b + 1) : r + (x - big) / b;
-    }
 };
 
 // ------------------------------------------------------------------------------------------
+// grid = n_units clusters of C CTAs; cluster u attends unit u.
 // kGatherOnly: calibration build of the same kernel (mkv_calibrate_gather): every K part and every
 // V part of the selection is staged exactly as in the real run (nothing is skipped), one word per
 // lane and group is read back, and all arithmetic, synchronisation and output are left out.
@@ -126,17 +131,18 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                             const int32_t* __restrict__ sel, const int32_t* __restrict__ sel_count, int k_max,
                             float scale_log2, float* __restrict__ out, float* __restrict__ lse, AttnScratch scr,
                             const uint16_t* __restrict__ upd_k, const uint16_t* __restrict__ upd_v,
-                            const int32_t* __restrict__ upd_count) {
+                            const int32_t* __restrict__ upd_count, int C) {
     extern __shared__ __align__(128) uint8_t smem[];
     constexpr int kNT = kWarps * 32;
-    constexpr int kRec = 2 * kWarps;  // partial records of the CTA: warp w -> 2w (head), 2w + 1 (tail)
-    int* s_cum = reinterpret_cast<int*>(smem + kWarps * kWS);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int gq = lane >> 2, qq = lane & 3;  // mma fragment coordinates (groupID, threadID_in_group)
+    const int G = g.group;
 
-    __shared__ int s_unit[kRec];                              // unit of each partial record, -1 = none
-    __shared__ __align__(8) float s_ml[kRec][kMaxGroup][2];   // its (reference maximum in log2 units, sum) per head
-    __shared__ uint32_t s_umax[kCtaUnits][kMaxGroup];         // the CTA's maxima of the first kCtaUnits units of its range (keys)
+    __shared__ uint32_t s_max[kMaxGroup];                 // the CTA's per-head maxima (keys); read by the whole cluster
+    __shared__ float s_l[kWarps][kMaxGroup];              // the warps' softmax sums
+    __shared__ float s_cta_l[kMaxGroup];                  // the CTA's partial sums (its partial O: s_cta_o)
+    __shared__ float s_M[kMaxGroup];                      // the unit's per-head maxima after the exchange
+    float* s_cta_o = reinterpret_cast<float*>(smem + kWarps * kWS);  // [G][128] floats behind the warps' regions
 
     uint8_t* wbase = smem + warp * kWS;
     const uint32_t ring0 = smem_u32(wbase);
@@ -151,81 +157,48 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         for (int s = 0; s < kSlots; ++s) mbar_init(bar0 + 8 * s, 1);
         mbar_init_fence();
     }
-    if (lane < 2) s_unit[warp * 2 + lane] = -1;
-    if (threadIdx.x < kCtaUnits * kMaxGroup) (&s_umax[0][0])[threadIdx.x] = 0u;  // below the key of every float
+    if (threadIdx.x < kMaxGroup) s_max[threadIdx.x] = 0u;  // below the key of every float
+    const int u = (int)blockIdx.x / C;                      // the cluster's unit
+    const unsigned rank = cluster_ctarank();
     __syncthreads();
-    pdl_wait();               // the producer of sel / sel_count / the plan / the cache (and the previous user of the scratch) is done
+    pdl_wait();               // the producer of sel / sel_count / the plan / the cache is done
     pdl_launch_dependents();  // the next kernel may be scheduled as SMs free up
 
     // tokens in the layer's update buffer: device-resident, so a captured graph stays valid across appends
     const int n_buf = min(max(__ldg(upd_count), 0), g.L);
-    const int upd_blocks = (n_buf + kB - 1) / kB;  // every unit ends with the blocks of its update buffer
-    // Prefix sums of the clamped selection counts -> s_cum[0 .. n_units].  Every warp runs the scan itself
-    // and writes the same values: no warp waits for another one before its first copy is in flight.
-    int T = 0;
-    {
-#pragma unroll 1
-        for (int i0 = 0; i0 < g.n_units; i0 += 32) {
-            const int i = i0 + lane;
-            const int c = (i < g.n_units) ? min(max(__ldg(sel_count + i), 0), k_max) + upd_blocks : 0;
-            int inc = c;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int v = __shfl_up_sync(kFull, inc, o);
-                if (lane >= o) inc += v;
-            }
-            if (i < g.n_units) s_cum[i] = T + inc - c;
-            T += __shfl_sync(kFull, inc, 31);
+    const int upd_blocks = (n_buf + kB - 1) / kB;  // the unit's stream ends with the blocks of its update buffer
+    const int cnt = min(max(__ldg(sel_count + u), 0), k_max);
+    const int T = cnt + upd_blocks;                // blocks of the unit
+    const size_t row = (size_t)(u / g.n_kv_heads) * g.n_q_heads + (size_t)(u % g.n_kv_heads) * G;
+    if (T == 0) {  // (uniform over the cluster) empty selection: out = 0, lse = -inf
+        if (rank == 0 && !kGatherOnly) {
+            for (int e = threadIdx.x; e < G * kD; e += kNT) out[row * kD + e] = 0.f;
+            if (lse != nullptr && threadIdx.x < G) lse[row + threadIdx.x] = -INFINITY;
         }
-        if (lane == 0) s_cum[g.n_units] = T;
-        __syncwarp();
+        return;
     }
-    // The stream is split in units of two positions, so every range starts at an even position: with even
-    // selection counts (units then start at even positions too) a range never holds two odd runs, which
-    // would cost an extra half-empty group -- the slowest warp sets the kernel's time.
-    const unsigned P = ((unsigned)T + 1u) >> 1;                     // position pairs
-    const unsigned Gd = min(gridDim.x, max(P, 1u));                 // CTAs that own >= 1 pair
-    Split cs;                                                       // pairs over CTAs
-    cs.b = P / Gd; cs.r = P - cs.b * Gd;
-    int clo = 0, chi = 0;
-    unsigned cplo = 0, cphi = 0;
-    if (blockIdx.x < Gd) { cplo = cs.begin(blockIdx.x); cphi = cs.begin(blockIdx.x + 1); }
-    clo = (int)(2u * cplo); chi = min((int)(2u * cphi), T);
-    Split ws;                                                       // the CTA's pairs over its warps
-    ws.b = (cphi - cplo) / kWarps; ws.r = (cphi - cplo) % kWarps;
-    const int lo = min(clo + 2 * (int)ws.begin(warp), chi), hi = min(clo + 2 * (int)ws.begin(warp + 1), chi);
-    const unsigned gw = blockIdx.x * kWarps + warp;
+    // The stream is split in units of two positions, so every range starts at an even position: a range never
+    // holds two odd runs, which would cost an extra half-empty group.
+    const unsigned P = ((unsigned)T + 1u) >> 1;  // position pairs, over the C * kWarps warps of the cluster
+    Split ws;
+    ws.b = P / (unsigned)(C * kWarps); ws.r = P % (unsigned)(C * kWarps);
+    const unsigned wi = rank * kWarps + (unsigned)warp;
+    const int lo = min(2 * (int)ws.begin(wi), T), hi = min(2 * (int)ws.begin(wi + 1), T);
     const int n_total = hi - lo;
-    const int G = g.group;
     const uint32_t zstride = 32u * (uint32_t)G;         // bytes of one block's logits: [head][token] floats
     const int zcap = kZBytes / (int)zstride;            // blocks of the range whose logits stay in shared memory
-    if (blockIdx.x == 0 && !kGatherOnly) {  // units with an empty selection: out = 0, lse = -inf
-#pragma unroll 1
-        for (int u = warp; u < g.n_units; u += kWarps) {
-            if (s_cum[u + 1] != s_cum[u]) continue;
-            const size_t row = (size_t)(u / g.n_kv_heads) * g.n_q_heads + (size_t)(u % g.n_kv_heads) * G;
-#pragma unroll 1
-            for (int e = lane; e < G * kD; e += 32) out[row * kD + e] = 0.f;
-            if (lse != nullptr && lane < G) lse[row + lane] = -INFINITY;
-        }
-    }
-    const int u_first = clo < chi ? find_unit(s_cum, g.n_units, clo) : 0;  // first unit of the CTA's range: slot 0 of its table
+    float* zglob = scr.zbuf + ((size_t)u * scr.z_unit_stride + (size_t)lo) * (size_t)(8 * G);
 
     int bbuilt = 0, gbuilt = 0;  // blocks / groups described so far
-    int ucur = n_total > 0 ? find_unit(s_cum, g.n_units, lo) : 0;  // unit of the first block not yet described (warp-uniform)
 
     // Describe the next <= kDescribe blocks of the range (one per lane) and pair them into groups: block i
-    // follows block i - 1 in a group if both belong to one unit, have the same strategy and their K parts
-    // and V parts fit one group; runs of such blocks are paired greedily from their start.
-    // A pure function of the inputs: when phase 2 has to describe a long range again it gets the same groups.
+    // follows block i - 1 in a group if both have the same strategy and their K parts and V parts fit one group;
+    // runs of such blocks are paired greedily from their start.  A pure function of the inputs: when phase 2
+    // has to describe a long range again it gets the same groups.
     auto describe = [&](int count) {
         uint32_t off16 = 0u, meta = 0u, updf = 0u;
-        int u = ucur;
         if (lane < count) {
-            const int gi = lo + bbuilt + lane;
-#pragma unroll 1
-            while (gi >= s_cum[u + 1]) ++u;
-            const int j = gi - s_cum[u], jb = j - (s_cum[u + 1] - s_cum[u] - upd_blocks);
+            const int j = lo + bbuilt + lane, jb = j - cnt;
             if (jb >= 0) {  // block jb of the unit's update buffer: raw rows [u][8 jb ..][128] of upd_k / upd_v
                 const uint32_t nb = (uint32_t)min(kB, n_buf - kB * jb);
                 off16 = (uint32_t)(((size_t)u * g.L + (size_t)kB * jb) * (kD * 2 / 16));
@@ -243,17 +216,14 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 else plan_lookup(g, lv, u, t0, off16, meta);
             }
         }
-        ucur = __shfl_sync(kFull, u, max(count - 1, 0));
-        if (lane >= count) u = -1;
         const uint32_t nb = meta >> 16, rk = meta & 255u, rv = (meta >> 8) & 255u;
         const uint32_t kb = nb * vecb(rk);                      // bytes of the K part
         const uint32_t sk = updf ? 0u : (kb & 15u);             // bytes between the last 16-B boundary and the V part
         const uint32_t kc = (kb + 15u) >> 4, vc = (sk + nb * vecb(rv) + 15u) >> 4;  // 16-B units staged in phase 1 / 2
         const uint32_t voff = updf ? off16 : off16 + (kb >> 4);
-        const int pu = __shfl_up_sync(kFull, u, 1);
         const uint32_t pmeta = __shfl_up_sync(kFull, meta, 1), pkc = __shfl_up_sync(kFull, kc, 1);
         const uint32_t pvc = __shfl_up_sync(kFull, vc, 1), pupd = __shfl_up_sync(kFull, updf, 1);
-        const bool follows = lane > 0 && lane < count && u == pu && ((meta ^ pmeta) & 0xffffu) == 0u && nb != 0u &&
+        const bool follows = lane > 0 && lane < count && ((meta ^ pmeta) & 0xffffu) == 0u && nb != 0u &&
                              (pmeta >> 16) != 0u && kc + pkc <= (uint32_t)kGroupMax16 && vc + pvc <= (uint32_t)kGroupMax16 &&
                              !updf && !pupd;
         const unsigned fm = __ballot_sync(kFull, follows);
@@ -269,10 +239,10 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             GDesc a, b;
             a.off0 = off16; a.off1 = two ? off1 : 0u;
             a.x = kc | ((two ? kc1 : 0u) << 8) | (nb << 16) | ((two ? nb1 : 0u) << 20) | (rk << 24);
-            a.y = (uint32_t)u | (updf << 16);
+            a.y = updf;
             b.off0 = voff; b.off1 = two ? voff1 : 0u;
             b.x = vc | ((two ? vc1 : 0u) << 8) | (sk << 16) | ((two ? sk1 : 0u) << 20) | (rv << 24);
-            b.y = (uint32_t)u | (updf << 16) | (nb << 20) | ((two ? nb1 : 0u) << 24);
+            b.y = updf | (nb << 4) | ((two ? nb1 : 0u) << 8);
             d1[slot] = a;
             d2[slot] = b;
         }
@@ -309,32 +279,26 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     };
 
     // =====================================================================================
-    // Phase 1: QK.  Logits (log2 domain, scaled) -> logit cache; per-(unit, head) maxima -> global.
+    // Phase 1: QK.  Logits (log2 domain, scaled) -> logit cache; per-head maxima -> the CTA's table.
     // =====================================================================================
-    uint32_t qa[8][2];
-    float mxA = -INFINITY, mxB = -INFINITY;  // this lane's maxima for heads 2qq, 2qq+1 of the current unit
-    int cur_unit = -1;
+    float mxA = -INFINITY, mxB = -INFINITY;  // this lane's maxima for heads 2qq, 2qq+1
     uint32_t calib = 0u;
     // this lane's slots inside a block's logits ([head][token] floats): phase 1 writes token gq of heads 2qq, 2qq+1;
     // phase 2 reads tokens 2qq, 2qq+1 of head gq
     const uint32_t zw = (uint32_t)(16 * qq + gq) * 4u, zr = (uint32_t)(8 * gq + 2 * qq) * 4u;
 
-    // The warp has seen every block it holds of cur_unit: fold its maxima into the CTA's table
-    auto publish_max = [&]() {
-        const int slot = cur_unit - u_first;
-        if (slot >= kCtaUnits) return;  // (a CTA that holds many tiny units: phase 2 rescans the warp's own logits)
-#pragma unroll
-        for (int o = 4; o < 32; o <<= 1) {
-            mxA = fmaxf(mxA, __shfl_xor_sync(kFull, mxA, o));
-            mxB = fmaxf(mxB, __shfl_xor_sync(kFull, mxB, o));
-        }
-        if (gq == 0) {  // lanes 0..3 hold heads 2qq, 2qq+1
-            if (2 * qq < G) atomicMax(&s_umax[slot][2 * qq], fkey(mxA));
-            if (2 * qq + 1 < G) atomicMax(&s_umax[slot][2 * qq + 1], fkey(mxB));
-        }
-    };
-
     if (n_total > 0) {
+        // q[head gq][32qq .. 32qq+31]: k-step ks uses channels 32qq + 4ks .. + 3
+        uint32_t qa[8][2];
+        {
+            const uint4* qrow = reinterpret_cast<const uint4*>(q + (row + gq) * kD + 32 * qq);
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                if (gq < G) v = __ldg(qrow + h);
+                qa[2 * h][0] = v.x; qa[2 * h][1] = v.y; qa[2 * h + 1][0] = v.z; qa[2 * h + 1][1] = v.w;
+            }
+        }
         int bposi = 0, gposi = 0, gposc = 0, bposc = 0;
 #pragma unroll 1
         for (;;) {
@@ -348,7 +312,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 if (!ring_alloc(c0 + c1, off)) break;
                 if (lane == 0) {
                     const uint32_t bar = bar0 + 8 * si, dst = ring0 + off;
-                    const unsigned long long src = (d.y & 0x10000u) ? reinterpret_cast<unsigned long long>(upd_k) : slice;
+                    const unsigned long long src = d.y ? reinterpret_cast<unsigned long long>(upd_k) : slice;
                     mbar_expect_tx(bar, c0 + c1);
                     if (c0) bulk_g2s(dst, src + ((unsigned long long)d.off0 << 4), c0, bar);
                     if (c1) bulk_g2s(dst + c0, src + ((unsigned long long)d.off1 << 4), c1, bar);
@@ -361,7 +325,6 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
 
             // ---- consume the oldest group
             const GDesc d = d1[gposc & (kDesc - 1)];
-            const int u = (int)(d.y & 0xffffu);
             const int r_k = (int)(d.x >> 24);
             const int nb0 = (int)((d.x >> 16) & 15u), nb1 = (int)((d.x >> 20) & 15u);
             const bool two = nb1 != 0;
@@ -374,21 +337,6 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 ++gposc;
                 bposc += two ? 2 : 1;
                 continue;
-            }
-            if (u != cur_unit) {
-                if (cur_unit >= 0) publish_max();
-                cur_unit = u;
-                mxA = mxB = -INFINITY;
-                const int bi = u / g.n_kv_heads, hk = u % g.n_kv_heads;
-                // q[head gq][32qq .. 32qq+31]: k-step ks uses channels 32qq + 4ks .. + 3
-                const uint4* qrow = reinterpret_cast<const uint4*>(
-                    q + ((size_t)bi * g.n_q_heads + (size_t)hk * g.group + gq) * kD + 32 * qq);
-#pragma unroll
-                for (int h = 0; h < 4; ++h) {
-                    uint4 v = make_uint4(0u, 0u, 0u, 0u);
-                    if (gq < g.group) v = __ldg(qrow + h);
-                    qa[2 * h][0] = v.x; qa[2 * h][1] = v.y; qa[2 * h + 1][0] = v.z; qa[2 * h + 1][1] = v.w;
-                }
             }
             const bool full = nb0 == kB && (!two || nb1 == kB);
 
@@ -443,7 +391,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                     if (2 * qq < G) sts_f32(za, zA0);
                     if (2 * qq + 1 < G) sts_f32(za + 32, zB0);
                 } else {
-                    float* z0 = scr.zbuf + (size_t)(lo + bposc) * (size_t)(8 * G) + (zw >> 2);
+                    float* z0 = zglob + (size_t)bposc * (size_t)(8 * G) + (zw >> 2);
                     if (2 * qq < G) z0[0] = zA0;
                     if (2 * qq + 1 < G) z0[8] = zB0;
                 }
@@ -453,20 +401,10 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                         if (2 * qq < G) sts_f32(za, zA1);
                         if (2 * qq + 1 < G) sts_f32(za + 32, zB1);
                     } else {
-                        float* z1 = scr.zbuf + (size_t)(lo + bposc + 1) * (size_t)(8 * G) + (zw >> 2);
+                        float* z1 = zglob + (size_t)(bposc + 1) * (size_t)(8 * G) + (zw >> 2);
                         if (2 * qq < G) z1[0] = zA1;
                         if (2 * qq + 1 < G) z1[8] = zB1;
                     }
-                }
-            }
-            else {  // an invalid `sel` entry: its block takes no part; -inf keeps every later reader of the cache honest
-                if (bposc < zcap) {
-                    if (lane < 8 * G) sts_f32(zs0 + (uint32_t)bposc * zstride + 4u * (uint32_t)lane, -INFINITY);
-                    if (lane + 32 < 8 * G) sts_f32(zs0 + (uint32_t)bposc * zstride + 4u * (uint32_t)lane + 128u, -INFINITY);
-                } else {
-                    float* zg = scr.zbuf + (size_t)(lo + bposc) * (size_t)(8 * G) + lane;
-                    if (lane < 8 * G) zg[0] = -INFINITY;
-                    if (lane + 32 < 8 * G) zg[32] = -INFINITY;
                 }
             }
             __syncwarp();  // every lane is done reading the slot
@@ -474,114 +412,55 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             ++gposc;
             bposc += two ? 2 : 1;
         }
-        if (!kGatherOnly && cur_unit >= 0) publish_max();
+        if (!kGatherOnly) {  // the warp's maxima -> the CTA's table
+#pragma unroll
+            for (int o = 4; o < 32; o <<= 1) {
+                mxA = fmaxf(mxA, __shfl_xor_sync(kFull, mxA, o));
+                mxB = fmaxf(mxB, __shfl_xor_sync(kFull, mxB, o));
+            }
+            if (gq == 0) {  // lanes 0..3 hold heads 2qq, 2qq+1
+                if (2 * qq < G) atomicMax(&s_max[2 * qq], fkey(mxA));
+                if (2 * qq + 1 < G) atomicMax(&s_max[2 * qq + 1], fkey(mxB));
+            }
+        }
     }
 
-    if (!kGatherOnly) __syncthreads();  // the CTA's table of maxima is complete
+    // =====================================================================================
+    // The cluster's CTAs exchange their maxima through distributed shared memory.
+    // =====================================================================================
+    float Mraw = -INFINITY;  // the unit's maximum logit of head gq (log2 domain)
+    if (!kGatherOnly) {
+        cluster_sync();  // every CTA's table is complete and visible to the cluster (also a CTA barrier)
+        if (gq < G) {
+            uint32_t k = 0u;
+            const uint32_t a = smem_u32(&s_max[gq]);
+#pragma unroll 1
+            for (int r = 0; r < C; ++r) k = max(k, ld_dsmem_u32(dsmem_addr(a, (uint32_t)r)));
+            Mraw = k == 0u ? -INFINITY : funkey(k);
+            if (warp == 0 && qq == 0) s_M[gq] = Mraw;
+        }
+    }
+    const float Mh = Mraw == -INFINITY ? 0.f : Mraw;  // 0 if the unit holds no valid token
 
     // =====================================================================================
     // Phase 2: softmax sums over every selected token, PV over the blocks that matter.
     // =====================================================================================
     float acc[8][4];    // O^T tile i: rows gq / gq+8 = channels 16gq + 2i / + 1, columns 2qq, 2qq+1 = heads
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
     float lsum = 0.f;   // this lane's share of the softmax sum of head gq
-    float Mh = 0.f;     // reference of head gq: the CTA's maximum logit of the unit (log2 domain); 0 if it holds no valid token
-    float Mraw = -INFINITY;
-    cur_unit = -1;
     unsigned st_vblocks = 0u, st_vbytes = 0u;
 
     // logits of head gq, tokens 2qq, 2qq+1 of block i of the range (shared-memory cache, or global scratch beyond it)
     auto z_pair = [&](int i) -> float2 {
         if (i < zcap) return lds_f32x2(zs0 + (uint32_t)i * zstride + zr);
-        return __ldcg(reinterpret_cast<const float2*>(scr.zbuf + (size_t)(lo + i) * (size_t)(8 * G) + (zr >> 2)));
-    };
-
-    // end of a unit inside this warp's range.  `last`: the range is finished and the ring is idle, so the
-    // partial lives in this warp's own shared memory (record 2w + 1); a unit that ends inside the range
-    // leaves its partial in global scratch (2w).
-    auto flush = [&](bool last) {
-        const int u = cur_unit;
-        const int a = s_cum[u], b = s_cum[u + 1];
-        lsum += __shfl_xor_sync(kFull, lsum, 1);
-        lsum += __shfl_xor_sync(kFull, lsum, 2);  // lanes (gq, *): the warp's sum of head gq
-        const int hA = 2 * qq, hB = 2 * qq + 1;
-        const float lA = __shfl_sync(kFull, lsum, 4 * hA), lB = __shfl_sync(kFull, lsum, 4 * hB);
-        const float mA = __shfl_sync(kFull, Mraw, 4 * hA), mB = __shfl_sync(kFull, Mraw, 4 * hB);
-        const bool whole = lo <= a && b <= hi;  // the whole unit was processed by this warp: final result
-        float fA = 1.f, fB = 1.f;
-        float* po;
-        if (whole) {
-            po = out + ((size_t)(u / g.n_kv_heads) * g.n_q_heads + (size_t)(u % g.n_kv_heads) * G) * kD;
-            fA = lA > 0.f ? 1.f / lA : 0.f;
-            fB = lB > 0.f ? 1.f / lB : 0.f;
-        } else {
-            po = last ? reinterpret_cast<float*>(wbase) : scr.part_o + (size_t)gw * 2 * (size_t)(G * kD);
-        }
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            const int ch = 16 * gq + 2 * i;
-            if (hA < G) *reinterpret_cast<float2*>(po + hA * kD + ch) = make_float2(acc[i][0] * fA, acc[i][2] * fA);
-            if (hB < G) *reinterpret_cast<float2*>(po + hB * kD + ch) = make_float2(acc[i][1] * fB, acc[i][3] * fB);
-        }
-        if (whole) {
-            if (lse != nullptr && gq == 0) {
-                float* pl = lse + (size_t)(u / g.n_kv_heads) * g.n_q_heads + (size_t)(u % g.n_kv_heads) * G;
-                if (hA < G) pl[hA] = lA > 0.f ? (mA + log2f(lA)) * kLn2 : -INFINITY;
-                if (hB < G) pl[hB] = lB > 0.f ? (mB + log2f(lB)) * kLn2 : -INFINITY;
-            }
-        } else {
-            const int rec = warp * 2 + (last ? 1 : 0);
-            if (gq == 0) {
-                if (hA < G) { s_ml[rec][hA][0] = mA; s_ml[rec][hA][1] = lA; }
-                if (hB < G) { s_ml[rec][hB][0] = mB; s_ml[rec][hB][1] = lB; }
-            }
-            if (lane == 0) s_unit[rec] = u;
-        }
-    };
-
-    // reference of unit u for this warp: the CTA's maxima; beyond the table, the maxima of the warp's own logits
-    // of the unit, which are blocks [p0, p1) of its range
-    auto begin_unit = [&](int u, int p0) {
-        cur_unit = u;
-        lsum = 0.f;
-#pragma unroll
-        for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
-        const int slot = u - u_first;
-        if (slot < kCtaUnits) {
-            Mraw = gq < G ? funkey(s_umax[slot][gq]) : -INFINITY;
-        } else {
-            // lane l looks at elements l and l + 32 of each block's [head][token] floats: heads l / 8 and l / 8 + 4
-            const int p1 = min(n_total, s_cum[u + 1] - lo);
-            float m_lo = -INFINITY, m_hi = -INFINITY;
-#pragma unroll 1
-            for (int i = p0; i < p1; ++i) {
-                float v0 = -INFINITY, v1 = -INFINITY;
-                if (i < zcap) {
-                    const uint32_t a = zs0 + (uint32_t)i * zstride + 4u * (uint32_t)lane;
-                    if (lane < 8 * G) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v0) : "r"(a));
-                    if (lane + 32 < 8 * G) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v1) : "r"(a + 128u));
-                } else {
-                    const float* zg = scr.zbuf + (size_t)(lo + i) * (size_t)(8 * G) + lane;
-                    if (lane < 8 * G) v0 = __ldcg(zg);
-                    if (lane + 32 < 8 * G) v1 = __ldcg(zg + 32);
-                }
-                m_lo = fmaxf(m_lo, v0);
-                m_hi = fmaxf(m_hi, v1);
-            }
-#pragma unroll
-            for (int o = 1; o < 8; o <<= 1) {
-                m_lo = fmaxf(m_lo, __shfl_xor_sync(kFull, m_lo, o));
-                m_hi = fmaxf(m_hi, __shfl_xor_sync(kFull, m_hi, o));
-            }
-            const float t_lo = __shfl_sync(kFull, m_lo, 8 * (gq & 3)), t_hi = __shfl_sync(kFull, m_hi, 8 * (gq & 3));
-            Mraw = gq < G ? (gq < 4 ? t_lo : t_hi) : -INFINITY;
-        }
-        Mh = Mraw == -INFINITY ? 0.f : Mraw;
+        return __ldcg(reinterpret_cast<const float2*>(zglob + (size_t)i * (size_t)(8 * G) + (zr >> 2)));
     };
 
     if (n_total > 0) {
         // the range's descriptors are still in shared memory unless it was longer than one ring: then describe again
         const bool redo = gbuilt > kDesc;
-        if (redo) { bbuilt = 0; gbuilt = 0; ucur = find_unit(s_cum, g.n_units, lo); }
+        if (redo) { bbuilt = 0; gbuilt = 0; }
         const int gtotal = gbuilt;
         int bposd = 0, gposd = 0;  // blocks / groups decided
 #pragma unroll 1
@@ -592,13 +471,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 if (redo) { if (gposd == gbuilt) describe(min(kDescribe, n_total - bbuilt)); }
                 else if (gposd == gtotal) break;
                 const GDesc d = d2[gposd & (kDesc - 1)];
-                const int u = (int)(d.y & 0xffffu);
-                if (!kGatherOnly && u != cur_unit) {
-                    if (pend != 0) break;  // drain the unit's groups in flight first
-                    if (cur_unit >= 0) flush(false);
-                    begin_unit(u, bposd);
-                }
-                uint32_t nb0 = (d.y >> 20) & 15u, nb1 = (d.y >> 24) & 15u;
+                uint32_t nb0 = (d.y >> 4) & 15u, nb1 = (d.y >> 8) & 15u;
                 const bool two = nb1 != 0u;
                 bool need0 = nb0 != 0u, need1 = two;
                 float add = 0.f;
@@ -623,15 +496,15 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                     if (!ring_alloc(c0 + c1, off)) break;  // no room yet: decide this group again after a consume
                     if (lane == 0) {
                         const uint32_t bar = bar0 + 8 * si, dst = ring0 + off;
-                        const unsigned long long src = (d.y & 0x10000u) ? reinterpret_cast<unsigned long long>(upd_v) : slice;
+                        const unsigned long long src = (d.y & 1u) ? reinterpret_cast<unsigned long long>(upd_v) : slice;
                         mbar_expect_tx(bar, c0 + c1);
                         bulk_g2s(dst, src + ((unsigned long long)off0 << 4), c0, bar);
                         if (c1) bulk_g2s(dst + c0, src + ((unsigned long long)off1 << 4), c1, bar);
                         GDesc e;
                         e.off0 = sk0 | (sk1 << 4) | (c0 << 8);                   // skews of the V parts, bytes of the first chunk
-                        e.off1 = (uint32_t)bposd;                                // index of the group's first block in the range
+                        e.off1 = (uint32_t)bposd + shift;                        // index of the first WALKED block in the range
                         e.x = d.x;
-                        e.y = nb0 | (nb1 << 4) | (shift << 8);                   // shift: only the group's second block is walked
+                        e.y = nb0 | (nb1 << 4);
                         slot_grp[si] = e;
                     }
                     st_vblocks += nb1 ? 2u : 1u;
@@ -642,16 +515,12 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 ++gposd;
                 bposd += two ? 2 : 1;
             }
-            if (pend == 0) {
-                if (bposd >= n_total) break;
-                continue;  // (a unit boundary with nothing in flight: the next pass begins the unit)
-            }
+            if (pend == 0) break;  // (nothing in flight means the decide loop ran to the end of the range)
 
             // ---- consume the oldest group in flight: PV
             const GDesc d = slot_grp[sc];
             const int r_v = (int)(d.x >> 24);
             const int nb0 = (int)(d.y & 15u), nb1 = (int)((d.y >> 4) & 15u), pos = (int)d.off1;
-            const uint32_t zsh = (d.y >> 8) & 1u;
             const bool two = nb1 != 0;
             const uint32_t vb0 = ring0 + slot_tab[sc].x + (d.off0 & 15u);
             const uint32_t vb1 = ring0 + slot_tab[sc].x + (d.off0 >> 8) + ((d.off0 >> 4) & 15u);
@@ -666,8 +535,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             // exactly the B fragments of O^T += V^T P^T (k = token, n = head)
             float2 za = make_float2(-INFINITY, -INFINITY), zb = za;
             if (gq < G) {
-                za = z_pair(pos + (int)zsh);
-                if (two) zb = z_pair(pos + (int)zsh + 1);
+                za = z_pair(pos);
+                if (two) zb = z_pair(pos + 1);
             }
             const float e00 = ex2(za.x - Mh), e01 = ex2(za.y - Mh), e10 = ex2(zb.x - Mh), e11 = ex2(zb.y - Mh);
             const uint32_t ph0 = pack_bf16(e00, e01), ph1 = pack_bf16(e10, e11);
@@ -727,137 +596,68 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             __syncwarp();  // every lane is done reading the slot
             ring_release();
         }
-        if (!kGatherOnly && cur_unit >= 0) flush(true);
     }
     if (kGatherOnly) {  // keep the read-back alive; nothing else is written
-        if (calib == 0x9e3779b9u && lane == 0) scr.part_l[(size_t)gw * 2 * (2 * kMaxGroup)] = 0.f;
+        if (calib == 0x9e3779b9u && lane == 0) scr.stats[7] = 1ull;
         return;
     }
     if (lane == 0 && st_vblocks != 0u) {
         atomicAdd(scr.stats + 1, (unsigned long long)st_vblocks);
         atomicAdd(scr.stats + 2, (unsigned long long)st_vbytes);
     }
-    if (threadIdx.x == 0 && blockIdx.x == 0) atomicAdd(scr.stats + 0, (unsigned long long)T);
+    if (threadIdx.x == 0 && rank == 0) atomicAdd(scr.stats + 0, (unsigned long long)T);
 
-    // ---- step 3d, fused: add the warps' partials; finish units that span several CTAs.
-    // Records are in warp order (2w = head, 2w + 1 = tail), hence in non-decreasing unit order: the
-    // partials of one unit form a run.  Thread tid owns four consecutive output channels of one head.
-    // All partials of a unit are relative to the same maximum, so folding is plain addition (the
-    // split-K rule of oracle pin P10 with equal references), always in the same order.
-    __syncthreads();  // orders the warps' partials (shared memory, or global scratch from flush(false))
-    const int GD = G * kD;
-    const size_t cta_slot_base = (size_t)gridDim.x * kWarps * 2;
-    const int tid = threadIdx.x;
-    // GD / 4 threads fold one unit, so a CTA folds kNT / (GD / 4) units side by side
-    const int tpr = GD / 4, nslots = max(1, kNT / tpr);
-    const int rs = tid / tpr, e = 4 * (tid - rs * tpr), h = e >> 7;
-    // each lane keeps the unit of record `lane`: searches and membership are votes
-    const int myu0 = lane < kRec ? s_unit[lane] : -1;
-    int run = -1;
-#pragma unroll 1
-    for (;;) {
-        // the next <= nslots units with partial records, ascending; `mine` = the one this thread folds
-        int mine = -1, last = run;
-#pragma unroll 1
-        for (int k = 0; k < nslots; ++k) {
-            const int nxt = __reduce_min_sync(kFull, myu0 > last ? myu0 : 0x7fffffff);
-            if (nxt == 0x7fffffff) break;
-            last = nxt;
-            if (k == rs) mine = nxt;
-        }
-        if (last == run) break;
-        run = last;
-        if (mine < 0) continue;  // uniform over a warp: GD / 4 is a multiple of 32
-        // records of this unit: bit r of `recs` (tail partials are the odd records, head partials the even ones)
-        const unsigned recs = __ballot_sync(kFull, myu0 == mine);
-        const int a = s_cum[mine], b = s_cum[mine + 1];
-        const bool whole = clo <= a && b <= chi;
-        const size_t row = (size_t)(mine / g.n_kv_heads) * g.n_q_heads + (size_t)(mine % g.n_kv_heads) * G;
-        float4 O = make_float4(0.f, 0.f, 0.f, 0.f);
-        float Lr = 0.f, Mr = -INFINITY;
-        {
-            // tail partials (record 2w + 1, in warp w's shared memory): straight-line, every load independent
-            float mw[kWarps], lw[kWarps];
-            float4 ow[kWarps];
+    // =====================================================================================
+    // Step 3d.  Every partial of the unit is relative to the same maximum, so combining is plain addition (the
+    // split-K rule of oracle pin P10 with equal references), always in the same order: warps inside the CTA, then
+    // the cluster's CTAs.
+    // =====================================================================================
+    {
+        // the warp's partial: O^T fragments -> [head][channel] floats in the warp's (now idle) ring; sums -> s_l
+        lsum += __shfl_xor_sync(kFull, lsum, 1);
+        lsum += __shfl_xor_sync(kFull, lsum, 2);  // lanes (gq, *): the warp's sum of head gq
+        if (qq == 0 && gq < G) s_l[warp][gq] = lsum;
+        float* po = reinterpret_cast<float*>(wbase);
+        const int hA = 2 * qq, hB = 2 * qq + 1;
 #pragma unroll
-            for (int w = 0; w < kWarps; ++w) {
-                const bool mem = (recs >> (2 * w + 1)) & 1u;
-                const float2 ml = *reinterpret_cast<const float2*>(&s_ml[2 * w + 1][h][0]);
-                ow[w] = *reinterpret_cast<const float4*>(smem + w * kWS + 4 * e);
-                mw[w] = mem ? ml.x : -INFINITY;
-                lw[w] = mem ? ml.y : 0.f;
-                Mr = fmaxf(Mr, mw[w]);
-            }
-            // head partials (record 2w, in global scratch): at most one per CTA in practice (the unit entering its range)
-#pragma unroll 1
-            for (unsigned m = recs & 0x55555555u; m; m &= m - 1u) Mr = fmaxf(Mr, s_ml[2 * ((__ffs(m) - 1) >> 1)][h][0]);
-            const float Mb = Mr == -INFINITY ? 0.f : Mr;
-#pragma unroll
-            for (int w = 0; w < kWarps; ++w) {
-                const float wt = ex2(mw[w] - Mb);  // 1 inside a CTA's table; 0 for a record of another unit (its O may be stale bits)
-                Lr = fmaf(lw[w], wt, Lr);
-                if (wt != 0.f) { O.x = fmaf(ow[w].x, wt, O.x); O.y = fmaf(ow[w].y, wt, O.y); O.z = fmaf(ow[w].z, wt, O.z); O.w = fmaf(ow[w].w, wt, O.w); }
-            }
-#pragma unroll 1
-            for (unsigned m = recs & 0x55555555u; m; m &= m - 1u) {
-                const int w = (__ffs(m) - 1) >> 1;
-                const float wt = ex2(s_ml[2 * w][h][0] - Mb);
-                Lr = fmaf(s_ml[2 * w][h][1], wt, Lr);
-                const float4 o = __ldcg(reinterpret_cast<const float4*>(
-                    scr.part_o + ((size_t)blockIdx.x * kWarps + w) * 2 * (size_t)GD + e));
-                O.x = fmaf(o.x, wt, O.x); O.y = fmaf(o.y, wt, O.y); O.z = fmaf(o.z, wt, O.z); O.w = fmaf(o.w, wt, O.w);
-            }
+        for (int i = 0; i < 8; ++i) {
+            const int ch = 16 * gq + 2 * i;
+            if (hA < G) *reinterpret_cast<float2*>(po + hA * kD + ch) = make_float2(acc[i][0], acc[i][2]);
+            if (hB < G) *reinterpret_cast<float2*>(po + hB * kD + ch) = make_float2(acc[i][1], acc[i][3]);
         }
-        if (whole) {
-            const float inv = Lr > 0.f ? 1.f / Lr : 0.f;
-            *reinterpret_cast<float4*>(out + row * kD + e) = make_float4(O.x * inv, O.y * inv, O.z * inv, O.w * inv);
-            if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = Lr > 0.f ? (Mr + log2f(Lr)) * kLn2 : -INFINITY;
-            continue;
-        }
-        // The unit spans CTAs c_first .. c_last.  This thread stores its four channels of the CTA's partial (slot 1 for
-        // c_first: the unit starts inside it, else slot 0) and takes a ticket of its own channel quad; the last of the
-        // sharers' threads to arrive adds the partials in CTA order.  Every quad proceeds on its own: no barrier.
-        const int c_first = (int)cs.owner((unsigned)a >> 1), c_last = (int)cs.owner(((unsigned)b - 1u) >> 1);
-        const size_t slot = cta_slot_base + blockIdx.x * 2 + (a < clo ? 0 : 1);
-        float* my_o = scr.part_o + slot * GD + e;
-        float* my_l = scr.part_l + slot * (2 * kMaxGroup) + 2 * h;
-        __stcg(reinterpret_cast<float4*>(my_o), O);
-        if ((e & (kD - 1)) == 0) __stcg(reinterpret_cast<float2*>(my_l), make_float2(Mr, Lr));
-        int32_t* tk = scr.ticket + (size_t)mine * (kMaxGroup * kD / 4) + (e >> 2);
-        int old;  // release this thread's partial, acquire the other sharers'
-        asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(tk) : "memory");
-        if (old != c_last - c_first) continue;
-        *tk = 0;  // self-cleaning: every sharer has arrived
-        float Mx = -INFINITY, Lx = 0.f;
-        float4 Ox = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll 1
-        for (int c0 = c_first; c0 <= c_last; c0 += 4) {  // four partials' loads in flight at once; LSE rule (oracle pin P10)
-            float2 pm[4];
-            float4 po[4];
-#pragma unroll
-            for (int t = 0; t < 4; ++t) {
-                const int c = min(c0 + t, c_last);  // a repeated partial gets weight 0 below
-                const size_t sl = cta_slot_base + (size_t)c * 2 + (c == c_first ? 1 : 0);
-                pm[t] = __ldcg(reinterpret_cast<const float2*>(scr.part_l + sl * (2 * kMaxGroup) + 2 * h));
-                po[t] = __ldcg(reinterpret_cast<const float4*>(scr.part_o + sl * (size_t)GD + e));
-                if (c0 + t > c_last) pm[t] = make_float2(-INFINITY, 0.f);
-            }
-            const float Mn = fmaxf(fmaxf(Mx, fmaxf(pm[0].x, pm[1].x)), fmaxf(pm[2].x, pm[3].x));
-            const float Mb = Mn == -INFINITY ? 0.f : Mn;
-            const float c_old = ex2(Mx - Mb);
-            Lx *= c_old; Ox.x *= c_old; Ox.y *= c_old; Ox.z *= c_old; Ox.w *= c_old; Mx = Mn;
-#pragma unroll
-            for (int t = 0; t < 4; ++t) {
-                const float w = ex2(pm[t].x - Mb);
-                Lx = fmaf(pm[t].y, w, Lx);
-                if (w != 0.f) { Ox.x = fmaf(po[t].x, w, Ox.x); Ox.y = fmaf(po[t].y, w, Ox.y); Ox.z = fmaf(po[t].z, w, Ox.z); Ox.w = fmaf(po[t].w, w, Ox.w); }
-            }
-        }
-        const float inv = Lx > 0.f ? 1.f / Lx : 0.f;
-        *reinterpret_cast<float4*>(out + row * kD + e) = make_float4(Ox.x * inv, Ox.y * inv, Ox.z * inv, Ox.w * inv);
-        if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = Lx > 0.f ? (Mx + log2f(Lx)) * kLn2 : -INFINITY;
     }
+    __syncthreads();
+    const int GD = G * kD;
+    for (int e = threadIdx.x; e < GD; e += kNT) {  // the CTA's partial
+        float o = 0.f;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) o += *reinterpret_cast<const float*>(smem + w * kWS + 4 * e);
+        s_cta_o[e] = o;
+    }
+    if (threadIdx.x < G) {
+        float l = 0.f;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) l += s_l[w][threadIdx.x];
+        s_cta_l[threadIdx.x] = l;
+    }
+    cluster_sync();  // every CTA's partial is complete and visible to the cluster
+    if (rank == 0) {
+        const uint32_t ao = smem_u32(s_cta_o), al = smem_u32(s_cta_l);
+        for (int e = threadIdx.x; e < GD; e += kNT) {
+            const int h = e >> 7;
+            float o = 0.f, l = 0.f;
+#pragma unroll 1
+            for (int r = 0; r < C; ++r) {
+                o += ld_dsmem_f32(dsmem_addr(ao + 4u * (uint32_t)e, (uint32_t)r));
+                l += ld_dsmem_f32(dsmem_addr(al + 4u * (uint32_t)h, (uint32_t)r));
+            }
+            out[row * kD + e] = l > 0.f ? o / l : 0.f;
+            if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = l > 0.f ? (s_M[h] + log2f(l)) * kLn2 : -INFINITY;
+        }
+    }
+    cluster_sync();  // no CTA leaves (and releases its shared memory) before the first one has read it
 }
+
 
 // calibration row (i) of SURVEY 8(d): a plain streaming read of `bytes` bytes in the attention kernel's launch shape
 __global__ void __launch_bounds__(kWarps * 32, 1)
@@ -889,39 +689,78 @@ mkv_stream_read_kernel(const uint4* __restrict__ base, unsigned long long n16, u
 
 }  // namespace
 
-int attention_partial_slots(int sm_count) { return sm_count * kWarps * 2 + sm_count * 2; }
-size_t attention_ticket_ints(const CacheGeom& g) { return (size_t)g.n_units * (kMaxGroup * kD / 4); }
+// logit scratch: per unit one entry of 8 G floats per position of its block stream (selected + update-buffer blocks)
+size_t attention_z_unit_stride(const CacheGeom& g) { return (size_t)g.score_stride + 1 + (size_t)(g.L + kB - 1) / kB; }
+size_t attention_zbuf_floats(const CacheGeom& g) { return (size_t)g.n_units * attention_z_unit_stride(g) * 8 * (size_t)g.group; }
 
-// logit scratch: one entry of 8 G floats per position of the block stream (selected blocks + update-buffer blocks)
-size_t attention_zbuf_floats(const CacheGeom& g) {
-    return (size_t)g.n_units * ((size_t)g.score_stride + 1 + (size_t)(g.L + kB - 1) / kB) * 8 * (size_t)g.group;
+// Cluster size for a layer of n_units units: the largest power of two C <= 16 with n_units * C <= SMs whose clusters
+// can all be resident at once (one CTA per SM; a cluster lives inside one GPC), else 1.
+template <bool GATHER>
+static int pick_cluster(const CacheGeom& g, int smem, int sm_count) {
+    cudaFuncSetAttribute(mkv_packed_attention_kernel<GATHER>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    for (int C = kMaxCluster; C > 1; C >>= 1) {
+        if ((long long)g.n_units * C > sm_count) continue;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(g.n_units * C); cfg.blockDim = dim3(kWarps * 32); cfg.dynamicSmemBytes = smem;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, mkv_packed_attention_kernel<GATHER>, &cfg) == cudaSuccess && n >= g.n_units)
+            return C;
+        cudaGetLastError();
+    }
+    return 1;
 }
 
 template <bool GATHER>
 static cudaError_t launch_attention_cfg(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
                                         const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
                                         const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v,
-                                        const int32_t* upd_count, int sm_count, cudaStream_t s) {
-    const int smem = kWarps * kWS + (g.n_units + 1) * 4;
+                                        const int32_t* upd_count, int sm_count, int* cluster_cache, cudaStream_t s) {
+    const int smem = kWarps * kWS + kMaxGroup * kD * 4;
     // the dynamic shared-memory opt-in is a per-device attribute of the function: set it on every launch (a cheap
     // host-side call) so that caches on different devices of one process are independent
     cudaError_t e = cudaFuncSetAttribute(mkv_packed_attention_kernel<GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
-    return launch_pdl(mkv_packed_attention_kernel<GATHER>, dim3(sm_count), dim3(kWarps * 32), (size_t)smem, s, g, lv, q, sel,
-                      sel_count, k_max, scale * kLog2e, out, lse, scr, upd_k, upd_v, upd_count);
+    if (*cluster_cache == 0) *cluster_cache = pick_cluster<GATHER>(g, smem, sm_count);  // (normally chosen at cache creation)
+    const int C = *cluster_cache;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(g.n_units * C); cfg.blockDim = dim3(kWarps * 32); cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute attr[2];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    attr[1].id = cudaLaunchAttributeClusterDimension;
+    attr[1].val.clusterDim.x = C; attr[1].val.clusterDim.y = 1; attr[1].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 2;
+    return cudaLaunchKernelEx(&cfg, mkv_packed_attention_kernel<GATHER>, g, lv, q, sel, sel_count, k_max, scale * kLog2e, out,
+                              lse, scr, upd_k, upd_v, upd_count, C);
 }
 
 cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
                              const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
                              const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v,
-                             const int32_t* upd_count, int sm_count, cudaStream_t s, int* n_kernels, bool gather_only) {
-    if (g.n_units > kMaxUnitsSmem) return cudaErrorInvalidValue;
+                             const int32_t* upd_count, int sm_count, int* cluster_cache, cudaStream_t s, int* n_kernels,
+                             bool gather_only) {
     if (n_kernels) *n_kernels = 1;
     if (gather_only)
         return launch_attention_cfg<true>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, upd_count,
-                                          sm_count, s);
+                                          sm_count, cluster_cache + 1, s);
     return launch_attention_cfg<false>(g, lv, q, sel, sel_count, k_max, scale, out, lse, scr, upd_k, upd_v, upd_count,
-                                       sm_count, s);
+                                       sm_count, cluster_cache, s);
+}
+
+// choose the cluster sizes of both kernels for this cache (occupancy queries: host-side, not capturable)
+cudaError_t attention_prepare(const CacheGeom& g, int sm_count, int* cluster_cache) {
+    const int smem = kWarps * kWS + kMaxGroup * kD * 4;
+    cudaError_t e = cudaFuncSetAttribute(mkv_packed_attention_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(mkv_packed_attention_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    cluster_cache[0] = pick_cluster<false>(g, smem, sm_count);
+    cluster_cache[1] = pick_cluster<true>(g, smem, sm_count);
+    return cudaSuccess;
 }
 
 cudaError_t launch_stream_read(const uint8_t* base, unsigned long long bytes, int sm_count, unsigned long long* sink,

@@ -59,6 +59,7 @@ struct mkv_cache {
     int32_t* upd_cnt = nullptr;               // [n_layers] tokens buffered per unit (read by the attention kernel)
     std::vector<int32_t> upd_n;               // host mirror (every unit of a layer holds the same number)
     AttnScratch attn{};
+    int attn_cluster[2] = {0, 0};             // cluster size of the attention / gather-only kernel for this cache (0 = not chosen yet)
     PlanRec* plan = nullptr;                  // [n_layers][n_units][sel_cap]: what top-k tells attention about each selected block
     uint32_t generation = 1;                  // bumped by mkv_cache_reset: invalidates every plan record
     unsigned long long* sink = nullptr;
@@ -110,7 +111,7 @@ int mkv_cache_free(mkv_cache* c) {
     cudaSetDevice(c->desc.device);
     cudaDeviceSynchronize();
     void* ptrs[] = {c->arena, c->strat, c->tok_off, c->bk_off, c->unit_nseg, c->unit_ntok, c->counters,
-                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->upd_k, c->upd_v, c->upd_cnt, c->attn.part_o, c->attn.part_l, c->attn.ticket, c->attn.zbuf, c->attn.stats, c->plan, c->sink, c->rot_k, c->rot_v, c->q_rot, c->q_dev,
+                    c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->upd_k, c->upd_v, c->upd_cnt, c->attn.zbuf, c->attn.stats, c->plan, c->sink, c->rot_k, c->rot_v, c->q_rot, c->q_dev,
                     c->sel_dev, c->selcnt_dev, c->out_dev};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -154,7 +155,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     c->slice_bytes = per_layer;
 
     const size_t tu = (size_t)g.n_layers * g.n_units;
-    c->attn.slots = attention_partial_slots(c->sm_count);
+    c->attn.z_unit_stride = attention_z_unit_stride(g);
     c->sel_cap = g.score_stride + 1;
     const size_t upd_bytes = (size_t)g.n_layers * g.n_units * g.L * kD * 2;
     c->upd_n.assign(g.n_layers, 0);
@@ -177,9 +178,6 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         {(void**)&c->upd_k, upd_bytes},
         {(void**)&c->upd_v, upd_bytes},
         {(void**)&c->upd_cnt, (size_t)g.n_layers * 4 + 252},
-        {(void**)&c->attn.part_o, (size_t)c->attn.slots * g.group * kD * 4},
-        {(void**)&c->attn.part_l, (size_t)c->attn.slots * kMaxGroup * 2 * 4},
-        {(void**)&c->attn.ticket, attention_ticket_ints(g) * 4},
         {(void**)&c->attn.zbuf, attention_zbuf_floats(g) * 4},
         {(void**)&c->attn.stats, 64},
         {(void**)&c->plan, tu * (size_t)c->sel_cap * sizeof(PlanRec)},
@@ -203,13 +201,13 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     cudaMemset(c->counters, 0, (size_t)g.n_layers * 4 * 8);
     cudaMemset(c->dev_flags, 0, 256);
     cudaMemset(c->upd_cnt, 0, (size_t)g.n_layers * 4);
-    cudaMemset(c->attn.ticket, 0, attention_ticket_ints(g) * 4);
     cudaMemset(c->attn.stats, 0, 64);
     cudaMemset(c->plan, 0, tu * (size_t)c->sel_cap * sizeof(PlanRec));
     cudaMemset(c->strat, 0, tu * g.S_max * sizeof(StratRec));
     c->host_nseg.assign((size_t)g.n_layers * g.batch, 0);
     c->host_ntok.assign((size_t)g.n_layers * g.batch, 0);
-    cudaError_t e = cudaDeviceSynchronize();
+    cudaError_t e = attention_prepare(g, c->sm_count, c->attn_cluster);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) {
         mkv_cache_free(c);
         return fail(MKV_E_CUDA, "create: %s", cudaGetErrorString(e));
@@ -225,7 +223,6 @@ int mkv_cache_reset(mkv_cache* c, int32_t layer, void* stream) {
     cudaStream_t s = (cudaStream_t)stream;
     const int l0 = layer < 0 ? 0 : layer, l1 = layer < 0 ? g.n_layers : layer + 1;
     ++c->generation;  // plan records written before the reset no longer match
-    MKV_CUDA(cudaMemsetAsync(c->attn.ticket, 0, attention_ticket_ints(g) * 4, s));
     for (int l = l0; l < l1; ++l) {
         MKV_CUDA(cudaMemsetAsync(c->unit_nseg + (size_t)l * g.n_units, 0, (size_t)g.n_units * 4, s));
         MKV_CUDA(cudaMemsetAsync(c->unit_ntok + (size_t)l * g.n_units, 0, (size_t)g.n_units * 4, s));
@@ -341,7 +338,7 @@ int mkv_packed_attention(const mkv_cache* cc, int32_t layer, const void* q, cons
     const size_t upd_off = (size_t)layer * g.n_units * g.L * kD;
     MKV_CUDA(launch_attention(g, c->view(layer), (const uint16_t*)q, sel, sel_count, k_max, scale, out, lse_opt,
                               c->attn_scratch(layer), c->upd_k + upd_off, c->upd_v + upd_off, c->upd_cnt + layer,
-                              c->sm_count, (cudaStream_t)stream, &c->last_attn));
+                              c->sm_count, c->attn_cluster, (cudaStream_t)stream, &c->last_attn));
     return MKV_OK;
 }
 
@@ -357,7 +354,7 @@ int mkv_calibrate_gather(const mkv_cache* cc, int32_t layer, const int32_t* sel,
     int n = 0;
     MKV_CUDA(launch_attention(g, c->view(layer), c->q_dev, sel, sel_count, k_max, 1.f, c->out_dev, nullptr,
                               c->attn_scratch(layer), c->upd_k + upd_off, c->upd_v + upd_off, c->upd_cnt + layer,
-                              c->sm_count, (cudaStream_t)stream, &n, true));
+                              c->sm_count, c->attn_cluster, (cudaStream_t)stream, &n, true));
     return MKV_OK;
 }
 

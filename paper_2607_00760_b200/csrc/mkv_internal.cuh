@@ -117,24 +117,22 @@ __device__ __forceinline__ void plan_lookup(const CacheGeom& g, const LayerView&
 #endif
 
 struct AttnScratch {
-    float* part_o;        // [slots][G][D]   unnormalised partial outputs (<= 2 slots per warp and per CTA of the grid)
-    float* part_l;        // [slots][8][2]   (reference maximum in log2 units, partial softmax sum) per head
-    int32_t* ticket;      // [n_units][256]  per channel quad: arrivals of the CTAs sharing a unit (step 3d); zero between launches
-    float* zbuf;          // [z_cap][8 G]    logits of blocks that do not fit a warp's shared-memory cache
+    float* zbuf;          // [n_units][z_unit_stride][8 G]  logits of blocks that do not fit a warp's shared-memory cache
+    size_t z_unit_stride; // positions per unit in zbuf
     unsigned long long* stats;  // [8]       counters of mkv_attention_stats
     PlanRec* plan;        // [n_units][plan_stride] of this layer (may be nullptr)
     int32_t plan_stride;
     uint32_t plan_tag;
-    int32_t slots;
 };
-int attention_partial_slots(int sm_count);
+size_t attention_z_unit_stride(const CacheGeom& g);
 size_t attention_zbuf_floats(const CacheGeom& g);
-size_t attention_ticket_ints(const CacheGeom& g);
+cudaError_t attention_prepare(const CacheGeom& g, int sm_count, int* cluster_cache);
+// cluster_cache: two ints owned by the cache (cluster size chosen for the attention / the gather-only kernel; 0 = not yet)
 cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint16_t* q,
                              const int32_t* sel, const int32_t* sel_count, int k_max, float scale,
                              float* out, float* lse, const AttnScratch& scr, const uint16_t* upd_k,
-                             const uint16_t* upd_v, const int32_t* upd_count, int sm_count, cudaStream_t s,
-                             int* n_kernels, bool gather_only = false);
+                             const uint16_t* upd_v, const int32_t* upd_count, int sm_count, int* cluster_cache,
+                             cudaStream_t s, int* n_kernels, bool gather_only = false);
 cudaError_t launch_stream_read(const uint8_t* base, unsigned long long bytes, int sm_count, unsigned long long* sink,
                                cudaStream_t s);
 // KV update buffer: copy n_new raw tokens of every unit into rows [n_have, n_have + n_new)
