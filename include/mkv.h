@@ -28,9 +28,9 @@
  *     calls on one cache must be ordered on one stream (or by events).
  *   - A *unit* is one (layer, request b, KV head h); units never interact.  Query head hq uses
  *     KV head hq / (n_q_heads / n_kv_heads).
- *   - Supported on the GPU today: head_dim = 128, token block B = 8, element group g = 1,
- *     segment_len a multiple of 8 in [8, 4096], group G = n_q_heads/n_kv_heads <= 8.  Anything
- *     else is MKV_E_UNSUPPORTED (host-visible) or MKV_DEV_BAD_STRATEGY (device-visible).
+ *   - Supported on the GPU today: head_dim = 128, token block B = 8, element groups g = 1, 2, 4 (kept elements a
+ *     multiple of g), segment_len a multiple of 8 in [8, 4096], group G = n_q_heads/n_kv_heads <= 8.  Anything
+ *     else is MKV_E_UNSUPPORTED / MKV_E_ARG (host-visible) or MKV_DEV_BAD_STRATEGY (device-visible).
  *   - Inputs must be finite; behaviour on NaN/Inf is unspecified.
  *
  * Canonical packed format (what mkv_cache_export returns; byte-identical to the CPU oracle):

@@ -52,6 +52,53 @@ __device__ __forceinline__ void topr_mask(const uint32_t (&mag)[4], int r, uint3
     }
 }
 
+// Element groups ("selects groups of adjacent elements together ... one bit per element group"): the
+// r / g groups of g adjacent channels with the largest energy sum_i x_i^2, evaluated in fp32 from left to right
+// (R4; the squares of bf16 values are exact in fp32), ties -> lower group.  x[j]: bf16 bits of channel
+// lane + 32 j, so a group lives in g adjacent lanes of one j.  Returns the mask EXPANDED to one bit per channel
+// (w[j] = channels 32 j .. 32 j + 31): the device keeps 128-bit bitmaps for every g, export packs them (mkv_api.cu).
+__device__ __forceinline__ void topr_mask_groups(const uint32_t (&x)[4], int r, int g, uint32_t (&w)[4], int lane) {
+    uint32_t key[4];  // energy of this lane's group, as an order-preserving integer (non-negative floats)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float f = bf16_bits_to_f32(x[j]);
+        const float sq = __fmul_rn(f, f);
+        const int l0 = lane & ~(g - 1);
+        float e = __shfl_sync(kFull, sq, l0);
+        e = __fadd_rn(e, __shfl_sync(kFull, sq, l0 + 1));
+        if (g == 4) {
+            e = __fadd_rn(e, __shfl_sync(kFull, sq, l0 + 2));
+            e = __fadd_rn(e, __shfl_sync(kFull, sq, l0 + 3));
+        }
+        key[j] = __float_as_uint(e);
+    }
+    const bool leader = (lane & (g - 1)) == 0;
+    const int nk = r / g;
+    uint32_t T = 0;
+#pragma unroll 1
+    for (int bit = 30; bit >= 0; --bit) {
+        const uint32_t cand = T | (1u << bit);
+        int c = 0;
+        if (leader) c = (key[0] >= cand) + (key[1] >= cand) + (key[2] >= cand) + (key[3] >= cand);
+        if (__reduce_add_sync(kFull, c) >= nk) T = cand;
+    }
+    int ngt = 0;
+    if (leader) ngt = (key[0] > T) + (key[1] > T) + (key[2] > T) + (key[3] > T);
+    ngt = __reduce_add_sync(kFull, ngt);
+    const int need = nk - ngt;  // >= 1 groups equal to T are kept, lowest groups first
+    const unsigned lt = lanemask_lt();
+    int seen = 0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const bool eq = leader && key[j] == T;
+        const unsigned e = __ballot_sync(kFull, eq);
+        const bool keep = leader && ((key[j] > T) || (eq && (seen + __popc(e & lt) < need)));
+        seen += __popc(e);
+        const unsigned kl = __ballot_sync(kFull, keep);            // one bit per leader
+        w[j] = kl | (kl << 1) | (g == 4 ? (kl << 2) | (kl << 3) : 0u);  // every channel of a kept group
+    }
+}
+
 // Write one packed vector: vector t of a group of n <= 8 vectors (the K or the V vectors of a token
 // block, or 8 block keys of a segment).  Physical layout of a group:
 // the n position bitmaps, then the kept values RANK-MAJOR: the value of rank rho (ascending
@@ -59,7 +106,7 @@ __device__ __forceinline__ void topr_mask(const uint32_t (&mag)[4], int r, uint3
 // through disjoint shared-memory banks in the decode kernels' walk.  Dense vectors (r = D) carry
 // no bitmap and stay vector-major.  x[j]: bf16 bits of channel lane + 32 j.
 // bm: this vector's bitmap; val: the GROUP's value area (2-byte aligned).
-__device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, uint8_t* bm, uint8_t* val, int t, int n,
+__device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, int g, uint8_t* bm, uint8_t* val, int t, int n,
                                             int lane) {
     uint16_t* v16 = reinterpret_cast<uint16_t*>(val);
     if (r == kD) {
@@ -70,7 +117,8 @@ __device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, uint8
     uint32_t mag[4], w[4];
 #pragma unroll
     for (int j = 0; j < 4; ++j) mag[j] = x[j] & 0x7FFFu;
-    topr_mask(mag, r, w);
+    if (g == 1) topr_mask(mag, r, w);
+    else topr_mask_groups(x, r, g, w, lane);
     const unsigned lt = lanemask_lt();
     int base = 0;
 #pragma unroll
@@ -86,7 +134,8 @@ __device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, uint8
 }
 
 __device__ __forceinline__ bool strat_supported(const mkv_strategy& s) {
-    return s.g == 1 && s.B == kB && s.r_k >= 1 && s.r_k <= kD && s.r_v >= 1 && s.r_v <= kD;
+    return (s.g == 1 || s.g == 2 || s.g == 4) && s.B == kB && s.r_k >= s.g && s.r_k <= kD && s.r_v >= s.g && s.r_v <= kD &&
+           s.r_k % s.g == 0 && s.r_v % s.g == 0;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -241,13 +290,13 @@ __global__ void __launch_bounds__(256) mkv_compress_kernel(CacheGeom g, LayerVie
         for (int j = 0; j < 4; ++j) x[j] = __ldg(ksrc + (size_t)t * a.stride_t + lane + 32 * j);
 #pragma unroll
         for (int j = 0; j < 4; ++j) sum[j] = __fadd_rn(sum[j], bf16_bits_to_f32(x[j]));
-        pack_vector(x, r_k, k_bm + t * bmk, k_val, t, nb, lane);
+        pack_vector(x, r_k, rec.g, k_bm + t * bmk, k_val, t, nb, lane);
     }
     for (int t = 0; t < nb; ++t) {
         uint32_t x[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) x[j] = __ldg(vsrc + (size_t)t * a.stride_t + lane + 32 * j);
-        pack_vector(x, r_v, v_bm + t * bmv, v_val, t, nb, lane);
+        pack_vector(x, r_v, rec.g, v_bm + t * bmv, v_val, t, nb, lane);
     }
     // zero the pad of a ragged token block
     {
@@ -263,7 +312,7 @@ __global__ void __launch_bounds__(256) mkv_compress_kernel(CacheGeom g, LayerVie
         for (int j = 0; j < 4; ++j) x[j] = f32_to_bf16_bits_rne(__fdiv_rn(sum[j], fnb));
         // the block keys of a segment form groups of 8 (one work item of the score kernel each)
         const int grp = blk >> 3, gn = min(8, nblk - 8 * grp);
-        pack_vector(x, r_k, bk_base + blk * bmk, bk_base + nblk * bmk + (size_t)grp * 8 * r_k * 2, blk & 7, gn, lane);
+        pack_vector(x, r_k, rec.g, bk_base + blk * bmk, bk_base + nblk * bmk + (size_t)grp * 8 * r_k * 2, blk & 7, gn, lane);
         if (blk == nblk - 1) {
             const uint32_t used = (uint32_t)nblk * vec_bytes(r_k);
             const uint32_t padded = pad16u(used);
@@ -276,7 +325,7 @@ __global__ void __launch_bounds__(256) mkv_compress_kernel(CacheGeom g, LayerVie
 // loss: CTA = one segment of one unit; warps stride over its tokens.  fp64 sums of the exact
 // fp32 squares of the dropped / all elements (R9).
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) mkv_segment_loss_kernel(CacheGeom g, CompressArgs a, int r_k, int r_v,
+__global__ void __launch_bounds__(256) mkv_segment_loss_kernel(CacheGeom g, CompressArgs a, int r_k, int r_v, int grp,
                                                                double* __restrict__ loss_k,
                                                                double* __restrict__ loss_v) {
     const int uc = blockIdx.y, seg_local = blockIdx.x;
@@ -296,8 +345,9 @@ __global__ void __launch_bounds__(256) mkv_segment_loss_kernel(CacheGeom g, Comp
                 x[j] = __ldg(src + (size_t)t * a.stride_t + lane + 32 * j);
                 mag[j] = x[j] & 0x7FFFu;
             }
-            if (r < kD) topr_mask(mag, r, w);
-            else w[0] = w[1] = w[2] = w[3] = kFull;
+            if (r == kD) w[0] = w[1] = w[2] = w[3] = kFull;
+            else if (grp == 1) topr_mask(mag, r, w);
+            else topr_mask_groups(x, r, grp, w, lane);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const float f = bf16_bits_to_f32(x[j]);
@@ -414,7 +464,7 @@ cudaError_t launch_update_copy(const CacheGeom& g, const CompressArgs& a, uint16
 cudaError_t launch_segment_loss(const CacheGeom& g, const CompressArgs& a, mkv_strategy cand, double* loss_k,
                                 double* loss_v, cudaStream_t s) {
     dim3 grid(a.nseg, a.nb * g.n_kv_heads);
-    mkv_segment_loss_kernel<<<grid, 256, 0, s>>>(g, a, cand.r_k, cand.r_v, loss_k, loss_v);
+    mkv_segment_loss_kernel<<<grid, 256, 0, s>>>(g, a, cand.r_k, cand.r_v, cand.g, loss_k, loss_v);
     return cudaGetLastError();
 }
 

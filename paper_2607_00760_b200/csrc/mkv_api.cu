@@ -253,7 +253,8 @@ int mkv_segment_loss(const mkv_cache* c, const void* k, const void* v, int64_t s
     if (rc) return rc;
     if (!loss_k || !loss_v) return fail(MKV_E_ARG, "mkv_segment_loss: NULL output");
     if (cand.r_k < 1 || cand.r_k > kD || cand.r_v < 1 || cand.r_v > kD) return fail(MKV_E_ARG, "candidate r out of range");
-    if (cand.g != 1) return fail(MKV_E_UNSUPPORTED, "element group %d: only g = 1 is built", cand.g);
+    if (cand.g != 1 && cand.g != 2 && cand.g != 4) return fail(MKV_E_ARG, "element group %d: must be 1, 2 or 4", cand.g);
+    if (cand.r_k % cand.g || cand.r_v % cand.g) return fail(MKV_E_ARG, "kept elements must be multiples of the element group");
     CompressArgs a{(const uint16_t*)k, (const uint16_t*)v, sb, sh, st, b0, nb, seg0, nseg, n_tok};
     MKV_CUDA(cudaSetDevice(c->desc.device));
     MKV_CUDA(launch_segment_loss(c->geom, a, cand, loss_k, loss_v, (cudaStream_t)stream));
@@ -522,10 +523,21 @@ int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, vo
         MKV_CUDA(cudaMemcpy(toff.data(), lv.tok_off + (size_t)unit * lv.S_max, (size_t)S * 4, cudaMemcpyDeviceToHost));
         MKV_CUDA(cudaMemcpy(koff.data(), lv.bk_off + (size_t)unit * lv.S_max, (size_t)S * 4, cudaMemcpyDeviceToHost));
     }
-    uint64_t tok_bytes = 0, bk_bytes = 0;
+    // canonical sizes (DESIGN.md format): the bitmap of a packed vector has D / g bits; the device keeps 128 bits for
+    // every g (the decode kernels read one layout), so sizes and offsets are recomputed here
+    auto vbc = [](int r, int gg) -> uint32_t { return 2u * (uint32_t)r + (r == kD ? 0u : (uint32_t)(kD / (8 * gg))); };
+    auto tokc = [&](const StratRec& r, int nb) -> uint32_t { return pad16u((uint32_t)nb * (vbc(r.r_k, r.g) + vbc(r.r_v, r.g))); };
+    auto segtokc = [&](const StratRec& r) -> uint64_t {
+        const int full = r.n_tok / kB, rem = r.n_tok % kB;
+        return (uint64_t)full * tokc(r, kB) + (rem ? tokc(r, rem) : 0u);
+    };
+    auto segbkc = [&](const StratRec& r) -> uint64_t { return pad16u((uint32_t)((r.n_tok + kB - 1) / kB) * vbc(r.r_k, r.g)); };
+    uint64_t tok_bytes = 0, bk_bytes = 0, ptok_bytes = 0, pbk_bytes = 0;
     for (int s = 0; s < S; ++s) {
-        tok_bytes += seg_tok_bytes(rec[s].r_k, rec[s].r_v, rec[s].n_tok);
-        bk_bytes += seg_bk_bytes(rec[s].r_k, rec[s].n_tok);
+        tok_bytes += segtokc(rec[s]);
+        bk_bytes += segbkc(rec[s]);
+        ptok_bytes += seg_tok_bytes(rec[s].r_k, rec[s].r_v, rec[s].n_tok);
+        pbk_bytes += seg_bk_bytes(rec[s].r_k, rec[s].n_tok);
     }
     const uint64_t tables = align_up(48 + (uint64_t)S * 16, 16);
     const uint64_t need = tables + tok_bytes + bk_bytes;
@@ -534,7 +546,7 @@ int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, vo
     if (cap < need) return fail(MKV_E_ARG, "mkv_cache_export: need %llu bytes, cap %llu", (unsigned long long)need,
                                 (unsigned long long)cap);
     uint8_t* p = (uint8_t*)buf;
-    memset(p, 0, tables);
+    memset(p, 0, need);
     const uint32_t hdr[6] = {0x31564B4Du, (uint32_t)kD, (uint32_t)N, (uint32_t)g.L, (uint32_t)S, 0u};
     memcpy(p, hdr, 24);
     memcpy(p + 24, &tok_bytes, 8);
@@ -544,54 +556,87 @@ int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, vo
     uint8_t* p_koff = p_toff + (size_t)S * 4;
     uint8_t* tok_arena = p + tables;
     uint8_t* bk_arena = tok_arena + tok_bytes;
-    // canonical offsets are exclusive prefix sums; physical runs that are contiguous are copied at once
-    uint64_t tpos = 0, kpos = 0;
-    int s = 0;
-    while (s < S) {
-        int e = s;
-        uint64_t trun = 0, krun = 0;
-        while (e < S) {
-            const uint64_t tb = seg_tok_bytes(rec[e].r_k, rec[e].r_v, rec[e].n_tok), kb = seg_bk_bytes(rec[e].r_k, rec[e].n_tok);
-            if (e > s && ((uint64_t)toff[e] * 16 != (uint64_t)toff[s] * 16 + trun || (uint64_t)koff[e] * 16 != (uint64_t)koff[s] * 16 + krun))
-                break;
-            const uint32_t ct = (uint32_t)((tpos + trun) / 16), ck = (uint32_t)((kpos + krun) / 16);
-            memcpy(p_strat + (size_t)e * 8, &rec[e], 8);
-            memcpy(p_toff + (size_t)e * 4, &ct, 4);
-            memcpy(p_koff + (size_t)e * 4, &ck, 4);
-            trun += tb;
-            krun += kb;
-            ++e;
+    // the unit's device payloads, segment after segment (physical runs that are contiguous are copied at once)
+    std::vector<uint8_t> ptok(ptok_bytes), pbk(pbk_bytes);
+    {
+        uint64_t tpos = 0, kpos = 0;
+        int s = 0;
+        while (s < S) {
+            int e = s;
+            uint64_t trun = 0, krun = 0;
+            while (e < S) {
+                const uint64_t tb = seg_tok_bytes(rec[e].r_k, rec[e].r_v, rec[e].n_tok), kb = seg_bk_bytes(rec[e].r_k, rec[e].n_tok);
+                if (e > s && ((uint64_t)toff[e] * 16 != (uint64_t)toff[s] * 16 + trun || (uint64_t)koff[e] * 16 != (uint64_t)koff[s] * 16 + krun))
+                    break;
+                trun += tb;
+                krun += kb;
+                ++e;
+            }
+            if (trun) MKV_CUDA(cudaMemcpy(ptok.data() + tpos, lv.slice + (uint64_t)toff[s] * 16, trun, cudaMemcpyDeviceToHost));
+            if (krun) MKV_CUDA(cudaMemcpy(pbk.data() + kpos, lv.slice + (uint64_t)koff[s] * 16, krun, cudaMemcpyDeviceToHost));
+            tpos += trun;
+            kpos += krun;
+            s = e;
         }
-        MKV_CUDA(cudaMemcpy(tok_arena + tpos, lv.slice + (uint64_t)toff[s] * 16, trun, cudaMemcpyDeviceToHost));
-        MKV_CUDA(cudaMemcpy(bk_arena + kpos, lv.slice + (uint64_t)koff[s] * 16, krun, cudaMemcpyDeviceToHost));
-        tpos += trun;
-        kpos += krun;
-        s = e;
     }
-    // The physical value order inside a group of <= 8 vectors is rank-major (compress.cu); the
-    // canonical blob is vector-major: transpose every group of packed (r < D) vectors.
-    auto to_canonical = [](uint8_t* vals, int r, int n) {
-        if (r == kD || n <= 1) return;
-        uint16_t tmp[8 * kD];
-        uint16_t* v = reinterpret_cast<uint16_t*>(vals);
-        for (int rho = 0; rho < r; ++rho)
-            for (int t = 0; t < n; ++t) tmp[t * r + rho] = v[rho * n + t];
-        memcpy(vals, tmp, (size_t)n * r * 2);
+    // One group of n <= 8 packed vectors, device -> canonical.  Device: n bitmaps of 128 bits (one bit per channel,
+    // every channel of a kept element group set), then the kept values RANK-major (compress.cu).  Canonical: n bitmaps
+    // of D / g bits (one per element group), then the values vector-major.  Dense vectors (r = D): values only.
+    auto repack = [](const uint8_t* src, uint8_t* dst, int r, int gg, int n) {
+        if (r == kD) { memcpy(dst, src, (size_t)n * kD * 2); return; }
+        const int bmc = kD / (8 * gg);
+        for (int t = 0; t < n; ++t)
+            for (int m = 0; m < kD / gg; ++m) {
+                const int c = m * gg;
+                if ((src[t * kBitmapBytes + (c >> 3)] >> (c & 7)) & 1) dst[t * bmc + (m >> 3)] |= (uint8_t)(1u << (m & 7));
+            }
+        const uint16_t* v = reinterpret_cast<const uint16_t*>(src + (size_t)n * kBitmapBytes);  // (2-byte aligned: sizes are even)
+        uint8_t* o = dst + (size_t)n * bmc;
+        for (int t = 0; t < n; ++t)
+            for (int rho = 0; rho < r; ++rho) {
+                uint16_t x;
+                memcpy(&x, reinterpret_cast<const uint8_t*>(v) + 2 * ((size_t)rho * n + t), 2);
+                memcpy(o + 2 * ((size_t)t * r + rho), &x, 2);
+            }
     };
-    uint8_t* tp = tok_arena;
-    uint8_t* kp = bk_arena;
+    uint64_t tpos = 0, kpos = 0;            // canonical positions
+    const uint8_t* tp = ptok.data();
+    const uint8_t* kp = pbk.data();
     for (int sg = 0; sg < S; ++sg) {
-        const int r_k = rec[sg].r_k, r_v = rec[sg].r_v, n_tok = rec[sg].n_tok, nblk = (n_tok + kB - 1) / kB;
-        const uint32_t bmk = r_k == kD ? 0u : (uint32_t)kBitmapBytes, bmv = r_v == kD ? 0u : (uint32_t)kBitmapBytes;
+        const StratRec& r = rec[sg];
+        const int r_k = r.r_k, r_v = r.r_v, gg = r.g ? r.g : 1, n_tok = r.n_tok, nblk = (n_tok + kB - 1) / kB;
+        const uint32_t ct = (uint32_t)(tpos / 16), ck = (uint32_t)(kpos / 16);
+        memcpy(p_strat + (size_t)sg * 8, &r, 8);
+        memcpy(p_toff + (size_t)sg * 4, &ct, 4);
+        memcpy(p_koff + (size_t)sg * 4, &ck, 4);
+        const uint32_t bmk = r_k == kD ? 0u : (uint32_t)kBitmapBytes;
         for (int blk = 0; blk < nblk; ++blk) {
             const int nb = std::min(kB, n_tok - blk * kB);
-            to_canonical(tp + nb * bmk, r_k, nb);
-            to_canonical(tp + nb * (bmk + 2 * r_k) + nb * bmv, r_v, nb);
+            uint8_t* d = tok_arena + tpos;
+            repack(tp, d, r_k, gg, nb);                                                                 // K vectors
+            repack(tp + (size_t)nb * (bmk + 2 * r_k), d + (size_t)nb * vbc(r_k, gg), r_v, gg, nb);      // V vectors
             tp += tokblock_bytes(r_k, r_v, nb);
+            tpos += tokc(r, nb);
         }
-        for (int grp = 0; grp * 8 < nblk; ++grp)
-            to_canonical(kp + nblk * bmk + (size_t)grp * 8 * r_k * 2, r_k, std::min(8, nblk - 8 * grp));
-        kp += seg_bk_bytes(r_k, n_tok);
+        // block keys of the segment: device [bitmaps nblk x 16][values, groups of 8 keys rank-major]; canonical
+        // [bitmaps nblk x D/(8g)][values nblk x r_k vector-major]
+        {
+            uint8_t* d = bk_arena + kpos;
+            const int bmc = r_k == kD ? 0 : kD / (8 * gg);
+            for (int grp = 0; grp * 8 < nblk; ++grp) {
+                const int n = std::min(8, nblk - 8 * grp);
+                if (r_k == kD) { memcpy(d + (size_t)grp * 8 * kD * 2, kp + (size_t)grp * 8 * kD * 2, (size_t)n * kD * 2); continue; }
+                // gather the group's bitmaps and values into one contiguous device-format group, then repack
+                std::vector<uint8_t> tmp((size_t)n * kBitmapBytes + (size_t)n * r_k * 2), outg((size_t)n * bmc + (size_t)n * r_k * 2);
+                memcpy(tmp.data(), kp + (size_t)grp * 8 * kBitmapBytes, (size_t)n * kBitmapBytes);
+                memcpy(tmp.data() + (size_t)n * kBitmapBytes, kp + (size_t)nblk * kBitmapBytes + (size_t)grp * 8 * r_k * 2, (size_t)n * r_k * 2);
+                repack(tmp.data(), outg.data(), r_k, gg, n);
+                memcpy(d + (size_t)grp * 8 * bmc, outg.data(), (size_t)n * bmc);
+                memcpy(d + (size_t)nblk * bmc + (size_t)grp * 8 * r_k * 2, outg.data() + (size_t)n * bmc, (size_t)n * r_k * 2);
+            }
+            kp += seg_bk_bytes(r_k, n_tok);
+            kpos += segbkc(r);
+        }
     }
     return MKV_OK;
 }

@@ -41,11 +41,11 @@ class Case:
         self.cache.free()
 
     # ---- step 1
-    def gpu_loss(self, r_k, r_v):
+    def gpu_loss(self, r_k, r_v, g=1):
         torch = self.torch
         lk = torch.zeros((self.Bt, self.Hkv, self.S), dtype=torch.float64, device=self.dev)
         lv = torch.zeros_like(lk)
-        self.cache.segment_loss(self.k_d, self.v_d, (r_k, r_v, 1, 8), lk, lv)
+        self.cache.segment_loss(self.k_d, self.v_d, (r_k, r_v, g, 8), lk, lv)
         torch.cuda.synchronize()
         return lk.cpu().numpy(), lv.cpu().numpy()
 

@@ -709,11 +709,14 @@ def test_errors_are_reported_not_thrown(env):
     try:
         lk = torch.zeros((1, 2, 4), dtype=torch.float64, device=dev)
         with pytest.raises(mkv.MkvError) as e:
-            c.cache.segment_loss(c.k_d, c.v_d, (32, 32, 2, 8), lk, lk.clone())
-        assert e.value.code == mkv.MKV_E_UNSUPPORTED
+            c.cache.segment_loss(c.k_d, c.v_d, (32, 32, 3, 8), lk, lk.clone())   # element group 3 does not exist
+        assert e.value.code == mkv.MKV_E_ARG
+        with pytest.raises(mkv.MkvError) as e:
+            c.cache.segment_loss(c.k_d, c.v_d, (38, 38, 4, 8), lk, lk.clone())   # 38 is not a multiple of 4
+        assert e.value.code == mkv.MKV_E_ARG
         # an invalid strategy record in device memory sets the sticky device flag; nothing is written
         bad = uniform_strat(1, 2, 4, 38)
-        bad[0, 1, 2] = (38, 38, 4, 8)
+        bad[0, 1, 2] = (38, 38, 4, 8)   # r not a multiple of g
         c.cache.compress_segment(0, c.k_d, c.v_d, torch.from_numpy(bad).to(dev))
         torch.cuda.synchronize()
         assert c.cache.status(raise_on_flag=False) & mkv.MKV_DEV_BAD_STRATEGY
@@ -731,6 +734,92 @@ def test_errors_are_reported_not_thrown(env):
         c2.free()
     finally:
         small.free()
+
+
+@pytest.mark.parametrize("g,r_k,r_v", [(2, 38, 38), (4, 32, 48), (2, 64, 2), (4, 124, 4), (2, 128, 38), (4, 36, 128)])
+def test_element_groups_end_to_end(env, g, r_k, r_v):
+    """element groups of 2 and 4 channels on the GPU.  Loss, packed blob (bit-exact,
+    one bit per element group in the canonical bitmap), selection and attention against the oracle; ties between equal
+    group energies (coarse integer data) go to the lower group."""
+    mkv, dev = env
+    c = Case(mkv, dev, 2, 2, 8, 64 * 9 + 13, seed=120 + g)
+    try:
+        rng = np.random.default_rng(g)
+        from paper_2607_00760_b200 import synth
+        # a stretch of coarse values: exact ties between group energies, zeros, -0
+        c.K[0, 0, 64:128] = synth.f32_to_bf16_bits(rng.integers(-2, 3, (64, 128)).astype(np.float32))
+        c.V[1, 1, 0:64] = synth.f32_to_bf16_bits(rng.integers(-1, 2, (64, 128)).astype(np.float32))
+        c.k_d, c.v_d = to_dev(c.K, dev), to_dev(c.V, dev)
+        lk, lv = c.gpu_loss(r_k, r_v, g)
+        for b in range(2):
+            for h in range(2):
+                rk_, rv_ = orc.segment_loss(c.K[b, h], c.V[b, h], 64, r_k, r_v, g)
+                np.testing.assert_allclose(lk[b, h], rk_, rtol=1e-12, atol=0)
+                np.testing.assert_allclose(lv[b, h], rv_, rtol=1e-12, atol=0)
+        strat = uniform_strat(2, 2, c.S, r_k, r_v, g=g)
+        strat[:, :, 3::4, 0:2] = 128            # dense segments in between (their g is kept in the record)
+        strat[:, :, 2::4] = (38, 38, 1, 8)      # and g = 1 segments: strategies differ per segment (PAPER.md:188)
+        c.compress(strat)
+        c.assert_export_equal()
+        total, swaps = c.check_select(200)
+        assert swaps * 10000 <= total
+        for budget in (8, 200, c.N):
+            sel, cnt = c.oracle_sel(budget)
+            c.check_attention(sel, cnt)
+    finally:
+        c.free()
+
+
+def test_threshold_rule_over_the_papers_grid(env):
+    """"evaluates the compression loss for each candidate compression rate (e.g., 87.5%, 75%, and 62.5%) and
+    element group size (e.g., 1, 2, and 4) ... The highest compression rate and largest group size whose loss remains
+    below a threshold are selected."  Nine candidates, most aggressive first; GPU losses and the chosen table equal the
+    oracle's, and the cache compressed with the mixed table is bit-exact and attends correctly."""
+    mkv, dev = env
+    import torch
+    c = Case(mkv, dev, 1, 2, 8, 64 * 24, seed=131)
+    try:
+        cands = [(r, r, g, 8) for r in (16, 32, 48) for g in (4, 2, 1)]
+        # segments whose vectors have equal magnitudes everywhere lose 1 - r / D whatever is kept (PAPER.md:134: "regions
+        # with relatively uniform magnitudes ... require a lower rate"): V only -> a milder rate; K and V -> dense
+        from paper_2607_00760_b200 import synth
+        rng = np.random.default_rng(7)
+        flat = lambda n: synth.f32_to_bf16_bits(rng.choice([-1.0, 1.0], (n, 128)).astype(np.float32))
+        c.V[0, 0, 5 * 64:8 * 64] = flat(3 * 64)
+        c.K[0, 1, 9 * 64:11 * 64] = flat(2 * 64)
+        c.V[0, 1, 9 * 64:11 * 64] = flat(2 * 64)
+        c.k_d, c.v_d = to_dev(c.K, dev), to_dev(c.V, dev)
+        lk_all = torch.zeros((len(cands), c.Bt, c.Hkv, c.S), dtype=torch.float64, device=dev)
+        lv_all = torch.zeros_like(lk_all)
+        ref_lk = np.zeros((len(cands), c.Bt, c.Hkv, c.S))
+        ref_lv = np.zeros_like(ref_lk)
+        for i, cd in enumerate(cands):
+            c.cache.segment_loss(c.k_d, c.v_d, cd, lk_all[i], lv_all[i])
+            for h in range(c.Hkv):
+                ref_lk[i, 0, h], ref_lv[i, 0, h] = orc.segment_loss(c.K[0, h], c.V[0, h], 64, cd[0], cd[1], cd[2])
+        torch.cuda.synchronize()
+        np.testing.assert_allclose(lk_all.cpu().numpy(), ref_lk, rtol=1e-12, atol=0)
+        np.testing.assert_allclose(lv_all.cpu().numpy(), ref_lv, rtol=1e-12, atol=0)
+        I = 0.5 * (ref_lk + ref_lv)
+        tau = 0.4  # inside the spread of the most aggressive candidates: a real mix of rates, group sizes and dense segments
+        assert not np.any(np.abs(I - tau) < 1e-9 * tau), "a loss sits on the decision boundary"
+        out = torch.zeros((c.Bt, c.Hkv, c.S, 4), dtype=torch.uint8, device=dev)
+        c.cache.strategy_threshold(lk_all, lv_all, c.S, cands, tau, out)
+        torch.cuda.synchronize()
+        strat = out.cpu().numpy()
+        for h in range(c.Hkv):
+            want = orc.strategy_threshold(ref_lk[:, 0, h], ref_lv[:, 0, h], np.array(cands, np.uint8), tau, 128)
+            np.testing.assert_array_equal(strat[0, h], want)
+        kinds = {tuple(x) for x in strat.reshape(-1, 4)}
+        assert {k[2] for k in kinds if k[0] < 128} == {1, 2, 4} and len({k[0] for k in kinds}) >= 3 and any(k[0] == 128 for k in kinds), kinds
+        c.compress(strat)
+        c.assert_export_equal()
+        total, swaps = c.check_select(512)
+        assert swaps * 10000 <= total
+        sel, cnt = c.oracle_sel(512)
+        c.check_attention(sel, cnt)
+    finally:
+        c.free()
 
 
 def test_rotation_fold(env):
