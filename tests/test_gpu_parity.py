@@ -894,6 +894,46 @@ def test_rotation_fold(env):
         c.free()
 
 
+def test_guard_bands_around_every_output(env):
+    """compute-sanitizer is closed on this GPU pool (profiles/r2/sanitizer.md), so out-of-bounds WRITES are looked for
+    with guard bands: every buffer the decode calls write (sel, sel_count, scores, out, lse) sits inside a larger
+    tensor filled with a sentinel; after select + attention (with a non-empty update buffer, ragged tail, k_max larger
+    than the selection) the bands must be untouched and everything inside must have been written."""
+    mkv, dev = env
+    import torch
+    c = Case(mkv, dev, 2, 2, 8, 64 * 11 + 21, seed=141)
+    try:
+        strat = uniform_strat(2, 2, c.S, 38)
+        strat[:, :, 1::3, 0:2] = 128
+        c.compress(strat)
+        c.cache.update_append(0, c.k_d[:, :, :13], c.v_d[:, :, :13])
+        budget, k_max, pad = 300, 300 // 8 + 5, 64
+        SENT_I, SENT_F = -123456789, 1.5e30
+
+        def banded(shape, dtype, sentinel):
+            n = int(np.prod(shape))
+            big = torch.full((n + 2 * pad,), sentinel, dtype=dtype, device=dev)
+            return big, big[pad:pad + n].view(*shape)
+
+        sel_b, sel = banded((2, 2, k_max), torch.int32, SENT_I)
+        cnt_b, cnt = banded((2, 2), torch.int32, SENT_I)
+        sc_b, sc = banded((2, 2, c.cache.score_stride), torch.float32, SENT_F)
+        out_b, out = banded((2, 8, 128), torch.float32, SENT_F)
+        lse_b, lse = banded((2, 8), torch.float32, SENT_F)
+        c.cache.select(0, c.q_d, budget, sel, cnt, scores=sc)
+        c.cache.packed_attention(0, c.q_d, sel, cnt, 1 / math.sqrt(128), out, lse)
+        torch.cuda.synchronize()
+        c.cache.status()
+        for big, inner, sent in ((sel_b, sel, SENT_I), (cnt_b, cnt, SENT_I), (sc_b, sc, SENT_F), (out_b, out, SENT_F), (lse_b, lse, SENT_F)):
+            assert bool((big[:pad] == sent).all()) and bool((big[-pad:] == sent).all()), "a guard band was written"
+        assert bool((cnt == budget // 8).all()) and bool((sel[:, :, :budget // 8] >= 0).all()) and bool((sel[:, :, budget // 8:] == -1).all())
+        nblk = (c.N + 7) // 8
+        assert bool((sc[:, :, :nblk] != SENT_F).all()) and bool((out != SENT_F).all()) and bool((lse != SENT_F).all())
+        assert bool(torch.isfinite(out).all()) and bool(torch.isfinite(lse).all())
+    finally:
+        c.free()
+
+
 def test_zz_report_lse_ulps(env):
     """runs last: the largest lse error, in fp32 spacings of |lse| beyond the 1e-3 absolute term, seen by this session"""
     import gpu_util
