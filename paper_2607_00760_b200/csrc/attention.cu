@@ -142,6 +142,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     __shared__ float s_l[kWarps][kMaxGroup];              // the warps' softmax sums
     __shared__ float s_cta_l[kMaxGroup];                  // the CTA's partial sums (its partial O: s_cta_o)
     __shared__ float s_M[kMaxGroup];                      // the unit's per-head maxima after the exchange
+    __shared__ unsigned s_active;                         // warps of the CTA that hold a partial result
     float* s_cta_o = reinterpret_cast<float*>(smem + kWarps * kWS);  // [G][128] floats behind the warps' regions
 
     uint8_t* wbase = smem + warp * kWS;
@@ -158,6 +159,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         mbar_init_fence();
     }
     if (threadIdx.x < kMaxGroup) s_max[threadIdx.x] = 0u;  // below the key of every float
+    if (threadIdx.x == 0) s_active = 0u;
     const int u = (int)blockIdx.x / C;                      // the cluster's unit
     const unsigned rank = cluster_ctarank();
     __syncthreads();
@@ -441,6 +443,13 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         }
     }
     const float Mh = Mraw == -INFINITY ? 0.f : Mraw;  // 0 if the unit holds no valid token
+    // A warp whose own maxima all lie more than kSkip below the unit's takes no further part: each of its tokens has a
+    // probability < 2^-40, which neither the sums nor the output can see (error bound).
+    bool active = kGatherOnly;
+    if (!kGatherOnly) {
+        const float MA = __shfl_sync(kFull, Mraw, 8 * qq), MB = __shfl_sync(kFull, Mraw, 8 * qq + 4);  // heads 2qq, 2qq+1
+        active = __any_sync(kFull, (2 * qq < G && mxA - MA >= -kSkip) || (2 * qq + 1 < G && mxB - MB >= -kSkip));
+    }
 
     // =====================================================================================
     // Phase 2: softmax sums over every selected token, PV over the blocks that matter.
@@ -457,7 +466,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         return __ldcg(reinterpret_cast<const float2*>(zglob + (size_t)i * (size_t)(8 * G) + (zr >> 2)));
     };
 
-    if (n_total > 0) {
+    if (n_total > 0 && active) {
         // the range's descriptors are still in shared memory unless it was longer than one ring: then describe again
         const bool redo = gbuilt > kDesc;
         if (redo) { bbuilt = 0; gbuilt = 0; }
@@ -612,8 +621,9 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     // split-K rule of oracle pin P10 with equal references), always in the same order: warps inside the CTA, then
     // the cluster's CTAs.
     // =====================================================================================
-    {
+    if (n_total > 0 && active) {
         // the warp's partial: O^T fragments -> [head][channel] floats in the warp's (now idle) ring; sums -> s_l
+        if (lane == 0) atomicOr(&s_active, 1u << warp);
         lsum += __shfl_xor_sync(kFull, lsum, 1);
         lsum += __shfl_xor_sync(kFull, lsum, 2);  // lanes (gq, *): the warp's sum of head gq
         if (qq == 0 && gq < G) s_l[warp][gq] = lsum;
@@ -628,16 +638,20 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     }
     __syncthreads();
     const int GD = G * kD;
+    const unsigned wmask = s_active;  // (in warp order: the sums are reproducible)
     for (int e = threadIdx.x; e < GD; e += kNT) {  // the CTA's partial
         float o = 0.f;
 #pragma unroll
-        for (int w = 0; w < kWarps; ++w) o += *reinterpret_cast<const float*>(smem + w * kWS + 4 * e);
+        for (int w = 0; w < kWarps; ++w) {
+            const float v = *reinterpret_cast<const float*>(smem + w * kWS + 4 * e);  // (stale bits where the warp left no partial)
+            if ((wmask >> w) & 1u) o += v;
+        }
         s_cta_o[e] = o;
     }
     if (threadIdx.x < G) {
         float l = 0.f;
-#pragma unroll
-        for (int w = 0; w < kWarps; ++w) l += s_l[w][threadIdx.x];
+#pragma unroll 1
+        for (unsigned m = wmask; m; m &= m - 1u) l += s_l[__ffs(m) - 1][threadIdx.x];
         s_cta_l[threadIdx.x] = l;
     }
     cluster_sync();  // every CTA's partial is complete and visible to the cluster
