@@ -28,8 +28,8 @@
  *     calls on one cache must be ordered on one stream (or by events).
  *   - A *unit* is one (layer, request b, KV head h); units never interact.  Query head hq uses
  *     KV head hq / (n_q_heads / n_kv_heads).
- *   - Supported on the GPU today: head_dim = 128, token block B = 8, element groups g = 1, 2, 4 (kept elements a
- *     multiple of g), segment_len a multiple of 8 in [8, 4096], group G = n_q_heads/n_kv_heads <= 8.  Anything
+ *   - Supported on the GPU today: head_dim = 128, token blocks B = 4, 8, 16 (one B per cache, mkv_cache_desc.token_block),
+ *     element groups g = 1, 2, 4 (kept elements a multiple of g), segment_len a multiple of 8 and of B in [8, 4096], group G = n_q_heads/n_kv_heads <= 8.  Anything
  *     else is MKV_E_UNSUPPORTED / MKV_E_ARG (host-visible) or MKV_DEV_BAD_STRATEGY (device-visible).
  *   - Inputs must be finite; behaviour on NaN/Inf is unspecified.
  *
@@ -85,6 +85,9 @@ typedef struct {
     int32_t device;       /* CUDA device ordinal */
     uint64_t arena_bytes; /* packed payload bytes for ALL layers (split evenly per layer);
                              0 = size for the dense worst case */
+    int32_t token_block;  /* B: tokens per token block = unit of selection, one block key each (4, 8 or 16;
+                             0 = 8).  Every strategy of the cache must carry this B; segment_len must be a multiple of it */
+    int32_t reserved;     /* 0 */
 } mkv_cache_desc;
 
 /* Per-segment compression strategy: kept elements per K / V vector (multiples of
@@ -147,8 +150,8 @@ MKV_API int mkv_compress_segment(mkv_cache* cache, int32_t layer, const void* k,
  * blocks by (score descending, index ascending) while they fit in `token_budget` tokens.
  * q: bf16 [batch][n_q_heads][D].  sel: int32 [batch][n_kv_heads][k_max], first-token index of each
  * chosen block, ascending; unused tail = -1.  sel_count: int32 [batch][n_kv_heads].
- * k_max must be >= min(token_budget / 8 + 1, blocks per unit).  scores_opt: float
- * [batch][n_kv_heads][score_stride] or NULL, score_stride = ceil(max_tokens / 8).
+ * k_max must be >= min(token_budget / B + 1, blocks per unit).  scores_opt: float
+ * [batch][n_kv_heads][score_stride] or NULL, score_stride = ceil(max_tokens / B).
  */
 MKV_API int mkv_select(const mkv_cache* cache, int32_t layer, const void* q, int32_t token_budget,
                int32_t reduce, int32_t* sel, int32_t* sel_count, int32_t k_max, float* scores_opt,
@@ -252,7 +255,7 @@ MKV_API int mkv_last_launch_count(const mkv_cache* cache, int32_t* select_kernel
                           int32_t* attention_kernels_host, int32_t* compress_kernels_host);
 
 MKV_API const char* mkv_last_error(void); /* thread-local, never NULL */
-MKV_API int mkv_version(void);            /* ABI version, currently 1 */
+MKV_API int mkv_version(void);            /* ABI version, currently 2 (mkv_cache_desc gained token_block) */
 
 #ifdef __cplusplus
 }

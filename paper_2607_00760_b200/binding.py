@@ -31,7 +31,8 @@ SYMBOLS = ["mkv_cache_create", "mkv_cache_free", "mkv_cache_reset", "mkv_segment
 class mkv_cache_desc(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("batch", C.c_int32), ("n_kv_heads", C.c_int32),
                 ("n_q_heads", C.c_int32), ("head_dim", C.c_int32), ("max_tokens", C.c_int32),
-                ("segment_len", C.c_int32), ("device", C.c_int32), ("arena_bytes", C.c_uint64)]
+                ("segment_len", C.c_int32), ("device", C.c_int32), ("arena_bytes", C.c_uint64),
+                ("token_block", C.c_int32), ("reserved", C.c_int32)]
 
 
 class mkv_strategy(C.Structure):
@@ -124,9 +125,9 @@ def _kv_strides(k, v):
 # ---- functions named as in include/mkv.h ---------------------------------------------------
 
 def mkv_cache_create(n_layers, batch, n_kv_heads, n_q_heads, head_dim, max_tokens, segment_len,
-                     device=0, arena_bytes=0):
+                     device=0, arena_bytes=0, token_block=0):
     desc = mkv_cache_desc(n_layers, batch, n_kv_heads, n_q_heads, head_dim, max_tokens, segment_len,
-                          device, arena_bytes)
+                          device, arena_bytes, token_block, 0)
     h = _vp()
     _check(_lib.mkv_cache_create(C.byref(desc), C.byref(h)))
     return h
@@ -273,14 +274,15 @@ class Cache:
     """Owns one mkv_cache; methods forward to the functions above (same names minus `mkv_`)."""
 
     def __init__(self, n_layers, batch, n_kv_heads, n_q_heads, head_dim=128, max_tokens=0,
-                 segment_len=64, device=0, arena_bytes=0):
+                 segment_len=64, device=0, arena_bytes=0, token_block=8):
         self.h = mkv_cache_create(n_layers, batch, n_kv_heads, n_q_heads, head_dim, max_tokens,
-                                  segment_len, device, arena_bytes)
+                                  segment_len, device, arena_bytes, token_block)
         _SEGLEN[self.h.value] = segment_len
         self.n_layers, self.batch, self.n_kv_heads, self.n_q_heads = n_layers, batch, n_kv_heads, n_q_heads
         self.head_dim, self.max_tokens, self.segment_len = head_dim, max_tokens, segment_len
         self.n_units = batch * n_kv_heads
-        self.score_stride = (max_tokens + 7) // 8
+        self.token_block = token_block
+        self.score_stride = (max_tokens + token_block - 1) // token_block
 
     def free(self):
         if self.h is not None:

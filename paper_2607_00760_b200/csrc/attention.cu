@@ -168,9 +168,10 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
 
     // tokens in the layer's update buffer: device-resident, so a captured graph stays valid across appends
     const int n_buf = min(max(__ldg(upd_count), 0), g.L);
-    const int upd_blocks = (n_buf + kB - 1) / kB;  // the unit's stream ends with the blocks of its update buffer
-    const int cnt = min(max(__ldg(sel_count + u), 0), k_max);
-    const int T = cnt + upd_blocks;                // blocks of the unit
+    const int upd_blocks = (n_buf + kPhys - 1) / kPhys;  // the unit's stream ends with the blocks of its update buffer
+    const int ppb = g.ppb;                                // device blocks per selected token block (2 at B = 16)
+    const int cnt = min(max(__ldg(sel_count + u), 0), k_max) * ppb;  // device blocks selected
+    const int T = cnt + upd_blocks;                       // device blocks of the unit's stream
     const size_t row = (size_t)(u / g.n_kv_heads) * g.n_q_heads + (size_t)(u % g.n_kv_heads) * G;
     if (T == 0) {  // (uniform over the cluster) empty selection: out = 0, lse = -inf
         if (rank == 0 && !kGatherOnly) {
@@ -202,12 +203,13 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         if (lane < count) {
             const int j = lo + bbuilt + lane, jb = j - cnt;
             if (jb >= 0) {  // block jb of the unit's update buffer: raw rows [u][8 jb ..][128] of upd_k / upd_v
-                const uint32_t nb = (uint32_t)min(kB, n_buf - kB * jb);
-                off16 = (uint32_t)(((size_t)u * g.L + (size_t)kB * jb) * (kD * 2 / 16));
+                const uint32_t nb = (uint32_t)min(kPhys, n_buf - kPhys * jb);
+                off16 = (uint32_t)(((size_t)u * g.L + (size_t)kPhys * jb) * (kD * 2 / 16));
                 meta = (uint32_t)kD | ((uint32_t)kD << 8) | (nb << 16);
                 updf = 1u;
             } else {
-                const int t0 = __ldg(sel + (size_t)u * k_max + j);
+                const int ts = __ldg(sel + (size_t)u * k_max + j / ppb);
+                const int t0 = (ts < 0 || (ts & (g.B - 1))) ? -1 : ts + kPhys * (j % ppb);  // (j odd: second half of 16 tokens)
                 PlanRec pr;
                 pr.t0 = -1; pr.off16 = 0u; pr.meta = 0u; pr.tag = 0u;
                 if (scr.plan != nullptr && j < scr.plan_stride) {
@@ -340,7 +342,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 bposc += two ? 2 : 1;
                 continue;
             }
-            const bool full = nb0 == kB && (!two || nb1 == kB);
+            const bool full = nb0 == kPhys && (!two || nb1 == kPhys);
 
             mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);  // the group's K parts have landed
 
@@ -551,7 +553,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             const uint32_t ph0 = pack_bf16(e00, e01), ph1 = pack_bf16(e10, e11);
             const uint32_t pl0 = pack_bf16(e00 - __uint_as_float(ph0 << 16), e01 - __uint_as_float(ph0 & 0xffff0000u));
             const uint32_t pl1 = pack_bf16(e10 - __uint_as_float(ph1 << 16), e11 - __uint_as_float(ph1 & 0xffff0000u));
-            const bool full = nb0 == kB && (!two || nb1 == kB);
+            const bool full = nb0 == kPhys && (!two || nb1 == kPhys);
 
             mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);  // the group's V parts have landed
 
@@ -704,7 +706,7 @@ mkv_stream_read_kernel(const uint4* __restrict__ base, unsigned long long n16, u
 }  // namespace
 
 // logit scratch: per unit one entry of 8 G floats per position of its block stream (selected + update-buffer blocks)
-size_t attention_z_unit_stride(const CacheGeom& g) { return (size_t)g.score_stride + 1 + (size_t)(g.L + kB - 1) / kB; }
+size_t attention_z_unit_stride(const CacheGeom& g) { return ((size_t)g.score_stride + 1) * g.ppb + (size_t)(g.L + kPhys - 1) / kPhys; }
 size_t attention_zbuf_floats(const CacheGeom& g) { return (size_t)g.n_units * attention_z_unit_stride(g) * 8 * (size_t)g.group; }
 
 // Cluster size for a layer of n_units units: the largest power of two C <= 16 with n_units * C <= SMs whose clusters

@@ -133,8 +133,8 @@ __device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, int g
     }
 }
 
-__device__ __forceinline__ bool strat_supported(const mkv_strategy& s) {
-    return (s.g == 1 || s.g == 2 || s.g == 4) && s.B == kB && s.r_k >= s.g && s.r_k <= kD && s.r_v >= s.g && s.r_v <= kD &&
+__device__ __forceinline__ bool strat_supported(const mkv_strategy& s, int B) {
+    return (s.g == 1 || s.g == 2 || s.g == 4) && s.B == B && s.r_k >= s.g && s.r_k <= kD && s.r_v >= s.g && s.r_v <= kD &&
            s.r_k % s.g == 0 && s.r_v % s.g == 0;
 }
 
@@ -162,9 +162,9 @@ __global__ void __launch_bounds__(256) mkv_plan_kernel(CacheGeom g, LayerView lv
     for (int i = tid; i < a.nseg; i += 256) {
         const mkv_strategy s = st[i];
         const int n_tok = (i == a.nseg - 1) ? a.n_tok - i * g.L : g.L;
-        if (!strat_supported(s)) { bad = 1; continue; }
-        tokb += seg_tok_bytes(s.r_k, s.r_v, n_tok);
-        bkb += seg_bk_bytes(s.r_k, n_tok);
+        if (!strat_supported(s, g.B)) { bad = 1; continue; }
+        tokb += seg_tok_bytes(s.r_k, s.r_v, n_tok, g.pb);
+        bkb += seg_bk_bytes(s.r_k, n_tok, g.B);
     }
 #pragma unroll
     for (int o = 16; o; o >>= 1) {
@@ -215,8 +215,8 @@ __global__ void __launch_bounds__(256) mkv_plan_kernel(CacheGeom g, LayerView lv
         if (i < a.nseg) {
             s = st[i];
             n_tok = (i == a.nseg - 1) ? a.n_tok - i * g.L : g.L;
-            t = seg_tok_bytes(s.r_k, s.r_v, n_tok);
-            k = seg_bk_bytes(s.r_k, n_tok);
+            t = seg_tok_bytes(s.r_k, s.r_v, n_tok, g.pb);
+            k = seg_bk_bytes(s.r_k, n_tok, g.B);
         }
         unsigned long long it = t, ik = k;  // inclusive warp scan
 #pragma unroll
@@ -264,14 +264,15 @@ __global__ void __launch_bounds__(256) mkv_compress_kernel(CacheGeom g, LayerVie
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const size_t e = (size_t)unit * lv.S_max + a.seg0 + seg_local;
     const StratRec rec = lv.strat[e];
-    const int n_tok = rec.n_tok, nblk = (n_tok + kB - 1) / kB;
+    const int pb = g.pb, B = g.B;
+    const int n_tok = rec.n_tok, nblk = (n_tok + pb - 1) / pb;  // device token blocks of the segment
     const int blk = chunk * 8 + warp;
     if (blk >= nblk) return;
-    const int nb = min(kB, n_tok - blk * kB);
+    const int nb = min(pb, n_tok - blk * pb);
     const int r_k = rec.r_k, r_v = rec.r_v;
     const uint32_t bmk = (r_k == kD) ? 0u : kBitmapBytes, bmv = (r_v == kD) ? 0u : kBitmapBytes;
 
-    uint8_t* base = lv.slice + ((size_t)lv.tok_off[e] << 4) + (size_t)blk * tokblock_bytes(r_k, r_v, kB);
+    uint8_t* base = lv.slice + ((size_t)lv.tok_off[e] << 4) + (size_t)blk * tokblock_bytes(r_k, r_v, pb);
     uint8_t* k_bm = base;
     uint8_t* k_val = k_bm + nb * bmk;
     uint8_t* v_bm = k_val + nb * r_k * 2;
@@ -279,7 +280,7 @@ __global__ void __launch_bounds__(256) mkv_compress_kernel(CacheGeom g, LayerVie
     uint8_t* bk_base = lv.slice + ((size_t)lv.bk_off[e] << 4);
 
     const size_t row0 = (size_t)(b - a.b0) * a.stride_b + (size_t)h * a.stride_h +
-                        (size_t)(seg_local * g.L + blk * kB) * a.stride_t;
+                        (size_t)(seg_local * g.L + blk * pb) * a.stride_t;
     const uint16_t* ksrc = a.k + row0;
     const uint16_t* vsrc = a.v + row0;
 
@@ -304,17 +305,30 @@ __global__ void __launch_bounds__(256) mkv_compress_kernel(CacheGeom g, LayerVie
         const uint32_t padded = pad16u(used);
         for (uint32_t o = used + lane; o < padded; o += 32) base[o] = 0;
     }
-    // block key
+    // block key of the token block (B tokens): a block of 16 tokens spans two device blocks; the warp of the first one
+    // goes on through the keys of the second (fp32 sum in token order over the whole block, R5)
+    int nbk = nb;  // tokens averaged
+    if (B > pb) {
+        if (blk & 1) return;
+        const int more = min(pb, n_tok - (blk + 1) * pb);
+        for (int t = 0; t < more; ++t) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                sum[j] = __fadd_rn(sum[j], bf16_bits_to_f32(__ldg(ksrc + (size_t)(pb + t) * a.stride_t + lane + 32 * j)));
+        }
+        nbk += max(more, 0);
+    }
     {
+        const int lb = B > pb ? blk >> 1 : blk, nlb = (n_tok + B - 1) / B;  // this token block, token blocks of the segment
         uint32_t x[4];
-        const float fnb = (float)nb;
+        const float fnb = (float)nbk;
 #pragma unroll
         for (int j = 0; j < 4; ++j) x[j] = f32_to_bf16_bits_rne(__fdiv_rn(sum[j], fnb));
         // the block keys of a segment form groups of 8 (one work item of the score kernel each)
-        const int grp = blk >> 3, gn = min(8, nblk - 8 * grp);
-        pack_vector(x, r_k, rec.g, bk_base + blk * bmk, bk_base + nblk * bmk + (size_t)grp * 8 * r_k * 2, blk & 7, gn, lane);
-        if (blk == nblk - 1) {
-            const uint32_t used = (uint32_t)nblk * vec_bytes(r_k);
+        const int grp = lb >> 3, gn = min(8, nlb - 8 * grp);
+        pack_vector(x, r_k, rec.g, bk_base + lb * bmk, bk_base + nlb * bmk + (size_t)grp * 8 * r_k * 2, lb & 7, gn, lane);
+        if (lb == nlb - 1) {
+            const uint32_t used = (uint32_t)nlb * vec_bytes(r_k);
             const uint32_t padded = pad16u(used);
             for (uint32_t o = used + lane; o < padded; o += 32) bk_base[o] = 0;
         }
@@ -492,7 +506,7 @@ cudaError_t launch_compress(const CacheGeom& g, const LayerView& lv, const Compr
     mkv_plan_kernel<<<units, 256, 0, s>>>(g, lv, a, strat, call_base, dev_flags);
     cudaError_t err = cudaGetLastError();
     if (err != cudaSuccess) return err;
-    const int chunks = (g.blocks_per_seg + 7) / 8;
+    const int chunks = (g.L / g.pb + 7) / 8;  // CTAs of 8 warps per segment: one warp per device token block
     dim3 grid(a.nseg * chunks, units);
     mkv_compress_kernel<<<grid, 256, 0, s>>>(g, lv, a, call_base, chunks);
     if (n_kernels) *n_kernels = 2;

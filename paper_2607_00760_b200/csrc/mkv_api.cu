@@ -78,8 +78,8 @@ struct mkv_cache {
 
     AttnScratch attn_scratch(int layer) const {
         AttnScratch a = attn;
-        a.plan = plan + (size_t)layer * geom.n_units * sel_cap;
-        a.plan_stride = sel_cap;
+        a.plan = plan + (size_t)layer * geom.n_units * sel_cap * geom.ppb;
+        a.plan_stride = sel_cap * geom.ppb;
         a.plan_tag = plan_tag(generation, layer);
         return a;
     }
@@ -104,7 +104,7 @@ struct mkv_cache {
 extern "C" {
 
 const char* mkv_last_error(void) { return g_err; }
-int mkv_version(void) { return 1; }
+int mkv_version(void) { return 2; }
 
 int mkv_cache_free(mkv_cache* c) {
     if (!c) return MKV_OK;
@@ -130,8 +130,10 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         return fail(MKV_E_UNSUPPORTED, "GQA group %d > %d", d->n_q_heads / d->n_kv_heads, kMaxGroup);
     if ((long long)d->batch * d->n_kv_heads > 2048)
         return fail(MKV_E_UNSUPPORTED, "batch * n_kv_heads = %lld units: at most 2048 are built", (long long)d->batch * d->n_kv_heads);
-    if (d->segment_len < kB || d->segment_len % kB || d->segment_len > 4096)
-        return fail(MKV_E_UNSUPPORTED, "segment_len %d: need a multiple of 8 in [8, 4096]", d->segment_len);
+    const int B = d->token_block ? d->token_block : 8;
+    if (B != 4 && B != 8 && B != 16) return fail(MKV_E_ARG, "token_block %d: must be 4, 8 or 16 (0 = 8)", d->token_block);
+    if (d->segment_len < 8 || d->segment_len % 8 || d->segment_len % B || d->segment_len > 4096)
+        return fail(MKV_E_UNSUPPORTED, "segment_len %d: need a multiple of 8 and of the token block in [8, 4096]", d->segment_len);
     int ndev = 0;
     MKV_CUDA(cudaGetDeviceCount(&ndev));
     if (d->device < 0 || d->device >= ndev) return fail(MKV_E_ARG, "device %d of %d", d->device, ndev);
@@ -144,11 +146,14 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     g.n_layers = d->n_layers; g.batch = d->batch; g.n_kv_heads = d->n_kv_heads; g.n_q_heads = d->n_q_heads;
     g.group = d->n_q_heads / d->n_kv_heads; g.max_tokens = d->max_tokens; g.L = d->segment_len;
     g.S_max = (d->max_tokens + g.L - 1) / g.L; g.n_units = d->batch * d->n_kv_heads;
-    g.blocks_per_seg = g.L / kB; g.score_stride = (d->max_tokens + kB - 1) / kB;
+    g.B = B; g.pb = B < kPhys ? B : kPhys; g.ppb = B / g.pb;
+    g.blocks_per_seg = g.L / B; g.score_stride = (d->max_tokens + B - 1) / B;
     MKV_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, d->device));
 
-    // largest payloads: r = 127 on both sides (bitmap + 254 B per vector): 8 * 2 * 270 B per token block, 270 B per block key
-    const uint64_t worst = (uint64_t)g.n_units * ((uint64_t)g.score_stride * (4320 + 272) + 64 + 16ull * g.S_max) + 4096;
+    // largest payloads: r = 127 on both sides (bitmap + 254 B per vector): 2 * 270 B per token (+ 16 B of padding per device
+    // block), 270 B (+ padding) per block key
+    const uint64_t worst = (uint64_t)g.n_units * ((uint64_t)d->max_tokens * 540 + ((uint64_t)d->max_tokens / g.pb + 1) * 16 +
+                                                  (uint64_t)g.score_stride * 272 + 64 + 32ull * g.S_max) + 4096;
     uint64_t per_layer = d->arena_bytes ? d->arena_bytes / (uint64_t)d->n_layers : worst;
     per_layer = per_layer / 256 * 256;
     if (per_layer < 256) { delete c; return fail(MKV_E_ARG, "arena_bytes too small"); }
@@ -180,7 +185,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         {(void**)&c->upd_cnt, (size_t)g.n_layers * 4 + 252},
         {(void**)&c->attn.zbuf, attention_zbuf_floats(g) * 4},
         {(void**)&c->attn.stats, 64},
-        {(void**)&c->plan, tu * (size_t)c->sel_cap * sizeof(PlanRec)},
+        {(void**)&c->plan, tu * (size_t)c->sel_cap * g.ppb * sizeof(PlanRec)},
         {(void**)&c->sink, 64},
         {(void**)&c->q_dev, (size_t)g.batch * g.n_q_heads * kD * 2},
         {(void**)&c->q_rot, (size_t)g.batch * g.n_q_heads * kD * 2},
@@ -202,7 +207,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     cudaMemset(c->dev_flags, 0, 256);
     cudaMemset(c->upd_cnt, 0, (size_t)g.n_layers * 4);
     cudaMemset(c->attn.stats, 0, 64);
-    cudaMemset(c->plan, 0, tu * (size_t)c->sel_cap * sizeof(PlanRec));
+    cudaMemset(c->plan, 0, tu * (size_t)c->sel_cap * g.ppb * sizeof(PlanRec));
     cudaMemset(c->strat, 0, tu * g.S_max * sizeof(StratRec));
     c->host_nseg.assign((size_t)g.n_layers * g.batch, 0);
     c->host_ntok.assign((size_t)g.n_layers * g.batch, 0);
@@ -316,13 +321,13 @@ int mkv_select(const mkv_cache* cc, int32_t layer, const void* q, int32_t budget
     const CacheGeom& g = c->geom;
     if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
     if (budget < 0 || (reduce != 0 && reduce != 1)) return fail(MKV_E_ARG, "mkv_select: bad budget/reduce");
-    const long long need = (long long)budget / kB + 1;
+    const long long need = (long long)budget / g.B + 1;
     if (k_max < 1 || k_max < (need < g.score_stride ? need : g.score_stride))
         return fail(MKV_E_ARG, "mkv_select: k_max %d too small for budget %d", k_max, budget);
     MKV_CUDA(cudaSetDevice(c->desc.device));
     MKV_CUDA(launch_select(g, c->view(layer), (const uint16_t*)q, budget, reduce, sel, sel_count, k_max,
                            scores_opt ? scores_opt : c->scores, c->cand_key, c->cand_idx,
-                           c->plan + (size_t)layer * g.n_units * c->sel_cap, c->sel_cap, plan_tag(c->generation, layer),
+                           c->plan + (size_t)layer * g.n_units * c->sel_cap * g.ppb, c->sel_cap * g.ppb, plan_tag(c->generation, layer),
                            c->sm_count, (cudaStream_t)stream, &c->last_select));
     return MKV_OK;
 }
@@ -480,7 +485,7 @@ int mkv_decode_host(mkv_cache* c, int32_t layer, const void* q_host, int32_t bud
     if (!c || !q_host || !out_host) return fail(MKV_E_ARG, "mkv_decode_host: NULL argument");
     const CacheGeom& g = c->geom;
     cudaStream_t s = (cudaStream_t)stream;
-    long long k_max = (long long)budget / kB + 1;
+    long long k_max = (long long)budget / g.B + 1;
     if (k_max > c->sel_cap) k_max = c->sel_cap;
     MKV_CUDA(cudaSetDevice(c->desc.device));
     MKV_CUDA(cudaMemcpyAsync(c->q_dev, q_host, (size_t)g.batch * g.n_q_heads * kD * 2, cudaMemcpyHostToDevice, s));
@@ -527,17 +532,18 @@ int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, vo
     // every g (the decode kernels read one layout), so sizes and offsets are recomputed here
     auto vbc = [](int r, int gg) -> uint32_t { return 2u * (uint32_t)r + (r == kD ? 0u : (uint32_t)(kD / (8 * gg))); };
     auto tokc = [&](const StratRec& r, int nb) -> uint32_t { return pad16u((uint32_t)nb * (vbc(r.r_k, r.g) + vbc(r.r_v, r.g))); };
+    const int B = g.B, pb = g.pb;
     auto segtokc = [&](const StratRec& r) -> uint64_t {
-        const int full = r.n_tok / kB, rem = r.n_tok % kB;
-        return (uint64_t)full * tokc(r, kB) + (rem ? tokc(r, rem) : 0u);
+        const int full = r.n_tok / B, rem = r.n_tok % B;
+        return (uint64_t)full * tokc(r, B) + (rem ? tokc(r, rem) : 0u);
     };
-    auto segbkc = [&](const StratRec& r) -> uint64_t { return pad16u((uint32_t)((r.n_tok + kB - 1) / kB) * vbc(r.r_k, r.g)); };
+    auto segbkc = [&](const StratRec& r) -> uint64_t { return pad16u((uint32_t)((r.n_tok + B - 1) / B) * vbc(r.r_k, r.g)); };
     uint64_t tok_bytes = 0, bk_bytes = 0, ptok_bytes = 0, pbk_bytes = 0;
     for (int s = 0; s < S; ++s) {
         tok_bytes += segtokc(rec[s]);
         bk_bytes += segbkc(rec[s]);
-        ptok_bytes += seg_tok_bytes(rec[s].r_k, rec[s].r_v, rec[s].n_tok);
-        pbk_bytes += seg_bk_bytes(rec[s].r_k, rec[s].n_tok);
+        ptok_bytes += seg_tok_bytes(rec[s].r_k, rec[s].r_v, rec[s].n_tok, pb);
+        pbk_bytes += seg_bk_bytes(rec[s].r_k, rec[s].n_tok, B);
     }
     const uint64_t tables = align_up(48 + (uint64_t)S * 16, 16);
     const uint64_t need = tables + tok_bytes + bk_bytes;
@@ -565,7 +571,7 @@ int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, vo
             int e = s;
             uint64_t trun = 0, krun = 0;
             while (e < S) {
-                const uint64_t tb = seg_tok_bytes(rec[e].r_k, rec[e].r_v, rec[e].n_tok), kb = seg_bk_bytes(rec[e].r_k, rec[e].n_tok);
+                const uint64_t tb = seg_tok_bytes(rec[e].r_k, rec[e].r_v, rec[e].n_tok, pb), kb = seg_bk_bytes(rec[e].r_k, rec[e].n_tok, B);
                 if (e > s && ((uint64_t)toff[e] * 16 != (uint64_t)toff[s] * 16 + trun || (uint64_t)koff[e] * 16 != (uint64_t)koff[s] * 16 + krun))
                     break;
                 trun += tb;
@@ -579,44 +585,52 @@ int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, vo
             s = e;
         }
     }
-    // One group of n <= 8 packed vectors, device -> canonical.  Device: n bitmaps of 128 bits (one bit per channel,
-    // every channel of a kept element group set), then the kept values RANK-major (compress.cu).  Canonical: n bitmaps
-    // of D / g bits (one per element group), then the values vector-major.  Dense vectors (r = D): values only.
-    auto repack = [](const uint8_t* src, uint8_t* dst, int r, int gg, int n) {
-        if (r == kD) { memcpy(dst, src, (size_t)n * kD * 2); return; }
+    // One canonical group of n = n0 + n1 packed vectors from (up to) two device groups of n0 and n1 <= 8 vectors (a token
+    // block of 16 tokens is stored as two device blocks).  Device group: its vectors' bitmaps of 128 bits (one bit per
+    // channel, every channel of a kept element group set), then the kept values RANK-major (compress.cu).  Canonical: n
+    // bitmaps of D / g bits (one per element group), then the values vector-major.  Dense vectors (r = D): values only.
+    auto repack = [](const uint8_t* src0, int n0, const uint8_t* src1, int n1, uint8_t* dst, int r, int gg) {
+        const int n = n0 + n1;
+        if (r == kD) {
+            memcpy(dst, src0, (size_t)n0 * kD * 2);
+            if (n1) memcpy(dst + (size_t)n0 * kD * 2, src1, (size_t)n1 * kD * 2);
+            return;
+        }
         const int bmc = kD / (8 * gg);
-        for (int t = 0; t < n; ++t)
+        uint8_t* o = dst + (size_t)n * bmc;
+        for (int t = 0; t < n; ++t) {
+            const uint8_t* src = t < n0 ? src0 : src1;
+            const int tt = t < n0 ? t : t - n0, nn = t < n0 ? n0 : n1;
             for (int m = 0; m < kD / gg; ++m) {
                 const int c = m * gg;
-                if ((src[t * kBitmapBytes + (c >> 3)] >> (c & 7)) & 1) dst[t * bmc + (m >> 3)] |= (uint8_t)(1u << (m & 7));
+                if ((src[tt * kBitmapBytes + (c >> 3)] >> (c & 7)) & 1) dst[t * bmc + (m >> 3)] |= (uint8_t)(1u << (m & 7));
             }
-        const uint16_t* v = reinterpret_cast<const uint16_t*>(src + (size_t)n * kBitmapBytes);  // (2-byte aligned: sizes are even)
-        uint8_t* o = dst + (size_t)n * bmc;
-        for (int t = 0; t < n; ++t)
-            for (int rho = 0; rho < r; ++rho) {
-                uint16_t x;
-                memcpy(&x, reinterpret_cast<const uint8_t*>(v) + 2 * ((size_t)rho * n + t), 2);
-                memcpy(o + 2 * ((size_t)t * r + rho), &x, 2);
-            }
+            const uint8_t* v = src + (size_t)nn * kBitmapBytes;  // rank-major values of the device group
+            for (int rho = 0; rho < r; ++rho) memcpy(o + 2 * ((size_t)t * r + rho), v + 2 * ((size_t)rho * nn + tt), 2);
+        }
     };
     uint64_t tpos = 0, kpos = 0;            // canonical positions
     const uint8_t* tp = ptok.data();
     const uint8_t* kp = pbk.data();
     for (int sg = 0; sg < S; ++sg) {
         const StratRec& r = rec[sg];
-        const int r_k = r.r_k, r_v = r.r_v, gg = r.g ? r.g : 1, n_tok = r.n_tok, nblk = (n_tok + kB - 1) / kB;
+        const int r_k = r.r_k, r_v = r.r_v, gg = r.g ? r.g : 1, n_tok = r.n_tok, nblk = (n_tok + B - 1) / B;
         const uint32_t ct = (uint32_t)(tpos / 16), ck = (uint32_t)(kpos / 16);
         memcpy(p_strat + (size_t)sg * 8, &r, 8);
         memcpy(p_toff + (size_t)sg * 4, &ct, 4);
         memcpy(p_koff + (size_t)sg * 4, &ck, 4);
         const uint32_t bmk = r_k == kD ? 0u : (uint32_t)kBitmapBytes;
-        for (int blk = 0; blk < nblk; ++blk) {
-            const int nb = std::min(kB, n_tok - blk * kB);
+        for (int blk = 0; blk < nblk; ++blk) {  // token blocks of B tokens = one or two device blocks of <= pb tokens
+            const int nbt = std::min(B, n_tok - blk * B);
+            const int n0 = std::min(pb, nbt), n1 = nbt - n0;
+            const uint8_t* s0 = tp;
+            const uint8_t* s1 = tp + tokblock_bytes(r_k, r_v, n0);
             uint8_t* d = tok_arena + tpos;
-            repack(tp, d, r_k, gg, nb);                                                                 // K vectors
-            repack(tp + (size_t)nb * (bmk + 2 * r_k), d + (size_t)nb * vbc(r_k, gg), r_v, gg, nb);      // V vectors
-            tp += tokblock_bytes(r_k, r_v, nb);
-            tpos += tokc(r, nb);
+            repack(s0, n0, s1, n1, d, r_k, gg);                                                                     // K vectors
+            repack(s0 + (size_t)n0 * (bmk + 2 * r_k), n0, s1 + (size_t)n1 * (bmk + 2 * r_k), n1,
+                   d + (size_t)nbt * vbc(r_k, gg), r_v, gg);                                                        // V vectors
+            tp += tokblock_bytes(r_k, r_v, n0) + (n1 ? tokblock_bytes(r_k, r_v, n1) : 0u);
+            tpos += tokc(r, nbt);
         }
         // block keys of the segment: device [bitmaps nblk x 16][values, groups of 8 keys rank-major]; canonical
         // [bitmaps nblk x D/(8g)][values nblk x r_k vector-major]
@@ -630,11 +644,11 @@ int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, vo
                 std::vector<uint8_t> tmp((size_t)n * kBitmapBytes + (size_t)n * r_k * 2), outg((size_t)n * bmc + (size_t)n * r_k * 2);
                 memcpy(tmp.data(), kp + (size_t)grp * 8 * kBitmapBytes, (size_t)n * kBitmapBytes);
                 memcpy(tmp.data() + (size_t)n * kBitmapBytes, kp + (size_t)nblk * kBitmapBytes + (size_t)grp * 8 * r_k * 2, (size_t)n * r_k * 2);
-                repack(tmp.data(), outg.data(), r_k, gg, n);
+                repack(tmp.data(), n, nullptr, 0, outg.data(), r_k, gg);
                 memcpy(d + (size_t)grp * 8 * bmc, outg.data(), (size_t)n * bmc);
                 memcpy(d + (size_t)nblk * bmc + (size_t)grp * 8 * r_k * 2, outg.data() + (size_t)n * bmc, (size_t)n * r_k * 2);
             }
-            kp += seg_bk_bytes(r_k, n_tok);
+            kp += seg_bk_bytes(r_k, n_tok, B);
             kpos += segbkc(r);
         }
     }

@@ -10,7 +10,7 @@
 namespace mkv {
 
 constexpr int kD = 128;          // head_dim supported on the GPU
-constexpr int kB = 8;            // token-block size supported on the GPU
+constexpr int kPhys = 8;         // tokens of a device token block at most (one half of an mma M tile)
 constexpr int kMaxGroup = 8;     // GQA group size limit
 constexpr int kBitmapBytes = 16; // D/g/8 at g = 1
 
@@ -38,8 +38,11 @@ struct LayerView {
 
 struct CacheGeom {
     int32_t n_layers, batch, n_kv_heads, n_q_heads, group, max_tokens, L, S_max, n_units;
-    int32_t blocks_per_seg;   // L / 8
-    int32_t score_stride;     // ceil(max_tokens / 8): blocks per unit capacity
+    int32_t blocks_per_seg;   // L / B
+    int32_t score_stride;     // ceil(max_tokens / B): blocks per unit capacity
+    int32_t B;                // token-block size of the cache (4, 8 or 16): unit of selection, one block key each
+    int32_t pb;               // tokens of a DEVICE token block: min(B, 8); a block of 16 tokens is stored as two of them
+    int32_t ppb;              // device blocks per token block: B / pb (1 or 2)
 };
 
 // bytes of payloads (canonical sizes)
@@ -48,12 +51,13 @@ __host__ __device__ inline uint32_t vec_bytes(int r) { return (r == kD ? 0u : (u
 __host__ __device__ inline uint32_t tokblock_bytes(int r_k, int r_v, int nb) {
     return pad16u((uint32_t)nb * (vec_bytes(r_k) + vec_bytes(r_v)));
 }
-__host__ __device__ inline uint32_t seg_tok_bytes(int r_k, int r_v, int n_tok) {
-    int full = n_tok / kB, rem = n_tok % kB;
-    return (uint32_t)full * tokblock_bytes(r_k, r_v, kB) + (rem ? tokblock_bytes(r_k, r_v, rem) : 0u);
+// device token blocks hold pb tokens, a segment's block keys one vector per B tokens
+__host__ __device__ inline uint32_t seg_tok_bytes(int r_k, int r_v, int n_tok, int pb) {
+    int full = n_tok / pb, rem = n_tok % pb;
+    return (uint32_t)full * tokblock_bytes(r_k, r_v, pb) + (rem ? tokblock_bytes(r_k, r_v, rem) : 0u);
 }
-__host__ __device__ inline uint32_t seg_bk_bytes(int r_k, int n_tok) {
-    int nblk = (n_tok + kB - 1) / kB;
+__host__ __device__ inline uint32_t seg_bk_bytes(int r_k, int n_tok, int B) {
+    int nblk = (n_tok + B - 1) / B;
     return pad16u((uint32_t)nblk * vec_bytes(r_k));
 }
 
@@ -94,24 +98,24 @@ constexpr int kTopkSlice = 16384;  // blocks per top-k slice (select.cu); longer
 struct __align__(16) PlanRec {
     int32_t t0;      // first token of the block
     uint32_t off16;  // payload offset in the layer slice, 16-B units
-    uint32_t meta;   // r_k | r_v << 8 | nb << 16   (nb = tokens in the block, 1..8)
+    uint32_t meta;   // r_k | r_v << 8 | nb << 16   (nb = tokens in the device block, 1..8)
     uint32_t tag;    // plan_tag(generation, layer); 0 = never written
 };
 __host__ __device__ inline uint32_t plan_tag(uint32_t generation, int layer) {
     return ((generation & 0xffffu) << 16) | ((uint32_t)layer & 0xffffu) | 0x80000000u;
 }
 #ifdef __CUDACC__
-// table lookup of the block that starts at token t0 of `unit`; meta = 0 if t0 is not a block start of the unit
+// table lookup of the DEVICE block that starts at token t0 of `unit`; meta = 0 if t0 is not a device-block start of the unit
 __device__ __forceinline__ void plan_lookup(const CacheGeom& g, const LayerView& lv, int unit, int t0, uint32_t& off16,
                                             uint32_t& meta) {
     off16 = 0u; meta = 0u;
-    if (t0 < 0 || t0 >= lv.unit_ntok[unit] || (t0 & (kB - 1)) != 0) return;
+    if (t0 < 0 || t0 >= lv.unit_ntok[unit] || (t0 % g.pb) != 0) return;
     const int seg = t0 / g.L, in_seg = t0 - seg * g.L;
     const size_t e = (size_t)unit * lv.S_max + seg;
     const StratRec rec = lv.strat[e];
     if ((int)rec.n_tok <= in_seg) return;
-    const uint32_t nb = (uint32_t)min(kB, (int)rec.n_tok - in_seg);
-    off16 = lv.tok_off[e] + (uint32_t)(in_seg >> 3) * (tokblock_bytes(rec.r_k, rec.r_v, kB) >> 4);
+    const uint32_t nb = (uint32_t)min(g.pb, (int)rec.n_tok - in_seg);
+    off16 = lv.tok_off[e] + (uint32_t)(in_seg / g.pb) * (tokblock_bytes(rec.r_k, rec.r_v, g.pb) >> 4);
     meta = (uint32_t)rec.r_k | ((uint32_t)rec.r_v << 8) | (nb << 16);
 }
 #endif

@@ -98,7 +98,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             if ((int)seg < lv.unit_nseg[u]) {
                 const size_t e = (size_t)u * lv.S_max + seg;
                 const StratRec rec = lv.strat[e];
-                const int nblk = ((int)rec.n_tok + kB - 1) / kB;
+                const int nblk = ((int)rec.n_tok + g.B - 1) / g.B;
                 const int n = min(8, nblk - 8 * (int)sub);
                 if (n > 0) {
                     const uint32_t off = lv.bk_off[e];

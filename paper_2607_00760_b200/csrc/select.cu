@@ -55,6 +55,7 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
     pdl_wait();  // the scores (MODE 0, 1) / the candidates (MODE 2) are complete
     pdl_launch_dependents();
     const int ntok = lv.unit_ntok[unit];
+    const int kB = g.B;                           // tokens per block (the cache's token-block size)
     const int nblk = (ntok + kB - 1) / kB;        // blocks of the unit
     const float* s = scores + (size_t)unit * g.score_stride;
     // the elements this CTA selects from: n of them; element i has key keyat(i) and block index idxat(i)
@@ -265,9 +266,10 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
         // what mkv_packed_attention needs to know about every selected block (payload offset, tokens, r_k, r_v): one
         // record per block, looked up by all threads at once (one round of table reads for the whole unit)
         __syncthreads();  // the CTA's writes to `out` are visible to its own threads
-        for (int p = tid; p < min(count, plan_stride); p += 1024) {
+        // (a block of 16 tokens is two device blocks: two records, at 2 p and 2 p + 1)
+        for (int p = tid; p < count * g.ppb && p < plan_stride; p += 1024) {
             PlanRec pr;
-            pr.t0 = out[p]; pr.tag = tag;
+            pr.t0 = out[p / g.ppb] + kPhys * (p % g.ppb); pr.tag = tag;
             plan_lookup(g, lv, unit, pr.t0, pr.off16, pr.meta);
             plan[(size_t)unit * plan_stride + p] = pr;
         }
@@ -289,7 +291,7 @@ cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_
     cudaError_t err = launch_score(g, lv, q, reduce, scores, sm_count, s);
     if (err != cudaSuccess) return err;
     const int n_slices = (g.score_stride + kKeyCap - 1) / kKeyCap;
-    const int cand_cap = budget / kB + 1 < kKeyCap ? budget / kB + 1 : kKeyCap;  // candidates kept per slice
+    const int cand_cap = budget / g.B + 1 < kKeyCap ? budget / g.B + 1 : kKeyCap;  // candidates kept per slice
     if (n_slices == 1) {
         err = launch_pdl(mkv_topk_kernel<0>, dim3(g.n_units), dim3(1024), 0, s, g, lv, (const float*)scores, budget, sel,
                          sel_count, k_max, (uint32_t*)nullptr, (int32_t*)nullptr, 1, 0, plan, plan_stride, tag);

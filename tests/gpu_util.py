@@ -26,14 +26,15 @@ def uniform_strat(Bt, Hkv, S, r_k, r_v=None, g=1, B=8):
 class Case:
     """One synthetic problem on the device + its oracle blobs."""
 
-    def __init__(self, mkv, dev, Bt, Hkv, Hq, N, L=64, seed=0, n_layers=1):
+    def __init__(self, mkv, dev, Bt, Hkv, Hq, N, L=64, seed=0, n_layers=1, B=8):
         import torch
         self.mkv, self.dev = mkv, dev
         self.Bt, self.Hkv, self.Hq, self.N, self.L, self.D = Bt, Hkv, Hq, N, L, 128
         self.G, self.S = Hq // Hkv, (N + L - 1) // L
         self.K, self.V, self.q = synth.make_inputs_np(Bt, Hkv, Hq, N, 128, L, seed=seed)
         self.k_d, self.v_d, self.q_d = to_dev(self.K, dev), to_dev(self.V, dev), to_dev(self.q, dev)
-        self.cache = mkv.Cache(n_layers, Bt, Hkv, Hq, 128, N, L)
+        self.B = B   # token-block size of the cache (PAPER.md:240: 4, 8 or 16)
+        self.cache = mkv.Cache(n_layers, Bt, Hkv, Hq, 128, N, L, token_block=B)
         self.torch = torch
         self.blobs = None
 
@@ -45,7 +46,7 @@ class Case:
         torch = self.torch
         lk = torch.zeros((self.Bt, self.Hkv, self.S), dtype=torch.float64, device=self.dev)
         lv = torch.zeros_like(lk)
-        self.cache.segment_loss(self.k_d, self.v_d, (r_k, r_v, g, 8), lk, lv)
+        self.cache.segment_loss(self.k_d, self.v_d, (r_k, r_v, g, self.B), lk, lv)
         torch.cuda.synchronize()
         return lk.cpu().numpy(), lv.cpu().numpy()
 
@@ -71,8 +72,8 @@ class Case:
     # ---- step 2
     def gpu_select(self, budget, reduce=0, layer=0, want_scores=False):
         torch = self.torch
-        nblk = (self.N + 7) // 8
-        k_max = min(budget // 8 + 1, nblk)
+        nblk = (self.N + self.B - 1) // self.B
+        k_max = min(budget // self.B + 1, nblk)
         k_max = max(k_max, 1)
         sel = torch.full((self.Bt, self.Hkv, k_max), -7, dtype=torch.int32, device=self.dev)
         cnt = torch.full((self.Bt, self.Hkv), -7, dtype=torch.int32, device=self.dev)
@@ -115,8 +116,8 @@ class Case:
 
     # ---- step 3
     def oracle_sel(self, budget, reduce=0):
-        nblk = (self.N + 7) // 8
-        k_max = max(1, min(budget // 8 + 1, nblk))
+        nblk = (self.N + self.B - 1) // self.B
+        k_max = max(1, min(budget // self.B + 1, nblk))
         sel = np.full((self.Bt, self.Hkv, k_max), -1, np.int32)
         cnt = np.zeros((self.Bt, self.Hkv), np.int32)
         for b in range(self.Bt):

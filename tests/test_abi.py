@@ -33,7 +33,7 @@ def test_library_exports_every_declared_symbol():
     for name in declared_symbols():
         assert hasattr(lib, name), f"libmkv.so does not export {name}"
     assert sorted(binding.SYMBOLS) == declared_symbols()
-    assert binding.mkv_version() == 1
+    assert binding.mkv_version() == 2
 
 
 def test_no_torch_types_in_the_boundary():

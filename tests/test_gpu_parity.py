@@ -770,6 +770,85 @@ def test_element_groups_end_to_end(env, g, r_k, r_v):
         c.free()
 
 
+@pytest.mark.parametrize("B,L,g", [(4, 64, 1), (16, 64, 1), (16, 32, 2), (4, 32, 4), (16, 64, 4)])
+def test_token_block_sizes_end_to_end(env, B, L, g):
+    """SURVEY 8(f) NEXT-2 ("block size (e.g., 4, 8, and 16)"): a cache whose token blocks hold 4 or 16
+    tokens.  Loss, packed blob (bit-exact: one block key and one payload group per B tokens), block scores, top-k by token
+    budget (k = budget / B blocks), attention over selections, the update buffer on top, and the host call."""
+    mkv, dev = env
+    import torch
+    N = L * 11 + 13  # ragged tail: a last block of 13 = 8 + 5 (B = 16) or 4 + 4 + 4 + 1 (B = 4) tokens
+    c = Case(mkv, dev, 2, 2, 8, N, L=L, seed=140 + B + g, B=B)
+    try:
+        r = 36 if g == 4 else 38
+        lk, lv = c.gpu_loss(r, r, g)
+        for b in range(2):
+            for h in range(2):
+                rk_, rv_ = orc.segment_loss(c.K[b, h], c.V[b, h], L, r, r, g)
+                np.testing.assert_allclose(lk[b, h], rk_, rtol=1e-12, atol=0)
+                np.testing.assert_allclose(lv[b, h], rv_, rtol=1e-12, atol=0)
+        strat = uniform_strat(2, 2, c.S, r, r, g=g, B=B)
+        strat[:, :, 3::4, 0:2] = 128            # dense segments
+        strat[:, :, 2::4, 0:2] = (64, 92)       # another rate
+        strat[0, 1, 1, 0:2] = (128, 4 * g)      # dense K over a nearly empty V
+        c.compress(strat)
+        c.assert_export_equal()
+        for budget in (B, 200, 8 * B + 3):
+            total, swaps = c.check_select(budget)
+            assert swaps * 1000 <= total
+        sel, cnt, _ = c.gpu_select(200)
+        assert np.all(cnt == 200 // B)
+        for budget in (B, 200, N):
+            sel, cnt = c.oracle_sel(budget)
+            c.check_attention(sel, cnt)
+        # a selection that holds the ragged last block and the last full one
+        sel = np.full((2, 2, 3), -1, np.int32)
+        sel[:, :, 0], sel[:, :, 1], sel[:, :, 2] = 0, (N // B - 1) * B, (N // B) * B
+        cnt = np.full((2, 2), 3, np.int32)
+        c.check_attention(sel, cnt)
+        # the update buffer on top (raw tokens, blocks of 8 whatever B is)
+        c.cache.update_append(0, c.k_d[:, :, :11], c.v_d[:, :, :11])
+        out, lse = c.gpu_attention(sel, cnt)
+        ref, ref_lse = np.zeros_like(out), np.zeros_like(lse)
+        for b in range(2):
+            for h in range(2):
+                o, l = orc.attention_with_update_buffer(c.blobs[b][h], c.q[b, 4 * h:4 * h + 4], sel[b, h], 1 / math.sqrt(128),
+                                                        c.K[b, h, :11], c.V[b, h, :11])
+                ref[b, 4 * h:4 * h + 4], ref_lse[b, 4 * h:4 * h + 4] = o, l
+        assert_attention_close(out, lse, ref, ref_lse)
+        c.cache.reset(0)
+        c.compress(strat)
+        # the host call (select + attention in one graph; the plan carries both halves of a 16-token block)
+        q_host = torch.from_numpy(c.q.view(np.int16)).view(torch.bfloat16).pin_memory()
+        out_host = torch.zeros((2, 8, 128), dtype=torch.float32).pin_memory()
+        k_max = 256 // B + 1
+        sel_host = torch.zeros((2, 2, k_max), dtype=torch.int32).pin_memory()
+        cnt_host = torch.zeros((2, 2), dtype=torch.int32).pin_memory()
+        c.cache.decode_host(0, q_host, 256, 1 / math.sqrt(128), out_host, sel_host=sel_host, sel_count_host=cnt_host)
+        torch.cuda.synchronize()
+        selh, cnth = sel_host.numpy(), cnt_host.numpy()
+        assert np.all(cnth == 256 // B)
+        ref = np.zeros((2, 8, 128))
+        for b in range(2):
+            for h in range(2):
+                ref[b, 4 * h:4 * h + 4], _ = orc.attention(c.blobs[b][h], c.q[b, 4 * h:4 * h + 4], selh[b, h, :cnth[b, h]],
+                                                            1 / math.sqrt(128))
+        o = out_host.numpy().astype(np.float64)
+        assert np.abs(o - ref).max() <= 3e-3 and np.linalg.norm(o - ref) / np.linalg.norm(ref) <= 1e-3
+        # a strategy that names another B is refused: one B per cache
+        bad = strat.copy()
+        bad[0, 0, 0, 3] = 8
+        c.cache.reset(0)
+        c.cache.compress_segment(0, c.k_d, c.v_d, torch.from_numpy(bad).to(dev))
+        torch.cuda.synchronize()
+        with pytest.raises(mkv.MkvError) as e:
+            c.cache.status()
+        assert e.value.code == mkv.MKV_E_DEVICE
+    finally:
+        c.free()
+
+
+
 def test_threshold_rule_over_the_papers_grid(env):
     """"evaluates the compression loss for each candidate compression rate (e.g., 87.5%, 75%, and 62.5%) and
     element group size (e.g., 1, 2, and 4) ... The highest compression rate and largest group size whose loss remains
