@@ -13,6 +13,7 @@ namespace {
 
 constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned long long kNoBase = ~0ull;
+constexpr int kStageBytes = 8 * 2 * (kBitmapBytes + 2 * 127);  // the largest packed token block; a dense one is 4096 B
 
 __device__ __forceinline__ unsigned lanemask_lt() {
     unsigned m;
@@ -106,8 +107,10 @@ __device__ __forceinline__ void topr_mask_groups(const uint32_t (&x)[4], int r, 
 // through disjoint shared-memory banks in the decode kernels' walk.  Dense vectors (r = D) carry
 // no bitmap and stay vector-major.  x[j]: bf16 bits of channel lane + 32 j.
 // bm: this vector's bitmap; val: the GROUP's value area (2-byte aligned).
+// cached: a mask found earlier for this vector by mkv_segment_loss (or nullptr).  It is used only if it keeps r elements
+// and every kept magnitude is strictly above every dropped one -- then it IS the top-r mask, whatever wrote it.
 __device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, int g, uint8_t* bm, uint8_t* val, int t, int n,
-                                            int lane) {
+                                            int lane, bool cached = false, uint4 cw = make_uint4(0u, 0u, 0u, 0u)) {
     uint16_t* v16 = reinterpret_cast<uint16_t*>(val);
     if (r == kD) {
 #pragma unroll
@@ -117,8 +120,24 @@ __device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, int g
     uint32_t mag[4], w[4];
 #pragma unroll
     for (int j = 0; j < 4; ++j) mag[j] = x[j] & 0x7FFFu;
-    if (g == 1) topr_mask(mag, r, w);
-    else topr_mask_groups(x, r, g, w, lane);
+    bool have = false;
+    if (g == 1 && cached) {
+        w[0] = cw.x; w[1] = cw.y; w[2] = cw.z; w[3] = cw.w;
+        uint32_t kmin = 0x8000u, dmax = 0u;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const bool kept = (w[j] >> lane) & 1u;
+            kmin = kept ? min(kmin, mag[j]) : kmin;
+            dmax = kept ? dmax : max(dmax, mag[j]);
+        }
+        kmin = __reduce_min_sync(kFull, kmin);
+        dmax = __reduce_max_sync(kFull, dmax);
+        have = __popc(w[0]) + __popc(w[1]) + __popc(w[2]) + __popc(w[3]) == r && kmin > dmax;
+    }
+    if (!have) {
+        if (g == 1) topr_mask(mag, r, w);
+        else topr_mask_groups(x, r, g, w, lane);
+    }
     const unsigned lt = lanemask_lt();
     int base = 0;
 #pragma unroll
@@ -253,7 +272,7 @@ __global__ void __launch_bounds__(256) mkv_plan_kernel(CacheGeom g, LayerView lv
 // compress: CTA = 8 warps = 8 consecutive token blocks of one segment; warp = one token block:
 // nb K vectors, nb V vectors, and the block key (fp32 sum in token order, IEEE /nb, RNE bf16).
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) mkv_compress_kernel(CacheGeom g, LayerView lv, CompressArgs a,
+__global__ void __launch_bounds__(256, 4) mkv_compress_kernel(CacheGeom g, LayerView lv, CompressArgs a,
                                                            const unsigned long long* __restrict__ call_base,
                                                            int chunks_per_seg) {
     const int uc = blockIdx.y;
@@ -273,7 +292,9 @@ __global__ void __launch_bounds__(256) mkv_compress_kernel(CacheGeom g, LayerVie
     const uint32_t bmk = (r_k == kD) ? 0u : kBitmapBytes, bmv = (r_v == kD) ? 0u : kBitmapBytes;
 
     uint8_t* base = lv.slice + ((size_t)lv.tok_off[e] << 4) + (size_t)blk * tokblock_bytes(r_k, r_v, pb);
-    uint8_t* k_bm = base;
+    // the block is packed in shared memory (2-byte stores at rank-major positions) and leaves in 16-byte stores
+    __shared__ __align__(16) uint8_t s_stage[8][kStageBytes];
+    uint8_t* k_bm = s_stage[warp];
     uint8_t* k_val = k_bm + nb * bmk;
     uint8_t* v_bm = k_val + nb * r_k * 2;
     uint8_t* v_val = v_bm + nb * bmv;
@@ -283,27 +304,51 @@ __global__ void __launch_bounds__(256) mkv_compress_kernel(CacheGeom g, LayerVie
                         (size_t)(seg_local * g.L + blk * pb) * a.stride_t;
     const uint16_t* ksrc = a.k + row0;
     const uint16_t* vsrc = a.v + row0;
+    // masks of this block's vectors as mkv_segment_loss left them, [token][K, V][4 words]: 64 words, two per lane
+    const bool mk = a.masks != nullptr;
+    uint32_t m0 = 0u, m1 = 0u;
+    if (mk) {
+        const uint32_t* m32 = reinterpret_cast<const uint32_t*>(
+            a.masks + 2 * ((size_t)unit * a.mask_stride + (size_t)(a.seg0 + seg_local) * g.L + blk * pb));
+        if (lane < 8 * nb) m0 = __ldg(m32 + lane);
+        if (32 + lane < 8 * nb) m1 = __ldg(m32 + 32 + lane);
+    }
+    auto cached_mask = [&](int t, int which) {  // words 8 t + 4 which .. + 3
+        const uint32_t src = t < 4 ? m0 : m1;
+        const int l0 = (8 * t + 4 * which) & 31;
+        return make_uint4(__shfl_sync(kFull, src, l0), __shfl_sync(kFull, src, l0 + 1), __shfl_sync(kFull, src, l0 + 2),
+                          __shfl_sync(kFull, src, l0 + 3));
+    };
 
     float sum[4] = {0.f, 0.f, 0.f, 0.f};
+    // token t + 1 is loaded while token t is searched and packed (the loads are what the warp would wait for)
+    uint32_t nk[4], nv[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { nk[j] = __ldg(ksrc + lane + 32 * j); nv[j] = __ldg(vsrc + lane + 32 * j); }
+#pragma unroll 1
     for (int t = 0; t < nb; ++t) {
-        uint32_t x[4];
+        uint32_t xk[4], xv[4];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) x[j] = __ldg(ksrc + (size_t)t * a.stride_t + lane + 32 * j);
+        for (int j = 0; j < 4; ++j) { xk[j] = nk[j]; xv[j] = nv[j]; }
+        if (t + 1 < nb) {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) sum[j] = __fadd_rn(sum[j], bf16_bits_to_f32(x[j]));
-        pack_vector(x, r_k, rec.g, k_bm + t * bmk, k_val, t, nb, lane);
+            for (int j = 0; j < 4; ++j) {
+                nk[j] = __ldg(ksrc + (size_t)(t + 1) * a.stride_t + lane + 32 * j);
+                nv[j] = __ldg(vsrc + (size_t)(t + 1) * a.stride_t + lane + 32 * j);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) sum[j] = __fadd_rn(sum[j], bf16_bits_to_f32(xk[j]));
+        pack_vector(xk, r_k, rec.g, k_bm + t * bmk, k_val, t, nb, lane, mk && r_k != kD, cached_mask(t, 0));
+        pack_vector(xv, r_v, rec.g, v_bm + t * bmv, v_val, t, nb, lane, mk && r_v != kD, cached_mask(t, 1));
     }
-    for (int t = 0; t < nb; ++t) {
-        uint32_t x[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) x[j] = __ldg(vsrc + (size_t)t * a.stride_t + lane + 32 * j);
-        pack_vector(x, r_v, rec.g, v_bm + t * bmv, v_val, t, nb, lane);
-    }
-    // zero the pad of a ragged token block
     {
         const uint32_t used = (uint32_t)nb * (vec_bytes(r_k) + vec_bytes(r_v));
         const uint32_t padded = pad16u(used);
-        for (uint32_t o = used + lane; o < padded; o += 32) base[o] = 0;
+        for (uint32_t o = used + lane; o < padded; o += 32) s_stage[warp][o] = 0;  // the pad of a ragged token block
+        __syncwarp();
+        for (uint32_t o = 16u * lane; o < padded; o += 512u)
+            *reinterpret_cast<uint4*>(base + o) = *reinterpret_cast<const uint4*>(s_stage[warp] + o);
     }
     // block key of the token block (B tokens): a block of 16 tokens spans two device blocks; the warp of the first one
     // goes on through the keys of the second (fp32 sum in token order over the whole block, R5)
@@ -349,6 +394,8 @@ __global__ void __launch_bounds__(256) mkv_segment_loss_kernel(CacheGeom g, Comp
     const size_t row0 = (size_t)(b - a.b0) * a.stride_b + (size_t)h * a.stride_h +
                         (size_t)(seg_local * g.L) * a.stride_t;
     double acc[4] = {0., 0., 0., 0.};  // dropped_k, total_k, dropped_v, total_v
+    const int unit = b * g.n_kv_heads + h;
+    uint4* masks = a.masks ? a.masks + 2 * ((size_t)unit * a.mask_stride + (size_t)(a.seg0 + seg_local) * g.L) : nullptr;
     for (int which = 0; which < 2; ++which) {
         const uint16_t* src = (which ? a.v : a.k) + row0;
         const int r = which ? r_v : r_k;
@@ -360,8 +407,10 @@ __global__ void __launch_bounds__(256) mkv_segment_loss_kernel(CacheGeom g, Comp
                 mag[j] = x[j] & 0x7FFFu;
             }
             if (r == kD) w[0] = w[1] = w[2] = w[3] = kFull;
-            else if (grp == 1) topr_mask(mag, r, w);
-            else topr_mask_groups(x, r, grp, w, lane);
+            else if (grp == 1) {
+                topr_mask(mag, r, w);
+                if (masks != nullptr && lane == 0) masks[2 * t + which] = make_uint4(w[0], w[1], w[2], w[3]);
+            } else topr_mask_groups(x, r, grp, w, lane);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const float f = bf16_bits_to_f32(x[j]);

@@ -68,6 +68,7 @@ struct mkv_cache {
     std::vector<uint8_t> rot_set;             // per layer: a rotation is installed
     uint16_t* q_rot = nullptr;                // [batch][n_q_heads][D] folded query of mkv_decode_host
     uint16_t* q_dev = nullptr;
+    uint4* masks = nullptr;                   // [n_units][max_tokens][2]: top-r masks found by mkv_segment_loss (compress.cu)
     int32_t* sel_dev = nullptr;
     int32_t* selcnt_dev = nullptr;
     float* out_dev = nullptr;
@@ -112,7 +113,7 @@ int mkv_cache_free(mkv_cache* c) {
     cudaDeviceSynchronize();
     void* ptrs[] = {c->arena, c->strat, c->tok_off, c->bk_off, c->unit_nseg, c->unit_ntok, c->counters,
                     c->dev_flags, c->call_base, c->scores, c->cand_key, c->cand_idx, c->upd_k, c->upd_v, c->upd_cnt, c->attn.zbuf, c->attn.stats, c->plan, c->sink, c->rot_k, c->rot_v, c->q_rot, c->q_dev,
-                    c->sel_dev, c->selcnt_dev, c->out_dev};
+                    c->sel_dev, c->selcnt_dev, c->out_dev, c->masks};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     delete c;
@@ -192,6 +193,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
         {(void**)&c->sel_dev, (size_t)g.n_units * c->sel_cap * 4},
         {(void**)&c->selcnt_dev, (size_t)g.n_units * 4},
         {(void**)&c->out_dev, (size_t)g.batch * g.n_q_heads * kD * 4},
+        {(void**)&c->masks, (size_t)g.n_units * (size_t)d->max_tokens * 32},
     };
     for (auto& a : allocs) {
         cudaError_t e = cudaMalloc(a.p, a.bytes);
@@ -209,6 +211,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     cudaMemset(c->attn.stats, 0, 64);
     cudaMemset(c->plan, 0, tu * (size_t)c->sel_cap * g.ppb * sizeof(PlanRec));
     cudaMemset(c->strat, 0, tu * g.S_max * sizeof(StratRec));
+    cudaMemset(c->masks, 0, (size_t)g.n_units * (size_t)d->max_tokens * 32);
     c->host_nseg.assign((size_t)g.n_layers * g.batch, 0);
     c->host_ntok.assign((size_t)g.n_layers * g.batch, 0);
     cudaError_t e = attention_prepare(g, c->sm_count, c->attn_cluster);
@@ -260,7 +263,7 @@ int mkv_segment_loss(const mkv_cache* c, const void* k, const void* v, int64_t s
     if (cand.r_k < 1 || cand.r_k > kD || cand.r_v < 1 || cand.r_v > kD) return fail(MKV_E_ARG, "candidate r out of range");
     if (cand.g != 1 && cand.g != 2 && cand.g != 4) return fail(MKV_E_ARG, "element group %d: must be 1, 2 or 4", cand.g);
     if (cand.r_k % cand.g || cand.r_v % cand.g) return fail(MKV_E_ARG, "kept elements must be multiples of the element group");
-    CompressArgs a{(const uint16_t*)k, (const uint16_t*)v, sb, sh, st, b0, nb, seg0, nseg, n_tok};
+    CompressArgs a{(const uint16_t*)k, (const uint16_t*)v, sb, sh, st, b0, nb, seg0, nseg, n_tok, c->masks, c->geom.max_tokens};
     MKV_CUDA(cudaSetDevice(c->desc.device));
     MKV_CUDA(launch_segment_loss(c->geom, a, cand, loss_k, loss_v, (cudaStream_t)stream));
     return MKV_OK;
@@ -303,7 +306,7 @@ int mkv_compress_segment(mkv_cache* c, int32_t layer, const void* k, const void*
         if (seg0 != have) return fail(MKV_E_STATE, "request %d holds %d segments; seg0 = %d (append-only)", b, have, seg0);
         if (tok != have * g.L) return fail(MKV_E_STATE, "request %d ends in a short segment; cannot append", b);
     }
-    CompressArgs a{(const uint16_t*)k, (const uint16_t*)v, sb, sh, st, b0, nb, seg0, nseg, n_tok};
+    CompressArgs a{(const uint16_t*)k, (const uint16_t*)v, sb, sh, st, b0, nb, seg0, nseg, n_tok, c->masks, c->geom.max_tokens};
     MKV_CUDA(cudaSetDevice(c->desc.device));
     MKV_CUDA(launch_compress(g, c->view(layer), a, strat, c->call_base, c->dev_flags, (cudaStream_t)stream,
                              &c->last_compress));
@@ -444,7 +447,7 @@ int mkv_update_append(mkv_cache* c, int32_t layer, const void* k_new, const void
     if (have + n_new > g.L)
         return fail(MKV_E_STATE, "mkv_update_append: buffer holds %d of %d tokens; %d more do not fit (flush first)", have,
                     g.L, n_new);
-    CompressArgs a{(const uint16_t*)k_new, (const uint16_t*)v_new, sb, sh, st, 0, g.batch, 0, 1, n_new};
+    CompressArgs a{(const uint16_t*)k_new, (const uint16_t*)v_new, sb, sh, st, 0, g.batch, 0, 1, n_new, nullptr, 0};
     MKV_CUDA(cudaSetDevice(c->desc.device));
     const size_t off = (size_t)layer * g.n_units * g.L * kD;
     MKV_CUDA(launch_update_copy(g, a, c->upd_k + off, c->upd_v + off, c->upd_cnt + layer, have, (cudaStream_t)stream));

@@ -67,6 +67,10 @@ struct CompressArgs {
     const uint16_t* v;
     int64_t stride_b, stride_h, stride_t;
     int32_t b0, nb, seg0, nseg, n_tok;
+    // top-r masks of the last mkv_segment_loss call, [unit][token][K, V] x 128 bits (or nullptr): mkv_compress_segment
+    // takes a mask from here after checking it against the vector itself, so a stale entry is only a missed shortcut
+    uint4* masks;
+    int64_t mask_stride;  // tokens per unit in `masks` (= max_tokens)
 };
 
 cudaError_t launch_segment_loss(const CacheGeom& g, const CompressArgs& a, mkv_strategy cand,

@@ -30,7 +30,7 @@ constexpr uint32_t kPairMaxR = 56;  // 128 + 16 r_k <= kItem1
 struct __align__(16) SDesc {
     uint32_t bm0, val0, bm1, val1;  // chunk offsets in the layer slice, 16-B units (dense: bm = the keys, val unused)
     uint32_t out0, out1;            // index of each item's first score: unit * score_stride + block index
-    uint32_t meta;                  // r_k | nb0 << 8 | nb1 << 12
+    uint32_t meta;                  // r_k | nb0 << 8 | nb1 << 12 | merged << 16: the group is ONE contiguous chunk of the slice
     uint32_t unit;
 };
 
@@ -89,6 +89,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
     // runs of such items are paired greedily from their start.  Items past a unit's end hold no keys.
     auto build = [&](int count) {
         uint32_t bm = 0u, val = 0u, out = 0u, r_k = 0u, nb = 0u, u = 0u;
+        uint32_t sz = 0u;  // 16-B units of the item when its bitmaps and values are one chunk (one item per segment), else 0
         if (lane < count) {
             const unsigned it = lo + (unsigned)(ibuilt + lane);
             u = it / items_per_unit;
@@ -106,6 +107,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                     if (rec.r_k == kD) { bm = off + 128u * sub; val = bm; }
                     else { bm = off + 8u * sub; val = off + (uint32_t)nblk + (uint32_t)rec.r_k * sub; }
                     out = u * (unsigned)g.score_stride + seg * (unsigned)g.blocks_per_seg + 8u * sub;
+                    if (rec.r_k != kD && nblk <= 8) sz = nb + ((nb * 2u * r_k + 15u) >> 4);
                 }
             }
         }
@@ -118,11 +120,14 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
         const unsigned gm = __ballot_sync(kFull, first);
         const uint32_t bm1 = __shfl_down_sync(kFull, bm, 1), val1 = __shfl_down_sync(kFull, val, 1);
         const uint32_t out1 = __shfl_down_sync(kFull, out, 1), nb1 = __shfl_down_sync(kFull, nb, 1);
+        const uint32_t sz1 = __shfl_down_sync(kFull, sz, 1);
+        // segments compressed by one call lie back to back in the slice (plan kernel): the usual group is one chunk
+        const bool merged = two && sz != 0u && sz1 != 0u && bm1 == bm + sz;
         if (first) {
             SDesc d;
             d.bm0 = bm; d.val0 = val; d.bm1 = two ? bm1 : 0u; d.val1 = two ? val1 : 0u;
             d.out0 = out; d.out1 = two ? out1 : 0u;
-            d.meta = r_k | (nb << 8) | ((two ? nb1 : 0u) << 12);
+            d.meta = r_k | (nb << 8) | ((two ? nb1 : 0u) << 12) | (merged ? 1u << 16 : 0u);
             d.unit = u;
             ring[(gbuilt + __popc(gm & lanemask_lt())) & (kRing - 1)] = d;
         }
@@ -145,10 +150,14 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             const uint32_t bb0 = r == (uint32_t)kD ? nb0 * 256u : nb0 * 16u, vb0 = r == (uint32_t)kD ? 0u : pad16u(nb0 * 2u * r);
             const uint32_t bb1 = r == (uint32_t)kD ? nb1 * 256u : nb1 * 16u, vb1 = r == (uint32_t)kD ? 0u : pad16u(nb1 * 2u * r);
             mbar_expect_tx(bar, bb0 + vb0 + bb1 + vb1);
-            bulk_g2s(dst, slice + ((unsigned long long)d.bm0 << 4), bb0, bar);
-            if (vb0) bulk_g2s(dst + bb0, slice + ((unsigned long long)d.val0 << 4), vb0, bar);
-            if (bb1) bulk_g2s(dst + kItem1, slice + ((unsigned long long)d.bm1 << 4), bb1, bar);
-            if (vb1) bulk_g2s(dst + kItem1 + bb1, slice + ((unsigned long long)d.val1 << 4), vb1, bar);
+            if (d.meta >> 16) {  // item 1 lands right behind item 0
+                bulk_g2s(dst, slice + ((unsigned long long)d.bm0 << 4), bb0 + vb0 + bb1 + vb1, bar);
+            } else {
+                bulk_g2s(dst, slice + ((unsigned long long)d.bm0 << 4), bb0, bar);
+                if (vb0) bulk_g2s(dst + bb0, slice + ((unsigned long long)d.val0 << 4), vb0, bar);
+                if (bb1) bulk_g2s(dst + kItem1, slice + ((unsigned long long)d.bm1 << 4), bb1, bar);
+                if (vb1) bulk_g2s(dst + kItem1 + bb1, slice + ((unsigned long long)d.val1 << 4), vb1, bar);
+            }
         }
         ++gposi;
     };
@@ -178,7 +187,8 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                 }
             }
             const int r_k = (int)(d.meta & 255u), nb0 = (int)((d.meta >> 8) & 15u), nb1 = (int)((d.meta >> 12) & 15u);
-            const uint32_t sp0 = stage0 + s * kScoreStage, sp1 = sp0 + kItem1;
+            const uint32_t sp0 = stage0 + s * kScoreStage;
+            const uint32_t sp1 = sp0 + ((d.meta >> 16) ? 16u * (uint32_t)nb0 + pad16u(2u * (uint32_t)(nb0 * r_k)) : (uint32_t)kItem1);
 
             mbar_wait(bar0 + 8 * s, parity);  // the group's bulk copies have landed
 

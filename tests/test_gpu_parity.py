@@ -770,6 +770,49 @@ def test_element_groups_end_to_end(env, g, r_k, r_v):
         c.free()
 
 
+def test_compress_after_loss_takes_only_valid_masks(env):
+    """mkv_segment_loss leaves its top-r masks in a scratch of the cache and mkv_compress_segment takes a mask from there
+    after checking it against the vector (r kept, every kept magnitude strictly above every dropped one).  Bit-exact blobs
+    (a) right after the loss call, on data with exact ties and zeros, (b) when the scratch holds masks of OTHER data, of
+    another rate, or only of a part of the tokens."""
+    mkv, dev = env
+    import torch
+    from paper_2607_00760_b200 import synth
+    c = Case(mkv, dev, 2, 2, 8, 64 * 6 + 29, seed=150)
+    d = Case(mkv, dev, 2, 2, 8, 64 * 6 + 29, seed=151)
+    try:
+        rng = np.random.default_rng(5)
+        c.K[0, 0, 64:128] = synth.f32_to_bf16_bits(rng.integers(-2, 3, (64, 128)).astype(np.float32))   # ties, zeros
+        c.V[1, 1, 0:64] = 0
+        c.k_d, c.v_d = to_dev(c.K, dev), to_dev(c.V, dev)
+        strat = uniform_strat(2, 2, c.S, 38, 50)
+        strat[:, :, 2::3, 0:2] = (64, 38)
+        strat[:, :, 4, 0:2] = 128
+        # (a) fresh masks of the same data: K rate 38 matches most segments, V rate 50 too
+        lk, lv = c.gpu_loss(38, 50)
+        for b in range(2):
+            for h in range(2):
+                rk_, rv_ = orc.segment_loss(c.K[b, h], c.V[b, h], 64, 38, 50, 1)
+                np.testing.assert_allclose(lk[b, h], rk_, rtol=1e-12, atol=0)
+        c.compress(strat)
+        c.assert_export_equal()
+        # (b) the scratch now describes c's data; compress d's data (other values, same shape) through the same cache
+        c.cache.reset(0)
+        c.K, c.V, c.k_d, c.v_d = d.K, d.V, d.k_d, d.v_d
+        c.compress(strat)
+        c.assert_export_equal()
+        # masks of another rate, and of the first segments only
+        c.cache.reset(0)
+        c.gpu_loss(64, 64)
+        lk = torch.zeros((2, 2, 2), dtype=torch.float64, device=dev)
+        c.cache.segment_loss(c.k_d[:, :, :128], c.v_d[:, :, :128], (38, 50, 1, 8), lk, lk.clone())
+        c.compress(strat)
+        c.assert_export_equal()
+    finally:
+        c.free()
+        d.free()
+
+
 @pytest.mark.parametrize("B,L,g", [(4, 64, 1), (16, 64, 1), (16, 32, 2), (4, 32, 4), (16, 64, 4)])
 def test_token_block_sizes_end_to_end(env, B, L, g):
     """SURVEY 8(f) NEXT-2 ("block size (e.g., 4, 8, and 16)"): a cache whose token blocks hold 4 or 16
