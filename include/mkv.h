@@ -209,10 +209,23 @@ MKV_API int mkv_rotate_query(const mkv_cache* cache, int32_t layer, const void* 
 MKV_API int mkv_rotate_output(const mkv_cache* cache, int32_t layer, float* out, void* stream);
 
 /*
+ * One decode step of a layer on DEVICE buffers (steps 2 and 3 as one chain): [query fold] ->
+ * block scores -> top-k -> PackedAttention -> [output fold], enqueued back to back on `stream` with programmatic
+ * dependent launch, so each kernel's prologue overlaps its predecessor's tail and the chain captures into one CUDA
+ * graph.  q: bf16 [batch][n_q_heads][D]; out: float [batch][n_q_heads][D]; lse_opt: float [batch][n_q_heads] or NULL.
+ * sel_opt / sel_count_opt (both or neither): int32 [batch][n_kv_heads][k_max] / [batch][n_kv_heads] receive the
+ * selection; with NULL the cache's own buffers are used and k_max is ignored.  A layer with an installed rotation
+ * (mkv_rotation_set) gets both folds.  Results are those of mkv_select followed by mkv_packed_attention, bit for bit.
+ */
+MKV_API int mkv_decode_step(mkv_cache* cache, int32_t layer, const void* q, int32_t token_budget, int32_t reduce,
+                    float softmax_scale, float* out, float* lse_opt, int32_t* sel_opt, int32_t* sel_count_opt,
+                    int32_t k_max, void* stream);
+
+/*
  * Steps 2+3 with HOST buffers (the end-to-end call): copies q_host (bf16 [batch][n_q_heads][D],
  * pinned for true async) to the device, runs select + attention, copies out_host (float
  * [batch][n_q_heads][D]) back.  Everything is enqueued on `stream`; the caller synchronises the
- * stream before reading out_host.  sel_host_opt [batch][n_kv_heads][token_budget/8 + 1] and
+ * stream before reading out_host.  sel_host_opt [batch][n_kv_heads][token_budget/B + 1] and
  * sel_count_host_opt [batch][n_kv_heads] may be NULL.
  */
 MKV_API int mkv_decode_host(mkv_cache* cache, int32_t layer, const void* q_host, int32_t token_budget,

@@ -24,7 +24,7 @@ MKV_DEV_ARENA_OVERFLOW, MKV_DEV_BAD_STRATEGY = 1, 2
 SYMBOLS = ["mkv_cache_create", "mkv_cache_free", "mkv_cache_reset", "mkv_segment_loss",
            "mkv_strategy_quantile", "mkv_strategy_threshold", "mkv_compress_segment", "mkv_select",
            "mkv_packed_attention", "mkv_update_append", "mkv_update_flush", "mkv_update_count", "mkv_calibrate_gather", "mkv_calibrate_stream",
-           "mkv_attention_stats", "mkv_rotation_set", "mkv_rotate_query", "mkv_rotate_output", "mkv_decode_host", "mkv_cache_export", "mkv_cache_bytes",
+           "mkv_attention_stats", "mkv_rotation_set", "mkv_rotate_query", "mkv_rotate_output", "mkv_decode_step", "mkv_decode_host", "mkv_cache_export", "mkv_cache_bytes",
            "mkv_cache_status", "mkv_last_launch_count", "mkv_last_error", "mkv_version"]
 
 
@@ -61,6 +61,7 @@ _lib.mkv_attention_stats.argtypes = [_vp, C.POINTER(_u64), C.POINTER(_u64), C.PO
 _lib.mkv_rotation_set.argtypes = [_vp, _i32, _vp, _vp, _vp]
 _lib.mkv_rotate_query.argtypes = [_vp, _i32, _vp, _vp, _vp]
 _lib.mkv_rotate_output.argtypes = [_vp, _i32, _vp, _vp]
+_lib.mkv_decode_step.argtypes = [_vp, _i32, _vp, _i32, _i32, C.c_float, _vp, _vp, _vp, _vp, _i32, _vp]
 _lib.mkv_decode_host.argtypes = [_vp, _i32, _vp, _i32, _i32, C.c_float, _vp, _vp, _vp, _vp]
 _lib.mkv_cache_export.argtypes = [_vp, _i32, _i32, _i32, _vp, _u64, C.POINTER(_u64)]
 _lib.mkv_cache_bytes.argtypes = [_vp, _i32, C.POINTER(_u64), C.POINTER(_u64), C.POINTER(_u64)]
@@ -227,6 +228,13 @@ def mkv_rotate_output(cache, layer, out, stream=None):
     _check(_lib.mkv_rotate_output(cache, layer, _ptr(out), _stream(stream)))
 
 
+def mkv_decode_step(cache, layer, q, token_budget, softmax_scale, out, reduce=0, lse=None, sel=None, sel_count=None,
+                    stream=None):
+    k_max = int(sel.shape[-1]) if sel is not None else 0
+    _check(_lib.mkv_decode_step(cache, layer, _ptr(q), token_budget, reduce, float(softmax_scale), _ptr(out),
+                                _ptr(lse), _ptr(sel), _ptr(sel_count), k_max, _stream(stream)))
+
+
 def mkv_decode_host(cache, layer, q_host, token_budget, softmax_scale, out_host, reduce=0,
                     sel_host=None, sel_count_host=None, stream=None):
     _check(_lib.mkv_decode_host(cache, layer, _ptr(q_host), token_budget, reduce, float(softmax_scale),
@@ -346,6 +354,10 @@ class Cache:
 
     def rotate_output(self, layer, out, stream=None):
         mkv_rotate_output(self.h, layer, out, stream)
+
+    def decode_step(self, layer, q, token_budget, softmax_scale, out, reduce=0, lse=None, sel=None, sel_count=None,
+                    stream=None):
+        mkv_decode_step(self.h, layer, q, token_budget, softmax_scale, out, reduce, lse, sel, sel_count, stream)
 
     def decode_host(self, layer, q_host, token_budget, softmax_scale, out_host, reduce=0,
                     sel_host=None, sel_count_host=None, stream=None):

@@ -483,6 +483,33 @@ int mkv_update_count(const mkv_cache* c, int32_t layer, int32_t* n_host) {
     return MKV_OK;
 }
 
+int mkv_decode_step(mkv_cache* c, int32_t layer, const void* q, int32_t budget, int32_t reduce, float scale, float* out,
+                    float* lse_opt, int32_t* sel_opt, int32_t* sel_count_opt, int32_t k_max, void* stream) {
+    if (!c || !q || !out) return fail(MKV_E_ARG, "mkv_decode_step: NULL argument");
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    if ((sel_opt == nullptr) != (sel_count_opt == nullptr)) return fail(MKV_E_ARG, "mkv_decode_step: sel and sel_count go together");
+    cudaStream_t s = (cudaStream_t)stream;
+    int32_t* sel = sel_opt ? sel_opt : c->sel_dev;
+    int32_t* cnt = sel_opt ? sel_count_opt : c->selcnt_dev;
+    if (!sel_opt) {
+        long long km = (long long)budget / g.B + 1;
+        k_max = (int32_t)(km > c->sel_cap ? c->sel_cap : km);
+    }
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    const uint16_t* qd = (const uint16_t*)q;
+    if (c->rot_set[layer]) {  // rotation fold: the cache holds K R_k^T, V R_v^T; attend with q R_k^T
+        MKV_CUDA(launch_rotate_query(g, qd, c->rot_k + (size_t)layer * g.n_kv_heads * kD * kD, c->q_rot, s));
+        qd = c->q_rot;
+    }
+    int rc = mkv_select(c, layer, qd, budget, reduce, sel, cnt, k_max, nullptr, stream);
+    if (rc) return rc;
+    rc = mkv_packed_attention(c, layer, qd, sel, cnt, k_max, scale, out, lse_opt, stream);
+    if (rc) return rc;
+    if (c->rot_set[layer]) MKV_CUDA(launch_rotate_output(g, out, c->rot_v + (size_t)layer * g.n_kv_heads * kD * kD, s));
+    return MKV_OK;
+}
+
 int mkv_decode_host(mkv_cache* c, int32_t layer, const void* q_host, int32_t budget, int32_t reduce, float scale,
                     float* out_host, int32_t* sel_host_opt, int32_t* sel_count_host_opt, void* stream) {
     if (!c || !q_host || !out_host) return fail(MKV_E_ARG, "mkv_decode_host: NULL argument");
@@ -490,19 +517,11 @@ int mkv_decode_host(mkv_cache* c, int32_t layer, const void* q_host, int32_t bud
     cudaStream_t s = (cudaStream_t)stream;
     long long k_max = (long long)budget / g.B + 1;
     if (k_max > c->sel_cap) k_max = c->sel_cap;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
     MKV_CUDA(cudaSetDevice(c->desc.device));
     MKV_CUDA(cudaMemcpyAsync(c->q_dev, q_host, (size_t)g.batch * g.n_q_heads * kD * 2, cudaMemcpyHostToDevice, s));
-    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
-    const uint16_t* qd = c->q_dev;
-    if (c->rot_set[layer]) {  // rotation fold: the cache holds K R_k^T, V R_v^T; attend with q R_k^T
-        MKV_CUDA(launch_rotate_query(g, c->q_dev, c->rot_k + (size_t)layer * g.n_kv_heads * kD * kD, c->q_rot, s));
-        qd = c->q_rot;
-    }
-    int rc = mkv_select(c, layer, qd, budget, reduce, c->sel_dev, c->selcnt_dev, (int)k_max, nullptr, stream);
+    const int rc = mkv_decode_step(c, layer, c->q_dev, budget, reduce, scale, c->out_dev, nullptr, nullptr, nullptr, 0, stream);
     if (rc) return rc;
-    rc = mkv_packed_attention(c, layer, qd, c->sel_dev, c->selcnt_dev, (int)k_max, scale, c->out_dev, nullptr, stream);
-    if (rc) return rc;
-    if (c->rot_set[layer]) MKV_CUDA(launch_rotate_output(g, c->out_dev, c->rot_v + (size_t)layer * g.n_kv_heads * kD * kD, s));
     MKV_CUDA(cudaMemcpyAsync(out_host, c->out_dev, (size_t)g.batch * g.n_q_heads * kD * 4, cudaMemcpyDeviceToHost, s));
     if (sel_host_opt)
         MKV_CUDA(cudaMemcpyAsync(sel_host_opt, c->sel_dev, (size_t)g.n_units * k_max * 4, cudaMemcpyDeviceToHost, s));

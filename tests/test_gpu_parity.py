@@ -770,6 +770,67 @@ def test_element_groups_end_to_end(env, g, r_k, r_v):
         c.free()
 
 
+def test_decode_step_equals_select_then_attention(env):
+    """mkv_decode_step = [query fold] -> scores -> top-k -> PackedAttention -> [output fold] as one
+    chain on device buffers.  Bit for bit the results of the separate calls; captured into a CUDA graph and replayed it
+    gives them again; with a rotation installed it applies both folds."""
+    mkv, dev = env
+    import torch
+    c = Case(mkv, dev, 2, 2, 8, 64 * 20 + 5, seed=160)
+    try:
+        strat = uniform_strat(2, 2, c.S, 38)
+        strat[:, :, ::5, 0:2] = 128
+        c.compress(strat)
+        c.cache.update_append(0, c.k_d[:, :, :9], c.v_d[:, :, :9])
+        budget, scale = 256, 1 / math.sqrt(128)
+        k_max = budget // 8 + 1
+        sel = torch.full((2, 2, k_max), -5, dtype=torch.int32, device=dev)
+        cnt = torch.full((2, 2), -5, dtype=torch.int32, device=dev)
+        out = torch.full((2, 8, 128), float("nan"), dtype=torch.float32, device=dev)
+        lse = torch.full((2, 8), float("nan"), dtype=torch.float32, device=dev)
+        c.cache.select(0, c.q_d, budget, sel, cnt)
+        c.cache.packed_attention(0, c.q_d, sel, cnt, scale, out, lse)
+        sel2, cnt2, out2, lse2 = torch.full_like(sel, -9), torch.full_like(cnt, -9), torch.zeros_like(out), torch.zeros_like(lse)
+        c.cache.decode_step(0, c.q_d, budget, scale, out2, lse=lse2, sel=sel2, sel_count=cnt2)
+        torch.cuda.synchronize()
+        assert torch.equal(sel, sel2) and torch.equal(cnt, cnt2) and torch.equal(out, out2) and torch.equal(lse, lse2)
+        out3 = torch.zeros_like(out)
+        c.cache.decode_step(0, c.q_d, budget, scale, out3)     # the cache's own selection buffers
+        torch.cuda.synchronize()
+        assert torch.equal(out, out3)
+        # one graph launch per step
+        st = torch.cuda.Stream()
+        out4 = torch.zeros_like(out)
+        with torch.cuda.stream(st):
+            c.cache.decode_step(0, c.q_d, budget, scale, out4, stream=st)   # warm-up outside the capture
+            st.synchronize()
+            gr = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gr, stream=st):
+                c.cache.decode_step(0, c.q_d, budget, scale, out4, stream=st)
+            out4.zero_()
+            gr.replay()
+            st.synchronize()
+        assert torch.equal(out, out4)
+        # with a rotation: both folds, equal to the three calls made by hand
+        rng = np.random.default_rng(9)
+        R = np.stack([np.linalg.qr(rng.standard_normal((128, 128)))[0] for _ in range(2)]).astype(np.float32)
+        Rd = torch.from_numpy(R).to(dev)
+        c.cache.rotation_set(0, Rd, Rd)
+        qr = torch.zeros_like(c.q_d)
+        c.cache.rotate_query(0, c.q_d, qr)
+        c.cache.select(0, qr, budget, sel, cnt)
+        c.cache.packed_attention(0, qr, sel, cnt, scale, out, lse)
+        c.cache.rotate_output(0, out)
+        c.cache.decode_step(0, c.q_d, budget, scale, out2, lse=lse2, sel=sel2, sel_count=cnt2)
+        torch.cuda.synchronize()
+        assert torch.equal(sel, sel2) and torch.equal(out, out2) and torch.equal(lse, lse2)
+        with pytest.raises(mkv.MkvError) as e:
+            c.cache.decode_step(0, c.q_d, budget, scale, out2, sel=sel2)    # sel without sel_count
+        assert e.value.code == mkv.MKV_E_ARG
+    finally:
+        c.free()
+
+
 def test_compress_after_loss_takes_only_valid_masks(env):
     """mkv_segment_loss leaves its top-r masks in a scratch of the cache and mkv_compress_segment takes a mask from there
     after checking it against the vector (r kept, every kept magnitude strictly above every dropped one).  Bit-exact blobs
