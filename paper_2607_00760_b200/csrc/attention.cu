@@ -208,8 +208,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 meta = (uint32_t)kD | ((uint32_t)kD << 8) | (nb << 16);
                 updf = 1u;
             } else {
-                const int ts = __ldg(sel + (size_t)u * k_max + j / ppb);
-                const int t0 = (ts < 0 || (ts & (g.B - 1))) ? -1 : ts + kPhys * (j % ppb);  // (j odd: second half of 16 tokens)
+                const int ts = __ldg(sel + (size_t)u * k_max + (j >> (ppb - 1)));  // ppb is 1 or 2
+                const int t0 = (ts < 0 || (ts & (g.B - 1))) ? -1 : ts + kPhys * (j & (ppb - 1));  // (j odd: second half of 16 tokens)
                 PlanRec pr;
                 pr.t0 = -1; pr.off16 = 0u; pr.meta = 0u; pr.tag = 0u;
                 if (scr.plan != nullptr && j < scr.plan_stride) {

@@ -440,20 +440,21 @@ __global__ void __launch_bounds__(256) mkv_segment_loss_kernel(CacheGeom g, Comp
 }
 
 // ------------------------------------------------------------------------------------------
-// strategy, quantile rule: one CTA per unit; a segment stays dense iff its rank by
-// (importance descending, index ascending) is below n_dense.  Rank by counting.
+// strategy, quantile rule: CTA (chunk, unit) ranks 256 segments of one unit; a segment stays dense iff its
+// rank by (importance descending, index ascending) is below n_dense.  Rank by counting against every
+// segment of the unit, 1024 at a time through shared memory (a long unit spreads over many CTAs).
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) mkv_strategy_quantile_kernel(const double* __restrict__ loss_k,
                                                                     const double* __restrict__ loss_v,
                                                                     int nseg, int n_dense, mkv_strategy sparse,
                                                                     mkv_strategy* __restrict__ out) {
-    const int u = blockIdx.x;
+    const int u = blockIdx.y;
     const double* lk = loss_k + (size_t)u * nseg;
     const double* lvv = loss_v + (size_t)u * nseg;
     constexpr int kTile = 1024;
     __shared__ double s_I[kTile];
-    for (int i0 = 0; i0 < nseg; i0 += 256) {
-        const int i = i0 + threadIdx.x;
+    {
+        const int i = blockIdx.x * 256 + threadIdx.x;
         const double mine = (i < nseg) ? 0.5 * (lk[i] + lvv[i]) : 0.;
         int rank = 0;
         for (int j0 = 0; j0 < nseg; j0 += kTile) {
@@ -533,7 +534,8 @@ cudaError_t launch_segment_loss(const CacheGeom& g, const CompressArgs& a, mkv_s
 
 cudaError_t launch_strategy_quantile(const double* loss_k, const double* loss_v, int n_units, int nseg,
                                      int n_dense, mkv_strategy sparse, mkv_strategy* out, cudaStream_t s) {
-    mkv_strategy_quantile_kernel<<<n_units, 256, 0, s>>>(loss_k, loss_v, nseg, n_dense, sparse, out);
+    if (n_units > 65535) return cudaErrorInvalidValue;
+    mkv_strategy_quantile_kernel<<<dim3((nseg + 255) / 256, n_units), 256, 0, s>>>(loss_k, loss_v, nseg, n_dense, sparse, out);
     return cudaGetLastError();
 }
 

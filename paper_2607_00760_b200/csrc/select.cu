@@ -269,7 +269,7 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
         // (a block of 16 tokens is two device blocks: two records, at 2 p and 2 p + 1)
         for (int p = tid; p < count * g.ppb && p < plan_stride; p += 1024) {
             PlanRec pr;
-            pr.t0 = out[p / g.ppb] + kPhys * (p % g.ppb); pr.tag = tag;
+            pr.t0 = out[p >> (g.ppb - 1)] + kPhys * (p & (g.ppb - 1)); pr.tag = tag;  // ppb is 1 or 2
             plan_lookup(g, lv, unit, pr.t0, pr.off16, pr.meta);
             plan[(size_t)unit * plan_stride + p] = pr;
         }
