@@ -119,6 +119,62 @@ struct Split {
     __device__ __forceinline__ unsigned begin(unsigned i) const { return i * b + min(i, r); }
 };
 
+// PV of one group in flight: O^T += V^T P^T with channels = M, heads = N, the group's <= 16 tokens = K.  vb0 / vb1: the
+// V parts of its blocks in shared memory; ph / pl: probabilities of head gq, tokens 2qq, 2qq+1 of each block, split into
+// bf16 hi + lo (exactly the B fragments: k = token, n = head).  Dense vectors (r = D) skip the walk.
+__device__ __forceinline__ void pv_group(float (&acc)[8][4], int r_v, int nb0, int nb1, uint32_t vb0, uint32_t vb1,
+                                         uint32_t ph0, uint32_t ph1, uint32_t pl0, uint32_t pl1, int gq, int qq) {
+    const bool two = nb1 != 0;
+    const bool full = nb0 == kPhys && (!two || nb1 == kPhys);
+    if (r_v == kD && full) {
+        const uint32_t rA0 = vb0 + 256 * (2 * qq) + 32 * gq, rA1 = vb1 + 256 * (2 * qq) + 32 * gq;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {  // 16-byte chunk h = channel slots 8h .. 8h+7 = tiles 4h .. 4h+3
+            const uint4 xa = lds_128(rA0 + 16 * h), xb = lds_128(rA0 + 256 + 16 * h);
+            uint4 ya = make_uint4(0u, 0u, 0u, 0u), yb = ya;
+            if (two) { ya = lds_128(rA1 + 16 * h); yb = lds_128(rA1 + 256 + 16 * h); }
+            const uint32_t xav[4] = {xa.x, xa.y, xa.z, xa.w}, xbv[4] = {xb.x, xb.y, xb.z, xb.w};
+            const uint32_t yav[4] = {ya.x, ya.y, ya.z, ya.w}, ybv[4] = {yb.x, yb.y, yb.z, yb.w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t a0 = prmt(xav[j], xbv[j], 0x5410u), a1 = prmt(xav[j], xbv[j], 0x7632u);
+                const uint32_t a2 = prmt(yav[j], ybv[j], 0x5410u), a3 = prmt(yav[j], ybv[j], 0x7632u);
+                mma_bf16(acc[4 * h + j], a0, a1, a2, a3, ph0, ph1);
+                mma_bf16(acc[4 * h + j], a0, a1, a2, a3, pl0, pl1);
+            }
+        }
+    } else {
+        const int tA = 2 * qq, tB = 2 * qq + 1;
+        uint32_t hA0 = 0u, hB0 = 0u, hA1 = 0u, hB1 = 0u, pA0, pB0, pA1, pB1, st0 = 2u, st1 = 2u;
+        if (r_v == kD) {  // ragged dense block
+            hA0 = tA < nb0 ? 0xffffu : 0u; hB0 = tB < nb0 ? 0xffffu : 0u;
+            hA1 = tA < nb1 ? 0xffffu : 0u; hB1 = tB < nb1 ? 0xffffu : 0u;
+            pA0 = vb0 + 256 * tA + 32 * gq; pB0 = pA0 + 256;
+            pA1 = vb1 + 256 * tA + 32 * gq; pB1 = pA1 + 256;
+        } else {
+            if (tA < nb0) hA0 = lds_u16(vb0 + 16 * tA + 2 * gq);
+            if (tB < nb0) hB0 = lds_u16(vb0 + 16 * tB + 2 * gq);
+            if (tA < nb1) hA1 = lds_u16(vb1 + 16 * tA + 2 * gq);
+            if (tB < nb1) hB1 = lds_u16(vb1 + 16 * tB + 2 * gq);
+            // exclusive prefix over the lower half-words (lanes gq' < gq, stride 4); four byte counters
+            const uint32_t cnt = (uint32_t)__popc(hA0) | ((uint32_t)__popc(hB0) << 8) |
+                                 ((uint32_t)__popc(hA1) << 16) | ((uint32_t)__popc(hB1) << 24);
+            uint32_t inc = cnt, t;
+            t = __shfl_up_sync(kFull, inc, 4); if (gq >= 1) inc += t;
+            t = __shfl_up_sync(kFull, inc, 8); if (gq >= 2) inc += t;
+            t = __shfl_up_sync(kFull, inc, 16); if (gq >= 4) inc += t;
+            const uint32_t ex = inc - cnt;
+            st0 = 2u * nb0; st1 = 2u * nb1;
+            pA0 = vb0 + 16 * nb0 + st0 * (ex & 255u) + 2 * tA;
+            pB0 = vb0 + 16 * nb0 + st0 * ((ex >> 8) & 255u) + 2 * tB;
+            pA1 = vb1 + 16 * nb1 + st1 * ((ex >> 16) & 255u) + 2 * tA;
+            pB1 = vb1 + 16 * nb1 + st1 * (ex >> 24) + 2 * tB;
+        }
+        v_walk_mma<0>(acc, hA0, hB0, hA1, hB1, pA0, pB0, pA1, pB1, st0, st1, ph0, ph1, pl0, pl1);
+        v_walk_mma<1>(acc, hA0, hB0, hA1, hB1, pA0, pB0, pA1, pB1, st0, st1, ph0, ph1, pl0, pl1);
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // grid = n_units clusters of C CTAs; cluster u attends unit u.
 // kGatherOnly: calibration build of the same kernel (mkv_calibrate_gather): every K part and every
@@ -143,6 +199,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     __shared__ float s_cta_l[kMaxGroup];                  // the CTA's partial sums (its partial O: s_cta_o)
     __shared__ float s_M[kMaxGroup];                      // the unit's per-head maxima after the exchange
     __shared__ unsigned s_active;                         // warps of the CTA that hold a partial result
+    __shared__ uint32_t s_q[kWarps][kDesc];               // phase 2: the groups of each warp's range that matter ...
+    __shared__ int s_qn[kWarps];                          // ... and how many
     float* s_cta_o = reinterpret_cast<float*>(smem + kWarps * kWS);  // [G][128] floats behind the warps' regions
 
     uint8_t* wbase = smem + warp * kWS;
@@ -286,6 +344,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     // Phase 1: QK.  Logits (log2 domain, scaled) -> logit cache; per-head maxima -> the CTA's table.
     // =====================================================================================
     float mxA = -INFINITY, mxB = -INFINITY;  // this lane's maxima for heads 2qq, 2qq+1
+    uint32_t twomask = 0u;                   // bit i: group i of the range holds two blocks (short ranges: phase 2 deals them out)
     uint32_t calib = 0u;
     // this lane's slots inside a block's logits ([head][token] floats): phase 1 writes token gq of heads 2qq, 2qq+1;
     // phase 2 reads tokens 2qq, 2qq+1 of head gq
@@ -324,6 +383,9 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 ring_commit();
                 ++gposi;
                 bposi += c1 ? 2 : 1;
+                // two groups are in flight and the oldest has landed: walk it now, issue the rest between the walks (at
+                // the start of the kernel every warp of the SM is issuing and nothing else hides the cost of it)
+                if (pend >= 2 && mbar_test(bar0 + 8 * sc, (parbits >> sc) & 1u)) break;
             }
             if (pend == 0) break;  // nothing in flight and nothing left to issue
 
@@ -413,6 +475,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             }
             __syncwarp();  // every lane is done reading the slot
             ring_release();
+            if (two && gposc < 32) twomask |= 1u << gposc;
             ++gposc;
             bposc += two ? 2 : 1;
         }
@@ -468,7 +531,117 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         return __ldcg(reinterpret_cast<const float2*>(zglob + (size_t)i * (size_t)(8 * G) + (zr >> 2)));
     };
 
-    if (n_total > 0 && active) {
+    // Short ranges (every range of the cluster fits its descriptor ring and its logit cache): phase 2 is a handful of
+    // blocks, and which warps hold them is an accident of the data.  Every warp lists the groups of its range that matter
+    // (and adds up its softmax sums); the lists are then dealt out over all warps of the CTA, so no warp walks more than
+    // ceil(groups that matter / warps) of them.  The order is a function of the data only: results are reproducible.
+    const bool redist = !kGatherOnly && 2 * ((int)ws.b + 1) <= min(kDesc, zcap);
+    bool walked = false;  // this warp holds a partial O
+    if (redist) {
+        int qn = 0;
+        if (n_total > 0 && active) {
+            // softmax sums and "this block matters" flags of the range's blocks, four blocks at a time (independent loads,
+            // exponentials and votes); then one entry per group with a block that matters
+            uint32_t needmask = 0u;
+#pragma unroll 1
+            for (int b0 = 0; b0 < n_total; b0 += 4) {
+                float2 z[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    z[j] = make_float2(-INFINITY, -INFINITY);
+                    if (gq < G && b0 + j < n_total) z[j] = lds_f32x2(zs0 + (uint32_t)(b0 + j) * zstride + zr);
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    lsum += ex2(z[j].x - Mh) + ex2(z[j].y - Mh);
+                    if (__any_sync(kFull, fmaxf(z[j].x, z[j].y) - Mh >= -kSkip)) needmask |= 1u << (b0 + j);
+                }
+            }
+            int bpos = 0;
+#pragma unroll 1
+            for (int gi = 0; gi < gbuilt; ++gi) {
+                const bool two = (twomask >> gi) & 1u;
+                const uint32_t nd = (needmask >> bpos) & (two ? 3u : 1u);
+                if (nd != 0u) {
+                    if (lane == 0) s_q[warp][qn] = (uint32_t)gi | (nd << 8) | ((uint32_t)bpos << 10);
+                    ++qn;
+                }
+                bpos += two ? 2 : 1;
+            }
+        }
+        if (lane == 0) s_qn[warp] = qn;
+        __syncthreads();
+        // inclusive prefix of the warps' counts (lane w: warps 0..w)
+        int incl = lane < kWarps ? s_qn[lane] : 0;
+#pragma unroll
+        for (int o = 1; o < kWarps; o <<= 1) {
+            const int t = __shfl_up_sync(kFull, incl, o);
+            if (lane >= o) incl += t;
+        }
+        const int Q = __shfl_sync(kFull, incl, kWarps - 1);
+        int e = warp;  // this warp walks entries warp, warp + kWarps, ...
+#pragma unroll 1
+        for (;;) {
+            // ---- start the V copies of this warp's next entries while the ring has room
+#pragma unroll 1
+            while (e < Q) {
+                const int owner = __popc(__ballot_sync(kFull, lane < kWarps && incl <= e));
+                const int excl = owner == 0 ? 0 : __shfl_sync(kFull, incl, owner - 1);
+                const uint32_t ent = s_q[owner][e - excl];
+                const GDesc d = *reinterpret_cast<const GDesc*>(smem + owner * kWS + kOffD2 + 16 * (int)(ent & 255u));
+                uint32_t nb0 = (d.y >> 4) & 15u, nb1 = (d.y >> 8) & 15u;
+                const bool need0 = (ent >> 8) & 1u, need1 = (ent >> 9) & 1u;
+                // a group with one block that matters becomes a one-block group
+                uint32_t off0 = d.off0, off1 = d.off1, c0 = (d.x & 255u) << 4, c1 = ((d.x >> 8) & 255u) << 4;
+                uint32_t sk0 = (d.x >> 16) & 15u, sk1 = (d.x >> 20) & 15u, shift = 0u;
+                if (!need0) { off0 = off1; c0 = c1; sk0 = sk1; nb0 = nb1; nb1 = 0u; c1 = 0u; shift = 1u; }
+                else if (!need1) { nb1 = 0u; c1 = 0u; }
+                uint32_t off;
+                if (!ring_alloc(c0 + c1, off)) break;
+                if (lane == 0) {
+                    const uint32_t bar = bar0 + 8 * si, dst = ring0 + off;
+                    const unsigned long long src = (d.y & 1u) ? reinterpret_cast<unsigned long long>(upd_v) : slice;
+                    mbar_expect_tx(bar, c0 + c1);
+                    bulk_g2s(dst, src + ((unsigned long long)off0 << 4), c0, bar);
+                    if (c1) bulk_g2s(dst + c0, src + ((unsigned long long)off1 << 4), c1, bar);
+                    GDesc g2;
+                    g2.off0 = sk0 | (sk1 << 4) | (c0 << 8);                  // skews of the V parts, bytes of the first chunk
+                    g2.off1 = (ent >> 10) + shift;                           // index of the first WALKED block in the owner's range
+                    g2.x = d.x;
+                    g2.y = nb0 | (nb1 << 4) | ((uint32_t)owner << 8);
+                    slot_grp[si] = g2;
+                }
+                st_vblocks += nb1 ? 2u : 1u;
+                st_vbytes += c0 + c1;
+                ring_commit();
+                e += kWarps;
+            }
+            if (pend == 0) break;
+            // ---- consume the oldest group in flight: PV with the owner's logits
+            const GDesc d = slot_grp[sc];
+            const int r_v = (int)(d.x >> 24);
+            const int nb0 = (int)(d.y & 15u), nb1 = (int)((d.y >> 4) & 15u), pos = (int)d.off1;
+            const bool two = nb1 != 0;
+            const uint32_t vb0 = ring0 + slot_tab[sc].x + (d.off0 & 15u);
+            const uint32_t vb1 = ring0 + slot_tab[sc].x + (d.off0 >> 8) + ((d.off0 >> 4) & 15u);
+            const uint32_t zo = smem_u32(smem + (d.y >> 8) * kWS) + kOffZ + zr;
+            float2 za = make_float2(-INFINITY, -INFINITY), zb = za;
+            if (gq < G) {
+                za = lds_f32x2(zo + (uint32_t)pos * zstride);
+                if (two) zb = lds_f32x2(zo + (uint32_t)(pos + 1) * zstride);
+            }
+            const float e00 = ex2(za.x - Mh), e01 = ex2(za.y - Mh), e10 = ex2(zb.x - Mh), e11 = ex2(zb.y - Mh);
+            const uint32_t ph0 = pack_bf16(e00, e01), ph1 = pack_bf16(e10, e11);
+            const uint32_t pl0 = pack_bf16(e00 - __uint_as_float(ph0 << 16), e01 - __uint_as_float(ph0 & 0xffff0000u));
+            const uint32_t pl1 = pack_bf16(e10 - __uint_as_float(ph1 << 16), e11 - __uint_as_float(ph1 & 0xffff0000u));
+            mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);  // the group's V parts have landed
+            pv_group(acc, r_v, nb0, nb1, vb0, vb1, ph0, ph1, pl0, pl1, gq, qq);
+            walked = true;
+            __syncwarp();  // every lane is done reading the slot
+            ring_release();
+        }
+    } else if (n_total > 0 && active) {
+        walked = true;
         // the range's descriptors are still in shared memory unless it was longer than one ring: then describe again
         const bool redo = gbuilt > kDesc;
         if (redo) { bbuilt = 0; gbuilt = 0; }
@@ -553,57 +726,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             const uint32_t ph0 = pack_bf16(e00, e01), ph1 = pack_bf16(e10, e11);
             const uint32_t pl0 = pack_bf16(e00 - __uint_as_float(ph0 << 16), e01 - __uint_as_float(ph0 & 0xffff0000u));
             const uint32_t pl1 = pack_bf16(e10 - __uint_as_float(ph1 << 16), e11 - __uint_as_float(ph1 & 0xffff0000u));
-            const bool full = nb0 == kPhys && (!two || nb1 == kPhys);
-
             mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);  // the group's V parts have landed
-
-            if (r_v == kD && full) {
-                const uint32_t rA0 = vb0 + 256 * (2 * qq) + 32 * gq, rA1 = vb1 + 256 * (2 * qq) + 32 * gq;
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {  // 16-byte chunk h = channel slots 8h .. 8h+7 = tiles 4h .. 4h+3
-                    const uint4 xa = lds_128(rA0 + 16 * h), xb = lds_128(rA0 + 256 + 16 * h);
-                    uint4 ya = make_uint4(0u, 0u, 0u, 0u), yb = ya;
-                    if (two) { ya = lds_128(rA1 + 16 * h); yb = lds_128(rA1 + 256 + 16 * h); }
-                    const uint32_t xav[4] = {xa.x, xa.y, xa.z, xa.w}, xbv[4] = {xb.x, xb.y, xb.z, xb.w};
-                    const uint32_t yav[4] = {ya.x, ya.y, ya.z, ya.w}, ybv[4] = {yb.x, yb.y, yb.z, yb.w};
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        const uint32_t a0 = prmt(xav[j], xbv[j], 0x5410u), a1 = prmt(xav[j], xbv[j], 0x7632u);
-                        const uint32_t a2 = prmt(yav[j], ybv[j], 0x5410u), a3 = prmt(yav[j], ybv[j], 0x7632u);
-                        mma_bf16(acc[4 * h + j], a0, a1, a2, a3, ph0, ph1);
-                        mma_bf16(acc[4 * h + j], a0, a1, a2, a3, pl0, pl1);
-                    }
-                }
-            } else {
-                const int tA = 2 * qq, tB = 2 * qq + 1;
-                uint32_t hA0 = 0u, hB0 = 0u, hA1 = 0u, hB1 = 0u, pA0, pB0, pA1, pB1, st0 = 2u, st1 = 2u;
-                if (r_v == kD) {  // ragged dense block
-                    hA0 = tA < nb0 ? 0xffffu : 0u; hB0 = tB < nb0 ? 0xffffu : 0u;
-                    hA1 = tA < nb1 ? 0xffffu : 0u; hB1 = tB < nb1 ? 0xffffu : 0u;
-                    pA0 = vb0 + 256 * tA + 32 * gq; pB0 = pA0 + 256;
-                    pA1 = vb1 + 256 * tA + 32 * gq; pB1 = pA1 + 256;
-                } else {
-                    if (tA < nb0) hA0 = lds_u16(vb0 + 16 * tA + 2 * gq);
-                    if (tB < nb0) hB0 = lds_u16(vb0 + 16 * tB + 2 * gq);
-                    if (tA < nb1) hA1 = lds_u16(vb1 + 16 * tA + 2 * gq);
-                    if (tB < nb1) hB1 = lds_u16(vb1 + 16 * tB + 2 * gq);
-                    // exclusive prefix over the lower half-words (lanes gq' < gq, stride 4); four byte counters
-                    const uint32_t cnt = (uint32_t)__popc(hA0) | ((uint32_t)__popc(hB0) << 8) |
-                                         ((uint32_t)__popc(hA1) << 16) | ((uint32_t)__popc(hB1) << 24);
-                    uint32_t inc = cnt, t;
-                    t = __shfl_up_sync(kFull, inc, 4); if (gq >= 1) inc += t;
-                    t = __shfl_up_sync(kFull, inc, 8); if (gq >= 2) inc += t;
-                    t = __shfl_up_sync(kFull, inc, 16); if (gq >= 4) inc += t;
-                    const uint32_t ex = inc - cnt;
-                    st0 = 2u * nb0; st1 = 2u * nb1;
-                    pA0 = vb0 + 16 * nb0 + st0 * (ex & 255u) + 2 * tA;
-                    pB0 = vb0 + 16 * nb0 + st0 * ((ex >> 8) & 255u) + 2 * tB;
-                    pA1 = vb1 + 16 * nb1 + st1 * ((ex >> 16) & 255u) + 2 * tA;
-                    pB1 = vb1 + 16 * nb1 + st1 * (ex >> 24) + 2 * tB;
-                }
-                v_walk_mma<0>(acc, hA0, hB0, hA1, hB1, pA0, pB0, pA1, pB1, st0, st1, ph0, ph1, pl0, pl1);
-                v_walk_mma<1>(acc, hA0, hB0, hA1, hB1, pA0, pB0, pA1, pB1, st0, st1, ph0, ph1, pl0, pl1);
-            }
+            pv_group(acc, r_v, nb0, nb1, vb0, vb1, ph0, ph1, pl0, pl1, gq, qq);
             __syncwarp();  // every lane is done reading the slot
             ring_release();
         }
@@ -623,12 +747,12 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     // split-K rule of oracle pin P10 with equal references), always in the same order: warps inside the CTA, then
     // the cluster's CTAs.
     // =====================================================================================
-    if (n_total > 0 && active) {
-        // the warp's partial: O^T fragments -> [head][channel] floats in the warp's (now idle) ring; sums -> s_l
+    lsum += __shfl_xor_sync(kFull, lsum, 1);
+    lsum += __shfl_xor_sync(kFull, lsum, 2);  // lanes (gq, *): the warp's sum of head gq (0 if it added nothing)
+    if (qq == 0 && gq < G) s_l[warp][gq] = lsum;
+    if (walked) {
+        // the warp's partial: O^T fragments -> [head][channel] floats in the warp's (now idle) ring
         if (lane == 0) atomicOr(&s_active, 1u << warp);
-        lsum += __shfl_xor_sync(kFull, lsum, 1);
-        lsum += __shfl_xor_sync(kFull, lsum, 2);  // lanes (gq, *): the warp's sum of head gq
-        if (qq == 0 && gq < G) s_l[warp][gq] = lsum;
         float* po = reinterpret_cast<float*>(wbase);
         const int hA = 2 * qq, hB = 2 * qq + 1;
 #pragma unroll
@@ -643,17 +767,14 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     const unsigned wmask = s_active;  // (in warp order: the sums are reproducible)
     for (int e = threadIdx.x; e < GD; e += kNT) {  // the CTA's partial
         float o = 0.f;
-#pragma unroll
-        for (int w = 0; w < kWarps; ++w) {
-            const float v = *reinterpret_cast<const float*>(smem + w * kWS + 4 * e);  // (stale bits where the warp left no partial)
-            if ((wmask >> w) & 1u) o += v;
-        }
+#pragma unroll 1
+        for (unsigned m = wmask; m; m &= m - 1u) o += *reinterpret_cast<const float*>(smem + (__ffs(m) - 1) * kWS + 4 * e);
         s_cta_o[e] = o;
     }
     if (threadIdx.x < G) {
         float l = 0.f;
 #pragma unroll 1
-        for (unsigned m = wmask; m; m &= m - 1u) l += s_l[__ffs(m) - 1][threadIdx.x];
+        for (int w = 0; w < kWarps; ++w) l += s_l[w][threadIdx.x];
         s_cta_l[threadIdx.x] = l;
     }
     cluster_sync();  // every CTA's partial is complete and visible to the cluster
