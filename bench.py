@@ -256,6 +256,25 @@ def run_mkv(args):
 
     ms_stream = timed_loop(torch, step_stream, args.steps, args.warmup, barrier, graph)
 
+    # calibration (iii): the QK expansion alone on groups of the real selection, resident in shared memory
+    def walk_us(reps):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        cache.calibrate_walk(0, built.q[0], sel[0], cnt[0], reps)
+        torch.cuda.synchronize()
+        ev0.record()
+        cache.calibrate_walk(0, built.q[0], sel[0], cnt[0], reps)
+        ev1.record()
+        torch.cuda.synchronize()
+        return ev0.elapsed_time(ev1) * 1e3
+
+    WALK_R1, WALK_R2, WALK_WARPS = 200, 1200, 16
+    us_walk_group = (walk_us(WALK_R2) - walk_us(WALK_R1)) / (WALK_R2 - WALK_R1) / WALK_WARPS  # one SM, one group of 16 tokens
+    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+    groups_attn = sum(n_sel_total) / n_layers / 2.0                 # K groups of one attention launch
+    c_attn = max([c for c in (16, 8, 4, 2, 1) if Bt * Hkv * c <= sm_count] or [1])  # CTAs per unit (attention.cu: pick_cluster)
+    sms_attn = min(sm_count, Bt * Hkv * c_attn)
+    groups_score = Bt * Hkv * math.ceil(N / 8) / 16.0                # groups of 16 block keys of one score launch
+
     # end to end through the public host call: pinned q in, out back, every layer, every step
     q_host = [q.cpu().pin_memory() for q in built.q]
     out_host = [torch.zeros((Bt, Hq, 128), dtype=torch.float32).pin_memory() for _ in range(n_layers)]
@@ -342,6 +361,13 @@ def run_mkv(args):
                         "stream_read_gbs": round(a_bytes / (ms_stream * 1e-3 / n_layers) / 1e9, 1),
                         "gather_only_us_per_layer": round(ms_gather * 1e3 / n_layers, 3),
                         "gather_only_gbs": round(a_bytes / (ms_gather * 1e-3 / n_layers) / 1e9, 1),
+                        "walk_only_ns_per_group_per_sm": round(us_walk_group * 1e3, 2),
+                        "walk_only_attention_qk_us_per_layer": round(us_walk_group * groups_attn / sms_attn, 3),
+                        "walk_only_score_us_per_layer": round(us_walk_group * groups_score / sm_count, 3),
+                        "what_walk": "mkv_calibrate_walk: every warp (16 per SM) runs the QK expansion of one group (two selected "
+                                     "token blocks, already in shared memory) over and over; ns per group per SM from the "
+                                     "difference of two repeat counts.  x groups per launch / SMs in use = the time the "
+                                     "shared-memory pipe alone needs for phase 1 of PackedAttention and for the score kernel",
                         "what": "stream_read: mkv_calibrate_stream, a plain 16-byte-load read of algorithmic_bytes_per_launch bytes of "
                                 "the layer's arena in the attention kernel's launch shape (148 x 512).  gather_only: "
                                 "mkv_calibrate_gather, the attention kernel's own staging of every selected K part then every V "

@@ -240,6 +240,12 @@ MKV_API int mkv_decode_host(mkv_cache* cache, int32_t layer, const void* q_host,
  *         ceiling the memory side sets for this access pattern.
  * stream: a plain streaming read of the first `bytes` bytes of the layer's packed arena (clamped to its size) in
  *         the same launch shape (one 512-thread CTA per SM, 16-byte loads): launch + pure-bandwidth floor.
+ * walk:   the expansion of packed keys into tensor-core fragments alone: every warp of a one-CTA-
+ *         per-SM grid copies the K parts of ONE group of the given selection (two consecutive selected token blocks)
+ *         into shared memory once and runs the QK step on it `reps` times.  No staging, softmax, PV or output.  The
+ *         difference of two calls with different `reps` is the time the shared-memory side needs per group: the
+ *         floor of phase 1 of mkv_packed_attention and of the score kernel of mkv_select.  q: device bf16
+ *         [batch][n_q_heads][128].
  * stats:  counters accumulated by mkv_packed_attention since the last reset: token blocks attended, token blocks
  *         whose V part was fetched (phase 2 skips a block whose probabilities are all < 2^-40 of the largest
  *         the CTA holds of the unit), bytes of those V copies.  Synchronises.
@@ -247,6 +253,8 @@ MKV_API int mkv_decode_host(mkv_cache* cache, int32_t layer, const void* q_host,
 MKV_API int mkv_calibrate_gather(const mkv_cache* cache, int32_t layer, const int32_t* sel,
                          const int32_t* sel_count, int32_t k_max, void* stream);
 MKV_API int mkv_calibrate_stream(const mkv_cache* cache, int32_t layer, uint64_t bytes, void* stream);
+MKV_API int mkv_calibrate_walk(const mkv_cache* cache, int32_t layer, const void* q, const int32_t* sel,
+                       const int32_t* sel_count, int32_t k_max, int32_t reps, void* stream);
 MKV_API int mkv_attention_stats(const mkv_cache* cache, uint64_t* blocks_host, uint64_t* v_blocks_host,
                         uint64_t* v_bytes_host, int32_t reset);
 

@@ -23,7 +23,7 @@ MKV_DEV_ARENA_OVERFLOW, MKV_DEV_BAD_STRATEGY = 1, 2
 # every symbol include/mkv.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ["mkv_cache_create", "mkv_cache_free", "mkv_cache_reset", "mkv_segment_loss",
            "mkv_strategy_quantile", "mkv_strategy_threshold", "mkv_compress_segment", "mkv_select",
-           "mkv_packed_attention", "mkv_update_append", "mkv_update_flush", "mkv_update_count", "mkv_calibrate_gather", "mkv_calibrate_stream",
+           "mkv_packed_attention", "mkv_update_append", "mkv_update_flush", "mkv_update_count", "mkv_calibrate_gather", "mkv_calibrate_stream", "mkv_calibrate_walk",
            "mkv_attention_stats", "mkv_rotation_set", "mkv_rotate_query", "mkv_rotate_output", "mkv_decode_step", "mkv_decode_host", "mkv_cache_export", "mkv_cache_bytes",
            "mkv_cache_status", "mkv_last_launch_count", "mkv_last_error", "mkv_version"]
 
@@ -57,6 +57,7 @@ _lib.mkv_update_flush.argtypes = [_vp, _i32, _vp, _vp]
 _lib.mkv_update_count.argtypes = [_vp, _i32, C.POINTER(_i32)]
 _lib.mkv_calibrate_gather.argtypes = [_vp, _i32, _vp, _vp, _i32, _vp]
 _lib.mkv_calibrate_stream.argtypes = [_vp, _i32, _u64, _vp]
+_lib.mkv_calibrate_walk.argtypes = [_vp, _i32, _vp, _vp, _vp, _i32, _i32, _vp]
 _lib.mkv_attention_stats.argtypes = [_vp, C.POINTER(_u64), C.POINTER(_u64), C.POINTER(_u64), _i32]
 _lib.mkv_rotation_set.argtypes = [_vp, _i32, _vp, _vp, _vp]
 _lib.mkv_rotate_query.argtypes = [_vp, _i32, _vp, _vp, _vp]
@@ -209,6 +210,10 @@ def mkv_calibrate_stream(cache, layer, nbytes, stream=None):
     _check(_lib.mkv_calibrate_stream(cache, layer, int(nbytes), _stream(stream)))
 
 
+def mkv_calibrate_walk(cache, layer, q, sel, sel_count, reps, stream=None):
+    _check(_lib.mkv_calibrate_walk(cache, layer, _ptr(q), _ptr(sel), _ptr(sel_count), sel.shape[-1], int(reps), _stream(stream)))
+
+
 def mkv_attention_stats(cache, reset=False):
     a, b, c = _u64(0), _u64(0), _u64(0)
     _check(_lib.mkv_attention_stats(cache, C.byref(a), C.byref(b), C.byref(c), 1 if reset else 0))
@@ -342,6 +347,9 @@ class Cache:
 
     def calibrate_stream(self, layer, nbytes, stream=None):
         mkv_calibrate_stream(self.h, layer, nbytes, stream)
+
+    def calibrate_walk(self, layer, q, sel, sel_count, reps, stream=None):
+        mkv_calibrate_walk(self.h, layer, q, sel, sel_count, reps, stream)
 
     def attention_stats(self, reset=False):
         return mkv_attention_stats(self.h, reset)

@@ -119,6 +119,50 @@ struct Split {
     __device__ __forceinline__ unsigned begin(unsigned i) const { return i * b + min(i, r); }
 };
 
+// QK of one group in flight: S (16 tokens x 8 heads) += K q^T with the group's tokens = M (rows 0-7 = block 0, rows 8-15 =
+// block 1), heads = N, channels = K.  sp0 / sp1: the K parts of its blocks in shared memory; qa: q[head gq][32qq .. 32qq+31]
+// as B fragments.  Packed vectors are expanded straight into A fragments (mkv_walk.cuh); dense vectors skip the walk.
+__device__ __forceinline__ void qk_group(float (&S)[4], int r_k, int nb0, int nb1, uint32_t sp0, uint32_t sp1,
+                                         const uint32_t (&qa)[8][2], int lane) {
+    const int gq = lane >> 2, qq = lane & 3;
+    const bool two = nb1 != 0;
+    const bool full = nb0 == kPhys && (!two || nb1 == kPhys);
+    if (r_k == kD && full) {
+        const uint32_t a0 = sp0 + 256 * gq + 64 * qq, a1 = sp1 + 256 * gq + 64 * qq;
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+            const uint4 x = lds_128(a0 + 16 * h);
+            uint4 y = make_uint4(0u, 0u, 0u, 0u);
+            if (two) y = lds_128(a1 + 16 * h);
+            mma_bf16(S, x.x, y.x, x.y, y.y, qa[2 * h][0], qa[2 * h][1]);
+            mma_bf16(S, x.z, y.z, x.w, y.w, qa[2 * h + 1][0], qa[2 * h + 1][1]);
+        }
+    } else {
+        // run of (token gq, word qq): starts after the kept elements of the lower words
+        uint32_t w0 = 0u, w1 = 0u, p0, p1, st0 = 2u, st1 = 2u;
+        if (r_k == kD) {  // ragged dense block: all slots kept, no bitmap stored
+            w0 = gq < nb0 ? 0xffffffffu : 0u;
+            w1 = gq < nb1 ? 0xffffffffu : 0u;
+            p0 = sp0 + 256 * gq + 64 * qq;
+            p1 = sp1 + 256 * gq + 64 * qq;
+        } else {  // values rank-major: rank rho of token t at element rho * nb + t
+            if (gq < nb0) w0 = lds_u32(sp0 + 4 * lane);
+            if (gq < nb1) w1 = lds_u32(sp1 + 4 * lane);
+            uint32_t cnt = (uint32_t)__popc(w0) | ((uint32_t)__popc(w1) << 16), inc = cnt, t;
+            t = __shfl_up_sync(kFull, inc, 1); if (qq >= 1) inc += t;
+            t = __shfl_up_sync(kFull, inc, 2); if (qq >= 2) inc += t;
+            const uint32_t ex = inc - cnt;
+            st0 = 2u * nb0; st1 = 2u * nb1;
+            p0 = sp0 + 16 * nb0 + st0 * (ex & 0xffffu) + 2 * gq;
+            p1 = sp1 + 16 * nb1 + st1 * (ex >> 16) + 2 * gq;
+        }
+        k_walk_mma<0>(S, w0, w1, p0, p1, st0, st1, qa);
+        k_walk_mma<1>(S, w0, w1, p0, p1, st0, st1, qa);
+        k_walk_mma<2>(S, w0, w1, p0, p1, st0, st1, qa);
+        k_walk_mma<3>(S, w0, w1, p0, p1, st0, st1, qa);
+    }
+}
+
 // PV of one group in flight: O^T += V^T P^T with channels = M, heads = N, the group's <= 16 tokens = K.  vb0 / vb1: the
 // V parts of its blocks in shared memory; ph / pl: probabilities of head gq, tokens 2qq, 2qq+1 of each block, split into
 // bf16 hi + lo (exactly the B fragments: k = token, n = head).  Dense vectors (r = D) skip the walk.
@@ -411,40 +455,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             // ---- QK: S (tokens x heads); rows 0-7 = block 0, rows 8-15 = block 1
             if (nb0 != 0) {
                 float S[4] = {0.f, 0.f, 0.f, 0.f};
-                if (r_k == kD && full) {
-                    const uint32_t a0 = sp0 + 256 * gq + 64 * qq, a1 = sp1 + 256 * gq + 64 * qq;
-#pragma unroll
-                    for (int h = 0; h < 4; ++h) {
-                        const uint4 x = lds_128(a0 + 16 * h);
-                        uint4 y = make_uint4(0u, 0u, 0u, 0u);
-                        if (two) y = lds_128(a1 + 16 * h);
-                        mma_bf16(S, x.x, y.x, x.y, y.y, qa[2 * h][0], qa[2 * h][1]);
-                        mma_bf16(S, x.z, y.z, x.w, y.w, qa[2 * h + 1][0], qa[2 * h + 1][1]);
-                    }
-                } else {
-                    // run of (token gq, word qq): starts after the kept elements of the lower words
-                    uint32_t w0 = 0u, w1 = 0u, p0, p1, st0 = 2u, st1 = 2u;
-                    if (r_k == kD) {  // ragged dense block: all slots kept, no bitmap stored
-                        w0 = gq < nb0 ? 0xffffffffu : 0u;
-                        w1 = gq < nb1 ? 0xffffffffu : 0u;
-                        p0 = sp0 + 256 * gq + 64 * qq;
-                        p1 = sp1 + 256 * gq + 64 * qq;
-                    } else {  // values rank-major: rank rho of token t at element rho * nb + t
-                        if (gq < nb0) w0 = lds_u32(sp0 + 4 * lane);
-                        if (gq < nb1) w1 = lds_u32(sp1 + 4 * lane);
-                        uint32_t cnt = (uint32_t)__popc(w0) | ((uint32_t)__popc(w1) << 16), inc = cnt, t;
-                        t = __shfl_up_sync(kFull, inc, 1); if (qq >= 1) inc += t;
-                        t = __shfl_up_sync(kFull, inc, 2); if (qq >= 2) inc += t;
-                        const uint32_t ex = inc - cnt;
-                        st0 = 2u * nb0; st1 = 2u * nb1;
-                        p0 = sp0 + 16 * nb0 + st0 * (ex & 0xffffu) + 2 * gq;
-                        p1 = sp1 + 16 * nb1 + st1 * (ex >> 16) + 2 * gq;
-                    }
-                    k_walk_mma<0>(S, w0, w1, p0, p1, st0, st1, qa);
-                    k_walk_mma<1>(S, w0, w1, p0, p1, st0, st1, qa);
-                    k_walk_mma<2>(S, w0, w1, p0, p1, st0, st1, qa);
-                    k_walk_mma<3>(S, w0, w1, p0, p1, st0, st1, qa);
-                }
+                qk_group(S, r_k, nb0, nb1, sp0, sp1, qa, lane);
                 // ---- scaled logits of token gq of each block, heads 2qq, 2qq+1 -> cache [head][token]
                 const bool v0 = gq < nb0, v1 = gq < nb1;
                 const float zA0 = v0 ? S[0] * scale_log2 : -INFINITY, zB0 = v0 ? S[1] * scale_log2 : -INFINITY;
@@ -824,6 +835,61 @@ mkv_stream_read_kernel(const uint4* __restrict__ base, unsigned long long n16, u
     if (acc == 0x9e3779b9u) *sink = acc;  // keeps the loads alive
 }
 
+
+// calibration row (iii): the QK expansion alone.  Every warp copies the K parts of ONE group of the real selection (two
+// consecutive selected blocks of a unit) into shared memory and then runs qk_group() on it `reps` times: no staging, no
+// logits, no softmax, no output.  (t(reps2) - t(reps1)) / (reps2 - reps1) / kWarps is the time one SM needs per group
+// when nothing but the expansion runs: the floor the shared-memory pipe sets for phase 1 (and for the score kernel).
+__global__ void __launch_bounds__(kWarps * 32, 1)
+mkv_walk_probe_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, const int32_t* __restrict__ sel,
+                      const int32_t* __restrict__ sel_count, int k_max, int reps, unsigned long long* __restrict__ sink) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gq = lane >> 2, qq = lane & 3;
+    const int wi = blockIdx.x * kWarps + warp;
+    const int u = wi % g.n_units;
+    const int cnt = min(max(__ldg(sel_count + u), 0), k_max) * g.ppb;
+    const int pairs = cnt >> 1;
+    if (pairs == 0) return;
+    const int j = 2 * ((wi / g.n_units) % pairs);
+    uint32_t off[2], meta[2];
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const int ts = __ldg(sel + (size_t)u * k_max + ((j + i) >> (g.ppb - 1)));
+        plan_lookup(g, lv, u, ts < 0 ? -1 : ts + kPhys * ((j + i) & (g.ppb - 1)), off[i], meta[i]);
+    }
+    uint8_t* mine = smem + warp * 4096;
+    const uint32_t sp0 = smem_u32(mine), sp1 = sp0 + 2048;
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const uint32_t nb = meta[i] >> 16, kb = (nb * vecb(meta[i] & 255u) + 15u) >> 4;  // 16-B units of the K part (<= 128)
+        const uint4* src = reinterpret_cast<const uint4*>(lv.slice) + off[i];
+        for (uint32_t x = lane; x < kb; x += 32) reinterpret_cast<uint4*>(mine + 2048 * i)[x] = __ldg(src + x);
+    }
+    __syncwarp();
+    const int r_k = (int)(meta[0] & 255u);
+    const int nb0 = (int)(meta[0] >> 16), nb1 = (meta[1] & 255u) == (meta[0] & 255u) ? (int)(meta[1] >> 16) : 0;
+    const size_t row = (size_t)(u / g.n_kv_heads) * g.n_q_heads + (size_t)(u % g.n_kv_heads) * g.group;
+    uint32_t qa[8][2];
+    {
+        const uint4* qrow = reinterpret_cast<const uint4*>(q + (row + gq) * kD + 32 * qq);
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+            uint4 v = make_uint4(0u, 0u, 0u, 0u);
+            if (gq < g.group) v = __ldg(qrow + h);
+            qa[2 * h][0] = v.x; qa[2 * h][1] = v.y; qa[2 * h + 1][0] = v.z; qa[2 * h + 1][1] = v.w;
+        }
+    }
+    float acc = 0.f;
+#pragma unroll 1
+    for (int it = 0; it < reps; ++it) {
+        float S[4] = {0.f, 0.f, 0.f, 0.f};
+        qk_group(S, r_k, nb0, nb1, sp0, sp1, qa, lane);
+        acc += (S[0] + S[1]) + (S[2] + S[3]);
+        qa[0][0] ^= __float_as_uint(acc) & 0x10000u;  // loop-carried: the walk cannot be hoisted out of the loop
+    }
+    if (acc == 1234.56789f) *sink = 1ull;  // keeps the arithmetic alive
+}
+
 }  // namespace
 
 // logit scratch: per unit one entry of 8 G floats per position of its block stream (selected + update-buffer blocks)
@@ -904,6 +970,16 @@ cudaError_t launch_stream_read(const uint8_t* base, unsigned long long bytes, in
                                cudaStream_t s) {
     return launch_pdl(mkv_stream_read_kernel, dim3(sm_count), dim3(kWarps * 32), (size_t)0, s,
                       reinterpret_cast<const uint4*>(base), bytes / 16ull, sink);
+}
+
+cudaError_t launch_walk_probe(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
+                              const int32_t* sel_count, int k_max, int reps, int sm_count, unsigned long long* sink,
+                              cudaStream_t s) {
+    const int smem = kWarps * 4096;
+    cudaError_t e = cudaFuncSetAttribute(mkv_walk_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    mkv_walk_probe_kernel<<<sm_count, kWarps * 32, smem, s>>>(g, lv, q, sel, sel_count, k_max, reps, sink);
+    return cudaGetLastError();
 }
 
 }  // namespace mkv

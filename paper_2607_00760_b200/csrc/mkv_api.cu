@@ -367,6 +367,19 @@ int mkv_calibrate_gather(const mkv_cache* cc, int32_t layer, const int32_t* sel,
     return MKV_OK;
 }
 
+int mkv_calibrate_walk(const mkv_cache* cc, int32_t layer, const void* q, const int32_t* sel, const int32_t* sel_count,
+                       int32_t k_max, int32_t reps, void* stream) {
+    if (!cc || !q || !sel || !sel_count) return fail(MKV_E_ARG, "mkv_calibrate_walk: NULL argument");
+    mkv_cache* c = const_cast<mkv_cache*>(cc);
+    const CacheGeom& g = c->geom;
+    if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
+    if (k_max < 1 || reps < 1) return fail(MKV_E_ARG, "mkv_calibrate_walk: k_max < 1 or reps < 1");
+    MKV_CUDA(cudaSetDevice(c->desc.device));
+    MKV_CUDA(launch_walk_probe(g, c->view(layer), (const uint16_t*)q, sel, sel_count, k_max, reps, c->sm_count, c->sink,
+                               (cudaStream_t)stream));
+    return MKV_OK;
+}
+
 int mkv_calibrate_stream(const mkv_cache* cc, int32_t layer, uint64_t bytes, void* stream) {
     if (!cc) return fail(MKV_E_ARG, "mkv_calibrate_stream: NULL argument");
     mkv_cache* c = const_cast<mkv_cache*>(cc);

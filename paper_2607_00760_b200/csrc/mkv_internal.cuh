@@ -143,6 +143,9 @@ cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint
                              cudaStream_t s, int* n_kernels, bool gather_only = false);
 cudaError_t launch_stream_read(const uint8_t* base, unsigned long long bytes, int sm_count, unsigned long long* sink,
                                cudaStream_t s);
+cudaError_t launch_walk_probe(const CacheGeom& g, const LayerView& lv, const uint16_t* q, const int32_t* sel,
+                              const int32_t* sel_count, int k_max, int reps, int sm_count, unsigned long long* sink,
+                              cudaStream_t s);
 // KV update buffer: copy n_new raw tokens of every unit into rows [n_have, n_have + n_new)
 // and set the layer's device-side count to n_have + n_new
 cudaError_t launch_update_copy(const CacheGeom& g, const CompressArgs& a, uint16_t* upd_k, uint16_t* upd_v,
