@@ -73,13 +73,6 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
     uint8_t* wbase = smem + warp * kWS;
     const uint32_t stage0 = smem_u32(wbase);
     SDesc* ring = reinterpret_cast<SDesc*>(wbase + NSTAGE * kScoreStage);
-    const uint32_t bar0 = stage0 + NSTAGE * kScoreStage + kRing * 32;
-    if (lane == 0) {
-#pragma unroll
-        for (int s = 0; s < NSTAGE; ++s) mbar_init(bar0 + 8 * s, 1);
-        mbar_init_fence();
-    }
-    __syncwarp();
 
     int ibuilt = 0;                        // items described
     int gposc = 0, gposi = 0, gbuilt = 0;  // groups consumed / issued / described
@@ -127,7 +120,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             SDesc d;
             d.bm0 = bm; d.val0 = val; d.bm1 = two ? bm1 : 0u; d.val1 = two ? val1 : 0u;
             d.out0 = out; d.out1 = two ? out1 : 0u;
-            d.meta = r_k | (nb << 8) | ((two ? nb1 : 0u) << 12) | (merged ? 1u << 16 : 0u);
+            d.meta = r_k | (nb << 8) | ((two ? nb1 : 0u) << 12) | (merged ? (1u << 16) | ((sz + sz1) << 17) : 0u);
             d.unit = u;
             ring[(gbuilt + __popc(gm & lanemask_lt())) & (kRing - 1)] = d;
         }
@@ -136,30 +129,35 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
         __syncwarp();
     };
 
-    // start the copies of the next group into stage s (lane 0: <= 2 bulk copies per item)
+    // start the copies of the next group into stage s: every lane moves 16 bytes at a time (cp.async), one commit group
+    // per call (empty when nothing is left, so that "all but the newest NSTAGE - 1 groups" always means "group k")
     const unsigned long long slice = reinterpret_cast<unsigned long long>(lv.slice);
+    auto copy_chunk = [&](uint32_t dst, uint32_t src16, uint32_t bytes) {
+        const unsigned long long src = slice + ((unsigned long long)src16 << 4);
+#pragma unroll 1
+        for (uint32_t x = 16u * (uint32_t)lane; x < bytes; x += 512u) cp_async_16(dst + x, src + x);
+    };
     auto issue = [&](int s) {
 #pragma unroll 1
         while (gposi == gbuilt && ibuilt < n_total) build(min(32, n_total - ibuilt));
-        if (gposi == gbuilt) return;
-        if (lane == 0) {
+        if (gposi != gbuilt) {
             const SDesc d = ring[gposi & (kRing - 1)];
-            const uint32_t r = d.meta & 255u, nb0 = (d.meta >> 8) & 15u, nb1 = (d.meta >> 12) & 15u;
-            const uint32_t bar = bar0 + 8 * s, dst = stage0 + s * kScoreStage;
-            // bitmaps nb x 16 B, then the values padded to 16 B; dense: nb x 256 B in one chunk
-            const uint32_t bb0 = r == (uint32_t)kD ? nb0 * 256u : nb0 * 16u, vb0 = r == (uint32_t)kD ? 0u : pad16u(nb0 * 2u * r);
-            const uint32_t bb1 = r == (uint32_t)kD ? nb1 * 256u : nb1 * 16u, vb1 = r == (uint32_t)kD ? 0u : pad16u(nb1 * 2u * r);
-            mbar_expect_tx(bar, bb0 + vb0 + bb1 + vb1);
-            if (d.meta >> 16) {  // item 1 lands right behind item 0
-                bulk_g2s(dst, slice + ((unsigned long long)d.bm0 << 4), bb0 + vb0 + bb1 + vb1, bar);
+            const uint32_t dst = stage0 + s * kScoreStage;
+            if (d.meta & (1u << 16)) {  // item 1 lands right behind item 0: one chunk
+                copy_chunk(dst, d.bm0, (d.meta >> 17) << 4);
             } else {
-                bulk_g2s(dst, slice + ((unsigned long long)d.bm0 << 4), bb0, bar);
-                if (vb0) bulk_g2s(dst + bb0, slice + ((unsigned long long)d.val0 << 4), vb0, bar);
-                if (bb1) bulk_g2s(dst + kItem1, slice + ((unsigned long long)d.bm1 << 4), bb1, bar);
-                if (vb1) bulk_g2s(dst + kItem1 + bb1, slice + ((unsigned long long)d.val1 << 4), vb1, bar);
+                const uint32_t r = d.meta & 255u, nb0 = (d.meta >> 8) & 15u, nb1 = (d.meta >> 12) & 15u;
+                // bitmaps nb x 16 B, then the values padded to 16 B; dense: nb x 256 B in one chunk
+                const uint32_t bb0 = r == (uint32_t)kD ? nb0 * 256u : nb0 * 16u, vb0 = r == (uint32_t)kD ? 0u : pad16u(nb0 * 2u * r);
+                const uint32_t bb1 = r == (uint32_t)kD ? nb1 * 256u : nb1 * 16u, vb1 = r == (uint32_t)kD ? 0u : pad16u(nb1 * 2u * r);
+                copy_chunk(dst, d.bm0, bb0);
+                copy_chunk(dst + bb0, d.val0, vb0);
+                copy_chunk(dst + kItem1, d.bm1, bb1);
+                copy_chunk(dst + kItem1 + bb1, d.val1, vb1);
             }
+            ++gposi;
         }
-        ++gposi;
+        cp_async_commit();
     };
 
     uint32_t qa[8][2];
@@ -168,7 +166,6 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
     // ---- main loop.  Iteration k >= 0 consumes group k from stage k % NSTAGE and refills that stage
     // with group k + NSTAGE; iterations k < 0 only fill the pipeline (one call site for issue()).
     int s = 0;
-    uint32_t parity = 0u;
 #pragma unroll 1
     for (int k = -NSTAGE;; ++k) {
         if (k >= 0) {
@@ -190,7 +187,8 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             const uint32_t sp0 = stage0 + s * kScoreStage;
             const uint32_t sp1 = sp0 + ((d.meta >> 16) ? 16u * (uint32_t)nb0 + pad16u(2u * (uint32_t)(nb0 * r_k)) : (uint32_t)kItem1);
 
-            mbar_wait(bar0 + 8 * s, parity);  // the group's bulk copies have landed
+            cp_async_wait<NSTAGE - 1>();  // this lane's copies of the group have landed ...
+            __syncwarp();                 // ... and every other lane's
 
             float S[4] = {0.f, 0.f, 0.f, 0.f};  // rows gq / gq+8 = key gq of item 0 / 1, columns = heads 2qq, 2qq+1
             if (r_k == kD && nb0 == 8 && (nb1 == 0 || nb1 == 8)) {
@@ -249,7 +247,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             ++gposc;
         }
         issue(s);  // stage s is free (or, for k < 0, still empty): start the copies of group k + NSTAGE
-        if (++s == NSTAGE) { s = 0; if (k >= 0) parity ^= 1u; }
+        if (++s == NSTAGE) s = 0;
     }
 }
 
