@@ -510,10 +510,16 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     if (!kGatherOnly) {
         cluster_sync();  // every CTA's table is complete and visible to the cluster (also a CTA barrier)
         if (gq < G) {
+            // (four remote loads in flight at a time: a cluster of 16 would otherwise pay 16 round trips in a row)
             uint32_t k = 0u;
             const uint32_t a = smem_u32(&s_max[gq]);
 #pragma unroll 1
-            for (int r = 0; r < C; ++r) k = max(k, ld_dsmem_u32(dsmem_addr(a, (uint32_t)r)));
+            for (int r0 = 0; r0 < C; r0 += 4) {
+                uint32_t v[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) v[j] = ld_dsmem_u32(dsmem_addr(a, (uint32_t)min(r0 + j, C - 1)));
+                k = max(k, max(max(v[0], v[1]), max(v[2], v[3])));
+            }
             Mraw = k == 0u ? -INFINITY : funkey(k);
             if (warp == 0 && qq == 0) s_M[gq] = Mraw;
         }
@@ -795,9 +801,17 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             const int h = e >> 7;
             float o = 0.f, l = 0.f;
 #pragma unroll 1
-            for (int r = 0; r < C; ++r) {
-                o += ld_dsmem_f32(dsmem_addr(ao + 4u * (uint32_t)e, (uint32_t)r));
-                l += ld_dsmem_f32(dsmem_addr(al + 4u * (uint32_t)h, (uint32_t)r));
+            for (int r0 = 0; r0 < C; r0 += 4) {  // (eight remote loads in flight; ranks past the cluster add nothing)
+                float vo[4], vl[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const uint32_t r = (uint32_t)min(r0 + j, C - 1);
+                    vo[j] = ld_dsmem_f32(dsmem_addr(ao + 4u * (uint32_t)e, r));
+                    vl[j] = ld_dsmem_f32(dsmem_addr(al + 4u * (uint32_t)h, r));
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if (r0 + j < C) { o += vo[j]; l += vl[j]; }
             }
             out[row * kD + e] = l > 0.f ? o / l : 0.f;
             if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = l > 0.f ? (s_M[h] + log2f(l)) * kLn2 : -INFINITY;
@@ -897,7 +911,8 @@ size_t attention_z_unit_stride(const CacheGeom& g) { return ((size_t)g.score_str
 size_t attention_zbuf_floats(const CacheGeom& g) { return (size_t)g.n_units * attention_z_unit_stride(g) * 8 * (size_t)g.group; }
 
 // Cluster size for a layer of n_units units: the largest power of two C <= 16 with n_units * C <= SMs whose clusters
-// can all be resident at once (one CTA per SM; a cluster lives inside one GPC), else 1.
+// can all be resident at once (one CTA per SM; a cluster lives inside one GPC), else 1.  (Sizes that are not powers of
+// two were tried for 8 units: 10 CTAs per unit are schedulable, 16 are not, and 10 was no faster than 8.)
 template <bool GATHER>
 static int pick_cluster(const CacheGeom& g, int smem, int sm_count) {
     cudaFuncSetAttribute(mkv_packed_attention_kernel<GATHER>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
