@@ -336,7 +336,7 @@ def run_mkv(args):
                      "frac_of_nominal_8TBs": round(attn_gbs / NOMINAL_HBM_GBS, 4),
                      "algorithmic_bytes_per_launch": int(a_bytes),
                      "what": "frac = algorithmic bytes (every selected K and V payload, SURVEY 8(d)) / time / peak.  The kernel "
-                             "fetches every K part but only the V parts of blocks with a probability >= 2^-40 of the CTA's "
+                             "fetches every K part but only the V parts of blocks with a probability >= 2^-40 of the unit's "
                              "largest (bytes_fetched_per_launch, from the kernel's counters), so frac is NOT the DRAM rate",
                      "v_blocks_fetched_fraction": round(v_frac, 4),
                      "bytes_fetched_per_launch": bytes_fetched,
@@ -589,17 +589,27 @@ def run_sweep(args):
                 for l in range(NL):
                     cache.select(l, built.q[l], budget, sel[l], cnt[l])
 
+            cache.attention_stats(reset=True)
             ms_a = timed_loop(torch, step_attention, args.steps, max(3, args.warmup), lambda: None, True)
+            stats = cache.attention_stats(reset=True)
             ms_s = timed_loop(torch, step_select, args.steps, max(3, args.warmup), lambda: None, True)
             cache.status()
-            cache.attention_stats(reset=True)
-            ab = sum(workload.attention_bytes(built, l, sel[l], cnt[l]) for l in range(NL)) / NL
+            split = [workload.attention_bytes(built, l, sel[l], cnt[l], split=True) for l in range(NL)]
+            ab = sum(x[0] for x in split) / NL
+            v_parts = sum(x[2] for x in split) / NL
+            n_blocks = sum(int(c.sum().item()) for c in cnt) / NL
+            # bytes the kernel fetched: everything but the V parts phase 2 skipped (kernel counters).  `frac`
+            # is on the algorithmic bytes and exceeds 1 where most V parts are skipped: it is not a DRAM rate
+            fetched = ab - v_parts + stats["v_bytes"] / max(1, stats["blocks"]) * n_blocks
             us = ms_a * 1e3 / NL
             gbs = ab / (us * 1e-6) / 1e9
             points.append({"keep_ratio": keep, "r_keep": w.r_keep, "token_budget": budget,
                            "attention_us_per_layer": round(us, 2), "select_us_per_layer": round(ms_s * 1e3 / NL, 2),
                            "algorithmic_bytes_per_launch": int(ab), "achieved_gbs": round(gbs, 1),
-                           "frac": round(gbs / peak, 4), "frac_of_nominal_8TBs": round(gbs / NOMINAL_HBM_GBS, 4)})
+                           "frac": round(gbs / peak, 4), "frac_of_nominal_8TBs": round(gbs / NOMINAL_HBM_GBS, 4),
+                           "v_blocks_fetched_fraction": round(stats["v_blocks"] / max(1, stats["blocks"]), 4),
+                           "bytes_fetched_per_launch": int(fetched),
+                           "frac_on_bytes_fetched": round(fetched / (us * 1e-6) / 1e9 / peak, 4)})
             del sel, cnt, out
         built.free()
         del built

@@ -162,7 +162,8 @@ MKV_API int mkv_select(const mkv_cache* cache, int32_t layer, const void* q, int
  * tokens of the layer's KV update buffer if it holds any (see mkv_update_append).
  * sel / sel_count as written by mkv_select (any order of blocks is accepted; entries the caller changed after
  * mkv_select are honoured: the per-block records mkv_select leaves for this call are verified against `sel`).
- * One launch of one CTA per SM; no CTA waits for another one.
+ * One launch: one thread-block cluster per unit (one CTA per SM); the CTAs of a cluster meet at cluster barriers and read
+ * each other's shared memory, nothing else is shared between CTAs.
  * out: float [batch][n_q_heads][D].  lse_opt: float [batch][n_q_heads] or NULL (log-sum-exp of the
  * scaled logits; -inf and out = 0 for an empty selection).
  */
@@ -247,8 +248,8 @@ MKV_API int mkv_decode_host(mkv_cache* cache, int32_t layer, const void* q_host,
  *         floor of phase 1 of mkv_packed_attention and of the score kernel of mkv_select.  q: device bf16
  *         [batch][n_q_heads][128].
  * stats:  counters accumulated by mkv_packed_attention since the last reset: token blocks attended, token blocks
- *         whose V part was fetched (phase 2 skips a block whose probabilities are all < 2^-40 of the largest
- *         the CTA holds of the unit), bytes of those V copies.  Synchronises.
+ *         whose V part was fetched (phase 2 skips a block whose probabilities are all < 2^-40 of the unit's
+ *         largest), bytes of those V copies.  Synchronises.
  */
 MKV_API int mkv_calibrate_gather(const mkv_cache* cache, int32_t layer, const int32_t* sel,
                          const int32_t* sel_count, int32_t k_max, void* stream);
