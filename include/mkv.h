@@ -223,10 +223,11 @@ MKV_API int mkv_decode_step(mkv_cache* cache, int32_t layer, const void* q, int3
                     int32_t k_max, void* stream);
 
 /*
- * Steps 2+3 with HOST buffers (the end-to-end call): copies q_host (bf16 [batch][n_q_heads][D],
- * pinned for true async) to the device, runs select + attention, copies out_host (float
- * [batch][n_q_heads][D]) back.  Everything is enqueued on `stream`; the caller synchronises the
- * stream before reading out_host.  sel_host_opt [batch][n_kv_heads][token_budget/B + 1] and
+ * Steps 2+3 with HOST buffers (the end-to-end call): brings q_host (bf16 [batch][n_q_heads][D]) to the device, runs
+ * mkv_decode_step, delivers out_host (float [batch][n_q_heads][D]).  Pinned (page-locked) buffers are read and written
+ * by kernels of the chain itself (a 64-KB fetch kernel in front; the attention kernel stores straight into out_host, or
+ * a store kernel behind the output fold), so the step never leaves the compute engine; pageable buffers fall back to
+ * cudaMemcpyAsync.  Everything is enqueued on `stream`; the caller synchronises the stream before reading out_host.  sel_host_opt [batch][n_kv_heads][token_budget/B + 1] and
  * sel_count_host_opt [batch][n_kv_heads] may be NULL.
  */
 MKV_API int mkv_decode_host(mkv_cache* cache, int32_t layer, const void* q_host, int32_t token_budget,

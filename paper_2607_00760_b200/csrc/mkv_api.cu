@@ -523,6 +523,25 @@ int mkv_decode_step(mkv_cache* c, int32_t layer, const void* q, int32_t budget, 
     return MKV_OK;
 }
 
+namespace {
+
+// 16-byte copy between device memory and device-mapped (pinned) host memory: part of the decode chain (PDL), so a
+// host-buffer step stays on the compute engine instead of bouncing to a copy engine and back twice per layer
+__global__ void __launch_bounds__(256) mkv_copy16_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst, size_t n16) {
+    pdl_wait();
+    pdl_launch_dependents();
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x) dst[i] = src[i];
+}
+
+// device address of a pinned / registered host buffer the GPU can access directly, else nullptr
+void* mapped_host(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return a.type == cudaMemoryTypeHost ? a.devicePointer : nullptr;
+}
+
+}  // namespace
+
 int mkv_decode_host(mkv_cache* c, int32_t layer, const void* q_host, int32_t budget, int32_t reduce, float scale,
                     float* out_host, int32_t* sel_host_opt, int32_t* sel_count_host_opt, void* stream) {
     if (!c || !q_host || !out_host) return fail(MKV_E_ARG, "mkv_decode_host: NULL argument");
@@ -532,10 +551,25 @@ int mkv_decode_host(mkv_cache* c, int32_t layer, const void* q_host, int32_t bud
     if (k_max > c->sel_cap) k_max = c->sel_cap;
     if (layer < 0 || layer >= g.n_layers) return fail(MKV_E_ARG, "layer %d out of range", layer);
     MKV_CUDA(cudaSetDevice(c->desc.device));
-    MKV_CUDA(cudaMemcpyAsync(c->q_dev, q_host, (size_t)g.batch * g.n_q_heads * kD * 2, cudaMemcpyHostToDevice, s));
-    const int rc = mkv_decode_step(c, layer, c->q_dev, budget, reduce, scale, c->out_dev, nullptr, nullptr, nullptr, 0, stream);
+    const size_t q_bytes = (size_t)g.batch * g.n_q_heads * kD * 2, out_bytes = (size_t)g.batch * g.n_q_heads * kD * 4;
+    // Pinned host buffers are read and written by kernels of the chain itself (q: one small fetch kernel; out: the
+    // attention kernel's own stores, or a store kernel behind the output fold); pageable buffers take the copy engine.
+    void* q_map = mapped_host(q_host);
+    void* out_map = mapped_host(out_host);
+    const bool rotated = !c->rot_set.empty() && c->rot_set[layer];
+    if (q_map)
+        MKV_CUDA(launch_pdl(mkv_copy16_kernel, dim3(8), dim3(256), (size_t)0, s, (const uint4*)q_map, (uint4*)c->q_dev, q_bytes / 16));
+    else
+        MKV_CUDA(cudaMemcpyAsync(c->q_dev, q_host, q_bytes, cudaMemcpyHostToDevice, s));
+    float* out_arg = out_map && !rotated ? (float*)out_map : c->out_dev;
+    const int rc = mkv_decode_step(c, layer, c->q_dev, budget, reduce, scale, out_arg, nullptr, nullptr, nullptr, 0, stream);
     if (rc) return rc;
-    MKV_CUDA(cudaMemcpyAsync(out_host, c->out_dev, (size_t)g.batch * g.n_q_heads * kD * 4, cudaMemcpyDeviceToHost, s));
+    if (out_arg == c->out_dev) {
+        if (out_map)
+            MKV_CUDA(launch_pdl(mkv_copy16_kernel, dim3(16), dim3(256), (size_t)0, s, (const uint4*)c->out_dev, (uint4*)out_map, out_bytes / 16));
+        else
+            MKV_CUDA(cudaMemcpyAsync(out_host, c->out_dev, out_bytes, cudaMemcpyDeviceToHost, s));
+    }
     if (sel_host_opt)
         MKV_CUDA(cudaMemcpyAsync(sel_host_opt, c->sel_dev, (size_t)g.n_units * k_max * 4, cudaMemcpyDeviceToHost, s));
     if (sel_count_host_opt)

@@ -627,6 +627,12 @@ def test_layers_are_independent_and_decode_host_matches(env):
                                                             sel[i, h, :cnt[i, h]], 1 / math.sqrt(128))
         o = out_host.numpy().astype(np.float64)
         assert np.abs(o - ref).max() <= 3e-3 and np.linalg.norm(o - ref) / np.linalg.norm(ref) <= 1e-3
+        # pageable host buffers take the copy-engine path instead of the chain's own fetch / store: same bits
+        q_page = torch.from_numpy(a.q.view(np.int16).copy()).view(torch.bfloat16)
+        out_page = torch.zeros((2, 8, 128), dtype=torch.float32)
+        a.cache.decode_host(0, q_page, 256, 1 / math.sqrt(128), out_page)
+        torch.cuda.synchronize()
+        assert np.array_equal(out_page.numpy(), out_host.numpy())
         t, s = a.check_select(256)
         assert s == 0
     finally:
