@@ -353,7 +353,7 @@ def run_mkv(args):
                      "frac": round(comp_gbs / peak, 4), "bytes_read": comp_bytes["read"], "bytes_written": comp_bytes["write"],
                      "build_all_layers_s": round(build_s, 2)},
         "e2e": {"value": round(ms_e2e * 1e3 / n_layers, 3), "unit": UNIT,
-                "what": "select + attention through mkv_decode_host: pinned host q in, host out back, both copies timed",
+                "what": "select + attention through mkv_decode_host: pinned host q in, host out back, both transfers inside the timed region (kernels of the chain read q_host and write out_host over PCIe)",
                 "launch": "cuda-graph of one decode step of mkv_decode_host calls" if graph else "eager, synchronised per step",
                 "h2d_bytes_per_step": n_layers * Bt * Hq * 128 * 2, "d2h_bytes_per_step": n_layers * Bt * Hq * 128 * 4,
                 "ms_per_step": round(ms_e2e, 4)},

@@ -101,6 +101,9 @@ __device__ __forceinline__ uint32_t ld_dsmem_u32(uint32_t a) {
     asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
     return v;
 }
+__device__ __forceinline__ void st_dsmem_f32(uint32_t a, float v) {
+    asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory");
+}
 __device__ __forceinline__ float ld_dsmem_f32(uint32_t a) {
     float v;
     asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory");
@@ -241,11 +244,13 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     __shared__ uint32_t s_max[kMaxGroup];                 // the CTA's per-head maxima (keys); read by the whole cluster
     __shared__ float s_l[kWarps][kMaxGroup];              // the warps' softmax sums
     __shared__ float s_cta_l[kMaxGroup];                  // the CTA's partial sums (its partial O: s_cta_o)
+    __shared__ float s_peer_l[kMaxGroup];                 // clusters of two: the second CTA's sums, pushed into the first
     __shared__ float s_M[kMaxGroup];                      // the unit's per-head maxima after the exchange
     __shared__ unsigned s_active;                         // warps of the CTA that hold a partial result
     __shared__ uint32_t s_q[kWarps][kDesc];               // phase 2: the groups of each warp's range that matter ...
     __shared__ int s_qn[kWarps];                          // ... and how many
     float* s_cta_o = reinterpret_cast<float*>(smem + kWarps * kWS);  // [G][128] floats behind the warps' regions
+    float* s_peer_o = s_cta_o + kMaxGroup * kD;                      // clusters of two: the second CTA's partial O
 
     uint8_t* wbase = smem + warp * kWS;
     const uint32_t ring0 = smem_u32(wbase);
@@ -781,20 +786,38 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     }
     __syncthreads();
     const int GD = G * kD;
+    // A cluster of two (64 units on 148 SMs): the second CTA PUSHES its partial into the first one's shared memory, so
+    // after the barrier the first CTA adds two local arrays and the second one is free to leave: no remote loads on the
+    // critical path and no third barrier.  Larger clusters are pulled by the first CTA (no room for 16 partials).
+    const bool push = C == 2;
     const unsigned wmask = s_active;  // (in warp order: the sums are reproducible)
+    const uint32_t peer_o = dsmem_addr(smem_u32(s_peer_o), 0u), peer_l = dsmem_addr(smem_u32(s_peer_l), 0u);
     for (int e = threadIdx.x; e < GD; e += kNT) {  // the CTA's partial
         float o = 0.f;
 #pragma unroll 1
         for (unsigned m = wmask; m; m &= m - 1u) o += *reinterpret_cast<const float*>(smem + (__ffs(m) - 1) * kWS + 4 * e);
-        s_cta_o[e] = o;
+        if (push && rank != 0) st_dsmem_f32(peer_o + 4u * (uint32_t)e, o);
+        else s_cta_o[e] = o;
     }
     if (threadIdx.x < G) {
         float l = 0.f;
 #pragma unroll 1
         for (int w = 0; w < kWarps; ++w) l += s_l[w][threadIdx.x];
-        s_cta_l[threadIdx.x] = l;
+        if (push && rank != 0) st_dsmem_f32(peer_l + 4u * threadIdx.x, l);
+        else s_cta_l[threadIdx.x] = l;
     }
     cluster_sync();  // every CTA's partial is complete and visible to the cluster
+    if (push) {
+        if (rank == 0) {
+            for (int e = threadIdx.x; e < GD; e += kNT) {
+                const int h = e >> 7;
+                const float o = s_cta_o[e] + s_peer_o[e], l = s_cta_l[h] + s_peer_l[h];
+                out[row * kD + e] = l > 0.f ? o / l : 0.f;
+                if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = l > 0.f ? (s_M[h] + log2f(l)) * kLn2 : -INFINITY;
+            }
+        }
+        return;
+    }
     if (rank == 0) {
         const uint32_t ao = smem_u32(s_cta_o), al = smem_u32(s_cta_l);
         for (int e = threadIdx.x; e < GD; e += kNT) {
@@ -937,7 +960,7 @@ static cudaError_t launch_attention_cfg(const CacheGeom& g, const LayerView& lv,
                                         const int32_t* sel_count, int k_max, float scale, float* out, float* lse,
                                         const AttnScratch& scr, const uint16_t* upd_k, const uint16_t* upd_v,
                                         const int32_t* upd_count, int sm_count, int* cluster_cache, cudaStream_t s) {
-    const int smem = kWarps * kWS + kMaxGroup * kD * 4;
+    const int smem = kWarps * kWS + 2 * kMaxGroup * kD * 4;
     // the dynamic shared-memory opt-in is a per-device attribute of the function: set it on every launch (a cheap
     // host-side call) so that caches on different devices of one process are independent
     cudaError_t e = cudaFuncSetAttribute(mkv_packed_attention_kernel<GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -971,7 +994,7 @@ cudaError_t launch_attention(const CacheGeom& g, const LayerView& lv, const uint
 
 // choose the cluster sizes of both kernels for this cache (occupancy queries: host-side, not capturable)
 cudaError_t attention_prepare(const CacheGeom& g, int sm_count, int* cluster_cache) {
-    const int smem = kWarps * kWS + kMaxGroup * kD * 4;
+    const int smem = kWarps * kWS + 2 * kMaxGroup * kD * 4;
     cudaError_t e = cudaFuncSetAttribute(mkv_packed_attention_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(mkv_packed_attention_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
