@@ -150,7 +150,18 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                 // bitmaps nb x 16 B, then the values padded to 16 B; dense: nb x 256 B in one chunk
                 const uint32_t bb0 = r == (uint32_t)kD ? nb0 * 256u : nb0 * 16u, vb0 = r == (uint32_t)kD ? 0u : pad16u(nb0 * 2u * r);
                 const uint32_t bb1 = r == (uint32_t)kD ? nb1 * 256u : nb1 * 16u, vb1 = r == (uint32_t)kD ? 0u : pad16u(nb1 * 2u * r);
-                copy_chunk(dst, d.bm0, bb0);
+                if (r == (uint32_t)kD && nb0 == 8u && nb1 == 0u) {
+                    // a full dense item takes the LDS.128 path below: its 16-byte chunks are placed so that the eight lanes
+                    // of a load phase (two keys x four 64-byte quarters) hit eight different bank groups (rows are 256 B
+                    // apart, i.e. in the same banks): chunk c of key t goes to chunk c ^ 2 (c >> 3) ^ (t & 1)
+                    const unsigned long long src = slice + ((unsigned long long)d.bm0 << 4);
+#pragma unroll
+                    for (uint32_t i = 0; i < 4u; ++i) {
+                        const uint32_t ci = (uint32_t)lane + 32u * i, t = ci >> 4, c = ci & 15u;
+                        cp_async_16(dst + 256u * t + 16u * (c ^ ((c >> 3) << 1) ^ (t & 1u)), src + 16u * ci);
+                    }
+                } else
+                    copy_chunk(dst, d.bm0, bb0);
                 copy_chunk(dst + bb0, d.val0, vb0);
                 copy_chunk(dst + kItem1, d.bm1, bb1);
                 copy_chunk(dst + kItem1 + bb1, d.val1, vb1);
@@ -191,15 +202,13 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             __syncwarp();                 // ... and every other lane's
 
             float S[4] = {0.f, 0.f, 0.f, 0.f};  // rows gq / gq+8 = key gq of item 0 / 1, columns = heads 2qq, 2qq+1
-            if (r_k == kD && nb0 == 8 && (nb1 == 0 || nb1 == 8)) {
-                const uint32_t a0 = sp0 + 256 * gq + 64 * qq, a1 = sp1 + 256 * gq + 64 * qq;
+            if (r_k == kD && nb0 == 8 && nb1 == 0) {  // (dense items are never paired: two do not fit a stage)
+                const uint32_t a0 = sp0 + 256 * gq + 64 * qq, sw = (uint32_t)(2 * (qq >> 1)) ^ (uint32_t)(gq & 1);  // (swizzle of issue())
 #pragma unroll
                 for (int h = 0; h < 4; ++h) {
-                    const uint4 x = lds_128(a0 + 16 * h);
-                    uint4 y = make_uint4(0u, 0u, 0u, 0u);
-                    if (nb1) y = lds_128(a1 + 16 * h);
-                    mma_bf16(S, x.x, y.x, x.y, y.y, qa[2 * h][0], qa[2 * h][1]);
-                    mma_bf16(S, x.z, y.z, x.w, y.w, qa[2 * h + 1][0], qa[2 * h + 1][1]);
+                    const uint4 x = lds_128(a0 + 16 * ((uint32_t)h ^ sw));
+                    mma_bf16(S, x.x, 0u, x.y, 0u, qa[2 * h][0], qa[2 * h][1]);
+                    mma_bf16(S, x.z, 0u, x.w, 0u, qa[2 * h + 1][0], qa[2 * h + 1][1]);
                 }
             } else {
                 uint32_t w0 = 0u, w1 = 0u, p0, p1, st0 = 2u, st1 = 2u;
