@@ -382,6 +382,19 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         ++pend;
         __syncwarp();  // the slot table entry is visible to the whole warp
     };
+    // start the copies of one group (<= 2 chunks, 16-byte units) into ring offset `off`; `landed()` returns when the OLDEST
+    // group in flight is complete (groups complete in issue order)
+    auto stage = [&](const unsigned long long src, uint32_t off, uint32_t off0, uint32_t c0, uint32_t off1, uint32_t c1) {
+        // (one lane, one bulk copy per chunk on the slot's mbarrier; staging by all lanes with cp.async, which pays in the
+        // score kernel, was measured here too: 24.4 against 23.6 us/layer)
+        if (lane == 0) {
+            const uint32_t bar = bar0 + 8 * si, dst = ring0 + off;
+            mbar_expect_tx(bar, c0 + c1);
+            if (c0) bulk_g2s(dst, src + ((unsigned long long)off0 << 4), c0, bar);
+            if (c1) bulk_g2s(dst + c0, src + ((unsigned long long)off1 << 4), c1, bar);
+        }
+    };
+    auto landed = [&]() { mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u); };
     auto ring_release = [&]() {  // the oldest group has been consumed
         rused -= slot_tab[sc].y;
         parbits ^= 1u << sc;
@@ -422,13 +435,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 const uint32_t c0 = (d.x & 255u) << 4, c1 = ((d.x >> 8) & 255u) << 4;
                 uint32_t off;
                 if (!ring_alloc(c0 + c1, off)) break;
-                if (lane == 0) {
-                    const uint32_t bar = bar0 + 8 * si, dst = ring0 + off;
-                    const unsigned long long src = d.y ? reinterpret_cast<unsigned long long>(upd_k) : slice;
-                    mbar_expect_tx(bar, c0 + c1);
-                    if (c0) bulk_g2s(dst, src + ((unsigned long long)d.off0 << 4), c0, bar);
-                    if (c1) bulk_g2s(dst + c0, src + ((unsigned long long)d.off1 << 4), c1, bar);
-                }
+                stage(d.y ? reinterpret_cast<unsigned long long>(upd_k) : slice, off, d.off0, c0, d.off1, c1);
                 ring_commit();
                 ++gposi;
                 bposi += c1 ? 2 : 1;
@@ -445,7 +452,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             const bool two = nb1 != 0;
             const uint32_t sp0 = ring0 + slot_tab[sc].x, sp1 = sp0 + ((d.x & 255u) << 4);
             if (kGatherOnly) {
-                mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);
+                landed();
                 calib ^= lds_u32(sp0 + 4 * lane);
                 __syncwarp();
                 ring_release();
@@ -455,7 +462,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             }
             const bool full = nb0 == kPhys && (!two || nb1 == kPhys);
 
-            mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);  // the group's K parts have landed
+            landed();  // the group's K parts have landed
 
             // ---- QK: S (tokens x heads); rows 0-7 = block 0, rows 8-15 = block 1
             if (nb0 != 0) {
@@ -620,12 +627,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 else if (!need1) { nb1 = 0u; c1 = 0u; }
                 uint32_t off;
                 if (!ring_alloc(c0 + c1, off)) break;
+                stage((d.y & 1u) ? reinterpret_cast<unsigned long long>(upd_v) : slice, off, off0, c0, off1, c1);
                 if (lane == 0) {
-                    const uint32_t bar = bar0 + 8 * si, dst = ring0 + off;
-                    const unsigned long long src = (d.y & 1u) ? reinterpret_cast<unsigned long long>(upd_v) : slice;
-                    mbar_expect_tx(bar, c0 + c1);
-                    bulk_g2s(dst, src + ((unsigned long long)off0 << 4), c0, bar);
-                    if (c1) bulk_g2s(dst + c0, src + ((unsigned long long)off1 << 4), c1, bar);
                     GDesc g2;
                     g2.off0 = sk0 | (sk1 << 4) | (c0 << 8);                  // skews of the V parts, bytes of the first chunk
                     g2.off1 = (ent >> 10) + shift;                           // index of the first WALKED block in the owner's range
@@ -656,7 +659,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             const uint32_t ph0 = pack_bf16(e00, e01), ph1 = pack_bf16(e10, e11);
             const uint32_t pl0 = pack_bf16(e00 - __uint_as_float(ph0 << 16), e01 - __uint_as_float(ph0 & 0xffff0000u));
             const uint32_t pl1 = pack_bf16(e10 - __uint_as_float(ph1 << 16), e11 - __uint_as_float(ph1 & 0xffff0000u));
-            mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);  // the group's V parts have landed
+            landed();  // the group's V parts have landed
             pv_group(acc, r_v, nb0, nb1, vb0, vb1, ph0, ph1, pl0, pl1, gq, qq);
             walked = true;
             __syncwarp();  // every lane is done reading the slot
@@ -700,12 +703,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                     else if (!need1) { nb1 = 0u; c1 = 0u; }
                     uint32_t off;
                     if (!ring_alloc(c0 + c1, off)) break;  // no room yet: decide this group again after a consume
+                    stage((d.y & 1u) ? reinterpret_cast<unsigned long long>(upd_v) : slice, off, off0, c0, off1, c1);
                     if (lane == 0) {
-                        const uint32_t bar = bar0 + 8 * si, dst = ring0 + off;
-                        const unsigned long long src = (d.y & 1u) ? reinterpret_cast<unsigned long long>(upd_v) : slice;
-                        mbar_expect_tx(bar, c0 + c1);
-                        bulk_g2s(dst, src + ((unsigned long long)off0 << 4), c0, bar);
-                        if (c1) bulk_g2s(dst + c0, src + ((unsigned long long)off1 << 4), c1, bar);
                         GDesc e;
                         e.off0 = sk0 | (sk1 << 4) | (c0 << 8);                   // skews of the V parts, bytes of the first chunk
                         e.off1 = (uint32_t)bposd + shift;                        // index of the first WALKED block in the range
@@ -731,7 +730,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             const uint32_t vb0 = ring0 + slot_tab[sc].x + (d.off0 & 15u);
             const uint32_t vb1 = ring0 + slot_tab[sc].x + (d.off0 >> 8) + ((d.off0 >> 4) & 15u);
             if (kGatherOnly) {
-                mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);
+                landed();
                 calib ^= lds_u32((vb0 & ~3u) + 4 * lane);
                 __syncwarp();
                 ring_release();
@@ -748,7 +747,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             const uint32_t ph0 = pack_bf16(e00, e01), ph1 = pack_bf16(e10, e11);
             const uint32_t pl0 = pack_bf16(e00 - __uint_as_float(ph0 << 16), e01 - __uint_as_float(ph0 & 0xffff0000u));
             const uint32_t pl1 = pack_bf16(e10 - __uint_as_float(ph1 << 16), e11 - __uint_as_float(ph1 & 0xffff0000u));
-            mbar_wait(bar0 + 8 * sc, (parbits >> sc) & 1u);  // the group's V parts have landed
+            landed();  // the group's V parts have landed
             pv_group(acc, r_v, nb0, nb1, vb0, vb1, ph0, ph1, pl0, pl1, gq, qq);
             __syncwarp();  // every lane is done reading the slot
             ring_release();
