@@ -125,8 +125,9 @@ struct Split {
 // QK of one group in flight: S (16 tokens x 8 heads) += K q^T with the group's tokens = M (rows 0-7 = block 0, rows 8-15 =
 // block 1), heads = N, channels = K.  sp0 / sp1: the K parts of its blocks in shared memory; qa: q[head gq][32qq .. 32qq+31]
 // as B fragments.  Packed vectors are expanded straight into A fragments (mkv_walk.cuh); dense vectors skip the walk.
+// pairs: the vectors were kept in element groups g >= 2 and their values are stored pair-major (k_walk_mma_pairs).
 __device__ __forceinline__ void qk_group(float (&S)[4], int r_k, int nb0, int nb1, uint32_t sp0, uint32_t sp1,
-                                         const uint32_t (&qa)[8][2], int lane) {
+                                         const uint32_t (&qa)[8][2], int lane, bool pairs) {
     const int gq = lane >> 2, qq = lane & 3;
     const bool two = nb1 != 0;
     const bool full = nb0 == kPhys && (!two || nb1 == kPhys);
@@ -156,6 +157,16 @@ __device__ __forceinline__ void qk_group(float (&S)[4], int r_k, int nb0, int nb
             t = __shfl_up_sync(kFull, inc, 2); if (qq >= 2) inc += t;
             const uint32_t ex = inc - cnt;
             st0 = 2u * nb0; st1 = 2u * nb1;
+            if (pairs) {  // pair pi = rank / 2 of token t at byte 4 (pi n + t): the same 2 n bytes per kept element before it
+                p0 = sp0 + 16 * nb0 + st0 * (ex & 0xffffu) + 4 * gq;
+                p1 = sp1 + 16 * nb1 + st1 * (ex >> 16) + 4 * gq;
+                st0 *= 2u; st1 *= 2u;
+                k_walk_mma_pairs<0>(S, w0, w1, p0, p1, st0, st1, qa);
+                k_walk_mma_pairs<1>(S, w0, w1, p0, p1, st0, st1, qa);
+                k_walk_mma_pairs<2>(S, w0, w1, p0, p1, st0, st1, qa);
+                k_walk_mma_pairs<3>(S, w0, w1, p0, p1, st0, st1, qa);
+                return;
+            }
             p0 = sp0 + 16 * nb0 + st0 * (ex & 0xffffu) + 2 * gq;
             p1 = sp1 + 16 * nb1 + st1 * (ex >> 16) + 2 * gq;
         }
@@ -327,15 +338,15 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 else plan_lookup(g, lv, u, t0, off16, meta);
             }
         }
-        const uint32_t nb = meta >> 16, rk = meta & 255u, rv = (meta >> 8) & 255u;
+        const uint32_t nb = (meta >> 16) & 15u, rk = meta & 255u, rv = (meta >> 8) & 255u, kpairs = (meta >> 24) & 1u;
         const uint32_t kb = nb * vecb(rk);                      // bytes of the K part
         const uint32_t sk = updf ? 0u : (kb & 15u);             // bytes between the last 16-B boundary and the V part
         const uint32_t kc = (kb + 15u) >> 4, vc = (sk + nb * vecb(rv) + 15u) >> 4;  // 16-B units staged in phase 1 / 2
         const uint32_t voff = updf ? off16 : off16 + (kb >> 4);
         const uint32_t pmeta = __shfl_up_sync(kFull, meta, 1), pkc = __shfl_up_sync(kFull, kc, 1);
         const uint32_t pvc = __shfl_up_sync(kFull, vc, 1), pupd = __shfl_up_sync(kFull, updf, 1);
-        const bool follows = lane > 0 && lane < count && ((meta ^ pmeta) & 0xffffu) == 0u && nb != 0u &&
-                             (pmeta >> 16) != 0u && kc + pkc <= (uint32_t)kGroupMax16 && vc + pvc <= (uint32_t)kGroupMax16 &&
+        const bool follows = lane > 0 && lane < count && ((meta ^ pmeta) & 0x0100ffffu) == 0u && nb != 0u &&
+                             ((pmeta >> 16) & 15u) != 0u && kc + pkc <= (uint32_t)kGroupMax16 && vc + pvc <= (uint32_t)kGroupMax16 &&
                              !updf && !pupd;
         const unsigned fm = __ballot_sync(kFull, follows);
         const int start = 31 - __clz((int)(~fm & lanemask_le()));  // first block of this lane's run (bit 0 of ~fm is set)
@@ -350,7 +361,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             GDesc a, b;
             a.off0 = off16; a.off1 = two ? off1 : 0u;
             a.x = kc | ((two ? kc1 : 0u) << 8) | (nb << 16) | ((two ? nb1 : 0u) << 20) | (rk << 24);
-            a.y = updf;
+            a.y = updf | (kpairs << 1);
             b.off0 = voff; b.off1 = two ? voff1 : 0u;
             b.x = vc | ((two ? vc1 : 0u) << 8) | (sk << 16) | ((two ? sk1 : 0u) << 20) | (rv << 24);
             b.y = updf | (nb << 4) | ((two ? nb1 : 0u) << 8);
@@ -435,7 +446,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
                 const uint32_t c0 = (d.x & 255u) << 4, c1 = ((d.x >> 8) & 255u) << 4;
                 uint32_t off;
                 if (!ring_alloc(c0 + c1, off)) break;
-                stage(d.y ? reinterpret_cast<unsigned long long>(upd_k) : slice, off, d.off0, c0, d.off1, c1);
+                stage((d.y & 1u) ? reinterpret_cast<unsigned long long>(upd_k) : slice, off, d.off0, c0, d.off1, c1);
                 ring_commit();
                 ++gposi;
                 bposi += c1 ? 2 : 1;
@@ -467,7 +478,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             // ---- QK: S (tokens x heads); rows 0-7 = block 0, rows 8-15 = block 1
             if (nb0 != 0) {
                 float S[4] = {0.f, 0.f, 0.f, 0.f};
-                qk_group(S, r_k, nb0, nb1, sp0, sp1, qa, lane);
+                qk_group(S, r_k, nb0, nb1, sp0, sp1, qa, lane, (d.y & 2u) != 0u);
                 // ---- scaled logits of token gq of each block, heads 2qq, 2qq+1 -> cache [head][token]
                 const bool v0 = gq < nb0, v1 = gq < nb1;
                 const float zA0 = v0 ? S[0] * scale_log2 : -INFINITY, zB0 = v0 ? S[1] * scale_log2 : -INFINITY;
@@ -897,13 +908,14 @@ mkv_walk_probe_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q,
     const uint32_t sp0 = smem_u32(mine), sp1 = sp0 + 2048;
 #pragma unroll
     for (int i = 0; i < 2; ++i) {
-        const uint32_t nb = meta[i] >> 16, kb = (nb * vecb(meta[i] & 255u) + 15u) >> 4;  // 16-B units of the K part (<= 128)
+        const uint32_t nb = (meta[i] >> 16) & 15u, kb = (nb * vecb(meta[i] & 255u) + 15u) >> 4;  // 16-B units of the K part (<= 128)
         const uint4* src = reinterpret_cast<const uint4*>(lv.slice) + off[i];
         for (uint32_t x = lane; x < kb; x += 32) reinterpret_cast<uint4*>(mine + 2048 * i)[x] = __ldg(src + x);
     }
     __syncwarp();
     const int r_k = (int)(meta[0] & 255u);
-    const int nb0 = (int)(meta[0] >> 16), nb1 = (meta[1] & 255u) == (meta[0] & 255u) ? (int)(meta[1] >> 16) : 0;
+    const int nb0 = (int)((meta[0] >> 16) & 15u);
+    const int nb1 = ((meta[1] ^ meta[0]) & 0x010000ffu) == 0u ? (int)((meta[1] >> 16) & 15u) : 0;
     const size_t row = (size_t)(u / g.n_kv_heads) * g.n_q_heads + (size_t)(u % g.n_kv_heads) * g.group;
     uint32_t qa[8][2];
     {
@@ -919,7 +931,7 @@ mkv_walk_probe_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q,
 #pragma unroll 1
     for (int it = 0; it < reps; ++it) {
         float S[4] = {0.f, 0.f, 0.f, 0.f};
-        qk_group(S, r_k, nb0, nb1, sp0, sp1, qa, lane);
+        qk_group(S, r_k, nb0, nb1, sp0, sp1, qa, lane, (meta[0] >> 24) & 1u);
         acc += (S[0] + S[1]) + (S[2] + S[3]);
         qa[0][0] ^= __float_as_uint(acc) & 0x10000u;  // loop-carried: the walk cannot be hoisted out of the loop
     }

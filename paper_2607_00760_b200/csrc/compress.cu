@@ -109,8 +109,12 @@ __device__ __forceinline__ void topr_mask_groups(const uint32_t (&x)[4], int r, 
 // bm: this vector's bitmap; val: the GROUP's value area (2-byte aligned).
 // cached: a mask found earlier for this vector by mkv_segment_loss (or nullptr).  It is used only if it keeps r elements
 // and every kept magnitude is strictly above every dropped one -- then it IS the top-r mask, whatever wrote it.
+// pairs: K vectors and block keys kept in element groups g >= 2 store their values PAIR-major instead (the kept channels
+// come in aligned pairs; pair pi = rho / 2 of vector t sits at 32-bit element pi * n + t), so that the QK walk loads a whole
+// A-fragment register with one aligned LDS.32 (mkv_walk.cuh: k_walk_mma_pairs).  Same bytes, same bitmaps.
 __device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, int g, uint8_t* bm, uint8_t* val, int t, int n,
-                                            int lane, bool cached = false, uint4 cw = make_uint4(0u, 0u, 0u, 0u)) {
+                                            int lane, bool pairs, bool cached = false,
+                                            uint4 cw = make_uint4(0u, 0u, 0u, 0u)) {
     uint16_t* v16 = reinterpret_cast<uint16_t*>(val);
     if (r == kD) {
 #pragma unroll
@@ -142,7 +146,10 @@ __device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, int g
     int base = 0;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-        if ((w[j] >> lane) & 1u) v16[(base + __popc(w[j] & lt)) * n + t] = (uint16_t)x[j];
+        if ((w[j] >> lane) & 1u) {
+            const int rho = base + __popc(w[j] & lt);
+            v16[pairs ? ((rho >> 1) * n + t) * 2 + (rho & 1) : rho * n + t] = (uint16_t)x[j];
+        }
         base += __popc(w[j]);
     }
     if (lane < 8) {  // 2-byte stores: a ragged token block leaves the V bitmaps only 2-byte aligned
@@ -339,8 +346,8 @@ __global__ void __launch_bounds__(256, 4) mkv_compress_kernel(CacheGeom g, Layer
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j) sum[j] = __fadd_rn(sum[j], bf16_bits_to_f32(xk[j]));
-        pack_vector(xk, r_k, rec.g, k_bm + t * bmk, k_val, t, nb, lane, mk && r_k != kD, cached_mask(t, 0));
-        pack_vector(xv, r_v, rec.g, v_bm + t * bmv, v_val, t, nb, lane, mk && r_v != kD, cached_mask(t, 1));
+        pack_vector(xk, r_k, rec.g, k_bm + t * bmk, k_val, t, nb, lane, rec.g >= 2, mk && r_k != kD, cached_mask(t, 0));
+        pack_vector(xv, r_v, rec.g, v_bm + t * bmv, v_val, t, nb, lane, false, mk && r_v != kD, cached_mask(t, 1));
     }
     {
         const uint32_t used = (uint32_t)nb * (vec_bytes(r_k) + vec_bytes(r_v));
@@ -371,7 +378,7 @@ __global__ void __launch_bounds__(256, 4) mkv_compress_kernel(CacheGeom g, Layer
         for (int j = 0; j < 4; ++j) x[j] = f32_to_bf16_bits_rne(__fdiv_rn(sum[j], fnb));
         // the block keys of a segment form groups of 8 (one work item of the score kernel each)
         const int grp = lb >> 3, gn = min(8, nlb - 8 * grp);
-        pack_vector(x, r_k, rec.g, bk_base + lb * bmk, bk_base + nlb * bmk + (size_t)grp * 8 * r_k * 2, lb & 7, gn, lane);
+        pack_vector(x, r_k, rec.g, bk_base + lb * bmk, bk_base + nlb * bmk + (size_t)grp * 8 * r_k * 2, lb & 7, gn, lane, rec.g >= 2);
         if (lb == nlb - 1) {
             const uint32_t used = (uint32_t)nlb * vec_bytes(r_k);
             const uint32_t padded = pad16u(used);

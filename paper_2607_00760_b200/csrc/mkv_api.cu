@@ -658,7 +658,8 @@ int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, vo
     // block of 16 tokens is stored as two device blocks).  Device group: its vectors' bitmaps of 128 bits (one bit per
     // channel, every channel of a kept element group set), then the kept values RANK-major (compress.cu).  Canonical: n
     // bitmaps of D / g bits (one per element group), then the values vector-major.  Dense vectors (r = D): values only.
-    auto repack = [](const uint8_t* src0, int n0, const uint8_t* src1, int n1, uint8_t* dst, int r, int gg) {
+    // pairs: K vectors and block keys with g >= 2 hold their values pair-major (compress.cu: pack_vector).
+    auto repack = [](const uint8_t* src0, int n0, const uint8_t* src1, int n1, uint8_t* dst, int r, int gg, bool pairs) {
         const int n = n0 + n1;
         if (r == kD) {
             memcpy(dst, src0, (size_t)n0 * kD * 2);
@@ -675,7 +676,10 @@ int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, vo
                 if ((src[tt * kBitmapBytes + (c >> 3)] >> (c & 7)) & 1) dst[t * bmc + (m >> 3)] |= (uint8_t)(1u << (m & 7));
             }
             const uint8_t* v = src + (size_t)nn * kBitmapBytes;  // rank-major values of the device group
-            for (int rho = 0; rho < r; ++rho) memcpy(o + 2 * ((size_t)t * r + rho), v + 2 * ((size_t)rho * nn + tt), 2);
+            for (int rho = 0; rho < r; ++rho) {
+                const size_t at = pairs ? ((size_t)(rho >> 1) * nn + tt) * 2 + (rho & 1) : (size_t)rho * nn + tt;
+                memcpy(o + 2 * ((size_t)t * r + rho), v + 2 * at, 2);
+            }
         }
     };
     uint64_t tpos = 0, kpos = 0;            // canonical positions
@@ -695,9 +699,9 @@ int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, vo
             const uint8_t* s0 = tp;
             const uint8_t* s1 = tp + tokblock_bytes(r_k, r_v, n0);
             uint8_t* d = tok_arena + tpos;
-            repack(s0, n0, s1, n1, d, r_k, gg);                                                                     // K vectors
+            repack(s0, n0, s1, n1, d, r_k, gg, gg >= 2);                                                            // K vectors
             repack(s0 + (size_t)n0 * (bmk + 2 * r_k), n0, s1 + (size_t)n1 * (bmk + 2 * r_k), n1,
-                   d + (size_t)nbt * vbc(r_k, gg), r_v, gg);                                                        // V vectors
+                   d + (size_t)nbt * vbc(r_k, gg), r_v, gg, false);                                                 // V vectors
             tp += tokblock_bytes(r_k, r_v, n0) + (n1 ? tokblock_bytes(r_k, r_v, n1) : 0u);
             tpos += tokc(r, nbt);
         }
@@ -713,7 +717,7 @@ int mkv_cache_export(const mkv_cache* c, int32_t layer, int32_t b, int32_t h, vo
                 std::vector<uint8_t> tmp((size_t)n * kBitmapBytes + (size_t)n * r_k * 2), outg((size_t)n * bmc + (size_t)n * r_k * 2);
                 memcpy(tmp.data(), kp + (size_t)grp * 8 * kBitmapBytes, (size_t)n * kBitmapBytes);
                 memcpy(tmp.data() + (size_t)n * kBitmapBytes, kp + (size_t)nblk * kBitmapBytes + (size_t)grp * 8 * r_k * 2, (size_t)n * r_k * 2);
-                repack(tmp.data(), n, nullptr, 0, outg.data(), r_k, gg);
+                repack(tmp.data(), n, nullptr, 0, outg.data(), r_k, gg, gg >= 2);
                 memcpy(d + (size_t)grp * 8 * bmc, outg.data(), (size_t)n * bmc);
                 memcpy(d + (size_t)nblk * bmc + (size_t)grp * 8 * r_k * 2, outg.data() + (size_t)n * bmc, (size_t)n * r_k * 2);
             }

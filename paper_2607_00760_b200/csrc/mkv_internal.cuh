@@ -102,7 +102,8 @@ constexpr int kTopkSlice = 16384;  // blocks per top-k slice (select.cu); longer
 struct __align__(16) PlanRec {
     int32_t t0;      // first token of the block
     uint32_t off16;  // payload offset in the layer slice, 16-B units
-    uint32_t meta;   // r_k | r_v << 8 | nb << 16   (nb = tokens in the device block, 1..8)
+    uint32_t meta;   // r_k | r_v << 8 | nb << 16 | (g >= 2) << 24   (nb = tokens in the device block, 1..8; bit 24: the
+                     // K values are stored pair-major, see mkv_walk.cuh)
     uint32_t tag;    // plan_tag(generation, layer); 0 = never written
 };
 __host__ __device__ inline uint32_t plan_tag(uint32_t generation, int layer) {
@@ -120,7 +121,7 @@ __device__ __forceinline__ void plan_lookup(const CacheGeom& g, const LayerView&
     if ((int)rec.n_tok <= in_seg) return;
     const uint32_t nb = (uint32_t)min(g.pb, (int)rec.n_tok - in_seg);
     off16 = lv.tok_off[e] + (uint32_t)(in_seg / g.pb) * (tokblock_bytes(rec.r_k, rec.r_v, g.pb) >> 4);
-    meta = (uint32_t)rec.r_k | ((uint32_t)rec.r_v << 8) | (nb << 16);
+    meta = (uint32_t)rec.r_k | ((uint32_t)rec.r_v << 8) | (nb << 16) | (rec.g >= 2 && rec.r_k != kD ? 1u << 24 : 0u);
 }
 #endif
 

@@ -144,6 +144,34 @@ __device__ __forceinline__ void k_walk_mma(float (&S)[4], uint32_t w0, uint32_t 
              qa[2 * BYTE + 1][1]);
 }
 
+// K walk of vectors kept in element groups g = 2 or 4: the kept channels come in aligned pairs, the
+// values of a group of vectors are stored PAIR-major (pair pi of vector t at 32-bit element pi * n + t, compress.cu), and
+// a pair (c, c + 1) of one token IS one A-fragment register.  Byte BYTE of the (one bit per channel) bitmap word holds
+// four pairs: a set even bit loads the pair with one aligned LDS.32 and advances the run pointer by `step` = 4 n bytes.
+// Half the slots of the g = 1 walk, no packing of two halves.
+template <int BYTE>
+__device__ __forceinline__ void walk4_pairs(uint32_t w, uint32_t& ptr, uint32_t step, uint32_t (&v)[4]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        v[i] = 0u;
+        if (w & (1u << (8 * BYTE + 2 * i))) {
+            v[i] = lds_u32(ptr);
+            ptr += step;
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) asm volatile("" : "+r"(v[i]));
+}
+template <int BYTE>
+__device__ __forceinline__ void k_walk_mma_pairs(float (&S)[4], uint32_t w0, uint32_t w1, uint32_t& p0, uint32_t& p1,
+                                                 uint32_t st0, uint32_t st1, const uint32_t (&qa)[8][2]) {
+    uint32_t e[4], f[4];
+    walk4_pairs<BYTE>(w0, p0, st0, e);
+    walk4_pairs<BYTE>(w1, p1, st1, f);
+    mma_bf16(S, e[0], f[0], e[1], f[1], qa[2 * BYTE][0], qa[2 * BYTE][1]);
+    mma_bf16(S, e[2], f[2], e[3], f[3], qa[2 * BYTE + 1][0], qa[2 * BYTE + 1][1]);
+}
+
 // V walk: byte BYTE (8 channels of this lane's 16-channel half-word) of four runs -- tokens
 // A = 2qq and B = 2qq+1 of block 0 and of block 1 -- feeds four M tiles of O^T += V^T P^T with P
 // split into bf16 hi (ph) and lo (pl).  A register pairs two TOKENS of one channel.

@@ -6,9 +6,10 @@
 //     pairs (16 keys = the M of one mma.sync tile); the items of all units form one stream that is
 //     cut into equal contiguous ranges, one per warp of a one-CTA-per-SM grid.  Warps are
 //     independent (no __syncthreads at all).
-//   * Staging: an item's position bitmaps and its kept values (DESIGN.md format) are two contiguous
-//     16-B-aligned chunks; one lane moves each with ONE 1-D bulk copy (cp.async.bulk, the TMA
-//     engine) that completes on the stage's mbarrier; kStages groups are in flight per warp.
+//   * Staging: an item's position bitmaps and its kept values (DESIGN.md format) are contiguous
+//     16-B-aligned chunks (usually the whole pair is one); every lane moves 16 bytes at a time with
+//     cp.async, one commit group per stage, NSTAGE groups in flight per warp.  Full dense items are
+//     placed with their 16-byte chunks swizzled so that the LDS.128 path has no bank conflicts.
 //   * The packed keys are expanded straight into mma.sync A fragments by the same walk as
 //     PackedAttention's QK (mkv_walk.cuh): S = Kbar q^T, keys = M, heads = N, channels = K, fp32
 //     accumulate; the group reduction (max or sum over the G heads) is two shuffles.
@@ -30,7 +31,8 @@ constexpr uint32_t kPairMaxR = 56;  // 128 + 16 r_k <= kItem1
 struct __align__(16) SDesc {
     uint32_t bm0, val0, bm1, val1;  // chunk offsets in the layer slice, 16-B units (dense: bm = the keys, val unused)
     uint32_t out0, out1;            // index of each item's first score: unit * score_stride + block index
-    uint32_t meta;                  // r_k | nb0 << 8 | nb1 << 12 | merged << 16: the group is ONE contiguous chunk of the slice
+    uint32_t meta;                  // r_k | nb0 << 8 | nb1 << 12 | merged << 16 (the group is ONE contiguous chunk of the slice)
+                                    // | its size / 16 << 17 | pairs << 30 (element groups g >= 2: values pair-major, mkv_walk.cuh)
     uint32_t unit;
 };
 
@@ -81,7 +83,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
     // follows item i - 1 in a group if both hold keys, belong to one unit and have the same r_k;
     // runs of such items are paired greedily from their start.  Items past a unit's end hold no keys.
     auto build = [&](int count) {
-        uint32_t bm = 0u, val = 0u, out = 0u, r_k = 0u, nb = 0u, u = 0u;
+        uint32_t bm = 0u, val = 0u, out = 0u, r_k = 0u, nb = 0u, u = 0u, pairs = 0u;
         uint32_t sz = 0u;  // 16-B units of the item when its bitmaps and values are one chunk (one item per segment), else 0
         if (lane < count) {
             const unsigned it = lo + (unsigned)(ibuilt + lane);
@@ -97,6 +99,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                 if (n > 0) {
                     const uint32_t off = lv.bk_off[e];
                     r_k = rec.r_k; nb = (uint32_t)n;
+                    pairs = rec.g >= 2 && rec.r_k != kD ? 1u : 0u;
                     if (rec.r_k == kD) { bm = off + 128u * sub; val = bm; }
                     else { bm = off + 8u * sub; val = off + (uint32_t)nblk + (uint32_t)rec.r_k * sub; }
                     out = u * (unsigned)g.score_stride + seg * (unsigned)g.blocks_per_seg + 8u * sub;
@@ -104,8 +107,8 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                 }
             }
         }
-        const uint32_t pu = __shfl_up_sync(kFull, u, 1), prk = __shfl_up_sync(kFull, r_k, 1), pnb = __shfl_up_sync(kFull, nb, 1);
-        const bool follows = lane > 0 && nb != 0u && pnb != 0u && u == pu && r_k == prk && r_k <= kPairMaxR;  // two items must fit one stage
+        const uint32_t pu = __shfl_up_sync(kFull, u, 1), prk = __shfl_up_sync(kFull, r_k | (pairs << 8), 1), pnb = __shfl_up_sync(kFull, nb, 1);
+        const bool follows = lane > 0 && nb != 0u && pnb != 0u && u == pu && (r_k | (pairs << 8)) == prk && r_k <= kPairMaxR;  // two items must fit one stage
         const unsigned fm = __ballot_sync(kFull, follows);
         const int start = 31 - __clz((int)(~fm & lanemask_le()));  // first item of this lane's run (bit 0 of ~fm is set)
         const bool first = nb != 0u && ((lane - start) & 1) == 0;
@@ -120,7 +123,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             SDesc d;
             d.bm0 = bm; d.val0 = val; d.bm1 = two ? bm1 : 0u; d.val1 = two ? val1 : 0u;
             d.out0 = out; d.out1 = two ? out1 : 0u;
-            d.meta = r_k | (nb << 8) | ((two ? nb1 : 0u) << 12) | (merged ? (1u << 16) | ((sz + sz1) << 17) : 0u);
+            d.meta = r_k | (nb << 8) | ((two ? nb1 : 0u) << 12) | (merged ? (1u << 16) | ((sz + sz1) << 17) : 0u) | (pairs << 30);
             d.unit = u;
             ring[(gbuilt + __popc(gm & lanemask_lt())) & (kRing - 1)] = d;
         }
@@ -144,7 +147,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             const SDesc d = ring[gposi & (kRing - 1)];
             const uint32_t dst = stage0 + s * kScoreStage;
             if (d.meta & (1u << 16)) {  // item 1 lands right behind item 0: one chunk
-                copy_chunk(dst, d.bm0, (d.meta >> 17) << 4);
+                copy_chunk(dst, d.bm0, ((d.meta >> 17) & 0xffu) << 4);
             } else {
                 const uint32_t r = d.meta & 255u, nb0 = (d.meta >> 8) & 15u, nb1 = (d.meta >> 12) & 15u;
                 // bitmaps nb x 16 B, then the values padded to 16 B; dense: nb x 256 B in one chunk
@@ -196,7 +199,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             }
             const int r_k = (int)(d.meta & 255u), nb0 = (int)((d.meta >> 8) & 15u), nb1 = (int)((d.meta >> 12) & 15u);
             const uint32_t sp0 = stage0 + s * kScoreStage;
-            const uint32_t sp1 = sp0 + ((d.meta >> 16) ? 16u * (uint32_t)nb0 + pad16u(2u * (uint32_t)(nb0 * r_k)) : (uint32_t)kItem1);
+            const uint32_t sp1 = sp0 + (((d.meta >> 16) & 1u) ? 16u * (uint32_t)nb0 + pad16u(2u * (uint32_t)(nb0 * r_k)) : (uint32_t)kItem1);
 
             cp_async_wait<NSTAGE - 1>();  // this lane's copies of the group have landed ...
             __syncwarp();                 // ... and every other lane's
@@ -228,10 +231,19 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                     p0 = sp0 + 16 * nb0 + st0 * (ex & 0xffffu) + 2 * gq;
                     p1 = sp1 + 16 * nb1 + st1 * (ex >> 16) + 2 * gq;
                 }
-                k_walk_mma<0>(S, w0, w1, p0, p1, st0, st1, qa);
-                k_walk_mma<1>(S, w0, w1, p0, p1, st0, st1, qa);
-                k_walk_mma<2>(S, w0, w1, p0, p1, st0, st1, qa);
-                k_walk_mma<3>(S, w0, w1, p0, p1, st0, st1, qa);
+                if ((d.meta >> 30) & 1u) {  // element groups g >= 2: pair pi = rank / 2 of key t at byte 4 (pi n + t)
+                    p0 += 2 * gq; p1 += 2 * gq;
+                    st0 *= 2u; st1 *= 2u;
+                    k_walk_mma_pairs<0>(S, w0, w1, p0, p1, st0, st1, qa);
+                    k_walk_mma_pairs<1>(S, w0, w1, p0, p1, st0, st1, qa);
+                    k_walk_mma_pairs<2>(S, w0, w1, p0, p1, st0, st1, qa);
+                    k_walk_mma_pairs<3>(S, w0, w1, p0, p1, st0, st1, qa);
+                } else {
+                    k_walk_mma<0>(S, w0, w1, p0, p1, st0, st1, qa);
+                    k_walk_mma<1>(S, w0, w1, p0, p1, st0, st1, qa);
+                    k_walk_mma<2>(S, w0, w1, p0, p1, st0, st1, qa);
+                    k_walk_mma<3>(S, w0, w1, p0, p1, st0, st1, qa);
+                }
             }
             __syncwarp();  // every lane is done reading stage s
 
