@@ -381,6 +381,8 @@ def run_mkv(args):
     if rank == 0:
         line["update_buffer"] = measure_update_buffer(torch, mkv, synth, w, dev, Bt, cache, built, step_attention,
                                                       n_layers, graph, args)
+    if rank == 0 and world == 1:
+        line["element_groups_g2"] = measure_element_groups(torch, workload, w, dev, Bt, N, args, graph, us_attn, us_sel)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args, w, built, dev, n_units=args.cpu_units, repeats=1)
     built.free()
@@ -426,6 +428,42 @@ def measure_update_buffer(torch, mkv, synth, w, dev, Bt, cache, built, step_atte
     cache.status()
     res["attention_us_per_layer_with_32_buffered_tokens"] = round(ms * 1e3 / n_layers, 3)
     return res
+
+
+def measure_element_groups(torch, workload, w, dev, Bt, N, args, graph, us_attn_g1, us_sel_g1):
+    """The same workload compressed with element groups g = 2 (one of the paper's candidate group
+    sizes), six layers cycled (touched set > L2): K values and block keys are stored pair-major and the QK walk loads one
+    aligned 32-bit pair per kept group.  Printed BESIDE the g = 1 headline; the north-star config is g = 1."""
+    NL = 6
+    scale = 1.0 / math.sqrt(128)
+    built = workload.build(w, dev, n_layers=NL, batch=Bt, context=N, g=2)
+    try:
+        cache, Hkv, Hq, budget = built.cache, w.n_kv_heads, w.n_q_heads, w.token_budget
+        k_max = min(budget // 8 + 1, (N + 7) // 8)
+        sel = [torch.full((Bt, Hkv, k_max), -1, dtype=torch.int32, device=dev) for _ in range(NL)]
+        cnt = [torch.zeros((Bt, Hkv), dtype=torch.int32, device=dev) for _ in range(NL)]
+        out = torch.zeros((NL, Bt, Hq, 128), dtype=torch.float32, device=dev)
+
+        def step_select():
+            for l in range(NL):
+                cache.select(l, built.q[l], budget, sel[l], cnt[l])
+
+        def step_attention():
+            for l in range(NL):
+                cache.packed_attention(l, built.q[l], sel[l], cnt[l], scale, out[l])
+
+        step_select()
+        torch.cuda.synchronize()
+        ms_a = timed_loop(torch, step_attention, args.steps, args.warmup, lambda: None, graph)
+        ms_s = timed_loop(torch, step_select, args.steps, args.warmup, lambda: None, graph)
+        cache.status()
+        comp = [sum(x[i] for x in built.compress_ms[1:]) / max(1, len(built.compress_ms) - 1) for i in range(3)]
+        return {"g": 2, "n_layers": NL, "attention_us_per_layer": round(ms_a * 1e3 / NL, 3),
+                "select_us_per_layer": round(ms_s * 1e3 / NL, 3),
+                "attention_vs_g1": round(ms_a * 1e3 / NL / us_attn_g1, 3), "select_vs_g1": round(ms_s * 1e3 / NL / us_sel_g1, 3),
+                "loss_ms_per_layer": round(comp[0], 3), "compress_ms_per_layer": round(comp[2], 3)}
+    finally:
+        built.free()
 
 
 # ------------------------------------------------------------------------------ the oracle legs

@@ -47,10 +47,11 @@ class BuiltCache:
 
 
 def build(w: synth.Workload, dev, n_layers=None, batch=None, context=None, keep_units=(), keep_loss=False,
-          verbose=False) -> BuiltCache:
+          verbose=False, g=1) -> BuiltCache:
     """Generate (seeded, on the device), choose strategies (quantile rule) and compress every layer.
 
     keep_units: iterable of (layer, b, h) whose raw K/V bytes are copied to the host for the oracle.
+    g: element-group size of the sparse strategy (r_keep must be a multiple of it).
     """
     import numpy as np
     import torch
@@ -73,12 +74,12 @@ def build(w: synth.Workload, dev, n_layers=None, batch=None, context=None, keep_
         strat = torch.empty((Bt, Hkv, S, 4), dtype=torch.uint8, device=dev)
         ev[0].record()
         if w.dense_num > 0:
-            cache.segment_loss(K, V, (r, r, 1, 8), loss_k, loss_v)
+            cache.segment_loss(K, V, (r, r, g, 8), loss_k, loss_v)
         ev[1].record()
         if w.dense_num > 0:
-            cache.strategy_quantile(loss_k, loss_v, S, w.dense_num, w.dense_den, (r, r, 1, 8), strat)
+            cache.strategy_quantile(loss_k, loss_v, S, w.dense_num, w.dense_den, (r, r, g, 8), strat)
         else:
-            strat[:] = torch.tensor([r, r, 1, 8], dtype=torch.uint8, device=dev)
+            strat[:] = torch.tensor([r, r, g, 8], dtype=torch.uint8, device=dev)
         ev[2].record()
         cache.compress_segment(layer, K, V, strat)
         ev[3].record()
