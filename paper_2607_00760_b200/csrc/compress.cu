@@ -30,6 +30,8 @@ __device__ __forceinline__ void topr_mask(const uint32_t (&mag)[4], int r, uint3
     // two 15-bit magnitudes per register with bit 15 / 31 set: (pair - cand x 0x10001) keeps that bit exactly
     // where mag >= cand, and no borrow crosses the halves -- four compares in two subtractions
     const uint32_t p01 = mag[0] | (mag[1] << 16) | 0x80008000u, p23 = mag[2] | (mag[3] << 16) | 0x80008000u;
+    // (as soon as exactly r magnitudes lie at or above a candidate they ARE the top r: no lower bit can change the set,
+    // and no tie straddles its edge -- the warp-uniform early exit saves the last steps of most searches)
 #pragma unroll
     for (int bit = 14; bit >= 0; --bit) {
         const uint32_t cand = T | (1u << bit);
@@ -37,6 +39,11 @@ __device__ __forceinline__ void topr_mask(const uint32_t (&mag)[4], int r, uint3
         const uint32_t z = ((p01 - c2) & 0x80008000u) | (((p23 - c2) >> 1) & 0x40004000u);
         const int c = __reduce_add_sync(kFull, __popc(z));
         if (c >= r) T = cand;
+        if (c == r) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) w[j] = __ballot_sync(kFull, mag[j] >= cand);
+            return;
+        }
     }
     int ngt = (mag[0] > T) + (mag[1] > T) + (mag[2] > T) + (mag[3] > T);
     ngt = __reduce_add_sync(kFull, ngt);
@@ -81,7 +88,16 @@ __device__ __forceinline__ void topr_mask_groups(const uint32_t (&x)[4], int r, 
         const uint32_t cand = T | (1u << bit);
         int c = 0;
         if (leader) c = (key[0] >= cand) + (key[1] >= cand) + (key[2] >= cand) + (key[3] >= cand);
-        if (__reduce_add_sync(kFull, c) >= nk) T = cand;
+        c = __reduce_add_sync(kFull, c);
+        if (c >= nk) T = cand;
+        if (c == nk) {  // exactly r / g groups at or above the candidate: they are the kept set (see topr_mask)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const unsigned kl = __ballot_sync(kFull, leader && key[j] >= cand);
+                w[j] = kl | (kl << 1) | (g == 4 ? (kl << 2) | (kl << 3) : 0u);
+            }
+            return;
+        }
     }
     int ngt = 0;
     if (leader) ngt = (key[0] > T) + (key[1] > T) + (key[2] > T) + (key[3] > T);
