@@ -160,13 +160,21 @@ __device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, int g
     }
     const unsigned lt = lanemask_lt();
     int base = 0;
+    if (!pairs) {  // (warp-uniform: two tight loops instead of one with a select per element)
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        if ((w[j] >> lane) & 1u) {
-            const int rho = base + __popc(w[j] & lt);
-            v16[pairs ? ((rho >> 1) * n + t) * 2 + (rho & 1) : rho * n + t] = (uint16_t)x[j];
+        for (int j = 0; j < 4; ++j) {
+            if ((w[j] >> lane) & 1u) v16[(base + __popc(w[j] & lt)) * n + t] = (uint16_t)x[j];
+            base += __popc(w[j]);
         }
-        base += __popc(w[j]);
+    } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if ((w[j] >> lane) & 1u) {
+                const int rho = base + __popc(w[j] & lt);
+                v16[((rho >> 1) * n + t) * 2 + (rho & 1)] = (uint16_t)x[j];
+            }
+            base += __popc(w[j]);
+        }
     }
     if (lane < 8) {  // 2-byte stores: a ragged token block leaves the V bitmaps only 2-byte aligned
         const int j = lane >> 1;

@@ -1123,6 +1123,34 @@ def test_guard_bands_around_every_output(env):
         c.free()
 
 
+def test_calibration_calls_run_and_leave_the_cache_intact(env):
+    """the measurement aids (mkv_calibrate_stream / _gather / _walk: SURVEY 8(d) calibration rows) take the same selection
+    as the decode calls, write nothing a decode call reads, and work on g = 1 and g = 2 caches (pair walk)."""
+    mkv, dev = env
+    import torch
+    for g in (1, 2):
+        c = Case(mkv, dev, 2, 2, 8, 64 * 9 + 5, seed=151 + g)
+        try:
+            strat = uniform_strat(2, 2, c.S, 38)
+            strat[:, :, :, 2] = g
+            strat[:, :, 2::4, 0:2] = 128
+            c.compress(strat)
+            c.assert_export_equal()
+            sel, cnt, _ = c.gpu_select(256)
+            before = c.gpu_attention(sel, cnt)
+            sel_d = torch.from_numpy(sel).to(dev)
+            cnt_d = torch.from_numpy(cnt).to(dev)
+            c.cache.calibrate_stream(0, 1 << 16)
+            c.cache.calibrate_gather(0, sel_d, cnt_d)
+            c.cache.calibrate_walk(0, c.q_d, sel_d, cnt_d, 3)
+            torch.cuda.synchronize()
+            c.cache.status()
+            after = c.gpu_attention(sel, cnt)
+            assert np.array_equal(before[0], after[0])
+        finally:
+            c.free()
+
+
 def test_zz_report_lse_ulps(env):
     """runs last: the largest lse error, in fp32 spacings of |lse| beyond the 1e-3 absolute term, seen by this session"""
     import gpu_util
