@@ -354,6 +354,26 @@ def test_other_segment_lengths_end_to_end(env, L):
         c.free()
 
 
+@pytest.mark.parametrize("Bt,Hkv", [(5, 4), (10, 4), (20, 4), (38, 4)])
+def test_attention_every_cluster_size(env, Bt, Hkv):
+    """PackedAttention runs one cluster of C CTAs per unit, C = the largest power of two with units x C <= SMs: 20 units ->
+    4 (pulled combine), 40 -> 2 (pushed combine), 80 and 152 -> 1 (no peer; 152 units are more CTAs than SMs).  The other
+    tests only reach C = 8 / 16 (a handful of units) and C = 2 (full-size configs)."""
+    mkv, dev = env
+    N = 64 * 6 + 11
+    c = Case(mkv, dev, Bt, Hkv, 2 * Hkv, N, seed=500 + Bt)
+    try:
+        strat = uniform_strat(Bt, Hkv, c.S, 38)
+        strat[:, :, 1::3, 0:2] = 128
+        c.compress(strat)
+        sel, cnt = c.oracle_sel(160)
+        c.check_attention(sel, cnt)
+        sel, cnt = c.oracle_sel(N)
+        c.check_attention(sel, cnt)
+    finally:
+        c.free()
+
+
 @pytest.mark.parametrize("seed", range(8))
 def test_attention_random_selections(env, seed):
     """random unit shapes and selections: odd counts (units then start at odd stream positions), empty units,
