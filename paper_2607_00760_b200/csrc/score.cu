@@ -146,8 +146,12 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
         if (gposi != gbuilt) {
             const SDesc d = ring[gposi & (kRing - 1)];
             const uint32_t dst = stage0 + s * kScoreStage;
-            if (d.meta & (1u << 16)) {  // item 1 lands right behind item 0: one chunk
-                copy_chunk(dst, d.bm0, ((d.meta >> 17) & 0xffu) << 4);
+            if (d.meta & (1u << 16)) {  // item 1 lands right behind item 0: one chunk of <= kScoreStage bytes
+                const uint32_t bytes = ((d.meta >> 17) & 0xffu) << 4, x = 16u * (uint32_t)lane;
+                const unsigned long long src = slice + ((unsigned long long)d.bm0 << 4) + x;
+#pragma unroll
+                for (uint32_t i = 0; i < (kScoreStage + 511) / 512; ++i)  // (straight line: constant offsets, no loop counter)
+                    if (x + 512u * i < bytes) cp_async_16(dst + x + 512u * i, src + 512u * i);
             } else {
                 const uint32_t r = d.meta & 255u, nb0 = (d.meta >> 8) & 15u, nb1 = (d.meta >> 12) & 15u;
                 // bitmaps nb x 16 B, then the values padded to 16 B; dense: nb x 256 B in one chunk
@@ -254,17 +258,15 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
                 v0 = (hA ? S[0] : 0.f) + (hB ? S[1] : 0.f);
                 v1 = (hA ? S[2] : 0.f) + (hB ? S[3] : 0.f);
                 v0 += __shfl_xor_sync(kFull, v0, 1); v1 += __shfl_xor_sync(kFull, v1, 1);
-                v0 += __shfl_xor_sync(kFull, v0, 2); v1 += __shfl_xor_sync(kFull, v1, 2);
+                if (G > 4) { v0 += __shfl_xor_sync(kFull, v0, 2); v1 += __shfl_xor_sync(kFull, v1, 2); }  // (G <= 4: lanes qq = 2, 3 hold nothing)
             } else {
                 v0 = fmaxf(hA ? S[0] : -INFINITY, hB ? S[1] : -INFINITY);
                 v1 = fmaxf(hA ? S[2] : -INFINITY, hB ? S[3] : -INFINITY);
                 v0 = fmaxf(v0, __shfl_xor_sync(kFull, v0, 1)); v1 = fmaxf(v1, __shfl_xor_sync(kFull, v1, 1));
-                v0 = fmaxf(v0, __shfl_xor_sync(kFull, v0, 2)); v1 = fmaxf(v1, __shfl_xor_sync(kFull, v1, 2));
+                if (G > 4) { v0 = fmaxf(v0, __shfl_xor_sync(kFull, v0, 2)); v1 = fmaxf(v1, __shfl_xor_sync(kFull, v1, 2)); }
             }
-            if (qq == 0) {
-                if (gq < nb0) scores[d.out0 + gq] = v0 + 0.0f;
-                if (gq < nb1) scores[d.out1 + gq] = v1 + 0.0f;
-            }
+            // (after the reduction every lane of a row holds both results: lane qq = 0 stores item 0's, qq = 1 item 1's)
+            if (qq < 2 && gq < (qq == 0 ? nb0 : nb1)) scores[(qq == 0 ? d.out0 : d.out1) + gq] = (qq == 0 ? v0 : v1) + 0.0f;
             ++gposc;
         }
         issue(s);  // stage s is free (or, for k < 0, still empty): start the copies of group k + NSTAGE
