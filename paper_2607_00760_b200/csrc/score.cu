@@ -33,7 +33,7 @@ struct __align__(16) SDesc {
     uint32_t out0, out1;            // index of each item's first score: unit * score_stride + block index
     uint32_t meta;                  // r_k | nb0 << 8 | nb1 << 12 | merged << 16 (the group is ONE contiguous chunk of the slice)
                                     // | its size / 16 << 17 | pairs << 30 (element groups g >= 2: values pair-major, mkv_walk.cuh)
-    uint32_t unit;
+    uint32_t unit;                  // unit | (stage offset of item 1 / 16) << 24
 };
 
 __device__ __forceinline__ unsigned lanemask_le() {
@@ -124,7 +124,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             d.bm0 = bm; d.val0 = val; d.bm1 = two ? bm1 : 0u; d.val1 = two ? val1 : 0u;
             d.out0 = out; d.out1 = two ? out1 : 0u;
             d.meta = r_k | (nb << 8) | ((two ? nb1 : 0u) << 12) | (merged ? (1u << 16) | ((sz + sz1) << 17) : 0u) | (pairs << 30);
-            d.unit = u;
+            d.unit = u | ((merged ? sz : (uint32_t)(kItem1 / 16)) << 24);  // (units < 2^24: checked by the launcher)
             ring[(gbuilt + __popc(gm & lanemask_lt())) & (kRing - 1)] = d;
         }
         gbuilt += __popc(gm);
@@ -189,8 +189,8 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
         if (k >= 0) {
             if (gposc == gbuilt) break;  // issue() runs ahead: nothing described means nothing left
             const SDesc d = ring[gposc & (kRing - 1)];
-            if ((int)d.unit != cur_unit) {
-                cur_unit = (int)d.unit;
+            if ((int)(d.unit & 0xffffffu) != cur_unit) {
+                cur_unit = (int)(d.unit & 0xffffffu);
                 const int bi = cur_unit / g.n_kv_heads, hk = cur_unit % g.n_kv_heads;
                 const uint4* qrow = reinterpret_cast<const uint4*>(
                     q + ((size_t)bi * g.n_q_heads + (size_t)hk * G + gq) * kD + 32 * qq);
@@ -203,7 +203,7 @@ mkv_score_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q, int 
             }
             const int r_k = (int)(d.meta & 255u), nb0 = (int)((d.meta >> 8) & 15u), nb1 = (int)((d.meta >> 12) & 15u);
             const uint32_t sp0 = stage0 + s * kScoreStage;
-            const uint32_t sp1 = sp0 + (((d.meta >> 16) & 1u) ? 16u * (uint32_t)nb0 + pad16u(2u * (uint32_t)(nb0 * r_k)) : (uint32_t)kItem1);
+            const uint32_t sp1 = sp0 + ((d.unit >> 24) << 4);
 
             cp_async_wait<NSTAGE - 1>();  // this lane's copies of the group have landed ...
             __syncwarp();                 // ... and every other lane's
@@ -284,7 +284,7 @@ static cudaError_t launch_score_cfg(const CacheGeom& g, const LayerView& lv, con
     cudaError_t e = cudaFuncSetAttribute(mkv_score_kernel<NSTAGE, NWARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     const int subs = (g.blocks_per_seg + 7) / 8;
-    if ((unsigned long long)g.n_units * g.S_max * subs >= (1ull << 32)) return cudaErrorInvalidValue;
+    if ((unsigned long long)g.n_units * g.S_max * subs >= (1ull << 32) || g.n_units >= (1 << 24)) return cudaErrorInvalidValue;
     return launch_pdl(mkv_score_kernel<NSTAGE, NWARPS>, dim3(sm_count), dim3(NWARPS * 32), (size_t)smem, s, g, lv, q, reduce,
                       subs, (unsigned)g.S_max * (unsigned)subs, scores);
 }
