@@ -65,8 +65,8 @@ __device__ __forceinline__ void topr_mask(const uint32_t (&mag)[4], int r, uint3
 // (R4; the squares of bf16 values are exact in fp32), ties -> lower group.  x[j]: bf16 bits of channel
 // lane + 32 j, so a group lives in g adjacent lanes of one j.  Returns the mask EXPANDED to one bit per channel
 // (w[j] = channels 32 j .. 32 j + 31): the device keeps 128-bit bitmaps for every g, export packs them (mkv_api.cu).
-__device__ __forceinline__ void topr_mask_groups(const uint32_t (&x)[4], int r, int g, uint32_t (&w)[4], int lane) {
-    uint32_t key[4];  // energy of this lane's group, as an order-preserving integer (non-negative floats)
+// energy of this lane's group (g adjacent lanes of one j), fp32 left to right, as an order-preserving integer
+__device__ __forceinline__ void group_keys(const uint32_t (&x)[4], int g, int lane, uint32_t (&key)[4]) {
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const float f = bf16_bits_to_f32(x[j]);
@@ -80,6 +80,11 @@ __device__ __forceinline__ void topr_mask_groups(const uint32_t (&x)[4], int r, 
         }
         key[j] = __float_as_uint(e);
     }
+}
+
+__device__ __forceinline__ void topr_mask_groups(const uint32_t (&x)[4], int r, int g, uint32_t (&w)[4], int lane) {
+    uint32_t key[4];  // energy of this lane's group, as an order-preserving integer (non-negative floats)
+    group_keys(x, g, lane, key);
     const bool leader = (lane & (g - 1)) == 0;
     const int nk = r / g;
     uint32_t T = 0;
@@ -141,7 +146,7 @@ __device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, int g
 #pragma unroll
     for (int j = 0; j < 4; ++j) mag[j] = x[j] & 0x7FFFu;
     bool have = false;
-    if (g == 1 && cached) {
+    if (g == 1 && cached) {  // (a kept magnitude equal to a dropped one means a tie: searched again, never guessed)
         w[0] = cw.x; w[1] = cw.y; w[2] = cw.z; w[3] = cw.w;
         uint32_t kmin = 0x8000u, dmax = 0u;
 #pragma unroll
@@ -153,6 +158,29 @@ __device__ __forceinline__ void pack_vector(const uint32_t (&x)[4], int r, int g
         kmin = __reduce_min_sync(kFull, kmin);
         dmax = __reduce_max_sync(kFull, dmax);
         have = __popc(w[0]) + __popc(w[1]) + __popc(w[2]) + __popc(w[3]) == r && kmin > dmax;
+    } else if (cached) {
+        // element groups: the cached mask must be made of whole groups, keep r / g of them, and every kept group's energy
+        // must lie strictly above every dropped one's
+        w[0] = cw.x; w[1] = cw.y; w[2] = cw.z; w[3] = cw.w;
+        uint32_t key[4];
+        group_keys(x, g, lane, key);
+        const bool leader = (lane & (g - 1)) == 0;
+        const uint32_t lead = g == 2 ? 0x55555555u : 0x11111111u;
+        uint32_t kmin = 0xffffffffu, dmax = 0u;
+        bool whole = true;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t m = w[j] & lead;
+            whole = whole && w[j] == (m | (m << 1) | (g == 4 ? (m << 2) | (m << 3) : 0u));
+            const bool kept = (w[j] >> lane) & 1u;
+            if (leader) {
+                kmin = kept ? min(kmin, key[j]) : kmin;
+                dmax = kept ? dmax : max(dmax, key[j] + 1u);  // (+ 1: a dropped group of energy 0 still counts)
+            }
+        }
+        kmin = __reduce_min_sync(kFull, kmin);
+        dmax = __reduce_max_sync(kFull, dmax);
+        have = whole && __popc(w[0]) + __popc(w[1]) + __popc(w[2]) + __popc(w[3]) == r && kmin >= dmax;
     }
     if (!have) {
         if (g == 1) topr_mask(mag, r, w);
@@ -441,7 +469,10 @@ __global__ void __launch_bounds__(256) mkv_segment_loss_kernel(CacheGeom g, Comp
             else if (grp == 1) {
                 topr_mask(mag, r, w);
                 if (masks != nullptr && lane == 0) masks[2 * t + which] = make_uint4(w[0], w[1], w[2], w[3]);
-            } else topr_mask_groups(x, r, grp, w, lane);
+            } else {
+                topr_mask_groups(x, r, grp, w, lane);
+                if (masks != nullptr && lane == 0) masks[2 * t + which] = make_uint4(w[0], w[1], w[2], w[3]);
+            }
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const float f = bf16_bits_to_f32(x[j]);
