@@ -2,7 +2,7 @@
 // selected packed keys, softmax, PV over the packed values, split-K combine.  sm_100a.
 //
 // Design: one launch; every unit is attended by ONE thread-block
-// cluster of C CTAs (C = 2 for 64 units on 148 SMs, 16 for 8 units), one CTA per SM.
+// cluster of C CTAs (C = 2 for 64 units on 148 SMs, 8 for 8 units), one CTA per SM.
 //   * The unit's selected blocks are cut into equal ranges, one per warp of the cluster.  A warp
 //     walks its range in groups of <= 2 token blocks (16 tokens = the M of one mma tile).  What a
 //     block is (payload offset, tokens, r_k, r_v) comes from the plan record mkv_select wrote next
@@ -22,10 +22,13 @@
 //   * Phase 2 (PV, deferred): the softmax sum runs over every selected token; the V part of a block
 //     is fetched and walked only if one of its probabilities is >= 2^-40 (error bound).
 //     O^T = V^T P^T with channels = M, heads = N, the group's 16 tokens = K; P is split into bf16
-//     hi + lo (fp32-class accuracy).  Dense vectors (r = D) skip the walk.
+//     hi + lo (fp32-class accuracy).  Dense vectors (r = D) skip the walk.  When every range of the
+//     cluster is short, each warp lists the groups of its range that matter and the lists are dealt
+//     out over all warps of the CTA (which warps hold those groups is an accident of the data).
 //   * Step 3d (split-K combine): the warps' partials are added inside the CTA (shared memory), the
-//     CTAs' partials by the cluster's first CTA through distributed shared memory, in a fixed order:
-//     no global scratch, no atomics, no second kernel, bit-reproducible.
+//     CTAs' partials by the cluster's first CTA (pushed into its shared memory by the second CTA of a
+//     cluster of two, pulled through distributed shared memory otherwise), in a fixed order: no
+//     global scratch, no atomics, no second kernel, bit-reproducible.
 #include "mkv_internal.cuh"
 #include "mkv_walk.cuh"
 
