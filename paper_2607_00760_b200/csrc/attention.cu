@@ -478,10 +478,12 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
 
             landed();  // the group's K parts have landed
 
-            // ---- QK: S (tokens x heads); rows 0-7 = block 0, rows 8-15 = block 1
-            if (nb0 != 0) {
+            // ---- QK: S (tokens x heads); rows 0-7 = block 0, rows 8-15 = block 1.  (A position that holds no block -- an
+            // invalid `sel` entry, the missing second half of a ragged 16-token block -- still gets its logits: -inf, so
+            // that whoever reads the cache in phase 2 sees "no token" instead of stale shared memory.)
+            {
                 float S[4] = {0.f, 0.f, 0.f, 0.f};
-                qk_group(S, r_k, nb0, nb1, sp0, sp1, qa, lane, (d.y & 2u) != 0u);
+                if (nb0 != 0) qk_group(S, r_k, nb0, nb1, sp0, sp1, qa, lane, (d.y & 2u) != 0u);
                 // ---- scaled logits of token gq of each block, heads 2qq, 2qq+1 -> cache [head][token]
                 const bool v0 = gq < nb0, v1 = gq < nb1;
                 const float zA0 = v0 ? S[0] * scale_log2 : -INFINITY, zB0 = v0 ? S[1] * scale_log2 : -INFINITY;

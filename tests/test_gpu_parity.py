@@ -354,6 +354,35 @@ def test_other_segment_lengths_end_to_end(env, L):
         c.free()
 
 
+@pytest.mark.parametrize("B", [8, 16])
+def test_attention_positions_without_a_block(env, B):
+    """stream positions that hold no tokens: the missing second half of a ragged 16-token block (a block of 16 is two
+    device blocks) and `sel` entries the caller invalidated (-1, a token that is not a block start, a token past the
+    end).  Such a position must read as "no token" in both phases (regression: its logit slots were never written and
+    phase 2 summed stale shared memory), alone in the selection and between valid blocks."""
+    mkv, dev = env
+    N = 64 * 7 + 22  # last block: 6 tokens at B = 16 and at B = 8
+    c = Case(mkv, dev, 1, 1, 7, N, seed=610 + B, B=B)
+    try:
+        strat = uniform_strat(1, 1, c.S, 38, 38, B=B)
+        strat[:, :, -1] = (128, 124, 1, B)      # dense K over a sparse V in the ragged last segment
+        strat[:, :, 2] = (128, 128, 1, B)
+        c.compress(strat)
+        last = (N - 1) // B * B
+        scale = 1 / math.sqrt(128)
+        # (i) the ragged last block alone
+        sel = np.full((1, 1, 4), -1, np.int32); sel[0, 0, 0] = last
+        c.check_attention(sel, np.array([[1]], np.int32))
+        # (ii) invalid entries between valid ones: the GPU must give what the oracle gives on the valid ones alone
+        mixed = np.array([[[0, -1, 2 * B, 3, last, N + B, 5 * B]]], np.int32)
+        out, lse = c.gpu_attention(mixed, np.array([[7]], np.int32))
+        valid = np.array([0, 2 * B, last, 5 * B], np.int32)
+        o, l = orc.attention(c.blobs[0][0], c.q[0], valid, scale)
+        assert_attention_close(out, lse, o[None], l[None])
+    finally:
+        c.free()
+
+
 @pytest.mark.parametrize("Bt,Hkv", [(5, 4), (10, 4), (20, 4), (38, 4)])
 def test_attention_every_cluster_size(env, Bt, Hkv):
     """PackedAttention runs one cluster of C CTAs per unit, C = the largest power of two with units x C <= SMs: 20 units ->
