@@ -383,6 +383,27 @@ def test_attention_positions_without_a_block(env, B):
         c.free()
 
 
+def test_attention_long_ranges(env):
+    """ranges of more than 32 blocks per warp: logits beyond the shared-memory cache go through the global scratch, the
+    descriptor ring is described a second time in phase 2, and phase 2 runs per warp (the lists are only dealt out for
+    short ranges).  76 units -> one CTA per unit (16 warps), 1120 blocks per unit -> 70 blocks = 35 groups per warp."""
+    mkv, dev = env
+    c = Case(mkv, dev, 19, 4, 32, 64 * 140, seed=640)
+    try:
+        strat = uniform_strat(19, 4, c.S, 38)
+        strat[:, :, 3::7, 0:2] = 128
+        strat[:, :, 5::11, 0:2] = (90, 7)
+        c.compress(strat)
+        sel, cnt = c.oracle_sel(c.N)
+        assert int(cnt.min()) == 1120
+        c.check_attention(sel, cnt)
+        # the peaked case next to it: a budget that still gives long ranges
+        sel, cnt = c.oracle_sel(64 * 100)
+        c.check_attention(sel, cnt)
+    finally:
+        c.free()
+
+
 @pytest.mark.parametrize("Bt,Hkv", [(5, 4), (10, 4), (20, 4), (38, 4)])
 def test_attention_every_cluster_size(env, Bt, Hkv):
     """PackedAttention runs one cluster of C CTAs per unit, C = the largest power of two with units x C <= SMs: 20 units ->
