@@ -1221,6 +1221,71 @@ def test_calibration_calls_run_and_leave_the_cache_intact(env):
             c.free()
 
 
+@pytest.mark.parametrize("chunk", range(4))
+def test_randomised_configurations(env, chunk):
+    """a seeded sweep over what the focused tests hold fixed: token blocks B in {4, 8, 16}, segment lengths, GQA groups 1-8,
+    a fresh (r_k, r_v, g) per segment, ragged lengths; a loss pass of some other candidate before the compressor (its
+    masks sit in the cache's scratch and may be used only where they fit); selection by three budgets; then the update
+    buffer plus a selection in arbitrary order with invalid entries.  (A sweep of this kind found the stale-logit bug of
+    test_attention_positions_without_a_block.)"""
+    mkv, dev = env
+    import torch
+    for seed in range(16 * chunk, 16 * chunk + 16):
+        rng = np.random.default_rng(9000 + seed)
+        B = int(rng.choice([4, 8, 16])); L = int(rng.choice([32, 64, 128]))
+        Hkv = int(rng.choice([1, 2, 4])); G = int(rng.choice([1, 2, 4, 7, 8]))
+        Bt = int(rng.integers(1, 4)); N = int(rng.integers(L // 2, 12 * L))
+        c = Case(mkv, dev, Bt, Hkv, Hkv * G, N, L=L, seed=7000 + seed, B=B)
+        try:
+            strat = np.zeros((Bt, Hkv, c.S, 4), np.uint8)
+            for idx in np.ndindex(Bt, Hkv, c.S):
+                g = int(rng.choice([1, 2, 4]))
+                rk = int(rng.choice([128, g * int(rng.integers(1, 128 // g + 1))]))
+                rv = int(rng.choice([128, g * int(rng.integers(1, 128 // g + 1))]))
+                strat[idx] = (rk, rv, g, B)
+            gc = int(rng.choice([1, 2, 4])); rc = gc * int(rng.integers(1, 128 // gc + 1))
+            lk, lv = c.gpu_loss(rc, rc, gc)
+            b0, h0 = int(rng.integers(0, Bt)), int(rng.integers(0, Hkv))
+            rk_, rv_ = orc.segment_loss(c.K[b0, h0], c.V[b0, h0], L, rc, rc, gc)
+            np.testing.assert_allclose(lk[b0, h0], rk_, rtol=1e-12, atol=0)
+            np.testing.assert_allclose(lv[b0, h0], rv_, rtol=1e-12, atol=0)
+            c.compress(strat)
+            c.assert_export_equal()
+            for budget in (B, int(rng.integers(B, N + 1)), N):
+                tot, sw = c.check_select(budget, reduce=int(rng.integers(0, 2)))
+                assert sw * 10000 <= tot, (seed, sw, tot)
+                sel, cnt = c.oracle_sel(budget)
+                c.check_attention(sel, cnt)
+            n_buf = int(rng.integers(1, L + 1))
+            rk = torch.from_numpy(rng.standard_normal((Bt, Hkv, n_buf, 128)).astype(np.float32)).to(torch.bfloat16)
+            rv = torch.from_numpy(rng.standard_normal((Bt, Hkv, n_buf, 128)).astype(np.float32)).to(torch.bfloat16)
+            c.cache.update_append(0, rk.to(dev), rv.to(dev))
+            rk_u, rv_u = rk.view(torch.int16).numpy().view(np.uint16), rv.view(torch.int16).numpy().view(np.uint16)
+            nblk = (N + B - 1) // B
+            kk = int(rng.integers(0, min(nblk, 40) + 1))
+            sel = np.full((Bt, Hkv, kk + 3), -1, np.int32)
+            cnt = np.zeros((Bt, Hkv), np.int32)
+            scale = 1 / math.sqrt(128)
+            ref, ref_lse = [], []
+            for b in range(Bt):
+                for h in range(Hkv):
+                    pick = rng.permutation(nblk)[:kk] * B
+                    row = list(pick)
+                    for _ in range(int(rng.integers(0, 3))):
+                        row.insert(int(rng.integers(0, len(row) + 1)), int(rng.choice([-1, N + B, 3])))
+                    sel[b, h, :len(row)], cnt[b, h] = row, len(row)
+                    o, l = orc.attention_with_update_buffer(c.blobs[b][h], c.q[b, h * G:(h + 1) * G], np.array(pick, np.int32),
+                                                            scale, rk_u[b, h], rv_u[b, h])
+                    ref.append(o); ref_lse.append(l)
+            out, lse = c.gpu_attention(sel, cnt)
+            assert_attention_close(out, lse, np.concatenate(ref).reshape(out.shape), np.concatenate(ref_lse).reshape(lse.shape))
+        except Exception:
+            print("randomised configuration", seed, dict(B=B, L=L, Hkv=Hkv, G=G, Bt=Bt, N=N))
+            raise
+        finally:
+            c.free()
+
+
 def test_zz_report_lse_ulps(env):
     """runs last: the largest lse error, in fp32 spacings of |lse| beyond the 1e-3 absolute term, seen by this session"""
     import gpu_util
