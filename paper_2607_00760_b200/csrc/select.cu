@@ -71,9 +71,8 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
     const int cap = MODE == 1 ? cand_cap : k_max;
     const bool cached = n <= kKeyCap;
 
-    __shared__ unsigned hist[4096];
-    __shared__ uint32_t s_prefix;
-    __shared__ int s_krem, s_neq;
+    __shared__ unsigned hist[2 * 4096];
+    __shared__ int s_krem;
     __shared__ unsigned long long s_warp[32];
 
     const int k0 = budget / kB, rem = budget % kB, nbR = ntok % kB;
@@ -106,72 +105,92 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
         uint32_t prefix = 0;
         int krem = kq;
         // MSB-first radix select in three passes of 12 + 12 + 8 bits: with 4096 bins the scores spread
-        // over enough bins for plain shared-memory atomics, and later passes touch few elements
+        // over enough bins for plain shared-memory atomics, and later passes touch few elements.
+        // Two barriers per pass: the histograms alternate between two buffers (a buffer is cleared one pass ahead, between
+        // the barriers of the pass in between), and once the warps' totals are known every warp finds the bin of the
+        // wanted key on its own -- from the totals the warp that holds it, from that warp's bins the bin -- so nothing has
+        // to be broadcast.
+        for (int i = tid; i < 2 * 4096; i += 1024) hist[i] = 0;
+        __syncthreads();
+        int n_eq = 0;
         for (int pass = 0; pass < 3; ++pass) {
             const int shift = pass == 0 ? 20 : (pass == 1 ? 8 : 0);
             const int nbins = pass == 2 ? 256 : 4096;
-            for (int i = tid; i < nbins; i += 1024) hist[i] = 0;
-            __syncthreads();
+            unsigned* cur = hist + (pass & 1) * 4096;
             const uint32_t hi_mask = pass == 0 ? 0u : (0xffffffffu << (pass == 1 ? 20 : 8));
             if (cached) {
 #pragma unroll
                 for (int j = 0; j < kPerThread; ++j) {
                     const uint32_t u = kv[j];
                     if (kPerThread * tid + j < n && (u & hi_mask) == prefix)
-                        atomicAdd(&hist[(u >> shift) & (uint32_t)(nbins - 1)], 1u);
+                        atomicAdd(&cur[(u >> shift) & (uint32_t)(nbins - 1)], 1u);
                 }
             } else {
                 for (int i = tid; i < n; i += 1024) {
                     const uint32_t u = keyat(i);
-                    if ((u & hi_mask) == prefix) atomicAdd(&hist[(u >> shift) & (uint32_t)(nbins - 1)], 1u);
+                    if ((u & hi_mask) == prefix) atomicAdd(&cur[(u >> shift) & (uint32_t)(nbins - 1)], 1u);
                 }
             }
             __syncthreads();
-            // thread t owns bins [t bpt, (t+1) bpt); counts in the bins above it by a block-wide suffix scan
+            if (pass == 1 && tid < 256) hist[tid] = 0;  // buffer 0 is free since this barrier: cleared for the last pass
+            // thread t owns bins [t bpt, (t+1) bpt); suffix scan inside the warp (higher lanes hold higher bins)
             const int bpt = nbins >> 10;  // 4 or 0 (256 bins: one bin for each of the first 256 threads)
-            unsigned mine[4] = {0u, 0u, 0u, 0u}, tot = 0;
+            unsigned tot = 0;
             if (bpt) {
 #pragma unroll
-                for (int j = 0; j < 4; ++j) { mine[j] = hist[4 * tid + j]; tot += mine[j]; }
+                for (int j = 0; j < 4; ++j) tot += cur[4 * tid + j];
             } else if (tid < 256) {
-                mine[0] = hist[tid]; tot = mine[0];
+                tot = cur[tid];
             }
-            unsigned incl = tot;
+#pragma unroll
+            for (int o = 16; o >= 1; o >>= 1) tot += __shfl_xor_sync(kFull, tot, o);
+            if (lane == 0) s_warp[warp] = tot;
+            __syncthreads();
+            // every warp: the warp W whose bins hold the krem-th key from the top, and the count above W
+            const unsigned wt = (unsigned)s_warp[lane];
+            unsigned wincl = wt;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
-                const unsigned v = __shfl_down_sync(kFull, incl, o);
-                if (lane + o < 32) incl += v;
+                const unsigned v = __shfl_down_sync(kFull, wincl, o);
+                if (lane + o < 32) wincl += v;
             }
-            if (lane == 0) s_warp[warp] = incl;
-            __syncthreads();
-            if (warp == 0) {
-                const unsigned w = (unsigned)s_warp[lane];
-                unsigned wi = w;
+            const unsigned hitw = __ballot_sync(kFull, wincl - wt < (unsigned)krem && (unsigned)krem <= wincl);
+            const int W = __ffs(hitw) - 1;
+            const unsigned aboveW = __shfl_sync(kFull, wincl - wt, W);
+            // the bins of W's threads, one thread's worth per lane
+            const int tW = 32 * W + lane;
+            unsigned b4[4] = {0u, 0u, 0u, 0u}, bt = 0;
+            if (bpt) {
 #pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const unsigned v = __shfl_down_sync(kFull, wi, o);
-                    if (lane + o < 32) wi += v;
-                }
-                s_warp[lane] = wi - w;  // counts in the warps above
+                for (int j = 0; j < 4; ++j) { b4[j] = cur[4 * tW + j]; bt += b4[j]; }
+            } else if (tW < 256) {
+                b4[0] = cur[tW]; bt = b4[0];
             }
-            __syncthreads();
-            unsigned cum = (unsigned)s_warp[warp] + incl - tot;
-            const int nb_mine = bpt ? 4 : 1, bin0 = bpt ? 4 * tid : tid;
-            for (int j = nb_mine - 1; j >= 0; --j) {
-                if (cum < (unsigned)krem && (unsigned)krem <= cum + mine[j]) {
-                    s_prefix = prefix | ((uint32_t)(bin0 + j) << shift);
-                    s_krem = krem - (int)cum;
-                    s_neq = (int)mine[j];
-                }
-                cum += mine[j];
+            unsigned bincl = bt;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const unsigned v = __shfl_down_sync(kFull, bincl, o);
+                if (lane + o < 32) bincl += v;
             }
-            __syncthreads();
-            prefix = s_prefix;
-            krem = s_krem;
+            unsigned cum = aboveW + bincl - bt;
+            const int nb_mine = bpt ? 4 : 1, bin0 = bpt ? 4 * tW : tW;
+            int f_bin = -1;
+            unsigned f_cum = 0u, f_cnt = 0u;
+#pragma unroll
+            for (int j = 3; j >= 0; --j) {
+                if (j < nb_mine) {
+                    if (cum < (unsigned)krem && (unsigned)krem <= cum + b4[j]) { f_bin = bin0 + j; f_cum = cum; f_cnt = b4[j]; }
+                    cum += b4[j];
+                }
+            }
+            const int src = __ffs(__ballot_sync(kFull, f_bin >= 0)) - 1;
+            prefix |= (uint32_t)__shfl_sync(kFull, f_bin, src) << shift;
+            krem -= (int)__shfl_sync(kFull, f_cum, src);
+            n_eq = (int)__shfl_sync(kFull, f_cnt, src);
         }
         Ts = prefix;
         take_eq = krem;            // equals (by ascending index) inside the kq best
-        const int n_eq = s_neq;    // all elements whose key equals the threshold key
+        // (n_eq: all elements whose key equals the threshold key)
         if (ragged_try) {
             // the short block is the highest index: it is inside the k0+1 best iff it beats Ts or
             // ties with it and every tie is taken (MODE 2: and it survived as a candidate, i.e. it is
