@@ -31,7 +31,7 @@ FALLBACK_HBM_GBS = 6650.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the committed `ncu --set full` captures.  NOT measured by
 # this run: printed under "traffic_from_capture" with the file it came from; "traffic" itself stays null.
 NCU_CAPTURE = {"llama8b-128k-b8": {"source": "profiles/r2/ncu_decode_config2.md (ncu --set full, first launch of each kernel)",
-                                   "attention": 28746240, "score+topk": 125799936},
+                                   "attention": 28720896, "score+topk": 125432064},
                "llama8b-1m-b1": {"source": "profiles/r2/ncu_decode_config3.md", "attention": None, "score+topk": None},
                "qwen7b-64k-b16": {"source": "profiles/r2/ncu_decode_config4.md", "attention": None, "score+topk": None}}
 
