@@ -260,6 +260,49 @@ MKV_API int mkv_calibrate_walk(const mkv_cache* cache, int32_t layer, const void
 MKV_API int mkv_attention_stats(const mkv_cache* cache, uint64_t* blocks_host, uint64_t* v_blocks_host,
                         uint64_t* v_bytes_host, int32_t reset);
 
+/*
+ * Step 2b alone, for callers that cannot allocate device memory (keep the best-scored token blocks
+ * that fit the token budget).
+ *
+ * Who this is for.  Every other call works on an mkv_cache, and mkv_cache_create gets its arenas and scratch from
+ * cudaMalloc.  That is not open to everyone: a decode loop inside a serving engine whose pool allocator took the whole
+ * GPU at start-up (cudaMalloc finds no memory left, and where it succeeds it holds up every stream of the device while
+ * it runs); a plug-in that is handed device pointers by its host program and owns no allocator; code that runs only
+ * between the launches of somebody else's latency-critical step.  Such a caller brings block scores of its own (or the
+ * ones mkv_select returned in scores_opt) and gets the selection without this library allocating or freeing anything:
+ * no cudaMalloc, no cudaFree, no library routine that allocates, no mkv_cache.
+ *
+ * What it computes: exactly what mkv_select does after scoring.  Unit u has ceil(n_tokens[u] / token_block) blocks;
+ * block i has score scores[u * score_stride + i] and token_block tokens (the last block of a unit may be shorter).
+ * Blocks are taken by (score descending, index ascending) while they fit in token_budget tokens.
+ *   scores:    device, float [n_units][score_stride], finite
+ *   n_tokens:  device, int32 [n_units], 0 <= n_tokens[u] <= score_stride * token_block (NOT checked: a larger value
+ *              reads past the unit's scores)
+ *   sel:       device, int32 [n_units][k_max]: first-token index of every chosen block, ascending; unused tail = -1
+ *   sel_count: device, int32 [n_units]
+ *   k_max >= min(token_budget / token_block + 1, score_stride); token_block is 4, 8 or 16
+ *   device:    ordinal of the GPU all four buffers live on; the call makes it the current device
+ * The caller owns all four buffers; they are read / written on `stream` and the call returns without waiting.
+ *
+ * Scratch and its limit.  Units of more than 16384 blocks are selected in two stages (every 16384-block slice keeps
+ * its token_budget / token_block + 1 best as candidates, then one pass picks among the candidates); the candidate
+ * lists are the only scratch, and they live in an array compiled into the library: MKV_TOPK_STATIC_MAX_CANDIDATES
+ * entries of 8 bytes = 4 MB, held by every GPU that loads libmkv until the process ends.  A call needs
+ * n_units * ceil(score_stride / 16384) * min(token_budget / token_block + 1, 16384) entries; one that needs more is
+ * refused with MKV_E_ARG and a message that names the three factors (nothing is enqueued) -- lower the budget or pass
+ * the units in several calls.  Calls with score_stride <= 16384 use no scratch and have no such limit.
+ *
+ * The first call on a device looks up the array's device address (cudaGetSymbolAddress, which may also load the
+ * library's device code on that GPU); make that first call before any stream capture begins.  All calls on a device
+ * share the one array.  It needs no clearing -- every call overwrites all entries it later reads, so the previous
+ * call's contents never matter -- but two calls that can run on the GPU at the same time (different streams without
+ * an event between them, or two host threads) overwrite each other's candidates and return garbage: order them.
+ */
+#define MKV_TOPK_STATIC_MAX_CANDIDATES (1 << 19)
+MKV_API int mkv_topk_static(int32_t device, const float* scores, const int32_t* n_tokens, int32_t n_units,
+                    int32_t score_stride, int32_t token_block, int32_t token_budget, int32_t* sel,
+                    int32_t* sel_count, int32_t k_max, void* stream);
+
 /* Parity / dump: canonical blob of unit (layer, b, h) into host memory.  *need_host receives the
  * blob size; if cap < need nothing is copied and MKV_E_ARG is returned.  Synchronises. */
 MKV_API int mkv_cache_export(const mkv_cache* cache, int32_t layer, int32_t b, int32_t h, void* buf_host,

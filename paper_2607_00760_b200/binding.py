@@ -25,7 +25,7 @@ SYMBOLS = ["mkv_cache_create", "mkv_cache_free", "mkv_cache_reset", "mkv_segment
            "mkv_strategy_quantile", "mkv_strategy_threshold", "mkv_compress_segment", "mkv_select",
            "mkv_packed_attention", "mkv_update_append", "mkv_update_flush", "mkv_update_count", "mkv_calibrate_gather", "mkv_calibrate_stream", "mkv_calibrate_walk",
            "mkv_attention_stats", "mkv_rotation_set", "mkv_rotate_query", "mkv_rotate_output", "mkv_decode_step", "mkv_decode_host", "mkv_cache_export", "mkv_cache_bytes",
-           "mkv_cache_status", "mkv_last_launch_count", "mkv_last_error", "mkv_version"]
+           "mkv_cache_status", "mkv_last_launch_count", "mkv_last_error", "mkv_version", "mkv_topk_static"]
 
 
 class mkv_cache_desc(C.Structure):
@@ -68,6 +68,7 @@ _lib.mkv_cache_export.argtypes = [_vp, _i32, _i32, _i32, _vp, _u64, C.POINTER(_u
 _lib.mkv_cache_bytes.argtypes = [_vp, _i32, C.POINTER(_u64), C.POINTER(_u64), C.POINTER(_u64)]
 _lib.mkv_cache_status.argtypes = [_vp, C.POINTER(C.c_uint32)]
 _lib.mkv_last_launch_count.argtypes = [_vp, C.POINTER(_i32), C.POINTER(_i32), C.POINTER(_i32)]
+_lib.mkv_topk_static.argtypes = [_i32, _vp, _vp, _i32, _i32, _i32, _i32, _vp, _vp, _i32, _vp]
 _lib.mkv_last_error.restype = C.c_char_p
 for _n in SYMBOLS:
     if _n != "mkv_last_error":
@@ -178,6 +179,17 @@ def mkv_compress_segment(cache, layer, k, v, b0, seg0, strat, stream=None):
 def mkv_select(cache, layer, q, token_budget, sel, sel_count, reduce=0, scores=None, stream=None):
     _check(_lib.mkv_select(cache, layer, _ptr(q), token_budget, reduce, _ptr(sel), _ptr(sel_count),
                            sel.shape[-1], _ptr(scores), _stream(stream)))
+
+
+MKV_TOPK_STATIC_MAX_CANDIDATES = 1 << 19
+
+
+def mkv_topk_static(device, scores, n_tokens, token_block, token_budget, sel, sel_count, stream=None):
+    """Budgeted top-k on caller-owned scores [n_units][score_stride] with the library's static scratch: no
+    cache, no device allocation (include/mkv.h).  n_tokens, sel [n_units][k_max], sel_count: int32 on the device."""
+    n_units, score_stride = int(scores.shape[0]), int(scores.shape[-1])
+    _check(_lib.mkv_topk_static(device, _ptr(scores), _ptr(n_tokens), n_units, score_stride, token_block,
+                                token_budget, _ptr(sel), _ptr(sel_count), sel.shape[-1], _stream(stream)))
 
 
 def mkv_packed_attention(cache, layer, q, sel, sel_count, softmax_scale, out, lse=None, stream=None):

@@ -61,6 +61,10 @@ __host__ __device__ inline uint32_t seg_bk_bytes(int r_k, int n_tok, int B) {
     return pad16u((uint32_t)nblk * vec_bytes(r_k));
 }
 
+// records the message mkv_last_error() returns on the calling thread and hands `code` back (mkv_api.cu): for entry
+// points that live beside their kernels instead of in mkv_api.cu
+int set_error(int code, const char* fmt, ...);
+
 // ---- launchers (each enqueues on `stream`; returns cudaError) -----------------------------
 struct CompressArgs {
     const uint16_t* k;

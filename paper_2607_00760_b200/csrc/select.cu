@@ -1,5 +1,7 @@
 // select.cu — step 2b of the hot path: top-k block selection by token budget
 // on the scores of score.cu (step 2a).  sm_100a.
+#include <mutex>
+
 #include "mkv_internal.cuh"
 
 namespace mkv {
@@ -328,4 +330,103 @@ cudaError_t launch_select(const CacheGeom& g, const LayerView& lv, const uint16_
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------
+// mkv_topk_static — the budgeted top-k for callers that may not allocate device memory.
+//
+// Everything else in this library works on an mkv_cache, and mkv_cache_create obtains its arenas and
+// scratch with some two dozen cudaMalloc calls.  Some users can do neither that nor an allocation of
+// their own at the point where they need a selection: a decode loop running inside a serving engine
+// whose pool allocator was given all of the GPU's memory at start-up (a raw cudaMalloc there fails
+// for lack of memory, and one that succeeds stalls every stream of the device while it runs), a
+// plug-in that is handed device pointers by its host program and has no allocator to ask, or code
+// that is only ever called between the launches of someone else's latency-critical step.  Such a
+// caller already has block scores of its own (or took them from mkv_select's scores_opt earlier)
+// and needs step 2b alone.
+//
+// The one piece of scratch the selection needs -- the candidate lists that the first stage of the
+// two-stage selection (units of more than kKeyCap blocks) hands to the second -- therefore lives in
+// the library image itself: a file-scope __device__ array of kStaticCand entries (key + index,
+// 8 bytes each = 4 MB) that every GPU which loads this library holds until the process exits.
+// Host code cannot use the array's name as an address (on the host the symbol is only a handle), so the
+// device address is looked up once per device with cudaGetSymbolAddress, with that device current,
+// and kept; the kernels receive that pointer like any other buffer.
+//
+// All calls on one device share the array.  Nothing in it has to start at zero: the first stage
+// writes every entry of every (unit, slice) list it then reads, real candidates first and padding
+// after them, so what an earlier call left behind is never read.  Two calls whose kernels can run
+// at the same time on one device (different streams, or threads) would overwrite each other's
+// candidates: order them.
+// ------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kStaticCand = MKV_TOPK_STATIC_MAX_CANDIDATES;
+static __device__ __align__(256) unsigned char g_static_cand[(size_t)kStaticCand * 8];  // [keys: kStaticCand x u32][indices: kStaticCand x i32]
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+void* g_static_addr[kStaticMaxDevices] = {};  // device address of g_static_cand on each device, once looked up
+
+// device address of the static scratch on `device` (which must be the current device)
+cudaError_t static_scratch(int device, unsigned char** p) {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[device]) {
+        void* a = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&a, g_static_cand);
+        if (e != cudaSuccess) return e;
+        g_static_addr[device] = a;
+    }
+    *p = (unsigned char*)g_static_addr[device];
+    return cudaSuccess;
+}
+
+}  // namespace
+
 }  // namespace mkv
+
+extern "C" int mkv_topk_static(int32_t device, const float* scores, const int32_t* n_tokens, int32_t n_units,
+                               int32_t score_stride, int32_t token_block, int32_t token_budget, int32_t* sel,
+                               int32_t* sel_count, int32_t k_max, void* stream) {
+    using namespace mkv;
+    if (!scores || !n_tokens || !sel || !sel_count) return set_error(MKV_E_ARG, "mkv_topk_static: NULL argument");
+    if (n_units < 1 || score_stride < 1 || token_budget < 0) return set_error(MKV_E_ARG, "mkv_topk_static: bad sizes");
+    if (token_block != 4 && token_block != 8 && token_block != 16)
+        return set_error(MKV_E_ARG, "mkv_topk_static: token_block %d: must be 4, 8 or 16", token_block);
+    const long long need = (long long)token_budget / token_block + 1;
+    if (k_max < 1 || k_max < (need < score_stride ? need : score_stride))
+        return set_error(MKV_E_ARG, "mkv_topk_static: k_max %d too small for budget %d", k_max, token_budget);
+    if (device < 0 || device >= kStaticMaxDevices) return set_error(MKV_E_ARG, "mkv_topk_static: device %d out of range", device);
+    const int n_slices = (score_stride + kKeyCap - 1) / kKeyCap;
+    const int cand_cap = (int)(need < kKeyCap ? need : kKeyCap);  // candidates kept per slice
+    const long long entries = n_slices > 1 ? (long long)n_units * n_slices * cand_cap : 0;
+    if (entries > kStaticCand)
+        return set_error(MKV_E_ARG,
+                         "mkv_topk_static: %d units x %d slices x %d candidates = %lld entries of scratch; the static "
+                         "array holds MKV_TOPK_STATIC_MAX_CANDIDATES = %d (lower the budget or split the units over calls)",
+                         n_units, n_slices, cand_cap, entries, kStaticCand);
+    cudaError_t e = cudaSetDevice(device);
+    unsigned char* scratch = nullptr;
+    if (e == cudaSuccess) e = static_scratch(device, &scratch);
+    if (e != cudaSuccess) return set_error(MKV_E_CUDA, "mkv_topk_static: %s", cudaGetErrorString(e));
+    // the kernels of mkv_select, given a geometry that holds only what they read: B, the score stride and the token counts
+    CacheGeom g{};
+    g.n_units = n_units; g.B = token_block; g.pb = token_block < kPhys ? token_block : kPhys; g.ppb = token_block / g.pb;
+    g.score_stride = score_stride;
+    LayerView lv{};
+    lv.unit_ntok = const_cast<int32_t*>(n_tokens);
+    cudaStream_t s = (cudaStream_t)stream;
+    if (n_slices == 1) {  // one stage: no scratch at all
+        e = launch_pdl(mkv_topk_kernel<0>, dim3(n_units), dim3(1024), 0, s, g, lv, scores, (int)token_budget, sel, sel_count,
+                       (int)k_max, (uint32_t*)nullptr, (int32_t*)nullptr, 1, 0, (PlanRec*)nullptr, 0, 0u);
+    } else {
+        uint32_t* cand_key = reinterpret_cast<uint32_t*>(scratch);
+        int32_t* cand_idx = reinterpret_cast<int32_t*>(scratch + (size_t)kStaticCand * 4);
+        e = launch_pdl(mkv_topk_kernel<1>, dim3(n_units * n_slices), dim3(1024), 0, s, g, lv, scores, (int)token_budget, sel,
+                       sel_count, (int)k_max, cand_key, cand_idx, n_slices, cand_cap, (PlanRec*)nullptr, 0, 0u);
+        if (e == cudaSuccess)
+            e = launch_pdl(mkv_topk_kernel<2>, dim3(n_units), dim3(1024), 0, s, g, lv, scores, (int)token_budget, sel,
+                           sel_count, (int)k_max, cand_key, cand_idx, n_slices, cand_cap, (PlanRec*)nullptr, 0, 0u);
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return set_error(MKV_E_CUDA, "mkv_topk_static: %s", cudaGetErrorString(e));
+    return MKV_OK;
+}
