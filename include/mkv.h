@@ -87,7 +87,7 @@ typedef struct {
                              0 = size for the dense worst case */
     int32_t token_block;  /* B: tokens per token block = unit of selection, one block key each (4, 8 or 16;
                              0 = 8).  Every strategy of the cache must carry this B; segment_len must be a multiple of it */
-    int32_t reserved;     /* 0 */
+    int32_t reserved;     /* must be 0 (anything else: MKV_E_ARG) */
 } mkv_cache_desc;
 
 /* Per-segment compression strategy: kept elements per K / V vector (multiples of
@@ -162,6 +162,8 @@ MKV_API int mkv_select(const mkv_cache* cache, int32_t layer, const void* q, int
  * tokens of the layer's KV update buffer if it holds any (see mkv_update_append).
  * sel / sel_count as written by mkv_select (any order of blocks is accepted; entries the caller changed after
  * mkv_select are honoured: the per-block records mkv_select leaves for this call are verified against `sel`).
+ * At most ceil(max_tokens / B) + 1 entries per unit are attended (one more than the unit has blocks); a caller-built
+ * list that is longer (k_max and sel_count beyond that, which takes duplicates) is cut there.
  * One launch: one thread-block cluster per unit (one CTA per SM); the CTAs of a cluster meet at cluster barriers and read
  * each other's shared memory, nothing else is shared between CTAs.
  * out: float [batch][n_q_heads][D].  lse_opt: float [batch][n_q_heads] or NULL (log-sum-exp of the
@@ -184,6 +186,9 @@ MKV_API int mkv_packed_attention(const mkv_cache* cache, int32_t layer, const vo
  *           number of full segments, else MKV_E_STATE.  Flushing fewer than segment_len tokens
  *           leaves a short last segment, after which nothing can be appended to the packed cache.
  *   count:  tokens currently buffered per unit (host value; no synchronisation).
+ * A layer with an installed rotation (mkv_rotation_set) holds K R_k^T and V R_v^T, and so must its buffer: pass tokens
+ * that are rotated the same way.  The buffer is attended with the folded query and its result goes through the output
+ * fold like the packed part, so raw K / V in the buffer of a rotated layer give wrong results without any error.
  * mkv_cache_reset also empties the buffer.  The count lives in device memory and is updated on the stream, so a
  * captured CUDA graph of mkv_packed_attention stays valid across appends and flushes.
  */
@@ -226,8 +231,8 @@ MKV_API int mkv_decode_step(mkv_cache* cache, int32_t layer, const void* q, int3
  * Steps 2+3 with HOST buffers (the end-to-end call): brings q_host (bf16 [batch][n_q_heads][D]) to the device, runs
  * mkv_decode_step, delivers out_host (float [batch][n_q_heads][D]).  Pinned (page-locked) buffers are read and written
  * by kernels of the chain itself (a 64-KB fetch kernel in front; the attention kernel stores straight into out_host, or
- * a store kernel behind the output fold), so the step never leaves the compute engine; pageable buffers fall back to
- * cudaMemcpyAsync.  Everything is enqueued on `stream`; the caller synchronises the stream before reading out_host.  sel_host_opt [batch][n_kv_heads][token_budget/B + 1] and
+ * a store kernel behind the output fold), so the step never leaves the compute engine; pageable buffers, and pinned
+ * ones that are not 16-byte aligned, fall back to cudaMemcpyAsync.  Everything is enqueued on `stream`; the caller synchronises the stream before reading out_host.  sel_host_opt [batch][n_kv_heads][token_budget/B + 1] and
  * sel_count_host_opt [batch][n_kv_heads] may be NULL.
  */
 MKV_API int mkv_decode_host(mkv_cache* cache, int32_t layer, const void* q_host, int32_t token_budget,

@@ -291,7 +291,10 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     const int n_buf = min(max(__ldg(upd_count), 0), g.L);
     const int upd_blocks = (n_buf + kPhys - 1) / kPhys;  // the unit's stream ends with the blocks of its update buffer
     const int ppb = g.ppb;                                // device blocks per selected token block (2 at B = 16)
-    const int cnt = min(max(__ldg(sel_count + u), 0), k_max) * ppb;  // device blocks selected
+    // device blocks selected: at most sel_cap = blocks per unit + 1 entries of `sel` are attended (plan_stride = sel_cap
+    // * ppb), which is also what the unit's share of the logit scratch is sized for; a caller-built selection longer
+    // than that (k_max beyond sel_cap, duplicates) is cut there instead of running into the next unit's scratch
+    const int cnt = min(min(max(__ldg(sel_count + u), 0), k_max) * ppb, scr.plan_stride);
     const int T = cnt + upd_blocks;                       // device blocks of the unit's stream
     const size_t row = (size_t)(u / g.n_kv_heads) * g.n_q_heads + (size_t)(u % g.n_kv_heads) * G;
     if (T == 0) {  // (uniform over the cluster) empty selection: out = 0, lse = -inf
@@ -899,7 +902,7 @@ mkv_walk_probe_kernel(CacheGeom g, LayerView lv, const uint16_t* __restrict__ q,
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gq = lane >> 2, qq = lane & 3;
     const int wi = blockIdx.x * kWarps + warp;
     const int u = wi % g.n_units;
-    const int cnt = min(max(__ldg(sel_count + u), 0), k_max) * g.ppb;
+    const int cnt = min(min(max(__ldg(sel_count + u), 0), k_max), g.score_stride + 1) * g.ppb;  // as mkv_packed_attention cuts it
     const int pairs = cnt >> 1;
     if (pairs == 0) return;
     const int j = 2 * ((wi / g.n_units) % pairs);

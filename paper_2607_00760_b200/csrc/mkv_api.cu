@@ -134,6 +134,7 @@ int mkv_cache_create(const mkv_cache_desc* d, mkv_cache** out) {
     if (d->n_layers < 1 || d->batch < 1 || d->n_kv_heads < 1 || d->n_q_heads < 1 || d->max_tokens < 1)
         return fail(MKV_E_ARG, "mkv_cache_create: non-positive size");
     if (d->n_q_heads % d->n_kv_heads) return fail(MKV_E_ARG, "n_q_heads must be a multiple of n_kv_heads");
+    if (d->reserved != 0) return fail(MKV_E_ARG, "mkv_cache_create: reserved = %d, must be 0", d->reserved);
     if (d->head_dim != kD) return fail(MKV_E_UNSUPPORTED, "head_dim %d: only 128 is built", d->head_dim);
     if (d->n_q_heads / d->n_kv_heads > kMaxGroup)
         return fail(MKV_E_UNSUPPORTED, "GQA group %d > %d", d->n_q_heads / d->n_kv_heads, kMaxGroup);
@@ -246,6 +247,10 @@ int mkv_cache_reset(mkv_cache* c, int32_t layer, void* stream) {
         for (int b = 0; b < g.batch; ++b) c->host_nseg[(size_t)l * g.batch + b] = c->host_ntok[(size_t)l * g.batch + b] = 0;
         MKV_CUDA(cudaMemsetAsync(c->upd_cnt + l, 0, 4, s));
         c->upd_n[l] = 0;
+        // the layer's plan records describe payloads that are gone: cleared on the stream, so that also a launch
+        // captured before the reset (its tag is a kernel argument) finds none of them when it is replayed afterwards
+        const size_t per_layer = (size_t)g.n_units * c->sel_cap * g.ppb;
+        MKV_CUDA(cudaMemsetAsync(c->plan + (size_t)l * per_layer, 0, per_layer * sizeof(PlanRec), s));
     }
     return MKV_OK;
 }
@@ -541,11 +546,14 @@ __global__ void __launch_bounds__(256) mkv_copy16_kernel(const uint4* __restrict
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x) dst[i] = src[i];
 }
 
-// device address of a pinned / registered host buffer the GPU can access directly, else nullptr
+// device address of a pinned / registered host buffer the GPU can access directly, else nullptr.  The kernels that use
+// it move 16 bytes per access, so a buffer that is not 16-byte aligned (a view into a pinned block at an odd offset)
+// counts as not mapped: it takes the cudaMemcpyAsync path like pageable memory.
 void* mapped_host(const void* p) {
     cudaPointerAttributes a;
     if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return nullptr; }
-    return a.type == cudaMemoryTypeHost ? a.devicePointer : nullptr;
+    if (a.type != cudaMemoryTypeHost || (reinterpret_cast<uintptr_t>(a.devicePointer) & 15u) != 0) return nullptr;
+    return a.devicePointer;
 }
 
 }  // namespace

@@ -110,8 +110,12 @@ struct __align__(16) PlanRec {
                      // K values are stored pair-major, see mkv_walk.cuh)
     uint32_t tag;    // plan_tag(generation, layer); 0 = never written
 };
+// bit 31: written at all; bits 16-30: generation (15 bits); bits 0-15: layer.  The generation alone would let a record
+// survive 32768 resets, so mkv_cache_reset also clears the records of the layers it resets (mkv_api.cu): a tag never
+// has to tell two fillings of a layer apart on its own, and a captured launch that still carries an older tag finds
+// no record of its own after a reset and falls back to the tables.
 __host__ __device__ inline uint32_t plan_tag(uint32_t generation, int layer) {
-    return ((generation & 0xffffu) << 16) | ((uint32_t)layer & 0xffffu) | 0x80000000u;
+    return ((generation & 0x7fffu) << 16) | ((uint32_t)layer & 0xffffu) | 0x80000000u;
 }
 #ifdef __CUDACC__
 // table lookup of the DEVICE block that starts at token t0 of `unit`; meta = 0 if t0 is not a device-block start of the unit

@@ -51,6 +51,15 @@ def test_fails_loudly_without_a_gpu():
     assert binding.mkv_last_error() != ""
 
 
+def test_create_rejects_a_nonzero_reserved_field():
+    """mkv_cache_desc.reserved must be 0 (include/mkv.h): checked on the host before any CUDA call"""
+    from paper_2607_00760_b200 import binding
+    desc = binding.mkv_cache_desc(1, 1, 2, 8, 128, 4096, 64, 0, 0, 8, 1)
+    h = ctypes.c_void_p()
+    assert binding._lib.mkv_cache_create(ctypes.byref(desc), ctypes.byref(h)) == binding.MKV_E_ARG
+    assert "reserved" in binding.mkv_last_error() and not h.value
+
+
 def test_product_does_not_import_the_oracle():
     pkg = os.path.join(ROOT, "paper_2607_00760_b200")
     for dirpath, _, files in os.walk(pkg):

@@ -404,6 +404,95 @@ def test_attention_long_ranges(env):
         c.free()
 
 
+def test_attention_selection_longer_than_the_unit(env):
+    """A caller-built selection with more entries than the unit has blocks + 1 (duplicates; k_max far beyond the cache's
+    own capacity): mkv_packed_attention attends the first ceil(max_tokens / B) + 1 entries and ignores the rest
+    (include/mkv.h).  Uncut, 1200 positions over the 16 warps of a one-CTA unit are 75 blocks per warp, beyond the
+    16-block logit cache at G = 8: the spilled logits would run over the next unit's share of the scratch and, for the
+    last unit, past its end."""
+    mkv, dev = env
+    c = Case(mkv, dev, 19, 4, 32, 64 * 10, seed=641)
+    try:
+        strat = uniform_strat(19, 4, c.S, 38)
+        strat[:, :, 1::3, 0:2] = 128
+        c.compress(strat)
+        nblk, cap = 80, 81
+        rng = np.random.default_rng(5)
+        k_max = 1200
+        sel = np.zeros((19, 4, k_max), np.int32)
+        for b in range(19):
+            for h in range(4):
+                sel[b, h] = rng.integers(0, nblk, size=k_max) * 8
+                sel[b, h, :nblk] = rng.permutation(nblk) * 8   # every block once, then one duplicate inside the cut
+        cnt = np.full((19, 4), k_max, np.int32)
+        out, lse = c.gpu_attention(sel, cnt)
+        ref, ref_lse = np.zeros_like(out), np.zeros_like(lse)
+        for b in range(19):
+            for h in range(4):
+                o, l = orc.attention(c.blobs[b][h], c.q[b, 8 * h:8 * h + 8], sel[b, h, :cap], 1 / math.sqrt(128))
+                ref[b, 8 * h:8 * h + 8], ref_lse[b, 8 * h:8 * h + 8] = o, l
+        assert_attention_close(out, lse, ref, ref_lse)
+        # and the calls after it see an intact cache and scratch
+        s2, c2 = c.oracle_sel(c.N)
+        c.check_attention(s2, c2)
+    finally:
+        c.free()
+
+
+def test_captured_attention_after_reset_and_refill(env):
+    """A CUDA graph of mkv_packed_attention on a caller-owned `sel` is replayed after mkv_cache_reset and a refill with
+    other data under other strategies (other payload offsets).  The per-block records mkv_select left before the reset
+    carry the tag the captured launch was given and the same first tokens; mkv_cache_reset clears them, so the replay
+    looks every block up in the tables of the new filling."""
+    mkv, dev = env
+    import torch
+    N = 64 * 9
+    a = Case(mkv, dev, 2, 2, 8, N, seed=81)
+    b = Case(mkv, dev, 2, 2, 8, N, seed=82)
+    try:
+        a.compress(uniform_strat(2, 2, a.S, 38))
+        budget, scale = 200, 1 / math.sqrt(128)
+        k_max = budget // 8 + 1
+        sel = torch.full((2, 2, k_max), -1, dtype=torch.int32, device=dev)
+        cnt = torch.zeros((2, 2), dtype=torch.int32, device=dev)
+        a.cache.select(0, a.q_d, budget, sel, cnt)   # writes the records of this filling
+        out = torch.zeros((2, 8, 128), dtype=torch.float32, device=dev)
+        lse = torch.zeros((2, 8), dtype=torch.float32, device=dev)
+        st = torch.cuda.Stream()
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            a.cache.packed_attention(0, a.q_d, sel, cnt, scale, out, lse, stream=st)
+            st.synchronize()
+            gr = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gr, stream=st):
+                a.cache.packed_attention(0, a.q_d, sel, cnt, scale, out, lse, stream=st)
+            gr.replay()
+            st.synchronize()
+            first = out.clone()
+            # refill the layer with b's K / V under a different strategy mix: every payload offset changes
+            a.cache.reset(0, stream=st)
+            sb = uniform_strat(2, 2, a.S, 64)
+            sb[:, :, ::2, :2] = 128
+            a.cache.compress_segment(0, b.k_d, b.v_d, torch.from_numpy(sb).to(dev), stream=st)
+            out.zero_()
+            gr.replay()
+            st.synchronize()
+        a.cache.status()
+        assert not torch.equal(first, out)
+        sel_h, cnt_h = sel.cpu().numpy(), cnt.cpu().numpy()
+        got, got_lse = out.cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64)
+        ref, ref_lse = np.zeros_like(got), np.zeros_like(got_lse)
+        for i in range(2):
+            for h in range(2):
+                blob = orc.compress_unit(b.K[i, h], b.V[i, h], 64, sb[i, h])
+                o, l = orc.attention(blob, a.q[i, 4 * h:4 * h + 4], sel_h[i, h, :cnt_h[i, h]], scale)
+                ref[i, 4 * h:4 * h + 4], ref_lse[i, 4 * h:4 * h + 4] = o, l
+        assert_attention_close(got, got_lse, ref, ref_lse)
+    finally:
+        a.free()
+        b.free()
+
+
 @pytest.mark.parametrize("Bt,Hkv", [(5, 4), (10, 4), (20, 4), (38, 4)])
 def test_attention_every_cluster_size(env, Bt, Hkv):
     """PackedAttention runs one cluster of C CTAs per unit, C = the largest power of two with units x C <= SMs: 20 units ->
@@ -703,6 +792,15 @@ def test_layers_are_independent_and_decode_host_matches(env):
         a.cache.decode_host(0, q_page, 256, 1 / math.sqrt(128), out_page)
         torch.cuda.synchronize()
         assert np.array_equal(out_page.numpy(), out_host.numpy())
+        # pinned buffers that are not 16-byte aligned (views 2 / 4 bytes into a pinned block): the chain's 16-byte fetch
+        # and store kernels cannot take them, so they go through the copy engine too: same bits, no misaligned access
+        q_odd = torch.zeros(2 * 8 * 128 + 1, dtype=torch.bfloat16).pin_memory()[1:].view(2, 8, 128)
+        q_odd.copy_(q_host)
+        out_odd = torch.zeros(2 * 8 * 128 + 1, dtype=torch.float32).pin_memory()[1:].view(2, 8, 128)
+        assert q_odd.data_ptr() % 16 == 2 and out_odd.data_ptr() % 16 == 4 and q_odd.is_pinned()
+        a.cache.decode_host(0, q_odd, 256, 1 / math.sqrt(128), out_odd)
+        torch.cuda.synchronize()
+        assert np.array_equal(out_odd.numpy(), out_host.numpy())
         t, s = a.check_select(256)
         assert s == 0
     finally:
@@ -1149,6 +1247,71 @@ def test_rotation_fold(env):
         c.cache.decode_host(0, q_host, budget, scale, out_host)
         torch.cuda.synchronize()
         assert np.abs(out_host.numpy().astype(np.float64) - ref).max() > 1e-3
+    finally:
+        c.free()
+
+
+def test_rotation_fold_with_update_buffer(env):
+    """Rotation fold and KV update buffer together (include/mkv.h: the buffered tokens of a rotated
+    layer must be rotated like the packed ones).  mkv_decode_step on a rotated cache with buffered rotated tokens equals
+    the oracle's rotate_query -> scores -> top-k -> attention over packed blocks + buffer -> rotate_output; raw tokens
+    in the buffer instead give a different (wrong) result, which is what the header warns about."""
+    mkv, dev = env
+    import torch
+    from paper_2607_00760_b200 import synth
+    Bt, Hkv, Hq, L, n_buf = 2, 2, 8, 64, 21
+    N0 = L * 7
+    G, D = Hq // Hkv, 128
+    rng = np.random.default_rng(43)
+    c = Case(mkv, dev, Bt, Hkv, Hq, N0 + L, seed=98)
+    try:
+        Rk = np.stack([np.linalg.qr(rng.standard_normal((D, D)))[0] for _ in range(Hkv)]).astype(np.float32)
+        Rv = np.stack([np.linalg.qr(rng.standard_normal((D, D)))[0] for _ in range(Hkv)]).astype(np.float32)
+        f = lambda a: (a.astype(np.uint32) << np.uint32(16)).view(np.float32)
+        # the first buffered key of every unit points along the unit's first query head (x 400: above the generator's
+        # heavy hitters), so the buffer carries most of that head's softmax mass and a wrong basis cannot go unnoticed
+        for b in range(Bt):
+            for h in range(Hkv):
+                c.K[b, h, N0] = synth.f32_to_bf16_bits(np.float32(400) * f(c.q[b, h * G]))
+        raw_k, raw_v = to_dev(c.K, dev), c.v_d.clone()
+        for h in range(Hkv):
+            c.K[:, h] = synth.f32_to_bf16_bits(f(c.K[:, h]) @ Rk[h].T)
+            c.V[:, h] = synth.f32_to_bf16_bits(f(c.V[:, h]) @ Rv[h].T)
+        c.k_d, c.v_d = to_dev(c.K, dev), to_dev(c.V, dev)
+        strat = uniform_strat(Bt, Hkv, N0 // L, 38)
+        strat[:, :, ::3, 0:2] = 128
+        c.cache.compress_segment(0, c.k_d[:, :, :N0], c.v_d[:, :, :N0], torch.from_numpy(strat).to(dev))
+        c.cache.rotation_set(0, torch.from_numpy(Rk).to(dev), torch.from_numpy(Rv).to(dev))
+        c.cache.update_append(0, c.k_d[:, :, N0:N0 + n_buf], c.v_d[:, :, N0:N0 + n_buf])
+        budget, scale = 160, 1.0 / math.sqrt(D)
+        k_max = budget // 8 + 1
+        sel = torch.full((Bt, Hkv, k_max), -1, dtype=torch.int32, device=dev)
+        cnt = torch.zeros((Bt, Hkv), dtype=torch.int32, device=dev)
+        out = torch.zeros((Bt, Hq, D), dtype=torch.float32, device=dev)
+        c.cache.decode_step(0, c.q_d, budget, scale, out, sel=sel, sel_count=cnt)
+        torch.cuda.synchronize()
+        c.cache.status()
+        sel_h, cnt_h = sel.cpu().numpy(), cnt.cpu().numpy()
+        ref = np.zeros((Bt, Hq, D))
+        for b in range(Bt):
+            for h in range(Hkv):
+                qh = np.stack([orc.rotate_query(c.q[b, hq:hq + 1], Rk[h])[0] for hq in range(h * G, (h + 1) * G)])
+                blob = orc.compress_unit(c.K[b, h, :N0], c.V[b, h, :N0], L, strat[b, h])
+                ft, nt = orc.blob_blocks(blob)
+                want = orc.topk(orc.scores(blob, qh, 0), ft, nt, budget)
+                np.testing.assert_array_equal(sel_h[b, h, :cnt_h[b, h]], want)
+                o_, _ = orc.attention_with_update_buffer(blob, qh, want, scale, c.K[b, h, N0:N0 + n_buf],
+                                                         c.V[b, h, N0:N0 + n_buf])
+                ref[b, h * G:(h + 1) * G] = orc.rotate_output(o_, Rv[h])
+        got = out.cpu().numpy().astype(np.float64)
+        assert np.abs(got - ref).max() <= ATOL and np.linalg.norm(got - ref) / np.linalg.norm(ref) <= RTOL
+        # the misuse the header names: the same tokens unrotated in the buffer of the rotated layer
+        c.cache.reset(0)
+        c.cache.compress_segment(0, c.k_d[:, :, :N0], c.v_d[:, :, :N0], torch.from_numpy(strat).to(dev))
+        c.cache.update_append(0, raw_k[:, :, N0:N0 + n_buf], raw_v[:, :, N0:N0 + n_buf])
+        c.cache.decode_step(0, c.q_d, budget, scale, out)
+        torch.cuda.synchronize()
+        assert np.abs(out.cpu().numpy().astype(np.float64) - ref).max() > 10 * ATOL
     finally:
         c.free()
 
