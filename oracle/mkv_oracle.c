@@ -715,7 +715,7 @@ int orc_attention_units(uint8_t* const* blobs, int n_units, const uint16_t* q, i
  * single query vector and uses the rotated query to compute the attention scores.  This approach is mathematically
  * equivalent".  With K' = K R_k^T stored, q K^T = (q R_k^T) K'^T, so the folded query is q' = q R_k^T:
  *   q'[i] = sum_j q[j] * R_k[i][j].
- * Reading (R22): q' is an INPUT of the bf16 kernels, so its rounding is part of the definition: the sum is
+ * Reading (R18): q' is an INPUT of the bf16 kernels, so its rounding is part of the definition: the sum is
  * accumulated in fp32 with one fused multiply-add per j in ascending j, then rounded to bf16 (RNE).
  * q: [n][D] bf16, R: [D][D] fp32 row-major, out: [n][D] bf16.
  */

@@ -48,18 +48,25 @@ def test_tiny_config_end_to_end(env):
 
 # ------------------------------------------------------------------ configs 2-4 at full size (the bench's launch configuration)
 
-def _full_size_sampled(env, name, n_layers, units_per_layer):
+def _full_size_sampled(env, name, n_layers, units_per_layer, budgets=(None,), keep_ratio=None):
     """One BASELINE workload at FULL size, built exactly as bench.py builds it (same generator, kernels and grids).
     For `units_per_layer` units of each of `n_layers` layers (always unit (0, 0) and the last unit) the oracle
     recomputes everything from the raw bytes the GPU consumed: strategy table (equal), packed blob (bit-exact),
     selection (tie-band protocol, swaps counted) and the attention output on the GPU's own selection; plus count /
-    order / range properties on every unit of every layer."""
+    order / range properties on every unit of every layer.  Every selection is attended a second time with q = 0 (flat
+    softmax: phase 2 fetches every V part through the dealt-out lists -- the launch bench.py times as
+    `flat_softmax_q0`) and compared with the oracle as well.
+    budgets: token budgets run on the one built cache (None = the workload's own); keep_ratio: BASELINE config 5's
+    sweep axis (None = the workload's own; 1.0 = every segment dense)."""
     mkv, dev = env
+    import dataclasses
     import os
     from concurrent.futures import ThreadPoolExecutor
     import torch
     from paper_2607_00760_b200 import synth, workload
     w = synth.WORKLOADS[name]
+    if keep_ratio is not None:
+        w = dataclasses.replace(w, keep_ratio=keep_ratio)
     Bt, Hkv, Hq, G, N, L = w.batch, w.n_kv_heads, w.n_q_heads, w.group, w.context, w.segment_len
     n_units = Bt * Hkv
     pick = sorted({(i * (n_units - 1)) // max(1, units_per_layer - 1) for i in range(units_per_layer)})
@@ -67,55 +74,73 @@ def _full_size_sampled(env, name, n_layers, units_per_layer):
     built = workload.build(w, dev, n_layers=n_layers, keep_units=units)
     cache = built.cache
     try:
-        budget, scale = w.token_budget, 1.0 / math.sqrt(128)
-        k0 = budget // 8
-        k_max = k0 + 1
+        scale = 1.0 / math.sqrt(128)
+        budgets = [w.token_budget if x is None else x for x in budgets]
         res = {}
         for l in range(n_layers):
-            sel = torch.full((Bt, Hkv, k_max), -1, dtype=torch.int32, device=dev)
-            cnt = torch.zeros((Bt, Hkv), dtype=torch.int32, device=dev)
-            out = torch.zeros((Bt, Hq, 128), dtype=torch.float32, device=dev)
-            lse = torch.zeros((Bt, Hq), dtype=torch.float32, device=dev)
-            cache.select(l, built.q[l], budget, sel, cnt)
-            cache.packed_attention(l, built.q[l], sel, cnt, scale, out, lse)
-            torch.cuda.synchronize()
-            cache.status()
-            sel_h, cnt_h = sel.cpu().numpy(), cnt.cpu().numpy()
-            out_h, lse_h = out.cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64)
-            # properties that hold for every unit: counts, order, range
-            assert np.all(cnt_h == k0)
-            assert np.all(np.diff(sel_h[:, :, :k0], axis=-1) > 0) and sel_h.max() < N and np.all(sel_h[:, :, :k0] % 8 == 0)
-            assert np.all(sel_h[:, :, k0:] == -1)
-            assert np.all(np.isfinite(out_h)) and np.all(np.isfinite(lse_h))
-            res[l] = (sel_h, cnt_h, out_h, lse_h, built.q[l].view(torch.int16).cpu().numpy().view(np.uint16),
-                      built.strat[l].cpu().numpy())
+            q_zero = torch.zeros_like(built.q[l])
+            q_h = built.q[l].view(torch.int16).cpu().numpy().view(np.uint16)
+            strat_h = built.strat[l].cpu().numpy()
+            for budget in budgets:
+                k0 = min(budget // 8, N // 8)
+                k_max = min(budget // 8 + 1, N // 8)
+                sel = torch.full((Bt, Hkv, k_max), -1, dtype=torch.int32, device=dev)
+                cnt = torch.zeros((Bt, Hkv), dtype=torch.int32, device=dev)
+                out = torch.zeros((Bt, Hq, 128), dtype=torch.float32, device=dev)
+                lse = torch.zeros((Bt, Hq), dtype=torch.float32, device=dev)
+                out0, lse0 = torch.zeros_like(out), torch.zeros_like(lse)
+                cache.select(l, built.q[l], budget, sel, cnt)
+                cache.packed_attention(l, built.q[l], sel, cnt, scale, out, lse)
+                cache.attention_stats(reset=True)
+                cache.packed_attention(l, q_zero, sel, cnt, scale, out0, lse0)
+                st0 = cache.attention_stats(reset=True)
+                cache.status()
+                sel_h, cnt_h = sel.cpu().numpy(), cnt.cpu().numpy()
+                out_h, lse_h = out.cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64)
+                out0_h, lse0_h = out0.cpu().numpy().astype(np.float64), lse0.cpu().numpy().astype(np.float64)
+                # properties that hold for every unit: counts, order, range
+                assert np.all(cnt_h == k0)
+                assert np.all(np.diff(sel_h[:, :, :k0], axis=-1) > 0) and sel_h.max() < N and np.all(sel_h[:, :, :k0] % 8 == 0)
+                assert np.all(sel_h[:, :, k0:] == -1)
+                assert np.all(np.isfinite(out_h)) and np.all(np.isfinite(lse_h))
+                assert np.all(np.isfinite(out0_h)) and np.all(np.isfinite(lse0_h))
+                # flat softmax: nothing may be skipped, and lse = log(number of attended tokens) for every head
+                assert st0["blocks"] == int(cnt_h.sum()) and st0["v_blocks"] == st0["blocks"], st0
+                assert np.abs(lse0_h - math.log(8 * k0)).max() <= 1e-3
+                res[(l, budget)] = (sel_h, cnt_h, out_h, lse_h, out0_h, lse0_h, q_h, strat_h)
+                del sel, cnt, out, lse, out0, lse0
 
         def check(unit):
             l, b, h = unit
-            sel_h, cnt_h, out_h, lse_h, q_h, strat_h = res[l]
             K, V = built.raw_units[(l, b, h)]
             lk, lv = orc.segment_loss(K, V, L, w.r_keep, w.r_keep)
             st = orc.strategy_quantile(lk, lv, w.dense_num, w.dense_den, 128, w.r_keep, w.r_keep)
-            np.testing.assert_array_equal(strat_h[b, h], st)
             blob = orc.compress_unit(K, V, L, st)
             np.testing.assert_array_equal(cache.export(l, b, h), blob)
-            qh = q_h[b, h * G:(h + 1) * G]
             ft, nt = orc.blob_blocks(blob)
-            s = orc.scores(blob, qh, 0)
-            ref = orc.topk(s, ft, nt, budget)
-            n = int(cnt_h[b, h])
-            got = sel_h[b, h, :n]
-            assert n == len(ref)
-            swaps = 0
-            if not np.array_equal(got, ref):
-                diff = np.setxor1d(got, ref)
-                kth = np.sort(s)[::-1][len(ref) - 1]
-                band = 1e-5 * max(abs(kth), 1e-3 * np.abs(s).max())
-                assert np.all(np.abs(s[diff // 8] - kth) <= band), ("selection differs outside the tie band", unit)
-                swaps = len(diff) // 2
-            o, lref = orc.attention(blob, qh, got, scale)
-            assert_attention_close(out_h[b:b + 1, h * G:(h + 1) * G], lse_h[b:b + 1, h * G:(h + 1) * G], o[None], lref[None])
-            return n, swaps
+            total = swaps = 0
+            for budget in budgets:
+                sel_h, cnt_h, out_h, lse_h, out0_h, lse0_h, q_h, strat_h = res[(l, budget)]
+                np.testing.assert_array_equal(strat_h[b, h], st)
+                qh = q_h[b, h * G:(h + 1) * G]
+                s = orc.scores(blob, qh, 0)
+                ref = orc.topk(s, ft, nt, budget)
+                n = int(cnt_h[b, h])
+                got = sel_h[b, h, :n]
+                assert n == len(ref)
+                if not np.array_equal(got, ref):
+                    diff = np.setxor1d(got, ref)
+                    kth = np.sort(s)[::-1][len(ref) - 1]
+                    band = 1e-5 * max(abs(kth), 1e-3 * np.abs(s).max())
+                    assert np.all(np.abs(s[diff // 8] - kth) <= band), ("selection differs outside the tie band", unit)
+                    swaps += len(diff) // 2
+                total += n
+                rows = slice(h * G, (h + 1) * G)
+                o, lref = orc.attention(blob, qh, got, scale)
+                assert_attention_close(out_h[b:b + 1, rows], lse_h[b:b + 1, rows], o[None], lref[None])
+                o, lref = orc.attention(blob, np.zeros_like(qh), got, scale)
+                assert_attention_close(out0_h[b:b + 1, rows], lse0_h[b:b + 1, rows], o[None], lref[None])
+            return total, swaps
 
         # the oracle is single-threaded C behind ctypes (the GIL is released): one thread per unit
         with ThreadPoolExecutor(max(1, min(len(units), os.cpu_count() or 1, 16))) as ex:
@@ -141,6 +166,16 @@ def test_full_size_config3_sampled_units(env):
 def test_full_size_config4_sampled_units(env):
     """BASELINE config 4 (qwen7b-64k-b16: batch 16, 4 KV heads, GQA group 7, 65 536 tokens): 8 units on each of 4 layers."""
     _full_size_sampled(env, "qwen7b-64k-b16", 4, 8)
+
+
+def test_full_size_config5_sampled_units(env):
+    """BASELINE config 5 (the compression sweep on the config-2 shape), the points whose launch no other test reaches:
+    token budget 16 384 at keep ratio 0.3 and at 1.0, and the dense-full point (keep 1.0, budget = context).  64 units
+    run as clusters of two CTAs with 64 / 512 blocks per warp: logits beyond the shared-memory cache go through the
+    global scratch, phase 2 runs per warp, and the second CTA pushes its partial into the first (bench.py --sweep
+    times exactly these launches).  2 layers, 8 sampled units each, peaked q and q = 0."""
+    _full_size_sampled(env, "llama8b-128k-b8", 2, 8, budgets=(16384,))
+    _full_size_sampled(env, "llama8b-128k-b8", 2, 8, budgets=(16384, 131072), keep_ratio=1.0)
 
 
 # ------------------------------------------------------------------ step 1
@@ -491,6 +526,39 @@ def test_captured_attention_after_reset_and_refill(env):
     finally:
         a.free()
         b.free()
+
+
+@pytest.mark.parametrize("Bt,Hkv,Hq", [(10, 4, 16), (40, 1, 7)])
+def test_attention_clusters_with_long_ranges(env, Bt, Hkv, Hq):
+    """Clusters of two CTAs AND ranges beyond the per-warp logit cache, every unit compared with the oracle: 40 units ->
+    C = 2, 32 warps per unit, 1126 blocks per unit = 35-36 blocks per warp (the cache holds 32 at G = 4, 18 at G = 7).
+    Phase 1 spills logits to the global scratch, phase 2 describes the range a second time and runs per warp, and
+    rank 1 pushes its partial into rank 0's shared memory.  Peaked (the generator's q) and flat (q = 0: nothing
+    skipped) selections of every block, and a budget of a third of them."""
+    mkv, dev = env
+    N = 9003
+    c = Case(mkv, dev, Bt, Hkv, Hq, N, seed=650 + Hq)
+    try:
+        strat = uniform_strat(Bt, Hkv, c.S, 38)
+        strat[:, :, 3::7, 0:2] = 128
+        strat[:, :, 5::11, 0:2] = (90, 7)
+        strat[:, :, 2::13, 0:2] = (128, 38)
+        c.compress(strat)
+        q_gen = c.q.copy()
+        for flat in (False, True):
+            c.q[:] = 0 if flat else q_gen
+            c.q_d = to_dev(c.q, dev)
+            sel, cnt = c.oracle_sel(N)
+            assert int(cnt.min()) == 1126
+            c.cache.attention_stats(reset=True)
+            c.check_attention(sel, cnt)
+            st = c.cache.attention_stats(reset=True)
+            assert st["blocks"] == int(cnt.sum())
+            assert (st["v_blocks"] == st["blocks"]) if flat else (0 < st["v_blocks"] <= st["blocks"]), st
+            sel, cnt = c.oracle_sel(3000)
+            c.check_attention(sel, cnt)
+    finally:
+        c.free()
 
 
 @pytest.mark.parametrize("Bt,Hkv", [(5, 4), (10, 4), (20, 4), (38, 4)])
