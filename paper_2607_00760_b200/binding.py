@@ -10,7 +10,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmkv.so")
+# MKV_LIBRARY: another build of the same sources (the -DMKV_TRACE library of trace.py); never set by tests or bench.py
+LIB_PATH = os.environ.get("MKV_LIBRARY") or os.path.join(_HERE, "libmkv.so")
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} not found: run `python -m paper_2607_00760_b200.build` "

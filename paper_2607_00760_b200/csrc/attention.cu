@@ -50,6 +50,25 @@ constexpr int kZBytes = 4096;      // per-warp logit cache: 32 blocks at G = 4
 constexpr int kMaxCluster = 16;
 constexpr float kSkip = 40.f;      // a block whose probabilities are all < 2^-40 is not walked in phase 2
 
+// -DMKV_TRACE (python -m paper_2607_00760_b200.trace; never defined in libmkv.so): lane 0 of every warp stamps %globaltimer
+// at the phase boundaries of the LAST launch into a file-scope array that mkv_trace_read copies out.  The stamps are the
+// committed evidence for "where the time of a launch goes" (profiles/r3/trace_attention_config2.md).
+#ifdef MKV_TRACE
+constexpr int kTraceCtas = 160, kTraceStamps = 16;
+__device__ unsigned long long g_trace[kTraceCtas][kWarps][kTraceStamps];
+__device__ __forceinline__ unsigned long long trace_now() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)::"memory");
+    return t;
+}
+#define MKV_STAMP(i)                                                                                         \
+    do {                                                                                                     \
+        if ((threadIdx.x & 31) == 0 && blockIdx.x < kTraceCtas) g_trace[blockIdx.x][threadIdx.x >> 5][i] = trace_now(); \
+    } while (0)
+#else
+#define MKV_STAMP(i) do { } while (0)
+#endif
+
 // One group of the stream: <= 2 consecutive selected token blocks with the same strategy whose K parts and V
 // parts each fit kGroupMax16.  Every size the hot loops need is worked out once, by the describing lane.
 struct __align__(16) GDesc {
@@ -124,6 +143,14 @@ struct Split {
     unsigned b, r;
     __device__ __forceinline__ unsigned begin(unsigned i) const { return i * b + min(i, r); }
 };
+
+// Where element e = head * 128 + channel of a partial O sits in shared memory: channel 16 a + 2 i + p of head h at
+// h * 128 + ((16 i + 2 a + p + 8 (h / 2)) mod 128) -- a bijection per head that makes the warps' fragment stores (lane
+// (a, qq) holds channels 16 a + 2 i, + 1 of heads 2 qq, 2 qq + 1) free of bank conflicts.
+__device__ __forceinline__ int o_slot(int e) {
+    const int h = e >> 7, ch = e & 127;
+    return (e & ~127) | ((((ch & 15) >> 1) * 16 + (ch >> 4) * 2 + (ch & 1) + 8 * (h >> 1)) & 127);
+}
 
 // QK of one group in flight: S (16 tokens x 8 heads) += K q^T with the group's tokens = M (rows 0-7 = block 0, rows 8-15 =
 // block 1), heads = N, channels = K.  sp0 / sp1: the K parts of its blocks in shared memory; qa: q[head gq][32qq .. 32qq+31]
@@ -284,8 +311,10 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     const int u = (int)blockIdx.x / C;                      // the cluster's unit
     const unsigned rank = cluster_ctarank();
     __syncthreads();
+    MKV_STAMP(0);             // scheduled, barriers initialised
     pdl_wait();               // the producer of sel / sel_count / the plan / the cache is done
     pdl_launch_dependents();  // the next kernel may be scheduled as SMs free up
+    MKV_STAMP(1);             // griddepcontrol.wait returned
 
     // tokens in the layer's update buffer: device-resident, so a captured graph stays valid across appends
     const int n_buf = min(max(__ldg(upd_count), 0), g.L);
@@ -296,6 +325,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     // than that (k_max beyond sel_cap, duplicates) is cut there instead of running into the next unit's scratch
     const int cnt = min(min(max(__ldg(sel_count + u), 0), k_max) * ppb, scr.plan_stride);
     const int T = cnt + upd_blocks;                       // device blocks of the unit's stream
+    MKV_STAMP(2);                                         // counts known
     const size_t row = (size_t)(u / g.n_kv_heads) * g.n_q_heads + (size_t)(u % g.n_kv_heads) * G;
     if (T == 0) {  // (uniform over the cluster) empty selection: out = 0, lse = -inf
         if (rank == 0 && !kGatherOnly) {
@@ -447,7 +477,12 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             // ---- issue: K parts of the next groups while the ring has room
 #pragma unroll 1
             while (bposi < n_total) {
-                if (gposi == gbuilt) describe(min(kDescribe, n_total - bbuilt));
+                if (gposi == gbuilt) {
+                    describe(min(kDescribe, n_total - bbuilt));
+#ifdef MKV_TRACE
+                    if (gposi == 0) MKV_STAMP(3);  // first blocks described
+#endif
+                }
                 const GDesc d = d1[gposi & (kDesc - 1)];
                 const uint32_t c0 = (d.x & 255u) << 4, c1 = ((d.x >> 8) & 255u) << 4;
                 uint32_t off;
@@ -480,6 +515,9 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
             const bool full = nb0 == kPhys && (!two || nb1 == kPhys);
 
             landed();  // the group's K parts have landed
+#ifdef MKV_TRACE
+            if (gposc == 0) MKV_STAMP(4);  // first K part landed
+#endif
 
             // ---- QK: S (tokens x heads); rows 0-7 = block 0, rows 8-15 = block 1.  (A position that holds no block -- an
             // invalid `sel` entry, the missing second half of a ragged 16-token block -- still gets its logits: -inf, so
@@ -538,8 +576,10 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     // The cluster's CTAs exchange their maxima through distributed shared memory.
     // =====================================================================================
     float Mraw = -INFINITY;  // the unit's maximum logit of head gq (log2 domain)
+    MKV_STAMP(5);            // phase 1 of this warp done
     if (!kGatherOnly) {
         cluster_sync();  // every CTA's table is complete and visible to the cluster (also a CTA barrier)
+        MKV_STAMP(6);    // first cluster barrier passed
         if (gq < G) {
             // (four remote loads in flight at a time: a cluster of 16 would otherwise pay 16 round trips in a row)
             uint32_t k = 0u;
@@ -776,6 +816,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         if (calib == 0x9e3779b9u && lane == 0) scr.stats[7] = 1ull;
         return;
     }
+    MKV_STAMP(7);  // phase 2 of this warp done (sums, lists, V parts fetched and walked)
     if (lane == 0 && st_vblocks != 0u) {
         atomicAdd(scr.stats + 1, (unsigned long long)st_vblocks);
         atomicAdd(scr.stats + 2, (unsigned long long)st_vbytes);
@@ -793,16 +834,21 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     if (walked) {
         // the warp's partial: O^T fragments -> [head][channel] floats in the warp's (now idle) ring
         if (lane == 0) atomicOr(&s_active, 1u << warp);
+        // Partials live in a swizzled order (o_slot): stored plainly, the 32 lanes of one of these stores would hit two
+        // bank pairs (channel stride 16 floats over gq, head stride 128 floats over qq), 16 wavefronts each -- measured:
+        // 2 us of shared-memory pipe per launch.  In o_slot order a half-warp's float2 stores cover 32 banks.  The sums
+        // below run element-wise in that order; only the final store to `out` maps back.
         float* po = reinterpret_cast<float*>(wbase);
         const int hA = 2 * qq, hB = 2 * qq + 1;
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
-            const int ch = 16 * gq + 2 * i;
-            if (hA < G) *reinterpret_cast<float2*>(po + hA * kD + ch) = make_float2(acc[i][0], acc[i][2]);
-            if (hB < G) *reinterpret_cast<float2*>(po + hB * kD + ch) = make_float2(acc[i][1], acc[i][3]);
+            const int in = (16 * i + 2 * gq + 8 * qq) & (kD - 1);  // o_slot of channel 16 gq + 2 i for heads 2 qq, 2 qq + 1
+            if (hA < G) *reinterpret_cast<float2*>(po + hA * kD + in) = make_float2(acc[i][0], acc[i][2]);
+            if (hB < G) *reinterpret_cast<float2*>(po + hB * kD + in) = make_float2(acc[i][1], acc[i][3]);
         }
     }
     __syncthreads();
+    MKV_STAMP(8);  // warps' partials stored, CTA barrier passed
     const int GD = G * kD;
     // A cluster of two (64 units on 148 SMs): the second CTA PUSHES its partial into the first one's shared memory, so
     // after the barrier the first CTA adds two local arrays and the second one is free to leave: no remote loads on the
@@ -817,6 +863,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         if (push && rank != 0) st_dsmem_f32(peer_o + 4u * (uint32_t)e, o);
         else s_cta_o[e] = o;
     }
+    MKV_STAMP(12);  // (between 8 and 9) the CTA's partial O summed
     if (threadIdx.x < G) {
         float l = 0.f;
 #pragma unroll 1
@@ -824,22 +871,25 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         if (push && rank != 0) st_dsmem_f32(peer_l + 4u * threadIdx.x, l);
         else s_cta_l[threadIdx.x] = l;
     }
+    MKV_STAMP(9);    // CTA partial summed (and pushed)
     cluster_sync();  // every CTA's partial is complete and visible to the cluster
+    MKV_STAMP(10);   // second cluster barrier passed
     if (push) {
         if (rank == 0) {
             for (int e = threadIdx.x; e < GD; e += kNT) {
-                const int h = e >> 7;
-                const float o = s_cta_o[e] + s_peer_o[e], l = s_cta_l[h] + s_peer_l[h];
+                const int h = e >> 7, es = o_slot(e);
+                const float o = s_cta_o[es] + s_peer_o[es], l = s_cta_l[h] + s_peer_l[h];
                 out[row * kD + e] = l > 0.f ? o / l : 0.f;
                 if (lse != nullptr && (e & (kD - 1)) == 0) lse[row + h] = l > 0.f ? (s_M[h] + log2f(l)) * kLn2 : -INFINITY;
             }
         }
+        MKV_STAMP(11);  // output stored (rank 0) / leaving (rank 1)
         return;
     }
     if (rank == 0) {
         const uint32_t ao = smem_u32(s_cta_o), al = smem_u32(s_cta_l);
         for (int e = threadIdx.x; e < GD; e += kNT) {
-            const int h = e >> 7;
+            const int h = e >> 7, es = o_slot(e);
             float o = 0.f, l = 0.f;
 #pragma unroll 1
             for (int r0 = 0; r0 < C; r0 += 4) {  // (eight remote loads in flight; ranks past the cluster add nothing)
@@ -847,7 +897,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     const uint32_t r = (uint32_t)min(r0 + j, C - 1);
-                    vo[j] = ld_dsmem_f32(dsmem_addr(ao + 4u * (uint32_t)e, r));
+                    vo[j] = ld_dsmem_f32(dsmem_addr(ao + 4u * (uint32_t)es, r));
                     vl[j] = ld_dsmem_f32(dsmem_addr(al + 4u * (uint32_t)h, r));
                 }
 #pragma unroll
@@ -859,6 +909,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         }
     }
     cluster_sync();  // no CTA leaves (and releases its shared memory) before the first one has read it
+    MKV_STAMP(11);   // output stored, third cluster barrier passed
 }
 
 
@@ -1040,3 +1091,20 @@ cudaError_t launch_walk_probe(const CacheGeom& g, const LayerView& lv, const uin
 }
 
 }  // namespace mkv
+
+#ifdef MKV_TRACE
+// trace build only (not in include/mkv.h, not in libmkv.so): the stamps of the last mkv_packed_attention launch on the
+// current device, [kTraceCtas = 160][16 warps][16] x u64 nanoseconds of %globaltimer (0 = never written).  Synchronises.
+extern "C" __attribute__((visibility("default"))) int mkv_trace_read(unsigned long long* host, unsigned long long cap_bytes,
+                                                                     int clear) {
+    using namespace mkv;
+    if (!host || cap_bytes < sizeof(g_trace)) return MKV_E_ARG;
+    if (cudaDeviceSynchronize() != cudaSuccess) return MKV_E_CUDA;
+    if (cudaMemcpyFromSymbol(host, g_trace, sizeof(g_trace)) != cudaSuccess) return MKV_E_CUDA;
+    if (clear) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_trace) != cudaSuccess || cudaMemset(p, 0, sizeof(g_trace)) != cudaSuccess) return MKV_E_CUDA;
+    }
+    return MKV_OK;
+}
+#endif
