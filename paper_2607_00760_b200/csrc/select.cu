@@ -76,6 +76,7 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
     __shared__ unsigned hist[2 * 4096];
     __shared__ int s_krem;
     __shared__ unsigned long long s_warp[32];
+    __shared__ unsigned long long s_scan[32];  // the emission's scan (its own array: a warp may still be reading s_warp)
 
     const int k0 = budget / kB, rem = budget % kB, nbR = ntok % kB;
     // MODE 1 keeps k0 + 1 per slice (the most the final stage can ask for); every element if fewer
@@ -115,6 +116,7 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
         for (int i = tid; i < 2 * 4096; i += 1024) hist[i] = 0;
         __syncthreads();
         int n_eq = 0;
+        bool all_of_bin = false;
         for (int pass = 0; pass < 3; ++pass) {
             const int shift = pass == 0 ? 20 : (pass == 1 ? 8 : 0);
             const int nbins = pass == 2 ? 256 : 4096;
@@ -189,9 +191,14 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
             prefix |= (uint32_t)__shfl_sync(kFull, f_bin, src) << shift;
             krem -= (int)__shfl_sync(kFull, f_cum, src);
             n_eq = (int)__shfl_sync(kFull, f_cnt, src);
+            // Every key of the bin is wanted (the usual case after 24 bits: the bin holds one key): the selection is
+            // "every key >= prefix", and the remaining bits need not be resolved.  (Uniform over the CTA: every warp
+            // derives krem and n_eq from the same histogram.  Not with a short last block: its rule needs the exact
+            // threshold key and the number of keys equal to it.)
+            if (pass < 2 && krem == n_eq && !ragged_try) { all_of_bin = true; break; }
         }
         Ts = prefix;
-        take_eq = krem;            // equals (by ascending index) inside the kq best
+        take_eq = all_of_bin ? 0x7fffffff : krem;  // equals (by ascending index) inside the kq best
         // (n_eq: all elements whose key equals the threshold key)
         if (ragged_try) {
             // the short block is the highest index: it is inside the k0+1 best iff it beats Ts or
@@ -240,21 +247,21 @@ __global__ void __launch_bounds__(1024) mkv_topk_kernel(CacheGeom g, LayerView l
             const unsigned long long v = __shfl_up_sync(kFull, incl, o);
             if (lane >= o) incl += v;
         }
-        if (lane == 31) s_warp[warp] = incl;
+        if (lane == 31) s_scan[warp] = incl;
         __syncthreads();
         if (warp == 0) {
-            const unsigned long long w = s_warp[lane];
+            const unsigned long long w = s_scan[lane];
             unsigned long long wi = w;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 const unsigned long long v = __shfl_up_sync(kFull, wi, o);
                 if (lane >= o) wi += v;
             }
-            s_warp[lane] = wi - w;
+            s_scan[lane] = wi - w;
             if (lane == 31) s_krem = (int)((uint32_t)wi + min((uint32_t)take_eq, (uint32_t)(wi >> 32)));
         }
         __syncthreads();
-        const unsigned long long before = s_warp[warp] + incl - mine;
+        const unsigned long long before = s_scan[warp] + incl - mine;
         int gt_before = (int)(uint32_t)before, eq_before = (int)(before >> 32);
         count = s_krem;
         auto emit = [&](int i, uint32_t u) {
