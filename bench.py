@@ -29,9 +29,10 @@ UNIT = "us/layer"
 NOMINAL_HBM_GBS = 8000.0
 FALLBACK_HBM_GBS = 6650.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the committed `ncu --set full` captures.  NOT measured by
-# this run: printed under "traffic_from_capture" with the file it came from; "traffic" itself stays null.
-NCU_CAPTURE = {"llama8b-128k-b8": {"source": "profiles/r2/ncu_decode_config2.md (ncu --set full, first launch of each kernel)",
-                                   "attention": 28720896, "score+topk": 125432064},
+# this run: "traffic" carries the number of the capture (null for a workload without one) and "traffic_from_capture"
+# names the file it came from.
+NCU_CAPTURE = {"llama8b-128k-b8": {"source": "profiles/r3/ncu_decode_config2.md (ncu --set full, first launch of each kernel)",
+                                   "attention": 28732672, "score+topk": 125498880},
                "llama8b-1m-b1": {"source": "profiles/r2/ncu_decode_config3.md", "attention": None, "score+topk": None},
                "qwen7b-64k-b16": {"source": "profiles/r2/ncu_decode_config4.md", "attention": None, "score+topk": None}}
 
@@ -345,7 +346,7 @@ def run_mkv(args):
                      "unit": "GB/s", "frac": round(attn_gbs / peak, 4),
                      "frac_flat": round(a_bytes / (ms_flat * 1e-3 / n_layers) / 1e9 / peak, 4),
                      "frac_on_bytes_fetched": round((bytes_fetched or 0) / (us_attn * 1e-6) / 1e9 / peak, 4),
-                     "traffic": None,
+                     "traffic": cap.get("attention"),
                      "traffic_from_capture": {"bytes": cap.get("attention"), "source": cap.get("source")},
                      "peak_source": peak_src,
                      "frac_of_nominal_8TBs": round(attn_gbs / NOMINAL_HBM_GBS, 4),
@@ -363,7 +364,7 @@ def run_mkv(args):
                                          "v_blocks_fetched_fraction": round(stats_flat["v_blocks"] / max(1, stats_flat["blocks"]), 4),
                                          "frac": round(a_bytes / (ms_flat * 1e-3 / n_layers) / 1e9 / peak, 4)}},
         "roofline_select": {"kernel": "mkv_select", "bound": "hbm", "achieved": round(sel_gbs, 1), "peak": peak,
-                            "unit": "GB/s", "frac": round(sel_gbs / peak, 4), "traffic": None,
+                            "unit": "GB/s", "frac": round(sel_gbs / peak, 4), "traffic": cap.get("score+topk"),
                             "traffic_from_capture": {"bytes": cap.get("score+topk"), "source": cap.get("source")},
                             "algorithmic_bytes_per_launch": int(s_bytes)},
         "compress": {"loss_ms_per_layer": round(float(comp_ms[0]), 3), "strategy_ms_per_layer": round(float(comp_ms[1]), 3),

@@ -288,6 +288,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     __shared__ float s_peer_l[kMaxGroup];                 // clusters of two: the second CTA's sums, pushed into the first
     __shared__ float s_M[kMaxGroup];                      // the unit's per-head maxima after the exchange
     __shared__ unsigned s_active;                         // warps of the CTA that hold a partial result
+    __shared__ unsigned s_stat[2];                        // V blocks / V bytes this CTA fetched (mkv_attention_stats)
     __shared__ uint32_t s_q[kWarps][kDesc];               // phase 2: the groups of each warp's range that matter ...
     __shared__ int s_qn[kWarps];                          // ... and how many
     float* s_cta_o = reinterpret_cast<float*>(smem + kWarps * kWS);  // [G][128] floats behind the warps' regions
@@ -307,7 +308,7 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         mbar_init_fence();
     }
     if (threadIdx.x < kMaxGroup) s_max[threadIdx.x] = 0u;  // below the key of every float
-    if (threadIdx.x == 0) s_active = 0u;
+    if (threadIdx.x == 0) { s_active = 0u; s_stat[0] = s_stat[1] = 0u; }
     const int u = (int)blockIdx.x / C;                      // the cluster's unit
     const unsigned rank = cluster_ctarank();
     __syncthreads();
@@ -817,11 +818,13 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         return;
     }
     MKV_STAMP(7);  // phase 2 of this warp done (sums, lists, V parts fetched and walked)
+    // counters of mkv_attention_stats: added up per CTA in shared memory; the CTA's three global reductions are issued
+    // at the very end (4224 same-address reductions per launch, two per warp, used to sit in front of the cluster
+    // barrier's release fence, which waits for them)
     if (lane == 0 && st_vblocks != 0u) {
-        atomicAdd(scr.stats + 1, (unsigned long long)st_vblocks);
-        atomicAdd(scr.stats + 2, (unsigned long long)st_vbytes);
+        atomicAdd(&s_stat[0], st_vblocks);
+        atomicAdd(&s_stat[1], st_vbytes);
     }
-    if (threadIdx.x == 0 && rank == 0) atomicAdd(scr.stats + 0, (unsigned long long)T);
 
     // =====================================================================================
     // Step 3d.  Every partial of the unit is relative to the same maximum, so combining is plain addition (the
@@ -857,16 +860,18 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     const unsigned wmask = s_active;  // (in warp order: the sums are reproducible)
     const uint32_t peer_o = dsmem_addr(smem_u32(s_peer_o), 0u), peer_l = dsmem_addr(smem_u32(s_peer_l), 0u);
     for (int e = threadIdx.x; e < GD; e += kNT) {  // the CTA's partial
-        float o = 0.f;
-#pragma unroll 1
-        for (unsigned m = wmask; m; m &= m - 1u) o += *reinterpret_cast<const float*>(smem + (__ffs(m) - 1) * kWS + 4 * e);
+        float o = 0.f, v[kWarps];
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) v[w] = (wmask >> w) & 1u ? *reinterpret_cast<const float*>(smem + w * kWS + 4 * e) : 0.f;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) o += v[w];  // (warp order, as ever: an idle warp adds +0)
         if (push && rank != 0) st_dsmem_f32(peer_o + 4u * (uint32_t)e, o);
         else s_cta_o[e] = o;
     }
     MKV_STAMP(12);  // (between 8 and 9) the CTA's partial O summed
     if (threadIdx.x < G) {
         float l = 0.f;
-#pragma unroll 1
+#pragma unroll
         for (int w = 0; w < kWarps; ++w) l += s_l[w][threadIdx.x];
         if (push && rank != 0) st_dsmem_f32(peer_l + 4u * threadIdx.x, l);
         else s_cta_l[threadIdx.x] = l;
@@ -874,6 +879,13 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     MKV_STAMP(9);    // CTA partial summed (and pushed)
     cluster_sync();  // every CTA's partial is complete and visible to the cluster
     MKV_STAMP(10);   // second cluster barrier passed
+    if (threadIdx.x == 0) {  // (s_stat is complete since the CTA barrier above)
+        if (s_stat[0] != 0u) {
+            atomicAdd(scr.stats + 1, (unsigned long long)s_stat[0]);
+            atomicAdd(scr.stats + 2, (unsigned long long)s_stat[1]);
+        }
+        if (rank == 0) atomicAdd(scr.stats + 0, (unsigned long long)T);
+    }
     if (push) {
         if (rank == 0) {
             for (int e = threadIdx.x; e < GD; e += kNT) {
