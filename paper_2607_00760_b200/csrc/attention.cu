@@ -113,6 +113,14 @@ __device__ __forceinline__ uint32_t cluster_ctarank() {
 __device__ __forceinline__ void cluster_sync() {  // also orders shared-memory accesses cluster-wide (release / acquire)
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.aligned;" ::: "memory"); }
+// 4 bytes into another CTA's shared memory, counted on an mbarrier of THAT CTA when they have landed: the receiver waits on
+// its own mbarrier and then sees the data.  No fence on either side (a cluster-scope release, which is what a plain remote
+// store followed by barrier.cluster needs, is a MEMBAR.ALL.GPU on this machine: it waits for every outstanding access).
+__device__ __forceinline__ void st_async_b32(uint32_t dst, uint32_t v, uint32_t mbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(dst), "r"(v), "r"(mbar) : "memory");
+}
 __device__ __forceinline__ uint32_t dsmem_addr(uint32_t local, uint32_t rank) {  // the same offset in CTA `rank` of the cluster
     uint32_t r;
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local), "r"(rank));
@@ -289,6 +297,9 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     __shared__ float s_M[kMaxGroup];                      // the unit's per-head maxima after the exchange
     __shared__ unsigned s_active;                         // warps of the CTA that hold a partial result
     __shared__ unsigned s_stat[2];                        // V blocks / V bytes this CTA fetched (mkv_attention_stats)
+    __shared__ __align__(8) unsigned long long s_xbar[2]; // mbarriers: [0] the peers' maxima have landed; [1] (first CTA of a
+                                                          // cluster of two) the second CTA's partial has landed
+    __shared__ uint32_t s_peer_max[kMaxCluster][kMaxGroup];  // maxima (keys) sent by the other CTAs of the cluster
     __shared__ uint32_t s_q[kWarps][kDesc];               // phase 2: the groups of each warp's range that matter ...
     __shared__ int s_qn[kWarps];                          // ... and how many
     float* s_cta_o = reinterpret_cast<float*>(smem + kWarps * kWS);  // [G][128] floats behind the warps' regions
@@ -308,7 +319,15 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         mbar_init_fence();
     }
     if (threadIdx.x < kMaxGroup) s_max[threadIdx.x] = 0u;  // below the key of every float
-    if (threadIdx.x == 0) { s_active = 0u; s_stat[0] = s_stat[1] = 0u; }
+    if (threadIdx.x == 0) {
+        s_active = 0u; s_stat[0] = s_stat[1] = 0u;
+        // what the peers will send: (C - 1) x 8 maxima; to the first CTA of a cluster of two also G x 128 floats + G sums
+        mbar_init(smem_u32(&s_xbar[0]), 1);
+        mbar_init(smem_u32(&s_xbar[1]), 1);
+        mbar_init_fence();
+        if (C > 1) mbar_expect_tx(smem_u32(&s_xbar[0]), (uint32_t)(C - 1) * kMaxGroup * 4u);
+        if (C == 2) mbar_expect_tx(smem_u32(&s_xbar[1]), (uint32_t)G * (kD + 1) * 4u);
+    }
     const int u = (int)blockIdx.x / C;                      // the cluster's unit
     const unsigned rank = cluster_ctarank();
     __syncthreads();
@@ -335,6 +354,8 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         }
         return;
     }
+    // this CTA's mbarriers are ready for its peers: arrive here, wait (for every peer's arrival) right before the first send
+    if (!kGatherOnly && C > 1) cluster_arrive_relaxed();
     // The stream is split in units of two positions, so every range starts at an even position: a range never
     // holds two odd runs, which would cost an extra half-empty group.
     const unsigned P = ((unsigned)T + 1u) >> 1;  // position pairs, over the C * kWarps warps of the cluster
@@ -579,19 +600,25 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     float Mraw = -INFINITY;  // the unit's maximum logit of head gq (log2 domain)
     MKV_STAMP(5);            // phase 1 of this warp done
     if (!kGatherOnly) {
-        cluster_sync();  // every CTA's table is complete and visible to the cluster (also a CTA barrier)
-        MKV_STAMP(6);    // first cluster barrier passed
-        if (gq < G) {
-            // (four remote loads in flight at a time: a cluster of 16 would otherwise pay 16 round trips in a row)
-            uint32_t k = 0u;
-            const uint32_t a = smem_u32(&s_max[gq]);
-#pragma unroll 1
-            for (int r0 = 0; r0 < C; r0 += 4) {
-                uint32_t v[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) v[j] = ld_dsmem_u32(dsmem_addr(a, (uint32_t)min(r0 + j, C - 1)));
-                k = max(k, max(max(v[0], v[1]), max(v[2], v[3])));
+        __syncthreads();  // the CTA's table is complete
+        if (C > 1) {
+            // every CTA SENDS its eight maxima to each peer (asynchronous remote stores counted on the receiver's mbarrier)
+            // and waits for the C - 1 sets sent to it: no cluster barrier, no fence, no remote load
+            cluster_wait();  // every peer has initialised its mbarriers (it arrived at the start of its kernel)
+            if (warp == 0) {
+                for (int i = lane; i < (C - 1) * kMaxGroup; i += 32) {
+                    const int p = i / kMaxGroup, j = i % kMaxGroup;
+                    const uint32_t r = (uint32_t)(p >= (int)rank ? p + 1 : p);
+                    st_async_b32(dsmem_addr(smem_u32(&s_peer_max[rank][j]), r), s_max[j], dsmem_addr(smem_u32(&s_xbar[0]), r));
+                }
             }
+            mbar_wait(smem_u32(&s_xbar[0]), 0u);
+        }
+        MKV_STAMP(6);    // maxima exchanged
+        if (gq < G) {
+            uint32_t k = s_max[gq];
+            for (int r = 0; r < C; ++r)
+                if (r != (int)rank) k = max(k, s_peer_max[r][gq]);
             Mraw = k == 0u ? -INFINITY : funkey(k);
             if (warp == 0 && qq == 0) s_M[gq] = Mraw;
         }
@@ -859,13 +886,23 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
     const bool push = C == 2;
     const unsigned wmask = s_active;  // (in warp order: the sums are reproducible)
     const uint32_t peer_o = dsmem_addr(smem_u32(s_peer_o), 0u), peer_l = dsmem_addr(smem_u32(s_peer_l), 0u);
+    const uint32_t peer_bar = dsmem_addr(smem_u32(&s_xbar[1]), 0u);
+    auto flush_stats = [&]() {  // (s_stat is complete since the CTA barrier above)
+        if (threadIdx.x == 0) {
+            if (s_stat[0] != 0u) {
+                atomicAdd(scr.stats + 1, (unsigned long long)s_stat[0]);
+                atomicAdd(scr.stats + 2, (unsigned long long)s_stat[1]);
+            }
+            if (rank == 0) atomicAdd(scr.stats + 0, (unsigned long long)T);
+        }
+    };
     for (int e = threadIdx.x; e < GD; e += kNT) {  // the CTA's partial
         float o = 0.f, v[kWarps];
 #pragma unroll
         for (int w = 0; w < kWarps; ++w) v[w] = (wmask >> w) & 1u ? *reinterpret_cast<const float*>(smem + w * kWS + 4 * e) : 0.f;
 #pragma unroll
         for (int w = 0; w < kWarps; ++w) o += v[w];  // (warp order, as ever: an idle warp adds +0)
-        if (push && rank != 0) st_dsmem_f32(peer_o + 4u * (uint32_t)e, o);
+        if (push && rank != 0) st_async_b32(peer_o + 4u * (uint32_t)e, __float_as_uint(o), peer_bar);
         else s_cta_o[e] = o;
     }
     MKV_STAMP(12);  // (between 8 and 9) the CTA's partial O summed
@@ -873,20 +910,19 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         float l = 0.f;
 #pragma unroll
         for (int w = 0; w < kWarps; ++w) l += s_l[w][threadIdx.x];
-        if (push && rank != 0) st_dsmem_f32(peer_l + 4u * threadIdx.x, l);
+        if (push && rank != 0) st_async_b32(peer_l + 4u * threadIdx.x, __float_as_uint(l), peer_bar);
         else s_cta_l[threadIdx.x] = l;
     }
     MKV_STAMP(9);    // CTA partial summed (and pushed)
-    cluster_sync();  // every CTA's partial is complete and visible to the cluster
-    MKV_STAMP(10);   // second cluster barrier passed
-    if (threadIdx.x == 0) {  // (s_stat is complete since the CTA barrier above)
-        if (s_stat[0] != 0u) {
-            atomicAdd(scr.stats + 1, (unsigned long long)s_stat[0]);
-            atomicAdd(scr.stats + 2, (unsigned long long)s_stat[1]);
-        }
-        if (rank == 0) atomicAdd(scr.stats + 0, (unsigned long long)T);
-    }
     if (push) {
+        // A cluster of two: the second CTA has sent its partial (asynchronous remote stores counted on the first CTA's
+        // mbarrier) and leaves; the first waits for the G x 129 floats to land.  No cluster barrier, no fence.
+        if (rank == 0) {
+            __syncthreads();  // s_cta_o / s_cta_l of this CTA are complete
+            mbar_wait(smem_u32(&s_xbar[1]), 0u);
+        }
+        MKV_STAMP(10);   // (first CTA) the peer's partial has landed
+        flush_stats();
         if (rank == 0) {
             for (int e = threadIdx.x; e < GD; e += kNT) {
                 const int h = e >> 7, es = o_slot(e);
@@ -898,6 +934,9 @@ mkv_packed_attention_kernel(CacheGeom g, LayerView lv, const uint16_t* __restric
         MKV_STAMP(11);  // output stored (rank 0) / leaving (rank 1)
         return;
     }
+    cluster_sync();  // every CTA's partial is complete and visible to the cluster
+    MKV_STAMP(10);   // second cluster barrier passed
+    flush_stats();
     if (rank == 0) {
         const uint32_t ao = smem_u32(s_cta_o), al = smem_u32(s_cta_l);
         for (int e = threadIdx.x; e < GD; e += kNT) {
