@@ -60,6 +60,18 @@ def test_create_rejects_a_nonzero_reserved_field():
     assert "reserved" in binding.mkv_last_error() and not h.value
 
 
+def test_trace_build_is_a_separate_library():
+    """-DMKV_TRACE (paper_2607_00760_b200/trace.py) goes into libmkv_trace.so: the product library carries neither the
+    stamps' reader nor anything else the header does not declare"""
+    from paper_2607_00760_b200 import build as mkv_build
+    lib = ctypes.CDLL(mkv_build.build())
+    assert not hasattr(lib, "mkv_trace_read")
+    trace = ctypes.CDLL(mkv_build.build(trace=True))
+    assert hasattr(trace, "mkv_trace_read")
+    for name in declared_symbols():
+        assert hasattr(trace, name), name
+
+
 def test_product_does_not_import_the_oracle():
     pkg = os.path.join(ROOT, "paper_2607_00760_b200")
     for dirpath, _, files in os.walk(pkg):
