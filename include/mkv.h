@@ -164,8 +164,9 @@ MKV_API int mkv_select(const mkv_cache* cache, int32_t layer, const void* q, int
  * mkv_select are honoured: the per-block records mkv_select leaves for this call are verified against `sel`).
  * At most ceil(max_tokens / B) + 1 entries per unit are attended (one more than the unit has blocks); a caller-built
  * list that is longer (k_max and sel_count beyond that, which takes duplicates) is cut there.
- * One launch: one thread-block cluster per unit (one CTA per SM); the CTAs of a cluster meet at cluster barriers and read
- * each other's shared memory, nothing else is shared between CTAs.
+ * One launch: one thread-block cluster per unit (one CTA per SM); the CTAs of a cluster exchange their maxima and partial
+ * results through each other's shared memory (counted asynchronous stores, cluster barriers for clusters larger than two),
+ * nothing else is shared between CTAs.
  * out: float [batch][n_q_heads][D].  lse_opt: float [batch][n_q_heads] or NULL (log-sum-exp of the
  * scaled logits; -inf and out = 0 for an empty selection).
  */

@@ -16,9 +16,10 @@
 //     vectors are expanded straight into mma.sync fragments (mkv_walk.cuh).  The scaled logits go
 //     to the warp's logit cache (shared memory; global scratch beyond its capacity), the warp's
 //     per-head maxima into the CTA's table (shared-memory atomic max).
-//   * The CTAs of the cluster exchange their maxima through distributed shared memory (one cluster
-//     barrier).  Every warp then knows the unit's exact maximum M: probabilities are 2^(z - M),
-//     nothing is ever rescaled, and partial results simply add.
+//   * The CTAs of the cluster exchange their maxima through distributed shared memory: every CTA
+//     sends its table to each peer with asynchronous remote stores counted on the receiver's mbarrier
+//     (st.async, no fence, no cluster barrier).  Every warp then knows the unit's exact maximum M:
+//     probabilities are 2^(z - M), nothing is ever rescaled, and partial results simply add.
 //   * Phase 2 (PV, deferred): the softmax sum runs over every selected token; the V part of a block
 //     is fetched and walked only if one of its probabilities is >= 2^-40 (error bound).
 //     O^T = V^T P^T with channels = M, heads = N, the group's 16 tokens = K; P is split into bf16
@@ -26,8 +27,9 @@
 //     cluster is short, each warp lists the groups of its range that matter and the lists are dealt
 //     out over all warps of the CTA (which warps hold those groups is an accident of the data).
 //   * Step 3d (split-K combine): the warps' partials are added inside the CTA (shared memory), the
-//     CTAs' partials by the cluster's first CTA (pushed into its shared memory by the second CTA of a
-//     cluster of two, pulled through distributed shared memory otherwise), in a fixed order: no
+//     CTAs' partials by the cluster's first CTA (sent into its shared memory by the second CTA of a
+//     cluster of two, again with counted asynchronous stores, after which the sender leaves; pulled
+//     through distributed shared memory behind a cluster barrier otherwise), in a fixed order: no
 //     global scratch, no atomics, no second kernel, bit-reproducible.
 #include "mkv_internal.cuh"
 #include "mkv_walk.cuh"
